@@ -1,0 +1,836 @@
+/*
+ * gmnn_oracle.c -- TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+ *
+ * A plain, slow, fp64 CPU statement of the Gaussian Moment Neural Network energy-and-force
+ * evaluation of arxiv 2505.22168 (apax), written from PAPER.md Eq. 1-6 and the readings listed
+ * in DESIGN.md section 3.  It is the parity reference for the CUDA path and the timed
+ * `cpu_baseline` of bench.py.  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+ * --impl reference legs may load it.  It shares no code, header, table or helper with
+ * paper_2505_22168_b200/ and is never tuned for speed: naive loops over full (un-symmetrised)
+ * tensors, O(N^2 * images) neighbour search, OpenMP over atoms only so that it finishes.
+ *
+ * Pins (tests/test_oracle_*.py, all `-m "not gpu"`): forces == central finite differences of the
+ * energy; sum F = 0; E invariant under rotation / translation+wrap / permutation; brute-force ==
+ * cell-list neighbour sets; dimer and simple-cubic closed forms; trace identities of the moments;
+ * MLP == numpy matmul; Eq. 6 linearity of the ensemble; NVE dt^2 scaling and time reversal.
+ * Parity unpinned by the paper itself: PAPER.md prints no numeric E or F for any geometry, and the
+ * constants of DESIGN.md readings R1-R4, R7-R10 are readings, not quotes.
+ *
+ * Passages followed:
+ *   O-1  neighbour set ............ PAPER.md:49 ("local neighbors"), :171 (several images), :381 (skin)
+ *   O-2  radial functions ......... PAPER.md:49-52 (equidistant Gaussians, element-pair coefficients)
+ *   O-3  moments .................. PAPER.md:51 (Eq. 2)
+ *   O-4  invariants ............... PAPER.md:54-61 (Eq. 3; "up to L=3 and 4-body terms")
+ *   O-5  readout + scale-shift .... PAPER.md:63-65 (Eq. 4), :151 (ensemble axis not summed)
+ *   O-6  total energy ............. PAPER.md:46 (Eq. 1)
+ *   O-7..O-9 forces = -dE/dR ...... PAPER.md:127, 153 (gradient of the energy), chain rule by hand
+ *   O-10 ensemble ................. PAPER.md:75-88 (Eq. 5 with 1/N_ens, Eq. 6)
+ *   O-11 NVE velocity Verlet ...... BASELINE.json configs 2, 5; dt PAPER.md:367; skin :381
+ *
+ * Build: gcc -O2 -std=c11 -fPIC -shared -fopenmp -ffp-contract=off gmnn_oracle.c -lm
+ *        (-ffp-contract=off: the neighbour predicate is specified in unfused fp32, reading R20.)
+ */
+#define _GNU_SOURCE
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define NC 40 /* components per radial channel: 1 (L=0) + 3 (L=1) + 9 (L=2) + 27 (L=3) */
+#define O0 0
+#define O1 1
+#define O2 4
+#define O3 13
+#define ACC_CONV 9.648533212e-3 /* (eV/Ang/amu) -> Ang/fs^2 */
+
+typedef struct {
+    int32_t n_species, n_basis, n_radial;
+    double r_cut, r_min, gamma;
+    int32_t n_hidden;
+    int32_t hidden[4];
+    int32_t n_heads;
+} oracle_hparams;
+
+typedef struct {
+    const double *beta;  /* [S][S][n_radial][n_basis], centre species first */
+    const double *W[5];  /* layer l: [fan_in][fan_out] row-major */
+    const double *b[5];  /* layer l: [fan_out] */
+    const double *scale; /* [S] sigma_Z */
+    const double *shift; /* [S] mu_Z */
+} oracle_weights;
+
+int oracle_num_threads(void) {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+void oracle_set_num_threads(int n) {
+#ifdef _OPENMP
+    if (n > 0) omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}
+
+/* Feature count of O-4 (blocks 0..7). */
+int oracle_n_features(int n) {
+    int pairs = n * (n + 1) / 2;
+    int triples = n * (n + 1) * (n + 2) / 6;
+    return n + 3 * pairs + triples + 2 * pairs * n + n * n * n;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O-1  Neighbour set.  r_list = r_cut + skin.  Orthorhombic cell diag(L).  For every i, j and
+ * image n in [-k..k]^3 (k_a = pbc_a ? ceil(r_list / L_a) : 0), excluding (j == i, n == 0):
+ * keep (i, j, n) iff |x_j - x_i + n L|^2 < r_list^2, strict.  Full list (both directions).
+ * The predicate is SPECIFIED in unfused fp32 (reading R20):
+ *   s_a = fl(n_a * L_a);  d_a = fl(fl(x_j,a - x_i,a) + s_a);  r2 = fl(fl(dx*dx + dy*dy) + dz*dz)
+ *   keep iff r2 < fl(r_list * r_list).
+ * Output sorted by (i, j, nx, ny, nz).  Returns the number of pairs; writes at most cap of them.
+ * ------------------------------------------------------------------------------------------ */
+static inline int pair_predicate(const float *pos, int64_t i, int64_t j, float sx, float sy, float sz, float rl2) {
+    float dx = (pos[3 * j + 0] - pos[3 * i + 0]) + sx;
+    float dy = (pos[3 * j + 1] - pos[3 * i + 1]) + sy;
+    float dz = (pos[3 * j + 2] - pos[3 * i + 2]) + sz;
+    float r2 = (dx * dx + dy * dy) + dz * dz;
+    return r2 < rl2;
+}
+
+int64_t oracle_neighbors_brute(int64_t N, const float *pos, const float *L, const int32_t *pbc, float r_list,
+                               int64_t cap, int32_t *out_i, int32_t *out_j, int32_t *out_n) {
+    int k[3];
+    for (int a = 0; a < 3; ++a) k[a] = pbc[a] ? (int)ceilf(r_list / L[a]) : 0;
+    const float rl2 = r_list * r_list;
+    int64_t count = 0;
+    for (int64_t i = 0; i < N; ++i)
+        for (int64_t j = 0; j < N; ++j)
+            for (int nx = -k[0]; nx <= k[0]; ++nx)
+                for (int ny = -k[1]; ny <= k[1]; ++ny)
+                    for (int nz = -k[2]; nz <= k[2]; ++nz) {
+                        if (j == i && nx == 0 && ny == 0 && nz == 0) continue;
+                        float sx = (float)nx * L[0], sy = (float)ny * L[1], sz = (float)nz * L[2];
+                        if (pair_predicate(pos, i, j, sx, sy, sz, rl2)) {
+                            if (count < cap) {
+                                out_i[count] = (int32_t)i;
+                                out_j[count] = (int32_t)j;
+                                out_n[3 * count + 0] = nx;
+                                out_n[3 * count + 1] = ny;
+                                out_n[3 * count + 2] = nz;
+                            }
+                            ++count;
+                        }
+                    }
+    return count;
+}
+
+typedef struct {
+    int32_t j, nx, ny, nz;
+} cand_t;
+
+static int cand_cmp(const void *a, const void *b) {
+    const cand_t *x = (const cand_t *)a, *y = (const cand_t *)b;
+    if (x->j != y->j) return x->j < y->j ? -1 : 1;
+    if (x->nx != y->nx) return x->nx < y->nx ? -1 : 1;
+    if (x->ny != y->ny) return x->ny < y->ny ? -1 : 1;
+    if (x->nz != y->nz) return x->nz < y->nz ? -1 : 1;
+    return 0;
+}
+
+/* The oracle's own O(N) search (linked cells), used for N > 8192 and itself pinned against the
+ * brute force above.  Same predicate, same output order.  Needs >= 3 cells on every periodic
+ * axis (else returns -1: use the brute force). */
+int64_t oracle_neighbors_cells(int64_t N, const float *pos, const float *L, const int32_t *pbc, float r_list,
+                               int64_t cap, int32_t *out_i, int32_t *out_j, int32_t *out_n) {
+    int nc[3];
+    double edge[3];
+    for (int a = 0; a < 3; ++a) {
+        nc[a] = (int)floor((double)L[a] / ((double)r_list * (1.0 + 1e-6)));
+        if (nc[a] < 1) nc[a] = 1;
+        if (pbc[a] && nc[a] < 3) return -1;
+        edge[a] = (double)L[a] / nc[a];
+    }
+    const float rl2 = r_list * r_list;
+    int64_t ncell = (int64_t)nc[0] * nc[1] * nc[2];
+    int64_t *head = (int64_t *)malloc(sizeof(int64_t) * (size_t)ncell);
+    int64_t *next = (int64_t *)malloc(sizeof(int64_t) * (size_t)N);
+    int32_t *cidx = (int32_t *)malloc(sizeof(int32_t) * 3 * (size_t)N);
+    for (int64_t c = 0; c < ncell; ++c) head[c] = -1;
+    for (int64_t i = N - 1; i >= 0; --i) {
+        int c[3];
+        for (int a = 0; a < 3; ++a) {
+            c[a] = (int)floor((double)pos[3 * i + a] / edge[a]);
+            if (c[a] < 0) c[a] = 0;
+            if (c[a] >= nc[a]) c[a] = nc[a] - 1;
+            cidx[3 * i + a] = c[a];
+        }
+        int64_t cc = ((int64_t)c[0] * nc[1] + c[1]) * nc[2] + c[2];
+        next[i] = head[cc];
+        head[cc] = i;
+    }
+    int64_t count = 0;
+    size_t cand_cap = 1024;
+    cand_t *cand = (cand_t *)malloc(sizeof(cand_t) * cand_cap);
+    for (int64_t i = 0; i < N; ++i) {
+        size_t nc_i = 0;
+        for (int ox = -1; ox <= 1; ++ox)
+            for (int oy = -1; oy <= 1; ++oy)
+                for (int oz = -1; oz <= 1; ++oz) {
+                    int o[3] = {ox, oy, oz}, c[3], n[3];
+                    int skip = 0;
+                    for (int a = 0; a < 3; ++a) {
+                        c[a] = cidx[3 * i + a] + o[a];
+                        n[a] = 0;
+                        if (c[a] < 0) {
+                            if (!pbc[a]) { skip = 1; break; }
+                            c[a] += nc[a];
+                            n[a] = -1;
+                        } else if (c[a] >= nc[a]) {
+                            if (!pbc[a]) { skip = 1; break; }
+                            c[a] -= nc[a];
+                            n[a] = 1;
+                        }
+                    }
+                    if (skip) continue;
+                    /* with fewer than 3 cells on a NON-periodic axis, offsets can alias: visit once */
+                    int dup = 0;
+                    for (int a = 0; a < 3; ++a)
+                        if (!pbc[a] && nc[a] < 3 && (cidx[3 * i + a] + o[a] < 0 || cidx[3 * i + a] + o[a] >= nc[a])) dup = 1;
+                    if (dup) continue;
+                    float sx = (float)n[0] * L[0], sy = (float)n[1] * L[1], sz = (float)n[2] * L[2];
+                    int64_t cc = ((int64_t)c[0] * nc[1] + c[1]) * nc[2] + c[2];
+                    for (int64_t j = head[cc]; j >= 0; j = next[j]) {
+                        if (j == i && n[0] == 0 && n[1] == 0 && n[2] == 0) continue;
+                        if (pair_predicate(pos, i, j, sx, sy, sz, rl2)) {
+                            if (nc_i == cand_cap) {
+                                cand_cap *= 2;
+                                cand = (cand_t *)realloc(cand, sizeof(cand_t) * cand_cap);
+                            }
+                            cand[nc_i].j = (int32_t)j;
+                            cand[nc_i].nx = n[0];
+                            cand[nc_i].ny = n[1];
+                            cand[nc_i].nz = n[2];
+                            ++nc_i;
+                        }
+                    }
+                }
+        qsort(cand, nc_i, sizeof(cand_t), cand_cmp);
+        for (size_t q = 0; q < nc_i; ++q) {
+            if (count < cap) {
+                out_i[count] = (int32_t)i;
+                out_j[count] = cand[q].j;
+                out_n[3 * count + 0] = cand[q].nx;
+                out_n[3 * count + 1] = cand[q].ny;
+                out_n[3 * count + 2] = cand[q].nz;
+            }
+            ++count;
+        }
+    }
+    free(cand);
+    free(head);
+    free(next);
+    free(cidx);
+    return count;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O-2  Radial functions of one pair (readings R1-R4).
+ *   mu_k = r_min + k Delta, Delta = (r_cut - r_min)/(n_b - 1);  Phi_k = exp(-gamma (r - mu_k)^2)
+ *   f_c = 1/2 [1 + cos(pi r / r_cut)]  (r < r_cut, else 0)
+ *   R_s = f_c sum_k beta[Zi][Zj][s][k] Phi_k
+ *   R'_s = f_c' sum_k beta Phi_k + f_c sum_k beta Phi_k (-2 gamma (r - mu_k)),
+ *   f_c' = -(pi / (2 r_cut)) sin(pi r / r_cut)
+ * ------------------------------------------------------------------------------------------ */
+void oracle_radial(const oracle_hparams *hp, const double *beta, int zi, int zj, double r, double *R, double *dR) {
+    const int nb = hp->n_basis, nr = hp->n_radial, S = hp->n_species;
+    if (r >= hp->r_cut) {
+        for (int s = 0; s < nr; ++s) {
+            R[s] = 0.0;
+            if (dR) dR[s] = 0.0;
+        }
+        return;
+    }
+    const double delta = (hp->r_cut - hp->r_min) / (nb - 1);
+    const double fc = 0.5 * (1.0 + cos(M_PI * r / hp->r_cut));
+    const double dfc = -0.5 * M_PI / hp->r_cut * sin(M_PI * r / hp->r_cut);
+    for (int s = 0; s < nr; ++s) {
+        double sum = 0.0, dsum = 0.0;
+        for (int k = 0; k < nb; ++k) {
+            double mu = hp->r_min + k * delta;
+            double phi = exp(-hp->gamma * (r - mu) * (r - mu));
+            double bk = beta[(((size_t)zi * S + zj) * nr + s) * nb + k];
+            sum += bk * phi;
+            dsum += bk * phi * (-2.0 * hp->gamma * (r - mu));
+        }
+        R[s] = fc * sum;
+        if (dR) dR[s] = dfc * sum + fc * dsum;
+    }
+}
+
+/* d = x_j - x_i + n L in fp64 (positions are fp32 values promoted to fp64). */
+static inline void pair_vector(const double *pos, const double *L, int64_t i, int64_t j, const int32_t *n, double *d) {
+    for (int a = 0; a < 3; ++a) d[a] = pos[3 * j + a] - pos[3 * i + a] + n[a] * L[a];
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O-3  Moments of one atom (Eq. 2): u = d / r (direction i -> j);
+ *   P0[s] += R_s;  P1[s]_a += R_s u_a;  P2[s]_ab += R_s u_a u_b;  P3[s]_abc += R_s u_a u_b u_c.
+ * P is [n_radial][NC] with offsets O0, O1 + a, O2 + 3a + b, O3 + 9a + 3b + c.
+ * Pairs in the skin shell (r >= r_cut) contribute nothing.
+ * ------------------------------------------------------------------------------------------ */
+static void moments_of_atom(const oracle_hparams *hp, const double *beta, const double *pos, const int32_t *species,
+                            const double *L, int64_t i, int64_t p_begin, int64_t p_end, const int32_t *pj,
+                            const int32_t *pn, double *P) {
+    const int nr = hp->n_radial;
+    double R[16];
+    memset(P, 0, sizeof(double) * (size_t)nr * NC);
+    for (int64_t p = p_begin; p < p_end; ++p) {
+        double d[3];
+        pair_vector(pos, L, i, pj[p], pn + 3 * p, d);
+        double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+        if (r >= hp->r_cut) continue;
+        double u[3] = {d[0] / r, d[1] / r, d[2] / r};
+        oracle_radial(hp, beta, species[i], species[pj[p]], r, R, NULL);
+        for (int s = 0; s < nr; ++s) {
+            double *Ps = P + (size_t)s * NC;
+            Ps[O0] += R[s];
+            for (int a = 0; a < 3; ++a) {
+                Ps[O1 + a] += R[s] * u[a];
+                for (int b = 0; b < 3; ++b) {
+                    Ps[O2 + 3 * a + b] += R[s] * u[a] * u[b];
+                    for (int c = 0; c < 3; ++c) Ps[O3 + 9 * a + 3 * b + c] += R[s] * u[a] * u[b] * u[c];
+                }
+            }
+        }
+    }
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O-4  Invariants (Eq. 3).  First printed line = block 1, last printed line = block 7; the
+ * elided middle is completed with every full contraction of <= 3 moments with L <= 3 that is not
+ * a product of smaller ones (reading R7).  Blocks concatenated in this order; inside a block the
+ * index tuples run in lexicographic order and only symmetry-unique tuples are kept (R8):
+ *   0: P0[s]                                      s
+ *   1: P1[s1]_a   P1[s2]_a                        s1 <= s2
+ *   2: P2[s1]_ab  P2[s2]_ab                       s1 <= s2
+ *   3: P3[s1]_abc P3[s2]_abc                      s1 <= s2
+ *   4: P2[s1]_ab  P2[s2]_bc  P2[s3]_ca            s1 <= s2 <= s3
+ *   5: P1[s1]_a   P1[s2]_b   P2[s3]_ab            s1 <= s2, all s3
+ *   6: P3[s1]_abc P3[s2]_abd P2[s3]_cd            s1 <= s2, all s3
+ *   7: P1[s1]_a   P3[s2]_abc P2[s3]_bc            all s1, s2, s3
+ * ------------------------------------------------------------------------------------------ */
+#define P1_(s, a) P[(size_t)(s) * NC + O1 + (a)]
+#define P2_(s, a, b) P[(size_t)(s) * NC + O2 + 3 * (a) + (b)]
+#define P3_(s, a, b, c) P[(size_t)(s) * NC + O3 + 9 * (a) + 3 * (b) + (c)]
+#define Q1_(s, a) Q[(size_t)(s) * NC + O1 + (a)]
+#define Q2_(s, a, b) Q[(size_t)(s) * NC + O2 + 3 * (a) + (b)]
+#define Q3_(s, a, b, c) Q[(size_t)(s) * NC + O3 + 9 * (a) + 3 * (b) + (c)]
+
+void oracle_invariants(int nr, const double *P, double *G) {
+    int f = 0;
+    for (int s = 0; s < nr; ++s) G[f++] = P[(size_t)s * NC + O0];
+    for (int s1 = 0; s1 < nr; ++s1)
+        for (int s2 = s1; s2 < nr; ++s2) {
+            double g = 0.0;
+            for (int a = 0; a < 3; ++a) g += P1_(s1, a) * P1_(s2, a);
+            G[f++] = g;
+        }
+    for (int s1 = 0; s1 < nr; ++s1)
+        for (int s2 = s1; s2 < nr; ++s2) {
+            double g = 0.0;
+            for (int a = 0; a < 3; ++a)
+                for (int b = 0; b < 3; ++b) g += P2_(s1, a, b) * P2_(s2, a, b);
+            G[f++] = g;
+        }
+    for (int s1 = 0; s1 < nr; ++s1)
+        for (int s2 = s1; s2 < nr; ++s2) {
+            double g = 0.0;
+            for (int a = 0; a < 3; ++a)
+                for (int b = 0; b < 3; ++b)
+                    for (int c = 0; c < 3; ++c) g += P3_(s1, a, b, c) * P3_(s2, a, b, c);
+            G[f++] = g;
+        }
+    for (int s1 = 0; s1 < nr; ++s1)
+        for (int s2 = s1; s2 < nr; ++s2)
+            for (int s3 = s2; s3 < nr; ++s3) {
+                double g = 0.0;
+                for (int a = 0; a < 3; ++a)
+                    for (int b = 0; b < 3; ++b)
+                        for (int c = 0; c < 3; ++c) g += P2_(s1, a, b) * P2_(s2, b, c) * P2_(s3, c, a);
+                G[f++] = g;
+            }
+    for (int s1 = 0; s1 < nr; ++s1)
+        for (int s2 = s1; s2 < nr; ++s2)
+            for (int s3 = 0; s3 < nr; ++s3) {
+                double g = 0.0;
+                for (int a = 0; a < 3; ++a)
+                    for (int b = 0; b < 3; ++b) g += P1_(s1, a) * P1_(s2, b) * P2_(s3, a, b);
+                G[f++] = g;
+            }
+    for (int s1 = 0; s1 < nr; ++s1)
+        for (int s2 = s1; s2 < nr; ++s2)
+            for (int s3 = 0; s3 < nr; ++s3) {
+                double g = 0.0;
+                for (int a = 0; a < 3; ++a)
+                    for (int b = 0; b < 3; ++b)
+                        for (int c = 0; c < 3; ++c)
+                            for (int d = 0; d < 3; ++d) g += P3_(s1, a, b, c) * P3_(s2, a, b, d) * P2_(s3, c, d);
+                G[f++] = g;
+            }
+    for (int s1 = 0; s1 < nr; ++s1)
+        for (int s2 = 0; s2 < nr; ++s2)
+            for (int s3 = 0; s3 < nr; ++s3) {
+                double g = 0.0;
+                for (int a = 0; a < 3; ++a)
+                    for (int b = 0; b < 3; ++b)
+                        for (int c = 0; c < 3; ++c) g += P1_(s1, a) * P3_(s2, a, b, c) * P2_(s3, b, c);
+                G[f++] = g;
+            }
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O-8  Backward of O-4: Q = dE/dP given gb = dE/dG, every one of the 1+3+9+27 entries per
+ * channel treated as independent; a contribution is added for EACH slot even when channel
+ * indices coincide.  Q2, Q3 come out non-symmetric; that is intended.
+ * ------------------------------------------------------------------------------------------ */
+void oracle_invariants_bwd(int nr, const double *P, const double *gb, double *Q) {
+    memset(Q, 0, sizeof(double) * (size_t)nr * NC);
+    int f = 0;
+    for (int s = 0; s < nr; ++s) Q[(size_t)s * NC + O0] += gb[f++];
+    for (int s1 = 0; s1 < nr; ++s1)
+        for (int s2 = s1; s2 < nr; ++s2) {
+            double g = gb[f++];
+            for (int a = 0; a < 3; ++a) {
+                Q1_(s1, a) += g * P1_(s2, a);
+                Q1_(s2, a) += g * P1_(s1, a);
+            }
+        }
+    for (int s1 = 0; s1 < nr; ++s1)
+        for (int s2 = s1; s2 < nr; ++s2) {
+            double g = gb[f++];
+            for (int a = 0; a < 3; ++a)
+                for (int b = 0; b < 3; ++b) {
+                    Q2_(s1, a, b) += g * P2_(s2, a, b);
+                    Q2_(s2, a, b) += g * P2_(s1, a, b);
+                }
+        }
+    for (int s1 = 0; s1 < nr; ++s1)
+        for (int s2 = s1; s2 < nr; ++s2) {
+            double g = gb[f++];
+            for (int a = 0; a < 3; ++a)
+                for (int b = 0; b < 3; ++b)
+                    for (int c = 0; c < 3; ++c) {
+                        Q3_(s1, a, b, c) += g * P3_(s2, a, b, c);
+                        Q3_(s2, a, b, c) += g * P3_(s1, a, b, c);
+                    }
+        }
+    for (int s1 = 0; s1 < nr; ++s1)
+        for (int s2 = s1; s2 < nr; ++s2)
+            for (int s3 = s2; s3 < nr; ++s3) {
+                double g = gb[f++];
+                for (int a = 0; a < 3; ++a)
+                    for (int b = 0; b < 3; ++b)
+                        for (int c = 0; c < 3; ++c) {
+                            /* term = P2[s1]_ab P2[s2]_bc P2[s3]_ca */
+                            Q2_(s1, a, b) += g * P2_(s2, b, c) * P2_(s3, c, a);
+                            Q2_(s2, b, c) += g * P2_(s1, a, b) * P2_(s3, c, a);
+                            Q2_(s3, c, a) += g * P2_(s1, a, b) * P2_(s2, b, c);
+                        }
+            }
+    for (int s1 = 0; s1 < nr; ++s1)
+        for (int s2 = s1; s2 < nr; ++s2)
+            for (int s3 = 0; s3 < nr; ++s3) {
+                double g = gb[f++];
+                for (int a = 0; a < 3; ++a)
+                    for (int b = 0; b < 3; ++b) {
+                        /* term = P1[s1]_a P1[s2]_b P2[s3]_ab */
+                        Q1_(s1, a) += g * P1_(s2, b) * P2_(s3, a, b);
+                        Q1_(s2, b) += g * P1_(s1, a) * P2_(s3, a, b);
+                        Q2_(s3, a, b) += g * P1_(s1, a) * P1_(s2, b);
+                    }
+            }
+    for (int s1 = 0; s1 < nr; ++s1)
+        for (int s2 = s1; s2 < nr; ++s2)
+            for (int s3 = 0; s3 < nr; ++s3) {
+                double g = gb[f++];
+                for (int a = 0; a < 3; ++a)
+                    for (int b = 0; b < 3; ++b)
+                        for (int c = 0; c < 3; ++c)
+                            for (int d = 0; d < 3; ++d) {
+                                /* term = P3[s1]_abc P3[s2]_abd P2[s3]_cd */
+                                Q3_(s1, a, b, c) += g * P3_(s2, a, b, d) * P2_(s3, c, d);
+                                Q3_(s2, a, b, d) += g * P3_(s1, a, b, c) * P2_(s3, c, d);
+                                Q2_(s3, c, d) += g * P3_(s1, a, b, c) * P3_(s2, a, b, d);
+                            }
+            }
+    for (int s1 = 0; s1 < nr; ++s1)
+        for (int s2 = 0; s2 < nr; ++s2)
+            for (int s3 = 0; s3 < nr; ++s3) {
+                double g = gb[f++];
+                for (int a = 0; a < 3; ++a)
+                    for (int b = 0; b < 3; ++b)
+                        for (int c = 0; c < 3; ++c) {
+                            /* term = P1[s1]_a P3[s2]_abc P2[s3]_bc */
+                            Q1_(s1, a) += g * P3_(s2, a, b, c) * P2_(s3, b, c);
+                            Q3_(s2, a, b, c) += g * P1_(s1, a) * P2_(s3, b, c);
+                            Q2_(s3, b, c) += g * P1_(s1, a) * P3_(s2, a, b, c);
+                        }
+            }
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O-5  Readout (Eq. 4): z1 = G W1 + b1; h1 = swish(z1); ...; y = h W_last + b_last
+ * in R^M.  swish(x) = x sigmoid(x) (reading R10).  zs holds the pre-activations of the hidden
+ * layers back to back (sum of hidden[] doubles).
+ * ------------------------------------------------------------------------------------------ */
+static inline double sigmoid_(double x) { return 1.0 / (1.0 + exp(-x)); }
+static inline double swish_(double x) { return x * sigmoid_(x); }
+static inline double dswish_(double x) {
+    double s = sigmoid_(x);
+    return s * (1.0 + x * (1.0 - s));
+}
+double oracle_swish(double x) { return swish_(x); }
+double oracle_dswish(double x) { return dswish_(x); }
+
+void oracle_mlp_forward(const oracle_hparams *hp, const oracle_weights *w, int n_in, const double *G, double *zs,
+                        double *y) {
+    const double *h = G;
+    int fan_in = n_in;
+    double hbuf[2][4096];
+    double *z = zs;
+    for (int l = 0; l < hp->n_hidden; ++l) {
+        int fo = hp->hidden[l];
+        for (int o = 0; o < fo; ++o) {
+            double acc = w->b[l][o];
+            for (int k = 0; k < fan_in; ++k) acc += h[k] * w->W[l][(size_t)k * fo + o];
+            z[o] = acc;
+        }
+        double *hn = hbuf[l & 1];
+        for (int o = 0; o < fo; ++o) hn[o] = swish_(z[o]);
+        h = hn;
+        z += fo;
+        fan_in = fo;
+    }
+    const int L = hp->n_hidden, M = hp->n_heads;
+    for (int m = 0; m < M; ++m) {
+        double acc = w->b[L][m];
+        for (int k = 0; k < fan_in; ++k) acc += h[k] * w->W[L][(size_t)k * M + m];
+        y[m] = acc;
+    }
+}
+
+/* O-7  Backward to the features: ybar[m] given; hbar = W_last ybar; zbar = hbar * swish'(z);
+ * ... ; Gbar = W1 zbar1. */
+void oracle_mlp_backward(const oracle_hparams *hp, const oracle_weights *w, int n_in, const double *zs,
+                         const double *ybar, double *Gbar) {
+    const int L = hp->n_hidden, M = hp->n_heads;
+    double buf[2][4096];
+    int width_last = L > 0 ? hp->hidden[L - 1] : n_in;
+    double *hb = buf[0];
+    for (int k = 0; k < width_last; ++k) {
+        double acc = 0.0;
+        for (int m = 0; m < M; ++m) acc += w->W[L][(size_t)k * M + m] * ybar[m];
+        hb[k] = acc;
+    }
+    int zoff = 0;
+    for (int l = 0; l < L; ++l) zoff += hp->hidden[l];
+    for (int l = L - 1; l >= 0; --l) {
+        int fo = hp->hidden[l];
+        int fi = l > 0 ? hp->hidden[l - 1] : n_in;
+        zoff -= fo;
+        const double *z = zs + zoff;
+        double *nb = buf[(L - l) & 1];
+        for (int k = 0; k < fi; ++k) nb[k] = 0.0;
+        for (int o = 0; o < fo; ++o) {
+            double zb = hb[o] * dswish_(z[o]);
+            for (int k = 0; k < fi; ++k) nb[k] += w->W[l][(size_t)k * fo + o] * zb;
+        }
+        hb = nb;
+    }
+    for (int k = 0; k < n_in; ++k) Gbar[k] = hb[k];
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O-9  Pair gradient for one kept pair with r < r_cut, using Q of the centre atom i:
+ *   c_s = Q0[s] + Q1[s]_a u_a + Q2[s]_ab u_a u_b + Q3[s]_abc u_a u_b u_c
+ *   w_a = sum_s R_s [ Q1[s]_a + (Q2[s]_ab + Q2[s]_ba) u_b
+ *                     + (Q3[s]_abc + Q3[s]_bac + Q3[s]_bca) u_b u_c ]
+ *   g   = (sum_s R'_s c_s) u + (w - (w.u) u) / r        ( = dE/dd )
+ * F_i += g;  F_j -= g   (d = x_j - x_i + shift, so dE/dx_i = -g and F = -dE/dx).
+ * ------------------------------------------------------------------------------------------ */
+static void pair_gradient(const oracle_hparams *hp, const double *beta, int zi, int zj, const double *d,
+                          const double *Q, double *g) {
+    const int nr = hp->n_radial;
+    double R[16], dR[16];
+    double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+    g[0] = g[1] = g[2] = 0.0;
+    if (r >= hp->r_cut) return;
+    double u[3] = {d[0] / r, d[1] / r, d[2] / r};
+    oracle_radial(hp, beta, zi, zj, r, R, dR);
+    double radial = 0.0, w[3] = {0.0, 0.0, 0.0};
+    for (int s = 0; s < nr; ++s) {
+        double c = Q[(size_t)s * NC + O0];
+        for (int a = 0; a < 3; ++a) {
+            c += Q1_(s, a) * u[a];
+            for (int b = 0; b < 3; ++b) {
+                c += Q2_(s, a, b) * u[a] * u[b];
+                for (int cc = 0; cc < 3; ++cc) c += Q3_(s, a, b, cc) * u[a] * u[b] * u[cc];
+            }
+        }
+        radial += dR[s] * c;
+        for (int a = 0; a < 3; ++a) {
+            double t = Q1_(s, a);
+            for (int b = 0; b < 3; ++b) {
+                t += (Q2_(s, a, b) + Q2_(s, b, a)) * u[b];
+                for (int cc = 0; cc < 3; ++cc)
+                    t += (Q3_(s, a, b, cc) + Q3_(s, b, a, cc) + Q3_(s, b, cc, a)) * u[b] * u[cc];
+            }
+            w[a] += R[s] * t;
+        }
+    }
+    double wu = w[0] * u[0] + w[1] * u[1] + w[2] * u[2];
+    for (int a = 0; a < 3; ++a) g[a] = radial * u[a] + (w[a] - wu * u[a]) / r;
+}
+
+/* CSR row offsets of a pair list sorted by i. */
+static int64_t *row_offsets(int64_t N, int64_t npairs, const int32_t *pi) {
+    int64_t *off = (int64_t *)calloc((size_t)N + 1, sizeof(int64_t));
+    for (int64_t p = 0; p < npairs; ++p) off[pi[p] + 1]++;
+    for (int64_t i = 0; i < N; ++i) off[i + 1] += off[i];
+    return off;
+}
+
+static int total_hidden(const oracle_hparams *hp) {
+    int t = 0;
+    for (int l = 0; l < hp->n_hidden; ++l) t += hp->hidden[l];
+    return t;
+}
+
+/* Forward of every atom: P [N][nr][NC], G [N][F], zs [N][sum hidden], E_heads [N][M]
+ * (E_i^(m) = sigma[Z_i] y_m + mu[Z_i], reading R12). */
+static void forward_all(const oracle_hparams *hp, const oracle_weights *w, int64_t N, const double *pos,
+                        const int32_t *species, const double *L, const int64_t *off, const int32_t *pj,
+                        const int32_t *pn, double *P, double *G, double *zs, double *E_heads) {
+    const int nr = hp->n_radial, F = oracle_n_features(nr), H = total_hidden(hp), M = hp->n_heads;
+#pragma omp parallel for schedule(dynamic, 8)
+    for (int64_t i = 0; i < N; ++i) {
+        double y[64];
+        double *Pi = P + (size_t)i * nr * NC;
+        moments_of_atom(hp, w->beta, pos, species, L, i, off[i], off[i + 1], pj, pn, Pi);
+        oracle_invariants(nr, Pi, G + (size_t)i * F);
+        oracle_mlp_forward(hp, w, F, G + (size_t)i * F, zs + (size_t)i * H, y);
+        for (int m = 0; m < M; ++m) E_heads[(size_t)i * M + m] = w->scale[species[i]] * y[m] + w->shift[species[i]];
+    }
+}
+
+/* Backward of the energy E_c = sum_i sum_m head_w[m] E_i^(m): forces [N][3]; optional dG, Q. */
+static void backward_all(const oracle_hparams *hp, const oracle_weights *w, int64_t N, const double *pos,
+                         const int32_t *species, const double *L, int64_t npairs, const int64_t *off,
+                         const int32_t *pj, const int32_t *pn, const double *P, const double *zs,
+                         const double *head_w, double *Fout, double *dG_out, double *Q_out) {
+    const int nr = hp->n_radial, F = oracle_n_features(nr), H = total_hidden(hp), M = hp->n_heads;
+    double *gpair = (double *)malloc(sizeof(double) * 3 * (size_t)(npairs > 0 ? npairs : 1));
+    memset(Fout, 0, sizeof(double) * 3 * (size_t)N);
+#pragma omp parallel for schedule(dynamic, 8)
+    for (int64_t i = 0; i < N; ++i) {
+        double ybar[64], Gbar[1024], Qloc[16 * NC];
+        for (int m = 0; m < M; ++m) ybar[m] = w->scale[species[i]] * head_w[m];
+        oracle_mlp_backward(hp, w, F, zs + (size_t)i * H, ybar, Gbar);
+        oracle_invariants_bwd(nr, P + (size_t)i * nr * NC, Gbar, Qloc);
+        if (dG_out) memcpy(dG_out + (size_t)i * F, Gbar, sizeof(double) * F);
+        if (Q_out) memcpy(Q_out + (size_t)i * nr * NC, Qloc, sizeof(double) * nr * NC);
+        for (int64_t p = off[i]; p < off[i + 1]; ++p) {
+            double d[3];
+            pair_vector(pos, L, i, pj[p], pn + 3 * p, d);
+            pair_gradient(hp, w->beta, species[i], species[pj[p]], d, Qloc, gpair + 3 * p);
+            for (int a = 0; a < 3; ++a) Fout[3 * i + a] += gpair[3 * p + a];
+        }
+    }
+    for (int64_t i = 0; i < N; ++i)
+        for (int64_t p = off[i]; p < off[i + 1]; ++p)
+            for (int a = 0; a < 3; ++a) Fout[3 * (size_t)pj[p] + a] -= gpair[3 * p + a];
+    free(gpair);
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O-1..O-9 on a given pair list (sorted by i).  head_w[M]: weights of the heads in the energy
+ * whose gradient becomes F (single model: M = 1, head_w = {1}; mean energy: 1/M each).
+ * Outputs: E_heads [N][M]; F [N][3]; nullable P [N][nr][40], G [N][F], dG [N][F], Q [N][nr][40].
+ * Returns 0, or -1 on a bad argument.
+ * ------------------------------------------------------------------------------------------ */
+int oracle_energy_forces(const oracle_hparams *hp, const oracle_weights *w, int64_t N, const double *pos,
+                         const int32_t *species, const double *L, int64_t npairs, const int32_t *pi,
+                         const int32_t *pj, const int32_t *pn, const double *head_w, double *E_heads, double *Fout,
+                         double *P_out, double *G_out, double *dG_out, double *Q_out) {
+    if (hp->n_radial > 16 || hp->n_heads > 64 || hp->n_hidden > 4) return -1;
+    const int nr = hp->n_radial, F = oracle_n_features(nr), H = total_hidden(hp);
+    if (F > 1024) return -1;
+    for (int l = 0; l < hp->n_hidden; ++l)
+        if (hp->hidden[l] > 4096) return -1;
+    int64_t *off = row_offsets(N, npairs, pi);
+    double *P = P_out ? P_out : (double *)malloc(sizeof(double) * (size_t)N * nr * NC);
+    double *G = G_out ? G_out : (double *)malloc(sizeof(double) * (size_t)N * F);
+    double *zs = (double *)malloc(sizeof(double) * (size_t)N * (H > 0 ? H : 1));
+    forward_all(hp, w, N, pos, species, L, off, pj, pn, P, G, zs, E_heads);
+    if (Fout) backward_all(hp, w, N, pos, species, L, npairs, off, pj, pn, P, zs, head_w, Fout, dG_out, Q_out);
+    free(off);
+    if (!P_out) free(P);
+    if (!G_out) free(G);
+    free(zs);
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O-10  Shallow ensemble (Eq. 5, 6): forward once; for every head m the backward with
+ * ybar = sigma e_m gives F^(m).  e_mean_i = 1/M sum_m E_i^(m); e_var_i = 1/M sum_m (E_i^(m) -
+ * mean)^2 (population divisor, reading R13); f_mean, f_var likewise per atom and component.
+ * F_heads [M][N][3] nullable.
+ * ------------------------------------------------------------------------------------------ */
+int oracle_ensemble(const oracle_hparams *hp, const oracle_weights *w, int64_t N, const double *pos,
+                    const int32_t *species, const double *L, int64_t npairs, const int32_t *pi, const int32_t *pj,
+                    const int32_t *pn, double *E_heads, double *e_mean, double *e_var, double *f_mean, double *f_var,
+                    double *F_heads) {
+    if (hp->n_radial > 16 || hp->n_heads > 64 || hp->n_hidden > 4) return -1;
+    const int nr = hp->n_radial, F = oracle_n_features(nr), H = total_hidden(hp), M = hp->n_heads;
+    int64_t *off = row_offsets(N, npairs, pi);
+    double *P = (double *)malloc(sizeof(double) * (size_t)N * nr * NC);
+    double *G = (double *)malloc(sizeof(double) * (size_t)N * F);
+    double *zs = (double *)malloc(sizeof(double) * (size_t)N * (H > 0 ? H : 1));
+    double *Fall = F_heads ? F_heads : (double *)malloc(sizeof(double) * (size_t)M * N * 3);
+    forward_all(hp, w, N, pos, species, L, off, pj, pn, P, G, zs, E_heads);
+    for (int m = 0; m < M; ++m) {
+        double hw[64];
+        for (int q = 0; q < M; ++q) hw[q] = (q == m) ? 1.0 : 0.0;
+        backward_all(hp, w, N, pos, species, L, npairs, off, pj, pn, P, zs, hw, Fall + (size_t)m * N * 3, NULL, NULL);
+    }
+    for (int64_t i = 0; i < N; ++i) {
+        double mean = 0.0, var = 0.0;
+        for (int m = 0; m < M; ++m) mean += E_heads[(size_t)i * M + m];
+        mean /= M;
+        for (int m = 0; m < M; ++m) var += (E_heads[(size_t)i * M + m] - mean) * (E_heads[(size_t)i * M + m] - mean);
+        e_mean[i] = mean;
+        e_var[i] = var / M;
+        for (int a = 0; a < 3; ++a) {
+            double fm = 0.0, fv = 0.0;
+            for (int m = 0; m < M; ++m) fm += Fall[((size_t)m * N + i) * 3 + a];
+            fm /= M;
+            for (int m = 0; m < M; ++m) {
+                double dlt = Fall[((size_t)m * N + i) * 3 + a] - fm;
+                fv += dlt * dlt;
+            }
+            f_mean[3 * i + a] = fm;
+            f_var[3 * i + a] = fv / M;
+        }
+    }
+    free(off);
+    free(P);
+    free(G);
+    free(zs);
+    if (!F_heads) free(Fall);
+    return 0;
+}
+
+/* Neighbour list of fp64 positions (cast to fp32 for the predicate), growing buffers. */
+typedef struct {
+    int64_t n, cap;
+    int32_t *i, *j, *n3;
+} pairlist_t;
+
+static void build_list(pairlist_t *pl, int64_t N, const double *pos, const double *L, const int32_t *pbc,
+                       double r_list) {
+    float *p32 = (float *)malloc(sizeof(float) * 3 * (size_t)N);
+    float L32[3] = {(float)L[0], (float)L[1], (float)L[2]};
+    for (int64_t q = 0; q < 3 * N; ++q) p32[q] = (float)pos[q];
+    for (;;) {
+        int64_t n = oracle_neighbors_cells(N, p32, L32, pbc, (float)r_list, pl->cap, pl->i, pl->j, pl->n3);
+        if (n < 0) n = oracle_neighbors_brute(N, p32, L32, pbc, (float)r_list, pl->cap, pl->i, pl->j, pl->n3);
+        if (n <= pl->cap) {
+            pl->n = n;
+            break;
+        }
+        pl->cap = n + n / 8 + 64;
+        pl->i = (int32_t *)realloc(pl->i, sizeof(int32_t) * (size_t)pl->cap);
+        pl->j = (int32_t *)realloc(pl->j, sizeof(int32_t) * (size_t)pl->cap);
+        pl->n3 = (int32_t *)realloc(pl->n3, sizeof(int32_t) * 3 * (size_t)pl->cap);
+    }
+    free(p32);
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O-11  NVE velocity Verlet, n_steps steps of dt (fs):
+ *   v += (dt/2) a(F);  x += dt v;  wrap x into [0, L) on periodic axes;
+ *   if max_i |x_i - x_ref,i| > skin/2 (unwrapped displacement since the last build): rebuild,
+ *   x_ref <- x;   F <- O-1..O-9;   v += (dt/2) a(F).      a = F/m * 9.648533212e-3.
+ * E_kin = 1/2 sum m v^2 / 9.648533212e-3.  epot/ekin [n_steps + 1] (index 0 = initial state).
+ * x, v are updated in place; x is returned wrapped.
+ *
+ * The image vectors n of a list refer to the coordinates it was built from, so between builds
+ * the pair vectors are taken from xu, the unwrapped continuation of the build coordinates
+ * (xu = x_ref + displacement); the wrapped x is xu folded back into the cell.  E and F do not
+ * depend on which image of an atom is used, so this is O-11 exactly.  With skin == 0 any motion
+ * exceeds skin/2 and the list is rebuilt every step.
+ * ------------------------------------------------------------------------------------------ */
+int oracle_nve(const oracle_hparams *hp, const oracle_weights *w, int64_t N, double *x, double *v,
+               const double *masses, const int32_t *species, const double *L, const int32_t *pbc, double skin,
+               double dt, int64_t n_steps, double *epot, double *ekin, int64_t *n_rebuilds) {
+    if (hp->n_heads != 1) return -1;
+    pairlist_t pl = {0, 0, NULL, NULL, NULL};
+    double *F = (double *)malloc(sizeof(double) * 3 * (size_t)N);
+    double *Ei = (double *)malloc(sizeof(double) * (size_t)N);
+    double *xu = (double *)malloc(sizeof(double) * 3 * (size_t)N);   /* list-consistent coordinates */
+    double *xref = (double *)malloc(sizeof(double) * 3 * (size_t)N); /* xu at the last build */
+    const double one = 1.0;
+    int64_t rebuilds = 0;
+    for (int64_t i = 0; i < N; ++i)
+        for (int a = 0; a < 3; ++a)
+            if (pbc[a]) x[3 * i + a] -= floor(x[3 * i + a] / L[a]) * L[a];
+    memcpy(xu, x, sizeof(double) * 3 * (size_t)N);
+    memcpy(xref, x, sizeof(double) * 3 * (size_t)N);
+    build_list(&pl, N, x, L, pbc, hp->r_cut + skin);
+    oracle_energy_forces(hp, w, N, xu, species, L, pl.n, pl.i, pl.j, pl.n3, &one, Ei, F, NULL, NULL, NULL, NULL);
+    for (int64_t step = 0;; ++step) {
+        double ep = 0.0, ek = 0.0;
+        for (int64_t i = 0; i < N; ++i) {
+            ep += Ei[i];
+            ek += 0.5 * masses[i] * (v[3 * i] * v[3 * i] + v[3 * i + 1] * v[3 * i + 1] + v[3 * i + 2] * v[3 * i + 2]);
+        }
+        epot[step] = ep;
+        ekin[step] = ek / ACC_CONV;
+        if (step == n_steps) break;
+        double maxd2 = 0.0;
+        for (int64_t i = 0; i < N; ++i) {
+            double d2 = 0.0;
+            for (int a = 0; a < 3; ++a) {
+                v[3 * i + a] += 0.5 * dt * F[3 * i + a] / masses[i] * ACC_CONV;
+                xu[3 * i + a] += dt * v[3 * i + a];
+                x[3 * i + a] = pbc[a] ? xu[3 * i + a] - floor(xu[3 * i + a] / L[a]) * L[a] : xu[3 * i + a];
+                double dd = xu[3 * i + a] - xref[3 * i + a];
+                d2 += dd * dd;
+            }
+            if (d2 > maxd2) maxd2 = d2;
+        }
+        if (sqrt(maxd2) > 0.5 * skin) {
+            memcpy(xu, x, sizeof(double) * 3 * (size_t)N);
+            memcpy(xref, x, sizeof(double) * 3 * (size_t)N);
+            build_list(&pl, N, x, L, pbc, hp->r_cut + skin);
+            ++rebuilds;
+        }
+        oracle_energy_forces(hp, w, N, xu, species, L, pl.n, pl.i, pl.j, pl.n3, &one, Ei, F, NULL, NULL, NULL, NULL);
+        for (int64_t i = 0; i < N; ++i)
+            for (int a = 0; a < 3; ++a) v[3 * i + a] += 0.5 * dt * F[3 * i + a] / masses[i] * ACC_CONV;
+    }
+    if (n_rebuilds) *n_rebuilds = rebuilds;
+    free(F);
+    free(Ei);
+    free(xu);
+    free(xref);
+    free(pl.i);
+    free(pl.j);
+    free(pl.n3);
+    return 0;
+}

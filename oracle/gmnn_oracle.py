@@ -1,0 +1,322 @@
+"""ctypes face of oracle/gmnn_oracle.c -- TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+import this module.  It imports nothing from paper_2505_22168_b200/ and shares no code with it.
+All floating point crosses this boundary as fp64 (fp32 inputs are promoted, never the reverse),
+except the positions handed to the neighbour search, whose predicate is specified in fp32
+(reading R20).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from dataclasses import dataclass
+from typing import Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "gmnn_oracle.c")
+_LIB = os.path.join(_HERE, "libgmnn_oracle.so")
+NC = 40  # components per channel: 1 + 3 + 9 + 27
+GCC_FLAGS = ["-O2", "-std=c11", "-fPIC", "-shared", "-fopenmp", "-ffp-contract=off"]
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with gcc if the shared object is missing or older than its source."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + ".tmp%d" % os.getpid()
+        subprocess.check_call(["gcc", *GCC_FLAGS, _SRC, "-lm", "-o", tmp])
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+class _HParams(C.Structure):
+    _fields_ = [
+        ("n_species", C.c_int32), ("n_basis", C.c_int32), ("n_radial", C.c_int32),
+        ("r_cut", C.c_double), ("r_min", C.c_double), ("gamma", C.c_double),
+        ("n_hidden", C.c_int32), ("hidden", C.c_int32 * 4), ("n_heads", C.c_int32),
+    ]
+
+
+class _Weights(C.Structure):
+    _fields_ = [
+        ("beta", C.c_void_p), ("W", C.c_void_p * 5), ("b", C.c_void_p * 5),
+        ("scale", C.c_void_p), ("shift", C.c_void_p),
+    ]
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(build())
+        _lib.oracle_neighbors_brute.restype = C.c_int64
+        _lib.oracle_neighbors_cells.restype = C.c_int64
+        _lib.oracle_swish.restype = C.c_double
+        _lib.oracle_dswish.restype = C.c_double
+        _lib.oracle_swish.argtypes = [C.c_double]
+        _lib.oracle_dswish.argtypes = [C.c_double]
+    return _lib
+
+
+def _p(a: Optional[np.ndarray]):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+def _f64(a) -> np.ndarray:
+    return np.ascontiguousarray(np.asarray(a), dtype=np.float64)
+
+
+def _i32(a) -> np.ndarray:
+    return np.ascontiguousarray(np.asarray(a), dtype=np.int32)
+
+
+def num_threads() -> int:
+    return int(lib().oracle_num_threads())
+
+
+def set_num_threads(n: int) -> None:
+    lib().oracle_set_num_threads(C.c_int(n))
+
+
+def n_features(n_radial: int) -> int:
+    return int(lib().oracle_n_features(C.c_int(n_radial)))
+
+
+class Model:
+    """fp64 copy of a model (any object with the attributes of workloads.ModelSpec)."""
+
+    def __init__(self, spec):
+        self.n_species = int(spec.n_species)
+        self.n_basis = int(spec.n_basis)
+        self.n_radial = int(spec.n_radial)
+        self.r_cut = float(spec.r_cut)
+        self.r_min = float(spec.r_min)
+        self.gamma = float(spec.gamma)
+        self.hidden = tuple(int(h) for h in spec.hidden)
+        self.n_heads = int(spec.n_heads)
+        self.beta = _f64(spec.beta)
+        self.W = [_f64(w) for w in spec.W]
+        self.b = [_f64(b) for b in spec.b]
+        self.scale = _f64(spec.scale)
+        self.shift = _f64(spec.shift)
+        assert len(self.W) == len(self.hidden) + 1
+        self.n_features = n_features(self.n_radial)
+        assert self.W[0].shape[0] == self.n_features, (self.W[0].shape, self.n_features)
+        self.hp = _HParams()
+        self.hp.n_species, self.hp.n_basis, self.hp.n_radial = self.n_species, self.n_basis, self.n_radial
+        self.hp.r_cut, self.hp.r_min, self.hp.gamma = self.r_cut, self.r_min, self.gamma
+        self.hp.n_hidden = len(self.hidden)
+        for l, h in enumerate(self.hidden):
+            self.hp.hidden[l] = h
+        self.hp.n_heads = self.n_heads
+        self.w = _Weights()
+        self.w.beta = _p(self.beta)
+        for l in range(len(self.W)):
+            self.w.W[l] = self.W[l].ctypes.data
+            self.w.b[l] = self.b[l].ctypes.data
+        self.w.scale = _p(self.scale)
+        self.w.shift = _p(self.shift)
+
+
+@dataclass
+class Pairs:
+    i: np.ndarray  # [n] i32
+    j: np.ndarray  # [n] i32
+    n: np.ndarray  # [n][3] i32 image vector
+
+    def __len__(self):
+        return int(self.i.shape[0])
+
+    def as_set_array(self) -> np.ndarray:
+        """[n][5] int32 rows (i, j, nx, ny, nz), already sorted by the oracle."""
+        return np.concatenate([self.i[:, None], self.j[:, None], self.n], axis=1)
+
+
+def neighbors(positions, cell, pbc, r_list: float, method: str = "brute") -> Pairs:
+    """O-1.  positions [N][3] are rounded to fp32 (the predicate's precision); cell [3]."""
+    pos = np.ascontiguousarray(np.asarray(positions), dtype=np.float32)
+    L = np.ascontiguousarray(np.asarray(cell), dtype=np.float32).reshape(-1)
+    assert L.shape[0] == 3
+    pb = _i32(pbc)
+    N = pos.shape[0]
+    fn = {"brute": lib().oracle_neighbors_brute, "cells": lib().oracle_neighbors_cells}[method]
+    cap = max(1024, 128 * N)
+    while True:
+        oi = np.empty(cap, np.int32)
+        oj = np.empty(cap, np.int32)
+        on = np.empty((cap, 3), np.int32)
+        n = fn(C.c_int64(N), _p(pos), _p(L), _p(pb), C.c_float(r_list), C.c_int64(cap), _p(oi), _p(oj), _p(on))
+        if n < 0:
+            raise ValueError("cell list needs >= 3 cells on every periodic axis; use method='brute'")
+        if n <= cap:
+            return Pairs(oi[:n].copy(), oj[:n].copy(), on[:n].copy())
+        cap = int(n)
+
+
+def auto_neighbors(positions, cell, pbc, r_list: float) -> Pairs:
+    """Brute force up to 8192 atoms, the oracle's own cell list above."""
+    N = np.asarray(positions).shape[0]
+    if N <= 8192:
+        return neighbors(positions, cell, pbc, r_list, "brute")
+    try:
+        return neighbors(positions, cell, pbc, r_list, "cells")
+    except ValueError:
+        return neighbors(positions, cell, pbc, r_list, "brute")
+
+
+def radial(model: Model, zi: int, zj: int, r: float):
+    """O-2 for one pair: (R [n_radial], dR/dr [n_radial])."""
+    R = np.zeros(model.n_radial)
+    dR = np.zeros(model.n_radial)
+    lib().oracle_radial(C.byref(model.hp), _p(model.beta), C.c_int(zi), C.c_int(zj), C.c_double(r), _p(R), _p(dR))
+    return R, dR
+
+
+def invariants(n_radial: int, P) -> np.ndarray:
+    """O-4 for one atom: P [n_radial][40] -> G [F]."""
+    P = _f64(P)
+    assert P.shape == (n_radial, NC)
+    G = np.zeros(n_features(n_radial))
+    lib().oracle_invariants(C.c_int(n_radial), _p(P), _p(G))
+    return G
+
+
+def invariants_bwd(n_radial: int, P, gbar) -> np.ndarray:
+    """O-8 for one atom: Q [n_radial][40] = dE/dP given gbar = dE/dG."""
+    P = _f64(P)
+    gbar = _f64(gbar)
+    Q = np.zeros((n_radial, NC))
+    lib().oracle_invariants_bwd(C.c_int(n_radial), _p(P), _p(gbar), _p(Q))
+    return Q
+
+
+def mlp_forward(model: Model, G):
+    """O-5 for one atom: (y [M], zs [sum hidden])."""
+    G = _f64(G)
+    zs = np.zeros(max(1, sum(model.hidden)))
+    y = np.zeros(model.n_heads)
+    lib().oracle_mlp_forward(C.byref(model.hp), C.byref(model.w), C.c_int(G.shape[0]), _p(G), _p(zs), _p(y))
+    return y, zs
+
+
+def mlp_backward(model: Model, zs, ybar, n_in: int) -> np.ndarray:
+    """O-7 for one atom: dE/dG given ybar [M]."""
+    zs = _f64(zs)
+    ybar = _f64(ybar)
+    Gbar = np.zeros(n_in)
+    lib().oracle_mlp_backward(C.byref(model.hp), C.byref(model.w), C.c_int(n_in), _p(zs), _p(ybar), _p(Gbar))
+    return Gbar
+
+
+def swish(x: float) -> float:
+    return float(lib().oracle_swish(C.c_double(x)))
+
+
+def dswish(x: float) -> float:
+    return float(lib().oracle_dswish(C.c_double(x)))
+
+
+@dataclass
+class Result:
+    energy: float  # sum_i sum_m head_w[m] E_i^(m)
+    e_heads: np.ndarray  # [N][M]
+    forces: Optional[np.ndarray]  # [N][3]
+    P: Optional[np.ndarray] = None  # [N][n_radial][40]
+    G: Optional[np.ndarray] = None  # [N][F]
+    dG: Optional[np.ndarray] = None  # [N][F]
+    Q: Optional[np.ndarray] = None  # [N][n_radial][40]
+
+    @property
+    def e_atom(self) -> np.ndarray:
+        return self.e_heads[:, 0]
+
+
+def energy_forces(model: Model, positions, species, cell, pairs: Pairs, head_w: Optional[Sequence[float]] = None,
+                  forces: bool = True, intermediates: bool = False) -> Result:
+    """O-2..O-9 on a pair list.  head_w: weights of the heads in the differentiated energy
+    (default: 1 for a single head, 1/M each for an ensemble = gradient of the mean energy)."""
+    pos = _f64(positions)
+    sp = _i32(species)
+    L = _f64(cell).reshape(-1)
+    N = pos.shape[0]
+    M = model.n_heads
+    hw = _f64(np.full(M, 1.0 / M) if head_w is None else head_w)
+    assert hw.shape == (M,)
+    F = model.n_features
+    e_heads = np.zeros((N, M))
+    f = np.zeros((N, 3)) if forces else None
+    Pm = np.zeros((N, model.n_radial, NC)) if intermediates else None
+    G = np.zeros((N, F)) if intermediates else None
+    dG = np.zeros((N, F)) if (intermediates and forces) else None
+    Q = np.zeros((N, model.n_radial, NC)) if (intermediates and forces) else None
+    pi, pj, pn = _i32(pairs.i), _i32(pairs.j), _i32(pairs.n)
+    rc = lib().oracle_energy_forces(
+        C.byref(model.hp), C.byref(model.w), C.c_int64(N), _p(pos), _p(sp), _p(L), C.c_int64(len(pairs)),
+        _p(pi), _p(pj), _p(pn), _p(hw), _p(e_heads), _p(f), _p(Pm), _p(G), _p(dG), _p(Q))
+    if rc != 0:
+        raise ValueError("oracle_energy_forces: bad argument")
+    return Result(float((e_heads @ hw).sum()), e_heads, f, Pm, G, dG, Q)
+
+
+@dataclass
+class EnsembleResult:
+    e_heads: np.ndarray  # [N][M]
+    e_mean: np.ndarray  # [N]
+    e_var: np.ndarray  # [N]
+    f_mean: np.ndarray  # [N][3]
+    f_var: np.ndarray  # [N][3]
+    f_heads: Optional[np.ndarray]  # [M][N][3]
+
+
+def ensemble(model: Model, positions, species, cell, pairs: Pairs, keep_heads: bool = False) -> EnsembleResult:
+    """O-10 (Eq. 5 with the 1/N_ens divisor, Eq. 6)."""
+    pos = _f64(positions)
+    sp = _i32(species)
+    L = _f64(cell).reshape(-1)
+    N = pos.shape[0]
+    M = model.n_heads
+    e_heads = np.zeros((N, M))
+    e_mean, e_var = np.zeros(N), np.zeros(N)
+    f_mean, f_var = np.zeros((N, 3)), np.zeros((N, 3))
+    fh = np.zeros((M, N, 3)) if keep_heads else None
+    pi, pj, pn = _i32(pairs.i), _i32(pairs.j), _i32(pairs.n)
+    rc = lib().oracle_ensemble(
+        C.byref(model.hp), C.byref(model.w), C.c_int64(N), _p(pos), _p(sp), _p(L), C.c_int64(len(pairs)),
+        _p(pi), _p(pj), _p(pn), _p(e_heads), _p(e_mean), _p(e_var), _p(f_mean), _p(f_var), _p(fh))
+    if rc != 0:
+        raise ValueError("oracle_ensemble: bad argument")
+    return EnsembleResult(e_heads, e_mean, e_var, f_mean, f_var, fh)
+
+
+@dataclass
+class NVEResult:
+    positions: np.ndarray
+    velocities: np.ndarray
+    epot: np.ndarray  # [n_steps + 1]
+    ekin: np.ndarray  # [n_steps + 1]
+    n_rebuilds: int
+
+
+def nve(model: Model, positions, velocities, masses, species, cell, pbc, skin: float, dt_fs: float,
+        n_steps: int) -> NVEResult:
+    """O-11 velocity Verlet."""
+    x = _f64(positions).copy()
+    v = _f64(velocities).copy()
+    m = _f64(masses)
+    sp = _i32(species)
+    L = _f64(cell).reshape(-1)
+    pb = _i32(pbc)
+    epot = np.zeros(n_steps + 1)
+    ekin = np.zeros(n_steps + 1)
+    nreb = C.c_int64(0)
+    rc = lib().oracle_nve(
+        C.byref(model.hp), C.byref(model.w), C.c_int64(x.shape[0]), _p(x), _p(v), _p(m), _p(sp), _p(L), _p(pb),
+        C.c_double(skin), C.c_double(dt_fs), C.c_int64(n_steps), _p(epot), _p(ekin), C.byref(nreb))
+    if rc != 0:
+        raise ValueError("oracle_nve: bad argument")
+    return NVEResult(x, v, epot, ekin, int(nreb.value))
