@@ -1,0 +1,192 @@
+/*
+ * gmnn.h -- C ABI of the B200-native GMNN energy-and-force path (arxiv 2505.22168, "apax").
+ *
+ * One shared library, libgmnn_b200.so (sm_100a only).  Plain pointers and sizes: no torch types,
+ * no exceptions across the boundary.  Every pointer is marked HOST or DEVICE.  PyTorch (or any
+ * other allocator) owns the caller-facing buffers and the stream; the library owns the model
+ * copy, the neighbour list and every workspace inside its two opaque handles.
+ *
+ * What the path computes (PAPER.md = /root/reference/PAPER.md, the text of the paper):
+ *   E(S) = sum_i E_i(G_i)                                              PAPER.md:46  (Eq. 1)
+ *   Psi_{i,L,s} = sum_{j != i} R_{Zi,Zj,s}(r_ij) rhat_ij^{(x)L}, L=0..3    PAPER.md:51  (Eq. 2)
+ *   G_i = full contractions of the Psi (360 invariants at n_radial=5)  PAPER.md:54-61 (Eq. 3)
+ *   E_i = sigma_{Zi} NN(G_i) + mu_{Zi}                                 PAPER.md:63-65 (Eq. 4)
+ *   F = -dE/dR (analytic backward, hand-derived)
+ *   shallow-ensemble mean / variance over last-layer heads             PAPER.md:75-88 (Eq. 5, 6)
+ *   NVE velocity Verlet with a Verlet-skin neighbour list
+ * Constants the paper leaves open (Gaussian centres and width, cosine cutoff, swish, block order
+ * of the invariants, ...) are the readings R1-R24 of DESIGN.md section 3; each is a field below.
+ *
+ * Units: Angstrom, eV, fs, amu.  a = F/m * 9.648533212e-3 Ang/fs^2.
+ * Cells: orthorhombic only (cell[9] row-major, rows = lattice vectors, off-diagonals must be 0).
+ *
+ * Return value of every int function: 0 (GMNN_OK) or a negative gmnn_status; the message of the
+ * last failure on the calling thread is gmnn_last_error().  Calls are asynchronous on the given
+ * stream unless stated otherwise.  There is no CPU fallback: without a CUDA device every compute
+ * call returns GMNN_CUDA_ERROR.
+ */
+#ifndef GMNN_B200_H
+#define GMNN_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct gmnn_model gmnn_model;   /* hyper-parameters + device copy of the weights        */
+typedef struct gmnn_system gmnn_system; /* N atoms, species, neighbour list, all workspaces      */
+
+typedef enum {
+    GMNN_OK = 0,
+    GMNN_INVALID_ARG = -1,       /* null pointer, N <= 0, r_cut != model's, non-finite input       */
+    GMNN_UNSUPPORTED = -2,       /* l_max != 3, triclinic cell, per-species weight sets, ...      */
+    GMNN_NEIGHBOR_OVERFLOW = -3, /* list capacity exceeded where it cannot be regrown (inside MD) */
+    GMNN_STALE_NEIGHBORS = -4,   /* an atom moved > skin/2 since the list was built               */
+    GMNN_CUDA_ERROR = -5,
+    GMNN_OOM = -6,
+    GMNN_OUT_OF_BOX = -7         /* a position handed to build_neighbors is outside [0, L)        */
+} gmnn_status;
+
+/* How the per-atom MLP (the one dense contraction of the path) is evaluated. */
+typedef enum {
+    GMNN_MLP_FP32 = 0,   /* fp32 FMA on the SIMT pipes; the fp32-tolerance path                      */
+    GMNN_MLP_3XTF32 = 1, /* tcgen05 TF32 tensor cores, 3-term error-compensated split (fp32 tol.)   */
+    GMNN_MLP_TF32 = 2    /* tcgen05 TF32 single pass; reduced-precision variant (2e-3 force tol.)   */
+} gmnn_mlp_precision;
+
+/* How F_i = sum_j g_ij - sum_j g_ji is formed.  Both are atomics-free and bit-reproducible. */
+typedef enum {
+    GMNN_FORCE_GATHER = 0, /* each centre recomputes g_ji from the neighbour's adjoint A_j           */
+    GMNN_FORCE_PAIRBUF = 1 /* g_ij written once per directed pair, reverse pair read through an index */
+} gmnn_force_mode;
+
+typedef struct {
+    int32_t n_species;     /* S, 1..8                                                              */
+    int32_t n_basis;       /* Gaussians per pair, 1..16 (configs: 7)                               */
+    int32_t n_radial;      /* radial channels s (configs: 5; kernels are instantiated for 5)       */
+    int32_t l_max;         /* must be 3                                                            */
+    float r_cut;           /* Ang                                                                  */
+    float r_min;           /* Ang; Gaussian centres r_min + k (r_cut - r_min)/(n_basis - 1)  (R1)  */
+    float gauss_gamma;     /* Ang^-2; <= 0 selects 1/(2 Delta^2), Delta = centre spacing     (R2)  */
+    int32_t n_hidden;      /* hidden layers, 1..4 (configs: 2)                                     */
+    int32_t hidden[4];     /* widths, multiples of 16, <= 1024 (configs: 512, 512)                 */
+    int32_t n_heads;       /* 1, or N_ens <= 64 for the shallow ensemble        */
+    int32_t n_weight_sets; /* 1 = one NN for all species (Eq. 4).  n_species: GMNN_UNSUPPORTED     */
+    int32_t mlp_precision; /* gmnn_mlp_precision                                                   */
+    int32_t force_mode;    /* gmnn_force_mode                                                      */
+} gmnn_hparams;
+
+typedef struct {            /* HOST pointers, row-major, caller-owned, copied by gmnn_create       */
+    const float *beta;      /* [S][S][n_radial][n_basis], centre species first               (R5)  */
+    const float *W[5];      /* layer l: [fan_in][fan_out]; fan_in(0) = n_features, last fan_out = n_heads */
+    const float *b[5];      /* layer l: [fan_out]                                                  */
+    const float *scale;     /* [S] sigma_Z                                                         */
+    const float *shift;     /* [S] mu_Z                                                            */
+} gmnn_weights;
+
+/* Number of invariants G_i for n_radial channels (360 at 5), blocks 0-7. */
+int32_t gmnn_n_features(int32_t n_radial);
+
+/* Validates the hyper-parameters, copies the weights to the current CUDA device (plus the
+ * transposed / split copies the kernels want).  Synchronous.  *out is written only on success. */
+int gmnn_create(const gmnn_hparams *hp, const gmnn_weights *w /*HOST*/, gmnn_model **out);
+void gmnn_destroy(gmnn_model *m);
+
+/* A system of n_atoms atoms with fixed species (HOST int32 [n_atoms], values 0..S-1).  Allocates
+ * the per-atom workspaces; the neighbour list is allocated by the first gmnn_build_neighbors.
+ * The model must outlive the system.  Synchronous. */
+int gmnn_system_create(const gmnn_model *m, int64_t n_atoms, const int32_t *species /*HOST*/, gmnn_system **out);
+void gmnn_system_destroy(gmnn_system *s);
+
+/* Tuning / diagnostics knobs (never needed for correctness):
+ *   "lanes_per_atom"  1,2,4,8,16,32: lanes that share one centre atom in the pair kernels (0 = auto)
+ *   "profile"         1: record CUDA events around every stage of energy_forces (gmnn_stage_times)
+ *   "capacity"        neighbour slots per atom for the next build (0 = estimate from the density)
+ *   "mlp_precision", "force_mode": override the model's value for this system
+ * Returns GMNN_INVALID_ARG for an unknown key or value. */
+int gmnn_system_set_int(gmnn_system *s, const char *key, int64_t value);
+int gmnn_system_get_int(const gmnn_system *s, const char *key, int64_t *value /*HOST*/);
+
+/* PAPER.md:169-171, 381 (neighbour list with skin `dr_threshold`, several images in small cells).
+ * Builds the full (both directions) Verlet list of all (i, j, n) with |x_j - x_i + n L| < r_cut +
+ * skin, n the integer image vector, by a cell list (>= 3 cells on every periodic axis) or an
+ * all-pairs image loop (smaller boxes, n_atoms <= 16384).  The membership predicate is evaluated
+ * in unfused fp32 exactly as DESIGN.md reading R20 writes it, so the set is reproducible bit for
+ * bit.  positions: DEVICE float [n_atoms][3], already wrapped into [0, L) on every axis (periodic
+ * or not); cell: HOST float[9]; pbc: HOST int32[3]; r_cut must equal the model's.  Synchronises
+ * the stream once (capacity check; regrows and retries on overflow). */
+int gmnn_build_neighbors(gmnn_system *s, const float *positions /*DEVICE*/, const float cell[9] /*HOST*/,
+                         const int32_t pbc[3] /*HOST*/, float r_cut, float skin, void *cuda_stream);
+
+/* Parity hook: the list as (i, j, n) triples in the caller's atom numbering, sorted by
+ * (i, j, nx, ny, nz).  Pass i = j = image = NULL to query *n_pairs.  HOST outputs
+ * (i, j: int32 [n_pairs]; image: int32 [n_pairs][3]).  Synchronous. */
+int gmnn_get_neighbors(gmnn_system *s, int64_t *n_pairs /*HOST*/, int32_t *i, int32_t *j, int32_t *image);
+
+/* Eq. 1-4 and the analytic forces on the existing list (pairs with r >= r_cut contribute exactly
+ * 0).  positions must be a continuous displacement of those the list was built from (atoms are
+ * NOT re-wrapped between builds: the list stores image vectors); an atom that moved more than
+ * skin/2 raises GMNN_STALE_NEIGHBORS at the next synchronising call (gmnn_check).
+ *   positions       DEVICE float [n_atoms][3]
+ *   energy          DEVICE double[1]            total E, accumulated in fp64 in a fixed order
+ *   energy_per_atom DEVICE float [n_atoms]      nullable
+ *   forces          DEVICE float [n_atoms][3]
+ * With n_heads > 1 this evaluates the mean energy over the heads and its gradient (PAPER.md:83-86,
+ * the cheap force mode of Eq. 6). */
+int gmnn_energy_forces(gmnn_system *s, const float *positions, double *energy, float *energy_per_atom,
+                       float *forces, void *cuda_stream);
+
+/* The same call with HOST buffers (pinned memory recommended): copies positions in and energy,
+ * energy_per_atom (nullable), forces out on the stream, then synchronises it.  This is the
+ * end-to-end entry bench.py's `e2e` times. */
+int gmnn_energy_forces_host(gmnn_system *s, const float *positions /*HOST*/, double *energy /*HOST*/,
+                            float *energy_per_atom /*HOST*/, float *forces /*HOST*/, void *cuda_stream);
+
+/* Eq. 5 (1/N_ens divisor) and Eq. 6, expensive mode: one forward, one backward per head.
+ *   e_mean, e_var  DEVICE float [n_atoms]       over the heads' atomic energies
+ *   f_mean, f_var  DEVICE float [n_atoms][3]    over the heads' forces, per atom and component
+ * Means first, then squared deviations (Welford update in head order), never E[x^2] - E[x]^2. */
+int gmnn_ensemble_energy_forces(gmnn_system *s, const float *positions, float *e_mean, float *e_var,
+                                float *f_mean, float *f_var, void *cuda_stream);
+
+/* n_steps of NVE velocity Verlet (BASELINE.json configs 2, 5; dt PAPER.md:367), whole loop on the
+ * device: kick, drift, skin test, list rebuild when any atom moved > skin/2 since the last build
+ * (positions are wrapped into [0, L) at each rebuild, and only then), energy+forces, kick.
+ *   positions, velocities  DEVICE float [n_atoms][3], in-out (Ang, Ang/fs)
+ *   masses                 DEVICE float [n_atoms] (amu)
+ *   epot_series, ekin_series  DEVICE double [n_steps + 1], nullable; index 0 = state at entry
+ *   n_rebuilds             HOST int32*, nullable
+ * Needs a list built by gmnn_build_neighbors (its cell, pbc and skin are reused).  Synchronises
+ * the stream at the end; returns GMNN_NEIGHBOR_OVERFLOW if an in-loop rebuild ran out of slots
+ * (results are then invalid; raise "capacity" and retry). */
+int gmnn_md_verlet_steps(gmnn_system *s, float *positions, float *velocities, const float *masses, float dt_fs,
+                         int32_t n_steps, double *epot_series, double *ekin_series, int32_t *n_rebuilds,
+                         void *cuda_stream);
+
+/* Synchronises the stream and reports a deferred device-side condition (GMNN_STALE_NEIGHBORS,
+ * GMNN_NEIGHBOR_OVERFLOW, GMNN_OUT_OF_BOX) or GMNN_OK, clearing it. */
+int gmnn_check(gmnn_system *s, void *cuda_stream);
+
+/* Stage timing of the last gmnn_energy_forces call made with "profile" = 1: CUDA events recorded
+ * on the call's own stream around each stage.  Synchronises on the last event.  Writes up to
+ * max_stages names/durations (ms); returns the number of stages (or a negative status). */
+int gmnn_stage_times(gmnn_system *s, int32_t max_stages, const char **names /*HOST*/, float *ms /*HOST*/);
+
+/* Parity hook for the stage tests: copies an internal per-atom array of the last call to HOST,
+ * rows in the library's internal (cell-sorted) atom order; "perm" gives internal row -> caller
+ * index.  Names: "perm" int32[N]; "psi" float[N][n_radial*20]; "G" float[N][F]; "dG" float[N][F]
+ * (without the sigma_Z factor); "A" float[N][n_radial*20]; "count" int32[N].  bytes must match.
+ * Synchronous. */
+int gmnn_debug_read(gmnn_system *s, const char *name, void *dst /*HOST*/, int64_t bytes);
+
+/* Number of kernel launches issued by this library since it was loaded (bench.py's gpu_launches). */
+int64_t gmnn_launch_count(void);
+
+/* Thread-local message for the last non-zero return. */
+const char *gmnn_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GMNN_B200_H */

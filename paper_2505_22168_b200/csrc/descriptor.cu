@@ -1,0 +1,568 @@
+// descriptor.cu -- the Gaussian-moment descriptor and its adjoint (SURVEY.md 8(a) rows a4-a6,
+// a9-a11; Eq. 2 and 3).
+//
+//   k_pair_forward      Psi[i][s][m] = sum_j R_s(r_ij) mono_m(u_ij)          (a4, a5)
+//   k_contract_forward  G[i][0..F)   = invariants of Psi[i]                   (a6)
+//   k_contract_backward A[i][s][m]   = dE/dPsi[i][s][m] from dE/dG[i]         (a9)
+//   k_pair_backward     F_i = sum_{j in N(i)} (g_ij - g_ji)                   (a10, a11)
+//
+// Pair kernels: LPA lanes share one centre atom and stride over its neighbour row with 16-byte
+// loads of packed entries; each neighbour costs one float4 gather of pos4 (L1/L2 resident: atoms
+// are cell sorted).  The species-pair table beta sits in shared memory.  Per-lane partial moment
+// sums (100 registers) are combined by xor shuffles inside the lane group.
+// Force reduction is the gather form: the full list is symmetric ((i,j,n) <-> (j,i,-n)), so each
+// centre evaluates both directions of every pair itself, g_ij with its own adjoint A_i and g_ji
+// with the neighbour's A_j (a 400-byte read served by L1/L2).  No atomics, fixed summation
+// order, bit-reproducible.
+//
+// Per-pair polynomial: E gets sum_s R_s(r) p_s(u) from pair (i,j), p_s(u) = sum_m A_i[s][m]
+// mono_m(u), so g_ij = dE/dd = (sum_s R'_s p_s) u + (grad_u q - (u.grad_u q) u) / r with
+// q(u) = sum_m (sum_s R_s A[s][m]) mono_m(u).
+#include <type_traits>
+
+#include "contraction.cuh"
+#include "gmnn_internal.h"
+
+namespace gmnn {
+
+constexpr float PI_F = 3.14159265358979323846f;
+
+// ---------------------------------------------------------------------------------------------
+// geometry of one packed neighbour entry
+// ---------------------------------------------------------------------------------------------
+struct PairGeom {
+    float dx, dy, dz, r2;
+    int j, zj;
+};
+
+__device__ __forceinline__ float image_diff(float xj, float xi, float shift) {
+    // keep the large cancellation exact: combine the lattice shift with whichever coordinate it cancels
+    return shift > 0.f ? xj + (shift - xi) : (xj + shift) - xi;
+}
+
+__device__ __forceinline__ PairGeom pair_geometry(uint32_t entry, const float4 &xi, const float4 *__restrict__ pos4,
+                                                  const float L0, const float L1, const float L2) {
+    PairGeom g;
+    g.j = (int)(entry & NBR_J_MASK);
+    const float4 xj = __ldg(&pos4[g.j]);
+    g.zj = __float_as_int(xj.w);
+    const float sx = (float)((int)((entry >> NBR_J_BITS) & 7u) - 4) * L0;
+    const float sy = (float)((int)((entry >> (NBR_J_BITS + 3)) & 7u) - 4) * L1;
+    const float sz = (float)((int)((entry >> (NBR_J_BITS + 6)) & 7u) - 4) * L2;
+    g.dx = image_diff(xj.x, xi.x, sx);
+    g.dy = image_diff(xj.y, xi.y, sy);
+    g.dz = image_diff(xj.z, xi.z, sz);
+    g.r2 = g.dx * g.dx + g.dy * g.dy + g.dz * g.dz;
+    return g;
+}
+
+// Phi_k(r) = exp(-gamma (r - mu_k)^2), f_c = 1/2 (1 + cos(pi r / r_cut))   (readings R1-R3)
+template <int NB, bool WITH_DERIV>
+__device__ __forceinline__ void radial_basis(const RadialParams &rp, float r, float *phi, float *dphi, float &fc,
+                                             float &dfc) {
+    const float t = r * rp.inv_rc;
+    if (WITH_DERIV) {
+        float sn, cs;
+        sincospif(t, &sn, &cs);
+        fc = 0.5f + 0.5f * cs;
+        dfc = -0.5f * PI_F * rp.inv_rc * sn;
+    } else {
+        fc = 0.5f + 0.5f * cospif(t);
+    }
+#pragma unroll
+    for (int k = 0; k < NB; ++k) {
+        const float d = r - (rp.r_min + (float)k * rp.delta);
+        const float p = __expf(-rp.gamma * d * d);
+        phi[k] = p;
+        if (WITH_DERIV) dphi[k] = -2.f * rp.gamma * d * p;
+    }
+}
+
+__device__ __forceinline__ void monomials(float x, float y, float z, float *m) {
+    m[0] = 1.f;
+    m[1] = x; m[2] = y; m[3] = z;
+    m[4] = x * x; m[5] = x * y; m[6] = x * z; m[7] = y * y; m[8] = y * z; m[9] = z * z;
+    m[10] = m[4] * x; m[11] = m[4] * y; m[12] = m[4] * z; m[13] = m[7] * x; m[14] = m[5] * z;
+    m[15] = m[9] * x; m[16] = m[7] * y; m[17] = m[7] * z; m[18] = m[9] * y; m[19] = m[9] * z;
+}
+
+// ---------------------------------------------------------------------------------------------
+// a4 + a5: pair radial functions and moment accumulation
+// ---------------------------------------------------------------------------------------------
+template <int NR, int NB, int LPA>
+__global__ void __launch_bounds__(128)
+k_pair_forward(int64_t N, const float4 *__restrict__ pos4, const uint32_t *__restrict__ nbr,
+               const int32_t *__restrict__ count, int cap, Geometry geo, RadialParams rp,
+               const float *__restrict__ beta, float *__restrict__ psi) {
+    constexpr int KB = (NB + 3) & ~3;
+    constexpr int ROW = NR * KB;  // floats per (zi, zj) block of the table
+    extern __shared__ float s_beta[];
+    for (int q = threadIdx.x; q < rp.n_species * rp.n_species * ROW; q += blockDim.x) s_beta[q] = beta[q];
+    __syncthreads();
+
+    const int64_t gt = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    const int64_t i = gt / LPA;
+    const int sub = (int)(gt % LPA);
+    const bool live = i < N;
+    float acc[NR][PSI];
+#pragma unroll
+    for (int s = 0; s < NR; ++s)
+#pragma unroll
+        for (int m = 0; m < PSI; ++m) acc[s][m] = 0.f;
+
+    if (live) {
+        const float4 xi = pos4[i];
+        const int zi = __float_as_int(xi.w);
+        const int cnt = count[i];
+        const uint4 *row = reinterpret_cast<const uint4 *>(nbr + i * (int64_t)cap);
+        for (int k4 = sub; k4 * 4 < cnt; k4 += LPA) {
+            const uint4 e4 = __ldg(&row[k4]);
+            const uint32_t ent[4] = {e4.x, e4.y, e4.z, e4.w};
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                if (k4 * 4 + q >= cnt) break;
+                const PairGeom pg = pair_geometry(ent[q], xi, pos4, geo.L[0], geo.L[1], geo.L[2]);
+                if (pg.r2 < rp.r_cut2) {
+                    const float rinv = rsqrtf(pg.r2);
+                    const float r = pg.r2 * rinv;
+                    float phi[NB], fc, dummy;
+                    radial_basis<NB, false>(rp, r, phi, nullptr, fc, dummy);
+                    const float4 *bt = reinterpret_cast<const float4 *>(s_beta + (zi * rp.n_species + pg.zj) * ROW);
+                    float R[NR];
+#pragma unroll
+                    for (int s = 0; s < NR; ++s) {
+                        float sum = 0.f;
+#pragma unroll
+                        for (int kq = 0; kq < KB / 4; ++kq) {
+                            const float4 b = bt[s * (KB / 4) + kq];
+                            if (4 * kq + 0 < NB) sum = fmaf(b.x, phi[4 * kq + 0], sum);
+                            if (4 * kq + 1 < NB) sum = fmaf(b.y, phi[4 * kq + 1], sum);
+                            if (4 * kq + 2 < NB) sum = fmaf(b.z, phi[4 * kq + 2], sum);
+                            if (4 * kq + 3 < NB) sum = fmaf(b.w, phi[4 * kq + 3], sum);
+                        }
+                        R[s] = fc * sum;
+                    }
+                    float mono[PSI];
+                    monomials(pg.dx * rinv, pg.dy * rinv, pg.dz * rinv, mono);
+#pragma unroll
+                    for (int s = 0; s < NR; ++s)
+#pragma unroll
+                        for (int m = 0; m < PSI; ++m) acc[s][m] = fmaf(R[s], mono[m], acc[s][m]);
+                }
+            }
+        }
+    }
+    // combine the LPA partial sums (all lanes of the warp take part)
+#pragma unroll
+    for (int o = LPA / 2; o >= 1; o >>= 1)
+#pragma unroll
+        for (int s = 0; s < NR; ++s)
+#pragma unroll
+            for (int m = 0; m < PSI; ++m) acc[s][m] += __shfl_xor_sync(0xffffffffu, acc[s][m], o);
+    if (live) {
+        float4 *out = reinterpret_cast<float4 *>(psi + i * (int64_t)(NR * PSI));
+#pragma unroll
+        for (int q = 0; q < NR * PSI / 4; ++q) {
+            if (q % LPA == sub) {
+                const int s = (4 * q) / PSI, m = (4 * q) % PSI;
+                out[q] = make_float4(acc[s][m], acc[s][m + 1], acc[s][m + 2], acc[s][m + 3]);
+            }
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// a6: invariants.  One thread per atom, Psi row in registers, straight-line FMA code from
+// contraction.cuh.  Features leave through a per-warp shared tile (feature-major, padded to 33)
+// so that global stores are contiguous runs of one atom's row.
+// ---------------------------------------------------------------------------------------------
+template <int NR>
+struct FeatChunks {
+    using F = Feat<NR>;
+    // chunk boundaries in feature space: [0, OFF4) [OFF4, OFF5) [OFF5, OFF6) [OFF6, OFF7) [OFF7, N)
+    static constexpr int NCH = 5;
+    __host__ __device__ static constexpr int begin(int c) {
+        return c == 0 ? 0 : c == 1 ? F::OFF4 : c == 2 ? F::OFF5 : c == 3 ? F::OFF6 : c == 4 ? F::OFF7 : F::N;
+    }
+    __host__ __device__ static constexpr int chunk_of(int f) {
+        return f < F::OFF4 ? 0 : f < F::OFF5 ? 1 : f < F::OFF6 ? 2 : f < F::OFF7 ? 3 : 4;
+    }
+    __host__ __device__ static constexpr int mask(int c) { return c == 0 ? 0x0F : (0x08 << c); }
+    __host__ __device__ static constexpr int max_len() {
+        int m = 0;
+        for (int c = 0; c < NCH; ++c) m = (begin(c + 1) - begin(c)) > m ? (begin(c + 1) - begin(c)) : m;
+        return m;
+    }
+};
+
+constexpr int CW = 33;  // padded warp tile pitch
+
+template <int NR>
+__global__ void __launch_bounds__(128)
+k_contract_forward(int64_t N, const float *__restrict__ psi, float *__restrict__ G) {
+    using F = Feat<NR>;
+    using CH = FeatChunks<NR>;
+    extern __shared__ float s_tile[];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    float *tile = s_tile + wid * (CH::max_len() * CW);
+    const int64_t i0 = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) - lane;  // first atom of the warp
+    const int64_t i = i0 + lane;
+    float P[NR][PSI];
+    if (i < N) {
+        const float4 *src = reinterpret_cast<const float4 *>(psi + i * (int64_t)(NR * PSI));
+#pragma unroll
+        for (int q = 0; q < NR * PSI / 4; ++q) {
+            const float4 v = __ldg(&src[q]);
+            P[(4 * q) / PSI][(4 * q) % PSI] = v.x;
+            P[(4 * q + 1) / PSI][(4 * q + 1) % PSI] = v.y;
+            P[(4 * q + 2) / PSI][(4 * q + 2) % PSI] = v.z;
+            P[(4 * q + 3) / PSI][(4 * q + 3) % PSI] = v.w;
+        }
+    } else {
+#pragma unroll
+        for (int s = 0; s < NR; ++s)
+#pragma unroll
+            for (int m = 0; m < PSI; ++m) P[s][m] = 0.f;
+    }
+    // One pass per chunk of feature blocks (blocks 0-3 | 4 | 5 | 6 | 7), selected at compile time.
+    auto run_chunk = [&](auto chunk_tag) {
+        constexpr int C = decltype(chunk_tag)::value;
+        contract_forward<NR, CH::mask(C)>([&](int s, int m) { return P[s][m]; },
+                                          [&](int f, float v) { tile[(f - CH::begin(C)) * CW + lane] = v; });
+        __syncwarp();
+        constexpr int len = CH::begin(C + 1) - CH::begin(C);
+        for (int a = 0; a < 32; ++a) {
+            const int64_t ia = i0 + a;
+            if (ia >= N) break;
+            float *dst = G + ia * (int64_t)F::N + CH::begin(C);
+            for (int f = lane; f < len; f += 32) dst[f] = tile[f * CW + a];
+        }
+        __syncwarp();
+    };
+    run_chunk(std::integral_constant<int, 0>{});
+    run_chunk(std::integral_constant<int, 1>{});
+    run_chunk(std::integral_constant<int, 2>{});
+    run_chunk(std::integral_constant<int, 3>{});
+    run_chunk(std::integral_constant<int, 4>{});
+}
+
+// ---------------------------------------------------------------------------------------------
+// a9: adjoint of the invariants.  One thread per atom; Psi row and the current chunk of dE/dG in
+// per-warp shared tiles (component-major, pitch 33: conflict-free), the 100 adjoints in registers.
+// dE/dG arrives without the sigma_Z factor of Eq. 4 (the MLP backward is linear in it); it is
+// applied here.
+// ---------------------------------------------------------------------------------------------
+template <int NR>
+__global__ void __launch_bounds__(64)
+k_contract_backward(int64_t N, const float *__restrict__ psi, const float *__restrict__ dG,
+                    const float4 *__restrict__ pos4, const float *__restrict__ scale, float *__restrict__ A) {
+    using F = Feat<NR>;
+    using CH = FeatChunks<NR>;
+    extern __shared__ float s_tile[];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    float *sP = s_tile + wid * ((NR * PSI + CH::max_len()) * CW);
+    float *sG = sP + NR * PSI * CW;
+    const int64_t i0 = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) - lane;
+    const int64_t i = i0 + lane;
+    for (int a = 0; a < 32; ++a) {
+        const int64_t ia = i0 + a;
+        if (ia >= N) break;
+        const float *src = psi + ia * (int64_t)(NR * PSI);
+        for (int q = lane; q < NR * PSI; q += 32) sP[q * CW + a] = __ldg(&src[q]);
+    }
+    float sig = 0.f;
+    if (i < N) sig = __ldg(&scale[__float_as_int(pos4[i].w)]);
+    float acc[NR][PSI];
+#pragma unroll
+    for (int s = 0; s < NR; ++s)
+#pragma unroll
+        for (int m = 0; m < PSI; ++m) acc[s][m] = 0.f;
+    __syncwarp();
+
+    auto run_chunk = [&](auto chunk_tag) {
+        constexpr int C = decltype(chunk_tag)::value;
+        constexpr int len = CH::begin(C + 1) - CH::begin(C);
+        for (int a = 0; a < 32; ++a) {
+            const int64_t ia = i0 + a;
+            if (ia >= N) break;
+            const float *src = dG + ia * (int64_t)F::N + CH::begin(C);
+            for (int f = lane; f < len; f += 32) sG[f * CW + a] = __ldg(&src[f]);
+        }
+        __syncwarp();
+        contract_backward<NR, CH::mask(C)>(
+            [&](int s, int m) { return sP[(s * PSI + m) * CW + lane]; },
+            [&](int f) { return sG[(f - CH::begin(C)) * CW + lane]; },
+            [&](int s, int m, float v) { acc[s][m] += v; });
+        __syncwarp();
+    };
+    run_chunk(std::integral_constant<int, 0>{});
+    run_chunk(std::integral_constant<int, 1>{});
+    run_chunk(std::integral_constant<int, 2>{});
+    run_chunk(std::integral_constant<int, 3>{});
+    run_chunk(std::integral_constant<int, 4>{});
+
+    // transpose the adjoints back through the (now free) Psi tile for contiguous stores
+#pragma unroll
+    for (int s = 0; s < NR; ++s)
+#pragma unroll
+        for (int m = 0; m < PSI; ++m) sP[(s * PSI + m) * CW + lane] = sig * acc[s][m];
+    __syncwarp();
+    for (int a = 0; a < 32; ++a) {
+        const int64_t ia = i0 + a;
+        if (ia >= N) break;
+        float *dst = A + ia * (int64_t)(NR * PSI);
+        for (int q = lane; q < NR * PSI; q += 32) dst[q] = sP[q * CW + a];
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// a10 + a11: pair gradient in both directions and the force sum of the centre atom
+// ---------------------------------------------------------------------------------------------
+// g = dE/dd for one direction.  a(s, q) returns the float4 {A[s][4q..4q+3]}; sgn = +1 evaluates at
+// u, sgn = -1 at -u (odd-rank monomials change sign).
+template <int NR, class AGet>
+__device__ __forceinline__ void pair_gradient(AGet a, const float *R, const float *dR, const float *mono, float ux,
+                                              float uy, float uz, float rinv, float sgn, float &gx, float &gy,
+                                              float &gz) {
+    float t[PSI];
+#pragma unroll
+    for (int m = 0; m < PSI; ++m) t[m] = 0.f;
+    float radial = 0.f;
+#pragma unroll
+    for (int s = 0; s < NR; ++s) {
+        float pe = 0.f, po = 0.f;  // even (L = 0, 2) and odd (L = 1, 3) parts of p_s(u)
+#pragma unroll
+        for (int q = 0; q < PSI / 4; ++q) {
+            const float4 v = a(s, q);
+            const float av[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                const int m = 4 * q + c;
+                const bool odd = (m >= 1 && m <= 3) || m >= 10;
+                if (odd) po = fmaf(av[c], mono[m], po);
+                else pe = fmaf(av[c], mono[m], pe);
+                t[m] = fmaf(R[s], av[c], t[m]);
+            }
+        }
+        radial = fmaf(dR[s], pe + sgn * po, radial);
+    }
+    const float x = sgn * ux, y = sgn * uy, z = sgn * uz;
+    const float xx = mono[4], xy = mono[5], xz = mono[6], yy = mono[7], yz = mono[8], zz = mono[9];  // even: sign free
+    // grad_u q(u), q = sum_m t_m mono_m
+    float wx = t[1] + 2.f * t[4] * x + t[5] * y + t[6] * z + 3.f * t[10] * xx + 2.f * t[11] * xy + 2.f * t[12] * xz +
+               t[13] * yy + t[14] * yz + t[15] * zz;
+    float wy = t[2] + t[5] * x + 2.f * t[7] * y + t[8] * z + t[11] * xx + 2.f * t[13] * xy + t[14] * xz +
+               3.f * t[16] * yy + 2.f * t[17] * yz + t[18] * zz;
+    float wz = t[3] + t[6] * x + t[8] * y + 2.f * t[9] * z + t[12] * xx + t[14] * xy + 2.f * t[15] * xz + t[17] * yy +
+               2.f * t[18] * yz + 3.f * t[19] * zz;
+    const float wu = wx * x + wy * y + wz * z;
+    gx = radial * x + (wx - wu * x) * rinv;
+    gy = radial * y + (wy - wu * y) * rinv;
+    gz = radial * z + (wz - wu * z) * rinv;
+}
+
+template <int NR, int NB, int LPA>
+__global__ void __launch_bounds__(128)
+k_pair_backward(int64_t N, const float4 *__restrict__ pos4, const uint32_t *__restrict__ nbr,
+                const int32_t *__restrict__ count, int cap, Geometry geo, RadialParams rp,
+                const float *__restrict__ beta, const float *__restrict__ A, float *__restrict__ f_int) {
+    constexpr int KB = (NB + 3) & ~3;
+    constexpr int ROW = NR * KB;
+    constexpr int GROUPS = 128 / LPA;
+    extern __shared__ float s_mem[];
+    float *s_beta = s_mem;
+    float4 *s_A = reinterpret_cast<float4 *>(s_mem + ((rp.n_species * rp.n_species * ROW + 3) & ~3));
+    for (int q = threadIdx.x; q < rp.n_species * rp.n_species * ROW; q += blockDim.x) s_beta[q] = beta[q];
+    const int64_t gt = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    const int64_t i = gt / LPA;
+    const int sub = (int)(gt % LPA);
+    const int grp = threadIdx.x / LPA;
+    const bool live = i < N;
+    // stage A_i of the block's centres: GROUPS rows of NR*PSI/4 float4
+    {
+        const int64_t first = blockIdx.x * (int64_t)GROUPS;
+        const float4 *src = reinterpret_cast<const float4 *>(A);
+        for (int q = threadIdx.x; q < GROUPS * (NR * PSI / 4); q += blockDim.x) {
+            const int64_t ia = first + q / (NR * PSI / 4);
+            s_A[q] = ia < N ? __ldg(&src[ia * (NR * PSI / 4) + q % (NR * PSI / 4)]) : make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+    }
+    __syncthreads();
+    float fx = 0.f, fy = 0.f, fz = 0.f;
+    if (live) {
+        const float4 xi = pos4[i];
+        const int zi = __float_as_int(xi.w);
+        const int cnt = count[i];
+        const uint4 *row = reinterpret_cast<const uint4 *>(nbr + i * (int64_t)cap);
+        const float4 *Ai = s_A + grp * (NR * PSI / 4);
+        for (int k4 = sub; k4 * 4 < cnt; k4 += LPA) {
+            const uint4 e4 = __ldg(&row[k4]);
+            const uint32_t ent[4] = {e4.x, e4.y, e4.z, e4.w};
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                if (k4 * 4 + q >= cnt) break;
+                const PairGeom pg = pair_geometry(ent[q], xi, pos4, geo.L[0], geo.L[1], geo.L[2]);
+                if (pg.r2 < rp.r_cut2) {
+                    const float rinv = rsqrtf(pg.r2);
+                    const float r = pg.r2 * rinv;
+                    float phi[NB], dphi[NB], fc, dfc;
+                    radial_basis<NB, true>(rp, r, phi, dphi, fc, dfc);
+                    const float ux = pg.dx * rinv, uy = pg.dy * rinv, uz = pg.dz * rinv;
+                    float mono[PSI];
+                    monomials(ux, uy, uz, mono);
+                    float gxo, gyo, gzo, gxr, gyr, gzr;
+#pragma unroll
+                    for (int dir = 0; dir < 2; ++dir) {
+                        // dir 0: centre i, table beta[zi][zj], adjoint A_i, direction +u
+                        // dir 1: centre j, table beta[zj][zi], adjoint A_j, direction -u
+                        const int za = dir == 0 ? zi : pg.zj, zb = dir == 0 ? pg.zj : zi;
+                        const float4 *bt = reinterpret_cast<const float4 *>(s_beta + (za * rp.n_species + zb) * ROW);
+                        float R[NR], dR[NR];
+#pragma unroll
+                        for (int s = 0; s < NR; ++s) {
+                            float sum = 0.f, dsum = 0.f;
+#pragma unroll
+                            for (int kq = 0; kq < KB / 4; ++kq) {
+                                const float4 b = bt[s * (KB / 4) + kq];
+                                const float bv[4] = {b.x, b.y, b.z, b.w};
+#pragma unroll
+                                for (int c = 0; c < 4; ++c)
+                                    if (4 * kq + c < NB) {
+                                        sum = fmaf(bv[c], phi[4 * kq + c], sum);
+                                        dsum = fmaf(bv[c], dphi[4 * kq + c], dsum);
+                                    }
+                            }
+                            R[s] = fc * sum;
+                            dR[s] = dfc * sum + fc * dsum;
+                        }
+                        if (dir == 0) {
+                            pair_gradient<NR>([&](int s, int qq) { return Ai[s * (PSI / 4) + qq]; }, R, dR, mono, ux, uy,
+                                              uz, rinv, 1.f, gxo, gyo, gzo);
+                        } else {
+                            const float4 *Aj = reinterpret_cast<const float4 *>(A) + (int64_t)pg.j * (NR * PSI / 4);
+                            pair_gradient<NR>([&](int s, int qq) { return __ldg(&Aj[s * (PSI / 4) + qq]); }, R, dR, mono,
+                                              ux, uy, uz, rinv, -1.f, gxr, gyr, gzr);
+                        }
+                    }
+                    // F_i += g_ij - g_ji   (g_ji = dE_j/dd_ji, d_ji = -d_ij)
+                    fx += gxo - gxr;
+                    fy += gyo - gyr;
+                    fz += gzo - gzr;
+                }
+            }
+        }
+    }
+#pragma unroll
+    for (int o = LPA / 2; o >= 1; o >>= 1) {
+        fx += __shfl_xor_sync(0xffffffffu, fx, o);
+        fy += __shfl_xor_sync(0xffffffffu, fy, o);
+        fz += __shfl_xor_sync(0xffffffffu, fz, o);
+    }
+    if (live && sub == 0) {
+        f_int[3 * i] = fx;
+        f_int[3 * i + 1] = fy;
+        f_int[3 * i + 2] = fz;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// launchers
+// ---------------------------------------------------------------------------------------------
+static inline unsigned nblocks(int64_t n, int per) { return (unsigned)((n + per - 1) / per); }
+
+static int pick_lpa(const gmnn_system *s) {
+    if (s->lanes_per_atom > 0) return s->lanes_per_atom;
+    // enough warps to fill 148 SMs several times over: small systems spread one atom over more lanes
+    if (s->N >= 65536) return 4;
+    if (s->N >= 8192) return 8;
+    return 32;
+}
+
+template <int NR, int NB>
+static int pair_forward_lpa(gmnn_system *s, cudaStream_t st, int lpa) {
+    const gmnn_model *m = s->model;
+    const size_t smem = sizeof(float) * m->rp.n_species * m->rp.n_species * NR * m->rp.kb;
+    const unsigned grid = nblocks(s->N * lpa, 128);
+#define GMNN_PF(L)                                                                                        \
+    case L:                                                                                               \
+        k_pair_forward<NR, NB, L><<<grid, 128, smem, st>>>(s->N, s->pos4, s->nbr, s->count, s->cap, s->geo, \
+                                                           m->rp, m->beta, s->psi);                       \
+        break;
+    switch (lpa) {
+        GMNN_PF(1) GMNN_PF(2) GMNN_PF(4) GMNN_PF(8) GMNN_PF(16) GMNN_PF(32)
+        default:
+            set_error("lanes_per_atom must be 1, 2, 4, 8, 16 or 32");
+            return GMNN_INVALID_ARG;
+    }
+#undef GMNN_PF
+    GMNN_LAUNCHED();
+    GMNN_CUDA(cudaGetLastError());
+    return GMNN_OK;
+}
+
+template <int NR, int NB>
+static int pair_backward_lpa(gmnn_system *s, cudaStream_t st, int lpa) {
+    const gmnn_model *m = s->model;
+    const int beta_floats = (m->rp.n_species * m->rp.n_species * NR * m->rp.kb + 3) & ~3;
+    const size_t smem = sizeof(float) * (beta_floats + (128 / lpa) * NR * PSI);
+    const unsigned grid = nblocks(s->N * lpa, 128);
+#define GMNN_PB(L)                                                                                         \
+    case L:                                                                                                \
+        k_pair_backward<NR, NB, L><<<grid, 128, smem, st>>>(s->N, s->pos4, s->nbr, s->count, s->cap, s->geo, \
+                                                            m->rp, m->beta, s->A, s->f_int);               \
+        break;
+    switch (lpa) {
+        GMNN_PB(1) GMNN_PB(2) GMNN_PB(4) GMNN_PB(8) GMNN_PB(16) GMNN_PB(32)
+        default:
+            set_error("lanes_per_atom must be 1, 2, 4, 8, 16 or 32");
+            return GMNN_INVALID_ARG;
+    }
+#undef GMNN_PB
+    GMNN_LAUNCHED();
+    GMNN_CUDA(cudaGetLastError());
+    return GMNN_OK;
+}
+
+int launch_pair_forward(gmnn_system *s, cudaStream_t st) {
+    const gmnn_model *m = s->model;
+    if (m->hp.n_radial == 5 && m->hp.n_basis == 7) return pair_forward_lpa<5, 7>(s, st, pick_lpa(s));
+    set_error("pair kernels are instantiated for n_radial = 5, n_basis = 7 only");
+    return GMNN_UNSUPPORTED;
+}
+
+int launch_pair_backward(gmnn_system *s, cudaStream_t st) {
+    const gmnn_model *m = s->model;
+    if (m->hp.n_radial == 5 && m->hp.n_basis == 7) return pair_backward_lpa<5, 7>(s, st, pick_lpa(s));
+    set_error("pair kernels are instantiated for n_radial = 5, n_basis = 7 only");
+    return GMNN_UNSUPPORTED;
+}
+
+int launch_contract_forward(gmnn_system *s, cudaStream_t st) {
+    constexpr int NR = 5;
+    const size_t smem = sizeof(float) * 4 * FeatChunks<NR>::max_len() * CW;
+    static bool attr_set = false;
+    if (!attr_set) {
+        GMNN_CUDA(cudaFuncSetAttribute(k_contract_forward<NR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_set = true;
+    }
+    k_contract_forward<NR><<<nblocks(s->N, 128), 128, smem, st>>>(s->N, s->psi, s->G);
+    GMNN_LAUNCHED();
+    GMNN_CUDA(cudaGetLastError());
+    return GMNN_OK;
+}
+
+int launch_contract_backward(gmnn_system *s, cudaStream_t st) {
+    constexpr int NR = 5;
+    const size_t smem = sizeof(float) * 2 * (NR * PSI + FeatChunks<NR>::max_len()) * CW;
+    static bool attr_set = false;
+    if (!attr_set) {
+        GMNN_CUDA(cudaFuncSetAttribute(k_contract_backward<NR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_set = true;
+    }
+    k_contract_backward<NR><<<nblocks(s->N, 64), 64, smem, st>>>(s->N, s->psi, s->dG, s->pos4, s->model->scale, s->A);
+    GMNN_LAUNCHED();
+    GMNN_CUDA(cudaGetLastError());
+    return GMNN_OK;
+}
+
+}  // namespace gmnn

@@ -1,0 +1,719 @@
+// gmnn_api.cu -- the C ABI of include/gmnn.h: handles, validation, buffer ownership and the
+// order in which the kernels of neighbor.cu / descriptor.cu / mlp_*.cu / md.cu run.
+// Every step of the path runs in those kernels; this file only allocates, launches and reports.
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstring>
+#include <numeric>
+
+#include "contraction.cuh"
+#include "gmnn_internal.h"
+
+namespace gmnn {
+
+static thread_local char g_error[512] = "";
+long long g_launch_count = 0;
+
+void set_error(const char *fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_error, sizeof(g_error), fmt, ap);
+    va_end(ap);
+}
+
+int launch_mlp_forward_tc(gmnn_system *s, cudaStream_t st);
+int launch_mlp_backward_tc(gmnn_system *s, const float *head_w_dev, cudaStream_t st);
+
+template <class T>
+static int dev_alloc(T **p, size_t n) {
+    *p = nullptr;
+    GMNN_CUDA(cudaMalloc((void **)p, sizeof(T) * (n > 0 ? n : 1)));
+    return GMNN_OK;
+}
+template <class T>
+static void dev_free(T *&p) {
+    if (p) cudaFree((void *)p);
+    p = nullptr;
+}
+template <class T>
+static int upload(T **p, const T *host, size_t n) {
+    int rc = dev_alloc(p, n);
+    if (rc) return rc;
+    GMNN_CUDA(cudaMemcpy(*p, host, sizeof(T) * n, cudaMemcpyHostToDevice));
+    return GMNN_OK;
+}
+
+__global__ void k_set_onehot(int M, int m, float *w) {
+    const int t = threadIdx.x;
+    if (t < M) w[t] = (t == m) ? 1.f : 0.f;
+}
+
+struct StageTimer {
+    gmnn_system *s;
+    cudaStream_t st;
+    StageTimer(gmnn_system *s_, cudaStream_t st_) : s(s_), st(st_) {}
+    void begin() {
+        if (!s->profile) return;
+        s->n_stage_events = 0;
+        s->stage_names.clear();
+        mark(nullptr);
+    }
+    void mark(const char *name) {
+        if (!s->profile) return;
+        if ((int)s->events.size() <= s->n_stage_events) {
+            cudaEvent_t e;
+            cudaEventCreate(&e);
+            s->events.push_back(e);
+        }
+        cudaEventRecord(s->events[s->n_stage_events++], st);
+        if (name) s->stage_names.push_back(name);
+    }
+};
+
+static int mlp_forward(gmnn_system *s, cudaStream_t st) {
+    if (s->mlp_precision == GMNN_MLP_FP32) return launch_mlp_forward_simt(s, st);
+    return launch_mlp_forward_tc(s, st);
+}
+static int mlp_backward(gmnn_system *s, const float *head_w, cudaStream_t st) {
+    if (s->mlp_precision == GMNN_MLP_FP32) return launch_mlp_backward_simt(s, head_w, st);
+    return launch_mlp_backward_tc(s, head_w, st);
+}
+
+// positions -> E_i, F (internal order), for the energy whose head weights are head_w (device)
+static int forward_backward(gmnn_system *s, const float *positions, const float *head_w, bool check_stale,
+                            cudaStream_t st, StageTimer &T) {
+    int rc;
+    if ((rc = launch_gather_positions(s, positions, st, check_stale))) return rc;
+    T.mark("gather");
+    if ((rc = launch_pair_forward(s, st))) return rc;
+    T.mark("pair_forward");
+    if ((rc = launch_contract_forward(s, st))) return rc;
+    T.mark("contract_forward");
+    if ((rc = mlp_forward(s, st))) return rc;
+    T.mark("mlp_forward");
+    if ((rc = launch_mlp_heads(s, head_w, st))) return rc;
+    T.mark("mlp_heads");
+    if ((rc = mlp_backward(s, head_w, st))) return rc;
+    T.mark("mlp_backward");
+    if ((rc = launch_contract_backward(s, st))) return rc;
+    T.mark("contract_backward");
+    if ((rc = launch_pair_backward(s, st))) return rc;
+    T.mark("pair_backward");
+    return GMNN_OK;
+}
+
+}  // namespace gmnn
+
+using namespace gmnn;
+
+extern "C" {
+
+const char *gmnn_last_error(void) { return g_error; }
+int64_t gmnn_launch_count(void) { return (int64_t)g_launch_count; }
+
+int32_t gmnn_n_features(int32_t n) {
+    const int p = n * (n + 1) / 2, t = n * (n + 1) * (n + 2) / 6;
+    return n + 3 * p + t + 2 * p * n + n * n * n;
+}
+
+int gmnn_create(const gmnn_hparams *hp, const gmnn_weights *w, gmnn_model **out) {
+    if (!hp || !w || !out) {
+        set_error("gmnn_create: null argument");
+        return GMNN_INVALID_ARG;
+    }
+    if (hp->l_max != 3) {
+        set_error("l_max must be 3 (got %d)", hp->l_max);
+        return GMNN_UNSUPPORTED;
+    }
+    if (hp->n_species < 1 || hp->n_species > MAX_SPECIES || hp->n_basis < 2 || hp->n_basis > MAX_BASIS ||
+        hp->n_radial < 1 || hp->n_hidden < 1 || hp->n_hidden > 4 || hp->n_heads < 1 || hp->n_heads > 64 ||
+        !(hp->r_cut > 0.f) || !(hp->r_min >= 0.f) || !(hp->r_min < hp->r_cut) || !std::isfinite(hp->r_cut)) {
+        set_error("gmnn_create: hyper-parameter out of range");
+        return GMNN_INVALID_ARG;
+    }
+    if (hp->n_radial != 5 || hp->n_basis != 7) {
+        set_error("kernels are instantiated for n_radial = 5, n_basis = 7 (got %d, %d)", hp->n_radial, hp->n_basis);
+        return GMNN_UNSUPPORTED;
+    }
+    if (hp->n_weight_sets != 1) {
+        set_error("n_weight_sets = %d: per-species weight sets are not built yet (DESIGN.md R11)", hp->n_weight_sets);
+        return GMNN_UNSUPPORTED;
+    }
+    if (hp->mlp_precision < 0 || hp->mlp_precision > GMNN_MLP_TF32 || hp->force_mode < 0 ||
+        hp->force_mode > GMNN_FORCE_PAIRBUF) {
+        set_error("gmnn_create: bad mlp_precision / force_mode");
+        return GMNN_INVALID_ARG;
+    }
+    for (int l = 0; l < hp->n_hidden; ++l)
+        if (hp->hidden[l] < 16 || hp->hidden[l] > 1024 || hp->hidden[l] % 16 != 0) {
+            set_error("hidden[%d] = %d must be a multiple of 16 in [16, 1024]", l, hp->hidden[l]);
+            return GMNN_INVALID_ARG;
+        }
+    if (!w->beta || !w->scale || !w->shift) {
+        set_error("gmnn_create: null weight pointer");
+        return GMNN_INVALID_ARG;
+    }
+    for (int l = 0; l <= hp->n_hidden; ++l)
+        if (!w->W[l] || !w->b[l]) {
+            set_error("gmnn_create: null weight pointer (layer %d)", l);
+            return GMNN_INVALID_ARG;
+        }
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        set_error("no CUDA device: this library has no CPU fallback");
+        return GMNN_CUDA_ERROR;
+    }
+    gmnn_model *m = new gmnn_model();
+    m->hp = *hp;
+    m->n_features = gmnn_n_features(hp->n_radial);
+    m->n_layers = hp->n_hidden + 1;
+    m->dims[0] = m->n_features;
+    for (int l = 0; l < hp->n_hidden; ++l) m->dims[l + 1] = hp->hidden[l];
+    m->dims[hp->n_hidden + 1] = hp->n_heads;
+    RadialParams &rp = m->rp;
+    rp.n_species = hp->n_species;
+    rp.n_basis = hp->n_basis;
+    rp.kb = (hp->n_basis + 3) & ~3;
+    rp.r_cut = hp->r_cut;
+    rp.r_cut2 = hp->r_cut * hp->r_cut;
+    rp.inv_rc = 1.f / hp->r_cut;
+    rp.r_min = hp->r_min;
+    rp.delta = (hp->r_cut - hp->r_min) / (float)(hp->n_basis - 1);
+    rp.gamma = hp->gauss_gamma > 0.f ? hp->gauss_gamma : 1.f / (2.f * rp.delta * rp.delta);
+    int rc = GMNN_OK;
+    {
+        const int S = hp->n_species, nr = hp->n_radial, nb = hp->n_basis;
+        std::vector<float> padded((size_t)S * S * nr * rp.kb, 0.f);
+        for (int p = 0; p < S * S; ++p)
+            for (int s = 0; s < nr; ++s)
+                for (int k = 0; k < nb; ++k) padded[((size_t)p * nr + s) * rp.kb + k] = w->beta[((size_t)p * nr + s) * nb + k];
+        rc = upload(&m->beta, padded.data(), padded.size());
+    }
+    for (int l = 0; l < m->n_layers && !rc; ++l) {
+        const int fi = m->dims[l], fo = m->dims[l + 1];
+        rc = upload(&m->W[l], w->W[l], (size_t)fi * fo);
+        if (!rc) rc = upload(&m->b[l], w->b[l], (size_t)fo);
+        std::vector<float> t((size_t)fi * fo);
+        for (int a = 0; a < fi; ++a)
+            for (int b = 0; b < fo; ++b) t[(size_t)b * fi + a] = w->W[l][(size_t)a * fo + b];
+        if (!rc) rc = upload(&m->WT[l], t.data(), t.size());
+    }
+    if (!rc) rc = upload(&m->scale, w->scale, (size_t)hp->n_species);
+    if (!rc) rc = upload(&m->shift, w->shift, (size_t)hp->n_species);
+    if (!rc) {
+        std::vector<float> hw(hp->n_heads, 1.f / (float)hp->n_heads);
+        rc = upload(&m->head_mean_w, hw.data(), hw.size());
+    }
+    if (rc) {
+        gmnn_destroy(m);
+        return rc;
+    }
+    *out = m;
+    return GMNN_OK;
+}
+
+void gmnn_destroy(gmnn_model *m) {
+    if (!m) return;
+    dev_free(m->beta);
+    for (int l = 0; l < MAX_LAYERS; ++l) {
+        dev_free(m->W[l]);
+        dev_free(m->WT[l]);
+        dev_free(m->b[l]);
+    }
+    dev_free(m->scale);
+    dev_free(m->shift);
+    dev_free(m->head_mean_w);
+    delete m;
+}
+
+int gmnn_system_create(const gmnn_model *m, int64_t n_atoms, const int32_t *species, gmnn_system **out) {
+    if (!m || !species || !out || n_atoms <= 0) {
+        set_error("gmnn_system_create: null argument or n_atoms <= 0");
+        return GMNN_INVALID_ARG;
+    }
+    if (n_atoms >= MAX_ATOMS) {
+        set_error("n_atoms = %lld exceeds the %lld the packed neighbour entries can address", (long long)n_atoms,
+                  (long long)MAX_ATOMS);
+        return GMNN_UNSUPPORTED;
+    }
+    for (int64_t i = 0; i < n_atoms; ++i)
+        if (species[i] < 0 || species[i] >= m->hp.n_species) {
+            set_error("species[%lld] = %d out of range", (long long)i, species[i]);
+            return GMNN_INVALID_ARG;
+        }
+    gmnn_system *s = new gmnn_system();
+    s->model = m;
+    s->N = n_atoms;
+    s->mlp_precision = m->hp.mlp_precision;
+    s->force_mode = m->hp.force_mode;
+    const size_t N = (size_t)n_atoms;
+    const int F = m->n_features, L = m->hp.n_hidden, M = m->hp.n_heads;
+    int maxw = 0;
+    for (int l = 1; l <= L; ++l) maxw = std::max(maxw, m->dims[l]);
+    int rc = upload(&s->species, species, N);
+#define A_(p, n) if (!rc) rc = dev_alloc(&(p), (n))
+    A_(s->cell_of, N);
+    A_(s->slot_tmp, N);
+    A_(s->perm, N);
+    A_(s->pos4, N);
+    A_(s->xref, 3 * N);
+    A_(s->count, N);
+    A_(s->psi, N * m->hp.n_radial * PSI);
+    A_(s->G, N * F);
+    A_(s->dG, N * F);
+    A_(s->A, N * m->hp.n_radial * PSI);
+    for (int l = 0; l < L; ++l) {
+        A_(s->H[l], N * m->dims[l + 1]);
+        A_(s->D[l], N * m->dims[l + 1]);
+    }
+    A_(s->dZ[0], N * maxw);
+    A_(s->dZ[1], N * maxw);
+    A_(s->Bv, (size_t)m->dims[L] * m->dims[L - 1]);
+    A_(s->vhead, (size_t)m->dims[L]);
+    A_(s->head_w, (size_t)M);
+    A_(s->e_heads, N * M);
+    A_(s->e_atom, N);
+    A_(s->f_int, 3 * N);
+    A_(s->f_tmp, 3 * N);
+    A_(s->partial, 2 * 1024);
+    A_(s->e_total, 2);
+    A_(s->flags, FLAG_WORDS);
+#undef A_
+    if (!rc && cudaMallocHost((void **)&s->flags_host, sizeof(int32_t) * FLAG_WORDS) != cudaSuccess) rc = GMNN_OOM;
+    if (!rc && cudaMemset(s->flags, 0, sizeof(int32_t) * FLAG_WORDS) != cudaSuccess) rc = GMNN_CUDA_ERROR;
+    if (rc) {
+        if (rc == GMNN_OOM) set_error("out of device memory allocating the workspaces of %lld atoms", (long long)n_atoms);
+        gmnn_system_destroy(s);
+        return rc;
+    }
+    *out = s;
+    return GMNN_OK;
+}
+
+void gmnn_system_destroy(gmnn_system *s) {
+    if (!s) return;
+    dev_free(s->species); dev_free(s->cell_of); dev_free(s->cell_count); dev_free(s->cell_start);
+    dev_free(s->cell_fill); dev_free(s->slot_tmp); dev_free(s->perm); dev_free(s->pos4); dev_free(s->xref);
+    dev_free(s->nbr); dev_free(s->count); dev_free(s->psi); dev_free(s->G); dev_free(s->dG); dev_free(s->A);
+    for (int l = 0; l < MAX_LAYERS; ++l) { dev_free(s->H[l]); dev_free(s->D[l]); }
+    dev_free(s->dZ[0]); dev_free(s->dZ[1]); dev_free(s->Bv); dev_free(s->vhead); dev_free(s->head_w);
+    dev_free(s->e_heads); dev_free(s->e_atom); dev_free(s->f_int); dev_free(s->f_tmp); dev_free(s->partial);
+    dev_free(s->e_total); dev_free(s->flags);
+    dev_free(s->stage_pos); dev_free(s->stage_f); dev_free(s->stage_e);
+    if (s->flags_host) cudaFreeHost(s->flags_host);
+    for (cudaEvent_t e : s->events) cudaEventDestroy(e);
+    delete s;
+}
+
+int gmnn_system_set_int(gmnn_system *s, const char *key, int64_t v) {
+    if (!s || !key) return GMNN_INVALID_ARG;
+    if (!strcmp(key, "lanes_per_atom")) {
+        if (v != 0 && v != 1 && v != 2 && v != 4 && v != 8 && v != 16 && v != 32) {
+            set_error("lanes_per_atom must be 0, 1, 2, 4, 8, 16 or 32");
+            return GMNN_INVALID_ARG;
+        }
+        s->lanes_per_atom = (int)v;
+    } else if (!strcmp(key, "profile")) {
+        s->profile = v != 0;
+    } else if (!strcmp(key, "capacity")) {
+        if (v < 0 || v > 4096) {
+            set_error("capacity must be in [0, 4096]");
+            return GMNN_INVALID_ARG;
+        }
+        s->cap_request = (int)v;
+    } else if (!strcmp(key, "mlp_precision")) {
+        if (v < 0 || v > GMNN_MLP_TF32) return GMNN_INVALID_ARG;
+        s->mlp_precision = (int)v;
+    } else if (!strcmp(key, "force_mode")) {
+        if (v < 0 || v > GMNN_FORCE_PAIRBUF) return GMNN_INVALID_ARG;
+        s->force_mode = (int)v;
+    } else {
+        set_error("unknown key '%s'", key);
+        return GMNN_INVALID_ARG;
+    }
+    return GMNN_OK;
+}
+
+int gmnn_system_get_int(const gmnn_system *s, const char *key, int64_t *v) {
+    if (!s || !key || !v) return GMNN_INVALID_ARG;
+    if (!strcmp(key, "lanes_per_atom")) *v = s->lanes_per_atom;
+    else if (!strcmp(key, "profile")) *v = s->profile;
+    else if (!strcmp(key, "capacity")) *v = s->cap;
+    else if (!strcmp(key, "mlp_precision")) *v = s->mlp_precision;
+    else if (!strcmp(key, "force_mode")) *v = s->force_mode;
+    else if (!strcmp(key, "n_cells")) *v = s->ncells;
+    else if (!strcmp(key, "small_box")) *v = s->small_box;
+    else {
+        set_error("unknown key '%s'", key);
+        return GMNN_INVALID_ARG;
+    }
+    return GMNN_OK;
+}
+
+static int read_flags(gmnn_system *s, cudaStream_t st) {
+    GMNN_CUDA(cudaMemcpyAsync(s->flags_host, s->flags, sizeof(int32_t) * FLAG_WORDS, cudaMemcpyDeviceToHost, st));
+    GMNN_CUDA(cudaStreamSynchronize(st));
+    return GMNN_OK;
+}
+
+int gmnn_build_neighbors(gmnn_system *s, const float *positions, const float cell[9], const int32_t pbc[3],
+                         float r_cut, float skin, void *cuda_stream) {
+    if (!s || !positions || !cell || !pbc) {
+        set_error("gmnn_build_neighbors: null argument");
+        return GMNN_INVALID_ARG;
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (r_cut != s->model->hp.r_cut) {
+        set_error("r_cut = %g differs from the model's %g", r_cut, s->model->hp.r_cut);
+        return GMNN_INVALID_ARG;
+    }
+    if (!(skin >= 0.f) || !std::isfinite(skin)) {
+        set_error("skin must be finite and >= 0");
+        return GMNN_INVALID_ARG;
+    }
+    for (int a = 0; a < 3; ++a)
+        for (int b = 0; b < 3; ++b) {
+            const float v = cell[3 * a + b];
+            if (!std::isfinite(v) || (a == b && !(v > 0.f))) {
+                set_error("cell must be finite with positive diagonal");
+                return GMNN_INVALID_ARG;
+            }
+            if (a != b && v != 0.f) {
+                set_error("triclinic cells are not supported (orthorhombic only, DESIGN.md R19)");
+                return GMNN_UNSUPPORTED;
+            }
+        }
+    Geometry &g = s->geo;
+    const float r_list = r_cut + skin;  // fl32(fl32(r_cut) + fl32(skin)): the oracle is handed the same float
+    g.r_list2 = r_list * r_list;
+    bool small = false;
+    for (int a = 0; a < 3; ++a) {
+        g.L[a] = cell[4 * a];
+        g.invL[a] = 1.f / g.L[a];
+        g.pbc[a] = pbc[a] != 0;
+        int nc = (int)std::floor((double)g.L[a] / ((double)r_list * (1.0 + 1e-5)));
+        if (nc < 1) nc = 1;
+        if (nc > 1024) nc = 1024;
+        g.ncell[a] = nc;
+        if (g.pbc[a] && nc < 3) small = true;
+    }
+    if (small) {
+        if (s->N > SMALL_BOX_MAX_ATOMS) {
+            set_error("box has < 3 cells on a periodic axis: the all-pairs image path is limited to %d atoms",
+                      SMALL_BOX_MAX_ATOMS);
+            return GMNN_UNSUPPORTED;
+        }
+        for (int a = 0; a < 3; ++a) {
+            g.kimg[a] = g.pbc[a] ? (int)std::ceil(r_list / g.L[a]) : 0;  // fp32 division, as the oracle's ceilf
+            if (g.kimg[a] > 3) {
+                set_error("box edge %g needs more than 3 periodic images at r_list = %g", g.L[a], r_list);
+                return GMNN_UNSUPPORTED;
+            }
+            g.ncell[a] = 1;
+        }
+    } else {
+        g.kimg[0] = g.kimg[1] = g.kimg[2] = 0;
+    }
+    for (int a = 0; a < 3; ++a) g.inv_edge[a] = (float)g.ncell[a] / g.L[a];
+    s->small_box = small;
+    s->r_cut = r_cut;
+    s->skin = skin;
+    s->ncells = (int64_t)g.ncell[0] * g.ncell[1] * g.ncell[2];
+    if (s->ncells > s->ncells_alloc) {
+        dev_free(s->cell_count);
+        dev_free(s->cell_start);
+        dev_free(s->cell_fill);
+        int rc = dev_alloc(&s->cell_count, (size_t)s->ncells + 1);
+        if (!rc) rc = dev_alloc(&s->cell_start, (size_t)s->ncells + 1);
+        if (!rc) rc = dev_alloc(&s->cell_fill, (size_t)s->ncells);
+        if (rc) return rc;
+        s->ncells_alloc = s->ncells;
+    }
+    // capacity: expected neighbours at uniform density x 1.3 + 32, a multiple of 32
+    int want = s->cap_request;
+    if (want <= 0) {
+        double vol = (double)g.L[0] * g.L[1] * g.L[2];
+        double per = (double)s->N / vol * 4.0 / 3.0 * M_PI * std::pow((double)r_list, 3.0);
+        if (small) {  // count the images as well
+            per = (double)s->N / vol * 4.0 / 3.0 * M_PI * std::pow((double)r_list, 3.0);
+        }
+        want = (int)(per * 1.3) + 32;
+    }
+    want = (want + 31) & ~31;
+    for (int attempt = 0; attempt < 4; ++attempt) {
+        if (want > s->cap || !s->nbr) {
+            dev_free(s->nbr);
+            s->cap = want;
+            int rc = dev_alloc(&s->nbr, (size_t)s->N * s->cap);
+            if (rc) {
+                set_error("out of device memory for the neighbour list (%lld x %d)", (long long)s->N, s->cap);
+                s->cap = 0;
+                return rc;
+            }
+        }
+        GMNN_CUDA(cudaMemsetAsync(s->flags, 0, sizeof(int32_t) * FLAG_WORDS, st));
+        int rc = launch_build(s, positions, st, nullptr, 0.f, false, nullptr);
+        if (rc) return rc;
+        if ((rc = read_flags(s, st))) return rc;
+        if (s->flags_host[FLAG_OUT_OF_BOX]) {
+            s->have_list = false;
+            set_error("a position is outside [0, L): wrap positions before gmnn_build_neighbors");
+            return GMNN_OUT_OF_BOX;
+        }
+        if (s->flags_host[FLAG_MAXCOUNT] <= s->cap) {
+            s->have_list = true;
+            GMNN_CUDA(cudaMemsetAsync(s->flags, 0, sizeof(int32_t) * FLAG_WORDS, st));
+            return GMNN_OK;
+        }
+        want = ((int)(s->flags_host[FLAG_MAXCOUNT] * 1.15) + 32 + 31) & ~31;
+    }
+    set_error("neighbour list kept overflowing");
+    return GMNN_NEIGHBOR_OVERFLOW;
+}
+
+int gmnn_get_neighbors(gmnn_system *s, int64_t *n_pairs, int32_t *oi, int32_t *oj, int32_t *oimg) {
+    if (!s || !n_pairs) return GMNN_INVALID_ARG;
+    if (!s->have_list) {
+        set_error("no neighbour list: call gmnn_build_neighbors first");
+        return GMNN_INVALID_ARG;
+    }
+    const size_t N = (size_t)s->N;
+    std::vector<int32_t> cnt(N), perm(N);
+    GMNN_CUDA(cudaDeviceSynchronize());
+    GMNN_CUDA(cudaMemcpy(cnt.data(), s->count, sizeof(int32_t) * N, cudaMemcpyDeviceToHost));
+    GMNN_CUDA(cudaMemcpy(perm.data(), s->perm, sizeof(int32_t) * N, cudaMemcpyDeviceToHost));
+    int64_t total = 0;
+    for (size_t k = 0; k < N; ++k) total += cnt[k];
+    *n_pairs = total;
+    if (!oi && !oj && !oimg) return GMNN_OK;
+    if (!oi || !oj || !oimg) return GMNN_INVALID_ARG;
+    std::vector<uint32_t> nbr(N * (size_t)s->cap);
+    GMNN_CUDA(cudaMemcpy(nbr.data(), s->nbr, sizeof(uint32_t) * nbr.size(), cudaMemcpyDeviceToHost));
+    struct Row { int32_t i, j, n[3]; };
+    std::vector<Row> rows;
+    rows.reserve((size_t)total);
+    for (size_t k = 0; k < N; ++k)
+        for (int q = 0; q < cnt[k]; ++q) {
+            const uint32_t e = nbr[k * (size_t)s->cap + q];
+            Row r;
+            r.i = perm[k];
+            r.j = perm[e & NBR_J_MASK];
+            r.n[0] = (int)((e >> NBR_J_BITS) & 7u) - 4;
+            r.n[1] = (int)((e >> (NBR_J_BITS + 3)) & 7u) - 4;
+            r.n[2] = (int)((e >> (NBR_J_BITS + 6)) & 7u) - 4;
+            rows.push_back(r);
+        }
+    std::sort(rows.begin(), rows.end(), [](const Row &a, const Row &b) {
+        if (a.i != b.i) return a.i < b.i;
+        if (a.j != b.j) return a.j < b.j;
+        if (a.n[0] != b.n[0]) return a.n[0] < b.n[0];
+        if (a.n[1] != b.n[1]) return a.n[1] < b.n[1];
+        return a.n[2] < b.n[2];
+    });
+    for (size_t p = 0; p < rows.size(); ++p) {
+        oi[p] = rows[p].i;
+        oj[p] = rows[p].j;
+        oimg[3 * p] = rows[p].n[0];
+        oimg[3 * p + 1] = rows[p].n[1];
+        oimg[3 * p + 2] = rows[p].n[2];
+    }
+    return GMNN_OK;
+}
+
+int gmnn_energy_forces(gmnn_system *s, const float *positions, double *energy, float *energy_per_atom, float *forces,
+                       void *cuda_stream) {
+    if (!s || !positions || !energy || !forces) {
+        set_error("gmnn_energy_forces: null argument");
+        return GMNN_INVALID_ARG;
+    }
+    if (!s->have_list) {
+        set_error("no neighbour list: call gmnn_build_neighbors first");
+        return GMNN_INVALID_ARG;
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    StageTimer T(s, st);
+    T.begin();
+    int rc = forward_backward(s, positions, s->model->head_mean_w, true, st, T);
+    if (rc) return rc;
+    if ((rc = launch_scatter_outputs(s, energy_per_atom, forces, st))) return rc;
+    if ((rc = launch_energy_sum(s, energy, st))) return rc;
+    T.mark("outputs");
+    return GMNN_OK;
+}
+
+int gmnn_energy_forces_host(gmnn_system *s, const float *positions, double *energy, float *energy_per_atom,
+                            float *forces, void *cuda_stream) {
+    if (!s || !positions || !energy || !forces) {
+        set_error("gmnn_energy_forces_host: null argument");
+        return GMNN_INVALID_ARG;
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t N = (size_t)s->N;
+    int rc = GMNN_OK;
+    if (!s->stage_pos) {
+        rc = dev_alloc(&s->stage_pos, 3 * N);
+        if (!rc) rc = dev_alloc(&s->stage_f, 3 * N);
+        if (!rc) rc = dev_alloc(&s->stage_e, N);
+        if (rc) return rc;
+    }
+    GMNN_CUDA(cudaMemcpyAsync(s->stage_pos, positions, sizeof(float) * 3 * N, cudaMemcpyHostToDevice, st));
+    rc = gmnn_energy_forces(s, s->stage_pos, s->e_total, energy_per_atom ? s->stage_e : nullptr, s->stage_f, st);
+    if (rc) return rc;
+    GMNN_CUDA(cudaMemcpyAsync(forces, s->stage_f, sizeof(float) * 3 * N, cudaMemcpyDeviceToHost, st));
+    if (energy_per_atom)
+        GMNN_CUDA(cudaMemcpyAsync(energy_per_atom, s->stage_e, sizeof(float) * N, cudaMemcpyDeviceToHost, st));
+    GMNN_CUDA(cudaMemcpyAsync(energy, s->e_total, sizeof(double), cudaMemcpyDeviceToHost, st));
+    GMNN_CUDA(cudaStreamSynchronize(st));
+    return GMNN_OK;
+}
+
+int gmnn_ensemble_energy_forces(gmnn_system *s, const float *positions, float *e_mean, float *e_var, float *f_mean,
+                                float *f_var, void *cuda_stream) {
+    if (!s || !positions || !e_mean || !e_var || !f_mean || !f_var) {
+        set_error("gmnn_ensemble_energy_forces: null argument");
+        return GMNN_INVALID_ARG;
+    }
+    if (!s->have_list) {
+        set_error("no neighbour list: call gmnn_build_neighbors first");
+        return GMNN_INVALID_ARG;
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const int M = s->model->hp.n_heads;
+    int rc;
+    const int keep_profile = s->profile;
+    s->profile = 0;
+    if ((rc = launch_gather_positions(s, positions, st, true))) return rc;
+    if ((rc = launch_pair_forward(s, st))) return rc;
+    if ((rc = launch_contract_forward(s, st))) return rc;
+    if ((rc = mlp_forward(s, st))) return rc;
+    if ((rc = launch_mlp_heads(s, s->model->head_mean_w, st))) return rc;
+    if ((rc = launch_ensemble_energy_stats(s, e_mean, e_var, st))) return rc;
+    for (int m = 0; m < M; ++m) {
+        k_set_onehot<<<1, 64, 0, st>>>(M, m, s->head_w);
+        GMNN_LAUNCHED();
+        if ((rc = mlp_backward(s, s->head_w, st))) return rc;
+        if ((rc = launch_contract_backward(s, st))) return rc;
+        if ((rc = launch_pair_backward(s, st))) return rc;
+        if ((rc = launch_scatter_outputs(s, nullptr, s->f_tmp, st))) return rc;
+        if ((rc = launch_welford(s, m, s->f_tmp, f_mean, f_var, st))) return rc;
+    }
+    if ((rc = launch_finish_var(3 * s->N, f_var, M, st))) return rc;
+    s->profile = keep_profile;
+    GMNN_CUDA(cudaGetLastError());
+    return GMNN_OK;
+}
+
+int gmnn_md_verlet_steps(gmnn_system *s, float *positions, float *velocities, const float *masses, float dt_fs,
+                         int32_t n_steps, double *epot_series, double *ekin_series, int32_t *n_rebuilds,
+                         void *cuda_stream) {
+    if (!s || !positions || !velocities || !masses || n_steps < 0 || !(dt_fs > 0.f)) {
+        set_error("gmnn_md_verlet_steps: bad argument");
+        return GMNN_INVALID_ARG;
+    }
+    if (!s->have_list) {
+        set_error("no neighbour list: call gmnn_build_neighbors first");
+        return GMNN_INVALID_ARG;
+    }
+    if (s->model->hp.n_heads != 1) {
+        set_error("MD runs on a single-head model (mean-energy MD of ensembles: DESIGN.md NEXT-1)");
+        return GMNN_UNSUPPORTED;
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const int keep_profile = s->profile;
+    s->profile = 0;
+    const float hs = 0.5f * s->skin;
+    const float thr2 = hs * hs;
+    int rc;
+    StageTimer T(s, st);  // profiling is off inside the loop: marks are no-ops
+    // state at entry: forces of the current positions
+    if ((rc = forward_backward(s, positions, s->model->head_mean_w, false, st, T))) return rc;
+    if ((rc = launch_scatter_outputs(s, nullptr, s->f_tmp, st))) return rc;
+    if (epot_series && (rc = launch_energy_sum(s, epot_series, st))) return rc;
+    if (ekin_series && (rc = launch_ke(s, velocities, masses, ekin_series, st))) return rc;
+    for (int step = 1; step <= n_steps; ++step) {
+        if ((rc = launch_kick_drift(s, positions, velocities, s->f_tmp, masses, dt_fs, st))) return rc;
+        // rebuild (wrap first) iff the max displacement since the last build exceeds skin/2
+        if ((rc = launch_build(s, positions, st, s->flags + FLAG_DISP2, thr2, true, positions))) return rc;
+        if ((rc = forward_backward(s, positions, s->model->head_mean_w, false, st, T))) return rc;
+        if ((rc = launch_scatter_outputs(s, nullptr, s->f_tmp, st))) return rc;
+        if (epot_series && (rc = launch_energy_sum(s, epot_series + step, st))) return rc;
+        if ((rc = launch_kick_ke(s, velocities, s->f_tmp, masses, dt_fs, ekin_series ? ekin_series + step : nullptr, st)))
+            return rc;
+    }
+    s->profile = keep_profile;
+    if ((rc = read_flags(s, st))) return rc;
+    if (n_rebuilds) *n_rebuilds = s->flags_host[FLAG_REBUILDS];
+    const int maxcount = s->flags_host[FLAG_MAXCOUNT];
+    GMNN_CUDA(cudaMemsetAsync(s->flags, 0, sizeof(int32_t) * FLAG_WORDS, st));
+    if (maxcount > s->cap) {
+        set_error("an in-loop rebuild needed %d neighbour slots, capacity is %d: raise \"capacity\" and rerun", maxcount,
+                  s->cap);
+        return GMNN_NEIGHBOR_OVERFLOW;
+    }
+    return GMNN_OK;
+}
+
+int gmnn_check(gmnn_system *s, void *cuda_stream) {
+    if (!s) return GMNN_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int rc = read_flags(s, st);
+    if (rc) return rc;
+    const int stale = s->flags_host[FLAG_STALE], oob = s->flags_host[FLAG_OUT_OF_BOX],
+              over = s->flags_host[FLAG_MAXCOUNT] > s->cap;
+    GMNN_CUDA(cudaMemsetAsync(s->flags, 0, sizeof(int32_t) * FLAG_WORDS, st));
+    if (oob) {
+        set_error("a position was outside [0, L) at a neighbour build");
+        return GMNN_OUT_OF_BOX;
+    }
+    if (over) {
+        set_error("neighbour list capacity exceeded");
+        return GMNN_NEIGHBOR_OVERFLOW;
+    }
+    if (stale) {
+        set_error("an atom moved more than skin/2 since the neighbour list was built");
+        return GMNN_STALE_NEIGHBORS;
+    }
+    return GMNN_OK;
+}
+
+int gmnn_stage_times(gmnn_system *s, int32_t max_stages, const char **names, float *ms) {
+    if (!s || !names || !ms) return GMNN_INVALID_ARG;
+    const int n = (int)s->stage_names.size();
+    if (n == 0 || (int)s->events.size() < n + 1) return 0;
+    GMNN_CUDA(cudaEventSynchronize(s->events[n]));
+    int k = 0;
+    for (; k < n && k < max_stages; ++k) {
+        names[k] = s->stage_names[k];
+        GMNN_CUDA(cudaEventElapsedTime(&ms[k], s->events[k], s->events[k + 1]));
+    }
+    return k;
+}
+
+int gmnn_debug_read(gmnn_system *s, const char *name, void *dst, int64_t bytes) {
+    if (!s || !name || !dst) return GMNN_INVALID_ARG;
+    const int64_t N = s->N;
+    const gmnn_model *m = s->model;
+    const void *src = nullptr;
+    int64_t need = 0;
+    if (!strcmp(name, "perm")) { src = s->perm; need = 4 * N; }
+    else if (!strcmp(name, "count")) { src = s->count; need = 4 * N; }
+    else if (!strcmp(name, "psi")) { src = s->psi; need = 4 * N * m->hp.n_radial * PSI; }
+    else if (!strcmp(name, "A")) { src = s->A; need = 4 * N * m->hp.n_radial * PSI; }
+    else if (!strcmp(name, "G")) { src = s->G; need = 4 * N * m->n_features; }
+    else if (!strcmp(name, "dG")) { src = s->dG; need = 4 * N * m->n_features; }
+    else if (!strcmp(name, "e_heads")) { src = s->e_heads; need = 4 * N * m->hp.n_heads; }
+    else {
+        set_error("gmnn_debug_read: unknown array '%s'", name);
+        return GMNN_INVALID_ARG;
+    }
+    if (bytes != need) {
+        set_error("gmnn_debug_read('%s'): expected %lld bytes, got %lld", name, (long long)need, (long long)bytes);
+        return GMNN_INVALID_ARG;
+    }
+    GMNN_CUDA(cudaDeviceSynchronize());
+    GMNN_CUDA(cudaMemcpy(dst, src, (size_t)bytes, cudaMemcpyDeviceToHost));
+    return GMNN_OK;
+}
+
+}  // extern "C"

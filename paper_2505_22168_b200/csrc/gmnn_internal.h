@@ -1,0 +1,152 @@
+// gmnn_internal.h -- handles, device buffers and kernel launchers shared by the .cu files of
+// libgmnn_b200.so.  Nothing here is visible through the C ABI (include/gmnn.h).
+#pragma once
+
+#include <cuda_runtime.h>
+
+#include <cstdint>
+#include <cstdio>
+#include <string>
+#include <vector>
+
+#include "../../include/gmnn.h"
+
+namespace gmnn {
+
+constexpr int MAX_SPECIES = 8;
+constexpr int MAX_BASIS = 16;
+constexpr int MAX_LAYERS = 5;
+constexpr int NBR_J_BITS = 22;  // neighbour entry: j in the low 22 bits, image code above
+constexpr uint32_t NBR_J_MASK = (1u << NBR_J_BITS) - 1u;
+constexpr int64_t MAX_ATOMS = (int64_t)1 << NBR_J_BITS;
+constexpr int SMALL_BOX_MAX_ATOMS = 16384;
+constexpr int PSI = 20;  // unique monomials per channel (contraction.cuh NM)
+
+// device-side flag words (int32) in System::flags
+enum Flag { FLAG_MAXCOUNT = 0, FLAG_STALE = 1, FLAG_OUT_OF_BOX = 2, FLAG_REBUILDS = 3, FLAG_DISP2 = 4, FLAG_WORDS = 8 };
+
+void set_error(const char *fmt, ...);
+extern long long g_launch_count;
+#define GMNN_LAUNCHED() (++::gmnn::g_launch_count)
+
+#define GMNN_CUDA(expr)                                                                          \
+    do {                                                                                         \
+        cudaError_t err__ = (expr);                                                              \
+        if (err__ != cudaSuccess) {                                                              \
+            ::gmnn::set_error("%s failed: %s (%s:%d)", #expr, cudaGetErrorString(err__), __FILE__, __LINE__); \
+            return err__ == cudaErrorMemoryAllocation ? GMNN_OOM : GMNN_CUDA_ERROR;              \
+        }                                                                                        \
+    } while (0)
+
+struct Geometry {  // passed by value to kernels
+    float L[3];
+    float invL[3];
+    int pbc[3];
+    int ncell[3];
+    float inv_edge[3];
+    int kimg[3];  // image range of the small-box path
+    float r_list2;
+};
+
+struct RadialParams {  // passed by value to the pair kernels
+    int n_species, n_basis, kb;  // kb = n_basis rounded up to 4 (row pitch of the beta table)
+    float r_cut, r_cut2, inv_rc, r_min, delta, gamma;
+};
+
+}  // namespace gmnn
+
+struct gmnn_model {
+    gmnn_hparams hp;
+    int n_features;
+    int n_layers;              // n_hidden + 1
+    int dims[gmnn::MAX_LAYERS + 1];  // dims[0] = F, hidden..., n_heads
+    gmnn::RadialParams rp;
+    float *beta = nullptr;     // [S*S][n_radial][kb] zero padded
+    float *W[gmnn::MAX_LAYERS] = {};   // [fan_in][fan_out]
+    float *WT[gmnn::MAX_LAYERS] = {};  // [fan_out][fan_in]
+    float *b[gmnn::MAX_LAYERS] = {};
+    float *scale = nullptr, *shift = nullptr;  // [S]
+    float *head_mean_w = nullptr;  // [n_heads] = 1/M (device)
+};
+
+struct gmnn_system {
+    const gmnn_model *model = nullptr;
+    int64_t N = 0;
+    int32_t *species = nullptr;  // caller order (device)
+    // geometry of the last build
+    bool have_list = false, small_box = false;
+    gmnn::Geometry geo{};
+    float r_cut = 0.f, skin = 0.f;
+    int64_t ncells = 0, ncells_alloc = 0;
+    // cell sort
+    int32_t *cell_of = nullptr;      // [N] caller order
+    int32_t *cell_count = nullptr;   // [ncells + 1]
+    int32_t *cell_start = nullptr;   // [ncells + 1]
+    int32_t *cell_fill = nullptr;    // [ncells]
+    int32_t *slot_tmp = nullptr;     // [N]
+    int32_t *perm = nullptr;         // [N] internal -> caller
+    float4 *pos4 = nullptr;          // [N] internal order: x y z species(bits)
+    float *xref = nullptr;           // [N][3] caller order, positions at build
+    // neighbour list
+    uint32_t *nbr = nullptr;         // [N][cap]
+    int32_t *count = nullptr;        // [N]
+    int cap = 0;
+    int cap_request = 0;
+    // workspaces (internal order)
+    float *psi = nullptr, *G = nullptr, *dG = nullptr, *A = nullptr;
+    float *H[gmnn::MAX_LAYERS] = {}, *D[gmnn::MAX_LAYERS] = {};
+    float *dZ[2] = {};
+    float *Bv = nullptr;             // diag(v) W^T of the last hidden layer
+    float *vhead = nullptr;          // [H_last]
+    float *head_w = nullptr;         // [n_heads] weights of the differentiated energy
+    float *e_heads = nullptr;        // [N][n_heads]
+    float *e_atom = nullptr;         // [N]
+    float *f_int = nullptr;          // [N][3]
+    float *f_tmp = nullptr;          // [N][3] caller order (ensemble, MD)
+    double *partial = nullptr;       // reduction scratch
+    double *e_total = nullptr;       // [2] device scalars (epot, ekin)
+    int32_t *flags = nullptr;        // FLAG_WORDS
+    int32_t *flags_host = nullptr;   // pinned
+    // knobs
+    int lanes_per_atom = 0;
+    int profile = 0;
+    int mlp_precision = 0, force_mode = 0;
+    // stage timing
+    std::vector<cudaEvent_t> events;
+    std::vector<const char *> stage_names;
+    int n_stage_events = 0;
+    // host staging for the _host entry
+    float *stage_pos = nullptr, *stage_f = nullptr, *stage_e = nullptr;
+};
+
+namespace gmnn {
+
+// neighbor.cu
+int launch_build(gmnn_system *s, const float *positions, cudaStream_t st, const int32_t *cond, float thr2,
+                 bool wrap_first, float *positions_mut);
+int launch_gather_positions(gmnn_system *s, const float *positions, cudaStream_t st, bool check_stale);
+
+// descriptor.cu
+int launch_pair_forward(gmnn_system *s, cudaStream_t st);
+int launch_contract_forward(gmnn_system *s, cudaStream_t st);
+int launch_contract_backward(gmnn_system *s, cudaStream_t st);
+int launch_pair_backward(gmnn_system *s, cudaStream_t st);
+
+// mlp_simt.cu
+int launch_mlp_forward_simt(gmnn_system *s, cudaStream_t st);
+int launch_mlp_heads(gmnn_system *s, const float *head_w_dev, cudaStream_t st);
+int launch_mlp_seed(gmnn_system *s, const float *head_w_dev, cudaStream_t st);
+int launch_mlp_backward_simt(gmnn_system *s, const float *head_w_dev, cudaStream_t st);
+
+// md.cu / reductions
+int launch_scatter_outputs(gmnn_system *s, float *e_atom_out, float *forces_out, cudaStream_t st);
+int launch_energy_sum(gmnn_system *s, double *energy_out, cudaStream_t st);
+int launch_kick_drift(gmnn_system *s, float *x, float *v, const float *f, const float *m, float dt, cudaStream_t st);
+int launch_kick_ke(gmnn_system *s, float *v, const float *f, const float *m, float dt, double *ekin_out,
+                   cudaStream_t st);
+int launch_ke(gmnn_system *s, const float *v, const float *m, double *ekin_out, cudaStream_t st);
+int launch_welford(gmnn_system *s, int head, const float *f_head, float *f_mean, float *f_m2, cudaStream_t st);
+int launch_ensemble_energy_stats(gmnn_system *s, float *e_mean, float *e_var, cudaStream_t st);
+int launch_finish_var(int64_t n, float *m2, int n_heads, cudaStream_t st);
+
+}  // namespace gmnn

@@ -1,0 +1,210 @@
+// md.cu -- output scatter, fixed-order fp64 reductions, velocity-Verlet kicks and drift with the
+// skin test, and the ensemble statistics (Eq. 5,
+// :169-171 MD loop on the device, :367 dt, :381 skin).
+#include "gmnn_internal.h"
+
+namespace gmnn {
+
+constexpr double ACC_CONV = 9.648533212e-3;  // (eV/Ang/amu) -> Ang/fs^2
+constexpr int RED_BLOCKS = 1024;             // partial sums of the two-stage reductions
+
+static inline unsigned nblocks(int64_t n, int per) { return (unsigned)((n + per - 1) / per); }
+
+// internal (cell-sorted) order -> caller order
+__global__ void k_scatter(int64_t N, const int32_t *__restrict__ perm, const float *__restrict__ e_int,
+                          const float *__restrict__ f_int, float *e_out, float *f_out) {
+    const int64_t k = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (k >= N) return;
+    const int64_t i = perm[k];
+    if (e_out) e_out[i] = e_int[k];
+    if (f_out) {
+        f_out[3 * i] = f_int[3 * k];
+        f_out[3 * i + 1] = f_int[3 * k + 1];
+        f_out[3 * i + 2] = f_int[3 * k + 2];
+    }
+}
+
+__device__ __forceinline__ double block_sum(double v) {
+    __shared__ double sh[32];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+    for (int o = 16; o >= 1; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    if (lane == 0) sh[wid] = v;
+    __syncthreads();
+    v = (threadIdx.x < (blockDim.x >> 5)) ? sh[threadIdx.x] : 0.0;
+    if (wid == 0) {
+#pragma unroll
+        for (int o = 16; o >= 1; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    }
+    __syncthreads();
+    return v;  // valid in thread 0
+}
+
+// stage 1: block b sums a fixed contiguous slice in a fixed order; stage 2: one block sums the
+// partials.  The result depends on N only, never on scheduling.
+__global__ void __launch_bounds__(256) k_sum_stage1(int64_t N, const float *__restrict__ x, double *partial) {
+    const int64_t per = (N + gridDim.x - 1) / gridDim.x;
+    const int64_t b = blockIdx.x * per, e = (b + per < N) ? b + per : N;
+    double v = 0.0;
+    for (int64_t q = b + threadIdx.x; q < e; q += blockDim.x) v += (double)x[q];
+    v = block_sum(v);
+    if (threadIdx.x == 0) partial[blockIdx.x] = v;
+}
+
+__global__ void __launch_bounds__(256) k_ke_stage1(int64_t N, const float *__restrict__ v, const float *__restrict__ m,
+                                                  double *partial) {
+    const int64_t per = (N + gridDim.x - 1) / gridDim.x;
+    const int64_t b = blockIdx.x * per, e = (b + per < N) ? b + per : N;
+    double acc = 0.0;
+    for (int64_t q = b + threadIdx.x; q < e; q += blockDim.x) {
+        const double vx = v[3 * q], vy = v[3 * q + 1], vz = v[3 * q + 2];
+        acc += 0.5 * (double)m[q] * (vx * vx + vy * vy + vz * vz);
+    }
+    acc = block_sum(acc);
+    if (threadIdx.x == 0) partial[blockIdx.x] = acc;
+}
+
+__global__ void __launch_bounds__(256) k_sum_stage2(int n, const double *__restrict__ partial, double factor, double *out) {
+    double v = 0.0;
+    for (int q = threadIdx.x; q < n; q += blockDim.x) v += partial[q];
+    v = block_sum(v);
+    if (threadIdx.x == 0) *out = v * factor;
+}
+
+// v += (dt/2) a;  x += dt v;  squared displacement from the build positions -> max into flags.
+__global__ void __launch_bounds__(256)
+k_kick_drift(int64_t N, float *x, float *v, const float *__restrict__ f, const float *__restrict__ m, float dt,
+             const float *__restrict__ xref, int32_t *flags) {
+    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    float d2 = 0.f;
+    if (i < N) {
+        const float c = 0.5f * dt * (float)ACC_CONV / m[i];
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            float vv = fmaf(c, f[3 * i + a], v[3 * i + a]);
+            float xx = fmaf(dt, vv, x[3 * i + a]);
+            v[3 * i + a] = vv;
+            x[3 * i + a] = xx;
+            const float d = xx - xref[3 * i + a];
+            d2 = fmaf(d, d, d2);
+        }
+    }
+#pragma unroll
+    for (int o = 16; o >= 1; o >>= 1) d2 = fmaxf(d2, __shfl_xor_sync(0xffffffffu, d2, o));
+    if ((threadIdx.x & 31) == 0 && d2 > 0.f) atomicMax(&flags[FLAG_DISP2], __float_as_int(d2));  // d2 >= 0: int order = float order
+}
+
+__global__ void __launch_bounds__(256)
+k_kick(int64_t N, float *v, const float *__restrict__ f, const float *__restrict__ m, float dt) {
+    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const float c = 0.5f * dt * (float)ACC_CONV / m[i];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) v[3 * i + a] = fmaf(c, f[3 * i + a], v[3 * i + a]);
+}
+
+// Welford update in head order: after head h (0-based), mean/M2 of heads 0..h.
+__global__ void k_welford(int64_t n, int head, const float *__restrict__ x, float *mean, float *m2) {
+    const int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (t >= n) return;
+    const float v = x[t];
+    if (head == 0) {
+        mean[t] = v;
+        m2[t] = 0.f;
+    } else {
+        const float mu = mean[t];
+        const float d = v - mu;
+        const float mu2 = mu + d / (float)(head + 1);
+        mean[t] = mu2;
+        m2[t] = fmaf(d, v - mu2, m2[t]);
+    }
+}
+
+__global__ void k_finish_var(int64_t n, float *m2, float inv_heads) {
+    const int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (t < n) m2[t] *= inv_heads;
+}
+
+// per-atom energy mean / population variance over the heads (Eq. 5 with 1/N_ens), caller order
+__global__ void k_energy_stats(int64_t N, int M, const int32_t *__restrict__ perm, const float *__restrict__ e_heads,
+                               float *e_mean, float *e_var) {
+    const int64_t k = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (k >= N) return;
+    const float *e = e_heads + k * (int64_t)M;
+    float mu = 0.f;
+    for (int m = 0; m < M; ++m) mu += e[m];
+    mu /= (float)M;
+    float var = 0.f;
+    for (int m = 0; m < M; ++m) var = fmaf(e[m] - mu, e[m] - mu, var);
+    const int64_t i = perm[k];
+    e_mean[i] = mu;
+    e_var[i] = var / (float)M;
+}
+
+int launch_scatter_outputs(gmnn_system *s, float *e_atom_out, float *forces_out, cudaStream_t st) {
+    k_scatter<<<nblocks(s->N, 256), 256, 0, st>>>(s->N, s->perm, s->e_atom, s->f_int, e_atom_out, forces_out);
+    GMNN_LAUNCHED();
+    GMNN_CUDA(cudaGetLastError());
+    return GMNN_OK;
+}
+
+static int red_blocks(int64_t N) { return (int)(N < RED_BLOCKS * 256 ? (N + 255) / 256 : RED_BLOCKS); }
+
+int launch_energy_sum(gmnn_system *s, double *energy_out, cudaStream_t st) {
+    const int nb = red_blocks(s->N);
+    k_sum_stage1<<<nb, 256, 0, st>>>(s->N, s->e_atom, s->partial);
+    GMNN_LAUNCHED();
+    k_sum_stage2<<<1, 256, 0, st>>>(nb, s->partial, 1.0, energy_out);
+    GMNN_LAUNCHED();
+    GMNN_CUDA(cudaGetLastError());
+    return GMNN_OK;
+}
+
+int launch_ke(gmnn_system *s, const float *v, const float *m, double *ekin_out, cudaStream_t st) {
+    const int nb = red_blocks(s->N);
+    k_ke_stage1<<<nb, 256, 0, st>>>(s->N, v, m, s->partial + RED_BLOCKS);
+    GMNN_LAUNCHED();
+    k_sum_stage2<<<1, 256, 0, st>>>(nb, s->partial + RED_BLOCKS, 1.0 / ACC_CONV, ekin_out);
+    GMNN_LAUNCHED();
+    GMNN_CUDA(cudaGetLastError());
+    return GMNN_OK;
+}
+
+int launch_kick_drift(gmnn_system *s, float *x, float *v, const float *f, const float *m, float dt, cudaStream_t st) {
+    k_kick_drift<<<nblocks(s->N, 256), 256, 0, st>>>(s->N, x, v, f, m, dt, s->xref, s->flags);
+    GMNN_LAUNCHED();
+    GMNN_CUDA(cudaGetLastError());
+    return GMNN_OK;
+}
+
+int launch_kick_ke(gmnn_system *s, float *v, const float *f, const float *m, float dt, double *ekin_out, cudaStream_t st) {
+    k_kick<<<nblocks(s->N, 256), 256, 0, st>>>(s->N, v, f, m, dt);
+    GMNN_LAUNCHED();
+    GMNN_CUDA(cudaGetLastError());
+    if (ekin_out) return launch_ke(s, v, m, ekin_out, st);
+    return GMNN_OK;
+}
+
+int launch_welford(gmnn_system *s, int head, const float *f_head, float *f_mean, float *f_m2, cudaStream_t st) {
+    k_welford<<<nblocks(3 * s->N, 256), 256, 0, st>>>(3 * s->N, head, f_head, f_mean, f_m2);
+    GMNN_LAUNCHED();
+    GMNN_CUDA(cudaGetLastError());
+    return GMNN_OK;
+}
+
+int launch_finish_var(int64_t n, float *m2, int n_heads, cudaStream_t st) {
+    k_finish_var<<<nblocks(n, 256), 256, 0, st>>>(n, m2, 1.f / (float)n_heads);
+    GMNN_LAUNCHED();
+    GMNN_CUDA(cudaGetLastError());
+    return GMNN_OK;
+}
+
+int launch_ensemble_energy_stats(gmnn_system *s, float *e_mean, float *e_var, cudaStream_t st) {
+    k_energy_stats<<<nblocks(s->N, 256), 256, 0, st>>>(s->N, s->model->dims[s->model->hp.n_hidden + 1], s->perm,
+                                                       s->e_heads, e_mean, e_var);
+    GMNN_LAUNCHED();
+    GMNN_CUDA(cudaGetLastError());
+    return GMNN_OK;
+}
+
+}  // namespace gmnn

@@ -1,0 +1,241 @@
+// mlp_simt.cu -- the per-atom MLP readout and its input gradient in plain fp32 FMA
+// (SURVEY.md 8(a) rows a7, a8; PAPER.md:63-65 Eq. 4, :151 ensemble axis, :153 forces by gradient).
+// This is mlp_precision = GMNN_MLP_FP32: the reference-precision path (fp32 tolerance of
+// north_star).  The tcgen05 tensor-core variants live in mlp_tc.cu.
+//
+// Forward, layer l (weights W[l] : [dims[l]][dims[l+1]]):
+//     z = X W[l] + b[l];  H[l] = swish(z);  D[l] = swish'(z)          (both stored: D feeds the backward)
+// Heads:  y_m = H_last . W_last[:, m] + b_last[m];  E_i^(m) = sigma_Z y_m + mu_Z
+// Backward of E_c = sum_m c_m E^(m), WITHOUT the per-atom factor sigma_Z (applied later, the
+// chain is linear in it):  v = W_last c;  dZ_last = D_last * v  is folded into the weights,
+//     dH = D_last (diag(v) W^T),  dZ = dH * D[l-1], ...,  dG = dZ_1 W[0]^T.
+//
+// GEMM kernel: 128x128x8 tiles, 256 threads, 8x8 outputs per thread, double-buffered shared
+// memory with register prefetch, A tile stored transposed so both operands are read as float4.
+#include "gmnn_internal.h"
+
+namespace gmnn {
+
+enum { EPI_PLAIN = 0, EPI_HIDDEN = 1, EPI_MUL = 2 };
+
+__device__ __forceinline__ void swish_pair(float z, float &h, float &d) {
+    const float s = 1.f / (1.f + __expf(-z));
+    h = z * s;
+    d = s * (1.f + z * (1.f - s));
+}
+
+constexpr int BM = 128, BN = 128, BK = 8, APITCH = 132;
+
+template <int EPI>
+__global__ void __launch_bounds__(256)
+k_sgemm(int M, int N, int K, const float *__restrict__ A, int lda, const float *__restrict__ B, int ldb,
+        float *__restrict__ C, int ldc, const float *__restrict__ bias, float *__restrict__ C2,
+        const float *__restrict__ Dmul) {
+    __shared__ __align__(16) float As[2][BK][APITCH];
+    __shared__ __align__(16) float Bs[2][BK][BN];
+    const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
+    const int m0 = blockIdx.y * BM, n0 = blockIdx.x * BN;
+    const int ar = tid >> 1, ak = (tid & 1) * 4;   // A tile: row, k offset of this thread's float4
+    const int bk = tid >> 5, bc = (tid & 31) * 4;  // B tile: k row, column of this thread's float4
+    const bool a_ok = (m0 + ar) < M, b_ok = (n0 + bc) < N;
+    const float *Ap = A + (int64_t)(m0 + ar) * lda + ak;
+    const float *Bp = B + (int64_t)bk * ldb + n0 + bc;
+    float acc[8][8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i)
+#pragma unroll
+        for (int j = 0; j < 8; ++j) acc[i][j] = 0.f;
+
+    const int nk = K / BK;
+    float4 ra = a_ok ? __ldg(reinterpret_cast<const float4 *>(Ap)) : make_float4(0.f, 0.f, 0.f, 0.f);
+    float4 rb = b_ok ? __ldg(reinterpret_cast<const float4 *>(Bp)) : make_float4(0.f, 0.f, 0.f, 0.f);
+    As[0][ak + 0][ar] = ra.x; As[0][ak + 1][ar] = ra.y; As[0][ak + 2][ar] = ra.z; As[0][ak + 3][ar] = ra.w;
+    *reinterpret_cast<float4 *>(&Bs[0][bk][bc]) = rb;
+    __syncthreads();
+    int cur = 0;
+    for (int kt = 0; kt < nk; ++kt) {
+        if (kt + 1 < nk) {
+            ra = a_ok ? __ldg(reinterpret_cast<const float4 *>(Ap + (int64_t)(kt + 1) * BK)) : make_float4(0.f, 0.f, 0.f, 0.f);
+            rb = b_ok ? __ldg(reinterpret_cast<const float4 *>(Bp + (int64_t)(kt + 1) * BK * ldb)) : make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+#pragma unroll
+        for (int kk = 0; kk < BK; ++kk) {
+            const float4 a0 = *reinterpret_cast<const float4 *>(&As[cur][kk][ty * 4]);
+            const float4 a1 = *reinterpret_cast<const float4 *>(&As[cur][kk][64 + ty * 4]);
+            const float4 b0 = *reinterpret_cast<const float4 *>(&Bs[cur][kk][tx * 4]);
+            const float4 b1 = *reinterpret_cast<const float4 *>(&Bs[cur][kk][64 + tx * 4]);
+            const float av[8] = {a0.x, a0.y, a0.z, a0.w, a1.x, a1.y, a1.z, a1.w};
+            const float bv[8] = {b0.x, b0.y, b0.z, b0.w, b1.x, b1.y, b1.z, b1.w};
+#pragma unroll
+            for (int i = 0; i < 8; ++i)
+#pragma unroll
+                for (int j = 0; j < 8; ++j) acc[i][j] = fmaf(av[i], bv[j], acc[i][j]);
+        }
+        if (kt + 1 < nk) {
+            const int nx = cur ^ 1;
+            As[nx][ak + 0][ar] = ra.x; As[nx][ak + 1][ar] = ra.y; As[nx][ak + 2][ar] = ra.z; As[nx][ak + 3][ar] = ra.w;
+            *reinterpret_cast<float4 *>(&Bs[nx][bk][bc]) = rb;
+        }
+        __syncthreads();
+        cur ^= 1;
+    }
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        const int row = m0 + (i < 4 ? ty * 4 + i : 64 + ty * 4 + (i - 4));
+        if (row >= M) continue;
+#pragma unroll
+        for (int jh = 0; jh < 2; ++jh) {
+            const int col = n0 + jh * 64 + tx * 4;
+            if (col >= N) continue;
+            float4 v = make_float4(acc[i][jh * 4 + 0], acc[i][jh * 4 + 1], acc[i][jh * 4 + 2], acc[i][jh * 4 + 3]);
+            const int64_t o = (int64_t)row * ldc + col;
+            if (EPI == EPI_HIDDEN) {
+                const float4 bb = __ldg(reinterpret_cast<const float4 *>(bias + col));
+                float4 h, d;
+                swish_pair(v.x + bb.x, h.x, d.x);
+                swish_pair(v.y + bb.y, h.y, d.y);
+                swish_pair(v.z + bb.z, h.z, d.z);
+                swish_pair(v.w + bb.w, h.w, d.w);
+                *reinterpret_cast<float4 *>(C + o) = h;
+                *reinterpret_cast<float4 *>(C2 + o) = d;
+            } else if (EPI == EPI_MUL) {
+                const float4 dm = __ldg(reinterpret_cast<const float4 *>(Dmul + o));
+                v.x *= dm.x; v.y *= dm.y; v.z *= dm.z; v.w *= dm.w;
+                *reinterpret_cast<float4 *>(C + o) = v;
+            } else {
+                *reinterpret_cast<float4 *>(C + o) = v;
+            }
+        }
+    }
+}
+
+static int sgemm(int epi, int64_t M, int N, int K, const float *A, const float *B, float *C, const float *bias,
+                 float *C2, const float *Dmul, cudaStream_t st) {
+    if (K % BK != 0 || N % 4 != 0) {
+        set_error("MLP widths must be multiples of 8 (K = %d) and 4 (N = %d)", K, N);
+        return GMNN_UNSUPPORTED;
+    }
+    dim3 grid((N + BN - 1) / BN, (unsigned)((M + BM - 1) / BM));
+    switch (epi) {
+        case EPI_PLAIN: k_sgemm<EPI_PLAIN><<<grid, 256, 0, st>>>((int)M, N, K, A, K, B, N, C, N, bias, C2, Dmul); break;
+        case EPI_HIDDEN: k_sgemm<EPI_HIDDEN><<<grid, 256, 0, st>>>((int)M, N, K, A, K, B, N, C, N, bias, C2, Dmul); break;
+        default: k_sgemm<EPI_MUL><<<grid, 256, 0, st>>>((int)M, N, K, A, K, B, N, C, N, bias, C2, Dmul); break;
+    }
+    GMNN_LAUNCHED();
+    GMNN_CUDA(cudaGetLastError());
+    return GMNN_OK;
+}
+
+// One warp per atom: y_m = h . W_last[:, m] + b_last[m]; E^(m) = sigma y_m + mu; e_atom = sum_m c_m E^(m).
+__global__ void __launch_bounds__(256)
+k_heads(int64_t N, const float *__restrict__ H, int Hd, const float *__restrict__ Wl, const float *__restrict__ bl,
+        int M, const float4 *__restrict__ pos4, const float *__restrict__ scale, const float *__restrict__ shift,
+        const float *__restrict__ head_w, float *__restrict__ e_heads, float *__restrict__ e_atom) {
+    const int lane = threadIdx.x & 31;
+    const int64_t i = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
+    if (i >= N) return;
+    float h[32];
+#pragma unroll
+    for (int q = 0; q < 32; ++q) {
+        const int k = lane + 32 * q;
+        h[q] = k < Hd ? __ldg(&H[i * (int64_t)Hd + k]) : 0.f;
+    }
+    const int z = __float_as_int(pos4[i].w);
+    const float sg = __ldg(&scale[z]), mu = __ldg(&shift[z]);
+    float e = 0.f;
+    for (int m = 0; m < M; ++m) {
+        float p = 0.f;
+#pragma unroll
+        for (int q = 0; q < 32; ++q) {
+            const int k = lane + 32 * q;
+            if (k < Hd) p = fmaf(h[q], __ldg(&Wl[(int64_t)k * M + m]), p);
+        }
+#pragma unroll
+        for (int o = 16; o >= 1; o >>= 1) p += __shfl_xor_sync(0xffffffffu, p, o);
+        const float em = sg * (p + __ldg(&bl[m])) + mu;
+        if (lane == 0) e_heads[i * (int64_t)M + m] = em;
+        e = fmaf(__ldg(&head_w[m]), em, e);
+    }
+    if (lane == 0) e_atom[i] = e;
+}
+
+// v[k] = sum_m c_m W_last[k][m]
+__global__ void k_head_vec(int Hd, int M, const float *__restrict__ Wl, const float *__restrict__ c, float *v) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= Hd) return;
+    float a = 0.f;
+    for (int m = 0; m < M; ++m) a = fmaf(__ldg(&c[m]), __ldg(&Wl[(int64_t)k * M + m]), a);
+    v[k] = a;
+}
+
+// Bv[k][n] = v[k] WT[k][n]
+__global__ void k_scale_rows(int rows, int cols, const float *__restrict__ WT, const float *__restrict__ v, float *Bv) {
+    const int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (t >= (int64_t)rows * cols) return;
+    Bv[t] = __ldg(&v[t / cols]) * __ldg(&WT[t]);
+}
+
+int launch_mlp_forward_simt(gmnn_system *s, cudaStream_t st) {
+    const gmnn_model *m = s->model;
+    const float *X = s->G;
+    for (int l = 0; l < m->hp.n_hidden; ++l) {
+        int rc = sgemm(EPI_HIDDEN, s->N, m->dims[l + 1], m->dims[l], X, m->W[l], s->H[l], m->b[l], s->D[l], nullptr, st);
+        if (rc) return rc;
+        X = s->H[l];
+    }
+    return GMNN_OK;
+}
+
+int launch_mlp_heads(gmnn_system *s, const float *head_w_dev, cudaStream_t st) {
+    const gmnn_model *m = s->model;
+    const int L = m->hp.n_hidden;
+    if (m->dims[L] > 1024) {
+        set_error("last hidden width > 1024");
+        return GMNN_UNSUPPORTED;
+    }
+    k_heads<<<(unsigned)((s->N * 32 + 255) / 256), 256, 0, st>>>(s->N, s->H[L - 1], m->dims[L], m->W[L], m->b[L],
+                                                                 m->dims[L + 1], s->pos4, m->scale, m->shift, head_w_dev,
+                                                                 s->e_heads, s->e_atom);
+    GMNN_LAUNCHED();
+    GMNN_CUDA(cudaGetLastError());
+    return GMNN_OK;
+}
+
+// Seeds the backward for the head weights c (device [n_heads]): vhead = W_last c, Bv = diag(vhead) W^T.
+int launch_mlp_seed(gmnn_system *s, const float *head_w_dev, cudaStream_t st) {
+    const gmnn_model *m = s->model;
+    const int L = m->hp.n_hidden;
+    const int Hd = m->dims[L], prev = m->dims[L - 1];
+    k_head_vec<<<(Hd + 127) / 128, 128, 0, st>>>(Hd, m->dims[L + 1], m->W[L], head_w_dev, s->vhead);
+    GMNN_LAUNCHED();
+    k_scale_rows<<<(unsigned)(((int64_t)Hd * prev + 255) / 256), 256, 0, st>>>(Hd, prev, m->WT[L - 1], s->vhead, s->Bv);
+    GMNN_LAUNCHED();
+    GMNN_CUDA(cudaGetLastError());
+    return GMNN_OK;
+}
+
+int launch_mlp_backward_simt(gmnn_system *s, const float *head_w_dev, cudaStream_t st) {
+    const gmnn_model *m = s->model;
+    const int L = m->hp.n_hidden;
+    int rc = launch_mlp_seed(s, head_w_dev, st);
+    if (rc) return rc;
+    const float *Aop = s->D[L - 1];
+    const float *Bop = s->Bv;
+    int cur = 0;
+    for (int l = L - 1; l >= 0; --l) {
+        // out[N][dims[l]] = Aop[N][dims[l+1]] . Bop[dims[l+1]][dims[l]]
+        if (l > 0) {
+            rc = sgemm(EPI_MUL, s->N, m->dims[l], m->dims[l + 1], Aop, Bop, s->dZ[cur], nullptr, nullptr, s->D[l - 1], st);
+            if (rc) return rc;
+            Aop = s->dZ[cur];
+            Bop = m->WT[l - 1];
+            cur ^= 1;
+        } else {
+            rc = sgemm(EPI_PLAIN, s->N, m->dims[0], m->dims[1], Aop, Bop, s->dG, nullptr, nullptr, nullptr, st);
+            if (rc) return rc;
+        }
+    }
+    return GMNN_OK;
+}
+
+}  // namespace gmnn

@@ -1,0 +1,299 @@
+// neighbor.cu -- cell binning, deterministic cell sort and Verlet-list build (SURVEY.md 8(a) rows
+// a1-a3; PAPER.md:169-171 neighbour list with skin, :171 several images in small cells, :381).
+//
+// Data layout.  Atoms are renumbered into cell order ("internal" order, perm[k] = caller index of
+// internal atom k; inside a cell atoms are ordered by caller index, so the order is a pure
+// function of the positions).  pos4[k] = (x, y, z, species bits): one 16-byte gather per
+// neighbour in every later kernel.  The list is row-major nbr[k][cap] of packed entries
+//   entry = j | (nx+4) << 22 | (ny+4) << 25 | (nz+4) << 28,   j internal, n the image vector,
+// so a group of lanes reads a contiguous run of one atom's row with 16-byte loads.
+//
+// Membership predicate (reading R20), unfused fp32, identical to the oracle's:
+//   s_a = fl(n_a L_a); d_a = fl(fl(x_j,a - x_i,a) + s_a); r2 = fl(fl(dx dx + dy dy) + dz dz) < fl(r_list^2)
+//
+// Every kernel of the rebuild takes (cond, thr2): inside gmnn_md_verlet_steps the rebuild is
+// launched every step and exits immediately unless the squared max displacement stored in *cond
+// exceeds thr2 -- the loop never synchronises with the host.
+#include "gmnn_internal.h"
+
+namespace gmnn {
+
+__device__ __forceinline__ bool skip_rebuild(const int32_t *cond, float thr2) {
+    return cond != nullptr && __int_as_float(*((const volatile int32_t *)cond)) <= thr2;
+}
+
+__global__ void k_wrap(int64_t N, float *x, Geometry g, const int32_t *cond, float thr2) {
+    if (skip_rebuild(cond, thr2)) return;
+    int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (t >= 3 * N) return;
+    int a = (int)(t % 3);
+    if (!g.pbc[a]) return;
+    float v = x[t];
+    v -= g.L[a] * floorf(v * g.invL[a]);
+    if (!(v >= 0.f) || v >= g.L[a]) v = 0.f;
+    x[t] = v;
+}
+
+__global__ void k_zero_cells(int64_t ncells, int32_t *cell_count, int32_t *cell_fill, const int32_t *cond, float thr2) {
+    if (skip_rebuild(cond, thr2)) return;
+    int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (t <= ncells) cell_count[t] = 0;
+    if (t < ncells) cell_fill[t] = 0;
+}
+
+__device__ __forceinline__ int cell_coord(float x, float inv_edge, int nc) {
+    int c = (int)floorf(x * inv_edge);
+    return c < 0 ? 0 : (c >= nc ? nc - 1 : c);
+}
+
+__global__ void k_cell_assign(int64_t N, const float *__restrict__ x, Geometry g, int32_t *cell_of,
+                              int32_t *cell_count, int32_t *flags, const int32_t *cond, float thr2) {
+    if (skip_rebuild(cond, thr2)) return;
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    float p[3] = {x[3 * i], x[3 * i + 1], x[3 * i + 2]};
+    int c[3];
+    bool bad = false;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        bad |= !(p[a] >= 0.f && p[a] < g.L[a]);
+        c[a] = cell_coord(p[a], g.inv_edge[a], g.ncell[a]);
+    }
+    if (bad) flags[FLAG_OUT_OF_BOX] = 1;
+    int cid = (c[2] * g.ncell[1] + c[1]) * g.ncell[0] + c[0];
+    cell_of[i] = cid;
+    atomicAdd(&cell_count[cid], 1);
+}
+
+// Exclusive scan of cell_count[0..n) into cell_start[0..n]; one block of 1024 threads.
+__global__ void k_scan_cells(int64_t n, const int32_t *__restrict__ cnt, int32_t *start, const int32_t *cond,
+                             float thr2) {
+    if (skip_rebuild(cond, thr2)) return;
+    __shared__ int32_t warp_sums[32];
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const int64_t per = (n + blockDim.x - 1) / blockDim.x;
+    const int64_t b = tid * per, e = (b + per < n) ? b + per : n;
+    int32_t local = 0;
+    for (int64_t q = b; q < e; ++q) local += cnt[q];
+    int32_t incl = local;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        int32_t v = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += v;
+    }
+    if (lane == 31) warp_sums[wid] = incl;
+    __syncthreads();
+    if (wid == 0) {
+        int32_t w = warp_sums[lane];
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            int32_t v = __shfl_up_sync(0xffffffffu, w, o);
+            if (lane >= o) w += v;
+        }
+        warp_sums[lane] = w;
+    }
+    __syncthreads();
+    int32_t run = incl - local + (wid > 0 ? warp_sums[wid - 1] : 0);
+    for (int64_t q = b; q < e; ++q) {
+        start[q] = run;
+        run += cnt[q];
+    }
+    if (tid == blockDim.x - 1) start[n] = warp_sums[31];
+}
+
+__global__ void k_cell_fill(int64_t N, const int32_t *__restrict__ cell_of, const int32_t *__restrict__ cell_start,
+                            int32_t *cell_fill, int32_t *slot_tmp, const int32_t *cond, float thr2) {
+    if (skip_rebuild(cond, thr2)) return;
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    int c = cell_of[i];
+    int slot = atomicAdd(&cell_fill[c], 1);
+    slot_tmp[cell_start[c] + slot] = (int32_t)i;
+}
+
+// The atomics above fill a cell in arbitrary order; rank every atom inside its cell by caller
+// index so that the internal numbering (and with it every summation order) is reproducible.
+__global__ void k_cell_rank(int64_t N, const int32_t *__restrict__ slot_tmp, const int32_t *__restrict__ cell_of,
+                            const int32_t *__restrict__ cell_start, int32_t *perm, const int32_t *cond, float thr2) {
+    if (skip_rebuild(cond, thr2)) return;
+    int64_t k = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (k >= N) return;
+    int i = slot_tmp[k];
+    int c = cell_of[i];
+    int b = cell_start[c], e = cell_start[c + 1];
+    int rank = 0;
+    for (int q = b; q < e; ++q) rank += (slot_tmp[q] < i);
+    perm[b + rank] = i;
+}
+
+// pos4 (internal order) from the caller's positions; at a build also the reference copy xref;
+// otherwise the skin test of gmnn_energy_forces (GMNN_STALE_NEIGHBORS).
+__global__ void k_gather(int64_t N, const float *__restrict__ x, const int32_t *__restrict__ species,
+                         const int32_t *__restrict__ perm, float4 *pos4, float *xref, bool is_build,
+                         float half_skin2, int32_t *flags, const int32_t *cond, float thr2) {
+    if (is_build && skip_rebuild(cond, thr2)) return;
+    int64_t k = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (k >= N) return;
+    int i = perm[k];
+    float px = x[3 * (int64_t)i], py = x[3 * (int64_t)i + 1], pz = x[3 * (int64_t)i + 2];
+    pos4[k] = make_float4(px, py, pz, __int_as_float(species[i]));
+    if (is_build) {
+        xref[3 * (int64_t)i] = px;
+        xref[3 * (int64_t)i + 1] = py;
+        xref[3 * (int64_t)i + 2] = pz;
+    } else if (flags != nullptr) {
+        float dx = px - xref[3 * (int64_t)i], dy = py - xref[3 * (int64_t)i + 1], dz = pz - xref[3 * (int64_t)i + 2];
+        if (dx * dx + dy * dy + dz * dz > half_skin2) flags[FLAG_STALE] = 1;
+    }
+}
+
+__device__ __forceinline__ bool in_list(const float4 &xi, const float4 &xj, float sx, float sy, float sz, float rl2) {
+    float dx = __fadd_rn(__fsub_rn(xj.x, xi.x), sx);
+    float dy = __fadd_rn(__fsub_rn(xj.y, xi.y), sy);
+    float dz = __fadd_rn(__fsub_rn(xj.z, xi.z), sz);
+    float r2 = __fadd_rn(__fadd_rn(__fmul_rn(dx, dx), __fmul_rn(dy, dy)), __fmul_rn(dz, dz));
+    return r2 < rl2;
+}
+
+__device__ __forceinline__ uint32_t image_code(int nx, int ny, int nz) {
+    return ((uint32_t)(nx + 4) << NBR_J_BITS) | ((uint32_t)(ny + 4) << (NBR_J_BITS + 3)) |
+           ((uint32_t)(nz + 4) << (NBR_J_BITS + 6));
+}
+
+// One warp per centre atom; lanes test 32 candidates of a neighbouring cell at a time and append
+// the hits in candidate order (ballot + prefix popcount): the list order is deterministic.
+__global__ void __launch_bounds__(256)
+k_build_cells(int64_t N, const float4 *__restrict__ pos4, const int32_t *__restrict__ cell_start, Geometry g,
+              uint32_t *nbr, int32_t *count, int cap, int32_t *flags, const int32_t *cond, float thr2) {
+    if (skip_rebuild(cond, thr2)) return;
+    const int lane = threadIdx.x & 31;
+    const int64_t i = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
+    if (i >= N) return;
+    const float4 xi = pos4[i];
+    const int cx = cell_coord(xi.x, g.inv_edge[0], g.ncell[0]);
+    const int cy = cell_coord(xi.y, g.inv_edge[1], g.ncell[1]);
+    const int cz = cell_coord(xi.z, g.inv_edge[2], g.ncell[2]);
+    uint32_t *row = nbr + i * (int64_t)cap;
+    int n = 0;
+    for (int oz = -1; oz <= 1; ++oz) {
+        int z = cz + oz, nz = 0;
+        if (z < 0) { if (!g.pbc[2]) continue; z += g.ncell[2]; nz = -1; }
+        else if (z >= g.ncell[2]) { if (!g.pbc[2]) continue; z -= g.ncell[2]; nz = 1; }
+        for (int oy = -1; oy <= 1; ++oy) {
+            int y = cy + oy, ny = 0;
+            if (y < 0) { if (!g.pbc[1]) continue; y += g.ncell[1]; ny = -1; }
+            else if (y >= g.ncell[1]) { if (!g.pbc[1]) continue; y -= g.ncell[1]; ny = 1; }
+            for (int ox = -1; ox <= 1; ++ox) {
+                int x = cx + ox, nx = 0;
+                if (x < 0) { if (!g.pbc[0]) continue; x += g.ncell[0]; nx = -1; }
+                else if (x >= g.ncell[0]) { if (!g.pbc[0]) continue; x -= g.ncell[0]; nx = 1; }
+                const int c = (z * g.ncell[1] + y) * g.ncell[0] + x;
+                const int b = cell_start[c], e = cell_start[c + 1];
+                const float sx = __fmul_rn((float)nx, g.L[0]), sy = __fmul_rn((float)ny, g.L[1]),
+                            sz = __fmul_rn((float)nz, g.L[2]);
+                const uint32_t code = image_code(nx, ny, nz);
+                const bool home = (nx | ny | nz) == 0;
+                for (int base = b; base < e; base += 32) {
+                    const int j = base + lane;
+                    bool keep = false;
+                    if (j < e && !(home && j == (int)i)) keep = in_list(xi, pos4[j], sx, sy, sz, g.r_list2);
+                    const unsigned m = __ballot_sync(0xffffffffu, keep);
+                    const int p = n + __popc(m & ((1u << lane) - 1u));
+                    if (keep && p < cap) row[p] = (uint32_t)j | code;
+                    n += __popc(m);
+                }
+            }
+        }
+    }
+    if (lane == 0) {
+        count[i] = n < cap ? n : cap;
+        if (n > cap) atomicMax(&flags[FLAG_MAXCOUNT], n);
+    }
+}
+
+// Boxes with fewer than 3 cells on a periodic axis: explicit loop over all atoms and all images
+// n in [-k..k]^3 (minimum image is not enough there).  O(N^2 images), N <= 16384.
+__global__ void __launch_bounds__(256)
+k_build_small(int64_t N, const float4 *__restrict__ pos4, Geometry g, uint32_t *nbr, int32_t *count, int cap,
+              int32_t *flags, const int32_t *cond, float thr2) {
+    if (skip_rebuild(cond, thr2)) return;
+    const int lane = threadIdx.x & 31;
+    const int64_t i = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
+    if (i >= N) return;
+    const float4 xi = pos4[i];
+    uint32_t *row = nbr + i * (int64_t)cap;
+    int n = 0;
+    for (int nz = -g.kimg[2]; nz <= g.kimg[2]; ++nz)
+        for (int ny = -g.kimg[1]; ny <= g.kimg[1]; ++ny)
+            for (int nx = -g.kimg[0]; nx <= g.kimg[0]; ++nx) {
+                const float sx = __fmul_rn((float)nx, g.L[0]), sy = __fmul_rn((float)ny, g.L[1]),
+                            sz = __fmul_rn((float)nz, g.L[2]);
+                const uint32_t code = image_code(nx, ny, nz);
+                const bool home = (nx | ny | nz) == 0;
+                for (int base = 0; base < (int)N; base += 32) {
+                    const int j = base + lane;
+                    bool keep = false;
+                    if (j < (int)N && !(home && j == (int)i)) keep = in_list(xi, pos4[j], sx, sy, sz, g.r_list2);
+                    const unsigned m = __ballot_sync(0xffffffffu, keep);
+                    const int p = n + __popc(m & ((1u << lane) - 1u));
+                    if (keep && p < cap) row[p] = (uint32_t)j | code;
+                    n += __popc(m);
+                }
+            }
+    if (lane == 0) {
+        count[i] = n < cap ? n : cap;
+        if (n > cap) atomicMax(&flags[FLAG_MAXCOUNT], n);
+    }
+}
+
+__global__ void k_finish_rebuild(int32_t *flags, const int32_t *cond, float thr2) {
+    if (skip_rebuild(cond, thr2)) return;
+    flags[FLAG_DISP2] = 0;
+    flags[FLAG_REBUILDS] += 1;
+}
+
+static inline unsigned nblocks(int64_t n, int per) { return (unsigned)((n + per - 1) / per); }
+
+int launch_build(gmnn_system *s, const float *positions, cudaStream_t st, const int32_t *cond, float thr2,
+                 bool wrap_first, float *positions_mut) {
+    const int64_t N = s->N;
+    const Geometry g = s->geo;
+    if (wrap_first && positions_mut) {
+        k_wrap<<<nblocks(3 * N, 256), 256, 0, st>>>(N, positions_mut, g, cond, thr2);
+        GMNN_LAUNCHED();
+    }
+    k_zero_cells<<<nblocks(s->ncells + 1, 256), 256, 0, st>>>(s->ncells, s->cell_count, s->cell_fill, cond, thr2);
+    GMNN_LAUNCHED();
+    k_cell_assign<<<nblocks(N, 256), 256, 0, st>>>(N, positions, g, s->cell_of, s->cell_count, s->flags, cond, thr2);
+    GMNN_LAUNCHED();
+    k_scan_cells<<<1, 1024, 0, st>>>(s->ncells, s->cell_count, s->cell_start, cond, thr2);
+    GMNN_LAUNCHED();
+    k_cell_fill<<<nblocks(N, 256), 256, 0, st>>>(N, s->cell_of, s->cell_start, s->cell_fill, s->slot_tmp, cond, thr2);
+    GMNN_LAUNCHED();
+    k_cell_rank<<<nblocks(N, 256), 256, 0, st>>>(N, s->slot_tmp, s->cell_of, s->cell_start, s->perm, cond, thr2);
+    GMNN_LAUNCHED();
+    k_gather<<<nblocks(N, 256), 256, 0, st>>>(N, positions, s->species, s->perm, s->pos4, s->xref, true, 0.f,
+                                              nullptr, cond, thr2);
+    GMNN_LAUNCHED();
+    if (s->small_box)
+        k_build_small<<<nblocks(N * 32, 256), 256, 0, st>>>(N, s->pos4, g, s->nbr, s->count, s->cap, s->flags, cond, thr2);
+    else
+        k_build_cells<<<nblocks(N * 32, 256), 256, 0, st>>>(N, s->pos4, s->cell_start, g, s->nbr, s->count, s->cap,
+                                                            s->flags, cond, thr2);
+    GMNN_LAUNCHED();
+    k_finish_rebuild<<<1, 1, 0, st>>>(s->flags, cond, thr2);
+    GMNN_LAUNCHED();
+    GMNN_CUDA(cudaGetLastError());
+    return GMNN_OK;
+}
+
+int launch_gather_positions(gmnn_system *s, const float *positions, cudaStream_t st, bool check_stale) {
+    const float hs = 0.5f * s->skin;
+    k_gather<<<nblocks(s->N, 256), 256, 0, st>>>(s->N, positions, s->species, s->perm, s->pos4, s->xref, false,
+                                                 hs * hs, check_stale ? s->flags : nullptr, nullptr, 0.f);
+    GMNN_LAUNCHED();
+    GMNN_CUDA(cudaGetLastError());
+    return GMNN_OK;
+}
+
+}  // namespace gmnn

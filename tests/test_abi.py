@@ -1,0 +1,79 @@
+"""The C-ABI library loads on a CPU-only box and exports every symbol include/gmnn.h declares.
+No compute call is made here (there is no GPU and no CPU fallback)."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def gm():
+    from paper_2505_22168_b200 import build
+
+    build.build()
+    import paper_2505_22168_b200 as pkg
+
+    return pkg
+
+
+def _declared_symbols():
+    text = open(os.path.join(ROOT, "include", "gmnn.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(gmnn_[a-z_0-9]+)\s*\(", text)))
+
+
+def test_header_symbols_are_exported(gm):
+    declared = _declared_symbols()
+    assert len(declared) >= 18
+    lib = ctypes.CDLL(gm.LIB_PATH)
+    for name in declared:
+        assert hasattr(lib, name), name
+    assert sorted(gm.EXPORTS) == declared
+
+
+def test_feature_count_and_error_string(gm):
+    assert gm.n_features(5) == 360 and gm.n_features(1) == 8
+    assert isinstance(gm.binding.lib.gmnn_last_error(), bytes)
+    assert gm.launch_count() == 0
+
+
+def test_no_cpu_fallback_and_validation(gm):
+    """Argument validation runs on the host; a valid model then needs a CUDA device and must say so."""
+    import torch
+    import workloads as wl
+
+    spec = wl.tiny_box(hidden=(16, 16)).model
+    with pytest.raises(gm.GmnnError) as e:
+        gm.Model(spec, l_max=2)
+    assert e.value.code == gm.GMNN_UNSUPPORTED
+    with pytest.raises(gm.GmnnError) as e:
+        gm.Model(spec, n_weight_sets=2)
+    assert e.value.code == gm.GMNN_UNSUPPORTED
+    bad = wl.tiny_box(hidden=(20, 16)).model
+    with pytest.raises(gm.GmnnError) as e:
+        gm.Model(bad)
+    assert e.value.code == gm.GMNN_INVALID_ARG
+    if not torch.cuda.is_available():
+        with pytest.raises(gm.GmnnError) as e:
+            gm.Model(spec)
+        assert e.value.code == gm.GMNN_CUDA_ERROR and "no CPU fallback" in str(e.value)
+
+
+def test_product_never_imports_the_oracle():
+    pkg = os.path.join(ROOT, "paper_2505_22168_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                text = open(os.path.join(dirpath, f)).read()
+                assert "oracle" not in text.replace("oracle/ ", "").replace("the oracle", "").replace("oracle's", "") \
+                    or "import" not in [ln for ln in text.splitlines() if "oracle" in ln and "import" in ln] or True
+                for ln in text.splitlines():
+                    if re.search(r"^\s*(from|import)\s+oracle", ln) or "gmnn_oracle" in ln:
+                        raise AssertionError("%s references the oracle: %s" % (f, ln))
+    for f in ("gmnn_oracle.py", "gmnn_oracle.c"):
+        text = open(os.path.join(ROOT, "oracle", f)).read()
+        assert "paper_2505_22168_b200" not in text.replace("paper_2505_22168_b200/", "")
