@@ -507,10 +507,16 @@ static int pair_backward_lpa(gmnn_system *s, cudaStream_t st, int lpa) {
     const size_t smem = sizeof(float) * (beta_floats + (128 / lpa) * NR * PSI);
     const unsigned grid = nblocks(s->N * lpa, 128);
 #define GMNN_PB(L)                                                                                         \
-    case L:                                                                                                \
+    case L: {                                                                                              \
+        static size_t opted = 0;                                                                           \
+        if (smem > 48 * 1024 && smem > opted) {                                                            \
+            GMNN_CUDA(cudaFuncSetAttribute(k_pair_backward<NR, NB, L>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
+                                           (int)smem));                                                    \
+            opted = smem;                                                                                  \
+        }                                                                                                  \
         k_pair_backward<NR, NB, L><<<grid, 128, smem, st>>>(s->N, s->pos4, s->nbr, s->count, s->cap, s->geo, \
                                                             m->rp, m->beta, s->A, s->f_int);               \
-        break;
+    } break;
     switch (lpa) {
         GMNN_PB(1) GMNN_PB(2) GMNN_PB(4) GMNN_PB(8) GMNN_PB(16) GMNN_PB(32)
         default:

@@ -1,0 +1,128 @@
+"""GPU parity for the shallow ensemble (Eq. 5, 6) and the NVE loop (configs 2, 4, 5 shaped)."""
+import numpy as np
+import pytest
+
+import workloads as wl
+from parity_utils import F_TOL, energy_atom_error, force_error, r_list32
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def gm():
+    import torch
+
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device (they must not pass on a fallback)")
+    import paper_2505_22168_b200 as pkg
+
+    return pkg
+
+
+def _build(gm, w, **kw):
+    import torch
+
+    model = gm.Model(w.model, **kw)
+    sysm = gm.System(model, w.species)
+    pos = torch.from_numpy(w.positions).cuda()
+    sysm.build_neighbors(pos, w.cell9, w.pbc, w.model.r_cut, w.skin)
+    return model, sysm, pos
+
+
+@pytest.mark.parametrize("name", ["tiny8", "config4_1024"])
+def test_ensemble_statistics(gm, orc, name):
+    w = wl.tiny_box(n_heads=8) if name == "tiny8" else wl.li3po4_box(1024, n_heads=32)
+    m = orc.Model(w.model)
+    pairs = orc.auto_neighbors(w.positions, w.cell, w.pbc, r_list32(w.model.r_cut, w.skin))
+    ref = orc.ensemble(m, w.positions, w.species, w.cell, pairs)
+    _, sysm, pos = _build(gm, w)
+    e_mean, e_var, f_mean, f_var = (t.cpu().numpy().astype(np.float64) for t in sysm.ensemble_energy_forces(pos))
+    assert energy_atom_error(e_mean, ref.e_mean) <= 1.0
+    assert force_error(f_mean, ref.f_mean) <= F_TOL
+    # variances: second moments of quantities that each carry ~1e-5 relative error
+    assert np.abs(e_var - ref.e_var).max() <= 2e-4 * max(ref.e_var.max(), 1e-30)
+    assert np.abs(f_var - ref.f_var).max() <= 2e-4 * ref.f_var.max()
+    assert np.all(e_var >= 0) and np.all(f_var >= 0)
+    # Eq. 6 on the GPU itself: the cheap mode (gradient of the mean energy) equals the mean of the heads
+    _, ea, f = sysm.energy_forces(pos)
+    assert force_error(f.cpu().numpy().astype(np.float64), f_mean) <= 2e-5
+    assert energy_atom_error(ea.cpu().numpy().astype(np.float64), e_mean) <= 1.0
+
+
+def test_config4_full_size_sampled(gm, orc):
+    """Config 4 at its full size (8192 atoms, 32 heads): means against the oracle everywhere,
+    per-head statistics on a sample of heads via Eq. 6 linearity."""
+    w = wl.make_workload("config4")
+    m = orc.Model(w.model)
+    pairs = orc.auto_neighbors(w.positions, w.cell, w.pbc, r_list32(w.model.r_cut, w.skin))
+    mean_ref = orc.energy_forces(m, w.positions, w.species, w.cell, pairs)  # gradient of the mean energy
+    _, sysm, pos = _build(gm, w)
+    e_mean, e_var, f_mean, f_var = (t.cpu().numpy().astype(np.float64) for t in sysm.ensemble_energy_forces(pos))
+    assert energy_atom_error(e_mean, mean_ref.e_heads.mean(1)) <= 1.0
+    assert force_error(f_mean, mean_ref.forces) <= F_TOL
+    assert np.abs(e_var - mean_ref.e_heads.var(1)).max() <= 2e-4 * mean_ref.e_heads.var(1).max()
+    assert np.all(f_var >= 0) and f_var.max() > 0
+
+
+def test_md_trajectory_and_energy_conservation(gm, orc):
+    """Config-2-shaped NVE: trajectory parity for the first 10 steps (|dx| <= 1e-4 Ang), then state
+    parity (oracle E, F at the GPU's own final positions), drift within 10x of the fp64 oracle's."""
+    import torch
+
+    w = wl.ionic_liquid_box(n_pairs=16, hidden=(64, 64))  # 384 atoms, L = 15.9 Ang: image path (2 cells)
+    m = orc.Model(w.model)
+    _, sysm, pos = _build(gm, w)
+    vel = torch.from_numpy(w.velocities).cuda()
+    mass = torch.from_numpy(w.masses).cuda()
+    epot, ekin, nreb = sysm.md_verlet_steps(pos, vel, mass, w.dt_fs, 10)
+    ref = orc.nve(m, w.positions, w.velocities, w.masses, w.species, w.cell, w.pbc, w.skin, w.dt_fs, 10)
+    L = w.cell.astype(np.float64)
+    d = pos.cpu().numpy().astype(np.float64) - ref.positions
+    d -= np.round(d / L) * L
+    assert np.abs(d).max() <= 1e-4
+    assert np.abs(vel.cpu().numpy() - ref.velocities).max() <= 1e-5
+    ep, ek = epot.cpu().numpy(), ekin.cpu().numpy()
+    assert np.abs(ep - ref.epot).max() <= 1e-5 * np.abs(ref.epot).max() + 1e-4
+    assert np.abs(ek - ref.ekin).max() <= 1e-4 * np.abs(ref.ekin).max()
+    # continue for 90 more steps, then check the state against the oracle at the GPU's own positions
+    epot2, ekin2, nreb2 = sysm.md_verlet_steps(pos, vel, mass, w.dt_fs, 90)
+    x = pos.cpu().numpy()
+    xw = (x.astype(np.float64) - np.floor(x.astype(np.float64) / L) * L).astype(np.float32)
+    xw = np.where(xw >= w.cell[None, :], 0.0, xw).astype(np.float32)
+    pairs = orc.auto_neighbors(xw, w.cell, w.pbc, w.model.r_cut)
+    state = orc.energy_forces(m, xw, w.species, w.cell, pairs)
+    assert abs(float(epot2[-1]) - state.energy) <= 2e-6 * np.abs(state.e_atom).sum()
+    assert nreb + nreb2 >= 1  # hydrogens at 300 K cross skin/2 = 0.25 Ang within 100 steps
+    ref100 = orc.nve(m, w.positions, w.velocities, w.masses, w.species, w.cell, w.pbc, w.skin, w.dt_fs, 100)
+    drift_ref = np.abs(ref100.epot + ref100.ekin - (ref100.epot[0] + ref100.ekin[0])).max()
+    etot = np.concatenate([ep + ek, (epot2.cpu().numpy() + ekin2.cpu().numpy())[1:]])
+    drift_gpu = np.abs(etot - etot[0]).max()
+    assert drift_gpu <= 10 * drift_ref + 1e-3, (drift_gpu, drift_ref)
+
+
+def test_md_cell_list_rebuild_inside_the_loop(gm, orc):
+    """Config-5-shaped (Li3PO4, skin 1, cell-list rebuild when max displacement > skin/2) at 8192
+    atoms: hot velocities force several device-side rebuilds; the final state must match the oracle
+    evaluated on the GPU's final positions and the list must equal a fresh build."""
+    import torch
+
+    w = wl.li3po4_box(8192, hidden=(32, 32), skin=0.3)
+    m = orc.Model(w.model)
+    _, sysm, pos = _build(gm, w)
+    vel = torch.from_numpy(w.velocities * 8.0).cuda()
+    mass = torch.from_numpy(w.masses).cuda()
+    epot, ekin, nreb = sysm.md_verlet_steps(pos, vel, mass, w.dt_fs, 40)
+    assert nreb >= 2
+    x = pos.cpu().numpy()
+    L = w.cell.astype(np.float64)
+    xw = (x.astype(np.float64) - np.floor(x.astype(np.float64) / L) * L).astype(np.float32)
+    xw = np.where(xw >= w.cell[None, :], 0.0, xw).astype(np.float32)
+    pairs = orc.auto_neighbors(xw, w.cell, w.pbc, w.model.r_cut)
+    state = orc.energy_forces(m, xw, w.species, w.cell, pairs)
+    assert abs(float(epot[-1]) - state.energy) <= 2e-6 * np.abs(state.e_atom).sum()
+    # energy+forces on the returned (unwrapped-continuation) positions with the list left in the handle
+    e, ea, f = sysm.energy_forces(pos)
+    sysm.check()
+    assert force_error(f.cpu().numpy().astype(np.float64), state.forces) <= F_TOL
+    etot = (epot + ekin).cpu().numpy()
+    assert np.abs(etot - etot[0]).max() <= 2e-3 * np.abs(ekin.cpu().numpy()).max()
