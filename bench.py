@@ -1,0 +1,405 @@
+#!/usr/bin/env python
+"""bench.py -- atom-steps/s of the GMNN energy+force hot path on B200 (BASELINE.json `metric`).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload config5] [--mlp 3xtf32]
+    python bench.py --impl reference ...          # the fp64 CPU oracle on the host cores
+
+One "step" is one NVE velocity-Verlet step of the workload through gmnn_md_verlet_steps: kick,
+drift, skin test, neighbour rebuild when an atom moved more than skin/2, gather, pair forward,
+contraction, MLP forward + backward, contraction backward, pair backward with the force reduction,
+kick -- every row of SURVEY.md section 8(a) except the ensemble statistics (config 4, a parity
+case).  `value` = atoms x steps / device time (CUDA events on the launching stream, inputs resident
+in HBM).  `e2e` = the same metric through gmnn_energy_forces_host: every step copies the positions
+from pinned host memory, evaluates energy and forces and copies forces and energy back.
+N > 1 (torchrun): the path does not shard (replicas only) -- every rank runs an
+independent replica on its own GPU, no data-path collective; `value` sums the replicas over the
+slowest rank's time.
+
+Only the `cpu_baseline` leg and `--impl reference` execute oracle/ (test infrastructure).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "atom-steps/s (GMNN energy+forces)"
+UNIT = "atom-steps/s"
+N_FEATURES = 360
+MLP_NAMES = {"fp32": 0, "3xtf32": 1, "tf32": 2}
+FP32_LANES_PER_SM = 128  # B200_PROFILING.md / B300_MICROARCH.md: 4 SMSPs x 32 FMA lanes
+N_SMS = 148
+
+
+def load_peaks():
+    """MEASURED_PEAKS.json (driver-written) or the fallback B200_PROFILING.md states."""
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        return {"hbm_gbs": float(d["hbm_gbs"]), "bf16_burst": float(d["bf16_tflops"]),
+                "bf16_sustained": float(d.get("bf16_tflops_sustained", d["bf16_tflops"])),
+                "sm_max_mhz": float(d.get("sm_max_mhz", 1965.0)), "source": "measured"}
+    return {"hbm_gbs": 6650.0, "bf16_burst": 1590.0, "bf16_sustained": 1400.0, "sm_max_mhz": 1965.0,
+            "source": "fallback"}
+
+
+def stage_model(w, nl_mean, nc_mean, n_hidden_macs, mlp):
+    """Algorithmic HBM bytes and flops per atom of each stage, keyed by the
+    stage names gmnn_stage_times reports.  bound: which roof binds the stage by count."""
+    F = N_FEATURES
+    mlp_flops = 2.0 * n_hidden_macs  # one direction
+    tensor = mlp != "fp32"
+    return {
+        "gather": dict(bytes=36.0, flops=0.0, bound="hbm"),
+        "pair_forward": dict(bytes=4.0 * nl_mean + 420.0, flops=12.0 * nl_mean + 340.0 * nc_mean, bound="alu"),
+        "contract_forward": dict(bytes=400.0 + 4.0 * F, flops=2.0 * 5000.0, bound="hbm"),
+        "mlp_forward": dict(bytes=4.0 * F + 4.0, flops=mlp_flops, bound="tensor" if tensor else "alu"),
+        "mlp_heads": dict(bytes=2048.0 + 8.0, flops=1024.0, bound="hbm"),
+        "mlp_backward": dict(bytes=4.0 * F, flops=mlp_flops, bound="tensor" if tensor else "alu"),
+        "contract_backward": dict(bytes=4.0 * F + 800.0, flops=2.0 * 15000.0, bound="hbm"),
+        "pair_backward": dict(bytes=4.0 * nl_mean + 432.0, flops=12.0 * nl_mean + 1400.0 * nc_mean, bound="alu"),
+        "outputs": dict(bytes=48.0, flops=0.0, bound="hbm"),
+        "kick_drift": dict(bytes=76.0, flops=30.0, bound="hbm"),
+        "kick_ke": dict(bytes=56.0, flops=20.0, bound="hbm"),
+        "rebuild_if_moved": dict(bytes=0.0, flops=0.0, bound="hbm"),
+    }
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons, sampled every 200 ms while the timed region runs."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, device_index: int):
+        self.proc = None
+        self.path = "/tmp/gmnn_bench_clocks_%d.csv" % os.getpid()
+        sel = []
+        try:
+            import torch
+
+            uuid = str(torch.cuda.get_device_properties(device_index).uuid)
+            sel = ["-i", uuid if uuid.startswith("GPU-") else "GPU-" + uuid]
+        except Exception:
+            sel = ["-i", str(device_index)]
+        self.cmd = ["nvidia-smi", *sel, "--query-gpu=" + self.Q, "--format=csv,noheader,nounits", "-lms", "200"]
+
+    def start(self):
+        try:
+            self.out = open(self.path, "w")
+            self.proc = subprocess.Popen(self.cmd, stdout=self.out, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        self.out.close()
+        sm, smax, power, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        with open(self.path) as f:
+            for line in f:
+                c = [x.strip() for x in line.split(",")]
+                if len(c) < 8:
+                    continue
+                try:
+                    sm.append(float(c[0]))
+                    smax.append(float(c[1]))
+                    power.append(float(c[2]))
+                except ValueError:
+                    continue
+                for nm, v in zip(names, c[4:8]):
+                    if v.lower().startswith("active"):
+                        reasons.add(nm)
+        try:
+            os.remove(self.path)
+        except OSError:
+            pass
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        busy = [s for s, p in zip(sm, power) if p >= 0.5 * max(power)] or sm
+        return {"sm_mhz": float(np.median(busy)), "sm_max_mhz": float(max(smax)), "power_w_max": float(max(power)),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def make_bench_workload(name: str):
+    import workloads as wl
+
+    return wl.make_workload(name)
+
+
+# ------------------------------------------------------------------------------------------------
+# the oracle legs (cpu_baseline of our arm, and the whole reference arm)
+# ------------------------------------------------------------------------------------------------
+def oracle_sample_workload(workload_name: str, n_sample: int):
+    """A box of the benchmarked workload's own family (composition, density, cutoff, skin, model)
+    cut down to n_sample atoms so that the fp64 oracle finishes in seconds."""
+    import workloads as wl
+
+    if workload_name == "config2":
+        return wl.ionic_liquid_box(n_pairs=max(8, n_sample // 24))
+    if workload_name == "config1":
+        return wl.tiny_box()
+    skin = 1.0 if workload_name == "config5" else 0.0
+    cfg = 5 if workload_name == "config5" else 3
+    heads = 32 if workload_name == "config4" else 1
+    return wl.li3po4_box(n_sample, skin=skin, config=cfg, n_heads=heads)
+
+
+def oracle_prepare(w):
+    from oracle import gmnn_oracle as orc
+
+    r_list = float(np.float32(w.model.r_cut) + np.float32(w.skin))
+    pairs = orc.auto_neighbors(w.positions, w.cell, w.pbc, r_list)
+    return orc, orc.Model(w.model), pairs
+
+
+def oracle_step(orc, model, w, pairs):
+    t0 = time.perf_counter()
+    orc.energy_forces(model, w.positions, w.species, w.cell, pairs)
+    return time.perf_counter() - t0
+
+
+def cpu_baseline(workload_name: str, n_sample: int = 16384):
+    w = oracle_sample_workload(workload_name, n_sample)
+    orc, model, pairs = oracle_prepare(w)
+    dt = oracle_step(orc, model, w, pairs)
+    return {"value": w.n_atoms / dt, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle",
+            "sample": "one fp64 energy+forces evaluation (oracle/gmnn_oracle.c, OpenMP) of a %d-atom box of the "
+                      "same family as %s (same density, species ratio, r_cut, skin, model), neighbour list prebuilt; "
+                      "%.2f s" % (w.n_atoms, workload_name, dt)}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    budget_s = 150.0
+    probe = oracle_sample_workload(args.workload, 1024)
+    orc, model, pairs = oracle_prepare(probe)
+    oracle_step(orc, model, probe, pairs)
+    rate = probe.n_atoms / oracle_step(orc, model, probe, pairs)  # atom-steps/s on this host
+    n_sample = 1024
+    for cand in (2048, 4096, 8192, 16384, 32768):
+        if cand / rate * (args.steps + args.warmup) <= budget_s:
+            n_sample = cand
+    w = probe if n_sample == 1024 else oracle_sample_workload(args.workload, n_sample)
+    if w is not probe:
+        orc, model, pairs = oracle_prepare(w)
+    for _ in range(args.warmup):
+        oracle_step(orc, model, w, pairs)
+    total = 0.0
+    for _ in range(args.steps):
+        total += oracle_step(orc, model, w, pairs)
+    value = w.n_atoms * args.steps / total
+    sample = ("each step = one fp64 energy+forces evaluation (oracle, OpenMP) of a %d-atom box of the family of %s, "
+              "neighbour list prebuilt" % (w.n_atoms, args.workload))
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": args.workload, "sample_atoms": w.n_atoms},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ------------------------------------------------------------------------------------------------
+# our arm
+# ------------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    import paper_2505_22168_b200 as gm
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the GMNN path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    peaks = load_peaks()
+
+    w = make_bench_workload(args.workload)
+    N = w.n_atoms
+    mlp = MLP_NAMES[args.mlp]
+    model = gm.Model(w.model, mlp_precision=mlp)
+    sysm = gm.System(model, w.species)
+    pos0 = torch.from_numpy(w.positions).to(dev)
+    pos = pos0.clone()
+    vel = torch.from_numpy(w.velocities).to(dev)
+    masses = torch.from_numpy(w.masses).to(dev)
+    sysm.build_neighbors(pos, w.cell9, w.pbc, w.model.r_cut, w.skin)
+    counts = sysm.debug_read("count").astype(np.float64)
+    nl_mean = float(counts.mean())
+    r_list = w.model.r_cut + w.skin
+    nc_mean = nl_mean * (w.model.r_cut / r_list) ** 3
+    dims = [N_FEATURES, *w.model.hidden, w.model.n_heads]
+    hidden_macs = sum(dims[l] * dims[l + 1] for l in range(len(dims) - 1))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident MD steps -------------------------------------------------------------
+    sysm.set_int("md_continue", 1)
+    stream = torch.cuda.current_stream()
+    total_rebuilds = 0
+    if args.warmup > 0:
+        _, _, nreb = sysm.md_verlet_steps(pos, vel, masses, w.dt_fs, args.warmup, want_series=False)
+        total_rebuilds += nreb
+    sysm.set_int("profile", 1)
+    sampler = ClockSampler(local)
+    sampler.start()
+    barrier()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    launches0 = gm.launch_count()
+    ev0.record(stream)
+    epot, ekin, nreb = sysm.md_verlet_steps(pos, vel, masses, w.dt_fs, args.steps, want_series=True)
+    ev1.record(stream)
+    barrier()
+    launches = gm.launch_count() - launches0
+    clocks = sampler.stop()
+    total_rebuilds += nreb
+    ms = ev0.elapsed_time(ev1)
+    stages = sysm.stage_times()
+    sysm.set_int("profile", 0)
+    t = torch.tensor([ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_max = float(t.item())
+    value = world * N * args.steps / (ms_max * 1e-3)
+    etot = (epot + ekin).cpu().numpy()
+    drift = float(np.abs(etot - etot[0]).max() / N)
+
+    # ---- per-stage roofline (live CUDA events of the timed region) ------------------------------
+    sm = stage_model(w, nl_mean, nc_mean, hidden_macs, args.mlp)
+    sm_mhz = clocks.get("sm_mhz") or peaks["sm_max_mhz"]
+    fp32_peak_tflops = N_SMS * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
+    tf32_peak_tflops = 0.5 * peaks["bf16_sustained"]
+    stage_out = {}
+    per_step_ms = {}
+    for name, mean_ms, cnt in stages:
+        per_step = mean_ms * cnt / args.steps
+        per_step_ms[name] = per_step
+        info = sm.get(name, dict(bytes=0.0, flops=0.0, bound="hbm"))
+        sec = mean_ms * 1e-3
+        ent = {"ms": round(mean_ms, 4), "per_step_ms": round(per_step, 4), "ns_per_atom": round(mean_ms * 1e6 / N, 3),
+               "bound": info["bound"]}
+        if sec > 0 and info["bytes"] > 0:
+            ent["hbm_gbs"] = round(info["bytes"] * N / sec / 1e9, 1)
+            ent["hbm_frac"] = round(ent["hbm_gbs"] / peaks["hbm_gbs"], 4)
+        if sec > 0 and info["flops"] > 0:
+            tf = info["flops"] * N / sec / 1e12
+            ent["tflops"] = round(tf, 2)
+            ent["flop_frac"] = round(tf / (tf32_peak_tflops if info["bound"] == "tensor" else fp32_peak_tflops), 4)
+        stage_out[name] = ent
+    dom = max(per_step_ms, key=per_step_ms.get) if per_step_ms else None
+    roofline = None
+    if dom is not None:
+        info = sm.get(dom, dict(bytes=0.0, flops=0.0, bound="hbm"))
+        mean_ms = [m for n_, m, _ in stages if n_ == dom][0]
+        sec = mean_ms * 1e-3
+        if info["bound"] == "hbm":
+            ach, peak, unit = info["bytes"] * N / sec / 1e9, peaks["hbm_gbs"], "GB/s"
+        elif info["bound"] == "tensor":
+            ach, peak, unit = info["flops"] * N / sec / 1e12, tf32_peak_tflops, "TFLOP/s"
+        else:
+            ach, peak, unit = info["flops"] * N / sec / 1e12, fp32_peak_tflops, "TFLOP/s"
+        roofline = {"kernel": dom, "bound": info["bound"], "achieved": round(ach, 3), "peak": round(peak, 3),
+                    "unit": unit, "frac": round(ach / peak, 4), "traffic": None,
+                    "peak_source": {"hbm": "MEASURED_PEAKS.json hbm_gbs (%s)" % peaks["source"],
+                                    "tensor": "0.5 (nominal tf32:bf16) x bf16_tflops_sustained (%s)" % peaks["source"],
+                                    "alu": "148 SMs x 128 fp32 lanes x 2 flop x sm_max_mhz (derived, DESIGN.md 5)"}[info["bound"]],
+                    "share_of_step": round(per_step_ms[dom] / (ms_max / args.steps), 4),
+                    "algorithmic_per_atom": {"bytes": info["bytes"], "flops": info["flops"]}}
+
+    # ---- end to end through the host-buffer entry ----------------------------------------------
+    e2e_steps = max(3, min(args.steps, 10))
+    hpos = torch.from_numpy(w.positions).pin_memory()
+    hfrc = torch.empty(N, 3, dtype=torch.float32).pin_memory()
+    sysm.build_neighbors(pos0, w.cell9, w.pbc, w.model.r_cut, w.skin)
+    hp_np, hf_np = hpos.numpy(), hfrc.numpy()
+    for _ in range(2):
+        sysm.energy_forces_host(hp_np, hf_np)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        e_host = sysm.energy_forces_host(hp_np, hf_np)
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    e2e = {"value": world * N * e2e_steps / float(t.item()), "unit": UNIT, "h2d_bytes_per_step": 12 * N,
+           "d2h_bytes_per_step": 12 * N + 8, "steps": e2e_steps,
+           "what": "gmnn_energy_forces_host: pinned positions in, forces and total energy out, every step"}
+    sysm.check()
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": {"fp32": "f32", "3xtf32": "f32 (MLP: 3xTF32 split on tcgen05, fp32 accumulate)",
+                      "tf32": "tf32 MLP, f32 elsewhere"}[args.mlp],
+            "data": "synthetic",
+            "config": {"workload": args.workload, "n_atoms": N, "what": w.name + ", NVE velocity Verlet, dt %.2f fs, skin %.1f"
+                       % (w.dt_fs, w.skin), "mlp": args.mlp, "hidden": list(w.model.hidden), "n_heads": w.model.n_heads,
+                       "neighbors_in_list_mean": round(nl_mean, 2), "rebuilds_in_timed_region": nreb,
+                       "l2": "inputs_exceed_l2" if N >= 65536 else "working set of this small case is L2-resident",
+                       "replicas": world},
+            "gpu_launches": launches, "clocks": clocks, "e2e": e2e, "roofline": roofline, "stages": stage_out,
+            "energy_drift_ev_per_atom": drift, "ns_per_atom_step": ms_max * 1e6 / args.steps / N,
+        }
+        if world == 1 and not args.no_cpu_baseline:
+            line["cpu_baseline"] = cpu_baseline(args.workload)
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="config5",
+                    help="config5 (default, 1,048,576 atoms), config2, config3_<N>")
+    ap.add_argument("--mlp", default="fp32", choices=sorted(MLP_NAMES))
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -101,7 +101,11 @@ void gmnn_system_destroy(gmnn_system *s);
 
 /* Tuning / diagnostics knobs (never needed for correctness):
  *   "lanes_per_atom"  1,2,4,8,16,32: lanes that share one centre atom in the pair kernels (0 = auto)
- *   "profile"         1: record CUDA events around every stage of energy_forces (gmnn_stage_times)
+ *   "profile"         1: record a CUDA event after every stage of every later energy_forces / md call
+ *                     (gmnn_stage_times); setting it (to 0 or 1) discards what was recorded
+ *   "md_continue"     1: a gmnn_md_verlet_steps call whose positions and velocities are exactly the
+ *                     output of the previous call reuses that call's final forces and energies
+ *                     instead of evaluating them again at entry (the caller asserts this)
  *   "capacity"        neighbour slots per atom for the next build (0 = estimate from the density)
  *   "mlp_precision", "force_mode": override the model's value for this system
  * Returns GMNN_INVALID_ARG for an unknown key or value. */
@@ -168,10 +172,13 @@ int gmnn_md_verlet_steps(gmnn_system *s, float *positions, float *velocities, co
  * GMNN_NEIGHBOR_OVERFLOW, GMNN_OUT_OF_BOX) or GMNN_OK, clearing it. */
 int gmnn_check(gmnn_system *s, void *cuda_stream);
 
-/* Stage timing of the last gmnn_energy_forces call made with "profile" = 1: CUDA events recorded
- * on the call's own stream around each stage.  Synchronises on the last event.  Writes up to
- * max_stages names/durations (ms); returns the number of stages (or a negative status). */
-int gmnn_stage_times(gmnn_system *s, int32_t max_stages, const char **names /*HOST*/, float *ms /*HOST*/);
+/* Stage timing since "profile" was last set to 1: CUDA events recorded on each call's own stream
+ * after every stage (a stage is one kernel, or the few launches named in DESIGN.md section 5).
+ * Synchronises on the last event.  Writes, for up to max_stages distinct stage names in order of
+ * first appearance, the name, the MEAN duration of one occurrence (ms) and (counts nullable) the
+ * number of occurrences; returns the number of names (or a negative status). */
+int gmnn_stage_times(gmnn_system *s, int32_t max_stages, const char **names /*HOST*/, float *ms /*HOST*/,
+                     int32_t *counts /*HOST*/);
 
 /* Parity hook for the stage tests: copies an internal per-atom array of the last call to HOST,
  * rows in the library's internal (cell-sorted) atom order; "perm" gives internal row -> caller

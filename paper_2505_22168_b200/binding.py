@@ -58,6 +58,13 @@ class _Weights(C.Structure):
 
 def _load() -> C.CDLL:
     if not os.path.exists(LIB_PATH):
+        try:  # build in-tree (nvcc cross-compiles sm_100a); never a fallback to other code
+            from . import build as _build
+
+            _build.build()
+        except Exception:
+            pass
+    if not os.path.exists(LIB_PATH):
         raise ImportError(
             "%s is missing: build it with `python -m paper_2505_22168_b200.build` (nvcc, sm_100a). "
             "There is no CPU fallback." % LIB_PATH)
@@ -78,7 +85,7 @@ def _load() -> C.CDLL:
     lib.gmnn_system_get_int.argtypes = [C.c_void_p, C.c_char_p, C.c_void_p]
     lib.gmnn_get_neighbors.argtypes = [C.c_void_p] * 5
     lib.gmnn_check.argtypes = [C.c_void_p, C.c_void_p]
-    lib.gmnn_stage_times.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]
+    lib.gmnn_stage_times.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p]
     lib.gmnn_debug_read.argtypes = [C.c_void_p, C.c_char_p, C.c_void_p, C.c_int64]
     return lib
 
@@ -281,13 +288,14 @@ class System:
         _check(lib.gmnn_check(self.handle, _stream_ptr(stream)))
 
     def stage_times(self):
-        """[(stage name, ms)] of the last energy_forces call made with set_int('profile', 1)."""
-        names = (C.c_char_p * 32)()
-        ms = (C.c_float * 32)()
-        n = lib.gmnn_stage_times(self.handle, C.c_int32(32), names, ms)
+        """[(stage name, mean ms per occurrence, occurrences)] since set_int('profile', 1)."""
+        names = (C.c_char_p * 64)()
+        ms = (C.c_float * 64)()
+        cnt = (C.c_int32 * 64)()
+        n = lib.gmnn_stage_times(self.handle, C.c_int32(64), names, ms, cnt)
         if n < 0:
             _check(n)
-        return [(names[k].decode(), float(ms[k])) for k in range(n)]
+        return [(names[k].decode(), float(ms[k]), int(cnt[k])) for k in range(n)]
 
     def debug_read(self, name: str) -> np.ndarray:
         N, m = self.n_atoms, self.model

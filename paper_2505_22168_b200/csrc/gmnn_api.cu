@@ -49,25 +49,23 @@ __global__ void k_set_onehot(int M, int m, float *w) {
     if (t < M) w[t] = (t == m) ? 1.f : 0.f;
 }
 
+// Stage timing ("profile" = 1): one CUDA event after every stage of every call, on the call's own
+// stream, kept until "profile" is set again; gmnn_stage_times averages them per stage name.
 struct StageTimer {
     gmnn_system *s;
     cudaStream_t st;
     StageTimer(gmnn_system *s_, cudaStream_t st_) : s(s_), st(st_) {}
-    void begin() {
-        if (!s->profile) return;
-        s->n_stage_events = 0;
-        s->stage_names.clear();
-        mark(nullptr);
-    }
+    void begin() { mark(nullptr); }
     void mark(const char *name) {
-        if (!s->profile) return;
+        if (!s->profile || s->n_stage_events >= MAX_STAGE_EVENTS) return;
         if ((int)s->events.size() <= s->n_stage_events) {
             cudaEvent_t e;
             cudaEventCreate(&e);
             s->events.push_back(e);
+            s->stage_names.push_back(nullptr);
         }
+        s->stage_names[s->n_stage_events] = name;
         cudaEventRecord(s->events[s->n_stage_events++], st);
-        if (name) s->stage_names.push_back(name);
     }
 };
 
@@ -316,6 +314,9 @@ int gmnn_system_set_int(gmnn_system *s, const char *key, int64_t v) {
         s->lanes_per_atom = (int)v;
     } else if (!strcmp(key, "profile")) {
         s->profile = v != 0;
+        s->n_stage_events = 0;
+    } else if (!strcmp(key, "md_continue")) {
+        s->md_continue = v != 0;
     } else if (!strcmp(key, "capacity")) {
         if (v < 0 || v > 4096) {
             set_error("capacity must be in [0, 4096]");
@@ -339,6 +340,7 @@ int gmnn_system_get_int(const gmnn_system *s, const char *key, int64_t *v) {
     if (!s || !key || !v) return GMNN_INVALID_ARG;
     if (!strcmp(key, "lanes_per_atom")) *v = s->lanes_per_atom;
     else if (!strcmp(key, "profile")) *v = s->profile;
+    else if (!strcmp(key, "md_continue")) *v = s->md_continue;
     else if (!strcmp(key, "capacity")) *v = s->cap;
     else if (!strcmp(key, "mlp_precision")) *v = s->mlp_precision;
     else if (!strcmp(key, "force_mode")) *v = s->force_mode;
@@ -384,6 +386,7 @@ int gmnn_build_neighbors(gmnn_system *s, const float *positions, const float cel
                 return GMNN_UNSUPPORTED;
             }
         }
+    s->md_state_valid = false;
     Geometry &g = s->geo;
     const float r_list = r_cut + skin;  // fl32(fl32(r_cut) + fl32(skin)): the oracle is handed the same float
     g.r_list2 = r_list * r_list;
@@ -532,6 +535,7 @@ int gmnn_energy_forces(gmnn_system *s, const float *positions, double *energy, f
         return GMNN_INVALID_ARG;
     }
     cudaStream_t st = (cudaStream_t)cuda_stream;
+    s->md_state_valid = false;
     StageTimer T(s, st);
     T.begin();
     int rc = forward_backward(s, positions, s->model->head_mean_w, true, st, T);
@@ -581,6 +585,7 @@ int gmnn_ensemble_energy_forces(gmnn_system *s, const float *positions, float *e
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const int M = s->model->hp.n_heads;
     int rc;
+    s->md_state_valid = false;
     const int keep_profile = s->profile;
     s->profile = 0;
     if ((rc = launch_gather_positions(s, positions, st, true))) return rc;
@@ -620,28 +625,39 @@ int gmnn_md_verlet_steps(gmnn_system *s, float *positions, float *velocities, co
         return GMNN_UNSUPPORTED;
     }
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    const int keep_profile = s->profile;
-    s->profile = 0;
     const float hs = 0.5f * s->skin;
     const float thr2 = hs * hs;
     int rc;
-    StageTimer T(s, st);  // profiling is off inside the loop: marks are no-ops
-    // state at entry: forces of the current positions
-    if ((rc = forward_backward(s, positions, s->model->head_mean_w, false, st, T))) return rc;
-    if ((rc = launch_scatter_outputs(s, nullptr, s->f_tmp, st))) return rc;
-    if (epot_series && (rc = launch_energy_sum(s, epot_series, st))) return rc;
-    if (ekin_series && (rc = launch_ke(s, velocities, masses, ekin_series, st))) return rc;
-    for (int step = 1; step <= n_steps; ++step) {
-        if ((rc = launch_kick_drift(s, positions, velocities, s->f_tmp, masses, dt_fs, st))) return rc;
-        // rebuild (wrap first) iff the max displacement since the last build exceeds skin/2
-        if ((rc = launch_build(s, positions, st, s->flags + FLAG_DISP2, thr2, true, positions))) return rc;
+    StageTimer T(s, st);
+    T.begin();
+    double *const ep = s->e_total, *const ek = s->e_total + 1;  // energies of the latest step (device)
+    if (s->md_continue && s->md_state_valid) {
+        // the caller continues the trajectory of the previous call: f_tmp, e_total are current
+        if (epot_series) GMNN_CUDA(cudaMemcpyAsync(epot_series, ep, sizeof(double), cudaMemcpyDeviceToDevice, st));
+        if (ekin_series) GMNN_CUDA(cudaMemcpyAsync(ekin_series, ek, sizeof(double), cudaMemcpyDeviceToDevice, st));
+    } else {
+        // state at entry: forces of the current positions
         if ((rc = forward_backward(s, positions, s->model->head_mean_w, false, st, T))) return rc;
         if ((rc = launch_scatter_outputs(s, nullptr, s->f_tmp, st))) return rc;
-        if (epot_series && (rc = launch_energy_sum(s, epot_series + step, st))) return rc;
-        if ((rc = launch_kick_ke(s, velocities, s->f_tmp, masses, dt_fs, ekin_series ? ekin_series + step : nullptr, st)))
-            return rc;
+        if ((rc = launch_energy_sum(s, ep, st, epot_series))) return rc;
+        if ((rc = launch_ke(s, velocities, masses, ek, st, ekin_series))) return rc;
+        T.mark("outputs");
     }
-    s->profile = keep_profile;
+    s->md_state_valid = false;
+    for (int step = 1; step <= n_steps; ++step) {
+        if ((rc = launch_kick_drift(s, positions, velocities, s->f_tmp, masses, dt_fs, st))) return rc;
+        T.mark("kick_drift");
+        // rebuild (wrap first) iff the max displacement since the last build exceeds skin/2
+        if ((rc = launch_build(s, positions, st, s->flags + FLAG_DISP2, thr2, true, positions))) return rc;
+        T.mark("rebuild_if_moved");
+        if ((rc = forward_backward(s, positions, s->model->head_mean_w, false, st, T))) return rc;
+        if ((rc = launch_scatter_outputs(s, nullptr, s->f_tmp, st))) return rc;
+        if ((rc = launch_energy_sum(s, ep, st, epot_series ? epot_series + step : nullptr))) return rc;
+        T.mark("outputs");
+        if ((rc = launch_kick_ke(s, velocities, s->f_tmp, masses, dt_fs, ek, st, ekin_series ? ekin_series + step : nullptr)))
+            return rc;
+        T.mark("kick_ke");
+    }
     if ((rc = read_flags(s, st))) return rc;
     if (n_rebuilds) *n_rebuilds = s->flags_host[FLAG_REBUILDS];
     const int maxcount = s->flags_host[FLAG_MAXCOUNT];
@@ -651,6 +667,7 @@ int gmnn_md_verlet_steps(gmnn_system *s, float *positions, float *velocities, co
                   s->cap);
         return GMNN_NEIGHBOR_OVERFLOW;
     }
+    s->md_state_valid = true;
     return GMNN_OK;
 }
 
@@ -677,15 +694,35 @@ int gmnn_check(gmnn_system *s, void *cuda_stream) {
     return GMNN_OK;
 }
 
-int gmnn_stage_times(gmnn_system *s, int32_t max_stages, const char **names, float *ms) {
+int gmnn_stage_times(gmnn_system *s, int32_t max_stages, const char **names, float *ms, int32_t *counts) {
     if (!s || !names || !ms) return GMNN_INVALID_ARG;
-    const int n = (int)s->stage_names.size();
-    if (n == 0 || (int)s->events.size() < n + 1) return 0;
-    GMNN_CUDA(cudaEventSynchronize(s->events[n]));
+    const int n = s->n_stage_events;
+    if (n < 2) return 0;
+    GMNN_CUDA(cudaEventSynchronize(s->events[n - 1]));
+    std::vector<const char *> uniq;
+    std::vector<double> total;
+    std::vector<int> cnt;
+    for (int k = 1; k < n; ++k) {
+        const char *nm = s->stage_names[k];
+        if (!nm) continue;  // a begin() marker: the gap before it is not a stage
+        float t = 0.f;
+        GMNN_CUDA(cudaEventElapsedTime(&t, s->events[k - 1], s->events[k]));
+        size_t u = 0;
+        for (; u < uniq.size(); ++u)
+            if (!strcmp(uniq[u], nm)) break;
+        if (u == uniq.size()) {
+            uniq.push_back(nm);
+            total.push_back(0.0);
+            cnt.push_back(0);
+        }
+        total[u] += t;
+        cnt[u] += 1;
+    }
     int k = 0;
-    for (; k < n && k < max_stages; ++k) {
-        names[k] = s->stage_names[k];
-        GMNN_CUDA(cudaEventElapsedTime(&ms[k], s->events[k], s->events[k + 1]));
+    for (; k < (int)uniq.size() && k < max_stages; ++k) {
+        names[k] = uniq[k];
+        ms[k] = (float)(total[k] / cnt[k]);
+        if (counts) counts[k] = cnt[k];
     }
     return k;
 }

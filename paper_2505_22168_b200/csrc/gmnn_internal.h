@@ -20,6 +20,7 @@ constexpr int NBR_J_BITS = 22;  // neighbour entry: j in the low 22 bits, image 
 constexpr uint32_t NBR_J_MASK = (1u << NBR_J_BITS) - 1u;
 constexpr int64_t MAX_ATOMS = (int64_t)1 << NBR_J_BITS;
 constexpr int SMALL_BOX_MAX_ATOMS = 16384;
+constexpr int MAX_STAGE_EVENTS = 1 << 16;
 constexpr int PSI = 20;  // unique monomials per channel (contraction.cuh NM)
 
 // device-side flag words (int32) in System::flags
@@ -110,6 +111,8 @@ struct gmnn_system {
     // knobs
     int lanes_per_atom = 0;
     int profile = 0;
+    int md_continue = 0;             // knob: the next md call continues the previous one
+    bool md_state_valid = false;     // f_tmp / e_total hold the forces and energies of the last md step
     int mlp_precision = 0, force_mode = 0;
     // stage timing
     std::vector<cudaEvent_t> events;
@@ -140,11 +143,12 @@ int launch_mlp_backward_simt(gmnn_system *s, const float *head_w_dev, cudaStream
 
 // md.cu / reductions
 int launch_scatter_outputs(gmnn_system *s, float *e_atom_out, float *forces_out, cudaStream_t st);
-int launch_energy_sum(gmnn_system *s, double *energy_out, cudaStream_t st);
+int launch_energy_sum(gmnn_system *s, double *energy_out, cudaStream_t st, double *energy_out2 = nullptr);
 int launch_kick_drift(gmnn_system *s, float *x, float *v, const float *f, const float *m, float dt, cudaStream_t st);
 int launch_kick_ke(gmnn_system *s, float *v, const float *f, const float *m, float dt, double *ekin_out,
-                   cudaStream_t st);
-int launch_ke(gmnn_system *s, const float *v, const float *m, double *ekin_out, cudaStream_t st);
+                   cudaStream_t st, double *ekin_out2 = nullptr);
+int launch_ke(gmnn_system *s, const float *v, const float *m, double *ekin_out, cudaStream_t st,
+              double *ekin_out2 = nullptr);
 int launch_welford(gmnn_system *s, int head, const float *f_head, float *f_mean, float *f_m2, cudaStream_t st);
 int launch_ensemble_energy_stats(gmnn_system *s, float *e_mean, float *e_var, cudaStream_t st);
 int launch_finish_var(int64_t n, float *m2, int n_heads, cudaStream_t st);

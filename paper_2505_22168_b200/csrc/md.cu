@@ -64,11 +64,14 @@ __global__ void __launch_bounds__(256) k_ke_stage1(int64_t N, const float *__res
     if (threadIdx.x == 0) partial[blockIdx.x] = acc;
 }
 
-__global__ void __launch_bounds__(256) k_sum_stage2(int n, const double *__restrict__ partial, double factor, double *out) {
+__global__ void __launch_bounds__(256) k_sum_stage2(int n, const double *__restrict__ partial, double factor, double *out, double *out2) {
     double v = 0.0;
     for (int q = threadIdx.x; q < n; q += blockDim.x) v += partial[q];
     v = block_sum(v);
-    if (threadIdx.x == 0) *out = v * factor;
+    if (threadIdx.x == 0) {
+        *out = v * factor;
+        if (out2) *out2 = v * factor;
+    }
 }
 
 // v += (dt/2) a;  x += dt v;  squared displacement from the build positions -> max into flags.
@@ -150,21 +153,21 @@ int launch_scatter_outputs(gmnn_system *s, float *e_atom_out, float *forces_out,
 
 static int red_blocks(int64_t N) { return (int)(N < RED_BLOCKS * 256 ? (N + 255) / 256 : RED_BLOCKS); }
 
-int launch_energy_sum(gmnn_system *s, double *energy_out, cudaStream_t st) {
+int launch_energy_sum(gmnn_system *s, double *energy_out, cudaStream_t st, double *energy_out2) {
     const int nb = red_blocks(s->N);
     k_sum_stage1<<<nb, 256, 0, st>>>(s->N, s->e_atom, s->partial);
     GMNN_LAUNCHED();
-    k_sum_stage2<<<1, 256, 0, st>>>(nb, s->partial, 1.0, energy_out);
+    k_sum_stage2<<<1, 256, 0, st>>>(nb, s->partial, 1.0, energy_out, energy_out2);
     GMNN_LAUNCHED();
     GMNN_CUDA(cudaGetLastError());
     return GMNN_OK;
 }
 
-int launch_ke(gmnn_system *s, const float *v, const float *m, double *ekin_out, cudaStream_t st) {
+int launch_ke(gmnn_system *s, const float *v, const float *m, double *ekin_out, cudaStream_t st, double *ekin_out2) {
     const int nb = red_blocks(s->N);
     k_ke_stage1<<<nb, 256, 0, st>>>(s->N, v, m, s->partial + RED_BLOCKS);
     GMNN_LAUNCHED();
-    k_sum_stage2<<<1, 256, 0, st>>>(nb, s->partial + RED_BLOCKS, 1.0 / ACC_CONV, ekin_out);
+    k_sum_stage2<<<1, 256, 0, st>>>(nb, s->partial + RED_BLOCKS, 1.0 / ACC_CONV, ekin_out, ekin_out2);
     GMNN_LAUNCHED();
     GMNN_CUDA(cudaGetLastError());
     return GMNN_OK;
@@ -177,11 +180,12 @@ int launch_kick_drift(gmnn_system *s, float *x, float *v, const float *f, const 
     return GMNN_OK;
 }
 
-int launch_kick_ke(gmnn_system *s, float *v, const float *f, const float *m, float dt, double *ekin_out, cudaStream_t st) {
+int launch_kick_ke(gmnn_system *s, float *v, const float *f, const float *m, float dt, double *ekin_out, cudaStream_t st,
+                   double *ekin_out2) {
     k_kick<<<nblocks(s->N, 256), 256, 0, st>>>(s->N, v, f, m, dt);
     GMNN_LAUNCHED();
     GMNN_CUDA(cudaGetLastError());
-    if (ekin_out) return launch_ke(s, v, m, ekin_out, st);
+    if (ekin_out) return launch_ke(s, v, m, ekin_out, st, ekin_out2);
     return GMNN_OK;
 }
 
