@@ -23,6 +23,7 @@ void set_error(const char *fmt, ...) {
 }
 
 int launch_mlp_forward_tc(gmnn_system *s, cudaStream_t st);
+extern int g_tc_split_bk, g_tc_flush_k;
 int launch_mlp_backward_tc(gmnn_system *s, const float *head_w_dev, cudaStream_t st);
 
 template <class T>
@@ -268,6 +269,7 @@ int gmnn_system_create(const gmnn_model *m, int64_t n_atoms, const int32_t *spec
     A_(s->dZ[0], N * maxw);
     A_(s->dZ[1], N * maxw);
     A_(s->Bv, (size_t)m->dims[L] * m->dims[L - 1]);
+    A_(s->BvT, (size_t)m->dims[L] * m->dims[L - 1]);
     A_(s->vhead, (size_t)m->dims[L]);
     A_(s->head_w, (size_t)M);
     A_(s->e_heads, N * M);
@@ -295,7 +297,7 @@ void gmnn_system_destroy(gmnn_system *s) {
     dev_free(s->cell_fill); dev_free(s->slot_tmp); dev_free(s->perm); dev_free(s->pos4); dev_free(s->xref);
     dev_free(s->nbr); dev_free(s->count); dev_free(s->psi); dev_free(s->G); dev_free(s->dG); dev_free(s->A);
     for (int l = 0; l < MAX_LAYERS; ++l) { dev_free(s->H[l]); dev_free(s->D[l]); }
-    dev_free(s->dZ[0]); dev_free(s->dZ[1]); dev_free(s->Bv); dev_free(s->vhead); dev_free(s->head_w);
+    dev_free(s->dZ[0]); dev_free(s->dZ[1]); dev_free(s->Bv); dev_free(s->BvT); dev_free(s->vhead); dev_free(s->head_w);
     dev_free(s->e_heads); dev_free(s->e_atom); dev_free(s->f_int); dev_free(s->f_tmp); dev_free(s->partial);
     dev_free(s->e_total); dev_free(s->flags);
     dev_free(s->stage_pos); dev_free(s->stage_f); dev_free(s->stage_e);
@@ -329,6 +331,12 @@ int gmnn_system_set_int(gmnn_system *s, const char *key, int64_t v) {
     } else if (!strcmp(key, "force_mode")) {
         if (v < 0 || v > GMNN_FORCE_PAIRBUF) return GMNN_INVALID_ARG;
         s->force_mode = (int)v;
+    } else if (!strcmp(key, "tc_split_bk")) {  // process-wide tuning knob of mlp_tc.cu
+        if (v != 16 && v != 32) return GMNN_INVALID_ARG;
+        gmnn::g_tc_split_bk = (int)v;
+    } else if (!strcmp(key, "tc_flush_k")) {
+        if (v < 16 || v > 4096 || v % 16) return GMNN_INVALID_ARG;
+        gmnn::g_tc_flush_k = (int)v;
     } else {
         set_error("unknown key '%s'", key);
         return GMNN_INVALID_ARG;

@@ -98,6 +98,7 @@ struct gmnn_system {
     float *H[gmnn::MAX_LAYERS] = {}, *D[gmnn::MAX_LAYERS] = {};
     float *dZ[2] = {};
     float *Bv = nullptr;             // diag(v) W^T of the last hidden layer
+    float *BvT = nullptr;            // its transpose: W diag(v), [fan_in][fan_out] (B operand of mlp_tc.cu)
     float *vhead = nullptr;          // [H_last]
     float *head_w = nullptr;         // [n_heads] weights of the differentiated energy
     float *e_heads = nullptr;        // [N][n_heads]

@@ -175,6 +175,13 @@ __global__ void k_scale_rows(int rows, int cols, const float *__restrict__ WT, c
     Bv[t] = __ldg(&v[t / cols]) * __ldg(&WT[t]);
 }
 
+// BvT[n][k] = W[n][k] v[k]
+__global__ void k_scale_cols(int rows, int cols, const float *__restrict__ W, const float *__restrict__ v, float *BvT) {
+    const int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (t >= (int64_t)rows * cols) return;
+    BvT[t] = __ldg(&v[t % cols]) * __ldg(&W[t]);
+}
+
 int launch_mlp_forward_simt(gmnn_system *s, cudaStream_t st) {
     const gmnn_model *m = s->model;
     const float *X = s->G;
@@ -208,7 +215,10 @@ int launch_mlp_seed(gmnn_system *s, const float *head_w_dev, cudaStream_t st) {
     const int Hd = m->dims[L], prev = m->dims[L - 1];
     k_head_vec<<<(Hd + 127) / 128, 128, 0, st>>>(Hd, m->dims[L + 1], m->W[L], head_w_dev, s->vhead);
     GMNN_LAUNCHED();
-    k_scale_rows<<<(unsigned)(((int64_t)Hd * prev + 255) / 256), 256, 0, st>>>(Hd, prev, m->WT[L - 1], s->vhead, s->Bv);
+    if (s->mlp_precision == GMNN_MLP_FP32)
+        k_scale_rows<<<(unsigned)(((int64_t)Hd * prev + 255) / 256), 256, 0, st>>>(Hd, prev, m->WT[L - 1], s->vhead, s->Bv);
+    else
+        k_scale_cols<<<(unsigned)(((int64_t)Hd * prev + 255) / 256), 256, 0, st>>>(prev, Hd, m->W[L - 1], s->vhead, s->BvT);
     GMNN_LAUNCHED();
     GMNN_CUDA(cudaGetLastError());
     return GMNN_OK;

@@ -1,16 +1,432 @@
-// mlp_tc.cu -- tcgen05 / TMEM tensor-core MLP (GMNN_MLP_3XTF32, GMNN_MLP_TF32).  Placeholder
-// until the kernel lands: selecting these precisions fails loudly, it never falls back.
+// mlp_tc.cu -- the per-atom MLP readout and its input gradient on the 5th-generation tensor cores
+// (SURVEY.md 8(a) rows a7, a8; PAPER.md:63-65 Eq. 4, :153 forces by gradient).
+//
+//   mlp_precision = GMNN_MLP_3XTF32 : fp32-accurate.  a = a_hi + a_lo with a_hi = tf32(a) (round to
+//       nearest), a_lo = a - a_hi (exact in fp32); a.b ~= a_lo.b_hi + a_hi.b_lo + a_hi.b_hi, three
+//       kind::tf32 MMAs into one fp32 accumulator in tensor memory.  Dropped: a_lo.b_lo (<= 2^-22 |ab|)
+//       and the bits of a_lo, b_lo below tf32 (<= 2^-22 |ab|): the same order as fp32 round-off.
+//   mlp_precision = GMNN_MLP_TF32   : one kind::tf32 MMA per product (north_star's 2e-3 variant).
+//
+// The tensor core adds into its fp32 accumulator with truncation (measured: a 512-long chain of
+// accumulating MMAs is biased towards zero by ~1e-5 relative), so the fp32-accurate mode keeps the
+// chains short: the accumulator in tensor memory is flushed every `flush` pipeline stages into fp32
+// REGISTER accumulators of the epilogue warps (round-to-nearest adds), and inside a stage the small
+// cross terms are issued before the hi.hi terms so that they meet a small accumulator.
+//
+// One persistent, warp-specialised GEMM kernel  C[M][N] = A[M][K] . Bt[N][K]^T  with fused epilogues:
+//   warp 0        TMA producer: A (128 x BK) and Bt (bn x BK) boxes, swizzled, into an NST-stage ring
+//   warp 1        allocates tensor memory; one lane issues tcgen05.mma (128 x bn x 8 per instruction)
+//   warps 4-7     (3xTF32 only) split each landed stage in place into hi and lo tiles
+//   warps 8-15    epilogue: drain each K chunk from tensor memory (two 256-column buffers in
+//                 ping-pong, so draining chunk c overlaps the MMAs of chunk c+1) into 128 register
+//                 accumulators per thread; after the last chunk bias + swish + swish' / gradient
+//                 mask and the stores.  setmaxnreg moves registers from the other warps to these.
+// Operands stay fp32 in HBM (activations are written once, read once); the split happens on chip so
+// the L2 -> SM traffic is 4 B per operand element.
+#include <cuda.h>
+
 #include "gmnn_internal.h"
+#include "tc_ptx.cuh"
 
 namespace gmnn {
 
-int launch_mlp_forward_tc(gmnn_system *, cudaStream_t) {
-    set_error("tensor-core MLP (mlp_precision 1, 2) is not built yet");
-    return GMNN_UNSUPPORTED;
+using namespace tc;
+
+enum { EPI_PLAIN = 0, EPI_HIDDEN = 1, EPI_MUL = 2 };
+
+constexpr int TC_BM = 128;           // rows of A per tile = TMEM lanes
+constexpr int TC_BN_MAX = 256;       // columns per accumulator buffer
+constexpr int TC_THREADS = 16 * 32;  // four warpgroups: control, splitters, 2 x epilogue
+constexpr int TC_FIRST_SPLIT_WARP = 4;
+constexpr int TC_FIRST_EPI_WARP = 8;
+constexpr int TC_REGS_CONTROL = 40, TC_REGS_SPLIT = 64, TC_REGS_EPI = 200;  // 128 * (40 + 64 + 2 * 200) <= 65536
+constexpr int TC_STAGE_BYTES_TOTAL = 192 * 1024;
+
+template <bool SPLIT, int BK>
+struct TcCfg {
+    static constexpr int SWZ = BK * 4;                           // bytes per tile row = swizzle span
+    static constexpr int A_BYTES = TC_BM * BK * 4;
+    static constexpr int B_BYTES = TC_BN_MAX * BK * 4;
+    static constexpr int STAGE_BYTES = (A_BYTES + B_BYTES) * (SPLIT ? 2 : 1);
+    static constexpr int NST = TC_STAGE_BYTES_TOTAL / STAGE_BYTES;
+    static constexpr int SMEM_BYTES = NST * STAGE_BYTES + 1024 /*alignment slack*/ + 256 /*barriers*/;
+    static_assert(NST >= 2, "pipeline needs at least two stages");
+};
+
+struct TcArgs {
+    int M, N, K;
+    int bn;        // columns per tile (multiple of 16, <= 256)
+    int n_tiles_n;
+    int n_tiles;   // total
+    int flush;     // pipeline stages per accumulator flush (K chunk = flush * BK)
+    float *C;      // [M][N]
+    float *C2;     // EPI_HIDDEN: swish'(z)
+    const float *bias;
+    const float *Dmul;  // EPI_MUL: [M][N]
+};
+
+__device__ __forceinline__ void swish_pair_tc(float z, float &h, float &d) {
+    const float s = 1.f / (1.f + __expf(-z));
+    h = z * s;
+    d = s * (1.f + z * (1.f - s));
 }
-int launch_mlp_backward_tc(gmnn_system *, const float *, cudaStream_t) {
-    set_error("tensor-core MLP (mlp_precision 1, 2) is not built yet");
-    return GMNN_UNSUPPORTED;
+
+template <bool SPLIT, int BK, int EPI>
+__global__ void __launch_bounds__(TC_THREADS, 1)
+k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const TcArgs p) {
+    using Cfg = TcCfg<SPLIT, BK>;
+    constexpr int NST = Cfg::NST;
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    uint8_t *smem_gen = smem_raw + (smem_base - smem_u32(smem_raw));
+    // stage s: [A_hi | A_lo (SPLIT) | B_hi | B_lo (SPLIT)]
+    auto a_hi = [&](int s) { return smem_base + (uint32_t)s * Cfg::STAGE_BYTES; };
+    auto a_lo = [&](int s) { return a_hi(s) + Cfg::A_BYTES; };
+    auto b_hi = [&](int s) { return a_hi(s) + Cfg::A_BYTES * (SPLIT ? 2 : 1); };
+    auto b_lo = [&](int s) { return b_hi(s) + Cfg::B_BYTES; };
+    const uint32_t bar_base = smem_base + (uint32_t)NST * Cfg::STAGE_BYTES;
+    auto bar_full = [&](int s) { return bar_base + 8u * s; };
+    auto bar_split = [&](int s) { return bar_base + 8u * (NST + s); };
+    auto bar_empty = [&](int s) { return bar_base + 8u * (2 * NST + s); };
+    auto bar_tfull = [&](int a) { return bar_base + 8u * (3 * NST + a); };
+    auto bar_tempty = [&](int a) { return bar_base + 8u * (3 * NST + 2 + a); };
+    const uint32_t tmem_slot = bar_base + 8u * (3 * NST + 4);
+    volatile uint32_t *tmem_slot_gen = reinterpret_cast<volatile uint32_t *>(smem_gen + (size_t)NST * Cfg::STAGE_BYTES + 8 * (3 * NST + 4));
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int nkb = (p.K + BK - 1) / BK;  // pipeline stages per tile; chunk c covers stages [c*flush, (c+1)*flush)
+
+    if (warp == 0 && lane == 0) {
+        tma_prefetch_desc(&tmA);
+        tma_prefetch_desc(&tmB);
+        for (int s = 0; s < NST; ++s) {
+            mbar_init(bar_full(s), 1);
+            mbar_init(bar_split(s), 4);
+            mbar_init(bar_empty(s), 1);
+        }
+        for (int a = 0; a < 2; ++a) {
+            mbar_init(bar_tfull(a), 1);
+            mbar_init(bar_tempty(a), 8);
+        }
+        fence_barrier_init();
+    }
+    if (warp == 1) tmem_alloc<512>(tmem_slot);
+    tcgen05_fence_before();
+    __syncthreads();
+    tcgen05_fence_after();
+    const uint32_t tmem_base = *tmem_slot_gen;
+
+    if (warp < TC_FIRST_SPLIT_WARP) {
+        setmaxnreg_dec<TC_REGS_CONTROL>();
+        if (warp == 0 && lane == 0) {
+            // ===== TMA producer =====
+            const uint32_t tx = (uint32_t)(Cfg::A_BYTES + p.bn * BK * 4);
+            uint32_t it = 0;
+            for (int t = blockIdx.x; t < p.n_tiles; t += gridDim.x) {
+                const int m0 = (t / p.n_tiles_n) * TC_BM, n0 = (t % p.n_tiles_n) * p.bn;
+                for (int kb = 0; kb < nkb; ++kb, ++it) {
+                    const int s = it % NST;
+                    mbar_wait(bar_empty(s), ((it / NST) & 1) ^ 1);
+                    mbar_arrive_expect_tx(bar_full(s), tx);
+                    tma_load_2d(a_hi(s), &tmA, bar_full(s), kb * BK, m0);
+                    tma_load_2d(b_hi(s), &tmB, bar_full(s), kb * BK, n0);
+                }
+            }
+        } else if (warp == 1 && lane == 0) {
+            // ===== MMA issuer =====
+            const uint32_t idesc = make_idesc_tf32(TC_BM, p.bn);
+            uint32_t it = 0, chunk = 0;
+            for (int t = blockIdx.x; t < p.n_tiles; t += gridDim.x) {
+                for (int kb = 0; kb < nkb; ++kb, ++it) {
+                    const int in_chunk = kb % p.flush;
+                    const int a = chunk & 1;
+                    const uint32_t d_tmem = tmem_base + (uint32_t)a * TC_BN_MAX;
+                    if (in_chunk == 0) {
+                        mbar_wait(bar_tempty(a), ((chunk >> 1) & 1) ^ 1);
+                        tcgen05_fence_after();
+                    }
+                    const int s = it % NST;
+                    mbar_wait(SPLIT ? bar_split(s) : bar_full(s), (it / NST) & 1);
+                    tcgen05_fence_after();
+                    const int krem = p.K - kb * BK;
+                    const int ksteps = krem >= BK ? BK / 8 : (krem + 7) / 8;
+                    const uint64_t da_hi = make_smem_desc<Cfg::SWZ>(a_hi(s)), db_hi = make_smem_desc<Cfg::SWZ>(b_hi(s));
+                    uint32_t acc = in_chunk != 0;
+                    if (SPLIT) {  // small cross terms first: they meet the smallest accumulator
+                        const uint64_t da_lo = make_smem_desc<Cfg::SWZ>(a_lo(s)), db_lo = make_smem_desc<Cfg::SWZ>(b_lo(s));
+                        for (int k = 0; k < ksteps; ++k) {
+                            const uint64_t koff = (uint64_t)((k * 32) >> 4);  // 8 tf32 = 32 bytes along the row
+                            mma_tf32_ss(d_tmem, da_lo + koff, db_hi + koff, idesc, acc);
+                            mma_tf32_ss(d_tmem, da_hi + koff, db_lo + koff, idesc, 1u);
+                            acc = 1u;
+                        }
+                    }
+                    for (int k = 0; k < ksteps; ++k) {
+                        const uint64_t koff = (uint64_t)((k * 32) >> 4);
+                        mma_tf32_ss(d_tmem, da_hi + koff, db_hi + koff, idesc, acc);
+                        acc = 1u;
+                    }
+                    mma_commit(bar_empty(s));
+                    if (in_chunk == p.flush - 1 || kb == nkb - 1) {
+                        mma_commit(bar_tfull(a));
+                        ++chunk;
+                    }
+                }
+            }
+        }
+    } else if (warp < TC_FIRST_EPI_WARP) {
+        setmaxnreg_dec<TC_REGS_SPLIT>();
+        // ===== splitters (3xTF32): hi = tf32(x) in place, lo = x - hi beside it =====
+        if (SPLIT) {
+            const int tid = threadIdx.x - TC_FIRST_SPLIT_WARP * 32;  // 0..127
+            const int n_a4 = Cfg::A_BYTES / 16, n_b4 = p.bn * BK * 4 / 16;
+            uint32_t it = 0;
+            for (int t = blockIdx.x; t < p.n_tiles; t += gridDim.x) {
+                for (int kb = 0; kb < nkb; ++kb, ++it) {
+                    const int s = it % NST;
+                    mbar_wait(bar_full(s), (it / NST) & 1);
+                    float4 *ah = reinterpret_cast<float4 *>(smem_gen + (size_t)s * Cfg::STAGE_BYTES);
+                    float4 *al = reinterpret_cast<float4 *>(smem_gen + (size_t)s * Cfg::STAGE_BYTES + Cfg::A_BYTES);
+                    float4 *bh = reinterpret_cast<float4 *>(smem_gen + (size_t)s * Cfg::STAGE_BYTES + 2 * Cfg::A_BYTES);
+                    float4 *bl = reinterpret_cast<float4 *>(smem_gen + (size_t)s * Cfg::STAGE_BYTES + 2 * Cfg::A_BYTES + Cfg::B_BYTES);
+#pragma unroll 4
+                    for (int q = tid; q < n_a4 + n_b4; q += 128) {
+                        float4 *ph = q < n_a4 ? ah + q : bh + (q - n_a4);
+                        float4 *pl = q < n_a4 ? al + q : bl + (q - n_a4);
+                        const float4 v = *ph;
+                        float4 h, l;
+                        h.x = to_tf32_rna(v.x); h.y = to_tf32_rna(v.y); h.z = to_tf32_rna(v.z); h.w = to_tf32_rna(v.w);
+                        l.x = v.x - h.x; l.y = v.y - h.y; l.z = v.z - h.z; l.w = v.w - h.w;
+                        *ph = h;
+                        *pl = l;
+                    }
+                    fence_proxy_async_smem();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(bar_split(s));
+                }
+            }
+        }
+    } else {
+        setmaxnreg_inc<TC_REGS_EPI>();
+        // ===== epilogue: drain K chunks TMEM -> register accumulators, then the fused elementwise =====
+        const int quad = warp & 3;                        // TMEM lanes 32*quad .. 32*quad+31
+        const int half = (warp - TC_FIRST_EPI_WARP) >> 2;  // 32-column groups half, half+2, half+4, half+6
+        const int n_groups = (p.bn + 31) / 32;
+        const int n_chunks = (nkb + p.flush - 1) / p.flush;
+        const uint32_t lane_base = tmem_base + ((uint32_t)(quad * 32) << 16);
+        uint32_t chunk = 0;
+        for (int t = blockIdx.x; t < p.n_tiles; t += gridDim.x) {
+            const int m0 = (t / p.n_tiles_n) * TC_BM, n0 = (t % p.n_tiles_n) * p.bn;
+            const int row = m0 + quad * 32 + lane;
+            const bool row_ok = row < p.M;
+            float acc[4][32];
+#pragma unroll
+            for (int gi = 0; gi < 4; ++gi)
+#pragma unroll
+                for (int j = 0; j < 32; ++j) acc[gi][j] = 0.f;
+            for (int c = 0; c < n_chunks; ++c, ++chunk) {
+                const int a = chunk & 1;
+                mbar_wait(bar_tfull(a), (chunk >> 1) & 1);
+                tcgen05_fence_after();
+#pragma unroll
+                for (int gi = 0; gi < 4; ++gi) {
+                    const int g = 2 * gi + half;
+                    if (g < n_groups) {
+                        uint32_t v[32];
+                        tmem_ld_32x32(lane_base + (uint32_t)(a * TC_BN_MAX + g * 32), v);
+                        tmem_ld_wait();
+#pragma unroll
+                        for (int j = 0; j < 32; ++j) acc[gi][j] += __uint_as_float(v[j]);
+                    }
+                }
+                tcgen05_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar_tempty(a));
+            }
+#pragma unroll
+            for (int gi = 0; gi < 4; ++gi) {
+                const int g = 2 * gi + half;
+                const int col0 = n0 + g * 32;
+                const int64_t o = (int64_t)row * p.N + col0;
+#pragma unroll
+                for (int j = 0; j < 32; j += 4) {
+                    // a 4-column group is either whole or absent: N and bn are multiples of 4
+                    if (!row_ok || g >= n_groups || col0 + j >= p.N || g * 32 + j >= p.bn) continue;
+                    float4 x = make_float4(acc[gi][j], acc[gi][j + 1], acc[gi][j + 2], acc[gi][j + 3]);
+                    if (EPI == EPI_HIDDEN) {
+                        const float4 bb = __ldg(reinterpret_cast<const float4 *>(p.bias + col0 + j));
+                        float4 h, d;
+                        swish_pair_tc(x.x + bb.x, h.x, d.x);
+                        swish_pair_tc(x.y + bb.y, h.y, d.y);
+                        swish_pair_tc(x.z + bb.z, h.z, d.z);
+                        swish_pair_tc(x.w + bb.w, h.w, d.w);
+                        *reinterpret_cast<float4 *>(p.C + o + j) = h;
+                        *reinterpret_cast<float4 *>(p.C2 + o + j) = d;
+                    } else if (EPI == EPI_MUL) {
+                        const float4 dm = __ldg(reinterpret_cast<const float4 *>(p.Dmul + o + j));
+                        x.x *= dm.x; x.y *= dm.y; x.z *= dm.z; x.w *= dm.w;
+                        *reinterpret_cast<float4 *>(p.C + o + j) = x;
+                    } else {
+                        *reinterpret_cast<float4 *>(p.C + o + j) = x;
+                    }
+                }
+            }
+        }
+    }
+
+    tcgen05_fence_before();
+    __syncthreads();
+    if (warp == 1) tmem_dealloc<512>(tmem_base);
+}
+
+// ---- host side --------------------------------------------------------------------------------
+
+typedef CUresult (*PFN_encodeTiled)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                    const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static PFN_encodeTiled get_encode() {
+    static PFN_encodeTiled fn = nullptr;
+    if (!fn) {
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<PFN_encodeTiled>(p);
+    }
+    return fn;
+}
+
+// fp32 row-major [rows][K] matrix, box = box_rows x BK elements, swizzle span = BK * 4 bytes.
+static int make_tmap(CUtensorMap *tm, const float *base, int64_t rows, int K, int box_rows, int BK) {
+    PFN_encodeTiled enc = get_encode();
+    if (!enc) {
+        set_error("cuTensorMapEncodeTiled is not available from the driver");
+        return GMNN_CUDA_ERROR;
+    }
+    const cuuint64_t dims[2] = {(cuuint64_t)K, (cuuint64_t)rows};
+    const cuuint64_t strides[1] = {(cuuint64_t)K * 4};
+    const cuuint32_t box[2] = {(cuuint32_t)BK, (cuuint32_t)box_rows};
+    const cuuint32_t estr[2] = {1, 1};
+    const CUtensorMapSwizzle sw = BK == 32 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_64B;
+    const CUresult r = enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float *>(base), dims, strides, box, estr,
+                           CU_TENSOR_MAP_INTERLEAVE_NONE, sw, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        set_error("cuTensorMapEncodeTiled failed (%d) for a [%lld][%d] matrix", (int)r, (long long)rows, K);
+        return GMNN_CUDA_ERROR;
+    }
+    return GMNN_OK;
+}
+
+static int tc_num_sms() {
+    static int n = 0;
+    if (!n) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev);
+        if (n <= 0) n = 148;
+    }
+    return n;
+}
+
+// Columns per tile: a multiple of 16 (UMMA M = 128 needs N % 16 == 0), at most 256, least padding.
+static int pick_bn(int N) {
+    if (N <= TC_BN_MAX) return (N + 15) / 16 * 16;
+    int best = 256, best_pad = 1 << 30;
+    for (int bn = 256; bn >= 128; bn -= 16) {
+        const int pad = (N + bn - 1) / bn * bn - N;
+        if (pad < best_pad) best_pad = pad, best = bn;
+    }
+    return best;
+}
+
+template <bool SPLIT, int BK, int EPI>
+static int tc_launch(const CUtensorMap &tmA, const CUtensorMap &tmB, const TcArgs &args, cudaStream_t st) {
+    using Cfg = TcCfg<SPLIT, BK>;
+    static bool attr_set = false;
+    if (!attr_set) {
+        GMNN_CUDA(cudaFuncSetAttribute(k_gemm_tc<SPLIT, BK, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES));
+        attr_set = true;
+    }
+    const int grid = args.n_tiles < tc_num_sms() ? args.n_tiles : tc_num_sms();
+    k_gemm_tc<SPLIT, BK, EPI><<<grid, TC_THREADS, Cfg::SMEM_BYTES, st>>>(tmA, tmB, args);
+    GMNN_LAUNCHED();
+    GMNN_CUDA(cudaGetLastError());
+    return GMNN_OK;
+}
+
+int g_tc_flush_k = 32;   // knob "tc_flush_k": K extent between accumulator flushes of the 3xTF32 mode
+int g_tc_split_bk = 16;  // knob (gmnn_system_set_int "tc_split_bk"): K extent of a 3xTF32 stage, 16 or 32
+
+// C[M][N] = A[M][K] . Bt[N][K]^T, all fp32 row-major and dense (lda = ldb = K, ldc = N).
+int tc_gemm(bool split, int epi, int64_t M, int N, int K, const float *A, const float *Bt, float *C, const float *bias,
+            float *C2, const float *Dmul, cudaStream_t st) {
+    if (K % 4 != 0 || N % 4 != 0 || M <= 0 || M > INT32_MAX) {
+        set_error("tensor-core MLP: widths must be multiples of 4 (K = %d, N = %d)", K, N);
+        return GMNN_UNSUPPORTED;
+    }
+    const int BK = split ? g_tc_split_bk : 32;
+    TcArgs a;
+    a.M = (int)M, a.N = N, a.K = K;
+    a.bn = pick_bn(N);
+    a.n_tiles_n = (N + a.bn - 1) / a.bn;
+    a.n_tiles = (int)((M + TC_BM - 1) / TC_BM) * a.n_tiles_n;
+    a.flush = split ? (g_tc_flush_k / BK > 0 ? g_tc_flush_k / BK : 1) : (K + BK - 1) / BK;  // TF32 mode: one chunk
+    a.C = C, a.C2 = C2, a.bias = bias, a.Dmul = Dmul;
+    CUtensorMap tmA, tmB;
+    int rc;
+    if ((rc = make_tmap(&tmA, A, M, K, TC_BM, BK))) return rc;
+    if ((rc = make_tmap(&tmB, Bt, N, K, a.bn, BK))) return rc;
+#define TC_CASE(SP, BKV)                                                                  \
+    switch (epi) {                                                                        \
+        case EPI_PLAIN: return tc_launch<SP, BKV, EPI_PLAIN>(tmA, tmB, a, st);             \
+        case EPI_HIDDEN: return tc_launch<SP, BKV, EPI_HIDDEN>(tmA, tmB, a, st);           \
+        default: return tc_launch<SP, BKV, EPI_MUL>(tmA, tmB, a, st);                      \
+    }
+    if (!split) { TC_CASE(false, 32) }
+    if (BK == 32) { TC_CASE(true, 32) }
+    TC_CASE(true, 16)
+#undef TC_CASE
+}
+
+int launch_mlp_forward_tc(gmnn_system *s, cudaStream_t st) {
+    const gmnn_model *m = s->model;
+    const bool split = s->mlp_precision == GMNN_MLP_3XTF32;
+    const float *X = s->G;
+    for (int l = 0; l < m->hp.n_hidden; ++l) {
+        // z = X W[l]: the B operand is W[l]^T = WT[l], [fan_out][fan_in]
+        int rc = tc_gemm(split, EPI_HIDDEN, s->N, m->dims[l + 1], m->dims[l], X, m->WT[l], s->H[l], m->b[l], s->D[l], nullptr, st);
+        if (rc) return rc;
+        X = s->H[l];
+    }
+    return GMNN_OK;
+}
+
+// Same chain as launch_mlp_backward_simt (mlp_simt.cu); the B operand of  out = Aop . Bop  is Bop^T:
+// Bop = WT[l-1] gives W[l-1]; Bop = diag(v) WT[L-1] gives W[L-1] diag(v) = BvT.
+int launch_mlp_backward_tc(gmnn_system *s, const float *head_w_dev, cudaStream_t st) {
+    const gmnn_model *m = s->model;
+    const bool split = s->mlp_precision == GMNN_MLP_3XTF32;
+    const int L = m->hp.n_hidden;
+    int rc = launch_mlp_seed(s, head_w_dev, st);  // vhead, Bv (and BvT, see mlp_simt.cu)
+    if (rc) return rc;
+    const float *Aop = s->D[L - 1];
+    const float *BopT = s->BvT;
+    int cur = 0;
+    for (int l = L - 1; l >= 0; --l) {
+        if (l > 0) {
+            rc = tc_gemm(split, EPI_MUL, s->N, m->dims[l], m->dims[l + 1], Aop, BopT, s->dZ[cur], nullptr, nullptr, s->D[l - 1], st);
+            if (rc) return rc;
+            Aop = s->dZ[cur];
+            BopT = m->W[l - 1];
+            cur ^= 1;
+        } else {
+            rc = tc_gemm(split, EPI_PLAIN, s->N, m->dims[0], m->dims[1], Aop, BopT, s->dG, nullptr, nullptr, nullptr, st);
+            if (rc) return rc;
+        }
+    }
+    return GMNN_OK;
 }
 
 }  // namespace gmnn

@@ -1,0 +1,130 @@
+"""GPU parity of the tcgen05 tensor-core MLP (mlp_tc.cu) against the fp64 oracle.
+mlp_precision = 1 (3xTF32) must meet the fp32 tolerances of north_star (1e-5 per-atom energy,
+1e-4 force measure).  mlp_precision = 2 (single-pass TF32, operands truncated by the tensor core) is
+measured at 1e-2 .. 2.5e-2 on the force measure: it does NOT meet north_star's 2e-3 bound for a
+reduced-precision variant, is not offered as one, and is only characterised here."""
+import numpy as np
+import pytest
+
+import workloads as wl
+from parity_utils import E_TOTAL_RTOL, F_TOL, energy_atom_error, force_error, r_list32
+
+F_TOL_TF32_MEASURED = 5e-2  # characterisation bound of the unclaimed single-pass mode
+
+pytestmark = pytest.mark.gpu
+
+P3X, PTF32 = 1, 2
+
+
+@pytest.fixture(scope="module")
+def gm():
+    import torch
+
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device (they must not pass on a fallback)")
+    import paper_2505_22168_b200 as pkg
+
+    return pkg
+
+
+def _ref(orc, w, intermediates=False):
+    m = orc.Model(w.model)
+    pairs = orc.auto_neighbors(w.positions, w.cell, w.pbc, r_list32(w.model.r_cut, w.skin))
+    return orc.energy_forces(m, w.positions, w.species, w.cell, pairs, intermediates=intermediates)
+
+
+def _system(gm, w, precision):
+    import torch
+
+    model = gm.Model(w.model, mlp_precision=precision)
+    sysm = gm.System(model, w.species)
+    pos = torch.from_numpy(w.positions).cuda()
+    sysm.build_neighbors(pos, w.cell9, w.pbc, w.model.r_cut, w.skin)
+    return sysm, pos
+
+
+def _run(sysm, pos):
+    e, ea, f = sysm.energy_forces(pos)
+    sysm.check()
+    return float(e.cpu()[0]), ea.cpu().numpy().astype(np.float64), f.cpu().numpy().astype(np.float64)
+
+
+@pytest.mark.parametrize("split_bk,flush_k", [(16, 32), (32, 32), (16, 16), (32, 64)])
+@pytest.mark.parametrize("name", ["config1", "config2", "config3_1024", "config3_8192"])
+def test_3xtf32_meets_fp32_tolerance(gm, orc, name, split_bk, flush_k):
+    """Both stage shapes (64 B and 128 B swizzle) and several accumulator-flush intervals."""
+    w = wl.make_workload(name)
+    ref = _ref(orc, w)
+    sysm, pos = _system(gm, w, P3X)
+    sysm.set_int("tc_split_bk", split_bk)
+    sysm.set_int("tc_flush_k", flush_k)
+    try:
+        e, ea, f = _run(sysm, pos)
+    finally:
+        sysm.set_int("tc_split_bk", 16)
+        sysm.set_int("tc_flush_k", 32)
+    print("3xTF32 %s bk %d flush %d: energy err %.3f x 1e-5, force err %.2e" % (
+        name, split_bk, flush_k, energy_atom_error(ea, ref.e_atom), force_error(f, ref.forces)))
+    assert energy_atom_error(ea, ref.e_atom) <= 1.0
+    assert force_error(f, ref.forces) <= F_TOL
+    assert abs(e - ref.energy) <= E_TOTAL_RTOL * np.abs(ref.e_atom).sum()
+
+
+@pytest.mark.parametrize("name", ["config1", "config3_1024", "config3_8192"])
+def test_tf32_single_pass_characterised(gm, orc, name):
+    w = wl.make_workload(name)
+    ref = _ref(orc, w)
+    sysm, pos = _system(gm, w, PTF32)
+    e, ea, f = _run(sysm, pos)
+    assert force_error(f, ref.forces) <= F_TOL_TF32_MEASURED
+    assert np.abs(ea - ref.e_atom).max() <= 2e-2 * max(np.abs(ref.e_atom).max(), 1e-30)
+    # and it really is a different arithmetic from the fp32 path (guards against a silent alias)
+    sysm.set_int("mlp_precision", 0)
+    _, _, f32 = _run(sysm, pos)
+    assert np.abs(f32 - f).max() > 0
+
+
+@pytest.mark.parametrize("precision", [P3X, PTF32])
+@pytest.mark.parametrize("hidden", [(16, 16), (64, 48), (144, 272), (512, 512)])
+def test_ragged_shapes(gm, orc, precision, hidden):
+    """N = 1000 atoms (not a multiple of the 128-row tile), widths that are not multiples of the
+    K stage (16 / 32) nor of the column tile; 272 > 256 forces two ragged column tiles."""
+    w = wl.li3po4_box(1000, hidden=hidden)
+    ref = _ref(orc, w, intermediates=True)
+    sysm, pos = _system(gm, w, precision)
+    e, ea, f = _run(sysm, pos)
+    tol = F_TOL if precision == P3X else F_TOL_TF32_MEASURED
+    assert force_error(f, ref.forces) <= tol
+    perm = sysm.debug_read("perm")
+    sig = w.model.scale[w.species][perm][:, None]
+    dG_ref = ref.dG[perm] / sig
+    dG = sysm.debug_read("dG")
+    assert np.abs(dG - dG_ref).max() <= tol * np.abs(dG_ref).max()
+    if precision == P3X:
+        assert energy_atom_error(ea, ref.e_atom) <= 1.0
+
+
+def test_3xtf32_matches_fp32_simt_closely(gm):
+    """The two fp32-accurate MLPs agree far inside the oracle tolerance, and each is bit-reproducible."""
+    w = wl.li3po4_box(4096, hidden=(512, 512))
+    sysm, pos = _system(gm, w, P3X)
+    e1, ea1, f1 = _run(sysm, pos)
+    e1b, ea1b, f1b = _run(sysm, pos)
+    assert e1 == e1b and np.array_equal(ea1, ea1b) and np.array_equal(f1, f1b)
+    sysm.set_int("mlp_precision", 0)
+    e0, ea0, f0 = _run(sysm, pos)
+    assert force_error(f1, f0) <= 5e-5
+    assert np.abs(ea1 - ea0).max() <= 5e-6 * np.abs(ea0).mean()
+
+
+def test_ensemble_heads_with_tc(gm, orc):
+    """Shallow ensemble (config 4 shape, smaller box): M backward passes through the TC MLP."""
+    w = wl.li3po4_box(1024, n_heads=8)
+    m = orc.Model(w.model)
+    pairs = orc.auto_neighbors(w.positions, w.cell, w.pbc, r_list32(w.model.r_cut, w.skin))
+    ref = orc.ensemble(m, w.positions, w.species, w.cell, pairs)
+    sysm, pos = _system(gm, w, P3X)
+    e_mean, e_var, f_mean, f_var = (t.cpu().numpy().astype(np.float64) for t in sysm.ensemble_energy_forces(pos))
+    assert energy_atom_error(e_mean, ref.e_mean) <= 1.0
+    assert force_error(f_mean, ref.f_mean) <= F_TOL
+    assert np.abs(f_var - ref.f_var).max() <= 2e-4 * ref.f_var.max()
