@@ -14,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libgmnn_b200.so")
 SOURCES = ["gmnn_api.cu", "neighbor.cu", "descriptor.cu", "mlp_simt.cu", "mlp_tc.cu", "md.cu"]
-HEADERS = ["gmnn_internal.h", "contraction.cuh", os.path.join("..", "..", "include", "gmnn.h")]
+HEADERS = ["gmnn_internal.h", "contraction.cuh", "tc_ptx.cuh", os.path.join("..", "..", "include", "gmnn.h")]
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
     "-Xcompiler", "-fPIC", "-cudart", "static", "--expt-relaxed-constexpr",

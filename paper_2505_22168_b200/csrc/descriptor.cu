@@ -22,6 +22,7 @@
 
 #include "contraction.cuh"
 #include "gmnn_internal.h"
+#include "tc_ptx.cuh"
 
 namespace gmnn {
 
@@ -247,66 +248,118 @@ k_contract_forward(int64_t N, const float *__restrict__ psi, float *__restrict__
 }
 
 // ---------------------------------------------------------------------------------------------
-// a9: adjoint of the invariants.  One thread per atom; Psi row and the current chunk of dE/dG in
-// per-warp shared tiles (component-major, pitch 33: conflict-free), the 100 adjoints in registers.
+// a9: adjoint of the invariants.  One thread per atom, one block per 128-atom tile of dE/dG, which
+// the MLP backward writes tile-transposed ([N/128][F][128]): every chunk of feature blocks is one
+// contiguous run, brought into shared memory by 1-D bulk copies (cp.async.bulk + mbarrier) into two
+// slots so that the next chunk lands while the current one is consumed; reads sG[f][tid] are
+// conflict-free.  Psi row and the 100 adjoints live in registers (straight-line FMA code).
 // dE/dG arrives without the sigma_Z factor of Eq. 4 (the MLP backward is linear in it); it is
 // applied here.
 // ---------------------------------------------------------------------------------------------
 template <int NR>
-__global__ void __launch_bounds__(64)
-k_contract_backward(int64_t N, const float *__restrict__ psi, const float *__restrict__ dG,
+struct CbSmem {  // shared-memory plan of k_contract_backward, in floats
+    using CH = FeatChunks<NR>;
+    static constexpr int TB = 128;  // atoms per block = one dG tile
+    static constexpr int len(int c) { return CH::begin(c + 1) - CH::begin(c); }
+    static constexpr int cmax(int a, int b) { return a > b ? a : b; }
+    // slot X: chunk 4 (block 7), then chunks 1 and 3 back to back, then the output transpose
+    static constexpr int X = cmax(cmax(len(4), len(1) + len(3)) * TB, 4 * NR * PSI * CW);
+    // slot Y: chunk 0, then chunk 2
+    static constexpr int Y = cmax(len(0), len(2)) * TB;
+    static constexpr size_t BYTES = sizeof(float) * (X + Y) + 16;
+};
+
+template <int NR>
+__global__ void __launch_bounds__(128, 2)
+k_contract_backward(int64_t N, const float *__restrict__ psi, const float *__restrict__ dGt,
                     const float4 *__restrict__ pos4, const float *__restrict__ scale, float *__restrict__ A) {
     using F = Feat<NR>;
     using CH = FeatChunks<NR>;
-    extern __shared__ float s_tile[];
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    float *sP = s_tile + wid * ((NR * PSI + CH::max_len()) * CW);
-    float *sG = sP + NR * PSI * CW;
-    const int64_t i0 = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) - lane;
-    const int64_t i = i0 + lane;
-    for (int a = 0; a < 32; ++a) {
-        const int64_t ia = i0 + a;
-        if (ia >= N) break;
-        const float *src = psi + ia * (int64_t)(NR * PSI);
-        for (int q = lane; q < NR * PSI; q += 32) sP[q * CW + a] = __ldg(&src[q]);
+    using SM = CbSmem<NR>;
+    constexpr int TB = SM::TB;
+    extern __shared__ __align__(128) float s_cb[];
+    float *sX = s_cb, *sY = s_cb + SM::X;
+    const uint32_t barX = tc::smem_u32(s_cb + SM::X + SM::Y), barY = barX + 8;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const int64_t i = blockIdx.x * (int64_t)TB + tid;
+    const float *gt = dGt + blockIdx.x * (int64_t)(F::N * TB);  // this block's [F][128] tile
+    auto issue = [&](float *dst, int c, uint32_t bar) {
+        tc::bulk_load_1d(tc::smem_u32(dst), gt + CH::begin(c) * TB, (uint32_t)(SM::len(c) * TB * 4), bar);
+    };
+    if (tid == 0) {
+        tc::mbar_init(barX, 1);
+        tc::mbar_init(barY, 1);
+        tc::fence_barrier_init();
+        tc::mbar_arrive_expect_tx(barY, (uint32_t)(SM::len(0) * TB * 4));
+        issue(sY, 0, barY);
+        tc::mbar_arrive_expect_tx(barX, (uint32_t)(SM::len(4) * TB * 4));
+        issue(sX, 4, barX);
     }
+    float P[NR][PSI];
     float sig = 0.f;
-    if (i < N) sig = __ldg(&scale[__float_as_int(pos4[i].w)]);
+    if (i < N) {
+        const float4 *src = reinterpret_cast<const float4 *>(psi + i * (int64_t)(NR * PSI));
+#pragma unroll
+        for (int q = 0; q < NR * PSI / 4; ++q) {
+            const float4 v = __ldg(&src[q]);
+            P[(4 * q) / PSI][(4 * q) % PSI] = v.x;
+            P[(4 * q + 1) / PSI][(4 * q + 1) % PSI] = v.y;
+            P[(4 * q + 2) / PSI][(4 * q + 2) % PSI] = v.z;
+            P[(4 * q + 3) / PSI][(4 * q + 3) % PSI] = v.w;
+        }
+        sig = __ldg(&scale[__float_as_int(pos4[i].w)]);
+    } else {
+#pragma unroll
+        for (int s = 0; s < NR; ++s)
+#pragma unroll
+            for (int m = 0; m < PSI; ++m) P[s][m] = 0.f;
+    }
     float acc[NR][PSI];
 #pragma unroll
     for (int s = 0; s < NR; ++s)
 #pragma unroll
         for (int m = 0; m < PSI; ++m) acc[s][m] = 0.f;
-    __syncwarp();
+    __syncthreads();  // barrier initialisation visible to every waiter
 
-    auto run_chunk = [&](auto chunk_tag) {
+    auto run_chunk = [&](auto chunk_tag, const float *buf) {
         constexpr int C = decltype(chunk_tag)::value;
-        constexpr int len = CH::begin(C + 1) - CH::begin(C);
-        for (int a = 0; a < 32; ++a) {
-            const int64_t ia = i0 + a;
-            if (ia >= N) break;
-            const float *src = dG + ia * (int64_t)F::N + CH::begin(C);
-            for (int f = lane; f < len; f += 32) sG[f * CW + a] = __ldg(&src[f]);
-        }
-        __syncwarp();
         contract_backward<NR, CH::mask(C)>(
-            [&](int s, int m) { return sP[(s * PSI + m) * CW + lane]; },
-            [&](int f) { return sG[(f - CH::begin(C)) * CW + lane]; },
+            [&](int s, int m) { return P[s][m]; },
+            [&](int f) { return buf[(f - CH::begin(C)) * TB + tid]; },
             [&](int s, int m, float v) { acc[s][m] += v; });
-        __syncwarp();
     };
-    run_chunk(std::integral_constant<int, 0>{});
-    run_chunk(std::integral_constant<int, 1>{});
-    run_chunk(std::integral_constant<int, 2>{});
-    run_chunk(std::integral_constant<int, 3>{});
-    run_chunk(std::integral_constant<int, 4>{});
+    tc::mbar_wait(barY, 0);
+    run_chunk(std::integral_constant<int, 0>{}, sY);
+    __syncthreads();
+    if (tid == 0) {
+        tc::fence_proxy_async_smem();
+        tc::mbar_arrive_expect_tx(barY, (uint32_t)(SM::len(2) * TB * 4));
+        issue(sY, 2, barY);
+    }
+    tc::mbar_wait(barX, 0);
+    run_chunk(std::integral_constant<int, 4>{}, sX);
+    __syncthreads();
+    if (tid == 0) {
+        tc::fence_proxy_async_smem();
+        tc::mbar_arrive_expect_tx(barX, (uint32_t)((SM::len(1) + SM::len(3)) * TB * 4));
+        issue(sX, 1, barX);
+        issue(sX + SM::len(1) * TB, 3, barX);
+    }
+    tc::mbar_wait(barY, 1);
+    run_chunk(std::integral_constant<int, 2>{}, sY);
+    tc::mbar_wait(barX, 1);
+    run_chunk(std::integral_constant<int, 1>{}, sX);
+    run_chunk(std::integral_constant<int, 3>{}, sX + SM::len(1) * TB);
+    __syncthreads();
 
-    // transpose the adjoints back through the (now free) Psi tile for contiguous stores
+    // transpose the adjoints through slot X (per-warp [NR*PSI][33] tiles) for contiguous row stores
+    float *sP = sX + wid * (NR * PSI * CW);
 #pragma unroll
     for (int s = 0; s < NR; ++s)
 #pragma unroll
         for (int m = 0; m < PSI; ++m) sP[(s * PSI + m) * CW + lane] = sig * acc[s][m];
     __syncwarp();
+    const int64_t i0 = i - lane;
     for (int a = 0; a < 32; ++a) {
         const int64_t ia = i0 + a;
         if (ia >= N) break;
@@ -559,13 +612,13 @@ int launch_contract_forward(gmnn_system *s, cudaStream_t st) {
 
 int launch_contract_backward(gmnn_system *s, cudaStream_t st) {
     constexpr int NR = 5;
-    const size_t smem = sizeof(float) * 2 * (NR * PSI + FeatChunks<NR>::max_len()) * CW;
+    const size_t smem = CbSmem<NR>::BYTES;
     static bool attr_set = false;
     if (!attr_set) {
         GMNN_CUDA(cudaFuncSetAttribute(k_contract_backward<NR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         attr_set = true;
     }
-    k_contract_backward<NR><<<nblocks(s->N, 64), 64, smem, st>>>(s->N, s->psi, s->dG, s->pos4, s->model->scale, s->A);
+    k_contract_backward<NR><<<nblocks(s->N, 128), 128, smem, st>>>(s->N, s->psi, s->dG, s->pos4, s->model->scale, s->A);
     GMNN_LAUNCHED();
     GMNN_CUDA(cudaGetLastError());
     return GMNN_OK;

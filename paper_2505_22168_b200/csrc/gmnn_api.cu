@@ -260,7 +260,7 @@ int gmnn_system_create(const gmnn_model *m, int64_t n_atoms, const int32_t *spec
     A_(s->count, N);
     A_(s->psi, N * m->hp.n_radial * PSI);
     A_(s->G, N * F);
-    A_(s->dG, N * F);
+    A_(s->dG, (N + 127) / 128 * 128 * F);  // tile-transposed [N/128][F][128] (mlp_*.cu EPI_PLAIN_T)
     A_(s->A, N * m->hp.n_radial * PSI);
     for (int l = 0; l < L; ++l) {
         A_(s->H[l], N * m->dims[l + 1]);
@@ -757,6 +757,15 @@ int gmnn_debug_read(gmnn_system *s, const char *name, void *dst, int64_t bytes) 
         return GMNN_INVALID_ARG;
     }
     GMNN_CUDA(cudaDeviceSynchronize());
+    if (!strcmp(name, "dG")) {  // stored as [N/128][F][128] tiles: hand back [N][F]
+        const int64_t F = m->n_features, tiles = (N + 127) / 128;
+        std::vector<float> tmp((size_t)(tiles * 128 * F));
+        GMNN_CUDA(cudaMemcpy(tmp.data(), src, tmp.size() * 4, cudaMemcpyDeviceToHost));
+        float *out = static_cast<float *>(dst);
+        for (int64_t i = 0; i < N; ++i)
+            for (int64_t f = 0; f < F; ++f) out[i * F + f] = tmp[(size_t)(((i >> 7) * F + f) * 128 + (i & 127))];
+        return GMNN_OK;
+    }
     GMNN_CUDA(cudaMemcpy(dst, src, (size_t)bytes, cudaMemcpyDeviceToHost));
     return GMNN_OK;
 }

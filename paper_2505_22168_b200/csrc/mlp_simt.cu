@@ -16,7 +16,7 @@
 
 namespace gmnn {
 
-enum { EPI_PLAIN = 0, EPI_HIDDEN = 1, EPI_MUL = 2 };
+enum { EPI_PLAIN = 0, EPI_HIDDEN = 1, EPI_MUL = 2, EPI_PLAIN_T = 3 };  // _T: C written as [M/128][N][128] tiles
 
 __device__ __forceinline__ void swish_pair(float z, float &h, float &d) {
     const float s = 1.f / (1.f + __expf(-z));
@@ -79,6 +79,17 @@ k_sgemm(int M, int N, int K, const float *__restrict__ A, int lda, const float *
         __syncthreads();
         cur ^= 1;
     }
+    if (EPI == EPI_PLAIN_T) {  // dG for contract_backward: tile-transposed, BM = 128 atoms per tile
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            const int col = n0 + (j < 4 ? tx * 4 + j : 64 + tx * 4 + (j - 4));
+            if (col >= N) continue;
+            float *ct = C + ((int64_t)blockIdx.y * N + col) * BM;
+            *reinterpret_cast<float4 *>(ct + ty * 4) = make_float4(acc[0][j], acc[1][j], acc[2][j], acc[3][j]);
+            *reinterpret_cast<float4 *>(ct + 64 + ty * 4) = make_float4(acc[4][j], acc[5][j], acc[6][j], acc[7][j]);
+        }
+        return;
+    }
 #pragma unroll
     for (int i = 0; i < 8; ++i) {
         const int row = m0 + (i < 4 ? ty * 4 + i : 64 + ty * 4 + (i - 4));
@@ -119,6 +130,7 @@ static int sgemm(int epi, int64_t M, int N, int K, const float *A, const float *
     switch (epi) {
         case EPI_PLAIN: k_sgemm<EPI_PLAIN><<<grid, 256, 0, st>>>((int)M, N, K, A, K, B, N, C, N, bias, C2, Dmul); break;
         case EPI_HIDDEN: k_sgemm<EPI_HIDDEN><<<grid, 256, 0, st>>>((int)M, N, K, A, K, B, N, C, N, bias, C2, Dmul); break;
+        case EPI_PLAIN_T: k_sgemm<EPI_PLAIN_T><<<grid, 256, 0, st>>>((int)M, N, K, A, K, B, N, C, N, bias, C2, Dmul); break;
         default: k_sgemm<EPI_MUL><<<grid, 256, 0, st>>>((int)M, N, K, A, K, B, N, C, N, bias, C2, Dmul); break;
     }
     GMNN_LAUNCHED();
@@ -241,7 +253,7 @@ int launch_mlp_backward_simt(gmnn_system *s, const float *head_w_dev, cudaStream
             Bop = m->WT[l - 1];
             cur ^= 1;
         } else {
-            rc = sgemm(EPI_PLAIN, s->N, m->dims[0], m->dims[1], Aop, Bop, s->dG, nullptr, nullptr, nullptr, st);
+            rc = sgemm(EPI_PLAIN_T, s->N, m->dims[0], m->dims[1], Aop, Bop, s->dG, nullptr, nullptr, nullptr, st);
             if (rc) return rc;
         }
     }

@@ -32,7 +32,7 @@ namespace gmnn {
 
 using namespace tc;
 
-enum { EPI_PLAIN = 0, EPI_HIDDEN = 1, EPI_MUL = 2 };
+enum { EPI_PLAIN = 0, EPI_HIDDEN = 1, EPI_MUL = 2, EPI_PLAIN_T = 3 };  // _T: C written as [M/128][N][128] tiles
 
 constexpr int TC_BM = 128;           // rows of A per tile = TMEM lanes
 constexpr int TC_BN_MAX = 256;       // columns per accumulator buffer
@@ -253,7 +253,10 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
                     // a 4-column group is either whole or absent: N and bn are multiples of 4
                     if (!row_ok || g >= n_groups || col0 + j >= p.N || g * 32 + j >= p.bn) continue;
                     float4 x = make_float4(acc[gi][j], acc[gi][j + 1], acc[gi][j + 2], acc[gi][j + 3]);
-                    if (EPI == EPI_HIDDEN) {
+                    if (EPI == EPI_PLAIN_T) {  // one column = 128 consecutive floats: a warp stores 128 B runs
+                        float *ct = p.C + ((int64_t)(m0 / TC_BM) * p.N + col0 + j) * TC_BM + quad * 32 + lane;
+                        ct[0] = x.x; ct[TC_BM] = x.y; ct[2 * TC_BM] = x.z; ct[3 * TC_BM] = x.w;
+                    } else if (EPI == EPI_HIDDEN) {
                         const float4 bb = __ldg(reinterpret_cast<const float4 *>(p.bias + col0 + j));
                         float4 h, d;
                         swish_pair_tc(x.x + bb.x, h.x, d.x);
@@ -382,6 +385,7 @@ int tc_gemm(bool split, int epi, int64_t M, int N, int K, const float *A, const 
     switch (epi) {                                                                        \
         case EPI_PLAIN: return tc_launch<SP, BKV, EPI_PLAIN>(tmA, tmB, a, st);             \
         case EPI_HIDDEN: return tc_launch<SP, BKV, EPI_HIDDEN>(tmA, tmB, a, st);           \
+        case EPI_PLAIN_T: return tc_launch<SP, BKV, EPI_PLAIN_T>(tmA, tmB, a, st);         \
         default: return tc_launch<SP, BKV, EPI_MUL>(tmA, tmB, a, st);                      \
     }
     if (!split) { TC_CASE(false, 32) }
@@ -422,7 +426,7 @@ int launch_mlp_backward_tc(gmnn_system *s, const float *head_w_dev, cudaStream_t
             BopT = m->W[l - 1];
             cur ^= 1;
         } else {
-            rc = tc_gemm(split, EPI_PLAIN, s->N, m->dims[0], m->dims[1], Aop, BopT, s->dG, nullptr, nullptr, nullptr, st);
+            rc = tc_gemm(split, EPI_PLAIN_T, s->N, m->dims[0], m->dims[1], Aop, BopT, s->dG, nullptr, nullptr, nullptr, st);
             if (rc) return rc;
         }
     }
