@@ -247,7 +247,7 @@ def run_ours(args):
     w = make_bench_workload(args.workload)
     N = w.n_atoms
     mlp = MLP_NAMES[args.mlp]
-    model = gm.Model(w.model, mlp_precision=mlp)
+    model = gm.Model(w.model, mlp_precision=mlp, force_mode={"gather": 0, "pairbuf": 1}[args.forces])
     sysm = gm.System(model, w.species)
     pos0 = torch.from_numpy(w.positions).to(dev)
     pos = pos0.clone()
@@ -369,7 +369,7 @@ def run_ours(args):
                       "tf32": "tf32 MLP, f32 elsewhere"}[args.mlp],
             "data": "synthetic",
             "config": {"workload": args.workload, "n_atoms": N, "what": w.name + ", NVE velocity Verlet, dt %.2f fs, skin %.1f"
-                       % (w.dt_fs, w.skin), "mlp": args.mlp, "hidden": list(w.model.hidden), "n_heads": w.model.n_heads,
+                       % (w.dt_fs, w.skin), "mlp": args.mlp, "forces": args.forces, "hidden": list(w.model.hidden), "n_heads": w.model.n_heads,
                        "neighbors_in_list_mean": round(nl_mean, 2), "rebuilds_in_timed_region": nreb,
                        "l2": "inputs_exceed_l2" if N >= 65536 else "working set of this small case is L2-resident",
                        "replicas": world},
@@ -394,6 +394,8 @@ def main():
     ap.add_argument("--workload", default="config5",
                     help="config5 (default, 1,048,576 atoms), config2, config3_<N>")
     ap.add_argument("--mlp", default="fp32", choices=sorted(MLP_NAMES))
+    ap.add_argument("--forces", default="pairbuf", choices=["gather", "pairbuf"],
+                    help="force reduction: gather form, or pair buffer with a reverse-pair index (both deterministic)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":

@@ -414,11 +414,15 @@ __device__ __forceinline__ void pair_gradient(AGet a, const float *R, const floa
     gz = radial * z + (wz - wu * z) * rinv;
 }
 
-template <int NR, int NB, int LPA>
+// PAIRBUF = false: gather form, both directions per entry, F_i complete.
+// PAIRBUF = true : own direction only; g_ij goes to gbuf[j][rev] (the slot of (i, -n) in the row of
+//                  j), f_int gets sum_j g_ij, and k_force_reduce subtracts the received row.
+template <int NR, int NB, int LPA, bool PAIRBUF>
 __global__ void __launch_bounds__(128)
 k_pair_backward(int64_t N, const float4 *__restrict__ pos4, const uint32_t *__restrict__ nbr,
                 const int32_t *__restrict__ count, int cap, Geometry geo, RadialParams rp,
-                const float *__restrict__ beta, const float *__restrict__ A, float *__restrict__ f_int) {
+                const float *__restrict__ beta, const float *__restrict__ A, float *__restrict__ f_int,
+                const uint16_t *__restrict__ rev, float4 *__restrict__ gbuf) {
     constexpr int KB = (NB + 3) & ~3;
     constexpr int ROW = NR * KB;
     constexpr int GROUPS = 128 / LPA;
@@ -448,13 +452,22 @@ k_pair_backward(int64_t N, const float4 *__restrict__ pos4, const uint32_t *__re
         const int cnt = count[i];
         const uint4 *row = reinterpret_cast<const uint4 *>(nbr + i * (int64_t)cap);
         const float4 *Ai = s_A + grp * (NR * PSI / 4);
+        const uint2 *rrow = reinterpret_cast<const uint2 *>(rev + (PAIRBUF ? i * (int64_t)cap : 0));
         for (int k4 = sub; k4 * 4 < cnt; k4 += LPA) {
             const uint4 e4 = __ldg(&row[k4]);
             const uint32_t ent[4] = {e4.x, e4.y, e4.z, e4.w};
+            uint32_t rv[4] = {0u, 0u, 0u, 0u};
+            if (PAIRBUF) {
+                const uint2 r2 = __ldg(&rrow[k4]);
+                rv[0] = r2.x & 0xFFFFu, rv[1] = r2.x >> 16, rv[2] = r2.y & 0xFFFFu, rv[3] = r2.y >> 16;
+            }
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
                 if (k4 * 4 + q >= cnt) break;
                 const PairGeom pg = pair_geometry(ent[q], xi, pos4, geo.L[0], geo.L[1], geo.L[2]);
+                if (PAIRBUF && rv[q] == 0xFFFFu) continue;  // no partner (overflowed rebuild): flagged by k_build_rev
+                float4 *slot = PAIRBUF ? gbuf + (int64_t)pg.j * cap + rv[q] : nullptr;
+                if (PAIRBUF && pg.r2 >= rp.r_cut2) *slot = make_float4(0.f, 0.f, 0.f, 0.f);  // skin shell
                 if (pg.r2 < rp.r_cut2) {
                     const float rinv = rsqrtf(pg.r2);
                     const float r = pg.r2 * rinv;
@@ -463,9 +476,9 @@ k_pair_backward(int64_t N, const float4 *__restrict__ pos4, const uint32_t *__re
                     const float ux = pg.dx * rinv, uy = pg.dy * rinv, uz = pg.dz * rinv;
                     float mono[PSI];
                     monomials(ux, uy, uz, mono);
-                    float gxo, gyo, gzo, gxr, gyr, gzr;
+                    float gxo, gyo, gzo, gxr = 0.f, gyr = 0.f, gzr = 0.f;
 #pragma unroll
-                    for (int dir = 0; dir < 2; ++dir) {
+                    for (int dir = 0; dir < (PAIRBUF ? 1 : 2); ++dir) {
                         // dir 0: centre i, table beta[zi][zj], adjoint A_i, direction +u
                         // dir 1: centre j, table beta[zj][zi], adjoint A_j, direction -u
                         const int za = dir == 0 ? zi : pg.zj, zb = dir == 0 ? pg.zj : zi;
@@ -497,6 +510,7 @@ k_pair_backward(int64_t N, const float4 *__restrict__ pos4, const uint32_t *__re
                                               ux, uy, uz, rinv, -1.f, gxr, gyr, gzr);
                         }
                     }
+                    if (PAIRBUF) *slot = make_float4(gxo, gyo, gzo, 0.f);
                     // F_i += g_ij - g_ji   (g_ji = dE_j/dd_ji, d_ji = -d_ij)
                     fx += gxo - gxr;
                     fy += gyo - gyr;
@@ -515,6 +529,37 @@ k_pair_backward(int64_t N, const float4 *__restrict__ pos4, const uint32_t *__re
         f_int[3 * i] = fx;
         f_int[3 * i + 1] = fy;
         f_int[3 * i + 2] = fz;
+    }
+}
+
+// a11 (pair-buffer form): F_i = sum_j g_ij (already in f_int) - sum_k gbuf[i][k], the g_ji received
+// from the neighbours, summed in slot order by LPA lanes (fixed order: bit-reproducible).
+template <int LPA>
+__global__ void __launch_bounds__(256)
+k_force_reduce(int64_t N, const int32_t *__restrict__ count, int cap, const float4 *__restrict__ gbuf,
+               float *__restrict__ f_int) {
+    const int64_t gt = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    const int64_t i = gt / LPA;
+    const int sub = (int)(gt % LPA);
+    float fx = 0.f, fy = 0.f, fz = 0.f;
+    if (i < N) {
+        const int cnt = count[i];
+        const float4 *row = gbuf + i * (int64_t)cap;
+        for (int k = sub; k < cnt; k += LPA) {
+            const float4 g = __ldcs(&row[k]);
+            fx += g.x, fy += g.y, fz += g.z;
+        }
+    }
+#pragma unroll
+    for (int o = LPA / 2; o >= 1; o >>= 1) {
+        fx += __shfl_xor_sync(0xffffffffu, fx, o);
+        fy += __shfl_xor_sync(0xffffffffu, fy, o);
+        fz += __shfl_xor_sync(0xffffffffu, fz, o);
+    }
+    if (i < N && sub == 0) {
+        f_int[3 * i] -= fx;
+        f_int[3 * i + 1] -= fy;
+        f_int[3 * i + 2] -= fz;
     }
 }
 
@@ -559,16 +604,27 @@ static int pair_backward_lpa(gmnn_system *s, cudaStream_t st, int lpa) {
     const int beta_floats = (m->rp.n_species * m->rp.n_species * NR * m->rp.kb + 3) & ~3;
     const size_t smem = sizeof(float) * (beta_floats + (128 / lpa) * NR * PSI);
     const unsigned grid = nblocks(s->N * lpa, 128);
+    const bool pairbuf = s->force_mode == GMNN_FORCE_PAIRBUF;
+    if (pairbuf && !(s->list_has_rev && s->rev && s->gbuf)) {
+        set_error("force_mode changed after the list was built: call gmnn_build_neighbors again");
+        return GMNN_INVALID_ARG;
+    }
 #define GMNN_PB(L)                                                                                         \
     case L: {                                                                                              \
         static size_t opted = 0;                                                                           \
         if (smem > 48 * 1024 && smem > opted) {                                                            \
-            GMNN_CUDA(cudaFuncSetAttribute(k_pair_backward<NR, NB, L>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
-                                           (int)smem));                                                    \
+            GMNN_CUDA(cudaFuncSetAttribute(k_pair_backward<NR, NB, L, false>,                              \
+                                           cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));       \
+            GMNN_CUDA(cudaFuncSetAttribute(k_pair_backward<NR, NB, L, true>,                               \
+                                           cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));       \
             opted = smem;                                                                                  \
         }                                                                                                  \
-        k_pair_backward<NR, NB, L><<<grid, 128, smem, st>>>(s->N, s->pos4, s->nbr, s->count, s->cap, s->geo, \
-                                                            m->rp, m->beta, s->A, s->f_int);               \
+        if (pairbuf)                                                                                       \
+            k_pair_backward<NR, NB, L, true><<<grid, 128, smem, st>>>(s->N, s->pos4, s->nbr, s->count, s->cap, s->geo, \
+                                                                  m->rp, m->beta, s->A, s->f_int, s->rev, s->gbuf); \
+        else                                                                                               \
+            k_pair_backward<NR, NB, L, false><<<grid, 128, smem, st>>>(s->N, s->pos4, s->nbr, s->count, s->cap, s->geo, \
+                                                                   m->rp, m->beta, s->A, s->f_int, nullptr, nullptr); \
     } break;
     switch (lpa) {
         GMNN_PB(1) GMNN_PB(2) GMNN_PB(4) GMNN_PB(8) GMNN_PB(16) GMNN_PB(32)
@@ -578,6 +634,10 @@ static int pair_backward_lpa(gmnn_system *s, cudaStream_t st, int lpa) {
     }
 #undef GMNN_PB
     GMNN_LAUNCHED();
+    if (pairbuf) {
+        k_force_reduce<8><<<nblocks(s->N * 8, 256), 256, 0, st>>>(s->N, s->count, s->cap, s->gbuf, s->f_int);
+        GMNN_LAUNCHED();
+    }
     GMNN_CUDA(cudaGetLastError());
     return GMNN_OK;
 }

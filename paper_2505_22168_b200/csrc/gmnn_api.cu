@@ -295,7 +295,7 @@ void gmnn_system_destroy(gmnn_system *s) {
     if (!s) return;
     dev_free(s->species); dev_free(s->cell_of); dev_free(s->cell_count); dev_free(s->cell_start);
     dev_free(s->cell_fill); dev_free(s->slot_tmp); dev_free(s->perm); dev_free(s->pos4); dev_free(s->xref);
-    dev_free(s->nbr); dev_free(s->count); dev_free(s->psi); dev_free(s->G); dev_free(s->dG); dev_free(s->A);
+    dev_free(s->nbr); dev_free(s->rev); dev_free(s->gbuf); dev_free(s->count); dev_free(s->psi); dev_free(s->G); dev_free(s->dG); dev_free(s->A);
     for (int l = 0; l < MAX_LAYERS; ++l) { dev_free(s->H[l]); dev_free(s->D[l]); }
     dev_free(s->dZ[0]); dev_free(s->dZ[1]); dev_free(s->Bv); dev_free(s->BvT); dev_free(s->vhead); dev_free(s->head_w);
     dev_free(s->e_heads); dev_free(s->e_atom); dev_free(s->f_int); dev_free(s->f_tmp); dev_free(s->partial);
@@ -330,6 +330,7 @@ int gmnn_system_set_int(gmnn_system *s, const char *key, int64_t v) {
         s->mlp_precision = (int)v;
     } else if (!strcmp(key, "force_mode")) {
         if (v < 0 || v > GMNN_FORCE_PAIRBUF) return GMNN_INVALID_ARG;
+        if (s->force_mode != (int)v) s->have_list = false;  // the reverse-pair index is built with the list
         s->force_mode = (int)v;
     } else if (!strcmp(key, "tc_split_bk")) {  // process-wide tuning knob of mlp_tc.cu
         if (v != 16 && v != 32) return GMNN_INVALID_ARG;
@@ -457,12 +458,23 @@ int gmnn_build_neighbors(gmnn_system *s, const float *positions, const float cel
             dev_free(s->nbr);
             s->cap = want;
             int rc = dev_alloc(&s->nbr, (size_t)s->N * s->cap);
+            dev_free(s->rev);
+            dev_free(s->gbuf);
             if (rc) {
                 set_error("out of device memory for the neighbour list (%lld x %d)", (long long)s->N, s->cap);
                 s->cap = 0;
                 return rc;
             }
         }
+        if (s->force_mode == GMNN_FORCE_PAIRBUF && !s->rev) {
+            int rc = dev_alloc(&s->rev, (size_t)s->N * s->cap);
+            if (!rc) rc = dev_alloc(&s->gbuf, (size_t)s->N * s->cap);
+            if (rc) {
+                set_error("out of device memory for the pair buffer (%lld x %d)", (long long)s->N, s->cap);
+                return rc;
+            }
+        }
+        s->list_has_rev = s->force_mode == GMNN_FORCE_PAIRBUF;
         GMNN_CUDA(cudaMemsetAsync(s->flags, 0, sizeof(int32_t) * FLAG_WORDS, st));
         int rc = launch_build(s, positions, st, nullptr, 0.f, false, nullptr);
         if (rc) return rc;
@@ -473,6 +485,11 @@ int gmnn_build_neighbors(gmnn_system *s, const float *positions, const float cel
             return GMNN_OUT_OF_BOX;
         }
         if (s->flags_host[FLAG_MAXCOUNT] <= s->cap) {
+            if (s->flags_host[FLAG_REV_MISSING]) {
+                s->have_list = false;
+                set_error("internal: the neighbour list is not symmetric (reverse pair missing)");
+                return GMNN_CUDA_ERROR;
+            }
             s->have_list = true;
             GMNN_CUDA(cudaMemsetAsync(s->flags, 0, sizeof(int32_t) * FLAG_WORDS, st));
             return GMNN_OK;
@@ -669,7 +686,12 @@ int gmnn_md_verlet_steps(gmnn_system *s, float *positions, float *velocities, co
     if ((rc = read_flags(s, st))) return rc;
     if (n_rebuilds) *n_rebuilds = s->flags_host[FLAG_REBUILDS];
     const int maxcount = s->flags_host[FLAG_MAXCOUNT];
+    const int rev_missing = s->flags_host[FLAG_REV_MISSING];
     GMNN_CUDA(cudaMemsetAsync(s->flags, 0, sizeof(int32_t) * FLAG_WORDS, st));
+    if (rev_missing && maxcount <= s->cap) {
+        set_error("internal: an in-loop rebuild produced a neighbour list that is not symmetric");
+        return GMNN_CUDA_ERROR;
+    }
     if (maxcount > s->cap) {
         set_error("an in-loop rebuild needed %d neighbour slots, capacity is %d: raise \"capacity\" and rerun", maxcount,
                   s->cap);

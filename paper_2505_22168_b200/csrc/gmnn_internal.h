@@ -24,7 +24,7 @@ constexpr int MAX_STAGE_EVENTS = 1 << 16;
 constexpr int PSI = 20;  // unique monomials per channel (contraction.cuh NM)
 
 // device-side flag words (int32) in System::flags
-enum Flag { FLAG_MAXCOUNT = 0, FLAG_STALE = 1, FLAG_OUT_OF_BOX = 2, FLAG_REBUILDS = 3, FLAG_DISP2 = 4, FLAG_WORDS = 8 };
+enum Flag { FLAG_MAXCOUNT = 0, FLAG_STALE = 1, FLAG_OUT_OF_BOX = 2, FLAG_REBUILDS = 3, FLAG_DISP2 = 4, FLAG_REV_MISSING = 5, FLAG_WORDS = 8 };
 
 void set_error(const char *fmt, ...);
 extern long long g_launch_count;
@@ -91,6 +91,9 @@ struct gmnn_system {
     // neighbour list
     uint32_t *nbr = nullptr;         // [N][cap]
     int32_t *count = nullptr;        // [N]
+    uint16_t *rev = nullptr;         // [N][cap] slot of the reverse pair (GMNN_FORCE_PAIRBUF)
+    float4 *gbuf = nullptr;          // [N][cap] g_ij, stored in the row of j at the reverse slot
+    bool list_has_rev = false;
     int cap = 0;
     int cap_request = 0;
     // workspaces (internal order)
@@ -134,7 +137,7 @@ int launch_gather_positions(gmnn_system *s, const float *positions, cudaStream_t
 int launch_pair_forward(gmnn_system *s, cudaStream_t st);
 int launch_contract_forward(gmnn_system *s, cudaStream_t st);
 int launch_contract_backward(gmnn_system *s, cudaStream_t st);
-int launch_pair_backward(gmnn_system *s, cudaStream_t st);
+int launch_pair_backward(gmnn_system *s, cudaStream_t st);  // dispatches on force_mode
 
 // mlp_simt.cu
 int launch_mlp_forward_simt(gmnn_system *s, cudaStream_t st);

@@ -246,6 +246,50 @@ k_build_small(int64_t N, const float4 *__restrict__ pos4, Geometry g, uint32_t *
     }
 }
 
+// Reverse-pair index for the pair-buffer force reduction (GMNN_FORCE_PAIRBUF): rev[i][k] = slot of
+// (i, -n) in the row of j, for entry k = (j, n) of row i.  The list is symmetric by construction
+// (the membership predicate is exactly odd under i <-> j, n -> -n), so every entry has a partner;
+// a missing one raises FLAG_REV_MISSING.  One warp per atom: each lane owns one entry of a batch of
+// 32, the warp scans the partner row 32 slots at a time.
+__global__ void __launch_bounds__(256)
+k_build_rev(int64_t N, const uint32_t *__restrict__ nbr, const int32_t *__restrict__ count, int cap, uint16_t *rev,
+            int32_t *flags, const int32_t *cond, float thr2) {
+    if (skip_rebuild(cond, thr2)) return;
+    const int lane = threadIdx.x & 31;
+    const int64_t i = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
+    if (i >= N) return;
+    const int cnt = count[i];
+    const uint32_t *row = nbr + i * (int64_t)cap;
+    for (int k0 = 0; k0 < cnt; k0 += 32) {
+        const uint32_t e_mine = k0 + lane < cnt ? row[k0 + lane] : 0u;
+        int found = 0xFFFF;
+        const int nk = cnt - k0 < 32 ? cnt - k0 : 32;
+        for (int t = 0; t < nk; ++t) {
+            const uint32_t e = __shfl_sync(0xffffffffu, e_mine, t);
+            const int64_t j = e & NBR_J_MASK;
+            const uint32_t img = e >> NBR_J_BITS;  // three 3-bit fields n + 4; the inverse image is 8 - field
+            const uint32_t inv = (8u - (img & 7u)) | ((8u - ((img >> 3) & 7u)) << 3) | ((8u - ((img >> 6) & 7u)) << 6);
+            const uint32_t target = (uint32_t)i | (inv << NBR_J_BITS);
+            const uint32_t *rj = nbr + j * (int64_t)cap;
+            const int cj = count[j];
+            int pos = 0xFFFF;
+            for (int b = 0; b < cj; b += 32) {
+                const bool hit = b + lane < cj && rj[b + lane] == target;
+                const unsigned m = __ballot_sync(0xffffffffu, hit);
+                if (m) {
+                    pos = b + __ffs(m) - 1;
+                    break;
+                }
+            }
+            if (lane == t) found = pos;
+        }
+        if (k0 + lane < cnt) {
+            rev[i * (int64_t)cap + k0 + lane] = (uint16_t)found;
+            if (found == 0xFFFF) flags[FLAG_REV_MISSING] = 1;
+        }
+    }
+}
+
 __global__ void k_finish_rebuild(int32_t *flags, const int32_t *cond, float thr2) {
     if (skip_rebuild(cond, thr2)) return;
     flags[FLAG_DISP2] = 0;
@@ -281,6 +325,10 @@ int launch_build(gmnn_system *s, const float *positions, cudaStream_t st, const 
         k_build_cells<<<nblocks(N * 32, 256), 256, 0, st>>>(N, s->pos4, s->cell_start, g, s->nbr, s->count, s->cap,
                                                             s->flags, cond, thr2);
     GMNN_LAUNCHED();
+    if (s->force_mode == GMNN_FORCE_PAIRBUF) {
+        k_build_rev<<<nblocks(N * 32, 256), 256, 0, st>>>(N, s->nbr, s->count, s->cap, s->rev, s->flags, cond, thr2);
+        GMNN_LAUNCHED();
+    }
     k_finish_rebuild<<<1, 1, 0, st>>>(s->flags, cond, thr2);
     GMNN_LAUNCHED();
     GMNN_CUDA(cudaGetLastError());

@@ -100,7 +100,8 @@ def test_md_trajectory_and_energy_conservation(gm, orc):
     assert drift_gpu <= 10 * drift_ref + 1e-3, (drift_gpu, drift_ref)
 
 
-def test_md_cell_list_rebuild_inside_the_loop(gm, orc):
+@pytest.mark.parametrize("force_mode", [0, 1])
+def test_md_cell_list_rebuild_inside_the_loop(gm, orc, force_mode):
     """Config-5-shaped (Li3PO4, skin 1, cell-list rebuild when max displacement > skin/2) at 8192
     atoms: hot velocities force several device-side rebuilds; the final state must match the oracle
     evaluated on the GPU's final positions and the list must equal a fresh build."""
@@ -108,7 +109,7 @@ def test_md_cell_list_rebuild_inside_the_loop(gm, orc):
 
     w = wl.li3po4_box(8192, hidden=(32, 32), skin=0.3)
     m = orc.Model(w.model)
-    _, sysm, pos = _build(gm, w)
+    _, sysm, pos = _build(gm, w, force_mode=force_mode)  # 1: the reverse-pair index is rebuilt in the loop too
     vel = torch.from_numpy(w.velocities * 8.0).cuda()
     mass = torch.from_numpy(w.masses).cuda()
     epot, ekin, nreb = sysm.md_verlet_steps(pos, vel, mass, w.dt_fs, 40)

@@ -233,3 +233,31 @@ def test_single_atom_and_isolated_atoms(gm, orc):
         ref = orc.energy_forces(m, pos[:n], species[:n], [60, 60, 60], orc.neighbors(pos[:n], [60, 60, 60], (1, 1, 1), 6.0))
         assert np.all(f.cpu().numpy() == 0)
         assert np.allclose(ea.cpu().numpy(), ref.e_atom, rtol=1e-5)
+
+
+# ------------------------------------------------------------------ pair-buffer force reduction
+@pytest.mark.parametrize("name", ["config1", "config2", "config3_1024", "config3_8192", "cluster", "ragged"])
+def test_pair_buffer_force_mode(gm, orc, name):
+    """GMNN_FORCE_PAIRBUF: g_ij evaluated once per directed pair and delivered through the
+    reverse-pair index; same tolerances as the gather form, bit-reproducible, and the two forms
+    agree to round-off.  config1 has duplicate-by-image pairs and self images, cluster no PBC."""
+    if name == "cluster":
+        w = wl.cluster(24, 2)
+    elif name == "ragged":
+        w = wl.li3po4_box(1000, hidden=(64, 48), skin=0.7)
+    else:
+        w = wl.make_workload(name)
+    sysm, pos, ref = _check_energy_forces(gm, orc, w, force_mode=gm.GMNN_FORCE_PAIRBUF)
+    e1, ea1, f1 = sysm.energy_forces(pos)
+    e2, ea2, f2 = sysm.energy_forces(pos)
+    assert np.array_equal(f1.cpu().numpy(), f2.cpu().numpy())
+    _, sysg, _ = _gpu_system(gm, w)
+    _, _, fg = sysg.energy_forces(pos)
+    assert force_error(f1.cpu().numpy().astype(np.float64), fg.cpu().numpy().astype(np.float64)) <= 2e-5
+    # switching the mode on a built system asks for a rebuild instead of using a stale index
+    sysg.set_int("force_mode", gm.GMNN_FORCE_PAIRBUF)
+    with pytest.raises(gm.GmnnError):
+        sysg.energy_forces(pos)
+    sysg.build_neighbors(pos, w.cell9, w.pbc, w.model.r_cut, w.skin)
+    _, _, fp = sysg.energy_forces(pos)
+    assert np.array_equal(fp.cpu().numpy(), f1.cpu().numpy())
