@@ -139,6 +139,7 @@ class Model:
         hp = _HParams()
         hp.n_species, hp.n_basis, hp.n_radial, hp.l_max = spec.n_species, spec.n_basis, spec.n_radial, l_max
         hp.r_cut, hp.r_min, hp.gauss_gamma = spec.r_cut, spec.r_min, spec.gamma
+        self.hidden = tuple(int(h) for h in spec.hidden)
         hp.n_hidden = len(spec.hidden)
         for l, h in enumerate(spec.hidden[:4]):
             hp.hidden[l] = int(h)
@@ -304,6 +305,7 @@ class System:
             "psi": ((N, m.n_radial, 20), np.float32), "A": ((N, m.n_radial, 20), np.float32),
             "G": ((N, m.n_features), np.float32), "dG": ((N, m.n_features), np.float32),
             "e_heads": ((N, m.n_heads), np.float32),
+            "H0": ((N, m.hidden[0]), np.float32), "D0": ((N, m.hidden[0]), np.float32),
         }
         shape, dt = shapes[name]
         out = np.empty(shape, dt)

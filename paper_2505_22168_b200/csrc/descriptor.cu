@@ -200,14 +200,9 @@ constexpr int CW = 33;  // padded warp tile pitch
 
 template <int NR>
 __global__ void __launch_bounds__(128)
-k_contract_forward(int64_t N, const float *__restrict__ psi, float *__restrict__ G) {
+k_contract_forward(int64_t N, const float *__restrict__ psi, float *__restrict__ Gt) {
     using F = Feat<NR>;
-    using CH = FeatChunks<NR>;
-    extern __shared__ float s_tile[];
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    float *tile = s_tile + wid * (CH::max_len() * CW);
-    const int64_t i0 = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) - lane;  // first atom of the warp
-    const int64_t i = i0 + lane;
+    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;  // blockDim.x == 128 == tile
     float P[NR][PSI];
     if (i < N) {
         const float4 *src = reinterpret_cast<const float4 *>(psi + i * (int64_t)(NR * PSI));
@@ -225,26 +220,10 @@ k_contract_forward(int64_t N, const float *__restrict__ psi, float *__restrict__
 #pragma unroll
             for (int m = 0; m < PSI; ++m) P[s][m] = 0.f;
     }
-    // One pass per chunk of feature blocks (blocks 0-3 | 4 | 5 | 6 | 7), selected at compile time.
-    auto run_chunk = [&](auto chunk_tag) {
-        constexpr int C = decltype(chunk_tag)::value;
-        contract_forward<NR, CH::mask(C)>([&](int s, int m) { return P[s][m]; },
-                                          [&](int f, float v) { tile[(f - CH::begin(C)) * CW + lane] = v; });
-        __syncwarp();
-        constexpr int len = CH::begin(C + 1) - CH::begin(C);
-        for (int a = 0; a < 32; ++a) {
-            const int64_t ia = i0 + a;
-            if (ia >= N) break;
-            float *dst = G + ia * (int64_t)F::N + CH::begin(C);
-            for (int f = lane; f < len; f += 32) dst[f] = tile[f * CW + a];
-        }
-        __syncwarp();
-    };
-    run_chunk(std::integral_constant<int, 0>{});
-    run_chunk(std::integral_constant<int, 1>{});
-    run_chunk(std::integral_constant<int, 2>{});
-    run_chunk(std::integral_constant<int, 3>{});
-    run_chunk(std::integral_constant<int, 4>{});
+    // G is tile-transposed ([N/128][F][128], the A-operand layout of the MLP): feature f of the 128
+    // atoms of this block is one contiguous 512-byte run, so every store below is coalesced.
+    float *g = Gt + (int64_t)blockIdx.x * F::N * 128 + threadIdx.x;
+    contract_forward<NR>([&](int s, int m) { return P[s][m]; }, [&](int f, float v) { g[(int64_t)f * 128] = v; });
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -658,13 +637,7 @@ int launch_pair_backward(gmnn_system *s, cudaStream_t st) {
 
 int launch_contract_forward(gmnn_system *s, cudaStream_t st) {
     constexpr int NR = 5;
-    const size_t smem = sizeof(float) * 4 * FeatChunks<NR>::max_len() * CW;
-    static bool attr_set = false;
-    if (!attr_set) {
-        GMNN_CUDA(cudaFuncSetAttribute(k_contract_forward<NR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_set = true;
-    }
-    k_contract_forward<NR><<<nblocks(s->N, 128), 128, smem, st>>>(s->N, s->psi, s->G);
+    k_contract_forward<NR><<<nblocks(s->N, 128), 128, 0, st>>>(s->N, s->psi, s->G);
     GMNN_LAUNCHED();
     GMNN_CUDA(cudaGetLastError());
     return GMNN_OK;

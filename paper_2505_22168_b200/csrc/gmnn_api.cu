@@ -23,7 +23,7 @@ void set_error(const char *fmt, ...) {
 }
 
 int launch_mlp_forward_tc(gmnn_system *s, cudaStream_t st);
-extern int g_tc_split_bk, g_tc_flush_k;
+extern int g_tc_split_bk, g_tc_flush_k, g_tc_debug;
 int launch_mlp_backward_tc(gmnn_system *s, const float *head_w_dev, cudaStream_t st);
 
 template <class T>
@@ -259,15 +259,17 @@ int gmnn_system_create(const gmnn_model *m, int64_t n_atoms, const int32_t *spec
     A_(s->xref, 3 * N);
     A_(s->count, N);
     A_(s->psi, N * m->hp.n_radial * PSI);
-    A_(s->G, N * F);
-    A_(s->dG, (N + 127) / 128 * 128 * F);  // tile-transposed [N/128][F][128] (mlp_*.cu EPI_PLAIN_T)
+    // every matrix of the MLP is tile-transposed, [N/128][width][128], padded to whole tiles (mlp_tc.cu)
+    const size_t NP = (size_t)((N + 127) / 128 * 128);
+    A_(s->G, NP * F);
+    A_(s->dG, NP * F);
     A_(s->A, N * m->hp.n_radial * PSI);
     for (int l = 0; l < L; ++l) {
-        A_(s->H[l], N * m->dims[l + 1]);
-        A_(s->D[l], N * m->dims[l + 1]);
+        A_(s->H[l], NP * m->dims[l + 1]);
+        A_(s->D[l], NP * m->dims[l + 1]);
     }
-    A_(s->dZ[0], N * maxw);
-    A_(s->dZ[1], N * maxw);
+    A_(s->dZ[0], NP * maxw);
+    A_(s->dZ[1], NP * maxw);
     A_(s->Bv, (size_t)m->dims[L] * m->dims[L - 1]);
     A_(s->BvT, (size_t)m->dims[L] * m->dims[L - 1]);
     A_(s->vhead, (size_t)m->dims[L]);
@@ -282,6 +284,7 @@ int gmnn_system_create(const gmnn_model *m, int64_t n_atoms, const int32_t *spec
 #undef A_
     if (!rc && cudaMallocHost((void **)&s->flags_host, sizeof(int32_t) * FLAG_WORDS) != cudaSuccess) rc = GMNN_OOM;
     if (!rc && cudaMemset(s->flags, 0, sizeof(int32_t) * FLAG_WORDS) != cudaSuccess) rc = GMNN_CUDA_ERROR;
+    if (!rc && cudaMemset(s->G, 0, sizeof(float) * NP * F) != cudaSuccess) rc = GMNN_CUDA_ERROR;  // rows of the ragged last tile
     if (rc) {
         if (rc == GMNN_OOM) set_error("out of device memory allocating the workspaces of %lld atoms", (long long)n_atoms);
         gmnn_system_destroy(s);
@@ -335,6 +338,8 @@ int gmnn_system_set_int(gmnn_system *s, const char *key, int64_t v) {
     } else if (!strcmp(key, "tc_split_bk")) {  // process-wide tuning knob of mlp_tc.cu
         if (v != 16 && v != 32) return GMNN_INVALID_ARG;
         gmnn::g_tc_split_bk = (int)v;
+    } else if (!strcmp(key, "tc_debug")) {  // timing experiments (wrong results), see mlp_tc.cu
+        gmnn::g_tc_debug = (int)v;
     } else if (!strcmp(key, "tc_flush_k")) {
         if (v < 16 || v > 4096 || v % 16) return GMNN_INVALID_ARG;
         gmnn::g_tc_flush_k = (int)v;
@@ -770,6 +775,8 @@ int gmnn_debug_read(gmnn_system *s, const char *name, void *dst, int64_t bytes) 
     else if (!strcmp(name, "G")) { src = s->G; need = 4 * N * m->n_features; }
     else if (!strcmp(name, "dG")) { src = s->dG; need = 4 * N * m->n_features; }
     else if (!strcmp(name, "e_heads")) { src = s->e_heads; need = 4 * N * m->hp.n_heads; }
+    else if (!strcmp(name, "H0")) { src = s->H[0]; need = 4 * N * m->dims[1]; }
+    else if (!strcmp(name, "D0")) { src = s->D[0]; need = 4 * N * m->dims[1]; }
     else {
         set_error("gmnn_debug_read: unknown array '%s'", name);
         return GMNN_INVALID_ARG;
@@ -779,8 +786,9 @@ int gmnn_debug_read(gmnn_system *s, const char *name, void *dst, int64_t bytes) 
         return GMNN_INVALID_ARG;
     }
     GMNN_CUDA(cudaDeviceSynchronize());
-    if (!strcmp(name, "dG")) {  // stored as [N/128][F][128] tiles: hand back [N][F]
-        const int64_t F = m->n_features, tiles = (N + 127) / 128;
+    if (!strcmp(name, "dG") || !strcmp(name, "G") || !strcmp(name, "H0") || !strcmp(name, "D0")) {
+        // stored as [N/128][F][128] tiles: hand back [N][F]
+        const int64_t F = need / (4 * N), tiles = (N + 127) / 128;
         std::vector<float> tmp((size_t)(tiles * 128 * F));
         GMNN_CUDA(cudaMemcpy(tmp.data(), src, tmp.size() * 4, cudaMemcpyDeviceToHost));
         float *out = static_cast<float *>(dst);

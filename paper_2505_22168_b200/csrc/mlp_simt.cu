@@ -16,7 +16,7 @@
 
 namespace gmnn {
 
-enum { EPI_PLAIN = 0, EPI_HIDDEN = 1, EPI_MUL = 2, EPI_PLAIN_T = 3 };  // _T: C written as [M/128][N][128] tiles
+enum { EPI_PLAIN = 0, EPI_HIDDEN = 1, EPI_MUL = 2 };
 
 __device__ __forceinline__ void swish_pair(float z, float &h, float &d) {
     const float s = 1.f / (1.f + __expf(-z));
@@ -26,19 +26,21 @@ __device__ __forceinline__ void swish_pair(float z, float &h, float &d) {
 
 constexpr int BM = 128, BN = 128, BK = 8, APITCH = 132;
 
+// C = A . B with A, C, C2, Dmul tile-transposed ([M/128][cols][128], padded to whole tiles, the layout
+// every MLP matrix uses: see mlp_tc.cu) and B = W[l] row-major [K][N].
 template <int EPI>
 __global__ void __launch_bounds__(256)
-k_sgemm(int M, int N, int K, const float *__restrict__ A, int lda, const float *__restrict__ B, int ldb,
-        float *__restrict__ C, int ldc, const float *__restrict__ bias, float *__restrict__ C2,
-        const float *__restrict__ Dmul) {
+k_sgemm(int M, int N, int K, const float *__restrict__ At, const float *__restrict__ B, int ldb,
+        float *__restrict__ Ct, const float *__restrict__ bias, float *__restrict__ C2t,
+        const float *__restrict__ Dmult) {
     __shared__ __align__(16) float As[2][BK][APITCH];
     __shared__ __align__(16) float Bs[2][BK][BN];
     const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
-    const int m0 = blockIdx.y * BM, n0 = blockIdx.x * BN;
-    const int ar = tid >> 1, ak = (tid & 1) * 4;   // A tile: row, k offset of this thread's float4
+    const int n0 = blockIdx.x * BN;
+    const int ak = tid >> 5, ar = (tid & 31) * 4;  // A tile: k row, first of this thread's 4 atoms
     const int bk = tid >> 5, bc = (tid & 31) * 4;  // B tile: k row, column of this thread's float4
-    const bool a_ok = (m0 + ar) < M, b_ok = (n0 + bc) < N;
-    const float *Ap = A + (int64_t)(m0 + ar) * lda + ak;
+    const bool b_ok = (n0 + bc) < N;
+    const float *Ap = At + ((int64_t)blockIdx.y * K + ak) * BM + ar;
     const float *Bp = B + (int64_t)bk * ldb + n0 + bc;
     float acc[8][8];
 #pragma unroll
@@ -47,15 +49,15 @@ k_sgemm(int M, int N, int K, const float *__restrict__ A, int lda, const float *
         for (int j = 0; j < 8; ++j) acc[i][j] = 0.f;
 
     const int nk = K / BK;
-    float4 ra = a_ok ? __ldg(reinterpret_cast<const float4 *>(Ap)) : make_float4(0.f, 0.f, 0.f, 0.f);
+    float4 ra = __ldg(reinterpret_cast<const float4 *>(Ap));
     float4 rb = b_ok ? __ldg(reinterpret_cast<const float4 *>(Bp)) : make_float4(0.f, 0.f, 0.f, 0.f);
-    As[0][ak + 0][ar] = ra.x; As[0][ak + 1][ar] = ra.y; As[0][ak + 2][ar] = ra.z; As[0][ak + 3][ar] = ra.w;
+    *reinterpret_cast<float4 *>(&As[0][ak][ar]) = ra;
     *reinterpret_cast<float4 *>(&Bs[0][bk][bc]) = rb;
     __syncthreads();
     int cur = 0;
     for (int kt = 0; kt < nk; ++kt) {
         if (kt + 1 < nk) {
-            ra = a_ok ? __ldg(reinterpret_cast<const float4 *>(Ap + (int64_t)(kt + 1) * BK)) : make_float4(0.f, 0.f, 0.f, 0.f);
+            ra = __ldg(reinterpret_cast<const float4 *>(Ap + (int64_t)(kt + 1) * BK * BM));
             rb = b_ok ? __ldg(reinterpret_cast<const float4 *>(Bp + (int64_t)(kt + 1) * BK * ldb)) : make_float4(0.f, 0.f, 0.f, 0.f);
         }
 #pragma unroll
@@ -73,48 +75,36 @@ k_sgemm(int M, int N, int K, const float *__restrict__ A, int lda, const float *
         }
         if (kt + 1 < nk) {
             const int nx = cur ^ 1;
-            As[nx][ak + 0][ar] = ra.x; As[nx][ak + 1][ar] = ra.y; As[nx][ak + 2][ar] = ra.z; As[nx][ak + 3][ar] = ra.w;
+            *reinterpret_cast<float4 *>(&As[nx][ak][ar]) = ra;
             *reinterpret_cast<float4 *>(&Bs[nx][bk][bc]) = rb;
         }
         __syncthreads();
         cur ^= 1;
     }
-    if (EPI == EPI_PLAIN_T) {  // dG for contract_backward: tile-transposed, BM = 128 atoms per tile
+    // this thread holds atoms ty*4..+3 and 64+ty*4..+3 of the tile: float4 runs along the atom axis
 #pragma unroll
-        for (int j = 0; j < 8; ++j) {
-            const int col = n0 + (j < 4 ? tx * 4 + j : 64 + tx * 4 + (j - 4));
-            if (col >= N) continue;
-            float *ct = C + ((int64_t)blockIdx.y * N + col) * BM;
-            *reinterpret_cast<float4 *>(ct + ty * 4) = make_float4(acc[0][j], acc[1][j], acc[2][j], acc[3][j]);
-            *reinterpret_cast<float4 *>(ct + 64 + ty * 4) = make_float4(acc[4][j], acc[5][j], acc[6][j], acc[7][j]);
-        }
-        return;
-    }
+    for (int j = 0; j < 8; ++j) {
+        const int col = n0 + (j < 4 ? tx * 4 + j : 64 + tx * 4 + (j - 4));
+        if (col >= N) continue;
+        const float bb = EPI == EPI_HIDDEN ? __ldg(bias + col) : 0.f;
 #pragma unroll
-    for (int i = 0; i < 8; ++i) {
-        const int row = m0 + (i < 4 ? ty * 4 + i : 64 + ty * 4 + (i - 4));
-        if (row >= M) continue;
-#pragma unroll
-        for (int jh = 0; jh < 2; ++jh) {
-            const int col = n0 + jh * 64 + tx * 4;
-            if (col >= N) continue;
-            float4 v = make_float4(acc[i][jh * 4 + 0], acc[i][jh * 4 + 1], acc[i][jh * 4 + 2], acc[i][jh * 4 + 3]);
-            const int64_t o = (int64_t)row * ldc + col;
+        for (int ih = 0; ih < 2; ++ih) {
+            const int64_t o = ((int64_t)blockIdx.y * N + col) * BM + ih * 64 + ty * 4;
+            float4 v = make_float4(acc[ih * 4 + 0][j], acc[ih * 4 + 1][j], acc[ih * 4 + 2][j], acc[ih * 4 + 3][j]);
             if (EPI == EPI_HIDDEN) {
-                const float4 bb = __ldg(reinterpret_cast<const float4 *>(bias + col));
                 float4 h, d;
-                swish_pair(v.x + bb.x, h.x, d.x);
-                swish_pair(v.y + bb.y, h.y, d.y);
-                swish_pair(v.z + bb.z, h.z, d.z);
-                swish_pair(v.w + bb.w, h.w, d.w);
-                *reinterpret_cast<float4 *>(C + o) = h;
-                *reinterpret_cast<float4 *>(C2 + o) = d;
+                swish_pair(v.x + bb, h.x, d.x);
+                swish_pair(v.y + bb, h.y, d.y);
+                swish_pair(v.z + bb, h.z, d.z);
+                swish_pair(v.w + bb, h.w, d.w);
+                *reinterpret_cast<float4 *>(Ct + o) = h;
+                *reinterpret_cast<float4 *>(C2t + o) = d;
             } else if (EPI == EPI_MUL) {
-                const float4 dm = __ldg(reinterpret_cast<const float4 *>(Dmul + o));
+                const float4 dm = __ldg(reinterpret_cast<const float4 *>(Dmult + o));
                 v.x *= dm.x; v.y *= dm.y; v.z *= dm.z; v.w *= dm.w;
-                *reinterpret_cast<float4 *>(C + o) = v;
+                *reinterpret_cast<float4 *>(Ct + o) = v;
             } else {
-                *reinterpret_cast<float4 *>(C + o) = v;
+                *reinterpret_cast<float4 *>(Ct + o) = v;
             }
         }
     }
@@ -128,47 +118,50 @@ static int sgemm(int epi, int64_t M, int N, int K, const float *A, const float *
     }
     dim3 grid((N + BN - 1) / BN, (unsigned)((M + BM - 1) / BM));
     switch (epi) {
-        case EPI_PLAIN: k_sgemm<EPI_PLAIN><<<grid, 256, 0, st>>>((int)M, N, K, A, K, B, N, C, N, bias, C2, Dmul); break;
-        case EPI_HIDDEN: k_sgemm<EPI_HIDDEN><<<grid, 256, 0, st>>>((int)M, N, K, A, K, B, N, C, N, bias, C2, Dmul); break;
-        case EPI_PLAIN_T: k_sgemm<EPI_PLAIN_T><<<grid, 256, 0, st>>>((int)M, N, K, A, K, B, N, C, N, bias, C2, Dmul); break;
-        default: k_sgemm<EPI_MUL><<<grid, 256, 0, st>>>((int)M, N, K, A, K, B, N, C, N, bias, C2, Dmul); break;
+        case EPI_PLAIN: k_sgemm<EPI_PLAIN><<<grid, 256, 0, st>>>((int)M, N, K, A, B, N, C, bias, C2, Dmul); break;
+        case EPI_HIDDEN: k_sgemm<EPI_HIDDEN><<<grid, 256, 0, st>>>((int)M, N, K, A, B, N, C, bias, C2, Dmul); break;
+        default: k_sgemm<EPI_MUL><<<grid, 256, 0, st>>>((int)M, N, K, A, B, N, C, bias, C2, Dmul); break;
     }
     GMNN_LAUNCHED();
     GMNN_CUDA(cudaGetLastError());
     return GMNN_OK;
 }
 
-// One warp per atom: y_m = h . W_last[:, m] + b_last[m]; E^(m) = sigma y_m + mu; e_atom = sum_m c_m E^(m).
-__global__ void __launch_bounds__(256)
-k_heads(int64_t N, const float *__restrict__ H, int Hd, const float *__restrict__ Wl, const float *__restrict__ bl,
+// One thread per atom, H tile-transposed (coalesced along atoms): y_m = h . W_last[:, m] + b_last[m];
+// E^(m) = sigma y_m + mu; e_atom = sum_m c_m E^(m).  Heads are taken 8 at a time.
+__global__ void __launch_bounds__(128)
+k_heads(int64_t N, const float *__restrict__ Ht, int Hd, const float *__restrict__ Wl, const float *__restrict__ bl,
         int M, const float4 *__restrict__ pos4, const float *__restrict__ scale, const float *__restrict__ shift,
         const float *__restrict__ head_w, float *__restrict__ e_heads, float *__restrict__ e_atom) {
-    const int lane = threadIdx.x & 31;
-    const int64_t i = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
+    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;  // blockDim.x == 128 == tile
     if (i >= N) return;
-    float h[32];
-#pragma unroll
-    for (int q = 0; q < 32; ++q) {
-        const int k = lane + 32 * q;
-        h[q] = k < Hd ? __ldg(&H[i * (int64_t)Hd + k]) : 0.f;
-    }
+    const float *h = Ht + (int64_t)blockIdx.x * Hd * 128 + threadIdx.x;
     const int z = __float_as_int(pos4[i].w);
     const float sg = __ldg(&scale[z]), mu = __ldg(&shift[z]);
     float e = 0.f;
-    for (int m = 0; m < M; ++m) {
-        float p = 0.f;
+    for (int m0 = 0; m0 < M; m0 += 8) {
+        float p[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+        const int nm = M - m0 < 8 ? M - m0 : 8;
+        if (nm == 1) {
+#pragma unroll 8
+            for (int k = 0; k < Hd; ++k) p[0] = fmaf(__ldg(h + (int64_t)k * 128), __ldg(&Wl[(int64_t)k * M + m0]), p[0]);
+        } else {
+            for (int k = 0; k < Hd; ++k) {
+                const float hv = __ldg(h + (int64_t)k * 128);
 #pragma unroll
-        for (int q = 0; q < 32; ++q) {
-            const int k = lane + 32 * q;
-            if (k < Hd) p = fmaf(h[q], __ldg(&Wl[(int64_t)k * M + m]), p);
+                for (int c = 0; c < 8; ++c)
+                    if (c < nm) p[c] = fmaf(hv, __ldg(&Wl[(int64_t)k * M + m0 + c]), p[c]);
+            }
         }
 #pragma unroll
-        for (int o = 16; o >= 1; o >>= 1) p += __shfl_xor_sync(0xffffffffu, p, o);
-        const float em = sg * (p + __ldg(&bl[m])) + mu;
-        if (lane == 0) e_heads[i * (int64_t)M + m] = em;
-        e = fmaf(__ldg(&head_w[m]), em, e);
+        for (int c = 0; c < 8; ++c)
+            if (c < nm) {
+                const float em = sg * (p[c] + __ldg(&bl[m0 + c])) + mu;
+                e_heads[i * (int64_t)M + m0 + c] = em;
+                e = fmaf(__ldg(&head_w[m0 + c]), em, e);
+            }
     }
-    if (lane == 0) e_atom[i] = e;
+    e_atom[i] = e;
 }
 
 // v[k] = sum_m c_m W_last[k][m]
@@ -212,7 +205,7 @@ int launch_mlp_heads(gmnn_system *s, const float *head_w_dev, cudaStream_t st) {
         set_error("last hidden width > 1024");
         return GMNN_UNSUPPORTED;
     }
-    k_heads<<<(unsigned)((s->N * 32 + 255) / 256), 256, 0, st>>>(s->N, s->H[L - 1], m->dims[L], m->W[L], m->b[L],
+    k_heads<<<(unsigned)((s->N + 127) / 128), 128, 0, st>>>(s->N, s->H[L - 1], m->dims[L], m->W[L], m->b[L],
                                                                  m->dims[L + 1], s->pos4, m->scale, m->shift, head_w_dev,
                                                                  s->e_heads, s->e_atom);
     GMNN_LAUNCHED();
@@ -253,7 +246,7 @@ int launch_mlp_backward_simt(gmnn_system *s, const float *head_w_dev, cudaStream
             Bop = m->WT[l - 1];
             cur ^= 1;
         } else {
-            rc = sgemm(EPI_PLAIN_T, s->N, m->dims[0], m->dims[1], Aop, Bop, s->dG, nullptr, nullptr, nullptr, st);
+            rc = sgemm(EPI_PLAIN, s->N, m->dims[0], m->dims[1], Aop, Bop, s->dG, nullptr, nullptr, nullptr, st);
             if (rc) return rc;
         }
     }

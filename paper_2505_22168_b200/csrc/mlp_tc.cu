@@ -32,7 +32,7 @@ namespace gmnn {
 
 using namespace tc;
 
-enum { EPI_PLAIN = 0, EPI_HIDDEN = 1, EPI_MUL = 2, EPI_PLAIN_T = 3 };  // _T: C written as [M/128][N][128] tiles
+enum { EPI_PLAIN = 0, EPI_HIDDEN = 1, EPI_MUL = 2 };
 
 constexpr int TC_BM = 128;           // rows of A per tile = TMEM lanes
 constexpr int TC_BN_MAX = 256;       // columns per accumulator buffer
@@ -59,6 +59,7 @@ struct TcArgs {
     int n_tiles_n;
     int n_tiles;   // total
     int flush;     // pipeline stages per accumulator flush (K chunk = flush * BK)
+    int debug;     // timing experiments only (results wrong): 1 skip split work, 2 hi.hi MMA only, 4 skip stores
     float *C;      // [M][N]
     float *C2;     // EPI_HIDDEN: swish'(z)
     const float *bias;
@@ -128,13 +129,14 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
                     const int s = it % NST;
                     mbar_wait(bar_empty(s), ((it / NST) & 1) ^ 1);
                     mbar_arrive_expect_tx(bar_full(s), tx);
-                    tma_load_2d(a_hi(s), &tmA, bar_full(s), kb * BK, m0);
+                    for (int q = 0; q < 4; ++q)  // four 32-atom column blocks of the tile, [BK][32 floats] each
+                        tma_load_2d(a_hi(s) + q * (BK * 128), &tmA, bar_full(s), q * 32, (m0 / TC_BM) * p.K + kb * BK);
                     tma_load_2d(b_hi(s), &tmB, bar_full(s), kb * BK, n0);
                 }
             }
         } else if (warp == 1 && lane == 0) {
             // ===== MMA issuer =====
-            const uint32_t idesc = make_idesc_tf32(TC_BM, p.bn);
+            const uint32_t idesc = make_idesc_tf32(TC_BM, p.bn, true);
             uint32_t it = 0, chunk = 0;
             for (int t = blockIdx.x; t < p.n_tiles; t += gridDim.x) {
                 for (int kb = 0; kb < nkb; ++kb, ++it) {
@@ -148,22 +150,28 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
                     const int s = it % NST;
                     mbar_wait(SPLIT ? bar_split(s) : bar_full(s), (it / NST) & 1);
                     tcgen05_fence_after();
+                    if ((p.debug & 64) && it == 0 && blockIdx.x == 0) {
+                        const float *fa = reinterpret_cast<const float *>(smem_gen + (size_t)s * Cfg::STAGE_BYTES);
+                        const float *fb = reinterpret_cast<const float *>(smem_gen + (size_t)s * Cfg::STAGE_BYTES + Cfg::A_BYTES * (SPLIT ? 2 : 1));
+                        printf("A smem: %g %g %g %g | %g %g | B smem: %g %g %g %g K=%d bn=%d M=%d\n", fa[0], fa[1], fa[2], fa[3], fa[32], fa[1024], fb[0], fb[1], fb[2], fb[3], p.K, p.bn, p.M);
+                    }
                     const int krem = p.K - kb * BK;
                     const int ksteps = krem >= BK ? BK / 8 : (krem + 7) / 8;
-                    const uint64_t da_hi = make_smem_desc<Cfg::SWZ>(a_hi(s)), db_hi = make_smem_desc<Cfg::SWZ>(b_hi(s));
+                    const uint64_t da_hi = make_smem_desc_mn128(a_hi(s), BK * 128), db_hi = make_smem_desc<Cfg::SWZ>(b_hi(s));
                     uint32_t acc = in_chunk != 0;
-                    if (SPLIT) {  // small cross terms first: they meet the smallest accumulator
-                        const uint64_t da_lo = make_smem_desc<Cfg::SWZ>(a_lo(s)), db_lo = make_smem_desc<Cfg::SWZ>(b_lo(s));
+                    if (SPLIT && !(p.debug & 2)) {  // small cross terms first: they meet the smallest accumulator
+                        const uint64_t da_lo = make_smem_desc_mn128(a_lo(s), BK * 128), db_lo = make_smem_desc<Cfg::SWZ>(b_lo(s));
                         for (int k = 0; k < ksteps; ++k) {
-                            const uint64_t koff = (uint64_t)((k * 32) >> 4);  // 8 tf32 = 32 bytes along the row
-                            mma_tf32_ss(d_tmem, da_lo + koff, db_hi + koff, idesc, acc);
-                            mma_tf32_ss(d_tmem, da_hi + koff, db_lo + koff, idesc, 1u);
+                            const uint64_t koff = (uint64_t)((k * 32) >> 4);    // B: 8 tf32 = 32 bytes along the row
+                            const uint64_t aoff = (uint64_t)((k * 1024) >> 4);  // A: 8 k rows = one 1024-byte atom
+                            mma_tf32_ss(d_tmem, da_lo + aoff, db_hi + koff, idesc, acc);
+                            mma_tf32_ss(d_tmem, da_hi + aoff, db_lo + koff, idesc, 1u);
                             acc = 1u;
                         }
                     }
                     for (int k = 0; k < ksteps; ++k) {
-                        const uint64_t koff = (uint64_t)((k * 32) >> 4);
-                        mma_tf32_ss(d_tmem, da_hi + koff, db_hi + koff, idesc, acc);
+                        const uint64_t koff = (uint64_t)((k * 32) >> 4), aoff = (uint64_t)((k * 1024) >> 4);
+                        mma_tf32_ss(d_tmem, da_hi + aoff, db_hi + koff, idesc, acc);
                         acc = 1u;
                     }
                     mma_commit(bar_empty(s));
@@ -190,7 +198,7 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
                     float4 *bh = reinterpret_cast<float4 *>(smem_gen + (size_t)s * Cfg::STAGE_BYTES + 2 * Cfg::A_BYTES);
                     float4 *bl = reinterpret_cast<float4 *>(smem_gen + (size_t)s * Cfg::STAGE_BYTES + 2 * Cfg::A_BYTES + Cfg::B_BYTES);
 #pragma unroll 4
-                    for (int q = tid; q < n_a4 + n_b4; q += 128) {
+                    for (int q = tid; q < ((p.debug & 1) ? 0 : n_a4 + n_b4); q += 128) {
                         float4 *ph = q < n_a4 ? ah + q : bh + (q - n_a4);
                         float4 *pl = q < n_a4 ? al + q : bl + (q - n_a4);
                         const float4 v = *ph;
@@ -243,34 +251,27 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
                 __syncwarp();
                 if (lane == 0) mbar_arrive(bar_tempty(a));
             }
+            // every matrix the MLP touches is tile-transposed, [M / 128][N][128]: column c of this tile is
+            // 128 consecutive floats, so each warp store / load below is one full 128-byte line
+            const int64_t tbase = (int64_t)(m0 / TC_BM) * p.N * TC_BM + quad * 32 + lane;
 #pragma unroll
             for (int gi = 0; gi < 4; ++gi) {
                 const int g = 2 * gi + half;
                 const int col0 = n0 + g * 32;
-                const int64_t o = (int64_t)row * p.N + col0;
 #pragma unroll
-                for (int j = 0; j < 32; j += 4) {
-                    // a 4-column group is either whole or absent: N and bn are multiples of 4
-                    if (!row_ok || g >= n_groups || col0 + j >= p.N || g * 32 + j >= p.bn) continue;
-                    float4 x = make_float4(acc[gi][j], acc[gi][j + 1], acc[gi][j + 2], acc[gi][j + 3]);
-                    if (EPI == EPI_PLAIN_T) {  // one column = 128 consecutive floats: a warp stores 128 B runs
-                        float *ct = p.C + ((int64_t)(m0 / TC_BM) * p.N + col0 + j) * TC_BM + quad * 32 + lane;
-                        ct[0] = x.x; ct[TC_BM] = x.y; ct[2 * TC_BM] = x.z; ct[3 * TC_BM] = x.w;
-                    } else if (EPI == EPI_HIDDEN) {
-                        const float4 bb = __ldg(reinterpret_cast<const float4 *>(p.bias + col0 + j));
-                        float4 h, d;
-                        swish_pair_tc(x.x + bb.x, h.x, d.x);
-                        swish_pair_tc(x.y + bb.y, h.y, d.y);
-                        swish_pair_tc(x.z + bb.z, h.z, d.z);
-                        swish_pair_tc(x.w + bb.w, h.w, d.w);
-                        *reinterpret_cast<float4 *>(p.C + o + j) = h;
-                        *reinterpret_cast<float4 *>(p.C2 + o + j) = d;
+                for (int j = 0; j < 32; ++j) {
+                    if (!row_ok || g >= n_groups || col0 + j >= p.N || g * 32 + j >= p.bn || (p.debug & 4)) continue;
+                    const int64_t o = tbase + (int64_t)(col0 + j) * TC_BM;
+                    const float x = acc[gi][j];
+                    if (EPI == EPI_HIDDEN) {
+                        float h, d;
+                        swish_pair_tc(x + __ldg(p.bias + col0 + j), h, d);
+                        p.C[o] = h;
+                        p.C2[o] = d;
                     } else if (EPI == EPI_MUL) {
-                        const float4 dm = __ldg(reinterpret_cast<const float4 *>(p.Dmul + o + j));
-                        x.x *= dm.x; x.y *= dm.y; x.z *= dm.z; x.w *= dm.w;
-                        *reinterpret_cast<float4 *>(p.C + o + j) = x;
+                        p.C[o] = x * __ldg(p.Dmul + o);
                     } else {
-                        *reinterpret_cast<float4 *>(p.C + o + j) = x;
+                        p.C[o] = x;
                     }
                 }
             }
@@ -344,6 +345,30 @@ static int pick_bn(int N) {
     return best;
 }
 
+// Tile-transposed activations [tiles][K][128] as a 2-D tensor of 512-byte lines (line = tile * K + k),
+// box {32 floats, BK lines}: four loads per stage give [4][BK][32 floats], the MN-major
+// operand layout of make_smem_desc_mn128 (128-byte swizzle, 32-byte atomicity).
+static int make_tmap_a(CUtensorMap *tm, const float *base, int64_t M, int K, int BK) {
+    PFN_encodeTiled enc = get_encode();
+    if (!enc) {
+        set_error("cuTensorMapEncodeTiled is not available from the driver");
+        return GMNN_CUDA_ERROR;
+    }
+    const int64_t tiles = (M + TC_BM - 1) / TC_BM;
+    const cuuint64_t dims[2] = {(cuuint64_t)TC_BM, (cuuint64_t)(tiles * K)};
+    const cuuint64_t strides[1] = {(cuuint64_t)TC_BM * 4};
+    const cuuint32_t box[2] = {32, (cuuint32_t)BK};
+    const cuuint32_t estr[2] = {1, 1};
+    const CUresult r = enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float *>(base), dims, strides, box, estr,
+                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B,
+                           CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        set_error("cuTensorMapEncodeTiled failed (%d) for a tile-transposed [%lld][%d] matrix", (int)r, (long long)M, K);
+        return GMNN_CUDA_ERROR;
+    }
+    return GMNN_OK;
+}
+
 template <bool SPLIT, int BK, int EPI>
 static int tc_launch(const CUtensorMap &tmA, const CUtensorMap &tmB, const TcArgs &args, cudaStream_t st) {
     using Cfg = TcCfg<SPLIT, BK>;
@@ -359,14 +384,16 @@ static int tc_launch(const CUtensorMap &tmA, const CUtensorMap &tmB, const TcArg
     return GMNN_OK;
 }
 
+int g_tc_debug = 0;
 int g_tc_flush_k = 32;   // knob "tc_flush_k": K extent between accumulator flushes of the 3xTF32 mode
 int g_tc_split_bk = 16;  // knob (gmnn_system_set_int "tc_split_bk"): K extent of a 3xTF32 stage, 16 or 32
 
-// C[M][N] = A[M][K] . Bt[N][K]^T, all fp32 row-major and dense (lda = ldb = K, ldc = N).
+// C[M][N] = A[M][K] . Bt[N][K]^T.  A, C, C2, Dmul are tile-transposed ([M/128][cols][128], padded to whole
+// tiles); Bt (weights) is row-major [N][K].
 int tc_gemm(bool split, int epi, int64_t M, int N, int K, const float *A, const float *Bt, float *C, const float *bias,
             float *C2, const float *Dmul, cudaStream_t st) {
-    if (K % 4 != 0 || N % 4 != 0 || M <= 0 || M > INT32_MAX) {
-        set_error("tensor-core MLP: widths must be multiples of 4 (K = %d, N = %d)", K, N);
+    if (K % 8 != 0 || N % 4 != 0 || M <= 0 || M > INT32_MAX) {
+        set_error("tensor-core MLP: K must be a multiple of 8 and N of 4 (K = %d, N = %d)", K, N);
         return GMNN_UNSUPPORTED;
     }
     const int BK = split ? g_tc_split_bk : 32;
@@ -376,16 +403,16 @@ int tc_gemm(bool split, int epi, int64_t M, int N, int K, const float *A, const 
     a.n_tiles_n = (N + a.bn - 1) / a.bn;
     a.n_tiles = (int)((M + TC_BM - 1) / TC_BM) * a.n_tiles_n;
     a.flush = split ? (g_tc_flush_k / BK > 0 ? g_tc_flush_k / BK : 1) : (K + BK - 1) / BK;  // TF32 mode: one chunk
+    a.debug = g_tc_debug;
     a.C = C, a.C2 = C2, a.bias = bias, a.Dmul = Dmul;
     CUtensorMap tmA, tmB;
     int rc;
-    if ((rc = make_tmap(&tmA, A, M, K, TC_BM, BK))) return rc;
+    if ((rc = make_tmap_a(&tmA, A, M, K, BK))) return rc;
     if ((rc = make_tmap(&tmB, Bt, N, K, a.bn, BK))) return rc;
 #define TC_CASE(SP, BKV)                                                                  \
     switch (epi) {                                                                        \
         case EPI_PLAIN: return tc_launch<SP, BKV, EPI_PLAIN>(tmA, tmB, a, st);             \
         case EPI_HIDDEN: return tc_launch<SP, BKV, EPI_HIDDEN>(tmA, tmB, a, st);           \
-        case EPI_PLAIN_T: return tc_launch<SP, BKV, EPI_PLAIN_T>(tmA, tmB, a, st);         \
         default: return tc_launch<SP, BKV, EPI_MUL>(tmA, tmB, a, st);                      \
     }
     if (!split) { TC_CASE(false, 32) }
@@ -426,7 +453,7 @@ int launch_mlp_backward_tc(gmnn_system *s, const float *head_w_dev, cudaStream_t
             BopT = m->W[l - 1];
             cur ^= 1;
         } else {
-            rc = tc_gemm(split, EPI_PLAIN_T, s->N, m->dims[0], m->dims[1], Aop, BopT, s->dG, nullptr, nullptr, nullptr, st);
+            rc = tc_gemm(split, EPI_PLAIN, s->N, m->dims[0], m->dims[1], Aop, BopT, s->dG, nullptr, nullptr, nullptr, st);
             if (rc) return rc;
         }
     }

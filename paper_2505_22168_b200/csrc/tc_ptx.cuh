@@ -55,6 +55,14 @@ __device__ __forceinline__ void tma_load_2d(uint32_t dst, const void *tmap, uint
         : "memory");
 }
 
+// 3-D tiled load (c0 innermost).
+__device__ __forceinline__ void tma_load_3d(uint32_t dst, const void *tmap, uint32_t bar, int c0, int c1, int c2) {
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
+        ::"r"(dst), "l"((uint64_t)tmap), "r"(bar), "r"(c0), "r"(c1), "r"(c2)
+        : "memory");
+}
+
 // 1-D bulk copy global -> shared (bytes % 16 == 0, both addresses 16-byte aligned); completes on `bar`.
 __device__ __forceinline__ void bulk_load_1d(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
@@ -104,9 +112,25 @@ __device__ __forceinline__ uint64_t make_smem_desc(uint32_t saddr) {
     d |= layout << 61;                                        // layout type, bits [61,64)
     return d;
 }
-// Instruction descriptor: TF32 x TF32 -> F32, both operands K-major, dense.
-__host__ __device__ constexpr uint32_t make_idesc_tf32(int M, int N) {
-    return (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
+// MN-major tf32 operand tile.  The only swizzled layout the tensor core accepts for MN-major 32-bit
+// operands is "128-byte swizzle with 32-byte atomicity" (layout type 1; TMA:
+// CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B): the tile is [MN / 32][K][32 floats]; one 128-byte row holds
+// 32 consecutive MN elements of one k; 4 consecutive k rows make a 512-byte swizzle atom (stride
+// byte offset = distance between 4-row groups); the next 32 MN elements start `mn_block_bytes`
+// later (leading byte offset).
+__device__ __forceinline__ uint64_t make_smem_desc_mn128(uint32_t saddr, uint32_t mn_block_bytes) {
+    uint64_t d = 0;
+    d |= (uint64_t)((saddr & 0x3FFFFu) >> 4);
+    d |= (uint64_t)((mn_block_bytes >> 4) & 0x3FFFu) << 16;   // leading byte offset
+    d |= (uint64_t)(512 >> 4) << 32;                          // stride byte offset
+    d |= (uint64_t)1 << 46;                                   // version
+    d |= (uint64_t)1 << 61;                                   // SWIZZLE_128B_BASE32B
+    return d;
+}
+// Instruction descriptor: TF32 x TF32 -> F32, dense; B is K-major, A is K-major or MN-major.
+__host__ __device__ constexpr uint32_t make_idesc_tf32(int M, int N, bool a_mn_major = false) {
+    return (1u << 4) | (2u << 7) | (2u << 10) | ((a_mn_major ? 1u : 0u) << 15) | ((uint32_t)(N >> 3) << 17) |
+           ((uint32_t)(M >> 4) << 24);
 }
 // D[tmem] (+)= A[smem] . B[smem]^T ; one thread issues.
 __device__ __forceinline__ void mma_tf32_ss(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
