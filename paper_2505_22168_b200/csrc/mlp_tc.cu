@@ -67,7 +67,7 @@ struct TcArgs {
 };
 
 __device__ __forceinline__ void swish_pair_tc(float z, float &h, float &d) {
-    const float s = 1.f / (1.f + __expf(-z));
+    const float s = __fdividef(1.f, 1.f + __expf(-z));  // ex2.approx + rcp.approx: ~2 ulp, no slow path
     h = z * s;
     d = s * (1.f + z * (1.f - s));
 }
@@ -150,11 +150,6 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
                     const int s = it % NST;
                     mbar_wait(SPLIT ? bar_split(s) : bar_full(s), (it / NST) & 1);
                     tcgen05_fence_after();
-                    if ((p.debug & 64) && it == 0 && blockIdx.x == 0) {
-                        const float *fa = reinterpret_cast<const float *>(smem_gen + (size_t)s * Cfg::STAGE_BYTES);
-                        const float *fb = reinterpret_cast<const float *>(smem_gen + (size_t)s * Cfg::STAGE_BYTES + Cfg::A_BYTES * (SPLIT ? 2 : 1));
-                        printf("A smem: %g %g %g %g | %g %g | B smem: %g %g %g %g K=%d bn=%d M=%d\n", fa[0], fa[1], fa[2], fa[3], fa[32], fa[1024], fb[0], fb[1], fb[2], fb[3], p.K, p.bn, p.M);
-                    }
                     const int krem = p.K - kb * BK;
                     const int ksteps = krem >= BK ? BK / 8 : (krem + 7) / 8;
                     const uint64_t da_hi = make_smem_desc_mn128(a_hi(s), BK * 128), db_hi = make_smem_desc<Cfg::SWZ>(b_hi(s));
@@ -254,24 +249,40 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
             // every matrix the MLP touches is tile-transposed, [M / 128][N][128]: column c of this tile is
             // 128 consecutive floats, so each warp store / load below is one full 128-byte line
             const int64_t tbase = (int64_t)(m0 / TC_BM) * p.N * TC_BM + quad * 32 + lane;
+            float *__restrict__ Cout = p.C;
+            float *__restrict__ C2out = p.C2;
+            const float *__restrict__ bias = p.bias;
+            const float *__restrict__ Dmul = p.Dmul;
 #pragma unroll
             for (int gi = 0; gi < 4; ++gi) {
                 const int g = 2 * gi + half;
                 const int col0 = n0 + g * 32;
+                if (g >= n_groups || !row_ok || (p.debug & 4)) continue;
+                // eight columns at a time: loads first, then the arithmetic, then the stores, so that the
+                // eight dependency chains (ex2, rcp, fma) overlap
 #pragma unroll
-                for (int j = 0; j < 32; ++j) {
-                    if (!row_ok || g >= n_groups || col0 + j >= p.N || g * 32 + j >= p.bn || (p.debug & 4)) continue;
-                    const int64_t o = tbase + (int64_t)(col0 + j) * TC_BM;
-                    const float x = acc[gi][j];
+                for (int j0 = 0; j0 < 32; j0 += 8) {
+                    if (col0 + j0 >= p.N || g * 32 + j0 >= p.bn) continue;  // N and bn are multiples of 8 here
+                    const int64_t o = tbase + (int64_t)(col0 + j0) * TC_BM;
+                    float in[8], h[8], d[8];
                     if (EPI == EPI_HIDDEN) {
-                        float h, d;
-                        swish_pair_tc(x + __ldg(p.bias + col0 + j), h, d);
-                        p.C[o] = h;
-                        p.C2[o] = d;
+#pragma unroll
+                        for (int c = 0; c < 8; ++c) in[c] = __ldg(bias + col0 + j0 + c);
+#pragma unroll
+                        for (int c = 0; c < 8; ++c) swish_pair_tc(acc[gi][j0 + c] + in[c], h[c], d[c]);
+#pragma unroll
+                        for (int c = 0; c < 8; ++c) {
+                            Cout[o + c * TC_BM] = h[c];
+                            C2out[o + c * TC_BM] = d[c];
+                        }
                     } else if (EPI == EPI_MUL) {
-                        p.C[o] = x * __ldg(p.Dmul + o);
+#pragma unroll
+                        for (int c = 0; c < 8; ++c) in[c] = __ldg(Dmul + o + c * TC_BM);
+#pragma unroll
+                        for (int c = 0; c < 8; ++c) Cout[o + c * TC_BM] = acc[gi][j0 + c] * in[c];
                     } else {
-                        p.C[o] = x;
+#pragma unroll
+                        for (int c = 0; c < 8; ++c) Cout[o + c * TC_BM] = acc[gi][j0 + c];
                     }
                 }
             }
@@ -392,8 +403,8 @@ int g_tc_split_bk = 16;  // knob (gmnn_system_set_int "tc_split_bk"): K extent o
 // tiles); Bt (weights) is row-major [N][K].
 int tc_gemm(bool split, int epi, int64_t M, int N, int K, const float *A, const float *Bt, float *C, const float *bias,
             float *C2, const float *Dmul, cudaStream_t st) {
-    if (K % 8 != 0 || N % 4 != 0 || M <= 0 || M > INT32_MAX) {
-        set_error("tensor-core MLP: K must be a multiple of 8 and N of 4 (K = %d, N = %d)", K, N);
+    if (K % 8 != 0 || N % 8 != 0 || M <= 0 || M > INT32_MAX) {
+        set_error("tensor-core MLP: widths must be multiples of 8 (K = %d, N = %d)", K, N);
         return GMNN_UNSUPPORTED;
     }
     const int BK = split ? g_tc_split_bk : 32;
