@@ -298,7 +298,7 @@ void gmnn_system_destroy(gmnn_system *s) {
     if (!s) return;
     dev_free(s->species); dev_free(s->cell_of); dev_free(s->cell_count); dev_free(s->cell_start);
     dev_free(s->cell_fill); dev_free(s->slot_tmp); dev_free(s->perm); dev_free(s->pos4); dev_free(s->xref);
-    dev_free(s->nbr); dev_free(s->rev); dev_free(s->gbuf); dev_free(s->count); dev_free(s->psi); dev_free(s->G); dev_free(s->dG); dev_free(s->A);
+    dev_free(s->nbr); dev_free(s->rev); dev_free(s->gbuf); dev_free(s->runs); dev_free(s->count); dev_free(s->psi); dev_free(s->G); dev_free(s->dG); dev_free(s->A);
     for (int l = 0; l < MAX_LAYERS; ++l) { dev_free(s->H[l]); dev_free(s->D[l]); }
     dev_free(s->dZ[0]); dev_free(s->dZ[1]); dev_free(s->Bv); dev_free(s->BvT); dev_free(s->vhead); dev_free(s->head_w);
     dev_free(s->e_heads); dev_free(s->e_atom); dev_free(s->f_int); dev_free(s->f_tmp); dev_free(s->partial);
@@ -474,6 +474,7 @@ int gmnn_build_neighbors(gmnn_system *s, const float *positions, const float cel
         if (s->force_mode == GMNN_FORCE_PAIRBUF && !s->rev) {
             int rc = dev_alloc(&s->rev, (size_t)s->N * s->cap);
             if (!rc) rc = dev_alloc(&s->gbuf, (size_t)s->N * s->cap);
+            if (!rc && !s->runs) rc = dev_alloc(&s->runs, (size_t)s->N * 28);
             if (rc) {
                 set_error("out of device memory for the pair buffer (%lld x %d)", (long long)s->N, s->cap);
                 return rc;

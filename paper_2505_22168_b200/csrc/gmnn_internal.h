@@ -92,6 +92,7 @@ struct gmnn_system {
     uint32_t *nbr = nullptr;         // [N][cap]
     int32_t *count = nullptr;        // [N]
     uint16_t *rev = nullptr;         // [N][cap] slot of the reverse pair (GMNN_FORCE_PAIRBUF)
+    uint16_t *runs = nullptr;        // [N][28] first slot of each of the 27 cell runs of a row, and its length
     float4 *gbuf = nullptr;          // [N][cap] g_ij, stored in the row of j at the reverse slot
     bool list_has_rev = false;
     int cap = 0;

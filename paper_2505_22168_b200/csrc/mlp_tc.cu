@@ -49,7 +49,7 @@ struct TcCfg {
     static constexpr int B_BYTES = TC_BN_MAX * BK * 4;
     static constexpr int STAGE_BYTES = (A_BYTES + B_BYTES) * (SPLIT ? 2 : 1);
     static constexpr int NST = TC_STAGE_BYTES_TOTAL / STAGE_BYTES;
-    static constexpr int SMEM_BYTES = NST * STAGE_BYTES + 1024 /*alignment slack*/ + 256 /*barriers*/;
+    static constexpr int SMEM_BYTES = NST * STAGE_BYTES + 1024 /*alignment slack*/ + 512 /*barriers*/ + 4096 /*timeline (debug 32)*/;
     static_assert(NST >= 2, "pipeline needs at least two stages");
 };
 
@@ -94,6 +94,9 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
     const uint32_t tmem_slot = bar_base + 8u * (3 * NST + 4);
     volatile uint32_t *tmem_slot_gen = reinterpret_cast<volatile uint32_t *>(smem_gen + (size_t)NST * Cfg::STAGE_BYTES + 8 * (3 * NST + 4));
 
+    long long *ts = reinterpret_cast<long long *>(smem_gen + (size_t)NST * Cfg::STAGE_BYTES + 512);  // [8][64]
+    const bool tl = (p.debug & 32) && blockIdx.x == 0;
+#define TL(role, idx) do { if (tl && (idx) >= 64 && (idx) < 128) ts[(role) * 64 + (idx) - 64] = clock64(); } while (0)
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int nkb = (p.K + BK - 1) / BK;  // pipeline stages per tile; chunk c covers stages [c*flush, (c+1)*flush)
 
@@ -128,6 +131,7 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
                 for (int kb = 0; kb < nkb; ++kb, ++it) {
                     const int s = it % NST;
                     mbar_wait(bar_empty(s), ((it / NST) & 1) ^ 1);
+                    TL(0, it);
                     mbar_arrive_expect_tx(bar_full(s), tx);
                     for (int q = 0; q < 4; ++q)  // four 32-atom column blocks of the tile, [BK][32 floats] each
                         tma_load_2d(a_hi(s) + q * (BK * 128), &tmA, bar_full(s), q * 32, (m0 / TC_BM) * p.K + kb * BK);
@@ -144,12 +148,16 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
                     const int a = chunk & 1;
                     const uint32_t d_tmem = tmem_base + (uint32_t)a * TC_BN_MAX;
                     if (in_chunk == 0) {
+                        TL(5, it);
                         mbar_wait(bar_tempty(a), ((chunk >> 1) & 1) ^ 1);
                         tcgen05_fence_after();
+                        TL(6, it);
                     }
                     const int s = it % NST;
+                    TL(3, it);
                     mbar_wait(SPLIT ? bar_split(s) : bar_full(s), (it / NST) & 1);
                     tcgen05_fence_after();
+                    TL(4, it);
                     const int krem = p.K - kb * BK;
                     const int ksteps = krem >= BK ? BK / 8 : (krem + 7) / 8;
                     const uint64_t da_hi = make_smem_desc_mn128(a_hi(s), BK * 128), db_hi = make_smem_desc<Cfg::SWZ>(b_hi(s));
@@ -188,6 +196,7 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
                 for (int kb = 0; kb < nkb; ++kb, ++it) {
                     const int s = it % NST;
                     mbar_wait(bar_full(s), (it / NST) & 1);
+                    if (tid == 0) TL(1, it);
                     float4 *ah = reinterpret_cast<float4 *>(smem_gen + (size_t)s * Cfg::STAGE_BYTES);
                     float4 *al = reinterpret_cast<float4 *>(smem_gen + (size_t)s * Cfg::STAGE_BYTES + Cfg::A_BYTES);
                     float4 *bh = reinterpret_cast<float4 *>(smem_gen + (size_t)s * Cfg::STAGE_BYTES + 2 * Cfg::A_BYTES);
@@ -198,6 +207,13 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
                         float4 *pl = q < n_a4 ? al + q : bl + (q - n_a4);
                         const float4 v = *ph;
                         float4 h, l;
+                        if (p.debug & 128) {  // experiment: leave hi to the tensor core's own truncation
+                            h.x = __uint_as_float(__float_as_uint(v.x) & 0xFFFFE000u); h.y = __uint_as_float(__float_as_uint(v.y) & 0xFFFFE000u);
+                            h.z = __uint_as_float(__float_as_uint(v.z) & 0xFFFFE000u); h.w = __uint_as_float(__float_as_uint(v.w) & 0xFFFFE000u);
+                            l.x = v.x - h.x; l.y = v.y - h.y; l.z = v.z - h.z; l.w = v.w - h.w;
+                            *pl = l;
+                            continue;
+                        }
                         h.x = to_tf32_rna(v.x); h.y = to_tf32_rna(v.y); h.z = to_tf32_rna(v.z); h.w = to_tf32_rna(v.w);
                         l.x = v.x - h.x; l.y = v.y - h.y; l.z = v.z - h.z; l.w = v.w - h.w;
                         *ph = h;
@@ -206,6 +222,7 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
                     fence_proxy_async_smem();
                     __syncwarp();
                     if (lane == 0) mbar_arrive(bar_split(s));
+                    if (tid == 0) TL(2, it);
                 }
             }
         }
@@ -291,6 +308,12 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
 
     tcgen05_fence_before();
     __syncthreads();
+    if (tl && threadIdx.x == 0) {
+        for (int q = 0; q < 64; ++q)
+            printf("it %d  prod %lld  full %lld  splitdone %lld  mma_wait_begin %lld  mma_go %lld | tempty wait %lld..%lld\n", q + 64,
+                   ts[q] - ts[0], ts[64 + q] - ts[0], ts[128 + q] - ts[0], ts[192 + q] - ts[0], ts[256 + q] - ts[0],
+                   ts[320 + q] - ts[0], ts[384 + q] - ts[0]);
+    }
     if (warp == 1) tmem_dealloc<512>(tmem_base);
 }
 
@@ -396,8 +419,8 @@ static int tc_launch(const CUtensorMap &tmA, const CUtensorMap &tmB, const TcArg
 }
 
 int g_tc_debug = 0;
-int g_tc_flush_k = 32;   // knob "tc_flush_k": K extent between accumulator flushes of the 3xTF32 mode
-int g_tc_split_bk = 16;  // knob (gmnn_system_set_int "tc_split_bk"): K extent of a 3xTF32 stage, 16 or 32
+int g_tc_flush_k = 64;   // knob "tc_flush_k": K extent between accumulator flushes of the 3xTF32 mode
+int g_tc_split_bk = 32;  // knob (gmnn_system_set_int "tc_split_bk"): K extent of a 3xTF32 stage, 16 or 32
 
 // C[M][N] = A[M][K] . Bt[N][K]^T.  A, C, C2, Dmul are tile-transposed ([M/128][cols][128], padded to whole
 // tiles); Bt (weights) is row-major [N][K].

@@ -160,11 +160,14 @@ __device__ __forceinline__ uint32_t image_code(int nx, int ny, int nz) {
            ((uint32_t)(nz + 4) << (NBR_J_BITS + 6));
 }
 
+constexpr int RUNS_PITCH = 28;  // 27 run starts + the row length
+
 // One warp per centre atom; lanes test 32 candidates of a neighbouring cell at a time and append
 // the hits in candidate order (ballot + prefix popcount): the list order is deterministic.
 __global__ void __launch_bounds__(256)
 k_build_cells(int64_t N, const float4 *__restrict__ pos4, const int32_t *__restrict__ cell_start, Geometry g,
-              uint32_t *nbr, int32_t *count, int cap, int32_t *flags, const int32_t *cond, float thr2) {
+              uint32_t *nbr, int32_t *count, int cap, int32_t *flags, const int32_t *cond, float thr2,
+              uint16_t *runs) {
     if (skip_rebuild(cond, thr2)) return;
     const int lane = threadIdx.x & 31;
     const int64_t i = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
@@ -175,36 +178,38 @@ k_build_cells(int64_t N, const float4 *__restrict__ pos4, const int32_t *__restr
     const int cz = cell_coord(xi.z, g.inv_edge[2], g.ncell[2]);
     uint32_t *row = nbr + i * (int64_t)cap;
     int n = 0;
-    for (int oz = -1; oz <= 1; ++oz) {
+    // 27 cells in the fixed order idx = (oz+1)*9 + (oy+1)*3 + (ox+1); runs[idx] = first slot of the
+    // cell's run in this row (entries of a run ascend in atom index).  The reverse-pair index uses
+    // the runs: the partner of an entry in run idx sits in run 26 - idx of the partner's row.
+    for (int idx = 0; idx < 27; ++idx) {
+        if (runs && lane == 0) runs[i * RUNS_PITCH + idx] = (uint16_t)(n < cap ? n : cap);
+        const int oz = idx / 9 - 1, oy = (idx / 3) % 3 - 1, ox = idx % 3 - 1;
         int z = cz + oz, nz = 0;
         if (z < 0) { if (!g.pbc[2]) continue; z += g.ncell[2]; nz = -1; }
         else if (z >= g.ncell[2]) { if (!g.pbc[2]) continue; z -= g.ncell[2]; nz = 1; }
-        for (int oy = -1; oy <= 1; ++oy) {
-            int y = cy + oy, ny = 0;
-            if (y < 0) { if (!g.pbc[1]) continue; y += g.ncell[1]; ny = -1; }
-            else if (y >= g.ncell[1]) { if (!g.pbc[1]) continue; y -= g.ncell[1]; ny = 1; }
-            for (int ox = -1; ox <= 1; ++ox) {
-                int x = cx + ox, nx = 0;
-                if (x < 0) { if (!g.pbc[0]) continue; x += g.ncell[0]; nx = -1; }
-                else if (x >= g.ncell[0]) { if (!g.pbc[0]) continue; x -= g.ncell[0]; nx = 1; }
-                const int c = (z * g.ncell[1] + y) * g.ncell[0] + x;
-                const int b = cell_start[c], e = cell_start[c + 1];
-                const float sx = __fmul_rn((float)nx, g.L[0]), sy = __fmul_rn((float)ny, g.L[1]),
-                            sz = __fmul_rn((float)nz, g.L[2]);
-                const uint32_t code = image_code(nx, ny, nz);
-                const bool home = (nx | ny | nz) == 0;
-                for (int base = b; base < e; base += 32) {
-                    const int j = base + lane;
-                    bool keep = false;
-                    if (j < e && !(home && j == (int)i)) keep = in_list(xi, pos4[j], sx, sy, sz, g.r_list2);
-                    const unsigned m = __ballot_sync(0xffffffffu, keep);
-                    const int p = n + __popc(m & ((1u << lane) - 1u));
-                    if (keep && p < cap) row[p] = (uint32_t)j | code;
-                    n += __popc(m);
-                }
-            }
+        int y = cy + oy, ny = 0;
+        if (y < 0) { if (!g.pbc[1]) continue; y += g.ncell[1]; ny = -1; }
+        else if (y >= g.ncell[1]) { if (!g.pbc[1]) continue; y -= g.ncell[1]; ny = 1; }
+        int x = cx + ox, nx = 0;
+        if (x < 0) { if (!g.pbc[0]) continue; x += g.ncell[0]; nx = -1; }
+        else if (x >= g.ncell[0]) { if (!g.pbc[0]) continue; x -= g.ncell[0]; nx = 1; }
+        const int c = (z * g.ncell[1] + y) * g.ncell[0] + x;
+        const int b = cell_start[c], e = cell_start[c + 1];
+        const float sx = __fmul_rn((float)nx, g.L[0]), sy = __fmul_rn((float)ny, g.L[1]),
+                    sz = __fmul_rn((float)nz, g.L[2]);
+        const uint32_t code = image_code(nx, ny, nz);
+        const bool home = (nx | ny | nz) == 0;
+        for (int base = b; base < e; base += 32) {
+            const int j = base + lane;
+            bool keep = false;
+            if (j < e && !(home && j == (int)i)) keep = in_list(xi, pos4[j], sx, sy, sz, g.r_list2);
+            const unsigned m = __ballot_sync(0xffffffffu, keep);
+            const int p = n + __popc(m & ((1u << lane) - 1u));
+            if (keep && p < cap) row[p] = (uint32_t)j | code;
+            n += __popc(m);
         }
     }
+    if (runs && lane == 0) runs[i * RUNS_PITCH + 27] = (uint16_t)(n < cap ? n : cap);
     if (lane == 0) {
         count[i] = n < cap ? n : cap;
         if (n > cap) atomicMax(&flags[FLAG_MAXCOUNT], n);
@@ -290,6 +295,44 @@ k_build_rev(int64_t N, const uint32_t *__restrict__ nbr, const int32_t *__restri
     }
 }
 
+// The same index for lists built by k_build_cells, using the runs: lane = one entry; its run r in
+// row i comes from the run starts, the partner is searched only in run 26 - r of row j (about 5
+// entries instead of the whole row).
+__global__ void __launch_bounds__(256)
+k_build_rev_runs(int64_t N, const uint32_t *__restrict__ nbr, const int32_t *__restrict__ count, int cap,
+                 const uint16_t *__restrict__ runs, uint16_t *rev, int32_t *flags, const int32_t *cond, float thr2) {
+    if (skip_rebuild(cond, thr2)) return;
+    const int lane = threadIdx.x & 31;
+    const int64_t i = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
+    if (i >= N) return;
+    const int cnt = count[i];
+    const uint32_t *row = nbr + i * (int64_t)cap;
+    const int my_run_start = lane < RUNS_PITCH ? (int)runs[i * RUNS_PITCH + lane] : 0x7fffffff;
+    for (int k0 = 0; k0 < cnt; k0 += 32) {
+        const int k = k0 + lane;
+        int r = -1;  // run of slot k: number of run starts <= k, minus one
+#pragma unroll
+        for (int q = 0; q < 27; ++q) r += __shfl_sync(0xffffffffu, my_run_start, q) <= k ? 1 : 0;
+        if (k < cnt) {
+            const uint32_t e = row[k];
+            const int64_t j = e & NBR_J_MASK;
+            const uint32_t img = e >> NBR_J_BITS;
+            const uint32_t inv = (8u - (img & 7u)) | ((8u - ((img >> 3) & 7u)) << 3) | ((8u - ((img >> 6) & 7u)) << 6);
+            const uint32_t target = (uint32_t)i | (inv << NBR_J_BITS);
+            const uint32_t *rj = nbr + j * (int64_t)cap;
+            const int s0 = runs[j * RUNS_PITCH + (26 - r)], s1 = runs[j * RUNS_PITCH + (27 - r)];
+            int found = 0xFFFF;
+            for (int t = s0; t < s1; ++t)
+                if (rj[t] == target) {
+                    found = t;
+                    break;
+                }
+            rev[i * (int64_t)cap + k] = (uint16_t)found;
+            if (found == 0xFFFF) flags[FLAG_REV_MISSING] = 1;
+        }
+    }
+}
+
 __global__ void k_finish_rebuild(int32_t *flags, const int32_t *cond, float thr2) {
     if (skip_rebuild(cond, thr2)) return;
     flags[FLAG_DISP2] = 0;
@@ -323,10 +366,15 @@ int launch_build(gmnn_system *s, const float *positions, cudaStream_t st, const 
         k_build_small<<<nblocks(N * 32, 256), 256, 0, st>>>(N, s->pos4, g, s->nbr, s->count, s->cap, s->flags, cond, thr2);
     else
         k_build_cells<<<nblocks(N * 32, 256), 256, 0, st>>>(N, s->pos4, s->cell_start, g, s->nbr, s->count, s->cap,
-                                                            s->flags, cond, thr2);
+                                                            s->flags, cond, thr2,
+                                                            s->force_mode == GMNN_FORCE_PAIRBUF ? s->runs : nullptr);
     GMNN_LAUNCHED();
     if (s->force_mode == GMNN_FORCE_PAIRBUF) {
-        k_build_rev<<<nblocks(N * 32, 256), 256, 0, st>>>(N, s->nbr, s->count, s->cap, s->rev, s->flags, cond, thr2);
+        if (s->small_box)
+            k_build_rev<<<nblocks(N * 32, 256), 256, 0, st>>>(N, s->nbr, s->count, s->cap, s->rev, s->flags, cond, thr2);
+        else
+            k_build_rev_runs<<<nblocks(N * 32, 256), 256, 0, st>>>(N, s->nbr, s->count, s->cap, s->runs, s->rev, s->flags,
+                                                                   cond, thr2);
         GMNN_LAUNCHED();
     }
     k_finish_rebuild<<<1, 1, 0, st>>>(s->flags, cond, thr2);

@@ -61,8 +61,8 @@ def test_3xtf32_meets_fp32_tolerance(gm, orc, name, split_bk, flush_k):
     try:
         e, ea, f = _run(sysm, pos)
     finally:
-        sysm.set_int("tc_split_bk", 16)
-        sysm.set_int("tc_flush_k", 32)
+        sysm.set_int("tc_split_bk", 32)
+        sysm.set_int("tc_flush_k", 64)
     print("3xTF32 %s bk %d flush %d: energy err %.3f x 1e-5, force err %.2e" % (
         name, split_bk, flush_k, energy_atom_error(ea, ref.e_atom), force_error(f, ref.forces)))
     assert energy_atom_error(ea, ref.e_atom) <= 1.0
