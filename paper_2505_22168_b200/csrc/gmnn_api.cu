@@ -23,7 +23,7 @@ void set_error(const char *fmt, ...) {
 }
 
 int launch_mlp_forward_tc(gmnn_system *s, cudaStream_t st);
-extern int g_tc_split_bk, g_tc_flush_k, g_tc_debug;
+extern int g_tc_split_bk, g_tc_flush_k, g_tc_debug, g_tc_pair;
 int launch_mlp_backward_tc(gmnn_system *s, const float *head_w_dev, cudaStream_t st);
 
 template <class T>
@@ -338,6 +338,8 @@ int gmnn_system_set_int(gmnn_system *s, const char *key, int64_t v) {
     } else if (!strcmp(key, "tc_split_bk")) {  // process-wide tuning knob of mlp_tc.cu
         if (v != 16 && v != 32) return GMNN_INVALID_ARG;
         gmnn::g_tc_split_bk = (int)v;
+    } else if (!strcmp(key, "tc_pair")) {  // process-wide: 3xTF32 GEMMs on CTA pairs (1) or single CTAs (0)
+        gmnn::g_tc_pair = v != 0;
     } else if (!strcmp(key, "tc_debug")) {  // timing experiments (wrong results), see mlp_tc.cu
         gmnn::g_tc_debug = (int)v;
     } else if (!strcmp(key, "tc_flush_k")) {

@@ -72,6 +72,52 @@ __device__ __forceinline__ void swish_pair_tc(float z, float &h, float &d) {
     d = s * (1.f + z * (1.f - s));
 }
 
+// Fused elementwise and stores of one finished tile held in the epilogue warps' registers.
+template <int EPI>
+__device__ __forceinline__ void tc_store_tile(const TcArgs &p, float (&acc)[4][32], int m0, int n0, int quad, int lane,
+                                              int half, int n_groups, bool row_ok) {
+    // every matrix the MLP touches is tile-transposed, [M / 128][N][128]: column c of this tile is
+    // 128 consecutive floats, so each warp store / load below is one full 128-byte line
+    const int64_t tbase = (int64_t)(m0 / TC_BM) * p.N * TC_BM + quad * 32 + lane;
+    float *__restrict__ Cout = p.C;
+    float *__restrict__ C2out = p.C2;
+    const float *__restrict__ bias = p.bias;
+    const float *__restrict__ Dmul = p.Dmul;
+#pragma unroll
+    for (int gi = 0; gi < 4; ++gi) {
+        const int g = 2 * gi + half;
+        const int col0 = n0 + g * 32;
+        if (g >= n_groups || !row_ok || (p.debug & 4)) continue;
+        // eight columns at a time: loads first, then the arithmetic, then the stores, so that the
+        // eight dependency chains (ex2, rcp, fma) overlap
+#pragma unroll
+        for (int j0 = 0; j0 < 32; j0 += 8) {
+            if (col0 + j0 >= p.N || g * 32 + j0 >= p.bn) continue;  // N and bn are multiples of 8 here
+            const int64_t o = tbase + (int64_t)(col0 + j0) * TC_BM;
+            float in[8], h[8], d[8];
+            if (EPI == EPI_HIDDEN) {
+#pragma unroll
+                for (int c = 0; c < 8; ++c) in[c] = __ldg(bias + col0 + j0 + c);
+#pragma unroll
+                for (int c = 0; c < 8; ++c) swish_pair_tc(acc[gi][j0 + c] + in[c], h[c], d[c]);
+#pragma unroll
+                for (int c = 0; c < 8; ++c) {
+                    Cout[o + c * TC_BM] = h[c];
+                    C2out[o + c * TC_BM] = d[c];
+                }
+            } else if (EPI == EPI_MUL) {
+#pragma unroll
+                for (int c = 0; c < 8; ++c) in[c] = __ldg(Dmul + o + c * TC_BM);
+#pragma unroll
+                for (int c = 0; c < 8; ++c) Cout[o + c * TC_BM] = acc[gi][j0 + c] * in[c];
+            } else {
+#pragma unroll
+                for (int c = 0; c < 8; ++c) Cout[o + c * TC_BM] = acc[gi][j0 + c];
+            }
+        }
+    }
+}
+
 template <bool SPLIT, int BK, int EPI>
 __global__ void __launch_bounds__(TC_THREADS, 1)
 k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const TcArgs p) {
@@ -263,46 +309,7 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
                 __syncwarp();
                 if (lane == 0) mbar_arrive(bar_tempty(a));
             }
-            // every matrix the MLP touches is tile-transposed, [M / 128][N][128]: column c of this tile is
-            // 128 consecutive floats, so each warp store / load below is one full 128-byte line
-            const int64_t tbase = (int64_t)(m0 / TC_BM) * p.N * TC_BM + quad * 32 + lane;
-            float *__restrict__ Cout = p.C;
-            float *__restrict__ C2out = p.C2;
-            const float *__restrict__ bias = p.bias;
-            const float *__restrict__ Dmul = p.Dmul;
-#pragma unroll
-            for (int gi = 0; gi < 4; ++gi) {
-                const int g = 2 * gi + half;
-                const int col0 = n0 + g * 32;
-                if (g >= n_groups || !row_ok || (p.debug & 4)) continue;
-                // eight columns at a time: loads first, then the arithmetic, then the stores, so that the
-                // eight dependency chains (ex2, rcp, fma) overlap
-#pragma unroll
-                for (int j0 = 0; j0 < 32; j0 += 8) {
-                    if (col0 + j0 >= p.N || g * 32 + j0 >= p.bn) continue;  // N and bn are multiples of 8 here
-                    const int64_t o = tbase + (int64_t)(col0 + j0) * TC_BM;
-                    float in[8], h[8], d[8];
-                    if (EPI == EPI_HIDDEN) {
-#pragma unroll
-                        for (int c = 0; c < 8; ++c) in[c] = __ldg(bias + col0 + j0 + c);
-#pragma unroll
-                        for (int c = 0; c < 8; ++c) swish_pair_tc(acc[gi][j0 + c] + in[c], h[c], d[c]);
-#pragma unroll
-                        for (int c = 0; c < 8; ++c) {
-                            Cout[o + c * TC_BM] = h[c];
-                            C2out[o + c * TC_BM] = d[c];
-                        }
-                    } else if (EPI == EPI_MUL) {
-#pragma unroll
-                        for (int c = 0; c < 8; ++c) in[c] = __ldg(Dmul + o + c * TC_BM);
-#pragma unroll
-                        for (int c = 0; c < 8; ++c) Cout[o + c * TC_BM] = acc[gi][j0 + c] * in[c];
-                    } else {
-#pragma unroll
-                        for (int c = 0; c < 8; ++c) Cout[o + c * TC_BM] = acc[gi][j0 + c];
-                    }
-                }
-            }
+            tc_store_tile<EPI>(p, acc, m0, n0, quad, lane, half, n_groups, row_ok);
         }
     }
 
@@ -315,6 +322,220 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
                    ts[320 + q] - ts[0], ts[384 + q] - ts[0]);
     }
     if (warp == 1) tmem_dealloc<512>(tmem_base);
+}
+
+static int tc_num_sms();
+
+// ---- CTA-pair variant of the 3xTF32 kernel (cta_group::2) ------------------------------------------
+// Two CTAs of a cluster (one per SM of a TPC) work on a 256 x bn tile: each holds its own 128 rows of A
+// and HALF of the bn rows of B in shared memory, splits them into hi / lo itself, and owns the 128 x bn
+// accumulator rows in its tensor memory.  One thread of the leader CTA (cluster rank 0) issues the
+// M = 256 MMAs for both.  Per SM this halves the B bytes loaded from L2, split by the splitter warps and
+// read by the tensor core, which is what bounds the single-CTA kernel (shared-memory bandwidth).
+// Hand-shakes across the pair: split-done and accumulator-drained arrivals go to the leader's
+// barriers (mapa + remote arrive); the leader's tcgen05.commit multicasts to both CTAs' barriers.
+template <int BK>
+struct TcPairCfg {
+    static constexpr int A_BYTES = TC_BM * BK * 4;
+    static constexpr int B_BYTES = (TC_BN_MAX / 2) * BK * 4;       // this CTA's half of the B tile
+    static constexpr int STAGE_BYTES = 2 * (A_BYTES + B_BYTES);    // hi and lo of both
+    static constexpr int NST = TC_STAGE_BYTES_TOTAL / STAGE_BYTES;
+    static constexpr int SMEM_BYTES = NST * STAGE_BYTES + 1024 + 512;
+    static_assert(NST >= 2, "pipeline needs at least two stages");
+};
+
+template <int BK, int EPI>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(TC_THREADS, 1)
+k_gemm_tc_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const TcArgs p) {
+    using Cfg = TcPairCfg<BK>;
+    constexpr int NST = Cfg::NST;
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;  // identical offset in both CTAs
+    uint8_t *smem_gen = smem_raw + (smem_base - smem_u32(smem_raw));
+    auto a_hi = [&](int s) { return smem_base + (uint32_t)s * Cfg::STAGE_BYTES; };
+    auto a_lo = [&](int s) { return a_hi(s) + Cfg::A_BYTES; };
+    auto b_hi = [&](int s) { return a_hi(s) + 2 * Cfg::A_BYTES; };
+    auto b_lo = [&](int s) { return b_hi(s) + Cfg::B_BYTES; };
+    const uint32_t bar_base = smem_base + (uint32_t)NST * Cfg::STAGE_BYTES;
+    auto bar_full = [&](int s) { return bar_base + 8u * s; };               // own TMA landed
+    auto bar_split = [&](int s) { return bar_base + 8u * (NST + s); };      // leader's: both CTAs split
+    auto bar_empty = [&](int s) { return bar_base + 8u * (2 * NST + s); };  // own: MMAs of the stage done
+    auto bar_tfull = [&](int a) { return bar_base + 8u * (3 * NST + a); };  // own: chunk complete
+    auto bar_tempty = [&](int a) { return bar_base + 8u * (3 * NST + 2 + a); };  // leader's: both drained
+    const uint32_t tmem_slot = bar_base + 8u * (3 * NST + 4);
+    volatile uint32_t *tmem_slot_gen = reinterpret_cast<volatile uint32_t *>(smem_gen + (size_t)NST * Cfg::STAGE_BYTES + 8 * (3 * NST + 4));
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t rank = cluster_ctarank();
+    const int pair = blockIdx.x >> 1, n_pairs = gridDim.x >> 1;
+    const int nkb = (p.K + BK - 1) / BK;
+    const int hb = p.bn >> 1;  // B rows held by each CTA
+
+    if (warp == 0 && lane == 0) {
+        tma_prefetch_desc(&tmA);
+        tma_prefetch_desc(&tmB);
+        for (int s = 0; s < NST; ++s) {
+            mbar_init(bar_full(s), 1);
+            mbar_init(bar_split(s), 8);   // 4 splitter warps x 2 CTAs
+            mbar_init(bar_empty(s), 1);
+        }
+        for (int a = 0; a < 2; ++a) {
+            mbar_init(bar_tfull(a), 1);
+            mbar_init(bar_tempty(a), 16);  // 8 epilogue warps x 2 CTAs
+        }
+        fence_barrier_init();
+    }
+    if (warp == 1) tmem_alloc_pair<512>(tmem_slot);
+    tcgen05_fence_before();
+    cluster_sync_all();  // barriers of both CTAs initialised before any remote arrive
+    tcgen05_fence_after();
+    const uint32_t tmem_base = *tmem_slot_gen;
+
+    if (warp < TC_FIRST_SPLIT_WARP) {
+        setmaxnreg_dec<TC_REGS_CONTROL>();
+        if (warp == 0 && lane == 0) {
+            // ===== TMA producer: own A rows, own half of B =====
+            const uint32_t tx = (uint32_t)(Cfg::A_BYTES + hb * BK * 4);
+            uint32_t it = 0;
+            for (int t = pair; t < p.n_tiles; t += n_pairs) {
+                const int mt = 2 * (t / p.n_tiles_n) + (int)rank, n0 = (t % p.n_tiles_n) * p.bn;
+                for (int kb = 0; kb < nkb; ++kb, ++it) {
+                    const int s = it % NST;
+                    mbar_wait(bar_empty(s), ((it / NST) & 1) ^ 1);
+                    mbar_arrive_expect_tx(bar_full(s), tx);
+                    for (int q = 0; q < 4; ++q)
+                        tma_load_2d(a_hi(s) + q * (BK * 128), &tmA, bar_full(s), q * 32, mt * p.K + kb * BK);
+                    tma_load_2d(b_hi(s), &tmB, bar_full(s), kb * BK, n0 + (int)rank * hb);
+                }
+            }
+        } else if (warp == 1 && lane == 0 && rank == 0) {
+            // ===== MMA issuer (leader CTA only) =====
+            const uint32_t idesc = make_idesc_tf32(2 * TC_BM, p.bn, true);
+            uint32_t it = 0, chunk = 0;
+            for (int t = pair; t < p.n_tiles; t += n_pairs) {
+                for (int kb = 0; kb < nkb; ++kb, ++it) {
+                    const int in_chunk = kb % p.flush;
+                    const int a = chunk & 1;
+                    const uint32_t d_tmem = tmem_base + (uint32_t)a * TC_BN_MAX;
+                    if (in_chunk == 0) {
+                        mbar_wait(bar_tempty(a), ((chunk >> 1) & 1) ^ 1);
+                        tcgen05_fence_after();
+                    }
+                    const int s = it % NST;
+                    mbar_wait(bar_split(s), (it / NST) & 1);
+                    tcgen05_fence_after();
+                    const int krem = p.K - kb * BK;
+                    const int ksteps = krem >= BK ? BK / 8 : (krem + 7) / 8;
+                    const uint64_t da_hi = make_smem_desc_mn128(a_hi(s), BK * 128), db_hi = make_smem_desc<BK * 4>(b_hi(s));
+                    const uint64_t da_lo = make_smem_desc_mn128(a_lo(s), BK * 128), db_lo = make_smem_desc<BK * 4>(b_lo(s));
+                    uint32_t acc = in_chunk != 0;
+                    for (int k = 0; k < ksteps; ++k) {  // small cross terms first
+                        const uint64_t koff = (uint64_t)((k * 32) >> 4), aoff = (uint64_t)((k * 1024) >> 4);
+                        mma_tf32_ss_pair(d_tmem, da_lo + aoff, db_hi + koff, idesc, acc);
+                        mma_tf32_ss_pair(d_tmem, da_hi + aoff, db_lo + koff, idesc, 1u);
+                        acc = 1u;
+                    }
+                    for (int k = 0; k < ksteps; ++k) {
+                        const uint64_t koff = (uint64_t)((k * 32) >> 4), aoff = (uint64_t)((k * 1024) >> 4);
+                        mma_tf32_ss_pair(d_tmem, da_hi + aoff, db_hi + koff, idesc, 1u);
+                    }
+                    mma_commit_pair(bar_empty(s), 3);
+                    if (in_chunk == p.flush - 1 || kb == nkb - 1) {
+                        mma_commit_pair(bar_tfull(a), 3);
+                        ++chunk;
+                    }
+                }
+            }
+        }
+    } else if (warp < TC_FIRST_EPI_WARP) {
+        setmaxnreg_dec<TC_REGS_SPLIT>();
+        // ===== splitters: own A tile and own half of B, hi in place, lo beside it =====
+        const int tid = threadIdx.x - TC_FIRST_SPLIT_WARP * 32;
+        const int n_a4 = Cfg::A_BYTES / 16, n_b4 = hb * BK * 4 / 16;
+        uint32_t it = 0;
+        for (int t = pair; t < p.n_tiles; t += n_pairs) {
+            for (int kb = 0; kb < nkb; ++kb, ++it) {
+                const int s = it % NST;
+                mbar_wait(bar_full(s), (it / NST) & 1);
+                float4 *ah = reinterpret_cast<float4 *>(smem_gen + (size_t)s * Cfg::STAGE_BYTES);
+                float4 *al = ah + Cfg::A_BYTES / 16;
+                float4 *bh = ah + 2 * Cfg::A_BYTES / 16;
+                float4 *bl = bh + Cfg::B_BYTES / 16;
+#pragma unroll 4
+                for (int q = tid; q < n_a4 + n_b4; q += 128) {
+                    float4 *ph = q < n_a4 ? ah + q : bh + (q - n_a4);
+                    float4 *pl = q < n_a4 ? al + q : bl + (q - n_a4);
+                    const float4 v = *ph;
+                    float4 h, l;
+                    h.x = to_tf32_rna(v.x); h.y = to_tf32_rna(v.y); h.z = to_tf32_rna(v.z); h.w = to_tf32_rna(v.w);
+                    l.x = v.x - h.x; l.y = v.y - h.y; l.z = v.z - h.z; l.w = v.w - h.w;
+                    *ph = h;
+                    *pl = l;
+                }
+                fence_proxy_async_all();
+                __syncwarp();
+                if (lane == 0) mbar_arrive_cluster(bar_split(s), 0);
+            }
+        }
+    } else {
+        setmaxnreg_inc<TC_REGS_EPI>();
+        // ===== epilogue: this CTA's 128 rows =====
+        const int quad = warp & 3;
+        const int half = (warp - TC_FIRST_EPI_WARP) >> 2;
+        const int n_groups = (p.bn + 31) / 32;
+        const int n_chunks = (nkb + p.flush - 1) / p.flush;
+        const uint32_t lane_base = tmem_base + ((uint32_t)(quad * 32) << 16);
+        uint32_t chunk = 0;
+        for (int t = pair; t < p.n_tiles; t += n_pairs) {
+            const int m0 = (2 * (t / p.n_tiles_n) + (int)rank) * TC_BM, n0 = (t % p.n_tiles_n) * p.bn;
+            const int row = m0 + quad * 32 + lane;
+            const bool row_ok = row < p.M;
+            float acc[4][32];
+#pragma unroll
+            for (int gi = 0; gi < 4; ++gi)
+#pragma unroll
+                for (int j = 0; j < 32; ++j) acc[gi][j] = 0.f;
+            for (int c = 0; c < n_chunks; ++c, ++chunk) {
+                const int a = chunk & 1;
+                mbar_wait(bar_tfull(a), (chunk >> 1) & 1);
+                tcgen05_fence_after();
+#pragma unroll
+                for (int gi = 0; gi < 4; ++gi) {
+                    const int g = 2 * gi + half;
+                    if (g < n_groups) {
+                        uint32_t v[32];
+                        tmem_ld_32x32(lane_base + (uint32_t)(a * TC_BN_MAX + g * 32), v);
+                        tmem_ld_wait();
+#pragma unroll
+                        for (int j = 0; j < 32; ++j) acc[gi][j] += __uint_as_float(v[j]);
+                    }
+                }
+                tcgen05_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive_cluster(bar_tempty(a), 0);
+            }
+            tc_store_tile<EPI>(p, acc, m0, n0, quad, lane, half, n_groups, row_ok);
+        }
+    }
+
+    tcgen05_fence_before();
+    cluster_sync_all();  // no CTA leaves while its partner may still signal it or read its shared memory
+    if (warp == 1) tmem_dealloc_pair<512>(tmem_base);
+}
+
+template <int BK, int EPI>
+static int tc_launch_pair(const CUtensorMap &tmA, const CUtensorMap &tmB, const TcArgs &args, cudaStream_t st) {
+    using Cfg = TcPairCfg<BK>;
+    static bool attr_set = false;
+    if (!attr_set) {
+        GMNN_CUDA(cudaFuncSetAttribute(k_gemm_tc_pair<BK, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES));
+        attr_set = true;
+    }
+    int grid = 2 * args.n_tiles < tc_num_sms() ? 2 * args.n_tiles : (tc_num_sms() & ~1);
+    k_gemm_tc_pair<BK, EPI><<<grid, TC_THREADS, Cfg::SMEM_BYTES, st>>>(tmA, tmB, args);
+    GMNN_LAUNCHED();
+    GMNN_CUDA(cudaGetLastError());
+    return GMNN_OK;
 }
 
 // ---- host side --------------------------------------------------------------------------------
@@ -418,6 +639,7 @@ static int tc_launch(const CUtensorMap &tmA, const CUtensorMap &tmB, const TcArg
     return GMNN_OK;
 }
 
+int g_tc_pair = 1;    // knob "tc_pair": 3xTF32 GEMMs on CTA pairs (cta_group::2)
 int g_tc_debug = 0;
 int g_tc_flush_k = 64;   // knob "tc_flush_k": K extent between accumulator flushes of the 3xTF32 mode
 int g_tc_split_bk = 32;  // knob (gmnn_system_set_int "tc_split_bk"): K extent of a 3xTF32 stage, 16 or 32
@@ -448,6 +670,23 @@ int tc_gemm(bool split, int epi, int64_t M, int N, int K, const float *A, const 
         case EPI_PLAIN: return tc_launch<SP, BKV, EPI_PLAIN>(tmA, tmB, a, st);             \
         case EPI_HIDDEN: return tc_launch<SP, BKV, EPI_HIDDEN>(tmA, tmB, a, st);           \
         default: return tc_launch<SP, BKV, EPI_MUL>(tmA, tmB, a, st);                      \
+    }
+    if (split && g_tc_pair) {
+        // pair tiles: two adjacent 128-row tiles x one column tile; B box = this CTA's half of the columns
+        a.n_tiles = (int)(((M + TC_BM - 1) / TC_BM + 1) / 2) * a.n_tiles_n;
+        if ((rc = make_tmap(&tmB, Bt, N, K, a.bn / 2, BK))) return rc;
+        if (BK == 32) {
+            switch (epi) {
+                case EPI_PLAIN: return tc_launch_pair<32, EPI_PLAIN>(tmA, tmB, a, st);
+                case EPI_HIDDEN: return tc_launch_pair<32, EPI_HIDDEN>(tmA, tmB, a, st);
+                default: return tc_launch_pair<32, EPI_MUL>(tmA, tmB, a, st);
+            }
+        }
+        switch (epi) {
+            case EPI_PLAIN: return tc_launch_pair<16, EPI_PLAIN>(tmA, tmB, a, st);
+            case EPI_HIDDEN: return tc_launch_pair<16, EPI_HIDDEN>(tmA, tmB, a, st);
+            default: return tc_launch_pair<16, EPI_MUL>(tmA, tmB, a, st);
+        }
     }
     if (!split) { TC_CASE(false, 32) }
     if (BK == 32) { TC_CASE(true, 32) }
