@@ -49,7 +49,7 @@ struct TcCfg {
     static constexpr int B_BYTES = TC_BN_MAX * BK * 4;
     static constexpr int STAGE_BYTES = (A_BYTES + B_BYTES) * (SPLIT ? 2 : 1);
     static constexpr int NST = TC_STAGE_BYTES_TOTAL / STAGE_BYTES;
-    static constexpr int SMEM_BYTES = NST * STAGE_BYTES + 1024 /*alignment slack*/ + 512 /*barriers*/ + 4096 /*timeline (debug 32)*/;
+    static constexpr int SMEM_BYTES = NST * STAGE_BYTES + 1024 /*alignment slack*/ + 512 /*barriers*/;
     static_assert(NST >= 2, "pipeline needs at least two stages");
 };
 
@@ -70,6 +70,27 @@ __device__ __forceinline__ void swish_pair_tc(float z, float &h, float &d) {
     const float s = __fdividef(1.f, 1.f + __expf(-z));  // ex2.approx + rcp.approx: ~2 ulp, no slow path
     h = z * s;
     d = s * (1.f + z * (1.f - s));
+}
+
+// hi = tf32(x) (round to nearest) in place, lo = x - hi beside it, for `n4` float4 of one operand
+// tile, by 128 threads.  Eight independent loads are issued before the first store: hi and lo tiles
+// may alias as far as the compiler knows, so a plain loop would serialise load -> store -> load.
+__device__ __forceinline__ void split_hi_lo(float4 *hi, float4 *lo, int n4, int tid) {
+    for (int q0 = tid; q0 < n4; q0 += 8 * 128) {
+        float4 v[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u)
+            if (q0 + u * 128 < n4) v[u] = hi[q0 + u * 128];
+#pragma unroll
+        for (int u = 0; u < 8; ++u)
+            if (q0 + u * 128 < n4) {
+                float4 h, l;
+                h.x = to_tf32_rna(v[u].x); h.y = to_tf32_rna(v[u].y); h.z = to_tf32_rna(v[u].z); h.w = to_tf32_rna(v[u].w);
+                l.x = v[u].x - h.x; l.y = v[u].y - h.y; l.z = v[u].z - h.z; l.w = v[u].w - h.w;
+                hi[q0 + u * 128] = h;
+                lo[q0 + u * 128] = l;
+            }
+    }
 }
 
 // Fused elementwise and stores of one finished tile held in the epilogue warps' registers.
@@ -140,9 +161,6 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
     const uint32_t tmem_slot = bar_base + 8u * (3 * NST + 4);
     volatile uint32_t *tmem_slot_gen = reinterpret_cast<volatile uint32_t *>(smem_gen + (size_t)NST * Cfg::STAGE_BYTES + 8 * (3 * NST + 4));
 
-    long long *ts = reinterpret_cast<long long *>(smem_gen + (size_t)NST * Cfg::STAGE_BYTES + 512);  // [8][64]
-    const bool tl = (p.debug & 32) && blockIdx.x == 0;
-#define TL(role, idx) do { if (tl && (idx) >= 64 && (idx) < 128) ts[(role) * 64 + (idx) - 64] = clock64(); } while (0)
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int nkb = (p.K + BK - 1) / BK;  // pipeline stages per tile; chunk c covers stages [c*flush, (c+1)*flush)
 
@@ -177,7 +195,6 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
                 for (int kb = 0; kb < nkb; ++kb, ++it) {
                     const int s = it % NST;
                     mbar_wait(bar_empty(s), ((it / NST) & 1) ^ 1);
-                    TL(0, it);
                     mbar_arrive_expect_tx(bar_full(s), tx);
                     for (int q = 0; q < 4; ++q)  // four 32-atom column blocks of the tile, [BK][32 floats] each
                         tma_load_2d(a_hi(s) + q * (BK * 128), &tmA, bar_full(s), q * 32, (m0 / TC_BM) * p.K + kb * BK);
@@ -194,16 +211,12 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
                     const int a = chunk & 1;
                     const uint32_t d_tmem = tmem_base + (uint32_t)a * TC_BN_MAX;
                     if (in_chunk == 0) {
-                        TL(5, it);
                         mbar_wait(bar_tempty(a), ((chunk >> 1) & 1) ^ 1);
                         tcgen05_fence_after();
-                        TL(6, it);
                     }
                     const int s = it % NST;
-                    TL(3, it);
                     mbar_wait(SPLIT ? bar_split(s) : bar_full(s), (it / NST) & 1);
                     tcgen05_fence_after();
-                    TL(4, it);
                     const int krem = p.K - kb * BK;
                     const int ksteps = krem >= BK ? BK / 8 : (krem + 7) / 8;
                     const uint64_t da_hi = make_smem_desc_mn128(a_hi(s), BK * 128), db_hi = make_smem_desc<Cfg::SWZ>(b_hi(s));
@@ -242,33 +255,17 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
                 for (int kb = 0; kb < nkb; ++kb, ++it) {
                     const int s = it % NST;
                     mbar_wait(bar_full(s), (it / NST) & 1);
-                    if (tid == 0) TL(1, it);
                     float4 *ah = reinterpret_cast<float4 *>(smem_gen + (size_t)s * Cfg::STAGE_BYTES);
                     float4 *al = reinterpret_cast<float4 *>(smem_gen + (size_t)s * Cfg::STAGE_BYTES + Cfg::A_BYTES);
                     float4 *bh = reinterpret_cast<float4 *>(smem_gen + (size_t)s * Cfg::STAGE_BYTES + 2 * Cfg::A_BYTES);
                     float4 *bl = reinterpret_cast<float4 *>(smem_gen + (size_t)s * Cfg::STAGE_BYTES + 2 * Cfg::A_BYTES + Cfg::B_BYTES);
-#pragma unroll 4
-                    for (int q = tid; q < ((p.debug & 1) ? 0 : n_a4 + n_b4); q += 128) {
-                        float4 *ph = q < n_a4 ? ah + q : bh + (q - n_a4);
-                        float4 *pl = q < n_a4 ? al + q : bl + (q - n_a4);
-                        const float4 v = *ph;
-                        float4 h, l;
-                        if (p.debug & 128) {  // experiment: leave hi to the tensor core's own truncation
-                            h.x = __uint_as_float(__float_as_uint(v.x) & 0xFFFFE000u); h.y = __uint_as_float(__float_as_uint(v.y) & 0xFFFFE000u);
-                            h.z = __uint_as_float(__float_as_uint(v.z) & 0xFFFFE000u); h.w = __uint_as_float(__float_as_uint(v.w) & 0xFFFFE000u);
-                            l.x = v.x - h.x; l.y = v.y - h.y; l.z = v.z - h.z; l.w = v.w - h.w;
-                            *pl = l;
-                            continue;
-                        }
-                        h.x = to_tf32_rna(v.x); h.y = to_tf32_rna(v.y); h.z = to_tf32_rna(v.z); h.w = to_tf32_rna(v.w);
-                        l.x = v.x - h.x; l.y = v.y - h.y; l.z = v.z - h.z; l.w = v.w - h.w;
-                        *ph = h;
-                        *pl = l;
+                    if (!(p.debug & 1)) {
+                        split_hi_lo(ah, al, n_a4, tid);
+                        split_hi_lo(bh, bl, n_b4, tid);
                     }
                     fence_proxy_async_smem();
                     __syncwarp();
                     if (lane == 0) mbar_arrive(bar_split(s));
-                    if (tid == 0) TL(2, it);
                 }
             }
         }
@@ -315,12 +312,6 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
 
     tcgen05_fence_before();
     __syncthreads();
-    if (tl && threadIdx.x == 0) {
-        for (int q = 0; q < 64; ++q)
-            printf("it %d  prod %lld  full %lld  splitdone %lld  mma_wait_begin %lld  mma_go %lld | tempty wait %lld..%lld\n", q + 64,
-                   ts[q] - ts[0], ts[64 + q] - ts[0], ts[128 + q] - ts[0], ts[192 + q] - ts[0], ts[256 + q] - ts[0],
-                   ts[320 + q] - ts[0], ts[384 + q] - ts[0]);
-    }
     if (warp == 1) tmem_dealloc<512>(tmem_base);
 }
 
@@ -461,17 +452,8 @@ k_gemm_tc_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                 float4 *al = ah + Cfg::A_BYTES / 16;
                 float4 *bh = ah + 2 * Cfg::A_BYTES / 16;
                 float4 *bl = bh + Cfg::B_BYTES / 16;
-#pragma unroll 4
-                for (int q = tid; q < n_a4 + n_b4; q += 128) {
-                    float4 *ph = q < n_a4 ? ah + q : bh + (q - n_a4);
-                    float4 *pl = q < n_a4 ? al + q : bl + (q - n_a4);
-                    const float4 v = *ph;
-                    float4 h, l;
-                    h.x = to_tf32_rna(v.x); h.y = to_tf32_rna(v.y); h.z = to_tf32_rna(v.z); h.w = to_tf32_rna(v.w);
-                    l.x = v.x - h.x; l.y = v.y - h.y; l.z = v.z - h.z; l.w = v.w - h.w;
-                    *ph = h;
-                    *pl = l;
-                }
+                split_hi_lo(ah, al, n_a4, tid);
+                split_hi_lo(bh, bl, n_b4, tid);
                 fence_proxy_async_all();
                 __syncwarp();
                 if (lane == 0) mbar_arrive_cluster(bar_split(s), 0);
