@@ -170,49 +170,52 @@ k_build_cells(int64_t N, const float4 *__restrict__ pos4, const int32_t *__restr
               uint16_t *runs) {
     if (skip_rebuild(cond, thr2)) return;
     const int lane = threadIdx.x & 31;
-    const int64_t i = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
-    if (i >= N) return;
-    const float4 xi = pos4[i];
-    const int cx = cell_coord(xi.x, g.inv_edge[0], g.ncell[0]);
-    const int cy = cell_coord(xi.y, g.inv_edge[1], g.ncell[1]);
-    const int cz = cell_coord(xi.z, g.inv_edge[2], g.ncell[2]);
-    uint32_t *row = nbr + i * (int64_t)cap;
-    int n = 0;
-    // 27 cells in the fixed order idx = (oz+1)*9 + (oy+1)*3 + (ox+1); runs[idx] = first slot of the
-    // cell's run in this row (entries of a run ascend in atom index).  The reverse-pair index uses
-    // the runs: the partner of an entry in run idx sits in run 26 - idx of the partner's row.
-    for (int idx = 0; idx < 27; ++idx) {
-        if (runs && lane == 0) runs[i * RUNS_PITCH + idx] = (uint16_t)(n < cap ? n : cap);
-        const int oz = idx / 9 - 1, oy = (idx / 3) % 3 - 1, ox = idx % 3 - 1;
-        int z = cz + oz, nz = 0;
-        if (z < 0) { if (!g.pbc[2]) continue; z += g.ncell[2]; nz = -1; }
-        else if (z >= g.ncell[2]) { if (!g.pbc[2]) continue; z -= g.ncell[2]; nz = 1; }
-        int y = cy + oy, ny = 0;
-        if (y < 0) { if (!g.pbc[1]) continue; y += g.ncell[1]; ny = -1; }
-        else if (y >= g.ncell[1]) { if (!g.pbc[1]) continue; y -= g.ncell[1]; ny = 1; }
-        int x = cx + ox, nx = 0;
-        if (x < 0) { if (!g.pbc[0]) continue; x += g.ncell[0]; nx = -1; }
-        else if (x >= g.ncell[0]) { if (!g.pbc[0]) continue; x -= g.ncell[0]; nx = 1; }
-        const int c = (z * g.ncell[1] + y) * g.ncell[0] + x;
-        const int b = cell_start[c], e = cell_start[c + 1];
-        const float sx = __fmul_rn((float)nx, g.L[0]), sy = __fmul_rn((float)ny, g.L[1]),
-                    sz = __fmul_rn((float)nz, g.L[2]);
-        const uint32_t code = image_code(nx, ny, nz);
-        const bool home = (nx | ny | nz) == 0;
-        for (int base = b; base < e; base += 32) {
-            const int j = base + lane;
-            bool keep = false;
-            if (j < e && !(home && j == (int)i)) keep = in_list(xi, pos4[j], sx, sy, sz, g.r_list2);
-            const unsigned m = __ballot_sync(0xffffffffu, keep);
-            const int p = n + __popc(m & ((1u << lane) - 1u));
-            if (keep && p < cap) row[p] = (uint32_t)j | code;
-            n += __popc(m);
+    // grid-stride over atoms (one warp each): the launch is a few waves of blocks, so that the
+    // every-step launches that skip_rebuild() turns into no-ops stay cheap
+    const int64_t n_warps = (gridDim.x * (int64_t)blockDim.x) >> 5;
+    for (int64_t i = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5; i < N; i += n_warps) {
+        const float4 xi = pos4[i];
+        const int cx = cell_coord(xi.x, g.inv_edge[0], g.ncell[0]);
+        const int cy = cell_coord(xi.y, g.inv_edge[1], g.ncell[1]);
+        const int cz = cell_coord(xi.z, g.inv_edge[2], g.ncell[2]);
+        uint32_t *row = nbr + i * (int64_t)cap;
+        int n = 0;
+        // 27 cells in the fixed order idx = (oz+1)*9 + (oy+1)*3 + (ox+1); runs[idx] = first slot of the
+        // cell's run in this row (entries of a run ascend in atom index).  The reverse-pair index uses
+        // the runs: the partner of an entry in run idx sits in run 26 - idx of the partner's row.
+        for (int idx = 0; idx < 27; ++idx) {
+            if (runs && lane == 0) runs[i * RUNS_PITCH + idx] = (uint16_t)(n < cap ? n : cap);
+            const int oz = idx / 9 - 1, oy = (idx / 3) % 3 - 1, ox = idx % 3 - 1;
+            int z = cz + oz, nz = 0;
+            if (z < 0) { if (!g.pbc[2]) continue; z += g.ncell[2]; nz = -1; }
+            else if (z >= g.ncell[2]) { if (!g.pbc[2]) continue; z -= g.ncell[2]; nz = 1; }
+            int y = cy + oy, ny = 0;
+            if (y < 0) { if (!g.pbc[1]) continue; y += g.ncell[1]; ny = -1; }
+            else if (y >= g.ncell[1]) { if (!g.pbc[1]) continue; y -= g.ncell[1]; ny = 1; }
+            int x = cx + ox, nx = 0;
+            if (x < 0) { if (!g.pbc[0]) continue; x += g.ncell[0]; nx = -1; }
+            else if (x >= g.ncell[0]) { if (!g.pbc[0]) continue; x -= g.ncell[0]; nx = 1; }
+            const int c = (z * g.ncell[1] + y) * g.ncell[0] + x;
+            const int b = cell_start[c], e = cell_start[c + 1];
+            const float sx = __fmul_rn((float)nx, g.L[0]), sy = __fmul_rn((float)ny, g.L[1]),
+                        sz = __fmul_rn((float)nz, g.L[2]);
+            const uint32_t code = image_code(nx, ny, nz);
+            const bool home = (nx | ny | nz) == 0;
+            for (int base = b; base < e; base += 32) {
+                const int j = base + lane;
+                bool keep = false;
+                if (j < e && !(home && j == (int)i)) keep = in_list(xi, pos4[j], sx, sy, sz, g.r_list2);
+                const unsigned m = __ballot_sync(0xffffffffu, keep);
+                const int p = n + __popc(m & ((1u << lane) - 1u));
+                if (keep && p < cap) row[p] = (uint32_t)j | code;
+                n += __popc(m);
+            }
         }
-    }
-    if (runs && lane == 0) runs[i * RUNS_PITCH + 27] = (uint16_t)(n < cap ? n : cap);
-    if (lane == 0) {
-        count[i] = n < cap ? n : cap;
-        if (n > cap) atomicMax(&flags[FLAG_MAXCOUNT], n);
+        if (runs && lane == 0) runs[i * RUNS_PITCH + 27] = (uint16_t)(n < cap ? n : cap);
+        if (lane == 0) {
+            count[i] = n < cap ? n : cap;
+            if (n > cap) atomicMax(&flags[FLAG_MAXCOUNT], n);
+        }
     }
 }
 
@@ -223,31 +226,34 @@ k_build_small(int64_t N, const float4 *__restrict__ pos4, Geometry g, uint32_t *
               int32_t *flags, const int32_t *cond, float thr2) {
     if (skip_rebuild(cond, thr2)) return;
     const int lane = threadIdx.x & 31;
-    const int64_t i = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
-    if (i >= N) return;
-    const float4 xi = pos4[i];
-    uint32_t *row = nbr + i * (int64_t)cap;
-    int n = 0;
-    for (int nz = -g.kimg[2]; nz <= g.kimg[2]; ++nz)
-        for (int ny = -g.kimg[1]; ny <= g.kimg[1]; ++ny)
-            for (int nx = -g.kimg[0]; nx <= g.kimg[0]; ++nx) {
-                const float sx = __fmul_rn((float)nx, g.L[0]), sy = __fmul_rn((float)ny, g.L[1]),
-                            sz = __fmul_rn((float)nz, g.L[2]);
-                const uint32_t code = image_code(nx, ny, nz);
-                const bool home = (nx | ny | nz) == 0;
-                for (int base = 0; base < (int)N; base += 32) {
-                    const int j = base + lane;
-                    bool keep = false;
-                    if (j < (int)N && !(home && j == (int)i)) keep = in_list(xi, pos4[j], sx, sy, sz, g.r_list2);
-                    const unsigned m = __ballot_sync(0xffffffffu, keep);
-                    const int p = n + __popc(m & ((1u << lane) - 1u));
-                    if (keep && p < cap) row[p] = (uint32_t)j | code;
-                    n += __popc(m);
+    // grid-stride over atoms (one warp each): the launch is a few waves of blocks, so that the
+    // every-step launches that skip_rebuild() turns into no-ops stay cheap
+    const int64_t n_warps = (gridDim.x * (int64_t)blockDim.x) >> 5;
+    for (int64_t i = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5; i < N; i += n_warps) {
+        const float4 xi = pos4[i];
+        uint32_t *row = nbr + i * (int64_t)cap;
+        int n = 0;
+        for (int nz = -g.kimg[2]; nz <= g.kimg[2]; ++nz)
+            for (int ny = -g.kimg[1]; ny <= g.kimg[1]; ++ny)
+                for (int nx = -g.kimg[0]; nx <= g.kimg[0]; ++nx) {
+                    const float sx = __fmul_rn((float)nx, g.L[0]), sy = __fmul_rn((float)ny, g.L[1]),
+                                sz = __fmul_rn((float)nz, g.L[2]);
+                    const uint32_t code = image_code(nx, ny, nz);
+                    const bool home = (nx | ny | nz) == 0;
+                    for (int base = 0; base < (int)N; base += 32) {
+                        const int j = base + lane;
+                        bool keep = false;
+                        if (j < (int)N && !(home && j == (int)i)) keep = in_list(xi, pos4[j], sx, sy, sz, g.r_list2);
+                        const unsigned m = __ballot_sync(0xffffffffu, keep);
+                        const int p = n + __popc(m & ((1u << lane) - 1u));
+                        if (keep && p < cap) row[p] = (uint32_t)j | code;
+                        n += __popc(m);
+                    }
                 }
-            }
-    if (lane == 0) {
-        count[i] = n < cap ? n : cap;
-        if (n > cap) atomicMax(&flags[FLAG_MAXCOUNT], n);
+        if (lane == 0) {
+            count[i] = n < cap ? n : cap;
+            if (n > cap) atomicMax(&flags[FLAG_MAXCOUNT], n);
+        }
     }
 }
 
@@ -261,36 +267,39 @@ k_build_rev(int64_t N, const uint32_t *__restrict__ nbr, const int32_t *__restri
             int32_t *flags, const int32_t *cond, float thr2) {
     if (skip_rebuild(cond, thr2)) return;
     const int lane = threadIdx.x & 31;
-    const int64_t i = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
-    if (i >= N) return;
-    const int cnt = count[i];
-    const uint32_t *row = nbr + i * (int64_t)cap;
-    for (int k0 = 0; k0 < cnt; k0 += 32) {
-        const uint32_t e_mine = k0 + lane < cnt ? row[k0 + lane] : 0u;
-        int found = 0xFFFF;
-        const int nk = cnt - k0 < 32 ? cnt - k0 : 32;
-        for (int t = 0; t < nk; ++t) {
-            const uint32_t e = __shfl_sync(0xffffffffu, e_mine, t);
-            const int64_t j = e & NBR_J_MASK;
-            const uint32_t img = e >> NBR_J_BITS;  // three 3-bit fields n + 4; the inverse image is 8 - field
-            const uint32_t inv = (8u - (img & 7u)) | ((8u - ((img >> 3) & 7u)) << 3) | ((8u - ((img >> 6) & 7u)) << 6);
-            const uint32_t target = (uint32_t)i | (inv << NBR_J_BITS);
-            const uint32_t *rj = nbr + j * (int64_t)cap;
-            const int cj = count[j];
-            int pos = 0xFFFF;
-            for (int b = 0; b < cj; b += 32) {
-                const bool hit = b + lane < cj && rj[b + lane] == target;
-                const unsigned m = __ballot_sync(0xffffffffu, hit);
-                if (m) {
-                    pos = b + __ffs(m) - 1;
-                    break;
+    // grid-stride over atoms (one warp each): the launch is a few waves of blocks, so that the
+    // every-step launches that skip_rebuild() turns into no-ops stay cheap
+    const int64_t n_warps = (gridDim.x * (int64_t)blockDim.x) >> 5;
+    for (int64_t i = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5; i < N; i += n_warps) {
+        const int cnt = count[i];
+        const uint32_t *row = nbr + i * (int64_t)cap;
+        for (int k0 = 0; k0 < cnt; k0 += 32) {
+            const uint32_t e_mine = k0 + lane < cnt ? row[k0 + lane] : 0u;
+            int found = 0xFFFF;
+            const int nk = cnt - k0 < 32 ? cnt - k0 : 32;
+            for (int t = 0; t < nk; ++t) {
+                const uint32_t e = __shfl_sync(0xffffffffu, e_mine, t);
+                const int64_t j = e & NBR_J_MASK;
+                const uint32_t img = e >> NBR_J_BITS;  // three 3-bit fields n + 4; the inverse image is 8 - field
+                const uint32_t inv = (8u - (img & 7u)) | ((8u - ((img >> 3) & 7u)) << 3) | ((8u - ((img >> 6) & 7u)) << 6);
+                const uint32_t target = (uint32_t)i | (inv << NBR_J_BITS);
+                const uint32_t *rj = nbr + j * (int64_t)cap;
+                const int cj = count[j];
+                int pos = 0xFFFF;
+                for (int b = 0; b < cj; b += 32) {
+                    const bool hit = b + lane < cj && rj[b + lane] == target;
+                    const unsigned m = __ballot_sync(0xffffffffu, hit);
+                    if (m) {
+                        pos = b + __ffs(m) - 1;
+                        break;
+                    }
                 }
+                if (lane == t) found = pos;
             }
-            if (lane == t) found = pos;
-        }
-        if (k0 + lane < cnt) {
-            rev[i * (int64_t)cap + k0 + lane] = (uint16_t)found;
-            if (found == 0xFFFF) flags[FLAG_REV_MISSING] = 1;
+            if (k0 + lane < cnt) {
+                rev[i * (int64_t)cap + k0 + lane] = (uint16_t)found;
+                if (found == 0xFFFF) flags[FLAG_REV_MISSING] = 1;
+            }
         }
     }
 }
@@ -303,32 +312,35 @@ k_build_rev_runs(int64_t N, const uint32_t *__restrict__ nbr, const int32_t *__r
                  const uint16_t *__restrict__ runs, uint16_t *rev, int32_t *flags, const int32_t *cond, float thr2) {
     if (skip_rebuild(cond, thr2)) return;
     const int lane = threadIdx.x & 31;
-    const int64_t i = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
-    if (i >= N) return;
-    const int cnt = count[i];
-    const uint32_t *row = nbr + i * (int64_t)cap;
-    const int my_run_start = lane < RUNS_PITCH ? (int)runs[i * RUNS_PITCH + lane] : 0x7fffffff;
-    for (int k0 = 0; k0 < cnt; k0 += 32) {
-        const int k = k0 + lane;
-        int r = -1;  // run of slot k: number of run starts <= k, minus one
-#pragma unroll
-        for (int q = 0; q < 27; ++q) r += __shfl_sync(0xffffffffu, my_run_start, q) <= k ? 1 : 0;
-        if (k < cnt) {
-            const uint32_t e = row[k];
-            const int64_t j = e & NBR_J_MASK;
-            const uint32_t img = e >> NBR_J_BITS;
-            const uint32_t inv = (8u - (img & 7u)) | ((8u - ((img >> 3) & 7u)) << 3) | ((8u - ((img >> 6) & 7u)) << 6);
-            const uint32_t target = (uint32_t)i | (inv << NBR_J_BITS);
-            const uint32_t *rj = nbr + j * (int64_t)cap;
-            const int s0 = runs[j * RUNS_PITCH + (26 - r)], s1 = runs[j * RUNS_PITCH + (27 - r)];
-            int found = 0xFFFF;
-            for (int t = s0; t < s1; ++t)
-                if (rj[t] == target) {
-                    found = t;
-                    break;
-                }
-            rev[i * (int64_t)cap + k] = (uint16_t)found;
-            if (found == 0xFFFF) flags[FLAG_REV_MISSING] = 1;
+    // grid-stride over atoms (one warp each): the launch is a few waves of blocks, so that the
+    // every-step launches that skip_rebuild() turns into no-ops stay cheap
+    const int64_t n_warps = (gridDim.x * (int64_t)blockDim.x) >> 5;
+    for (int64_t i = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5; i < N; i += n_warps) {
+        const int cnt = count[i];
+        const uint32_t *row = nbr + i * (int64_t)cap;
+        const int my_run_start = lane < RUNS_PITCH ? (int)runs[i * RUNS_PITCH + lane] : 0x7fffffff;
+        for (int k0 = 0; k0 < cnt; k0 += 32) {
+            const int k = k0 + lane;
+            int r = -1;  // run of slot k: number of run starts <= k, minus one
+    #pragma unroll
+            for (int q = 0; q < 27; ++q) r += __shfl_sync(0xffffffffu, my_run_start, q) <= k ? 1 : 0;
+            if (k < cnt) {
+                const uint32_t e = row[k];
+                const int64_t j = e & NBR_J_MASK;
+                const uint32_t img = e >> NBR_J_BITS;
+                const uint32_t inv = (8u - (img & 7u)) | ((8u - ((img >> 3) & 7u)) << 3) | ((8u - ((img >> 6) & 7u)) << 6);
+                const uint32_t target = (uint32_t)i | (inv << NBR_J_BITS);
+                const uint32_t *rj = nbr + j * (int64_t)cap;
+                const int s0 = runs[j * RUNS_PITCH + (26 - r)], s1 = runs[j * RUNS_PITCH + (27 - r)];
+                int found = 0xFFFF;
+                for (int t = s0; t < s1; ++t)
+                    if (rj[t] == target) {
+                        found = t;
+                        break;
+                    }
+                rev[i * (int64_t)cap + k] = (uint16_t)found;
+                if (found == 0xFFFF) flags[FLAG_REV_MISSING] = 1;
+            }
         }
     }
 }
@@ -340,6 +352,11 @@ __global__ void k_finish_rebuild(int32_t *flags, const int32_t *cond, float thr2
 }
 
 static inline unsigned nblocks(int64_t n, int per) { return (unsigned)((n + per - 1) / per); }
+// blocks of 256 threads for a warp-per-atom grid-stride kernel: at most 16 waves of 148 SMs x 8 blocks
+static inline unsigned warp_grid(int64_t n_atoms) {
+    const int64_t want = (n_atoms * 32 + 255) / 256, cap = 148 * 8 * 16;
+    return (unsigned)(want < cap ? want : cap);
+}
 
 int launch_build(gmnn_system *s, const float *positions, cudaStream_t st, const int32_t *cond, float thr2,
                  bool wrap_first, float *positions_mut) {
@@ -363,17 +380,17 @@ int launch_build(gmnn_system *s, const float *positions, cudaStream_t st, const 
                                               nullptr, cond, thr2);
     GMNN_LAUNCHED();
     if (s->small_box)
-        k_build_small<<<nblocks(N * 32, 256), 256, 0, st>>>(N, s->pos4, g, s->nbr, s->count, s->cap, s->flags, cond, thr2);
+        k_build_small<<<warp_grid(N), 256, 0, st>>>(N, s->pos4, g, s->nbr, s->count, s->cap, s->flags, cond, thr2);
     else
-        k_build_cells<<<nblocks(N * 32, 256), 256, 0, st>>>(N, s->pos4, s->cell_start, g, s->nbr, s->count, s->cap,
+        k_build_cells<<<warp_grid(N), 256, 0, st>>>(N, s->pos4, s->cell_start, g, s->nbr, s->count, s->cap,
                                                             s->flags, cond, thr2,
                                                             s->force_mode == GMNN_FORCE_PAIRBUF ? s->runs : nullptr);
     GMNN_LAUNCHED();
     if (s->force_mode == GMNN_FORCE_PAIRBUF) {
         if (s->small_box)
-            k_build_rev<<<nblocks(N * 32, 256), 256, 0, st>>>(N, s->nbr, s->count, s->cap, s->rev, s->flags, cond, thr2);
+            k_build_rev<<<warp_grid(N), 256, 0, st>>>(N, s->nbr, s->count, s->cap, s->rev, s->flags, cond, thr2);
         else
-            k_build_rev_runs<<<nblocks(N * 32, 256), 256, 0, st>>>(N, s->nbr, s->count, s->cap, s->runs, s->rev, s->flags,
+            k_build_rev_runs<<<warp_grid(N), 256, 0, st>>>(N, s->nbr, s->count, s->cap, s->runs, s->rev, s->flags,
                                                                    cond, thr2);
         GMNN_LAUNCHED();
     }
