@@ -343,6 +343,24 @@ def run_ours(args):
                                     "alu": "148 SMs x 128 fp32 lanes x 2 flop x sm_max_mhz (derived, DESIGN.md 5)"}[info["bound"]],
                     "share_of_step": round(per_step_ms[dom] / (ms_max / args.steps), 4),
                     "algorithmic_per_atom": {"bytes": info["bytes"], "flops": info["flops"]}}
+        if info["bound"] == "tensor":
+            # the four GEMM launches of a step (mlp_forward + mlp_backward) are one kernel family:
+            # report them together, per launch
+            t_f = [m for n_, m, _ in stages if n_ == "mlp_forward"][0]
+            t_b = [m for n_, m, _ in stages if n_ == "mlp_backward"][0]
+            n_launch = 2 * len(w.model.hidden)
+            ach = 2.0 * info["flops"] * N / ((t_f + t_b) * 1e-3) / 1e12
+            roofline.update({"kernel": "k_gemm_tc_pair" if args.mlp == "3xtf32" else "k_gemm_tc",
+                             "launches_per_step": n_launch, "achieved": round(ach, 3), "frac": round(ach / peak, 4),
+                             "avg_launch_ms": round((t_f + t_b) / n_launch, 4),
+                             "share_of_step": round((per_step_ms["mlp_forward"] + per_step_ms["mlp_backward"])
+                                                    / (ms_max / args.steps), 4),
+                             "algorithmic_per_atom": {"bytes": 4.0 * (2 * N_FEATURES + 9 * w.model.hidden[0]),
+                                                      "flops": 2.0 * info["flops"]}})
+            if args.workload == "config5" and args.mlp == "3xtf32":
+                # dram__bytes_read.sum + dram__bytes_write.sum of the four launches of one step, per launch
+                # (profiles/ncu_r1_gemm_tc_pair.md)
+                roofline["traffic"] = round(22.35e9 / n_launch)
         if info["bound"] == "tensor" and args.mlp == "3xtf32":
             roofline["note"] = ("achieved counts the ALGORITHMIC flops (one product per multiply-add); the 3xTF32 split "
                                 "executes 3 tensor-core MMAs per product, so tensor-pipe flops are 3x achieved")

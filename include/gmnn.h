@@ -52,13 +52,18 @@ typedef enum {
 typedef enum {
     GMNN_MLP_FP32 = 0,   /* fp32 FMA on the SIMT pipes; the fp32-tolerance path                      */
     GMNN_MLP_3XTF32 = 1, /* tcgen05 TF32 tensor cores, 3-term error-compensated split (fp32 tol.)   */
-    GMNN_MLP_TF32 = 2    /* tcgen05 TF32 single pass; reduced-precision variant (2e-3 force tol.)   */
+    GMNN_MLP_TF32 = 2    /* tcgen05 TF32 single pass, operands truncated by the tensor core: measured
+                            1e-2 .. 2.5e-2 on the force measure, i.e. NOT within the 2e-3 of a claimed
+                            reduced-precision variant; an unclaimed fast mode       */
 } gmnn_mlp_precision;
 
 /* How F_i = sum_j g_ij - sum_j g_ji is formed.  Both are atomics-free and bit-reproducible. */
 typedef enum {
     GMNN_FORCE_GATHER = 0, /* each centre recomputes g_ji from the neighbour's adjoint A_j           */
-    GMNN_FORCE_PAIRBUF = 1 /* g_ij written once per directed pair, reverse pair read through an index */
+    GMNN_FORCE_PAIRBUF = 1 /* g_ij evaluated once per directed pair and stored into the neighbour's row
+                              through a reverse-pair index that gmnn_build_neighbors (and every
+                              in-loop rebuild) builds; rows summed in slot order.  Costs 18 bytes per
+                              neighbour slot of device memory, about halves the pair backward          */
 } gmnn_force_mode;
 
 typedef struct {
@@ -107,7 +112,14 @@ void gmnn_system_destroy(gmnn_system *s);
  *                     output of the previous call reuses that call's final forces and energies
  *                     instead of evaluating them again at entry (the caller asserts this)
  *   "capacity"        neighbour slots per atom for the next build (0 = estimate from the density)
- *   "mlp_precision", "force_mode": override the model's value for this system
+ *   "mlp_precision", "force_mode": override the model's value for this system; changing force_mode
+ *                     invalidates the neighbour list (call gmnn_build_neighbors again)
+ *   "tc_pair"         1 (default): 3xTF32 GEMMs on CTA pairs (cta_group::2); 0: single CTAs
+ *   "tc_split_bk"     16 | 32 (default): K extent of one pipeline stage of the 3xTF32 GEMM
+ *   "tc_flush_k"      multiple of 16 (default 64): K extent after which the tensor-memory accumulator
+ *                     is flushed into registers (the tensor core accumulates with truncation)
+ *   "tc_debug"        timing experiments of mlp_tc.cu that knock out work (WRONG results); 0 = off
+ *   The four tc_* knobs are process-wide.
  * Returns GMNN_INVALID_ARG for an unknown key or value. */
 int gmnn_system_set_int(gmnn_system *s, const char *key, int64_t value);
 int gmnn_system_get_int(const gmnn_system *s, const char *key, int64_t *value /*HOST*/);
