@@ -245,11 +245,14 @@ struct CbSmem {  // shared-memory plan of k_contract_backward, in floats
     static constexpr int X = cmax(cmax(len(4), len(1) + len(3)) * TB, 4 * NR * PSI * CW);
     // slot Y: chunk 0, then chunk 2
     static constexpr int Y = cmax(len(0), len(2)) * TB;
-    static constexpr size_t BYTES = sizeof(float) * (X + Y) + 16;
+    static constexpr size_t bytes(int halves) { return sizeof(float) * (X + Y) * halves + 16 * halves; }
 };
 
-template <int NR>
-__global__ void __launch_bounds__(128, 2)
+// HALVES = 2: one 256-thread block per SM works on two tiles in lock step (the block-wide barriers
+// between chunks keep all eight warps inside the same stretch of the ~12 k-instruction straight-line
+// body, so they share its instruction-cache lines); HALVES = 1: two independent 128-thread blocks per SM.
+template <int NR, int HALVES>
+__global__ void __launch_bounds__(128 * HALVES, 3 - HALVES)
 k_contract_backward(int64_t N, const float *__restrict__ psi, const float *__restrict__ dGt,
                     const float4 *__restrict__ pos4, const float *__restrict__ scale, float *__restrict__ A) {
     using F = Feat<NR>;
@@ -257,15 +260,18 @@ k_contract_backward(int64_t N, const float *__restrict__ psi, const float *__res
     using SM = CbSmem<NR>;
     constexpr int TB = SM::TB;
     extern __shared__ __align__(128) float s_cb[];
-    float *sX = s_cb, *sY = s_cb + SM::X;
-    const uint32_t barX = tc::smem_u32(s_cb + SM::X + SM::Y), barY = barX + 8;
-    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-    const int64_t i = blockIdx.x * (int64_t)TB + tid;
-    const float *gt = dGt + blockIdx.x * (int64_t)(F::N * TB);  // this block's [F][128] tile
+    const int hf = threadIdx.x >> 7;  // which tile of the block
+    float *sX = s_cb + hf * (SM::X + SM::Y), *sY = sX + SM::X;
+    const uint32_t barX = tc::smem_u32(s_cb + HALVES * (SM::X + SM::Y)) + 16 * hf, barY = barX + 8;
+    const int tid = threadIdx.x & 127, lane = tid & 31, wid = tid >> 5;
+    const int64_t tile = blockIdx.x * (int64_t)HALVES + hf;
+    const bool active = tile * TB < N;  // the last block of an odd tile count has an idle half
+    const int64_t i = tile * TB + tid;
+    const float *gt = dGt + tile * (int64_t)(F::N * TB);  // this half's [F][128] tile
     auto issue = [&](float *dst, int c, uint32_t bar) {
         tc::bulk_load_1d(tc::smem_u32(dst), gt + CH::begin(c) * TB, (uint32_t)(SM::len(c) * TB * 4), bar);
     };
-    if (tid == 0) {
+    if (tid == 0 && active) {
         tc::mbar_init(barX, 1);
         tc::mbar_init(barY, 1);
         tc::fence_barrier_init();
@@ -307,26 +313,26 @@ k_contract_backward(int64_t N, const float *__restrict__ psi, const float *__res
             [&](int f) { return buf[(f - CH::begin(C)) * TB + tid]; },
             [&](int s, int m, float v) { acc[s][m] += v; });
     };
-    tc::mbar_wait(barY, 0);
+    if (active) tc::mbar_wait(barY, 0);
     run_chunk(std::integral_constant<int, 0>{}, sY);
     __syncthreads();
-    if (tid == 0) {
+    if (tid == 0 && active) {
         tc::fence_proxy_async_smem();
         tc::mbar_arrive_expect_tx(barY, (uint32_t)(SM::len(2) * TB * 4));
         issue(sY, 2, barY);
     }
-    tc::mbar_wait(barX, 0);
+    if (active) tc::mbar_wait(barX, 0);
     run_chunk(std::integral_constant<int, 4>{}, sX);
     __syncthreads();
-    if (tid == 0) {
+    if (tid == 0 && active) {
         tc::fence_proxy_async_smem();
         tc::mbar_arrive_expect_tx(barX, (uint32_t)((SM::len(1) + SM::len(3)) * TB * 4));
         issue(sX, 1, barX);
         issue(sX + SM::len(1) * TB, 3, barX);
     }
-    tc::mbar_wait(barY, 1);
+    if (active) tc::mbar_wait(barY, 1);
     run_chunk(std::integral_constant<int, 2>{}, sY);
-    tc::mbar_wait(barX, 1);
+    if (active) tc::mbar_wait(barX, 1);
     run_chunk(std::integral_constant<int, 1>{}, sX);
     run_chunk(std::integral_constant<int, 3>{}, sX + SM::len(1) * TB);
     __syncthreads();
@@ -643,15 +649,25 @@ int launch_contract_forward(gmnn_system *s, cudaStream_t st) {
     return GMNN_OK;
 }
 
+int g_cb_halves = 1;  // knob "cb_halves": tiles per block of k_contract_backward (1 or 2)
+
 int launch_contract_backward(gmnn_system *s, cudaStream_t st) {
     constexpr int NR = 5;
-    const size_t smem = CbSmem<NR>::BYTES;
     static bool attr_set = false;
     if (!attr_set) {
-        GMNN_CUDA(cudaFuncSetAttribute(k_contract_backward<NR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        GMNN_CUDA(cudaFuncSetAttribute(k_contract_backward<NR, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                       (int)CbSmem<NR>::bytes(1)));
+        GMNN_CUDA(cudaFuncSetAttribute(k_contract_backward<NR, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                       (int)CbSmem<NR>::bytes(2)));
         attr_set = true;
     }
-    k_contract_backward<NR><<<nblocks(s->N, 128), 128, smem, st>>>(s->N, s->psi, s->dG, s->pos4, s->model->scale, s->A);
+    const unsigned tiles = nblocks(s->N, 128);
+    if (g_cb_halves == 2)
+        k_contract_backward<NR, 2><<<(tiles + 1) / 2, 256, CbSmem<NR>::bytes(2), st>>>(s->N, s->psi, s->dG, s->pos4,
+                                                                                        s->model->scale, s->A);
+    else
+        k_contract_backward<NR, 1><<<tiles, 128, CbSmem<NR>::bytes(1), st>>>(s->N, s->psi, s->dG, s->pos4,
+                                                                              s->model->scale, s->A);
     GMNN_LAUNCHED();
     GMNN_CUDA(cudaGetLastError());
     return GMNN_OK;

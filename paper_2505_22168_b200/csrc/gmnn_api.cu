@@ -23,7 +23,7 @@ void set_error(const char *fmt, ...) {
 }
 
 int launch_mlp_forward_tc(gmnn_system *s, cudaStream_t st);
-extern int g_tc_split_bk, g_tc_flush_k, g_tc_debug, g_tc_pair;
+extern int g_tc_split_bk, g_tc_flush_k, g_tc_debug, g_tc_pair, g_cb_halves;
 int launch_mlp_backward_tc(gmnn_system *s, const float *head_w_dev, cudaStream_t st);
 
 template <class T>
@@ -197,7 +197,12 @@ int gmnn_create(const gmnn_hparams *hp, const gmnn_weights *w, gmnn_model **out)
         for (int a = 0; a < fi; ++a)
             for (int b = 0; b < fo; ++b) t[(size_t)b * fi + a] = w->W[l][(size_t)a * fo + b];
         if (!rc) rc = upload(&m->WT[l], t.data(), t.size());
+        if (!rc) rc = dev_alloc(&m->Ws[l], 2 * (size_t)fi * fo);
+        if (!rc) rc = dev_alloc(&m->WTs[l], 2 * (size_t)fi * fo);
+        if (!rc) rc = launch_split_stack(m->W[l], m->Ws[l], (int64_t)fi * fo, nullptr);
+        if (!rc) rc = launch_split_stack(m->WT[l], m->WTs[l], (int64_t)fi * fo, nullptr);
     }
+    if (!rc && cudaDeviceSynchronize() != cudaSuccess) rc = GMNN_CUDA_ERROR;
     if (!rc) rc = upload(&m->scale, w->scale, (size_t)hp->n_species);
     if (!rc) rc = upload(&m->shift, w->shift, (size_t)hp->n_species);
     if (!rc) {
@@ -218,6 +223,8 @@ void gmnn_destroy(gmnn_model *m) {
     for (int l = 0; l < MAX_LAYERS; ++l) {
         dev_free(m->W[l]);
         dev_free(m->WT[l]);
+        dev_free(m->Ws[l]);
+        dev_free(m->WTs[l]);
         dev_free(m->b[l]);
     }
     dev_free(m->scale);
@@ -272,6 +279,7 @@ int gmnn_system_create(const gmnn_model *m, int64_t n_atoms, const int32_t *spec
     A_(s->dZ[1], NP * maxw);
     A_(s->Bv, (size_t)m->dims[L] * m->dims[L - 1]);
     A_(s->BvT, (size_t)m->dims[L] * m->dims[L - 1]);
+    A_(s->BvTs, 2 * (size_t)m->dims[L] * m->dims[L - 1]);
     A_(s->vhead, (size_t)m->dims[L]);
     A_(s->head_w, (size_t)M);
     A_(s->e_heads, N * M);
@@ -300,7 +308,7 @@ void gmnn_system_destroy(gmnn_system *s) {
     dev_free(s->cell_fill); dev_free(s->slot_tmp); dev_free(s->perm); dev_free(s->pos4); dev_free(s->xref);
     dev_free(s->nbr); dev_free(s->rev); dev_free(s->gbuf); dev_free(s->runs); dev_free(s->count); dev_free(s->psi); dev_free(s->G); dev_free(s->dG); dev_free(s->A);
     for (int l = 0; l < MAX_LAYERS; ++l) { dev_free(s->H[l]); dev_free(s->D[l]); }
-    dev_free(s->dZ[0]); dev_free(s->dZ[1]); dev_free(s->Bv); dev_free(s->BvT); dev_free(s->vhead); dev_free(s->head_w);
+    dev_free(s->dZ[0]); dev_free(s->dZ[1]); dev_free(s->Bv); dev_free(s->BvT); dev_free(s->BvTs); dev_free(s->vhead); dev_free(s->head_w);
     dev_free(s->e_heads); dev_free(s->e_atom); dev_free(s->f_int); dev_free(s->f_tmp); dev_free(s->partial);
     dev_free(s->e_total); dev_free(s->flags);
     dev_free(s->stage_pos); dev_free(s->stage_f); dev_free(s->stage_e);
@@ -338,6 +346,9 @@ int gmnn_system_set_int(gmnn_system *s, const char *key, int64_t v) {
     } else if (!strcmp(key, "tc_split_bk")) {  // process-wide tuning knob of mlp_tc.cu
         if (v != 16 && v != 32) return GMNN_INVALID_ARG;
         gmnn::g_tc_split_bk = (int)v;
+    } else if (!strcmp(key, "cb_halves")) {  // process-wide: tiles per block of k_contract_backward
+        if (v != 1 && v != 2) return GMNN_INVALID_ARG;
+        gmnn::g_cb_halves = (int)v;
     } else if (!strcmp(key, "tc_pair")) {  // process-wide: 3xTF32 GEMMs on CTA pairs (1) or single CTAs (0)
         gmnn::g_tc_pair = v != 0;
     } else if (!strcmp(key, "tc_debug")) {  // timing experiments (wrong results), see mlp_tc.cu

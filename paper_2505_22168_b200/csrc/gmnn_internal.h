@@ -65,6 +65,10 @@ struct gmnn_model {
     float *beta = nullptr;     // [S*S][n_radial][kb] zero padded
     float *W[gmnn::MAX_LAYERS] = {};   // [fan_in][fan_out]
     float *WT[gmnn::MAX_LAYERS] = {};  // [fan_out][fan_in]
+    // tf32 hi / lo split of the two, stacked: rows [0, R) hold hi = tf32(w), rows [R, 2R) lo = w - hi
+    // (the B operands of the 3xTF32 GEMMs of mlp_tc.cu; split once here instead of per tile on chip)
+    float *Ws[gmnn::MAX_LAYERS] = {};   // [2 * fan_in][fan_out]
+    float *WTs[gmnn::MAX_LAYERS] = {};  // [2 * fan_out][fan_in]
     float *b[gmnn::MAX_LAYERS] = {};
     float *scale = nullptr, *shift = nullptr;  // [S]
     float *head_mean_w = nullptr;  // [n_heads] = 1/M (device)
@@ -103,6 +107,7 @@ struct gmnn_system {
     float *dZ[2] = {};
     float *Bv = nullptr;             // diag(v) W^T of the last hidden layer
     float *BvT = nullptr;            // its transpose: W diag(v), [fan_in][fan_out] (B operand of mlp_tc.cu)
+    float *BvTs = nullptr;           // stacked hi / lo split of BvT
     float *vhead = nullptr;          // [H_last]
     float *head_w = nullptr;         // [n_heads] weights of the differentiated energy
     float *e_heads = nullptr;        // [N][n_heads]
@@ -139,6 +144,9 @@ int launch_pair_forward(gmnn_system *s, cudaStream_t st);
 int launch_contract_forward(gmnn_system *s, cudaStream_t st);
 int launch_contract_backward(gmnn_system *s, cudaStream_t st);
 int launch_pair_backward(gmnn_system *s, cudaStream_t st);  // dispatches on force_mode
+
+// mlp_tc.cu
+int launch_split_stack(const float *src, float *dst, int64_t n, cudaStream_t st);  // dst[0..n) hi, dst[n..2n) lo
 
 // mlp_simt.cu
 int launch_mlp_forward_simt(gmnn_system *s, cudaStream_t st);

@@ -188,7 +188,7 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
         setmaxnreg_dec<TC_REGS_CONTROL>();
         if (warp == 0 && lane == 0) {
             // ===== TMA producer =====
-            const uint32_t tx = (uint32_t)(Cfg::A_BYTES + p.bn * BK * 4);
+            const uint32_t tx = (uint32_t)(Cfg::A_BYTES + p.bn * BK * 4 * (SPLIT ? 2 : 1));
             uint32_t it = 0;
             for (int t = blockIdx.x; t < p.n_tiles; t += gridDim.x) {
                 const int m0 = (t / p.n_tiles_n) * TC_BM, n0 = (t % p.n_tiles_n) * p.bn;
@@ -199,6 +199,7 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
                     for (int q = 0; q < 4; ++q)  // four 32-atom column blocks of the tile, [BK][32 floats] each
                         tma_load_2d(a_hi(s) + q * (BK * 128), &tmA, bar_full(s), q * 32, (m0 / TC_BM) * p.K + kb * BK);
                     tma_load_2d(b_hi(s), &tmB, bar_full(s), kb * BK, n0);
+                    if (SPLIT) tma_load_2d(b_lo(s), &tmB, bar_full(s), kb * BK, p.N + n0);  // lo rows follow the N hi rows
                 }
             }
         } else if (warp == 1 && lane == 0) {
@@ -249,7 +250,7 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
         // ===== splitters (3xTF32): hi = tf32(x) in place, lo = x - hi beside it =====
         if (SPLIT) {
             const int tid = threadIdx.x - TC_FIRST_SPLIT_WARP * 32;  // 0..127
-            const int n_a4 = Cfg::A_BYTES / 16, n_b4 = p.bn * BK * 4 / 16;
+            const int n_a4 = Cfg::A_BYTES / 16;
             uint32_t it = 0;
             for (int t = blockIdx.x; t < p.n_tiles; t += gridDim.x) {
                 for (int kb = 0; kb < nkb; ++kb, ++it) {
@@ -257,12 +258,7 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
                     mbar_wait(bar_full(s), (it / NST) & 1);
                     float4 *ah = reinterpret_cast<float4 *>(smem_gen + (size_t)s * Cfg::STAGE_BYTES);
                     float4 *al = reinterpret_cast<float4 *>(smem_gen + (size_t)s * Cfg::STAGE_BYTES + Cfg::A_BYTES);
-                    float4 *bh = reinterpret_cast<float4 *>(smem_gen + (size_t)s * Cfg::STAGE_BYTES + 2 * Cfg::A_BYTES);
-                    float4 *bl = reinterpret_cast<float4 *>(smem_gen + (size_t)s * Cfg::STAGE_BYTES + 2 * Cfg::A_BYTES + Cfg::B_BYTES);
-                    if (!(p.debug & 1)) {
-                        split_hi_lo(ah, al, n_a4, tid);
-                        split_hi_lo(bh, bl, n_b4, tid);
-                    }
+                    if (!(p.debug & 1)) split_hi_lo(ah, al, n_a4, tid);  // B arrives split (model->Ws / WTs)
                     fence_proxy_async_smem();
                     __syncwarp();
                     if (lane == 0) mbar_arrive(bar_split(s));
@@ -386,7 +382,7 @@ k_gemm_tc_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
         setmaxnreg_dec<TC_REGS_CONTROL>();
         if (warp == 0 && lane == 0) {
             // ===== TMA producer: own A rows, own half of B =====
-            const uint32_t tx = (uint32_t)(Cfg::A_BYTES + hb * BK * 4);
+            const uint32_t tx = (uint32_t)(Cfg::A_BYTES + 2 * hb * BK * 4);
             uint32_t it = 0;
             for (int t = pair; t < p.n_tiles; t += n_pairs) {
                 const int mt = 2 * (t / p.n_tiles_n) + (int)rank, n0 = (t % p.n_tiles_n) * p.bn;
@@ -397,6 +393,7 @@ k_gemm_tc_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                     for (int q = 0; q < 4; ++q)
                         tma_load_2d(a_hi(s) + q * (BK * 128), &tmA, bar_full(s), q * 32, mt * p.K + kb * BK);
                     tma_load_2d(b_hi(s), &tmB, bar_full(s), kb * BK, n0 + (int)rank * hb);
+                    tma_load_2d(b_lo(s), &tmB, bar_full(s), kb * BK, p.N + n0 + (int)rank * hb);  // lo rows follow the hi rows
                 }
             }
         } else if (warp == 1 && lane == 0 && rank == 0) {
@@ -442,7 +439,7 @@ k_gemm_tc_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
         setmaxnreg_dec<TC_REGS_SPLIT>();
         // ===== splitters: own A tile and own half of B, hi in place, lo beside it =====
         const int tid = threadIdx.x - TC_FIRST_SPLIT_WARP * 32;
-        const int n_a4 = Cfg::A_BYTES / 16, n_b4 = hb * BK * 4 / 16;
+        const int n_a4 = Cfg::A_BYTES / 16;
         uint32_t it = 0;
         for (int t = pair; t < p.n_tiles; t += n_pairs) {
             for (int kb = 0; kb < nkb; ++kb, ++it) {
@@ -450,10 +447,7 @@ k_gemm_tc_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                 mbar_wait(bar_full(s), (it / NST) & 1);
                 float4 *ah = reinterpret_cast<float4 *>(smem_gen + (size_t)s * Cfg::STAGE_BYTES);
                 float4 *al = ah + Cfg::A_BYTES / 16;
-                float4 *bh = ah + 2 * Cfg::A_BYTES / 16;
-                float4 *bl = bh + Cfg::B_BYTES / 16;
-                split_hi_lo(ah, al, n_a4, tid);
-                split_hi_lo(bh, bl, n_b4, tid);
+                split_hi_lo(ah, al, n_a4, tid);  // B arrives split (model->Ws / WTs)
                 fence_proxy_async_all();
                 __syncwarp();
                 if (lane == 0) mbar_arrive_cluster(bar_split(s), 0);
@@ -627,7 +621,7 @@ int g_tc_flush_k = 64;   // knob "tc_flush_k": K extent between accumulator flus
 int g_tc_split_bk = 32;  // knob (gmnn_system_set_int "tc_split_bk"): K extent of a 3xTF32 stage, 16 or 32
 
 // C[M][N] = A[M][K] . Bt[N][K]^T.  A, C, C2, Dmul are tile-transposed ([M/128][cols][128], padded to whole
-// tiles); Bt (weights) is row-major [N][K].
+// tiles); Bt (weights) is row-major [N][K], or for split = true the stacked hi / lo split [2N][K].
 int tc_gemm(bool split, int epi, int64_t M, int N, int K, const float *A, const float *Bt, float *C, const float *bias,
             float *C2, const float *Dmul, cudaStream_t st) {
     if (K % 8 != 0 || N % 8 != 0 || M <= 0 || M > INT32_MAX) {
@@ -646,7 +640,7 @@ int tc_gemm(bool split, int epi, int64_t M, int N, int K, const float *A, const 
     CUtensorMap tmA, tmB;
     int rc;
     if ((rc = make_tmap_a(&tmA, A, M, K, BK))) return rc;
-    if ((rc = make_tmap(&tmB, Bt, N, K, a.bn, BK))) return rc;
+    if ((rc = make_tmap(&tmB, Bt, split ? 2 * (int64_t)N : N, K, a.bn, BK))) return rc;
 #define TC_CASE(SP, BKV)                                                                  \
     switch (epi) {                                                                        \
         case EPI_PLAIN: return tc_launch<SP, BKV, EPI_PLAIN>(tmA, tmB, a, st);             \
@@ -656,7 +650,7 @@ int tc_gemm(bool split, int epi, int64_t M, int N, int K, const float *A, const 
     if (split && g_tc_pair) {
         // pair tiles: two adjacent 128-row tiles x one column tile; B box = this CTA's half of the columns
         a.n_tiles = (int)(((M + TC_BM - 1) / TC_BM + 1) / 2) * a.n_tiles_n;
-        if ((rc = make_tmap(&tmB, Bt, N, K, a.bn / 2, BK))) return rc;
+        if ((rc = make_tmap(&tmB, Bt, 2 * (int64_t)N, K, a.bn / 2, BK))) return rc;
         if (BK == 32) {
             switch (epi) {
                 case EPI_PLAIN: return tc_launch_pair<32, EPI_PLAIN>(tmA, tmB, a, st);
@@ -676,13 +670,28 @@ int tc_gemm(bool split, int epi, int64_t M, int N, int K, const float *A, const 
 #undef TC_CASE
 }
 
+__global__ void k_split_stack(const float *__restrict__ src, float *__restrict__ dst, int64_t n) {
+    const int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (t >= n) return;
+    const float v = src[t], h = to_tf32_rna(v);
+    dst[t] = h;
+    dst[n + t] = v - h;
+}
+
+int launch_split_stack(const float *src, float *dst, int64_t n, cudaStream_t st) {
+    k_split_stack<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(src, dst, n);
+    GMNN_LAUNCHED();
+    GMNN_CUDA(cudaGetLastError());
+    return GMNN_OK;
+}
+
 int launch_mlp_forward_tc(gmnn_system *s, cudaStream_t st) {
     const gmnn_model *m = s->model;
     const bool split = s->mlp_precision == GMNN_MLP_3XTF32;
     const float *X = s->G;
     for (int l = 0; l < m->hp.n_hidden; ++l) {
         // z = X W[l]: the B operand is W[l]^T = WT[l], [fan_out][fan_in]
-        int rc = tc_gemm(split, EPI_HIDDEN, s->N, m->dims[l + 1], m->dims[l], X, m->WT[l], s->H[l], m->b[l], s->D[l], nullptr, st);
+        int rc = tc_gemm(split, EPI_HIDDEN, s->N, m->dims[l + 1], m->dims[l], X, split ? m->WTs[l] : m->WT[l], s->H[l], m->b[l], s->D[l], nullptr, st);
         if (rc) return rc;
         X = s->H[l];
     }
@@ -698,14 +707,15 @@ int launch_mlp_backward_tc(gmnn_system *s, const float *head_w_dev, cudaStream_t
     int rc = launch_mlp_seed(s, head_w_dev, st);  // vhead, Bv (and BvT, see mlp_simt.cu)
     if (rc) return rc;
     const float *Aop = s->D[L - 1];
-    const float *BopT = s->BvT;
+    if (split && (rc = launch_split_stack(s->BvT, s->BvTs, (int64_t)m->dims[L] * m->dims[L - 1], st))) return rc;
+    const float *BopT = split ? s->BvTs : s->BvT;
     int cur = 0;
     for (int l = L - 1; l >= 0; --l) {
         if (l > 0) {
             rc = tc_gemm(split, EPI_MUL, s->N, m->dims[l], m->dims[l + 1], Aop, BopT, s->dZ[cur], nullptr, nullptr, s->D[l - 1], st);
             if (rc) return rc;
             Aop = s->dZ[cur];
-            BopT = m->W[l - 1];
+            BopT = split ? m->Ws[l - 1] : m->W[l - 1];
             cur ^= 1;
         } else {
             rc = tc_gemm(split, EPI_PLAIN, s->N, m->dims[0], m->dims[1], Aop, BopT, s->dG, nullptr, nullptr, nullptr, st);
