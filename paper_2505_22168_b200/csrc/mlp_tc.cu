@@ -41,6 +41,9 @@ constexpr int TC_FIRST_SPLIT_WARP = 4;
 constexpr int TC_FIRST_EPI_WARP = 8;
 constexpr int TC_REGS_CONTROL = 40, TC_REGS_SPLIT = 64, TC_REGS_EPI = 200;  // 128 * (40 + 64 + 2 * 200) <= 65536
 constexpr int TC_STAGE_BYTES_TOTAL = 192 * 1024;
+#ifndef TC_EB
+#define TC_EB 16  // columns per batch of the fused epilogue
+#endif
 
 template <bool SPLIT, int BK>
 struct TcCfg {
@@ -109,31 +112,36 @@ __device__ __forceinline__ void tc_store_tile(const TcArgs &p, float (&acc)[4][3
         const int g = 2 * gi + half;
         const int col0 = n0 + g * 32;
         if (g >= n_groups || !row_ok || (p.debug & 4)) continue;
-        // eight columns at a time: loads first, then the arithmetic, then the stores, so that the
-        // eight dependency chains (ex2, rcp, fma) overlap
+        // TC_EB columns at a time: loads first, then the arithmetic, then the stores, so that the
+        // dependency chains (ex2, rcp, fma; DRAM latency of the multiplier) overlap
 #pragma unroll
-        for (int j0 = 0; j0 < 32; j0 += 8) {
-            if (col0 + j0 >= p.N || g * 32 + j0 >= p.bn) continue;  // N and bn are multiples of 8 here
+        for (int j0 = 0; j0 < 32; j0 += TC_EB) {
+            if (col0 + j0 >= p.N || g * 32 + j0 >= p.bn) continue;
+            // N and bn are multiples of 8: the second half of a 16-wide batch may be absent
+            const int nc = (col0 + j0 + TC_EB <= p.N && g * 32 + j0 + TC_EB <= p.bn) ? TC_EB : 8;
             const int64_t o = tbase + (int64_t)(col0 + j0) * TC_BM;
-            float in[8], h[8], d[8];
+            float in[TC_EB], h[TC_EB], d[TC_EB];
             if (EPI == EPI_HIDDEN) {
 #pragma unroll
-                for (int c = 0; c < 8; ++c) in[c] = __ldg(bias + col0 + j0 + c);
+                for (int c = 0; c < TC_EB; ++c) in[c] = c < nc ? __ldg(bias + col0 + j0 + c) : 0.f;
 #pragma unroll
-                for (int c = 0; c < 8; ++c) swish_pair_tc(acc[gi][j0 + c] + in[c], h[c], d[c]);
+                for (int c = 0; c < TC_EB; ++c) swish_pair_tc(acc[gi][j0 + c] + in[c], h[c], d[c]);
 #pragma unroll
-                for (int c = 0; c < 8; ++c) {
-                    Cout[o + c * TC_BM] = h[c];
-                    C2out[o + c * TC_BM] = d[c];
-                }
+                for (int c = 0; c < TC_EB; ++c)
+                    if (c < nc) {
+                        Cout[o + c * TC_BM] = h[c];
+                        C2out[o + c * TC_BM] = d[c];
+                    }
             } else if (EPI == EPI_MUL) {
 #pragma unroll
-                for (int c = 0; c < 8; ++c) in[c] = __ldg(Dmul + o + c * TC_BM);
+                for (int c = 0; c < TC_EB; ++c) in[c] = c < nc ? __ldg(Dmul + o + c * TC_BM) : 0.f;
 #pragma unroll
-                for (int c = 0; c < 8; ++c) Cout[o + c * TC_BM] = acc[gi][j0 + c] * in[c];
+                for (int c = 0; c < TC_EB; ++c)
+                    if (c < nc) Cout[o + c * TC_BM] = acc[gi][j0 + c] * in[c];
             } else {
 #pragma unroll
-                for (int c = 0; c < 8; ++c) Cout[o + c * TC_BM] = acc[gi][j0 + c];
+                for (int c = 0; c < TC_EB; ++c)
+                    if (c < nc) Cout[o + c * TC_BM] = acc[gi][j0 + c];
             }
         }
     }
