@@ -128,3 +128,38 @@ def test_ensemble_heads_with_tc(gm, orc):
     assert energy_atom_error(e_mean, ref.e_mean) <= 1.0
     assert force_error(f_mean, ref.f_mean) <= F_TOL
     assert np.abs(f_var - ref.f_var).max() <= 2e-4 * ref.f_var.max()
+
+
+@pytest.mark.parametrize("name", ["config2", "config3_8192", "ragged"])
+def test_cta_pair_and_single_cta_kernels(gm, orc, name):
+    """The 3xTF32 GEMM runs on CTA pairs (cta_group::2, default) or single CTAs: both meet the fp32
+    tolerances; 'ragged' has an odd number of 128-atom tiles (a pair with an empty second tile)."""
+    w = wl.li3po4_box(1000 + 128 * 2, hidden=(144, 272)) if name == "ragged" else wl.make_workload(name)
+    ref = _ref(orc, w)
+    sysm, pos = _system(gm, w, P3X)
+    out = {}
+    try:
+        for pair in (1, 0):
+            sysm.set_int("tc_pair", pair)
+            e, ea, f = _run(sysm, pos)
+            assert energy_atom_error(ea, ref.e_atom) <= 1.0, pair
+            assert force_error(f, ref.forces) <= F_TOL, pair
+            out[pair] = f
+    finally:
+        sysm.set_int("tc_pair", 1)
+    assert force_error(out[0], out[1]) <= 5e-5
+
+
+def test_contract_backward_block_shapes(gm, orc):
+    """k_contract_backward with one or two 128-atom tiles per block gives the same adjoints (odd tile count)."""
+    w = wl.li3po4_box(128 * 5 + 24, hidden=(32, 32))
+    sysm, pos = _system(gm, w, P3X)
+    res = []
+    try:
+        for halves in (1, 2):
+            sysm.set_int("cb_halves", halves)
+            _run(sysm, pos)
+            res.append(sysm.debug_read("A"))
+    finally:
+        sysm.set_int("cb_halves", 1)
+    assert np.array_equal(res[0], res[1])
