@@ -105,11 +105,13 @@ k_pair_forward(int64_t N, const float4 *__restrict__ pos4, const uint32_t *__res
     const int64_t i = gt / LPA;
     const int sub = (int)(gt % LPA);
     const bool live = i < N;
-    float acc[NR][PSI];
+    // moment sums as float2 pairs (m = 2q, 2q + 1): the accumulation runs on the packed fp32 FMA
+    // (FFMA2: same flop rate as FFMA, half the issue slots, and this kernel is issue-bound)
+    float2 acc[NR][PSI / 2];
 #pragma unroll
     for (int s = 0; s < NR; ++s)
 #pragma unroll
-        for (int m = 0; m < PSI; ++m) acc[s][m] = 0.f;
+        for (int q = 0; q < PSI / 2; ++q) acc[s][q] = make_float2(0.f, 0.f);
 
     if (live) {
         const float4 xi = pos4[i];
@@ -146,9 +148,12 @@ k_pair_forward(int64_t N, const float4 *__restrict__ pos4, const uint32_t *__res
                     float mono[PSI];
                     monomials(pg.dx * rinv, pg.dy * rinv, pg.dz * rinv, mono);
 #pragma unroll
-                    for (int s = 0; s < NR; ++s)
+                    for (int s = 0; s < NR; ++s) {
+                        const float2 R2 = make_float2(R[s], R[s]);
 #pragma unroll
-                        for (int m = 0; m < PSI; ++m) acc[s][m] = fmaf(R[s], mono[m], acc[s][m]);
+                        for (int q = 0; q < PSI / 2; ++q)
+                            acc[s][q] = __ffma2_rn(R2, make_float2(mono[2 * q], mono[2 * q + 1]), acc[s][q]);
+                    }
                 }
             }
         }
@@ -159,14 +164,17 @@ k_pair_forward(int64_t N, const float4 *__restrict__ pos4, const uint32_t *__res
 #pragma unroll
         for (int s = 0; s < NR; ++s)
 #pragma unroll
-            for (int m = 0; m < PSI; ++m) acc[s][m] += __shfl_xor_sync(0xffffffffu, acc[s][m], o);
+            for (int q = 0; q < PSI / 2; ++q) {
+                acc[s][q].x += __shfl_xor_sync(0xffffffffu, acc[s][q].x, o);
+                acc[s][q].y += __shfl_xor_sync(0xffffffffu, acc[s][q].y, o);
+            }
     if (live) {
         float4 *out = reinterpret_cast<float4 *>(psi + i * (int64_t)(NR * PSI));
 #pragma unroll
         for (int q = 0; q < NR * PSI / 4; ++q) {
             if (q % LPA == sub) {
-                const int s = (4 * q) / PSI, m = (4 * q) % PSI;
-                out[q] = make_float4(acc[s][m], acc[s][m + 1], acc[s][m + 2], acc[s][m + 3]);
+                const int s = (4 * q) / PSI, m = ((4 * q) % PSI) / 2;
+                out[q] = make_float4(acc[s][m].x, acc[s][m].y, acc[s][m + 1].x, acc[s][m + 1].y);
             }
         }
     }
