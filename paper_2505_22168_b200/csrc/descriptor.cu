@@ -364,36 +364,36 @@ k_contract_backward(int64_t N, const float *__restrict__ psi, const float *__res
 // ---------------------------------------------------------------------------------------------
 // a10 + a11: pair gradient in both directions and the force sum of the centre atom
 // ---------------------------------------------------------------------------------------------
-// g = dE/dd for one direction.  a(s, q) returns the float4 {A[s][4q..4q+3]}; sgn = +1 evaluates at
-// u, sgn = -1 at -u (odd-rank monomials change sign).
+// g = dE/dd for one direction.  a(s, q) returns the float4 {A[s][4q..4q+3]}; (x, y, z) is the unit
+// vector the centre's polynomial is evaluated at: +u for the centre itself, -u for its neighbour.
 template <int NR, class AGet>
-__device__ __forceinline__ void pair_gradient(AGet a, const float *R, const float *dR, const float *mono, float ux,
-                                              float uy, float uz, float rinv, float sgn, float &gx, float &gy,
-                                              float &gz) {
-    float t[PSI];
+__device__ __forceinline__ void pair_gradient(AGet a, const float *R, const float *dR, const float *mono, float x,
+                                              float y, float z, float rinv, float &gx, float &gy, float &gz) {
+    // mono = monomials of (x, y, z), the direction the polynomial is evaluated at (+u or -u).
+    // Both 100-term sums run on the packed fp32 FMA (FFMA2), two monomials per instruction.
+    float2 t2[PSI / 2];
 #pragma unroll
-    for (int m = 0; m < PSI; ++m) t[m] = 0.f;
+    for (int q = 0; q < PSI / 2; ++q) t2[q] = make_float2(0.f, 0.f);
     float radial = 0.f;
 #pragma unroll
     for (int s = 0; s < NR; ++s) {
-        float pe = 0.f, po = 0.f;  // even (L = 0, 2) and odd (L = 1, 3) parts of p_s(u)
+        float2 p2 = make_float2(0.f, 0.f);  // p_s(u) = sum_m A[s][m] mono_m, in two partial sums
+        const float2 R2 = make_float2(R[s], R[s]);
 #pragma unroll
         for (int q = 0; q < PSI / 4; ++q) {
             const float4 v = a(s, q);
-            const float av[4] = {v.x, v.y, v.z, v.w};
-#pragma unroll
-            for (int c = 0; c < 4; ++c) {
-                const int m = 4 * q + c;
-                const bool odd = (m >= 1 && m <= 3) || m >= 10;
-                if (odd) po = fmaf(av[c], mono[m], po);
-                else pe = fmaf(av[c], mono[m], pe);
-                t[m] = fmaf(R[s], av[c], t[m]);
-            }
+            const float2 a01 = make_float2(v.x, v.y), a23 = make_float2(v.z, v.w);
+            p2 = __ffma2_rn(a01, make_float2(mono[4 * q], mono[4 * q + 1]), p2);
+            p2 = __ffma2_rn(a23, make_float2(mono[4 * q + 2], mono[4 * q + 3]), p2);
+            t2[2 * q] = __ffma2_rn(R2, a01, t2[2 * q]);
+            t2[2 * q + 1] = __ffma2_rn(R2, a23, t2[2 * q + 1]);
         }
-        radial = fmaf(dR[s], pe + sgn * po, radial);
+        radial = fmaf(dR[s], p2.x + p2.y, radial);
     }
-    const float x = sgn * ux, y = sgn * uy, z = sgn * uz;
-    const float xx = mono[4], xy = mono[5], xz = mono[6], yy = mono[7], yz = mono[8], zz = mono[9];  // even: sign free
+    float t[PSI];
+#pragma unroll
+    for (int q = 0; q < PSI / 2; ++q) t[2 * q] = t2[q].x, t[2 * q + 1] = t2[q].y;
+    const float xx = mono[4], xy = mono[5], xz = mono[6], yy = mono[7], yz = mono[8], zz = mono[9];
     // grad_u q(u), q = sum_m t_m mono_m
     float wx = t[1] + 2.f * t[4] * x + t[5] * y + t[6] * z + 3.f * t[10] * xx + 2.f * t[11] * xy + 2.f * t[12] * xz +
                t[13] * yy + t[14] * yz + t[15] * zz;
@@ -496,11 +496,15 @@ k_pair_backward(int64_t N, const float4 *__restrict__ pos4, const uint32_t *__re
                         }
                         if (dir == 0) {
                             pair_gradient<NR>([&](int s, int qq) { return Ai[s * (PSI / 4) + qq]; }, R, dR, mono, ux, uy,
-                                              uz, rinv, 1.f, gxo, gyo, gzo);
+                                              uz, rinv, gxo, gyo, gzo);
                         } else {
                             const float4 *Aj = reinterpret_cast<const float4 *>(A) + (int64_t)pg.j * (NR * PSI / 4);
-                            pair_gradient<NR>([&](int s, int qq) { return __ldg(&Aj[s * (PSI / 4) + qq]); }, R, dR, mono,
-                                              ux, uy, uz, rinv, -1.f, gxr, gyr, gzr);
+                            float mono_r[PSI];  // the neighbour sees the bond reversed
+                            monomials(-ux, -uy, -uz, mono_r);
+                            float hx, hy, hz;  // gradient with respect to (-u): g_ji in the frame of d_ji = -d_ij
+                            pair_gradient<NR>([&](int s, int qq) { return __ldg(&Aj[s * (PSI / 4) + qq]); }, R, dR, mono_r,
+                                              -ux, -uy, -uz, rinv, hx, hy, hz);
+                            gxr = hx, gyr = hy, gzr = hz;
                         }
                     }
                     if (PAIRBUF) *slot = make_float4(gxo, gyo, gzo, 0.f);
