@@ -229,6 +229,23 @@ def run_reference(args):
     return 0
 
 
+def max_over_ranks(x: float, world: int, device) -> float:
+    """The slowest rank's time: replicas are independent, the job is as slow as its slowest member."""
+    if world <= 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(n_atoms: int, steps: int, world: int, ms_max: float) -> float:
+    """atom-steps/s of the whole job: every replica advances n_atoms atoms by `steps` steps."""
+    return world * n_atoms * steps / (ms_max * 1e-3)
+
+
 # ------------------------------------------------------------------------------------------------
 # our arm
 # ------------------------------------------------------------------------------------------------
@@ -294,11 +311,8 @@ def run_ours(args):
     ms = ev0.elapsed_time(ev1)
     stages = sysm.stage_times()
     sysm.set_int("profile", 0)
-    t = torch.tensor([ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_max = float(t.item())
-    value = world * N * args.steps / (ms_max * 1e-3)
+    ms_max = max_over_ranks(ms, world, dev)
+    value = whole_job_value(N, args.steps, world, ms_max)
     etot = (epot + ekin).cpu().numpy()
     drift = float(np.abs(etot - etot[0]).max() / N)
 
@@ -380,10 +394,7 @@ def run_ours(args):
         e_host = sysm.energy_forces_host(hp_np, hf_np)
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
-    t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    e2e = {"value": world * N * e2e_steps / float(t.item()), "unit": UNIT, "h2d_bytes_per_step": 12 * N,
+    e2e = {"value": world * N * e2e_steps / max_over_ranks(e2e_s, world, dev), "unit": UNIT, "h2d_bytes_per_step": 12 * N,
            "d2h_bytes_per_step": 12 * N + 8, "steps": e2e_steps,
            "what": "gmnn_energy_forces_host: pinned positions in, forces and total energy out, every step"}
     sysm.check()
