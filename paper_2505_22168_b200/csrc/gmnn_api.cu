@@ -282,6 +282,7 @@ int gmnn_system_create(const gmnn_model *m, int64_t n_atoms, const int32_t *spec
     A_(s->BvTs, 2 * (size_t)m->dims[L] * m->dims[L - 1]);
     A_(s->vhead, (size_t)m->dims[L]);
     A_(s->head_w, (size_t)M);
+    A_(s->ypart, (size_t)MAX_HEAD_SLOTS * NP);
     A_(s->e_heads, N * M);
     A_(s->e_atom, N);
     A_(s->f_int, 3 * N);
@@ -309,7 +310,7 @@ void gmnn_system_destroy(gmnn_system *s) {
     dev_free(s->nbr); dev_free(s->rev); dev_free(s->gbuf); dev_free(s->runs); dev_free(s->count); dev_free(s->psi); dev_free(s->G); dev_free(s->dG); dev_free(s->A);
     for (int l = 0; l < MAX_LAYERS; ++l) { dev_free(s->H[l]); dev_free(s->D[l]); }
     dev_free(s->dZ[0]); dev_free(s->dZ[1]); dev_free(s->Bv); dev_free(s->BvT); dev_free(s->BvTs); dev_free(s->vhead); dev_free(s->head_w);
-    dev_free(s->e_heads); dev_free(s->e_atom); dev_free(s->f_int); dev_free(s->f_tmp); dev_free(s->partial);
+    dev_free(s->ypart); dev_free(s->e_heads); dev_free(s->e_atom); dev_free(s->f_int); dev_free(s->f_tmp); dev_free(s->partial);
     dev_free(s->e_total); dev_free(s->flags);
     dev_free(s->stage_pos); dev_free(s->stage_f); dev_free(s->stage_e);
     if (s->flags_host) cudaFreeHost(s->flags_host);

@@ -21,6 +21,7 @@ constexpr uint32_t NBR_J_MASK = (1u << NBR_J_BITS) - 1u;
 constexpr int64_t MAX_ATOMS = (int64_t)1 << NBR_J_BITS;
 constexpr int SMALL_BOX_MAX_ATOMS = 16384;
 constexpr int MAX_STAGE_EVENTS = 1 << 16;
+constexpr int MAX_HEAD_SLOTS = 16;  // partial sums per atom of the head fused into the last GEMM epilogue
 constexpr int PSI = 20;  // unique monomials per channel (contraction.cuh NM)
 
 // device-side flag words (int32) in System::flags
@@ -110,6 +111,9 @@ struct gmnn_system {
     float *BvTs = nullptr;           // stacked hi / lo split of BvT
     float *vhead = nullptr;          // [H_last]
     float *head_w = nullptr;         // [n_heads] weights of the differentiated energy
+    float *ypart = nullptr;          // [MAX_HEAD_SLOTS][N padded to 128]: partial head sums (mlp_tc.cu EPI_HIDDEN_HEAD)
+    bool heads_fused = false;        // the last mlp_forward left ypart instead of H[L-1]
+    int head_slots = 0;
     float *e_heads = nullptr;        // [N][n_heads]
     float *e_atom = nullptr;         // [N]
     float *f_int = nullptr;          // [N][3]

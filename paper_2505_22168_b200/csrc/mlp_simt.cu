@@ -189,6 +189,7 @@ __global__ void k_scale_cols(int rows, int cols, const float *__restrict__ W, co
 
 int launch_mlp_forward_simt(gmnn_system *s, cudaStream_t st) {
     const gmnn_model *m = s->model;
+    s->heads_fused = false;
     const float *X = s->G;
     for (int l = 0; l < m->hp.n_hidden; ++l) {
         int rc = sgemm(EPI_HIDDEN, s->N, m->dims[l + 1], m->dims[l], X, m->W[l], s->H[l], m->b[l], s->D[l], nullptr, st);
@@ -198,9 +199,32 @@ int launch_mlp_forward_simt(gmnn_system *s, cudaStream_t st) {
     return GMNN_OK;
 }
 
+// Single head fused into the last GEMM epilogue (mlp_tc.cu): add the partial sums in slot order.
+__global__ void k_heads_finish(int64_t N, const float *__restrict__ ypart, int n_slots, int64_t m_pad,
+                               const float *__restrict__ bl, const float4 *__restrict__ pos4,
+                               const float *__restrict__ scale, const float *__restrict__ shift,
+                               const float *__restrict__ head_w, float *__restrict__ e_heads, float *__restrict__ e_atom) {
+    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    float y = 0.f;
+    for (int q = 0; q < n_slots; ++q) y += __ldg(ypart + q * m_pad + i);
+    const int z = __float_as_int(pos4[i].w);
+    const float em = __ldg(&scale[z]) * (y + __ldg(&bl[0])) + __ldg(&shift[z]);
+    e_heads[i] = em;
+    e_atom[i] = __ldg(&head_w[0]) * em;
+}
+
 int launch_mlp_heads(gmnn_system *s, const float *head_w_dev, cudaStream_t st) {
     const gmnn_model *m = s->model;
     const int L = m->hp.n_hidden;
+    if (s->heads_fused) {
+        k_heads_finish<<<(unsigned)((s->N + 255) / 256), 256, 0, st>>>(s->N, s->ypart, s->head_slots,
+                                                                        (s->N + 127) / 128 * 128, m->b[L], s->pos4, m->scale,
+                                                                        m->shift, head_w_dev, s->e_heads, s->e_atom);
+        GMNN_LAUNCHED();
+        GMNN_CUDA(cudaGetLastError());
+        return GMNN_OK;
+    }
     if (m->dims[L] > 1024) {
         set_error("last hidden width > 1024");
         return GMNN_UNSUPPORTED;

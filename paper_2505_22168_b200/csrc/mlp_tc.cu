@@ -32,7 +32,11 @@ namespace gmnn {
 
 using namespace tc;
 
-enum { EPI_PLAIN = 0, EPI_HIDDEN = 1, EPI_MUL = 2 };
+enum { EPI_PLAIN = 0, EPI_HIDDEN = 1, EPI_MUL = 2, EPI_HIDDEN_HEAD = 3 };
+// EPI_HIDDEN_HEAD: last hidden layer of a single-head model.  h = swish(z) is not stored (the backward
+// needs only swish'); its dot product with the head weights is: every thread writes the partial sum
+// over its columns to ypart[slot][atom], slot = 2 * column tile + column half, and k_heads_finish
+// adds the slots in order.
 
 constexpr int TC_BM = 128;           // rows of A per tile = TMEM lanes
 constexpr int TC_BN_MAX = 256;       // columns per accumulator buffer
@@ -67,6 +71,9 @@ struct TcArgs {
     float *C2;     // EPI_HIDDEN: swish'(z)
     const float *bias;
     const float *Dmul;  // EPI_MUL: [M][N]
+    const float *w_head;  // EPI_HIDDEN_HEAD: [N] weights of the single head
+    float *ypart;         // EPI_HIDDEN_HEAD: [2 * n_tiles_n][m_pad]
+    int64_t m_pad;
 };
 
 __device__ __forceinline__ void swish_pair_tc(float z, float &h, float &d) {
@@ -107,6 +114,7 @@ __device__ __forceinline__ void tc_store_tile(const TcArgs &p, float (&acc)[4][3
     float *__restrict__ C2out = p.C2;
     const float *__restrict__ bias = p.bias;
     const float *__restrict__ Dmul = p.Dmul;
+    float ysum = 0.f;
 #pragma unroll
     for (int gi = 0; gi < 4; ++gi) {
         const int g = 2 * gi + half;
@@ -121,7 +129,22 @@ __device__ __forceinline__ void tc_store_tile(const TcArgs &p, float (&acc)[4][3
             const int nc = (col0 + j0 + TC_EB <= p.N && g * 32 + j0 + TC_EB <= p.bn) ? TC_EB : 8;
             const int64_t o = tbase + (int64_t)(col0 + j0) * TC_BM;
             float in[TC_EB], h[TC_EB], d[TC_EB];
-            if (EPI == EPI_HIDDEN) {
+            if (EPI == EPI_HIDDEN_HEAD) {
+                float wh[TC_EB];
+#pragma unroll
+                for (int c = 0; c < TC_EB; ++c) {
+                    in[c] = c < nc ? __ldg(bias + col0 + j0 + c) : 0.f;
+                    wh[c] = c < nc ? __ldg(p.w_head + col0 + j0 + c) : 0.f;
+                }
+#pragma unroll
+                for (int c = 0; c < TC_EB; ++c) swish_pair_tc(acc[gi][j0 + c] + in[c], h[c], d[c]);
+#pragma unroll
+                for (int c = 0; c < TC_EB; ++c)
+                    if (c < nc) {
+                        ysum = fmaf(h[c], wh[c], ysum);
+                        C2out[o + c * TC_BM] = d[c];
+                    }
+            } else if (EPI == EPI_HIDDEN) {
 #pragma unroll
                 for (int c = 0; c < TC_EB; ++c) in[c] = c < nc ? __ldg(bias + col0 + j0 + c) : 0.f;
 #pragma unroll
@@ -145,6 +168,8 @@ __device__ __forceinline__ void tc_store_tile(const TcArgs &p, float (&acc)[4][3
             }
         }
     }
+    if (EPI == EPI_HIDDEN_HEAD && row_ok && !(p.debug & 4))
+        p.ypart[(int64_t)(2 * (n0 / p.bn) + half) * p.m_pad + m0 + quad * 32 + lane] = ysum;
 }
 
 template <bool SPLIT, int BK, int EPI>
@@ -631,7 +656,8 @@ int g_tc_split_bk = 32;  // knob (gmnn_system_set_int "tc_split_bk"): K extent o
 // C[M][N] = A[M][K] . Bt[N][K]^T.  A, C, C2, Dmul are tile-transposed ([M/128][cols][128], padded to whole
 // tiles); Bt (weights) is row-major [N][K], or for split = true the stacked hi / lo split [2N][K].
 int tc_gemm(bool split, int epi, int64_t M, int N, int K, const float *A, const float *Bt, float *C, const float *bias,
-            float *C2, const float *Dmul, cudaStream_t st) {
+            float *C2, const float *Dmul, cudaStream_t st, const float *w_head = nullptr, float *ypart = nullptr,
+            int *n_slots = nullptr) {
     if (K % 8 != 0 || N % 8 != 0 || M <= 0 || M > INT32_MAX) {
         set_error("tensor-core MLP: widths must be multiples of 8 (K = %d, N = %d)", K, N);
         return GMNN_UNSUPPORTED;
@@ -645,6 +671,8 @@ int tc_gemm(bool split, int epi, int64_t M, int N, int K, const float *A, const 
     a.flush = split ? (g_tc_flush_k / BK > 0 ? g_tc_flush_k / BK : 1) : (K + BK - 1) / BK;  // TF32 mode: one chunk
     a.debug = g_tc_debug;
     a.C = C, a.C2 = C2, a.bias = bias, a.Dmul = Dmul;
+    a.w_head = w_head, a.ypart = ypart, a.m_pad = (M + TC_BM - 1) / TC_BM * TC_BM;
+    if (n_slots) *n_slots = 2 * a.n_tiles_n;
     CUtensorMap tmA, tmB;
     int rc;
     if ((rc = make_tmap_a(&tmA, A, M, K, BK))) return rc;
@@ -653,6 +681,7 @@ int tc_gemm(bool split, int epi, int64_t M, int N, int K, const float *A, const 
     switch (epi) {                                                                        \
         case EPI_PLAIN: return tc_launch<SP, BKV, EPI_PLAIN>(tmA, tmB, a, st);             \
         case EPI_HIDDEN: return tc_launch<SP, BKV, EPI_HIDDEN>(tmA, tmB, a, st);           \
+        case EPI_HIDDEN_HEAD: return tc_launch<SP, BKV, EPI_HIDDEN_HEAD>(tmA, tmB, a, st); \
         default: return tc_launch<SP, BKV, EPI_MUL>(tmA, tmB, a, st);                      \
     }
     if (split && g_tc_pair) {
@@ -663,12 +692,14 @@ int tc_gemm(bool split, int epi, int64_t M, int N, int K, const float *A, const 
             switch (epi) {
                 case EPI_PLAIN: return tc_launch_pair<32, EPI_PLAIN>(tmA, tmB, a, st);
                 case EPI_HIDDEN: return tc_launch_pair<32, EPI_HIDDEN>(tmA, tmB, a, st);
+                case EPI_HIDDEN_HEAD: return tc_launch_pair<32, EPI_HIDDEN_HEAD>(tmA, tmB, a, st);
                 default: return tc_launch_pair<32, EPI_MUL>(tmA, tmB, a, st);
             }
         }
         switch (epi) {
             case EPI_PLAIN: return tc_launch_pair<16, EPI_PLAIN>(tmA, tmB, a, st);
             case EPI_HIDDEN: return tc_launch_pair<16, EPI_HIDDEN>(tmA, tmB, a, st);
+            case EPI_HIDDEN_HEAD: return tc_launch_pair<16, EPI_HIDDEN_HEAD>(tmA, tmB, a, st);
             default: return tc_launch_pair<16, EPI_MUL>(tmA, tmB, a, st);
         }
     }
@@ -699,7 +730,12 @@ int launch_mlp_forward_tc(gmnn_system *s, cudaStream_t st) {
     const float *X = s->G;
     for (int l = 0; l < m->hp.n_hidden; ++l) {
         // z = X W[l]: the B operand is W[l]^T = WT[l], [fan_out][fan_in]
-        int rc = tc_gemm(split, EPI_HIDDEN, s->N, m->dims[l + 1], m->dims[l], X, split ? m->WTs[l] : m->WT[l], s->H[l], m->b[l], s->D[l], nullptr, st);
+        // single head: the last hidden layer's epilogue takes the head's dot product itself
+        const bool fuse = l == m->hp.n_hidden - 1 && m->hp.n_heads == 1 && 2 * ((m->dims[l + 1] + 127) / 128) <= MAX_HEAD_SLOTS;
+        s->heads_fused = fuse;
+        int rc = tc_gemm(split, fuse ? EPI_HIDDEN_HEAD : EPI_HIDDEN, s->N, m->dims[l + 1], m->dims[l], X,
+                         split ? m->WTs[l] : m->WT[l], s->H[l], m->b[l], s->D[l], nullptr, st, m->W[l + 1], s->ypart,
+                         &s->head_slots);
         if (rc) return rc;
         X = s->H[l];
     }
