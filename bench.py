@@ -369,12 +369,12 @@ def run_ours(args):
                              "avg_launch_ms": round((t_f + t_b) / n_launch, 4),
                              "share_of_step": round((per_step_ms["mlp_forward"] + per_step_ms["mlp_backward"])
                                                     / (ms_max / args.steps), 4),
-                             "algorithmic_per_atom": {"bytes": 4.0 * (2 * N_FEATURES + 9 * w.model.hidden[0]),
+                             "algorithmic_per_atom": {"bytes": 4.0 * (2 * N_FEATURES + (8 if w.model.n_heads == 1 else 9) * w.model.hidden[0]),
                                                       "flops": 2.0 * info["flops"]}})
             if args.workload == "config5" and args.mlp == "3xtf32":
                 # dram__bytes_read.sum + dram__bytes_write.sum of the four launches of one step, per launch
                 # (profiles/ncu_r1_gemm_tc_pair.md)
-                roofline["traffic"] = round(22.35e9 / n_launch)
+                roofline["traffic"] = round(20.44e9 / n_launch)
         if info["bound"] == "tensor" and args.mlp == "3xtf32":
             roofline["note"] = ("achieved counts the ALGORITHMIC flops (one product per multiply-add); the 3xTF32 split "
                                 "executes 3 tensor-core MMAs per product, so tensor-pipe flops are 3x achieved")

@@ -5,7 +5,9 @@
 //       nearest), a_lo = a - a_hi (exact in fp32); a.b ~= a_lo.b_hi + a_hi.b_lo + a_hi.b_hi, three
 //       kind::tf32 MMAs into one fp32 accumulator in tensor memory.  Dropped: a_lo.b_lo (<= 2^-22 |ab|)
 //       and the bits of a_lo, b_lo below tf32 (<= 2^-22 |ab|): the same order as fp32 round-off.
-//   mlp_precision = GMNN_MLP_TF32   : one kind::tf32 MMA per product (north_star's 2e-3 variant).
+//   mlp_precision = GMNN_MLP_TF32   : one kind::tf32 MMA per product.  Measured 1e-2 .. 2.5e-2 on the
+//       force measure (rounding the operands to nearest instead of the tensor core's truncation does
+//       not change that): not north_star's 2e-3 variant, kept as an unclaimed fast mode.
 //
 // The tensor core adds into its fp32 accumulator with truncation (measured: a 512-long chain of
 // accumulating MMAs is biased towards zero by ~1e-5 relative), so the fp32-accurate mode keeps the
@@ -13,16 +15,23 @@
 // REGISTER accumulators of the epilogue warps (round-to-nearest adds), and inside a stage the small
 // cross terms are issued before the hi.hi terms so that they meet a small accumulator.
 //
-// One persistent, warp-specialised GEMM kernel  C[M][N] = A[M][K] . Bt[N][K]^T  with fused epilogues:
-//   warp 0        TMA producer: A (128 x BK) and Bt (bn x BK) boxes, swizzled, into an NST-stage ring
-//   warp 1        allocates tensor memory; one lane issues tcgen05.mma (128 x bn x 8 per instruction)
-//   warps 4-7     (3xTF32 only) split each landed stage in place into hi and lo tiles
+// One persistent, warp-specialised GEMM kernel  C[M][N] = A[M][K] . Bt[N][K]^T  with fused epilogues,
+// on single CTAs (k_gemm_tc, 128 x bn tiles) or on CTA pairs (k_gemm_tc_pair, cta_group::2,
+// 256 x bn tiles, each CTA holding half of the B rows):
+//   warp 0        TMA producer into an NST-stage ring.  A: the tile-transposed activations
+//                 ([M/128][K][128], every MLP matrix has this layout) as the MN-major operand, four
+//                 {32 atoms, BK} boxes, 128-byte swizzle with 32-byte atoms (the only swizzle tcgen05
+//                 accepts for an MN-major 32-bit operand).  B: weights, K-major; in 3xTF32 mode the hi
+//                 and lo parts were split once at model creation (model->Ws / WTs, stacked [2N][K])
+//                 and both are loaded
+//   warp 1        allocates tensor memory; one lane issues tcgen05.mma (128 or 256 x bn x 8 each)
+//   warps 4-7     (3xTF32) split the landed A tile: hi = tf32(a) in place, lo = a - hi beside it
 //   warps 8-15    epilogue: drain each K chunk from tensor memory (two 256-column buffers in
 //                 ping-pong, so draining chunk c overlaps the MMAs of chunk c+1) into 128 register
 //                 accumulators per thread; after the last chunk bias + swish + swish' / gradient
-//                 mask and the stores.  setmaxnreg moves registers from the other warps to these.
-// Operands stay fp32 in HBM (activations are written once, read once); the split happens on chip so
-// the L2 -> SM traffic is 4 B per operand element.
+//                 mask / head dot product, and coalesced stores into the tile-transposed output.
+//                 setmaxnreg moves registers from the other warps to these.
+// Activations stay fp32 in HBM, written once and read once (ncu: DRAM bytes = algorithmic bytes).
 #include <cuda.h>
 
 #include "gmnn_internal.h"
