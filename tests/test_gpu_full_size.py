@@ -1,0 +1,111 @@
+"""Parity at BASELINE.json's full sizes (config 3 at 65 536 and 131 072 atoms, config 5 at 1 048 576),
+in the launch configuration bench.py times (3xTF32 MLP on CTA pairs, pair-buffer forces, the
+config's skin).  The oracle cannot evaluate a million atoms in test time, but E_i and F_i of ONE atom
+depend only on the atoms within 2 r_cut of it: for a seeded sample of atoms the oracle evaluates that
+neighbourhood as a free cluster (fp64 differences of the fp32 positions, minimum image applied), and
+its central atom's energy and force are compared one by one.  Plus properties that hold at any size."""
+import numpy as np
+import pytest
+
+import workloads as wl
+from parity_utils import E_ATOM_RTOL, F_TOL
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def gm():
+    import torch
+
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device (they must not pass on a fallback)")
+    import paper_2505_22168_b200 as pkg
+
+    return pkg
+
+
+def _cluster_reference(orc, model, w, i, margin=1e-3):
+    """(E_i, F_i) of atom i from the oracle on the free cluster of all atoms within 2 r_cut of it."""
+    L = w.cell.astype(np.float64)
+    x = w.positions.astype(np.float64)
+    d = x - x[i]
+    d -= L * np.round(d / L)  # minimum image: the boxes here are far larger than 4 r_cut
+    keep = np.where((d * d).sum(1) < (2.0 * w.model.r_cut + margin) ** 2)[0]
+    centre = int(np.where(keep == i)[0][0])
+    pos = d[keep] + 2.5 * w.model.r_cut  # exact fp64 differences, shifted into a positive box
+    box = np.full(3, 5.0 * w.model.r_cut)
+    pairs = orc.neighbors(pos, box, (0, 0, 0), w.model.r_cut)
+    res = orc.energy_forces(model, pos, w.species[keep], box, pairs)
+    return res.e_atom[centre], res.forces[centre], len(keep)
+
+
+@pytest.mark.parametrize("name,n_samples", [("config3_65536", 24), ("config3_131072", 24), ("config5", 32)])
+def test_full_size_sampled_atoms(gm, orc, name, n_samples):
+    import torch
+
+    w = wl.make_workload(name)
+    model = gm.Model(w.model, mlp_precision=gm.GMNN_MLP_3XTF32, force_mode=gm.GMNN_FORCE_PAIRBUF)
+    sysm = gm.System(model, w.species)
+    pos = torch.from_numpy(w.positions).cuda()
+    sysm.build_neighbors(pos, w.cell9, w.pbc, w.model.r_cut, w.skin)
+    e, ea, f = sysm.energy_forces(pos)
+    sysm.check()
+    ea = ea.cpu().numpy().astype(np.float64)
+    f = f.cpu().numpy().astype(np.float64)
+    e = float(e.cpu()[0])
+    N = w.n_atoms
+
+    # properties that hold at any size
+    assert np.isfinite(ea).all() and np.isfinite(f).all()
+    assert abs(e - ea.sum()) <= 1e-6 * np.abs(ea).sum()               # fp64 fixed-order sum of the fp32 E_i
+    rms = np.sqrt((f ** 2).mean())
+    assert np.abs(f.sum(0)).max() <= 1e-4 * rms * np.sqrt(N)           # sum of forces = 0 up to round-off
+    counts = sysm.debug_read("count")
+    r_list = w.model.r_cut + w.skin
+    expect = N / float(np.prod(w.cell.astype(np.float64))) * 4.0 / 3.0 * np.pi * r_list ** 3
+    assert abs(counts.mean() - expect) <= 0.15 * expect                # list density (a jittered lattice has shells)
+    e2, ea2, f2 = sysm.energy_forces(pos)
+    assert np.array_equal(f2.cpu().numpy(), f.astype(np.float32))      # bit-reproducible at full size
+
+    # sampled atoms against the oracle, one by one
+    omodel = orc.Model(w.model)
+    from workloads.inputs import splitmix64
+
+    idx = (splitmix64(20250522 + N, n_samples) % np.uint64(N)).astype(np.int64)
+    e_scale = np.abs(ea).mean()
+    worst_e = worst_f = 0.0
+    for i in idx:
+        e_ref, f_ref, n_cluster = _cluster_reference(orc, omodel, w, int(i))
+        assert 500 < n_cluster < 1200
+        worst_e = max(worst_e, abs(ea[i] - e_ref) / (E_ATOM_RTOL * max(abs(e_ref), e_scale)))
+        worst_f = max(worst_f, np.abs(f[i] - f_ref).max() / rms)
+    print("%s: %d sampled atoms, worst energy error %.3f x 1e-5, worst force error %.2e of rms" % (
+        name, n_samples, worst_e, worst_f))
+    assert worst_e <= 1.0
+    assert worst_f <= F_TOL
+
+
+def test_config5_md_steps_conserve_energy(gm):
+    """Config 5 at full size through gmnn_md_verlet_steps in bench.py's configuration: the total
+    energy of the NVE run stays put (a property that holds at any size; the trajectory itself is
+    checked against the oracle at 1 536 and 8 192 atoms in test_gpu_ensemble_md.py)."""
+    import torch
+
+    w = wl.make_workload("config5")
+    model = gm.Model(w.model, mlp_precision=gm.GMNN_MLP_3XTF32, force_mode=gm.GMNN_FORCE_PAIRBUF)
+    sysm = gm.System(model, w.species)
+    pos = torch.from_numpy(w.positions).cuda()
+    vel = torch.from_numpy(w.velocities).cuda()
+    mass = torch.from_numpy(w.masses).cuda()
+    sysm.build_neighbors(pos, w.cell9, w.pbc, w.model.r_cut, w.skin)
+    epot, ekin, nreb = sysm.md_verlet_steps(pos, vel, mass, w.dt_fs, 12)
+    etot = (epot + ekin).cpu().numpy()
+    ek = ekin.cpu().numpy()
+    assert np.isfinite(etot).all() and nreb >= 0
+    # 300 K: E_kin = 3/2 N k_B T = 0.0388 eV per atom; the drift over 12 steps stays below 0.1 % of it
+    assert abs(ek[0] / w.n_atoms - 1.5 * wl.KB_EV * 300.0) <= 0.02 * 1.5 * wl.KB_EV * 300.0
+    assert np.abs(etot - etot[0]).max() / w.n_atoms <= 1e-3 * 1.5 * wl.KB_EV * 300.0
+    # momentum stays zero (forces sum to zero): centre-of-mass velocity below 1e-6 of the thermal one
+    p = (vel * mass[:, None]).sum(0).cpu().numpy()
+    v_th = np.sqrt(wl.KB_EV * 300.0 / np.mean(w.masses) * 9.648533212e-3)
+    assert np.abs(p).max() / w.masses.sum() <= 1e-5 * v_th
