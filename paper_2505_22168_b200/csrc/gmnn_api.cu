@@ -418,6 +418,7 @@ int gmnn_build_neighbors(gmnn_system *s, const float *positions, const float cel
     Geometry &g = s->geo;
     const float r_list = r_cut + skin;  // fl32(fl32(r_cut) + fl32(skin)): the oracle is handed the same float
     g.r_list2 = r_list * r_list;
+    g.r_cut2 = r_cut * r_cut;
     bool small = false;
     for (int a = 0; a < 3; ++a) {
         g.L[a] = cell[4 * a];
@@ -488,7 +489,7 @@ int gmnn_build_neighbors(gmnn_system *s, const float *positions, const float cel
         if (s->force_mode == GMNN_FORCE_PAIRBUF && !s->rev) {
             int rc = dev_alloc(&s->rev, (size_t)s->N * s->cap);
             if (!rc) rc = dev_alloc(&s->gbuf, (size_t)s->N * s->cap);
-            if (!rc && !s->runs) rc = dev_alloc(&s->runs, (size_t)s->N * 28);
+            if (!rc && !s->runs) rc = dev_alloc(&s->runs, (size_t)s->N * 56);
             if (rc) {
                 set_error("out of device memory for the pair buffer (%lld x %d)", (long long)s->N, s->cap);
                 return rc;

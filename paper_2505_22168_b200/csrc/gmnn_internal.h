@@ -48,6 +48,7 @@ struct Geometry {  // passed by value to kernels
     float inv_edge[3];
     int kimg[3];  // image range of the small-box path
     float r_list2;
+    float r_cut2;  // rows are built inside-r_cut first, skin shell last (neighbor.cu)
 };
 
 struct RadialParams {  // passed by value to the pair kernels
@@ -97,7 +98,7 @@ struct gmnn_system {
     uint32_t *nbr = nullptr;         // [N][cap]
     int32_t *count = nullptr;        // [N]
     uint16_t *rev = nullptr;         // [N][cap] slot of the reverse pair (GMNN_FORCE_PAIRBUF)
-    uint16_t *runs = nullptr;        // [N][28] first slot of each of the 27 cell runs of a row, and its length
+    uint16_t *runs = nullptr;        // [N][56] first slot of each of the 2 x 27 cell runs of a row, and its length
     float4 *gbuf = nullptr;          // [N][cap] g_ij, stored in the row of j at the reverse slot
     bool list_has_rev = false;
     int cap = 0;

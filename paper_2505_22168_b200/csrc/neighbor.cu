@@ -147,12 +147,16 @@ __global__ void k_gather(int64_t N, const float *__restrict__ x, const int32_t *
     }
 }
 
-__device__ __forceinline__ bool in_list(const float4 &xi, const float4 &xj, float sx, float sy, float sz, float rl2) {
+// squared distance in the unfused fp32 arithmetic that defines list membership (reading R20); exactly
+// symmetric under i <-> j with the opposite image
+__device__ __forceinline__ float list_r2(const float4 &xi, const float4 &xj, float sx, float sy, float sz) {
     float dx = __fadd_rn(__fsub_rn(xj.x, xi.x), sx);
     float dy = __fadd_rn(__fsub_rn(xj.y, xi.y), sy);
     float dz = __fadd_rn(__fsub_rn(xj.z, xi.z), sz);
-    float r2 = __fadd_rn(__fadd_rn(__fmul_rn(dx, dx), __fmul_rn(dy, dy)), __fmul_rn(dz, dz));
-    return r2 < rl2;
+    return __fadd_rn(__fadd_rn(__fmul_rn(dx, dx), __fmul_rn(dy, dy)), __fmul_rn(dz, dz));
+}
+__device__ __forceinline__ bool in_list(const float4 &xi, const float4 &xj, float sx, float sy, float sz, float rl2) {
+    return list_r2(xi, xj, sx, sy, sz) < rl2;
 }
 
 __device__ __forceinline__ uint32_t image_code(int nx, int ny, int nz) {
@@ -160,7 +164,7 @@ __device__ __forceinline__ uint32_t image_code(int nx, int ny, int nz) {
            ((uint32_t)(nz + 4) << (NBR_J_BITS + 6));
 }
 
-constexpr int RUNS_PITCH = 28;  // 27 run starts + the row length
+constexpr int RUNS_PITCH = 56;  // 2 parts x 27 run starts, the row length at [54]
 
 // One warp per centre atom; lanes test 32 candidates of a neighbouring cell at a time and append
 // the hits in candidate order (ballot + prefix popcount): the list order is deterministic.
@@ -180,11 +184,17 @@ k_build_cells(int64_t N, const float4 *__restrict__ pos4, const int32_t *__restr
         const int cz = cell_coord(xi.z, g.inv_edge[2], g.ncell[2]);
         uint32_t *row = nbr + i * (int64_t)cap;
         int n = 0;
-        // 27 cells in the fixed order idx = (oz+1)*9 + (oy+1)*3 + (ox+1); runs[idx] = first slot of the
-        // cell's run in this row (entries of a run ascend in atom index).  The reverse-pair index uses
-        // the runs: the partner of an entry in run idx sits in run 26 - idx of the partner's row.
-        for (int idx = 0; idx < 27; ++idx) {
-            if (runs && lane == 0) runs[i * RUNS_PITCH + idx] = (uint16_t)(n < cap ? n : cap);
+        // Two parts: first the pairs inside r_cut at build time, then the skin shell.  The pair kernels
+        // walk a row front to back, so the lanes of a warp reach the (mostly skipped) shell entries
+        // together instead of diverging entry by entry.  Inside a part, 27 cells in the fixed order
+        // idx = (oz+1)*9 + (oy+1)*3 + (ox+1); runs[part*27 + idx] = first slot of the cell's run
+        // (entries of a run ascend in atom index).  The reverse-pair index uses the runs: the partner
+        // of an entry in run (part, idx) sits in run (part, 26 - idx) of the partner's row (r2 is
+        // bitwise symmetric, so both directions fall in the same part).
+        for (int pi = 0; pi < 54; ++pi) {
+            const int part = pi / 27, idx = pi % 27;
+            if (runs && lane == 0) runs[i * RUNS_PITCH + pi] = (uint16_t)(n < cap ? n : cap);
+            if (part == 1 && !(g.r_cut2 < g.r_list2)) continue;  // no skin: the shell is empty
             const int oz = idx / 9 - 1, oy = (idx / 3) % 3 - 1, ox = idx % 3 - 1;
             int z = cz + oz, nz = 0;
             if (z < 0) { if (!g.pbc[2]) continue; z += g.ncell[2]; nz = -1; }
@@ -204,14 +214,17 @@ k_build_cells(int64_t N, const float4 *__restrict__ pos4, const int32_t *__restr
             for (int base = b; base < e; base += 32) {
                 const int j = base + lane;
                 bool keep = false;
-                if (j < e && !(home && j == (int)i)) keep = in_list(xi, pos4[j], sx, sy, sz, g.r_list2);
+                if (j < e && !(home && j == (int)i)) {
+                    const float r2 = list_r2(xi, pos4[j], sx, sy, sz);
+                    keep = r2 < g.r_list2 && (r2 < g.r_cut2) == (part == 0);
+                }
                 const unsigned m = __ballot_sync(0xffffffffu, keep);
                 const int p = n + __popc(m & ((1u << lane) - 1u));
                 if (keep && p < cap) row[p] = (uint32_t)j | code;
                 n += __popc(m);
             }
         }
-        if (runs && lane == 0) runs[i * RUNS_PITCH + 27] = (uint16_t)(n < cap ? n : cap);
+        if (runs && lane == 0) runs[i * RUNS_PITCH + 54] = (uint16_t)(n < cap ? n : cap);
         if (lane == 0) {
             count[i] = n < cap ? n : cap;
             if (n > cap) atomicMax(&flags[FLAG_MAXCOUNT], n);
@@ -318,12 +331,15 @@ k_build_rev_runs(int64_t N, const uint32_t *__restrict__ nbr, const int32_t *__r
     for (int64_t i = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5; i < N; i += n_warps) {
         const int cnt = count[i];
         const uint32_t *row = nbr + i * (int64_t)cap;
-        const int my_run_start = lane < RUNS_PITCH ? (int)runs[i * RUNS_PITCH + lane] : 0x7fffffff;
+        const int run_lo = (int)runs[i * RUNS_PITCH + lane];  // starts of runs 0..31
+        const int run_hi = lane + 32 < 54 ? (int)runs[i * RUNS_PITCH + 32 + lane] : 0x7fffffff;  // runs 32..53
         for (int k0 = 0; k0 < cnt; k0 += 32) {
             const int k = k0 + lane;
             int r = -1;  // run of slot k: number of run starts <= k, minus one
     #pragma unroll
-            for (int q = 0; q < 27; ++q) r += __shfl_sync(0xffffffffu, my_run_start, q) <= k ? 1 : 0;
+            for (int q = 0; q < 32; ++q) r += __shfl_sync(0xffffffffu, run_lo, q) <= k ? 1 : 0;
+#pragma unroll
+            for (int q = 0; q < 22; ++q) r += __shfl_sync(0xffffffffu, run_hi, q) <= k ? 1 : 0;
             if (k < cnt) {
                 const uint32_t e = row[k];
                 const int64_t j = e & NBR_J_MASK;
@@ -331,7 +347,8 @@ k_build_rev_runs(int64_t N, const uint32_t *__restrict__ nbr, const int32_t *__r
                 const uint32_t inv = (8u - (img & 7u)) | ((8u - ((img >> 3) & 7u)) << 3) | ((8u - ((img >> 6) & 7u)) << 6);
                 const uint32_t target = (uint32_t)i | (inv << NBR_J_BITS);
                 const uint32_t *rj = nbr + j * (int64_t)cap;
-                const int s0 = runs[j * RUNS_PITCH + (26 - r)], s1 = runs[j * RUNS_PITCH + (27 - r)];
+                const int rr = (r / 27) * 27 + 26 - r % 27;  // same part, mirrored cell
+                const int s0 = runs[j * RUNS_PITCH + rr], s1 = runs[j * RUNS_PITCH + rr + 1];
                 int found = 0xFFFF;
                 for (int t = s0; t < s1; ++t)
                     if (rj[t] == target) {
