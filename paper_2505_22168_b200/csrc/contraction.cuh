@@ -188,8 +188,14 @@ GMNN_HD void contract_forward(PGet P, Emit emit) {
 }
 
 // P(s, m) -> float;  g(f) -> float (dE/dG_f);  acc(s, m, value): A[s][m] += value.
-template <int NR, int BLOCKS = 0xFF, class PGet, class GGet, class Acc>
-GMNN_HD void contract_backward(PGet P, GGet g, Acc acc) {
+struct NoStep {
+    GMNN_HD void operator()() const {}
+};
+
+// step(): called after every channel-pair iteration of the straight-line body (a kernel can put a block
+// barrier there to keep its warps inside the same stretch of code).
+template <int NR, int BLOCKS = 0xFF, class PGet, class GGet, class Acc, class Step = NoStep>
+GMNN_HD void contract_backward(PGet P, GGet g, Acc acc, Step step = Step()) {
     using F = Feat<NR>;
     if constexpr ((BLOCKS & 0xF) != 0) {
 #pragma unroll
@@ -198,6 +204,7 @@ GMNN_HD void contract_backward(PGet P, GGet g, Acc acc) {
     for (int s1 = 0; s1 < NR; ++s1) {
 #pragma unroll
         for (int s2 = s1; s2 < NR; ++s2) {
+            step();
             const float g1 = g(F::OFF1 + F::pidx(s1, s2));
             const float g2 = g(F::OFF2 + F::pidx(s1, s2));
             const float g3 = g(F::OFF3 + F::pidx(s1, s2));
@@ -225,6 +232,7 @@ GMNN_HD void contract_backward(PGet P, GGet g, Acc acc) {
     for (int s1 = 0; s1 < NR; ++s1) {
 #pragma unroll
         for (int s2 = s1; s2 < NR; ++s2) {
+            step();
             float S[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
 #pragma unroll
             for (int a = 0; a < 3; ++a)
@@ -268,6 +276,7 @@ GMNN_HD void contract_backward(PGet P, GGet g, Acc acc) {
     for (int s1 = 0; s1 < NR; ++s1) {
 #pragma unroll
         for (int s2 = s1; s2 < NR; ++s2) {
+            step();
             float O[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
 #pragma unroll
             for (int a = 0; a < 3; ++a)
@@ -303,6 +312,7 @@ GMNN_HD void contract_backward(PGet P, GGet g, Acc acc) {
     for (int s1 = 0; s1 < NR; ++s1) {
 #pragma unroll
         for (int s2 = s1; s2 < NR; ++s2) {
+            step();
             float S[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
 #pragma unroll
             for (int c = 0; c < 3; ++c)
@@ -344,6 +354,7 @@ GMNN_HD void contract_backward(PGet P, GGet g, Acc acc) {
     for (int s2 = 0; s2 < NR; ++s2) {
 #pragma unroll
         for (int s3 = 0; s3 < NR; ++s3) {
+            step();
             float T[3] = {0.f, 0.f, 0.f};
 #pragma unroll
             for (int a = 0; a < 3; ++a)

@@ -259,7 +259,7 @@ struct CbSmem {  // shared-memory plan of k_contract_backward, in floats
 // HALVES = 2: one 256-thread block per SM works on two tiles in lock step (the block-wide barriers
 // between chunks keep all eight warps inside the same stretch of the ~12 k-instruction straight-line
 // body, so they share its instruction-cache lines); HALVES = 1: two independent 128-thread blocks per SM.
-template <int NR, int HALVES>
+template <int NR, int HALVES, bool LOCKSTEP>
 __global__ void __launch_bounds__(128 * HALVES, 3 - HALVES)
 k_contract_backward(int64_t N, const float *__restrict__ psi, const float *__restrict__ dGt,
                     const float4 *__restrict__ pos4, const float *__restrict__ scale, float *__restrict__ A) {
@@ -319,7 +319,10 @@ k_contract_backward(int64_t N, const float *__restrict__ psi, const float *__res
         contract_backward<NR, CH::mask(C)>(
             [&](int s, int m) { return P[s][m]; },
             [&](int f) { return buf[(f - CH::begin(C)) * TB + tid]; },
-            [&](int s, int m, float v) { acc[s][m] += v; });
+            [&](int s, int m, float v) { acc[s][m] += v; },
+            [&]() {  // keep the warps of the block in the same stretch of the instruction stream
+                if (LOCKSTEP) __syncthreads();
+            });
     };
     if (active) tc::mbar_wait(barY, 0);
     run_chunk(std::integral_constant<int, 0>{}, sY);
@@ -662,25 +665,30 @@ int launch_contract_forward(gmnn_system *s, cudaStream_t st) {
     return GMNN_OK;
 }
 
-int g_cb_halves = 1;  // knob "cb_halves": tiles per block of k_contract_backward (1 or 2)
+int g_cb_halves = 2;  // knob "cb_halves": 1 = one tile per block; 2 = two tiles, lock step (default); 3 = one tile, lock step
 
 int launch_contract_backward(gmnn_system *s, cudaStream_t st) {
     constexpr int NR = 5;
     static bool attr_set = false;
     if (!attr_set) {
-        GMNN_CUDA(cudaFuncSetAttribute(k_contract_backward<NR, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        GMNN_CUDA(cudaFuncSetAttribute(k_contract_backward<NR, 1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                        (int)CbSmem<NR>::bytes(1)));
-        GMNN_CUDA(cudaFuncSetAttribute(k_contract_backward<NR, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        GMNN_CUDA(cudaFuncSetAttribute(k_contract_backward<NR, 1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                       (int)CbSmem<NR>::bytes(1)));
+        GMNN_CUDA(cudaFuncSetAttribute(k_contract_backward<NR, 2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                        (int)CbSmem<NR>::bytes(2)));
         attr_set = true;
     }
     const unsigned tiles = nblocks(s->N, 128);
     if (g_cb_halves == 2)
-        k_contract_backward<NR, 2><<<(tiles + 1) / 2, 256, CbSmem<NR>::bytes(2), st>>>(s->N, s->psi, s->dG, s->pos4,
-                                                                                        s->model->scale, s->A);
+        k_contract_backward<NR, 2, true><<<(tiles + 1) / 2, 256, CbSmem<NR>::bytes(2), st>>>(s->N, s->psi, s->dG, s->pos4,
+                                                                                              s->model->scale, s->A);
+    else if (g_cb_halves == 3)
+        k_contract_backward<NR, 1, true><<<tiles, 128, CbSmem<NR>::bytes(1), st>>>(s->N, s->psi, s->dG, s->pos4,
+                                                                                    s->model->scale, s->A);
     else
-        k_contract_backward<NR, 1><<<tiles, 128, CbSmem<NR>::bytes(1), st>>>(s->N, s->psi, s->dG, s->pos4,
-                                                                              s->model->scale, s->A);
+        k_contract_backward<NR, 1, false><<<tiles, 128, CbSmem<NR>::bytes(1), st>>>(s->N, s->psi, s->dG, s->pos4,
+                                                                                     s->model->scale, s->A);
     GMNN_LAUNCHED();
     GMNN_CUDA(cudaGetLastError());
     return GMNN_OK;

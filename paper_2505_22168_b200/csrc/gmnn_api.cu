@@ -348,7 +348,7 @@ int gmnn_system_set_int(gmnn_system *s, const char *key, int64_t v) {
         if (v != 16 && v != 32) return GMNN_INVALID_ARG;
         gmnn::g_tc_split_bk = (int)v;
     } else if (!strcmp(key, "cb_halves")) {  // process-wide: tiles per block of k_contract_backward
-        if (v != 1 && v != 2) return GMNN_INVALID_ARG;
+        if (v < 1 || v > 3) return GMNN_INVALID_ARG;  // 1: 128 threads; 2: 256 threads in lock step; 3: 128, lock step
         gmnn::g_cb_halves = (int)v;
     } else if (!strcmp(key, "tc_pair")) {  // process-wide: 3xTF32 GEMMs on CTA pairs (1) or single CTAs (0)
         gmnn::g_tc_pair = v != 0;

@@ -151,15 +151,16 @@ def test_cta_pair_and_single_cta_kernels(gm, orc, name):
 
 
 def test_contract_backward_block_shapes(gm, orc):
-    """k_contract_backward with one or two 128-atom tiles per block gives the same adjoints (odd tile count)."""
+    """k_contract_backward with one or two 128-atom tiles per block, with and without the lock-step
+    barriers, gives the same adjoints (odd tile count)."""
     w = wl.li3po4_box(128 * 5 + 24, hidden=(32, 32))
     sysm, pos = _system(gm, w, P3X)
     res = []
     try:
-        for halves in (1, 2):
+        for halves in (1, 2, 3):
             sysm.set_int("cb_halves", halves)
             _run(sysm, pos)
             res.append(sysm.debug_read("A"))
     finally:
-        sysm.set_int("cb_halves", 1)
-    assert np.array_equal(res[0], res[1])
+        sysm.set_int("cb_halves", 2)
+    assert np.array_equal(res[0], res[1]) and np.array_equal(res[0], res[2])
