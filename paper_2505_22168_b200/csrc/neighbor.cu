@@ -166,14 +166,28 @@ __device__ __forceinline__ uint32_t image_code(int nx, int ny, int nz) {
 
 constexpr int RUNS_PITCH = 56;  // 2 parts x 27 run starts, the row length at [54]
 
+constexpr int SHELL_BUF = 256;  // skin-shell entries of one row staged in shared memory during the scan
+
 // One warp per centre atom; lanes test 32 candidates of a neighbouring cell at a time and append
 // the hits in candidate order (ballot + prefix popcount): the list order is deterministic.
+// A row has two parts: first the pairs inside r_cut at build time, then the skin shell.  The pair
+// kernels walk a row front to back, so the lanes of a warp reach the (mostly skipped) shell entries
+// together instead of diverging entry by entry.  Inside a part, 27 cells in the fixed order
+// idx = (oz+1)*9 + (oy+1)*3 + (ox+1); runs[part*27 + idx] = first slot of the cell's run (entries of
+// a run ascend in atom index).  The reverse-pair index uses the runs: the partner of an entry in run
+// (part, idx) sits in run (part, 26 - idx) of the partner's row (r2 is bitwise symmetric, so both
+// directions fall in the same part).  One scan: inside entries go straight to the row, shell entries
+// wait in shared memory until the inside count is known (rows with more than SHELL_BUF shell entries
+// scan a second time).
 __global__ void __launch_bounds__(256)
 k_build_cells(int64_t N, const float4 *__restrict__ pos4, const int32_t *__restrict__ cell_start, Geometry g,
               uint32_t *nbr, int32_t *count, int cap, int32_t *flags, const int32_t *cond, float thr2,
               uint16_t *runs) {
     if (skip_rebuild(cond, thr2)) return;
-    const int lane = threadIdx.x & 31;
+    __shared__ uint32_t s_shell[8][SHELL_BUF];
+    __shared__ int s_rel[8][28];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const unsigned below = (1u << lane) - 1u;
     // grid-stride over atoms (one warp each): the launch is a few waves of blocks, so that the
     // every-step launches that skip_rebuild() turns into no-ops stay cheap
     const int64_t n_warps = (gridDim.x * (int64_t)blockDim.x) >> 5;
@@ -183,28 +197,18 @@ k_build_cells(int64_t N, const float4 *__restrict__ pos4, const int32_t *__restr
         const int cy = cell_coord(xi.y, g.inv_edge[1], g.ncell[1]);
         const int cz = cell_coord(xi.z, g.inv_edge[2], g.ncell[2]);
         uint32_t *row = nbr + i * (int64_t)cap;
-        int n = 0;
-        // Two parts: first the pairs inside r_cut at build time, then the skin shell.  The pair kernels
-        // walk a row front to back, so the lanes of a warp reach the (mostly skipped) shell entries
-        // together instead of diverging entry by entry.  Inside a part, 27 cells in the fixed order
-        // idx = (oz+1)*9 + (oy+1)*3 + (ox+1); runs[part*27 + idx] = first slot of the cell's run
-        // (entries of a run ascend in atom index).  The reverse-pair index uses the runs: the partner
-        // of an entry in run (part, idx) sits in run (part, 26 - idx) of the partner's row (r2 is
-        // bitwise symmetric, so both directions fall in the same part).
-        for (int pi = 0; pi < 54; ++pi) {
-            const int part = pi / 27, idx = pi % 27;
-            if (runs && lane == 0) runs[i * RUNS_PITCH + pi] = (uint16_t)(n < cap ? n : cap);
-            if (part == 1 && !(g.r_cut2 < g.r_list2)) continue;  // no skin: the shell is empty
+        // visit(idx, fn): candidates of cell idx in chunks of 32; fn(entry, r2, valid) per lane
+        auto visit = [&](int idx, auto fn) {
             const int oz = idx / 9 - 1, oy = (idx / 3) % 3 - 1, ox = idx % 3 - 1;
             int z = cz + oz, nz = 0;
-            if (z < 0) { if (!g.pbc[2]) continue; z += g.ncell[2]; nz = -1; }
-            else if (z >= g.ncell[2]) { if (!g.pbc[2]) continue; z -= g.ncell[2]; nz = 1; }
+            if (z < 0) { if (!g.pbc[2]) return; z += g.ncell[2]; nz = -1; }
+            else if (z >= g.ncell[2]) { if (!g.pbc[2]) return; z -= g.ncell[2]; nz = 1; }
             int y = cy + oy, ny = 0;
-            if (y < 0) { if (!g.pbc[1]) continue; y += g.ncell[1]; ny = -1; }
-            else if (y >= g.ncell[1]) { if (!g.pbc[1]) continue; y -= g.ncell[1]; ny = 1; }
+            if (y < 0) { if (!g.pbc[1]) return; y += g.ncell[1]; ny = -1; }
+            else if (y >= g.ncell[1]) { if (!g.pbc[1]) return; y -= g.ncell[1]; ny = 1; }
             int x = cx + ox, nx = 0;
-            if (x < 0) { if (!g.pbc[0]) continue; x += g.ncell[0]; nx = -1; }
-            else if (x >= g.ncell[0]) { if (!g.pbc[0]) continue; x -= g.ncell[0]; nx = 1; }
+            if (x < 0) { if (!g.pbc[0]) return; x += g.ncell[0]; nx = -1; }
+            else if (x >= g.ncell[0]) { if (!g.pbc[0]) return; x -= g.ncell[0]; nx = 1; }
             const int c = (z * g.ncell[1] + y) * g.ncell[0] + x;
             const int b = cell_start[c], e = cell_start[c + 1];
             const float sx = __fmul_rn((float)nx, g.L[0]), sy = __fmul_rn((float)ny, g.L[1]),
@@ -213,22 +217,53 @@ k_build_cells(int64_t N, const float4 *__restrict__ pos4, const int32_t *__restr
             const bool home = (nx | ny | nz) == 0;
             for (int base = b; base < e; base += 32) {
                 const int j = base + lane;
-                bool keep = false;
-                if (j < e && !(home && j == (int)i)) {
-                    const float r2 = list_r2(xi, pos4[j], sx, sy, sz);
-                    keep = r2 < g.r_list2 && (r2 < g.r_cut2) == (part == 0);
-                }
-                const unsigned m = __ballot_sync(0xffffffffu, keep);
-                const int p = n + __popc(m & ((1u << lane) - 1u));
-                if (keep && p < cap) row[p] = (uint32_t)j | code;
-                n += __popc(m);
+                const bool valid = j < e && !(home && j == (int)i);
+                const float r2 = valid ? list_r2(xi, pos4[j], sx, sy, sz) : 3.0e38f;
+                fn((uint32_t)j | code, r2, valid);
             }
+        };
+        int n_in = 0, n_out = 0;
+        for (int idx = 0; idx < 27; ++idx) {
+            if (lane == 0) {
+                if (runs) runs[i * RUNS_PITCH + idx] = (uint16_t)(n_in < cap ? n_in : cap);
+                s_rel[wid][idx] = n_out;
+            }
+            visit(idx, [&](uint32_t entry, float r2, bool valid) {
+                const bool kin = valid && r2 < g.r_cut2 && r2 < g.r_list2;
+                const bool kout = valid && !(r2 < g.r_cut2) && r2 < g.r_list2;
+                const unsigned m_in = __ballot_sync(0xffffffffu, kin), m_out = __ballot_sync(0xffffffffu, kout);
+                const int p = n_in + __popc(m_in & below), q = n_out + __popc(m_out & below);
+                if (kin && p < cap) row[p] = entry;
+                if (kout && q < SHELL_BUF) s_shell[wid][q] = entry;
+                n_in += __popc(m_in);
+                n_out += __popc(m_out);
+            });
         }
-        if (runs && lane == 0) runs[i * RUNS_PITCH + 54] = (uint16_t)(n < cap ? n : cap);
+        __syncwarp();
+        if (n_out <= SHELL_BUF) {
+            for (int q = lane; q < n_out; q += 32)
+                if (n_in + q < cap) row[n_in + q] = s_shell[wid][q];
+        } else {  // the shell did not fit: scan it again, now that its place in the row is known
+            int q0 = n_in;
+            for (int idx = 0; idx < 27; ++idx)
+                visit(idx, [&](uint32_t entry, float r2, bool valid) {
+                    const bool kout = valid && !(r2 < g.r_cut2) && r2 < g.r_list2;
+                    const unsigned m_out = __ballot_sync(0xffffffffu, kout);
+                    const int q = q0 + __popc(m_out & below);
+                    if (kout && q < cap) row[q] = entry;
+                    q0 += __popc(m_out);
+                });
+        }
+        const int n = n_in + n_out;
+        if (runs) {
+            if (lane < 27) runs[i * RUNS_PITCH + 27 + lane] = (uint16_t)(n_in + s_rel[wid][lane] < cap ? n_in + s_rel[wid][lane] : cap);
+            if (lane == 0) runs[i * RUNS_PITCH + 54] = (uint16_t)(n < cap ? n : cap);
+        }
         if (lane == 0) {
             count[i] = n < cap ? n : cap;
             if (n > cap) atomicMax(&flags[FLAG_MAXCOUNT], n);
         }
+        __syncwarp();  // s_shell / s_rel are reused for the warp's next atom
     }
 }
 

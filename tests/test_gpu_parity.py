@@ -38,7 +38,7 @@ def _gpu_system(gm, w, **model_kw):
 
 
 # ------------------------------------------------------------------ neighbour sets: bit exact
-@pytest.mark.parametrize("name", ["tiny", "ionic_liquid", "li1024", "li8192", "cluster", "mixed_pbc", "ragged"])
+@pytest.mark.parametrize("name", ["tiny", "ionic_liquid", "li1024", "li8192", "li8192_wide_skin", "cluster", "mixed_pbc", "ragged"])
 def test_neighbor_sets_bit_exact(gm, orc, name):
     if name == "tiny":
         w = wl.tiny_box(hidden=(16, 16))  # image loop, duplicate-by-image pairs
@@ -48,6 +48,8 @@ def test_neighbor_sets_bit_exact(gm, orc, name):
         w = wl.li3po4_box(1024, hidden=(16, 16))  # exactly 3 cells per axis
     elif name == "li8192":
         w = wl.li3po4_box(8192, hidden=(16, 16), skin=1.0)
+    elif name == "li8192_wide_skin":
+        w = wl.li3po4_box(8192, hidden=(16, 16), skin=4.0)  # ~330 shell entries per row: more than the build kernel stages
     elif name == "cluster":
         w = wl.cluster(24, 2)  # no periodic axis
     elif name == "mixed_pbc":
@@ -236,7 +238,7 @@ def test_single_atom_and_isolated_atoms(gm, orc):
 
 
 # ------------------------------------------------------------------ pair-buffer force reduction
-@pytest.mark.parametrize("name", ["config1", "config2", "config3_1024", "config3_8192", "cluster", "ragged"])
+@pytest.mark.parametrize("name", ["config1", "config2", "config3_1024", "config3_8192", "cluster", "ragged", "wide_skin"])
 def test_pair_buffer_force_mode(gm, orc, name):
     """GMNN_FORCE_PAIRBUF: g_ij evaluated once per directed pair and delivered through the
     reverse-pair index; same tolerances as the gather form, bit-reproducible, and the two forms
@@ -245,6 +247,8 @@ def test_pair_buffer_force_mode(gm, orc, name):
         w = wl.cluster(24, 2)
     elif name == "ragged":
         w = wl.li3po4_box(1000, hidden=(64, 48), skin=0.7)
+    elif name == "wide_skin":
+        w = wl.li3po4_box(8192, hidden=(32, 32), skin=4.0)  # shell part of a row larger than the build kernel stages
     else:
         w = wl.make_workload(name)
     sysm, pos, ref = _check_energy_forces(gm, orc, w, force_mode=gm.GMNN_FORCE_PAIRBUF)
