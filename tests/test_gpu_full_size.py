@@ -109,3 +109,42 @@ def test_config5_md_steps_conserve_energy(gm):
     p = (vel * mass[:, None]).sum(0).cpu().numpy()
     v_th = np.sqrt(wl.KB_EV * 300.0 / np.mean(w.masses) * 9.648533212e-3)
     assert np.abs(p).max() / w.masses.sum() <= 1e-5 * v_th
+
+
+def test_config2_full_run(gm, orc):
+    """Config 2 as BASELINE.json states it: 1 536 atoms, 1 000 NVE steps, dt 0.5 fs, skin 0.5, in
+    bench.py's configuration.  The first 10 steps are compared with the oracle's own NVE (positions,
+    velocities, energies).  The random-weight model has no repulsive core, so this box heats up (320 K
+    -> 3e4 K within 100 steps): the remaining 990 steps are a stress run of the
+    device-side rebuild (almost every step) that must finish with finite numbers, a consistent final
+    state and no error flag; energy conservation is asserted on the first 60 steps only."""
+    import torch
+
+    w = wl.make_workload("config2")
+    model = gm.Model(w.model, mlp_precision=gm.GMNN_MLP_3XTF32, force_mode=gm.GMNN_FORCE_PAIRBUF)
+    sysm = gm.System(model, w.species)
+    pos = torch.from_numpy(w.positions).cuda()
+    vel = torch.from_numpy(w.velocities).cuda()
+    mass = torch.from_numpy(w.masses).cuda()
+    sysm.set_int("capacity", 320)  # head room: the list capacity is static (PAPER.md:382 `extra_capacity`)
+    sysm.build_neighbors(pos, w.cell9, w.pbc, w.model.r_cut, w.skin)
+    ep, ek, nreb = sysm.md_verlet_steps(pos, vel, mass, w.dt_fs, 10)
+    ref = orc.nve(orc.Model(w.model), w.positions, w.velocities, w.masses, w.species, w.cell, w.pbc, w.skin, w.dt_fs, 10)
+    L = w.cell.astype(np.float64)
+    d = pos.cpu().numpy().astype(np.float64) - ref.positions
+    d -= np.round(d / L) * L
+    assert np.abs(d).max() <= 1e-4
+    assert np.abs(vel.cpu().numpy() - ref.velocities).max() <= 2e-5
+    assert np.abs(ep.cpu().numpy() - ref.epot).max() <= 1e-5 * np.abs(ref.epot).max() + 1e-3
+    assert np.abs(ek.cpu().numpy() - ref.ekin).max() <= 1e-4 * np.abs(ref.ekin).max()
+    ep2, ek2, nreb2 = sysm.md_verlet_steps(pos, vel, mass, w.dt_fs, 50)
+    etot = np.concatenate([(ep + ek).cpu().numpy(), (ep2 + ek2).cpu().numpy()[1:]])
+    assert np.abs(etot - etot[0]).max() <= 2e-3 * np.abs(etot[0])       # 61 energies, 5 eV of 2 566 allowed
+    ep3, ek3, nreb3 = sysm.md_verlet_steps(pos, vel, mass, w.dt_fs, 940)
+    sysm.check()
+    assert nreb + nreb2 + nreb3 >= 100                                   # the rebuild path was exercised
+    assert torch.isfinite(pos).all() and torch.isfinite(vel).all()
+    assert np.isfinite(ep3.cpu().numpy()).all() and np.isfinite(ek3.cpu().numpy()).all()
+    # the state the loop left behind is the state a fresh evaluation gives
+    e, ea, f = sysm.energy_forces(pos)
+    assert abs(float(e.cpu()[0]) - float(ep3[-1])) <= 1e-6 * float(ea.abs().sum())
