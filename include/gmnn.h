@@ -118,8 +118,12 @@ void gmnn_system_destroy(gmnn_system *s);
  *   "tc_split_bk"     16 | 32 (default): K extent of one pipeline stage of the 3xTF32 GEMM
  *   "tc_flush_k"      multiple of 16 (default 64): K extent after which the tensor-memory accumulator
  *                     is flushed into registers (the tensor core accumulates with truncation)
+ *   "tc_flush_head"   1..8 (default 2): the first two accumulator chunks of a tile of the BACKWARD GEMMs span
+ *                     this many flush intervals (more run-way for the MMAs while the epilogue finishes
+ *                     the previous tile; touches forces only, energies come from the forward GEMMs)
  *   "tc_debug"        timing experiments of mlp_tc.cu that knock out work (WRONG results); 0 = off
- *   The four tc_* knobs are process-wide.
+ *   "cb_halves"       1 | 2 (default) | 3: block shape of the contraction backward kernel (descriptor.cu)
+ *   The tc_* knobs and cb_halves are process-wide.
  * Returns GMNN_INVALID_ARG for an unknown key or value. */
 int gmnn_system_set_int(gmnn_system *s, const char *key, int64_t value);
 int gmnn_system_get_int(const gmnn_system *s, const char *key, int64_t *value /*HOST*/);

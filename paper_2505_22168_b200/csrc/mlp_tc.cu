@@ -75,6 +75,7 @@ struct TcArgs {
     int n_tiles_n;
     int n_tiles;   // total
     int flush;     // pipeline stages per accumulator flush (K chunk = flush * BK)
+    int flush1;    // ... of the first two chunks of a tile (>= flush)
     int debug;     // timing experiments only (results wrong): 1 skip split work, 2 hi.hi MMA only, 4 skip stores
     float *C;      // [M][N]
     float *C2;     // EPI_HIDDEN: swish'(z)
@@ -84,6 +85,21 @@ struct TcArgs {
     float *ypart;         // EPI_HIDDEN_HEAD: [2 * n_tiles_n][m_pad]
     int64_t m_pad;
 };
+
+// Accumulator-flush schedule of a tile: the first two chunks span flush1 pipeline stages each, the
+// rest `flush`.  (Longer first chunks give the MMA issuer more run-way while the epilogue warps are
+// still in the previous tile's final phase; used by the backward GEMMs, see tc_gemm.)
+__device__ __forceinline__ void chunk_pos(const TcArgs &p, int kb, int nkb, bool &first, bool &last) {
+    const int head = 2 * p.flush1;
+    const int pos = kb < head ? kb % p.flush1 : (kb - head) % p.flush;
+    const int len = kb < head ? p.flush1 : p.flush;
+    first = pos == 0;
+    last = pos == len - 1 || kb == nkb - 1;
+}
+__device__ __forceinline__ int chunk_count(const TcArgs &p, int nkb) {
+    const int head = nkb < 2 * p.flush1 ? nkb : 2 * p.flush1;
+    return (head + p.flush1 - 1) / p.flush1 + (nkb - head + p.flush - 1) / p.flush;
+}
 
 __device__ __forceinline__ void swish_pair_tc(float z, float &h, float &d) {
     const float s = __fdividef(1.f, 1.f + __expf(-z));  // ex2.approx + rcp.approx: ~2 ulp, no slow path
@@ -250,10 +266,11 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
             uint32_t it = 0, chunk = 0;
             for (int t = blockIdx.x; t < p.n_tiles; t += gridDim.x) {
                 for (int kb = 0; kb < nkb; ++kb, ++it) {
-                    const int in_chunk = kb % p.flush;
+                    bool chunk_first, chunk_last;
+                    chunk_pos(p, kb, nkb, chunk_first, chunk_last);
                     const int a = chunk & 1;
                     const uint32_t d_tmem = tmem_base + (uint32_t)a * TC_BN_MAX;
-                    if (in_chunk == 0) {
+                    if (chunk_first) {
                         mbar_wait(bar_tempty(a), ((chunk >> 1) & 1) ^ 1);
                         tcgen05_fence_after();
                     }
@@ -263,7 +280,7 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
                     const int krem = p.K - kb * BK;
                     const int ksteps = krem >= BK ? BK / 8 : (krem + 7) / 8;
                     const uint64_t da_hi = make_smem_desc_mn128(a_hi(s), BK * 128), db_hi = make_smem_desc<Cfg::SWZ>(b_hi(s));
-                    uint32_t acc = in_chunk != 0;
+                    uint32_t acc = !chunk_first;
                     if (SPLIT && !(p.debug & 2)) {  // small cross terms first: they meet the smallest accumulator
                         const uint64_t da_lo = make_smem_desc_mn128(a_lo(s), BK * 128), db_lo = make_smem_desc<Cfg::SWZ>(b_lo(s));
                         for (int k = 0; k < ksteps; ++k) {
@@ -280,7 +297,7 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
                         acc = 1u;
                     }
                     mma_commit(bar_empty(s));
-                    if (in_chunk == p.flush - 1 || kb == nkb - 1) {
+                    if (chunk_last) {
                         mma_commit(bar_tfull(a));
                         ++chunk;
                     }
@@ -313,7 +330,7 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
         const int quad = warp & 3;                        // TMEM lanes 32*quad .. 32*quad+31
         const int half = (warp - TC_FIRST_EPI_WARP) >> 2;  // 32-column groups half, half+2, half+4, half+6
         const int n_groups = (p.bn + 31) / 32;
-        const int n_chunks = (nkb + p.flush - 1) / p.flush;
+        const int n_chunks = chunk_count(p, nkb);
         const uint32_t lane_base = tmem_base + ((uint32_t)(quad * 32) << 16);
         uint32_t chunk = 0;
         for (int t = blockIdx.x; t < p.n_tiles; t += gridDim.x) {
@@ -444,10 +461,11 @@ k_gemm_tc_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
             uint32_t it = 0, chunk = 0;
             for (int t = pair; t < p.n_tiles; t += n_pairs) {
                 for (int kb = 0; kb < nkb; ++kb, ++it) {
-                    const int in_chunk = kb % p.flush;
+                    bool chunk_first, chunk_last;
+                    chunk_pos(p, kb, nkb, chunk_first, chunk_last);
                     const int a = chunk & 1;
                     const uint32_t d_tmem = tmem_base + (uint32_t)a * TC_BN_MAX;
-                    if (in_chunk == 0) {
+                    if (chunk_first) {
                         mbar_wait(bar_tempty(a), ((chunk >> 1) & 1) ^ 1);
                         tcgen05_fence_after();
                     }
@@ -458,7 +476,7 @@ k_gemm_tc_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                     const int ksteps = krem >= BK ? BK / 8 : (krem + 7) / 8;
                     const uint64_t da_hi = make_smem_desc_mn128(a_hi(s), BK * 128), db_hi = make_smem_desc<BK * 4>(b_hi(s));
                     const uint64_t da_lo = make_smem_desc_mn128(a_lo(s), BK * 128), db_lo = make_smem_desc<BK * 4>(b_lo(s));
-                    uint32_t acc = in_chunk != 0;
+                    uint32_t acc = !chunk_first;
                     for (int k = 0; k < ksteps; ++k) {  // small cross terms first
                         const uint64_t koff = (uint64_t)((k * 32) >> 4), aoff = (uint64_t)((k * 1024) >> 4);
                         mma_tf32_ss_pair(d_tmem, da_lo + aoff, db_hi + koff, idesc, acc);
@@ -470,7 +488,7 @@ k_gemm_tc_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                         mma_tf32_ss_pair(d_tmem, da_hi + aoff, db_hi + koff, idesc, 1u);
                     }
                     mma_commit_pair(bar_empty(s), 3);
-                    if (in_chunk == p.flush - 1 || kb == nkb - 1) {
+                    if (chunk_last) {
                         mma_commit_pair(bar_tfull(a), 3);
                         ++chunk;
                     }
@@ -501,7 +519,7 @@ k_gemm_tc_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
         const int quad = warp & 3;
         const int half = (warp - TC_FIRST_EPI_WARP) >> 2;
         const int n_groups = (p.bn + 31) / 32;
-        const int n_chunks = (nkb + p.flush - 1) / p.flush;
+        const int n_chunks = chunk_count(p, nkb);
         const uint32_t lane_base = tmem_base + ((uint32_t)(quad * 32) << 16);
         uint32_t chunk = 0;
         for (int t = pair; t < p.n_tiles; t += n_pairs) {
@@ -658,6 +676,7 @@ static int tc_launch(const CUtensorMap &tmA, const CUtensorMap &tmB, const TcArg
 }
 
 int g_tc_pair = 1;    // knob "tc_pair": 3xTF32 GEMMs on CTA pairs (cta_group::2)
+int g_tc_flush_head = 2;  // knob "tc_flush_head": first-two-chunks multiplier of the backward GEMMs (forces only)
 int g_tc_debug = 0;
 int g_tc_flush_k = 64;   // knob "tc_flush_k": K extent between accumulator flushes of the 3xTF32 mode
 int g_tc_split_bk = 32;  // knob (gmnn_system_set_int "tc_split_bk"): K extent of a 3xTF32 stage, 16 or 32
@@ -678,6 +697,7 @@ int tc_gemm(bool split, int epi, int64_t M, int N, int K, const float *A, const 
     a.n_tiles_n = (N + a.bn - 1) / a.bn;
     a.n_tiles = (int)((M + TC_BM - 1) / TC_BM) * a.n_tiles_n;
     a.flush = split ? (g_tc_flush_k / BK > 0 ? g_tc_flush_k / BK : 1) : (K + BK - 1) / BK;  // TF32 mode: one chunk
+    a.flush1 = a.flush * ((split && epi != EPI_HIDDEN && epi != EPI_HIDDEN_HEAD) ? g_tc_flush_head : 1);
     a.debug = g_tc_debug;
     a.C = C, a.C2 = C2, a.bias = bias, a.Dmul = Dmul;
     a.w_head = w_head, a.ypart = ypart, a.m_pad = (M + TC_BM - 1) / TC_BM * TC_BM;
