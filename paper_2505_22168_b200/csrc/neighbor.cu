@@ -24,21 +24,22 @@ __device__ __forceinline__ bool skip_rebuild(const int32_t *cond, float thr2) {
 
 __global__ void k_wrap(int64_t N, float *x, Geometry g, const int32_t *cond, float thr2) {
     if (skip_rebuild(cond, thr2)) return;
-    int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    if (t >= 3 * N) return;
-    int a = (int)(t % 3);
-    if (!g.pbc[a]) return;
-    float v = x[t];
-    v -= g.L[a] * floorf(v * g.invL[a]);
-    if (!(v >= 0.f) || v >= g.L[a]) v = 0.f;
-    x[t] = v;
+    for (int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; t < 3 * N; t += gridDim.x * (int64_t)blockDim.x) {
+        int a = (int)(t % 3);
+        if (!g.pbc[a]) continue;
+        float v = x[t];
+        v -= g.L[a] * floorf(v * g.invL[a]);
+        if (!(v >= 0.f) || v >= g.L[a]) v = 0.f;
+        x[t] = v;
+    }
 }
 
 __global__ void k_zero_cells(int64_t ncells, int32_t *cell_count, int32_t *cell_fill, const int32_t *cond, float thr2) {
     if (skip_rebuild(cond, thr2)) return;
-    int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    if (t <= ncells) cell_count[t] = 0;
-    if (t < ncells) cell_fill[t] = 0;
+    for (int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; t <= ncells; t += gridDim.x * (int64_t)blockDim.x) {
+        cell_count[t] = 0;
+        if (t < ncells) cell_fill[t] = 0;
+    }
 }
 
 __device__ __forceinline__ int cell_coord(float x, float inv_edge, int nc) {
@@ -49,20 +50,20 @@ __device__ __forceinline__ int cell_coord(float x, float inv_edge, int nc) {
 __global__ void k_cell_assign(int64_t N, const float *__restrict__ x, Geometry g, int32_t *cell_of,
                               int32_t *cell_count, int32_t *flags, const int32_t *cond, float thr2) {
     if (skip_rebuild(cond, thr2)) return;
-    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    if (i >= N) return;
-    float p[3] = {x[3 * i], x[3 * i + 1], x[3 * i + 2]};
-    int c[3];
-    bool bad = false;
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < N; i += gridDim.x * (int64_t)blockDim.x) {
+        float p[3] = {x[3 * i], x[3 * i + 1], x[3 * i + 2]};
+        int c[3];
+        bool bad = false;
 #pragma unroll
-    for (int a = 0; a < 3; ++a) {
-        bad |= !(p[a] >= 0.f && p[a] < g.L[a]);
-        c[a] = cell_coord(p[a], g.inv_edge[a], g.ncell[a]);
+        for (int a = 0; a < 3; ++a) {
+            bad |= !(p[a] >= 0.f && p[a] < g.L[a]);
+            c[a] = cell_coord(p[a], g.inv_edge[a], g.ncell[a]);
+        }
+        if (bad) flags[FLAG_OUT_OF_BOX] = 1;
+        int cid = (c[2] * g.ncell[1] + c[1]) * g.ncell[0] + c[0];
+        cell_of[i] = cid;
+        atomicAdd(&cell_count[cid], 1);
     }
-    if (bad) flags[FLAG_OUT_OF_BOX] = 1;
-    int cid = (c[2] * g.ncell[1] + c[1]) * g.ncell[0] + c[0];
-    cell_of[i] = cid;
-    atomicAdd(&cell_count[cid], 1);
 }
 
 // Exclusive scan of cell_count[0..n) into cell_start[0..n]; one block of 1024 threads.
@@ -104,11 +105,11 @@ __global__ void k_scan_cells(int64_t n, const int32_t *__restrict__ cnt, int32_t
 __global__ void k_cell_fill(int64_t N, const int32_t *__restrict__ cell_of, const int32_t *__restrict__ cell_start,
                             int32_t *cell_fill, int32_t *slot_tmp, const int32_t *cond, float thr2) {
     if (skip_rebuild(cond, thr2)) return;
-    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    if (i >= N) return;
-    int c = cell_of[i];
-    int slot = atomicAdd(&cell_fill[c], 1);
-    slot_tmp[cell_start[c] + slot] = (int32_t)i;
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < N; i += gridDim.x * (int64_t)blockDim.x) {
+        int c = cell_of[i];
+        int slot = atomicAdd(&cell_fill[c], 1);
+        slot_tmp[cell_start[c] + slot] = (int32_t)i;
+    }
 }
 
 // The atomics above fill a cell in arbitrary order; rank every atom inside its cell by caller
@@ -116,14 +117,14 @@ __global__ void k_cell_fill(int64_t N, const int32_t *__restrict__ cell_of, cons
 __global__ void k_cell_rank(int64_t N, const int32_t *__restrict__ slot_tmp, const int32_t *__restrict__ cell_of,
                             const int32_t *__restrict__ cell_start, int32_t *perm, const int32_t *cond, float thr2) {
     if (skip_rebuild(cond, thr2)) return;
-    int64_t k = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    if (k >= N) return;
-    int i = slot_tmp[k];
-    int c = cell_of[i];
-    int b = cell_start[c], e = cell_start[c + 1];
-    int rank = 0;
-    for (int q = b; q < e; ++q) rank += (slot_tmp[q] < i);
-    perm[b + rank] = i;
+    for (int64_t k = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; k < N; k += gridDim.x * (int64_t)blockDim.x) {
+        int i = slot_tmp[k];
+        int c = cell_of[i];
+        int b = cell_start[c], e = cell_start[c + 1];
+        int rank = 0;
+        for (int q = b; q < e; ++q) rank += (slot_tmp[q] < i);
+        perm[b + rank] = i;
+    }
 }
 
 // pos4 (internal order) from the caller's positions; at a build also the reference copy xref;
@@ -404,6 +405,12 @@ __global__ void k_finish_rebuild(int32_t *flags, const int32_t *cond, float thr2
 }
 
 static inline unsigned nblocks(int64_t n, int per) { return (unsigned)((n + per - 1) / per); }
+// blocks of 256 threads for a thread-per-item grid-stride kernel: at most 8 blocks per SM, so that a
+// launch that skip_rebuild() turns into a no-op costs a few microseconds
+static inline unsigned small_grid(int64_t n_items) {
+    const int64_t want = (n_items + 255) / 256, cap = 148 * 8;
+    return (unsigned)(want < cap ? (want > 0 ? want : 1) : cap);
+}
 // blocks of 256 threads for a warp-per-atom grid-stride kernel: at most 16 waves of 148 SMs x 8 blocks
 static inline unsigned warp_grid(int64_t n_atoms) {
     const int64_t want = (n_atoms * 32 + 255) / 256, cap = 148 * 8 * 16;
@@ -415,18 +422,18 @@ int launch_build(gmnn_system *s, const float *positions, cudaStream_t st, const 
     const int64_t N = s->N;
     const Geometry g = s->geo;
     if (wrap_first && positions_mut) {
-        k_wrap<<<nblocks(3 * N, 256), 256, 0, st>>>(N, positions_mut, g, cond, thr2);
+        k_wrap<<<small_grid(3 * N), 256, 0, st>>>(N, positions_mut, g, cond, thr2);
         GMNN_LAUNCHED();
     }
-    k_zero_cells<<<nblocks(s->ncells + 1, 256), 256, 0, st>>>(s->ncells, s->cell_count, s->cell_fill, cond, thr2);
+    k_zero_cells<<<small_grid(s->ncells + 1), 256, 0, st>>>(s->ncells, s->cell_count, s->cell_fill, cond, thr2);
     GMNN_LAUNCHED();
-    k_cell_assign<<<nblocks(N, 256), 256, 0, st>>>(N, positions, g, s->cell_of, s->cell_count, s->flags, cond, thr2);
+    k_cell_assign<<<small_grid(N), 256, 0, st>>>(N, positions, g, s->cell_of, s->cell_count, s->flags, cond, thr2);
     GMNN_LAUNCHED();
     k_scan_cells<<<1, 1024, 0, st>>>(s->ncells, s->cell_count, s->cell_start, cond, thr2);
     GMNN_LAUNCHED();
-    k_cell_fill<<<nblocks(N, 256), 256, 0, st>>>(N, s->cell_of, s->cell_start, s->cell_fill, s->slot_tmp, cond, thr2);
+    k_cell_fill<<<small_grid(N), 256, 0, st>>>(N, s->cell_of, s->cell_start, s->cell_fill, s->slot_tmp, cond, thr2);
     GMNN_LAUNCHED();
-    k_cell_rank<<<nblocks(N, 256), 256, 0, st>>>(N, s->slot_tmp, s->cell_of, s->cell_start, s->perm, cond, thr2);
+    k_cell_rank<<<small_grid(N), 256, 0, st>>>(N, s->slot_tmp, s->cell_of, s->cell_start, s->perm, cond, thr2);
     GMNN_LAUNCHED();
     k_gather<<<nblocks(N, 256), 256, 0, st>>>(N, positions, s->species, s->perm, s->pos4, s->xref, true, 0.f,
                                               nullptr, cond, thr2);
