@@ -111,6 +111,9 @@ void gmnn_system_destroy(gmnn_system *s);
  *   "md_continue"     1: a gmnn_md_verlet_steps call whose positions and velocities are exactly the
  *                     output of the previous call reuses that call's final forces and energies
  *                     instead of evaluating them again at entry (the caller asserts this)
+ *   "md_graph"        1 (default): gmnn_md_verlet_steps captures one step as a CUDA graph after the first
+ *                     step and replays it (runs of >= 4 steps, not while "profile" is on); 0: eager loop.
+ *                     Results are bit-identical either way
  *   "capacity"        neighbour slots per atom for the next build (0 = estimate from the density)
  *   "mlp_precision", "force_mode": override the model's value for this system; changing force_mode
  *                     invalidates the neighbour list (call gmnn_build_neighbors again)

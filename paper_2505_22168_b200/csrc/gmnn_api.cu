@@ -315,6 +315,11 @@ void gmnn_system_destroy(gmnn_system *s) {
     dev_free(s->stage_pos); dev_free(s->stage_f); dev_free(s->stage_e);
     if (s->flags_host) cudaFreeHost(s->flags_host);
     for (cudaEvent_t e : s->events) cudaEventDestroy(e);
+    if (s->graph_stream) {
+        cudaStreamDestroy(s->graph_stream);
+        cudaEventDestroy(s->graph_ev[0]);
+        cudaEventDestroy(s->graph_ev[1]);
+    }
     delete s;
 }
 
@@ -331,6 +336,8 @@ int gmnn_system_set_int(gmnn_system *s, const char *key, int64_t v) {
         s->n_stage_events = 0;
     } else if (!strcmp(key, "md_continue")) {
         s->md_continue = v != 0;
+    } else if (!strcmp(key, "md_graph")) {
+        s->md_graph = v != 0;
     } else if (!strcmp(key, "capacity")) {
         if (v < 0 || v > 4096) {
             set_error("capacity must be in [0, 4096]");
@@ -372,6 +379,7 @@ int gmnn_system_get_int(const gmnn_system *s, const char *key, int64_t *v) {
     if (!strcmp(key, "lanes_per_atom")) *v = s->lanes_per_atom;
     else if (!strcmp(key, "profile")) *v = s->profile;
     else if (!strcmp(key, "md_continue")) *v = s->md_continue;
+    else if (!strcmp(key, "md_graph")) *v = s->md_graph;
     else if (!strcmp(key, "capacity")) *v = s->cap;
     else if (!strcmp(key, "mlp_precision")) *v = s->mlp_precision;
     else if (!strcmp(key, "force_mode")) *v = s->force_mode;
@@ -693,20 +701,72 @@ int gmnn_md_verlet_steps(gmnn_system *s, float *positions, float *velocities, co
         T.mark("outputs");
     }
     s->md_state_valid = false;
-    for (int step = 1; step <= n_steps; ++step) {
-        if ((rc = launch_kick_drift(s, positions, velocities, s->f_tmp, masses, dt_fs, st))) return rc;
+    // One step: every launch has the same arguments at every step (the energies go to the series
+    // through a device-side counter), so the body can be captured once and replayed as a CUDA graph.
+    auto md_step = [&](cudaStream_t q) -> int {
+        int r;
+        if ((r = launch_kick_drift(s, positions, velocities, s->f_tmp, masses, dt_fs, q))) return r;
         T.mark("kick_drift");
         // rebuild (wrap first) iff the max displacement since the last build exceeds skin/2
-        if ((rc = launch_build(s, positions, st, s->flags + FLAG_DISP2, thr2, true, positions))) return rc;
+        if ((r = launch_build(s, positions, q, s->flags + FLAG_DISP2, thr2, true, positions))) return r;
         T.mark("rebuild_if_moved");
-        if ((rc = forward_backward(s, positions, s->model->head_mean_w, false, st, T))) return rc;
-        if ((rc = launch_scatter_outputs(s, nullptr, s->f_tmp, st))) return rc;
-        if ((rc = launch_energy_sum(s, ep, st, epot_series ? epot_series + step : nullptr))) return rc;
+        if ((r = forward_backward(s, positions, s->model->head_mean_w, false, q, T))) return r;
+        if ((r = launch_scatter_outputs(s, nullptr, s->f_tmp, q))) return r;
+        if ((r = launch_energy_sum(s, ep, q, nullptr))) return r;
         T.mark("outputs");
-        if ((rc = launch_kick_ke(s, velocities, s->f_tmp, masses, dt_fs, ek, st, ekin_series ? ekin_series + step : nullptr)))
-            return rc;
+        if ((r = launch_kick_ke(s, velocities, s->f_tmp, masses, dt_fs, ek, q, nullptr))) return r;
+        if ((epot_series || ekin_series) && (r = launch_series_append(s, epot_series, ekin_series, q))) return r;
         T.mark("kick_ke");
+        return GMNN_OK;
+    };
+    if (n_steps > 0 && (rc = launch_series_reset(s, 1, st))) return rc;
+    int step = 1;
+    // the first step runs eagerly (one-time function attributes and driver lookups happen there)
+    if (n_steps >= 1) {
+        if ((rc = md_step(st))) return rc;
+        ++step;
     }
+    if (step <= n_steps && s->md_graph && !s->profile && n_steps >= 4) {
+        if (!s->graph_stream) {
+            GMNN_CUDA(cudaStreamCreateWithFlags(&s->graph_stream, cudaStreamNonBlocking));
+            GMNN_CUDA(cudaEventCreateWithFlags(&s->graph_ev[0], cudaEventDisableTiming));
+            GMNN_CUDA(cudaEventCreateWithFlags(&s->graph_ev[1], cudaEventDisableTiming));
+        }
+        cudaStream_t q = s->graph_stream;
+        GMNN_CUDA(cudaEventRecord(s->graph_ev[0], st));
+        GMNN_CUDA(cudaStreamWaitEvent(q, s->graph_ev[0], 0));
+        const long long launches_before = g_launch_count;
+        cudaGraph_t graph = nullptr;
+        cudaGraphExec_t exec = nullptr;
+        GMNN_CUDA(cudaStreamBeginCapture(q, cudaStreamCaptureModeThreadLocal));
+        rc = md_step(q);
+        const cudaError_t cap = cudaStreamEndCapture(q, &graph);
+        if (rc || cap != cudaSuccess) {
+            if (graph) cudaGraphDestroy(graph);
+            if (!rc) {
+                set_error("CUDA graph capture of the MD step failed: %s", cudaGetErrorString(cap));
+                rc = GMNN_CUDA_ERROR;
+            }
+            return rc;
+        }
+        const long long per_step = g_launch_count - launches_before;  // captured, not yet run
+        g_launch_count = launches_before;
+        cudaError_t ge = cudaGraphInstantiate(&exec, graph, 0);
+        for (; ge == cudaSuccess && step <= n_steps; ++step) {
+            ge = cudaGraphLaunch(exec, q);
+            g_launch_count += per_step;
+        }
+        if (exec) cudaGraphExecDestroy(exec);
+        cudaGraphDestroy(graph);
+        if (ge != cudaSuccess) {
+            set_error("CUDA graph replay of the MD step failed: %s", cudaGetErrorString(ge));
+            return GMNN_CUDA_ERROR;
+        }
+        GMNN_CUDA(cudaEventRecord(s->graph_ev[1], q));
+        GMNN_CUDA(cudaStreamWaitEvent(st, s->graph_ev[1], 0));
+    }
+    for (; step <= n_steps; ++step)
+        if ((rc = md_step(st))) return rc;
     if ((rc = read_flags(s, st))) return rc;
     if (n_rebuilds) *n_rebuilds = s->flags_host[FLAG_REBUILDS];
     const int maxcount = s->flags_host[FLAG_MAXCOUNT];

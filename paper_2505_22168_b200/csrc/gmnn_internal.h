@@ -25,7 +25,7 @@ constexpr int MAX_HEAD_SLOTS = 16;  // partial sums per atom of the head fused i
 constexpr int PSI = 20;  // unique monomials per channel (contraction.cuh NM)
 
 // device-side flag words (int32) in System::flags
-enum Flag { FLAG_MAXCOUNT = 0, FLAG_STALE = 1, FLAG_OUT_OF_BOX = 2, FLAG_REBUILDS = 3, FLAG_DISP2 = 4, FLAG_REV_MISSING = 5, FLAG_WORDS = 8 };
+enum Flag { FLAG_MAXCOUNT = 0, FLAG_STALE = 1, FLAG_OUT_OF_BOX = 2, FLAG_REBUILDS = 3, FLAG_DISP2 = 4, FLAG_REV_MISSING = 5, FLAG_MD_STEP = 6, FLAG_WORDS = 8 };
 
 void set_error(const char *fmt, ...);
 extern long long g_launch_count;
@@ -126,6 +126,9 @@ struct gmnn_system {
     // knobs
     int lanes_per_atom = 0;
     int profile = 0;
+    int md_graph = 1;                // knob: replay the MD step as a CUDA graph (not while profiling stages)
+    cudaStream_t graph_stream = nullptr;  // capture / replay stream (the caller's may be the legacy stream)
+    cudaEvent_t graph_ev[2] = {};
     int md_continue = 0;             // knob: the next md call continues the previous one
     bool md_state_valid = false;     // f_tmp / e_total hold the forces and energies of the last md step
     int mlp_precision = 0, force_mode = 0;
@@ -167,6 +170,8 @@ int launch_kick_ke(gmnn_system *s, float *v, const float *f, const float *m, flo
                    cudaStream_t st, double *ekin_out2 = nullptr);
 int launch_ke(gmnn_system *s, const float *v, const float *m, double *ekin_out, cudaStream_t st,
               double *ekin_out2 = nullptr);
+int launch_series_append(gmnn_system *s, double *epot_series, double *ekin_series, cudaStream_t st);
+int launch_series_reset(gmnn_system *s, int32_t next_index, cudaStream_t st);
 int launch_welford(gmnn_system *s, int head, const float *f_head, float *f_mean, float *f_m2, cudaStream_t st);
 int launch_ensemble_energy_stats(gmnn_system *s, float *e_mean, float *e_var, cudaStream_t st);
 int launch_finish_var(int64_t n, float *m2, int n_heads, cudaStream_t st);

@@ -189,6 +189,31 @@ int launch_kick_ke(gmnn_system *s, float *v, const float *f, const float *m, flo
     return GMNN_OK;
 }
 
+// Series output of the MD loop with a device-side step counter, so that every step issues the same
+// launches with the same arguments (the loop body is replayed as a CUDA graph).
+__global__ void k_series_append(const double *__restrict__ e_total, double *epot_series, double *ekin_series,
+                                int32_t *counter) {
+    const int32_t k = *counter;
+    if (epot_series) epot_series[k] = e_total[0];
+    if (ekin_series) ekin_series[k] = e_total[1];
+    *counter = k + 1;
+}
+__global__ void k_set_int(int32_t *p, int32_t v) { *p = v; }
+
+int launch_series_append(gmnn_system *s, double *epot_series, double *ekin_series, cudaStream_t st) {
+    k_series_append<<<1, 1, 0, st>>>(s->e_total, epot_series, ekin_series, s->flags + FLAG_MD_STEP);
+    GMNN_LAUNCHED();
+    GMNN_CUDA(cudaGetLastError());
+    return GMNN_OK;
+}
+
+int launch_series_reset(gmnn_system *s, int32_t next_index, cudaStream_t st) {
+    k_set_int<<<1, 1, 0, st>>>(s->flags + FLAG_MD_STEP, next_index);
+    GMNN_LAUNCHED();
+    GMNN_CUDA(cudaGetLastError());
+    return GMNN_OK;
+}
+
 int launch_welford(gmnn_system *s, int head, const float *f_head, float *f_mean, float *f_m2, cudaStream_t st) {
     k_welford<<<nblocks(3 * s->N, 256), 256, 0, st>>>(3 * s->N, head, f_head, f_mean, f_m2);
     GMNN_LAUNCHED();
