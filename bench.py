@@ -300,7 +300,7 @@ def run_ours(args):
     if args.warmup > 0:
         _, _, nreb = sysm.md_verlet_steps(pos, vel, masses, w.dt_fs, args.warmup, want_series=False)
         total_rebuilds += nreb
-    sysm.set_int("profile", 1)
+    sysm.set_int("profile", 0 if args.no_stages else 1)
     sampler = ClockSampler(local)
     sampler.start()
     barrier()
@@ -314,7 +314,7 @@ def run_ours(args):
     clocks = sampler.stop()
     total_rebuilds += nreb
     ms = ev0.elapsed_time(ev1)
-    stages = sysm.stage_times()
+    stages = [] if args.no_stages else sysm.stage_times()
     sysm.set_int("profile", 0)
     ms_max = max_over_ranks(ms, world, dev)
     value = whole_job_value(N, args.steps, world, ms_max)
@@ -440,6 +440,8 @@ def main():
                     help="3xtf32 (default): tcgen05 tensor cores, fp32-accurate; fp32: SIMT FMA; tf32: single pass")
     ap.add_argument("--forces", default="pairbuf", choices=["gather", "pairbuf"],
                     help="force reduction: gather form, or pair buffer with a reverse-pair index (both deterministic)")
+    ap.add_argument("--no-stages", action="store_true",
+                    help="no per-stage CUDA events: the MD loop then replays its step as a CUDA graph (no roofline entry)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":
