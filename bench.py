@@ -64,7 +64,9 @@ def stage_model(w, nl_mean, nc_mean, n_hidden_macs, mlp, forces="pairbuf"):
         "pair_forward": dict(bytes=4.0 * nl_mean + 420.0, flops=12.0 * nl_mean + 340.0 * nc_mean, bound="alu"),
         "contract_forward": dict(bytes=400.0 + 4.0 * F, flops=2.0 * 5000.0, bound="hbm"),
         "mlp_forward": dict(bytes=4.0 * F + 4.0, flops=mlp_flops, bound="tensor" if tensor else "alu"),
-        "mlp_heads": dict(bytes=2048.0 + 8.0, flops=1024.0, bound="hbm"),
+        # one head: fused into the last GEMM epilogue, what is left adds 4 partial sums per atom
+        "mlp_heads": (dict(bytes=16.0 + 16.0 + 8.0, flops=8.0, bound="hbm") if w.model.n_heads == 1 and mlp != "fp32"
+                      else dict(bytes=2048.0 + 8.0, flops=1024.0 * w.model.n_heads, bound="hbm")),
         "mlp_backward": dict(bytes=4.0 * F, flops=mlp_flops, bound="tensor" if tensor else "alu"),
         "contract_backward": dict(bytes=4.0 * F + 800.0, flops=2.0 * 15000.0, bound="hbm"),
         # gather form: both directions per entry; pair buffer: one direction, g_ij written to and read
