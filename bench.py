@@ -381,7 +381,7 @@ def run_ours(args):
             if args.workload == "config5" and args.mlp == "3xtf32":
                 # dram__bytes_read.sum + dram__bytes_write.sum of the four launches of one step, per launch
                 # (profiles/ncu_r1_gemm_tc_pair.md)
-                roofline["traffic"] = round(20.44e9 / n_launch)
+                roofline["traffic"] = round(20.43e9 / n_launch)
         if info["bound"] == "tensor" and args.mlp == "3xtf32":
             roofline["note"] = ("achieved counts the ALGORITHMIC flops (one product per multiply-add); the 3xTF32 split "
                                 "executes 3 tensor-core MMAs per product, so tensor-pipe flops are 3x achieved")
