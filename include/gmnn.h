@@ -52,9 +52,12 @@ typedef enum {
 typedef enum {
     GMNN_MLP_FP32 = 0,   /* fp32 FMA on the SIMT pipes; the fp32-tolerance path                      */
     GMNN_MLP_3XTF32 = 1, /* tcgen05 TF32 tensor cores, 3-term error-compensated split (fp32 tol.)   */
-    GMNN_MLP_TF32 = 2    /* tcgen05 TF32 single pass, operands truncated by the tensor core: measured
+    GMNN_MLP_TF32 = 2,   /* tcgen05 TF32 single pass, operands truncated by the tensor core: measured
                             1e-2 .. 2.5e-2 on the force measure, i.e. NOT within the 2e-3 of a claimed
                             reduced-precision variant; an unclaimed fast mode       */
+    GMNN_MLP_3XF16 = 3   /* tcgen05 FP16 tensor cores, the same 3-term split on operands scaled by a
+                            power of two from each matrix's absolute maximum (fp32 tol.; twice the
+                            MMA rate of 3XTF32)                                                     */
 } gmnn_mlp_precision;
 
 /* How F_i = sum_j g_ij - sum_j g_ji is formed.  Both are atomics-free and bit-reproducible. */

@@ -25,7 +25,7 @@ GMNN_STALE_NEIGHBORS = -4
 GMNN_CUDA_ERROR = -5
 GMNN_OOM = -6
 GMNN_OUT_OF_BOX = -7
-GMNN_MLP_FP32, GMNN_MLP_3XTF32, GMNN_MLP_TF32 = 0, 1, 2
+GMNN_MLP_FP32, GMNN_MLP_3XTF32, GMNN_MLP_TF32, GMNN_MLP_3XF16 = 0, 1, 2, 3
 GMNN_FORCE_GATHER, GMNN_FORCE_PAIRBUF = 0, 1
 
 EXPORTS = (

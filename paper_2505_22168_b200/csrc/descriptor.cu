@@ -208,7 +208,7 @@ constexpr int CW = 33;  // padded warp tile pitch
 
 template <int NR>
 __global__ void __launch_bounds__(128)
-k_contract_forward(int64_t N, const float *__restrict__ psi, float *__restrict__ Gt) {
+k_contract_forward(int64_t N, const float *__restrict__ psi, float *__restrict__ Gt, uint32_t *__restrict__ amax) {
     using F = Feat<NR>;
     const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;  // blockDim.x == 128 == tile
     float P[NR][PSI];
@@ -231,7 +231,16 @@ k_contract_forward(int64_t N, const float *__restrict__ psi, float *__restrict__
     // G is tile-transposed ([N/128][F][128], the A-operand layout of the MLP): feature f of the 128
     // atoms of this block is one contiguous 512-byte run, so every store below is coalesced.
     float *g = Gt + (int64_t)blockIdx.x * F::N * 128 + threadIdx.x;
-    contract_forward<NR>([&](int s, int m) { return P[s][m]; }, [&](int f, float v) { g[(int64_t)f * 128] = v; });
+    float gmax = 0.f;  // max |G| of the evaluation: the operand scale of the 3xFP16 MLP (mlp_tc.cu)
+    contract_forward<NR>([&](int s, int m) { return P[s][m]; }, [&](int f, float v) {
+        g[(int64_t)f * 128] = v;
+        gmax = fmaxf(gmax, fabsf(v));
+    });
+    if (amax) {
+#pragma unroll
+        for (int o = 16; o >= 1; o >>= 1) gmax = fmaxf(gmax, __shfl_xor_sync(0xffffffffu, gmax, o));
+        if ((threadIdx.x & 31) == 0 && gmax > 0.f) atomicMax(amax, __float_as_uint(gmax));
+    }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -659,7 +668,8 @@ int launch_pair_backward(gmnn_system *s, cudaStream_t st) {
 
 int launch_contract_forward(gmnn_system *s, cudaStream_t st) {
     constexpr int NR = 5;
-    k_contract_forward<NR><<<nblocks(s->N, 128), 128, 0, st>>>(s->N, s->psi, s->G);
+    k_contract_forward<NR><<<nblocks(s->N, 128), 128, 0, st>>>(s->N, s->psi, s->G,
+                                                               s->mlp_precision == GMNN_MLP_3XF16 ? s->amax + AMAX_G : nullptr);
     GMNN_LAUNCHED();
     GMNN_CUDA(cudaGetLastError());
     return GMNN_OK;

@@ -23,7 +23,7 @@ void set_error(const char *fmt, ...) {
 }
 
 int launch_mlp_forward_tc(gmnn_system *s, cudaStream_t st);
-extern int g_tc_split_bk, g_tc_flush_k, g_tc_debug, g_tc_pair, g_cb_halves, g_tc_flush_head;
+extern int g_tc_split_bk, g_tc_flush_k, g_tc_debug, g_tc_pair, g_cb_halves, g_tc_flush_head, g_tc_h_bk;
 int launch_mlp_backward_tc(gmnn_system *s, const float *head_w_dev, cudaStream_t st);
 
 template <class T>
@@ -85,6 +85,8 @@ static int forward_backward(gmnn_system *s, const float *positions, const float 
     int rc;
     if ((rc = launch_gather_positions(s, positions, st, check_stale))) return rc;
     T.mark("gather");
+    if (s->mlp_precision == GMNN_MLP_3XF16)  // maxima of G, H, dZ: rebuilt by this evaluation's kernels
+        GMNN_CUDA(cudaMemsetAsync(s->amax, 0, sizeof(uint32_t) * AMAX_BVT, st));
     if ((rc = launch_pair_forward(s, st))) return rc;
     T.mark("pair_forward");
     if ((rc = launch_contract_forward(s, st))) return rc;
@@ -139,7 +141,7 @@ int gmnn_create(const gmnn_hparams *hp, const gmnn_weights *w, gmnn_model **out)
         set_error("n_weight_sets = %d: per-species weight sets are not built yet (DESIGN.md R11)", hp->n_weight_sets);
         return GMNN_UNSUPPORTED;
     }
-    if (hp->mlp_precision < 0 || hp->mlp_precision > GMNN_MLP_TF32 || hp->force_mode < 0 ||
+    if (hp->mlp_precision < 0 || hp->mlp_precision > GMNN_MLP_3XF16 || hp->force_mode < 0 ||
         hp->force_mode > GMNN_FORCE_PAIRBUF) {
         set_error("gmnn_create: bad mlp_precision / force_mode");
         return GMNN_INVALID_ARG;
@@ -201,6 +203,11 @@ int gmnn_create(const gmnn_hparams *hp, const gmnn_weights *w, gmnn_model **out)
         if (!rc) rc = dev_alloc(&m->WTs[l], 2 * (size_t)fi * fo);
         if (!rc) rc = launch_split_stack(m->W[l], m->Ws[l], (int64_t)fi * fo, nullptr);
         if (!rc) rc = launch_split_stack(m->WT[l], m->WTs[l], (int64_t)fi * fo, nullptr);
+        if (!rc && l == 0) rc = dev_alloc(&m->wmax, (size_t)MAX_LAYERS);
+        if (!rc) rc = dev_alloc(&m->Wh[l], 2 * (size_t)fi * fo);
+        if (!rc) rc = dev_alloc(&m->WTh[l], 2 * (size_t)fi * fo);
+        if (!rc) rc = launch_split_stack_h(m->W[l], m->Wh[l], (int64_t)fi * fo, m->wmax + l, nullptr);
+        if (!rc) rc = launch_split_stack_h(m->WT[l], m->WTh[l], (int64_t)fi * fo, m->wmax + l, nullptr);
     }
     if (!rc && cudaDeviceSynchronize() != cudaSuccess) rc = GMNN_CUDA_ERROR;
     if (!rc) rc = upload(&m->scale, w->scale, (size_t)hp->n_species);
@@ -225,11 +232,14 @@ void gmnn_destroy(gmnn_model *m) {
         dev_free(m->WT[l]);
         dev_free(m->Ws[l]);
         dev_free(m->WTs[l]);
+        dev_free(m->Wh[l]);
+        dev_free(m->WTh[l]);
         dev_free(m->b[l]);
     }
     dev_free(m->scale);
     dev_free(m->shift);
     dev_free(m->head_mean_w);
+    dev_free(m->wmax);
     delete m;
 }
 
@@ -280,6 +290,8 @@ int gmnn_system_create(const gmnn_model *m, int64_t n_atoms, const int32_t *spec
     A_(s->Bv, (size_t)m->dims[L] * m->dims[L - 1]);
     A_(s->BvT, (size_t)m->dims[L] * m->dims[L - 1]);
     A_(s->BvTs, 2 * (size_t)m->dims[L] * m->dims[L - 1]);
+    A_(s->BvTh, 2 * (size_t)m->dims[L] * m->dims[L - 1]);
+    A_(s->amax, (size_t)AMAX_SLOTS);
     A_(s->vhead, (size_t)m->dims[L]);
     A_(s->head_w, (size_t)M);
     A_(s->ypart, (size_t)MAX_HEAD_SLOTS * NP);
@@ -294,6 +306,11 @@ int gmnn_system_create(const gmnn_model *m, int64_t n_atoms, const int32_t *spec
     if (!rc && cudaMallocHost((void **)&s->flags_host, sizeof(int32_t) * FLAG_WORDS) != cudaSuccess) rc = GMNN_OOM;
     if (!rc && cudaMemset(s->flags, 0, sizeof(int32_t) * FLAG_WORDS) != cudaSuccess) rc = GMNN_CUDA_ERROR;
     if (!rc && cudaMemset(s->G, 0, sizeof(float) * NP * F) != cudaSuccess) rc = GMNN_CUDA_ERROR;  // rows of the ragged last tile
+    if (!rc && cudaMemset(s->amax, 0, sizeof(uint32_t) * AMAX_SLOTS) != cudaSuccess) rc = GMNN_CUDA_ERROR;
+    if (!rc) {  // swish' lies in [-0.1, 1.1]: its scale is a constant
+        const float dmax = 1.5f;
+        if (cudaMemcpy(s->amax + AMAX_D, &dmax, sizeof(float), cudaMemcpyHostToDevice) != cudaSuccess) rc = GMNN_CUDA_ERROR;
+    }
     if (rc) {
         if (rc == GMNN_OOM) set_error("out of device memory allocating the workspaces of %lld atoms", (long long)n_atoms);
         gmnn_system_destroy(s);
@@ -309,7 +326,7 @@ void gmnn_system_destroy(gmnn_system *s) {
     dev_free(s->cell_fill); dev_free(s->slot_tmp); dev_free(s->perm); dev_free(s->pos4); dev_free(s->xref);
     dev_free(s->nbr); dev_free(s->rev); dev_free(s->gbuf); dev_free(s->runs); dev_free(s->count); dev_free(s->psi); dev_free(s->G); dev_free(s->dG); dev_free(s->A);
     for (int l = 0; l < MAX_LAYERS; ++l) { dev_free(s->H[l]); dev_free(s->D[l]); }
-    dev_free(s->dZ[0]); dev_free(s->dZ[1]); dev_free(s->Bv); dev_free(s->BvT); dev_free(s->BvTs); dev_free(s->vhead); dev_free(s->head_w);
+    dev_free(s->dZ[0]); dev_free(s->dZ[1]); dev_free(s->Bv); dev_free(s->BvT); dev_free(s->BvTs); dev_free(s->BvTh); dev_free(s->amax); dev_free(s->vhead); dev_free(s->head_w);
     dev_free(s->ypart); dev_free(s->e_heads); dev_free(s->e_atom); dev_free(s->f_int); dev_free(s->f_tmp); dev_free(s->partial);
     dev_free(s->e_total); dev_free(s->flags);
     dev_free(s->stage_pos); dev_free(s->stage_f); dev_free(s->stage_e);
@@ -345,7 +362,7 @@ int gmnn_system_set_int(gmnn_system *s, const char *key, int64_t v) {
         }
         s->cap_request = (int)v;
     } else if (!strcmp(key, "mlp_precision")) {
-        if (v < 0 || v > GMNN_MLP_TF32) return GMNN_INVALID_ARG;
+        if (v < 0 || v > GMNN_MLP_3XF16) return GMNN_INVALID_ARG;
         s->mlp_precision = (int)v;
     } else if (!strcmp(key, "force_mode")) {
         if (v < 0 || v > GMNN_FORCE_PAIRBUF) return GMNN_INVALID_ARG;
@@ -364,6 +381,9 @@ int gmnn_system_set_int(gmnn_system *s, const char *key, int64_t v) {
         gmnn::g_tc_pair = v != 0;
     } else if (!strcmp(key, "tc_debug")) {  // timing experiments (wrong results), see mlp_tc.cu
         gmnn::g_tc_debug = (int)v;
+    } else if (!strcmp(key, "tc_h_bk")) {  // process-wide: K extent of a 3xFP16 stage
+        if (v != 32 && v != 64) return GMNN_INVALID_ARG;
+        gmnn::g_tc_h_bk = (int)v;
     } else if (!strcmp(key, "tc_flush_k")) {
         if (v < 16 || v > 4096 || v % 16) return GMNN_INVALID_ARG;
         gmnn::g_tc_flush_k = (int)v;

@@ -21,6 +21,8 @@ constexpr uint32_t NBR_J_MASK = (1u << NBR_J_BITS) - 1u;
 constexpr int64_t MAX_ATOMS = (int64_t)1 << NBR_J_BITS;
 constexpr int SMALL_BOX_MAX_ATOMS = 16384;
 constexpr int MAX_STAGE_EVENTS = 1 << 16;
+// device scalars of gmnn_system::amax: absolute maxima (fp32 bit patterns) of the 3xFP16 GEMM operands
+enum AmaxSlot { AMAX_G = 0, AMAX_H = 1, AMAX_DZ = AMAX_H + MAX_LAYERS, AMAX_BVT = AMAX_DZ + 2, AMAX_D, AMAX_SLOTS };
 constexpr int MAX_HEAD_SLOTS = 16;  // partial sums per atom of the head fused into the last GEMM epilogue
 constexpr int PSI = 20;  // unique monomials per channel (contraction.cuh NM)
 
@@ -71,6 +73,10 @@ struct gmnn_model {
     // (the B operands of the 3xTF32 GEMMs of mlp_tc.cu; split once here instead of per tile on chip)
     float *Ws[gmnn::MAX_LAYERS] = {};   // [2 * fan_in][fan_out]
     float *WTs[gmnn::MAX_LAYERS] = {};  // [2 * fan_out][fan_in]
+    // fp16 hi / lo split of the two scaled by a power of two (3xFP16, mlp_tc.cu), stacked the same way, and
+    // the absolute maximum of each layer's weights (fp32 bit pattern) that fixes the scale
+    uint16_t *Wh[gmnn::MAX_LAYERS] = {}, *WTh[gmnn::MAX_LAYERS] = {};
+    uint32_t *wmax = nullptr;           // [MAX_LAYERS] device
     float *b[gmnn::MAX_LAYERS] = {};
     float *scale = nullptr, *shift = nullptr;  // [S]
     float *head_mean_w = nullptr;  // [n_heads] = 1/M (device)
@@ -110,6 +116,8 @@ struct gmnn_system {
     float *Bv = nullptr;             // diag(v) W^T of the last hidden layer
     float *BvT = nullptr;            // its transpose: W diag(v), [fan_in][fan_out] (B operand of mlp_tc.cu)
     float *BvTs = nullptr;           // stacked hi / lo split of BvT
+    uint16_t *BvTh = nullptr;        // ... in fp16 (3xFP16)
+    uint32_t *amax = nullptr;        // [AMAX_SLOTS] absolute maxima of the 3xFP16 GEMM operands (see gmnn::AmaxSlot)
     float *vhead = nullptr;          // [H_last]
     float *head_w = nullptr;         // [n_heads] weights of the differentiated energy
     float *ypart = nullptr;          // [MAX_HEAD_SLOTS][N padded to 128]: partial head sums (mlp_tc.cu EPI_HIDDEN_HEAD)
@@ -155,6 +163,7 @@ int launch_pair_backward(gmnn_system *s, cudaStream_t st);  // dispatches on for
 
 // mlp_tc.cu
 int launch_split_stack(const float *src, float *dst, int64_t n, cudaStream_t st);  // dst[0..n) hi, dst[n..2n) lo
+int launch_split_stack_h(const float *src, uint16_t *dst, int64_t n, uint32_t *amax, cudaStream_t st);  // fp16, scaled by *amax
 
 // mlp_simt.cu
 int launch_mlp_forward_simt(gmnn_system *s, cudaStream_t st);

@@ -33,6 +33,7 @@
 //                 setmaxnreg moves registers from the other warps to these.
 // Activations stay fp32 in HBM, written once and read once (ncu: DRAM bytes = algorithmic bytes).
 #include <cuda.h>
+#include <cuda_fp16.h>
 
 #include "gmnn_internal.h"
 #include "tc_ptx.cuh"
@@ -84,6 +85,10 @@ struct TcArgs {
     const float *w_head;  // EPI_HIDDEN_HEAD: [N] weights of the single head
     float *ypart;         // EPI_HIDDEN_HEAD: [2 * n_tiles_n][m_pad]
     int64_t m_pad;
+    // 3xFP16: absolute maxima (fp32 bit patterns, device scalars) of A and of the fp32 matrix behind Bt;
+    // amax_out (may be null) receives the maximum of what this GEMM stores in C
+    const uint32_t *amax_a, *amax_b;
+    uint32_t *amax_out;
 };
 
 // Accumulator-flush schedule of a tile: the first two chunks span flush1 pipeline stages each, the
@@ -129,9 +134,11 @@ __device__ __forceinline__ void split_hi_lo(float4 *hi, float4 *lo, int n4, int 
 }
 
 // Fused elementwise and stores of one finished tile held in the epilogue warps' registers.
-template <int EPI>
+// SCALED (3xFP16): the accumulator is multiplied by `oscale` first, and `tmax` follows the largest
+// magnitude stored in C (the next GEMM's operand scale).
+template <int EPI, bool SCALED = false>
 __device__ __forceinline__ void tc_store_tile(const TcArgs &p, float (&acc)[4][32], int m0, int n0, int quad, int lane,
-                                              int half, int n_groups, bool row_ok) {
+                                              int half, int n_groups, bool row_ok, float oscale, float &tmax) {
     // every matrix the MLP touches is tile-transposed, [M / 128][N][128]: column c of this tile is
     // 128 consecutive floats, so each warp store / load below is one full 128-byte line
     const int64_t tbase = (int64_t)(m0 / TC_BM) * p.N * TC_BM + quad * 32 + lane;
@@ -162,7 +169,7 @@ __device__ __forceinline__ void tc_store_tile(const TcArgs &p, float (&acc)[4][3
                     wh[c] = c < nc ? __ldg(p.w_head + col0 + j0 + c) : 0.f;
                 }
 #pragma unroll
-                for (int c = 0; c < TC_EB; ++c) swish_pair_tc(acc[gi][j0 + c] + in[c], h[c], d[c]);
+                for (int c = 0; c < TC_EB; ++c) swish_pair_tc(SCALED ? fmaf(acc[gi][j0 + c], oscale, in[c]) : acc[gi][j0 + c] + in[c], h[c], d[c]);
 #pragma unroll
                 for (int c = 0; c < TC_EB; ++c)
                     if (c < nc) {
@@ -173,23 +180,28 @@ __device__ __forceinline__ void tc_store_tile(const TcArgs &p, float (&acc)[4][3
 #pragma unroll
                 for (int c = 0; c < TC_EB; ++c) in[c] = c < nc ? __ldg(bias + col0 + j0 + c) : 0.f;
 #pragma unroll
-                for (int c = 0; c < TC_EB; ++c) swish_pair_tc(acc[gi][j0 + c] + in[c], h[c], d[c]);
+                for (int c = 0; c < TC_EB; ++c) swish_pair_tc(SCALED ? fmaf(acc[gi][j0 + c], oscale, in[c]) : acc[gi][j0 + c] + in[c], h[c], d[c]);
 #pragma unroll
                 for (int c = 0; c < TC_EB; ++c)
                     if (c < nc) {
                         Cout[o + c * TC_BM] = h[c];
                         C2out[o + c * TC_BM] = d[c];
+                        if (SCALED) tmax = fmaxf(tmax, fabsf(h[c]));
                     }
             } else if (EPI == EPI_MUL) {
 #pragma unroll
                 for (int c = 0; c < TC_EB; ++c) in[c] = c < nc ? __ldg(Dmul + o + c * TC_BM) : 0.f;
 #pragma unroll
                 for (int c = 0; c < TC_EB; ++c)
-                    if (c < nc) Cout[o + c * TC_BM] = acc[gi][j0 + c] * in[c];
+                    if (c < nc) {
+                        const float v = (SCALED ? acc[gi][j0 + c] * oscale : acc[gi][j0 + c]) * in[c];
+                        Cout[o + c * TC_BM] = v;
+                        if (SCALED) tmax = fmaxf(tmax, fabsf(v));
+                    }
             } else {
 #pragma unroll
                 for (int c = 0; c < TC_EB; ++c)
-                    if (c < nc) Cout[o + c * TC_BM] = acc[gi][j0 + c];
+                    if (c < nc) Cout[o + c * TC_BM] = SCALED ? acc[gi][j0 + c] * oscale : acc[gi][j0 + c];
             }
         }
     }
@@ -361,7 +373,8 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
                 __syncwarp();
                 if (lane == 0) mbar_arrive(bar_tempty(a));
             }
-            tc_store_tile<EPI>(p, acc, m0, n0, quad, lane, half, n_groups, row_ok);
+            float unused = 0.f;
+            tc_store_tile<EPI>(p, acc, m0, n0, quad, lane, half, n_groups, row_ok, 1.f, unused);
         }
     }
 
@@ -380,25 +393,78 @@ static int tc_num_sms();
 // read by the tensor core, which is what bounds the single-CTA kernel (shared-memory bandwidth).
 // Hand-shakes across the pair: split-done and accumulator-drained arrivals go to the leader's
 // barriers (mapa + remote arrive); the leader's tcgen05.commit multicasts to both CTAs' barriers.
-template <int BK>
+// F16 = true is the 3xFP16 mode (GMNN_MLP_3XF16): the same three-product split on kind::f16, whose
+// MMAs run at twice the tf32 rate on half the operand bytes.  a' = a * 2^s with 2^14 <= max |a'| < 2^15
+// (s from the matrix's absolute maximum, a device scalar the producing kernel left), hi = fp16(a'),
+// lo = fp16(a' - hi): 22 significand bits like the tf32 split; elements below 2^-18 of the maximum lose
+// relative (not absolute: <= 2^-40 of the maximum) accuracy to the fp16 exponent range.  The splitter
+// warps read the fp32 A tile where TMA landed it ([BK][128 atoms], not swizzled) and write hi / lo as
+// K-major fp16 rows in the 128- or 64-byte swizzle; B arrives split and scaled (model->Wh / WTh).  The
+// epilogue multiplies the accumulator by 2^-(s_a + s_b).
+template <bool F16, int BK>
 struct TcPairCfg {
-    static constexpr int A_BYTES = TC_BM * BK * 4;
-    static constexpr int B_BYTES = (TC_BN_MAX / 2) * BK * 4;       // this CTA's half of the B tile
-    static constexpr int STAGE_BYTES = 2 * (A_BYTES + B_BYTES);    // hi and lo of both
+    static constexpr int ES = F16 ? 2 : 4;                          // operand element size
+    static constexpr int ROWB = BK * ES;                            // bytes per K-major operand row = swizzle span
+    static constexpr int LAND_BYTES = F16 ? BK * TC_BM * 4 : 0;     // fp32 landing area of the A tile
+    static constexpr int A_BYTES = TC_BM * BK * ES;
+    static constexpr int B_BYTES = (TC_BN_MAX / 2) * BK * ES;       // this CTA's half of the B tile
+    static constexpr int STAGE_BYTES = LAND_BYTES + 2 * (A_BYTES + B_BYTES);  // hi and lo of both
     static constexpr int NST = TC_STAGE_BYTES_TOTAL / STAGE_BYTES;
     static constexpr int SMEM_BYTES = NST * STAGE_BYTES + 1024 + 512;
+    static constexpr int KSTEP = 32 / ES;                           // K per MMA instruction
     static_assert(NST >= 2, "pipeline needs at least two stages");
 };
 
-template <int BK, int EPI>
+// 2^e for the fp16 split: e = 14 - floor(log2(amax)), clamped so that all scales stay normal numbers
+__device__ __forceinline__ int amax_exponent(uint32_t bits) {
+    int e = bits ? (int)(bits >> 23) - 127 : 0;
+    return e < -40 ? -40 : (e > 40 ? 40 : e);
+}
+__device__ __forceinline__ float pow2i(int e) { return __int_as_float((127 + e) << 23); }
+
+// fp32 A tile [BK][128] -> hi / lo fp16 rows (K-major, swizzled), one atom (row) per thread.
+template <int BK>
+__device__ __forceinline__ void split_f16_tile(const float *__restrict__ land, uint8_t *__restrict__ hi, uint8_t *__restrict__ lo,
+                                               int m, float scale, int k_valid) {
+    constexpr int ROWB = BK * 2;
+#pragma unroll
+    for (int c0 = 0; c0 < BK / 8; c0 += 4) {
+        float x[4][8];
+#pragma unroll
+        for (int c = 0; c < 4; ++c)
+#pragma unroll
+            for (int k = 0; k < 8; ++k) x[c][k] = land[((c0 + c) * 8 + k) * TC_BM + m];
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            uint32_t h[4], l[4];
+            const bool ok = (c0 + c) * 8 < k_valid;  // K is a multiple of 8: a chunk is whole or absent
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const float a = ok ? x[c][2 * q] * scale : 0.f, b = ok ? x[c][2 * q + 1] * scale : 0.f;
+                const __half2 hh = __floats2half2_rn(a, b);
+                const float2 hf = __half22float2(hh);
+                const __half2 ll = __floats2half2_rn(a - hf.x, b - hf.y);
+                h[q] = *reinterpret_cast<const uint32_t *>(&hh);
+                l[q] = *reinterpret_cast<const uint32_t *>(&ll);
+            }
+            uint32_t o = (uint32_t)(m * ROWB + (c0 + c) * 16);
+            o ^= ((o >> 7) & (uint32_t)(ROWB / 16 - 1)) << 4;  // 128- / 64-byte swizzle of the 16-byte chunk index
+            *reinterpret_cast<uint4 *>(hi + o) = make_uint4(h[0], h[1], h[2], h[3]);
+            *reinterpret_cast<uint4 *>(lo + o) = make_uint4(l[0], l[1], l[2], l[3]);
+        }
+    }
+}
+
+template <bool F16, int BK, int EPI>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(TC_THREADS, 1)
 k_gemm_tc_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const TcArgs p) {
-    using Cfg = TcPairCfg<BK>;
+    using Cfg = TcPairCfg<F16, BK>;
     constexpr int NST = Cfg::NST;
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;  // identical offset in both CTAs
     uint8_t *smem_gen = smem_raw + (smem_base - smem_u32(smem_raw));
-    auto a_hi = [&](int s) { return smem_base + (uint32_t)s * Cfg::STAGE_BYTES; };
+    // stage: [fp32 A landing (F16) | A_hi | A_lo | B_hi | B_lo]
+    auto a_hi = [&](int s) { return smem_base + (uint32_t)s * Cfg::STAGE_BYTES + Cfg::LAND_BYTES; };
     auto a_lo = [&](int s) { return a_hi(s) + Cfg::A_BYTES; };
     auto b_hi = [&](int s) { return a_hi(s) + 2 * Cfg::A_BYTES; };
     auto b_lo = [&](int s) { return b_hi(s) + Cfg::B_BYTES; };
@@ -441,7 +507,7 @@ k_gemm_tc_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
         setmaxnreg_dec<TC_REGS_CONTROL>();
         if (warp == 0 && lane == 0) {
             // ===== TMA producer: own A rows, own half of B =====
-            const uint32_t tx = (uint32_t)(Cfg::A_BYTES + 2 * hb * BK * 4);
+            const uint32_t tx = (uint32_t)(TC_BM * BK * 4 + 2 * hb * BK * Cfg::ES);
             uint32_t it = 0;
             for (int t = pair; t < p.n_tiles; t += n_pairs) {
                 const int mt = 2 * (t / p.n_tiles_n) + (int)rank, n0 = (t % p.n_tiles_n) * p.bn;
@@ -449,15 +515,19 @@ k_gemm_tc_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                     const int s = it % NST;
                     mbar_wait(bar_empty(s), ((it / NST) & 1) ^ 1);
                     mbar_arrive_expect_tx(bar_full(s), tx);
-                    for (int q = 0; q < 4; ++q)
-                        tma_load_2d(a_hi(s) + q * (BK * 128), &tmA, bar_full(s), q * 32, mt * p.K + kb * BK);
+                    if (F16) {
+                        tma_load_2d(a_hi(s) - Cfg::LAND_BYTES, &tmA, bar_full(s), 0, mt * p.K + kb * BK);  // [BK][128] fp32
+                    } else {
+                        for (int q = 0; q < 4; ++q)
+                            tma_load_2d(a_hi(s) + q * (BK * 128), &tmA, bar_full(s), q * 32, mt * p.K + kb * BK);
+                    }
                     tma_load_2d(b_hi(s), &tmB, bar_full(s), kb * BK, n0 + (int)rank * hb);
                     tma_load_2d(b_lo(s), &tmB, bar_full(s), kb * BK, p.N + n0 + (int)rank * hb);  // lo rows follow the hi rows
                 }
             }
         } else if (warp == 1 && lane == 0 && rank == 0) {
             // ===== MMA issuer (leader CTA only) =====
-            const uint32_t idesc = make_idesc_tf32(2 * TC_BM, p.bn, true);
+            const uint32_t idesc = F16 ? make_idesc_f16(2 * TC_BM, p.bn) : make_idesc_tf32(2 * TC_BM, p.bn, true);
             uint32_t it = 0, chunk = 0;
             for (int t = pair; t < p.n_tiles; t += n_pairs) {
                 for (int kb = 0; kb < nkb; ++kb, ++it) {
@@ -473,19 +543,28 @@ k_gemm_tc_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                     mbar_wait(bar_split(s), (it / NST) & 1);
                     tcgen05_fence_after();
                     const int krem = p.K - kb * BK;
-                    const int ksteps = krem >= BK ? BK / 8 : (krem + 7) / 8;
-                    const uint64_t da_hi = make_smem_desc_mn128(a_hi(s), BK * 128), db_hi = make_smem_desc<BK * 4>(b_hi(s));
-                    const uint64_t da_lo = make_smem_desc_mn128(a_lo(s), BK * 128), db_lo = make_smem_desc<BK * 4>(b_lo(s));
+                    const int ksteps = krem >= BK ? BK / Cfg::KSTEP : (krem + Cfg::KSTEP - 1) / Cfg::KSTEP;
+                    const uint64_t db_hi = make_smem_desc<Cfg::ROWB>(b_hi(s)), db_lo = make_smem_desc<Cfg::ROWB>(b_lo(s));
+                    const uint64_t da_hi = F16 ? make_smem_desc<Cfg::ROWB>(a_hi(s)) : make_smem_desc_mn128(a_hi(s), BK * 128);
+                    const uint64_t da_lo = F16 ? make_smem_desc<Cfg::ROWB>(a_lo(s)) : make_smem_desc_mn128(a_lo(s), BK * 128);
+                    // per k step: B (and a K-major A) advance 32 bytes along the row, the MN-major A one 1024-byte atom
+                    const uint64_t astep = F16 ? 2 : 64;
                     uint32_t acc = !chunk_first;
                     for (int k = 0; k < ksteps; ++k) {  // small cross terms first
-                        const uint64_t koff = (uint64_t)((k * 32) >> 4), aoff = (uint64_t)((k * 1024) >> 4);
-                        mma_tf32_ss_pair(d_tmem, da_lo + aoff, db_hi + koff, idesc, acc);
-                        mma_tf32_ss_pair(d_tmem, da_hi + aoff, db_lo + koff, idesc, 1u);
+                        const uint64_t koff = (uint64_t)(2 * k), aoff = astep * k;
+                        if (F16) {
+                            mma_f16_ss_pair(d_tmem, da_lo + aoff, db_hi + koff, idesc, acc);
+                            mma_f16_ss_pair(d_tmem, da_hi + aoff, db_lo + koff, idesc, 1u);
+                        } else {
+                            mma_tf32_ss_pair(d_tmem, da_lo + aoff, db_hi + koff, idesc, acc);
+                            mma_tf32_ss_pair(d_tmem, da_hi + aoff, db_lo + koff, idesc, 1u);
+                        }
                         acc = 1u;
                     }
                     for (int k = 0; k < ksteps; ++k) {
-                        const uint64_t koff = (uint64_t)((k * 32) >> 4), aoff = (uint64_t)((k * 1024) >> 4);
-                        mma_tf32_ss_pair(d_tmem, da_hi + aoff, db_hi + koff, idesc, 1u);
+                        const uint64_t koff = (uint64_t)(2 * k), aoff = astep * k;
+                        if (F16) mma_f16_ss_pair(d_tmem, da_hi + aoff, db_hi + koff, idesc, 1u);
+                        else mma_tf32_ss_pair(d_tmem, da_hi + aoff, db_hi + koff, idesc, 1u);
                     }
                     mma_commit_pair(bar_empty(s), 3);
                     if (chunk_last) {
@@ -497,17 +576,22 @@ k_gemm_tc_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
         }
     } else if (warp < TC_FIRST_EPI_WARP) {
         setmaxnreg_dec<TC_REGS_SPLIT>();
-        // ===== splitters: own A tile and own half of B, hi in place, lo beside it =====
+        // ===== splitters: own A tile into hi and lo (B arrives split: model->Ws / WTs / Wh / WTh) =====
         const int tid = threadIdx.x - TC_FIRST_SPLIT_WARP * 32;
-        const int n_a4 = Cfg::A_BYTES / 16;
+        const float ascale = F16 ? pow2i(14 - amax_exponent(*p.amax_a)) : 1.f;
         uint32_t it = 0;
         for (int t = pair; t < p.n_tiles; t += n_pairs) {
             for (int kb = 0; kb < nkb; ++kb, ++it) {
                 const int s = it % NST;
                 mbar_wait(bar_full(s), (it / NST) & 1);
-                float4 *ah = reinterpret_cast<float4 *>(smem_gen + (size_t)s * Cfg::STAGE_BYTES);
-                float4 *al = ah + Cfg::A_BYTES / 16;
-                split_hi_lo(ah, al, n_a4, tid);  // B arrives split (model->Ws / WTs)
+                uint8_t *stage = smem_gen + (size_t)s * Cfg::STAGE_BYTES;
+                if (F16) {
+                    split_f16_tile<BK>(reinterpret_cast<const float *>(stage), stage + Cfg::LAND_BYTES,
+                                       stage + Cfg::LAND_BYTES + Cfg::A_BYTES, tid, ascale, p.K - kb * BK);
+                } else {
+                    float4 *ah = reinterpret_cast<float4 *>(stage);
+                    split_hi_lo(ah, ah + Cfg::A_BYTES / 16, Cfg::A_BYTES / 16, tid);
+                }
                 fence_proxy_async_all();
                 __syncwarp();
                 if (lane == 0) mbar_arrive_cluster(bar_split(s), 0);
@@ -521,6 +605,8 @@ k_gemm_tc_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
         const int n_groups = (p.bn + 31) / 32;
         const int n_chunks = chunk_count(p, nkb);
         const uint32_t lane_base = tmem_base + ((uint32_t)(quad * 32) << 16);
+        const float oscale = F16 ? pow2i(amax_exponent(*p.amax_a) + amax_exponent(*p.amax_b) - 28) : 1.f;
+        float tmax = 0.f;
         uint32_t chunk = 0;
         for (int t = pair; t < p.n_tiles; t += n_pairs) {
             const int m0 = (2 * (t / p.n_tiles_n) + (int)rank) * TC_BM, n0 = (t % p.n_tiles_n) * p.bn;
@@ -550,7 +636,12 @@ k_gemm_tc_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                 __syncwarp();
                 if (lane == 0) mbar_arrive_cluster(bar_tempty(a), 0);
             }
-            tc_store_tile<EPI>(p, acc, m0, n0, quad, lane, half, n_groups, row_ok);
+            tc_store_tile<EPI, F16>(p, acc, m0, n0, quad, lane, half, n_groups, row_ok, oscale, tmax);
+        }
+        if (F16 && p.amax_out && (EPI == EPI_HIDDEN || EPI == EPI_MUL)) {
+#pragma unroll
+            for (int o = 16; o >= 1; o >>= 1) tmax = fmaxf(tmax, __shfl_xor_sync(0xffffffffu, tmax, o));
+            if (lane == 0) atomicMax(p.amax_out, __float_as_uint(tmax));
         }
     }
 
@@ -559,16 +650,16 @@ k_gemm_tc_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     if (warp == 1) tmem_dealloc_pair<512>(tmem_base);
 }
 
-template <int BK, int EPI>
+template <bool F16, int BK, int EPI>
 static int tc_launch_pair(const CUtensorMap &tmA, const CUtensorMap &tmB, const TcArgs &args, cudaStream_t st) {
-    using Cfg = TcPairCfg<BK>;
+    using Cfg = TcPairCfg<F16, BK>;
     static bool attr_set = false;
     if (!attr_set) {
-        GMNN_CUDA(cudaFuncSetAttribute(k_gemm_tc_pair<BK, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES));
+        GMNN_CUDA(cudaFuncSetAttribute(k_gemm_tc_pair<F16, BK, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES));
         attr_set = true;
     }
     int grid = 2 * args.n_tiles < tc_num_sms() ? 2 * args.n_tiles : (tc_num_sms() & ~1);
-    k_gemm_tc_pair<BK, EPI><<<grid, TC_THREADS, Cfg::SMEM_BYTES, st>>>(tmA, tmB, args);
+    k_gemm_tc_pair<F16, BK, EPI><<<grid, TC_THREADS, Cfg::SMEM_BYTES, st>>>(tmA, tmB, args);
     GMNN_LAUNCHED();
     GMNN_CUDA(cudaGetLastError());
     return GMNN_OK;
@@ -678,19 +769,73 @@ static int tc_launch(const CUtensorMap &tmA, const CUtensorMap &tmB, const TcArg
 int g_tc_pair = 1;    // knob "tc_pair": 3xTF32 GEMMs on CTA pairs (cta_group::2)
 int g_tc_flush_head = 2;  // knob "tc_flush_head": first-two-chunks multiplier of the backward GEMMs (forces only)
 int g_tc_debug = 0;
-int g_tc_flush_k = 64;   // knob "tc_flush_k": K extent between accumulator flushes of the 3xTF32 mode
+int g_tc_flush_k = 64;   // knob "tc_flush_k": K extent between accumulator flushes of the 3xTF32 / 3xFP16 modes
 int g_tc_split_bk = 32;  // knob (gmnn_system_set_int "tc_split_bk"): K extent of a 3xTF32 stage, 16 or 32
+int g_tc_h_bk = 64;      // knob "tc_h_bk": K extent of a 3xFP16 stage, 32 or 64
+
+// fp16 row-major [rows][K] matrix (the stacked hi / lo weights), box = box_rows x BK, swizzle span = BK * 2 bytes.
+static int make_tmap_h(CUtensorMap *tm, const uint16_t *base, int64_t rows, int K, int box_rows, int BK) {
+    PFN_encodeTiled enc = get_encode();
+    if (!enc) {
+        set_error("cuTensorMapEncodeTiled is not available from the driver");
+        return GMNN_CUDA_ERROR;
+    }
+    const cuuint64_t dims[2] = {(cuuint64_t)K, (cuuint64_t)rows};
+    const cuuint64_t strides[1] = {(cuuint64_t)K * 2};
+    const cuuint32_t box[2] = {(cuuint32_t)BK, (cuuint32_t)box_rows};
+    const cuuint32_t estr[2] = {1, 1};
+    const CUtensorMapSwizzle sw = BK == 64 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_64B;
+    const CUresult r = enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2, const_cast<uint16_t *>(base), dims, strides, box, estr,
+                           CU_TENSOR_MAP_INTERLEAVE_NONE, sw, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        set_error("cuTensorMapEncodeTiled failed (%d) for a fp16 [%lld][%d] matrix", (int)r, (long long)rows, K);
+        return GMNN_CUDA_ERROR;
+    }
+    return GMNN_OK;
+}
+
+// Tile-transposed activations as whole [BK][128] fp32 boxes, not swizzled (3xFP16: the splitter warps
+// read them, the tensor core does not).
+static int make_tmap_a_land(CUtensorMap *tm, const float *base, int64_t M, int K, int BK) {
+    PFN_encodeTiled enc = get_encode();
+    if (!enc) {
+        set_error("cuTensorMapEncodeTiled is not available from the driver");
+        return GMNN_CUDA_ERROR;
+    }
+    const int64_t tiles = (M + TC_BM - 1) / TC_BM;
+    const cuuint64_t dims[2] = {(cuuint64_t)TC_BM, (cuuint64_t)(tiles * K)};
+    const cuuint64_t strides[1] = {(cuuint64_t)TC_BM * 4};
+    const cuuint32_t box[2] = {(cuuint32_t)TC_BM, (cuuint32_t)BK};
+    const cuuint32_t estr[2] = {1, 1};
+    const CUresult r = enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float *>(base), dims, strides, box, estr,
+                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        set_error("cuTensorMapEncodeTiled failed (%d) for a tile-transposed [%lld][%d] matrix (fp32 boxes)", (int)r, (long long)M, K);
+        return GMNN_CUDA_ERROR;
+    }
+    return GMNN_OK;
+}
+
+// 3xFP16 operands of one GEMM: stacked fp16 hi / lo weights and the absolute-maximum scalars (see TcArgs)
+struct TcHalf {
+    const uint16_t *Bh = nullptr;
+    const uint32_t *amax_a = nullptr, *amax_b = nullptr;
+    uint32_t *amax_out = nullptr;
+};
 
 // C[M][N] = A[M][K] . Bt[N][K]^T.  A, C, C2, Dmul are tile-transposed ([M/128][cols][128], padded to whole
-// tiles); Bt (weights) is row-major [N][K], or for split = true the stacked hi / lo split [2N][K].
+// tiles); Bt (weights) is row-major [N][K], or for split = true the stacked hi / lo split [2N][K]; with
+// `hf` (3xFP16, always on CTA pairs) the fp16 split hf->Bh replaces Bt.
 int tc_gemm(bool split, int epi, int64_t M, int N, int K, const float *A, const float *Bt, float *C, const float *bias,
             float *C2, const float *Dmul, cudaStream_t st, const float *w_head = nullptr, float *ypart = nullptr,
-            int *n_slots = nullptr) {
+            int *n_slots = nullptr, const TcHalf *hf = nullptr) {
     if (K % 8 != 0 || N % 8 != 0 || M <= 0 || M > INT32_MAX) {
         set_error("tensor-core MLP: widths must be multiples of 8 (K = %d, N = %d)", K, N);
         return GMNN_UNSUPPORTED;
     }
-    const int BK = split ? g_tc_split_bk : 32;
+    const int BK = hf ? g_tc_h_bk : (split ? g_tc_split_bk : 32);
     TcArgs a;
     a.M = (int)M, a.N = N, a.K = K;
     a.bn = pick_bn(N);
@@ -701,9 +846,24 @@ int tc_gemm(bool split, int epi, int64_t M, int N, int K, const float *A, const 
     a.debug = g_tc_debug;
     a.C = C, a.C2 = C2, a.bias = bias, a.Dmul = Dmul;
     a.w_head = w_head, a.ypart = ypart, a.m_pad = (M + TC_BM - 1) / TC_BM * TC_BM;
+    a.amax_a = hf ? hf->amax_a : nullptr, a.amax_b = hf ? hf->amax_b : nullptr, a.amax_out = hf ? hf->amax_out : nullptr;
     if (n_slots) *n_slots = 2 * a.n_tiles_n;
     CUtensorMap tmA, tmB;
     int rc;
+#define TC_PAIR_CASE(F16V, BKV)                                                                       \
+    switch (epi) {                                                                                    \
+        case EPI_PLAIN: return tc_launch_pair<F16V, BKV, EPI_PLAIN>(tmA, tmB, a, st);                  \
+        case EPI_HIDDEN: return tc_launch_pair<F16V, BKV, EPI_HIDDEN>(tmA, tmB, a, st);                \
+        case EPI_HIDDEN_HEAD: return tc_launch_pair<F16V, BKV, EPI_HIDDEN_HEAD>(tmA, tmB, a, st);      \
+        default: return tc_launch_pair<F16V, BKV, EPI_MUL>(tmA, tmB, a, st);                           \
+    }
+    if (hf) {
+        a.n_tiles = (int)(((M + TC_BM - 1) / TC_BM + 1) / 2) * a.n_tiles_n;
+        if ((rc = make_tmap_a_land(&tmA, A, M, K, BK))) return rc;
+        if ((rc = make_tmap_h(&tmB, hf->Bh, 2 * (int64_t)N, K, a.bn / 2, BK))) return rc;
+        if (BK == 64) { TC_PAIR_CASE(true, 64) }
+        TC_PAIR_CASE(true, 32)
+    }
     if ((rc = make_tmap_a(&tmA, A, M, K, BK))) return rc;
     if ((rc = make_tmap(&tmB, Bt, split ? 2 * (int64_t)N : N, K, a.bn, BK))) return rc;
 #define TC_CASE(SP, BKV)                                                                  \
@@ -717,25 +877,46 @@ int tc_gemm(bool split, int epi, int64_t M, int N, int K, const float *A, const 
         // pair tiles: two adjacent 128-row tiles x one column tile; B box = this CTA's half of the columns
         a.n_tiles = (int)(((M + TC_BM - 1) / TC_BM + 1) / 2) * a.n_tiles_n;
         if ((rc = make_tmap(&tmB, Bt, 2 * (int64_t)N, K, a.bn / 2, BK))) return rc;
-        if (BK == 32) {
-            switch (epi) {
-                case EPI_PLAIN: return tc_launch_pair<32, EPI_PLAIN>(tmA, tmB, a, st);
-                case EPI_HIDDEN: return tc_launch_pair<32, EPI_HIDDEN>(tmA, tmB, a, st);
-                case EPI_HIDDEN_HEAD: return tc_launch_pair<32, EPI_HIDDEN_HEAD>(tmA, tmB, a, st);
-                default: return tc_launch_pair<32, EPI_MUL>(tmA, tmB, a, st);
-            }
-        }
-        switch (epi) {
-            case EPI_PLAIN: return tc_launch_pair<16, EPI_PLAIN>(tmA, tmB, a, st);
-            case EPI_HIDDEN: return tc_launch_pair<16, EPI_HIDDEN>(tmA, tmB, a, st);
-            case EPI_HIDDEN_HEAD: return tc_launch_pair<16, EPI_HIDDEN_HEAD>(tmA, tmB, a, st);
-            default: return tc_launch_pair<16, EPI_MUL>(tmA, tmB, a, st);
-        }
+        if (BK == 32) { TC_PAIR_CASE(false, 32) }
+        TC_PAIR_CASE(false, 16)
     }
     if (!split) { TC_CASE(false, 32) }
     if (BK == 32) { TC_CASE(true, 32) }
     TC_CASE(true, 16)
 #undef TC_CASE
+#undef TC_PAIR_CASE
+}
+
+// ---- operand preparation ----------------------------------------------------------------------
+__global__ void k_absmax(const float *__restrict__ src, int64_t n, uint32_t *__restrict__ amax) {
+    float m = 0.f;
+    for (int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; t < n; t += (int64_t)gridDim.x * blockDim.x)
+        m = fmaxf(m, fabsf(src[t]));
+#pragma unroll
+    for (int o = 16; o >= 1; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if ((threadIdx.x & 31) == 0 && m > 0.f) atomicMax(amax, __float_as_uint(m));
+}
+
+// dst[0, n) = fp16(src * 2^s), dst[n, 2n) = fp16(src * 2^s - hi), 2^s from *amax (the 3xFP16 B operand)
+__global__ void k_split_stack_h(const float *__restrict__ src, __half *__restrict__ dst, int64_t n,
+                                const uint32_t *__restrict__ amax) {
+    const int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (t >= n) return;
+    const float v = src[t] * pow2i(14 - amax_exponent(*amax));
+    const __half h = __float2half_rn(v);
+    dst[t] = h;
+    dst[n + t] = __float2half_rn(v - __half2float(h));
+}
+
+// *amax = max |src| (reset first), then the stacked fp16 split
+int launch_split_stack_h(const float *src, uint16_t *dst, int64_t n, uint32_t *amax, cudaStream_t st) {
+    GMNN_CUDA(cudaMemsetAsync(amax, 0, sizeof(uint32_t), st));
+    k_absmax<<<(unsigned)((n + 1023) / 1024 < 256 ? (n + 1023) / 1024 : 256), 256, 0, st>>>(src, n, amax);
+    GMNN_LAUNCHED();
+    k_split_stack_h<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(src, reinterpret_cast<__half *>(dst), n, amax);
+    GMNN_LAUNCHED();
+    GMNN_CUDA(cudaGetLastError());
+    return GMNN_OK;
 }
 
 __global__ void k_split_stack(const float *__restrict__ src, float *__restrict__ dst, int64_t n) {
@@ -755,16 +936,20 @@ int launch_split_stack(const float *src, float *dst, int64_t n, cudaStream_t st)
 
 int launch_mlp_forward_tc(gmnn_system *s, cudaStream_t st) {
     const gmnn_model *m = s->model;
-    const bool split = s->mlp_precision == GMNN_MLP_3XTF32;
+    const bool f16 = s->mlp_precision == GMNN_MLP_3XF16;
+    const bool split = s->mlp_precision == GMNN_MLP_3XTF32 || f16;
     const float *X = s->G;
     for (int l = 0; l < m->hp.n_hidden; ++l) {
         // z = X W[l]: the B operand is W[l]^T = WT[l], [fan_out][fan_in]
         // single head: the last hidden layer's epilogue takes the head's dot product itself
         const bool fuse = l == m->hp.n_hidden - 1 && m->hp.n_heads == 1 && 2 * ((m->dims[l + 1] + 127) / 128) <= MAX_HEAD_SLOTS;
         s->heads_fused = fuse;
+        TcHalf hf;
+        hf.Bh = m->WTh[l], hf.amax_b = m->wmax + l;
+        hf.amax_a = s->amax + (l == 0 ? AMAX_G : AMAX_H + l - 1), hf.amax_out = s->amax + AMAX_H + l;
         int rc = tc_gemm(split, fuse ? EPI_HIDDEN_HEAD : EPI_HIDDEN, s->N, m->dims[l + 1], m->dims[l], X,
                          split ? m->WTs[l] : m->WT[l], s->H[l], m->b[l], s->D[l], nullptr, st, m->W[l + 1], s->ypart,
-                         &s->head_slots);
+                         &s->head_slots, f16 ? &hf : nullptr);
         if (rc) return rc;
         X = s->H[l];
     }
@@ -775,23 +960,36 @@ int launch_mlp_forward_tc(gmnn_system *s, cudaStream_t st) {
 // Bop = WT[l-1] gives W[l-1]; Bop = diag(v) WT[L-1] gives W[L-1] diag(v) = BvT.
 int launch_mlp_backward_tc(gmnn_system *s, const float *head_w_dev, cudaStream_t st) {
     const gmnn_model *m = s->model;
-    const bool split = s->mlp_precision == GMNN_MLP_3XTF32;
+    const bool f16 = s->mlp_precision == GMNN_MLP_3XF16;
+    const bool split = s->mlp_precision == GMNN_MLP_3XTF32 || f16;
     const int L = m->hp.n_hidden;
     int rc = launch_mlp_seed(s, head_w_dev, st);  // vhead, Bv (and BvT, see mlp_simt.cu)
     if (rc) return rc;
     const float *Aop = s->D[L - 1];
-    if (split && (rc = launch_split_stack(s->BvT, s->BvTs, (int64_t)m->dims[L] * m->dims[L - 1], st))) return rc;
+    const int64_t nbv = (int64_t)m->dims[L] * m->dims[L - 1];
+    if (f16) {
+        if ((rc = launch_split_stack_h(s->BvT, s->BvTh, nbv, s->amax + AMAX_BVT, st))) return rc;
+    } else if (split && (rc = launch_split_stack(s->BvT, s->BvTs, nbv, st))) {
+        return rc;
+    }
     const float *BopT = split ? s->BvTs : s->BvT;
+    TcHalf hf;
+    hf.Bh = s->BvTh, hf.amax_b = s->amax + AMAX_BVT, hf.amax_a = s->amax + AMAX_D;  // A = swish' of the last hidden layer
     int cur = 0;
     for (int l = L - 1; l >= 0; --l) {
         if (l > 0) {
-            rc = tc_gemm(split, EPI_MUL, s->N, m->dims[l], m->dims[l + 1], Aop, BopT, s->dZ[cur], nullptr, nullptr, s->D[l - 1], st);
+            hf.amax_out = s->amax + AMAX_DZ + cur;
+            rc = tc_gemm(split, EPI_MUL, s->N, m->dims[l], m->dims[l + 1], Aop, BopT, s->dZ[cur], nullptr, nullptr, s->D[l - 1], st,
+                         nullptr, nullptr, nullptr, f16 ? &hf : nullptr);
             if (rc) return rc;
             Aop = s->dZ[cur];
             BopT = split ? m->Ws[l - 1] : m->W[l - 1];
+            hf.Bh = m->Wh[l - 1], hf.amax_b = m->wmax + l - 1, hf.amax_a = s->amax + AMAX_DZ + cur;
             cur ^= 1;
         } else {
-            rc = tc_gemm(split, EPI_PLAIN, s->N, m->dims[0], m->dims[1], Aop, BopT, s->dG, nullptr, nullptr, nullptr, st);
+            hf.amax_out = nullptr;
+            rc = tc_gemm(split, EPI_PLAIN, s->N, m->dims[0], m->dims[1], Aop, BopT, s->dG, nullptr, nullptr, nullptr, st,
+                         nullptr, nullptr, nullptr, f16 ? &hf : nullptr);
             if (rc) return rc;
         }
     }

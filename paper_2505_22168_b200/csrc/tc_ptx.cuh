@@ -192,6 +192,20 @@ __device__ __forceinline__ void mma_commit_pair(uint32_t bar, uint16_t mask) {
                  : "memory");
 }
 
+// ---- kind::f16 (fp16 operands, fp32 accumulate; K = 16 per instruction, twice the tf32 rate) -------
+// Instruction descriptor: F16 x F16 -> F32, dense, both operands K-major.
+__host__ __device__ constexpr uint32_t make_idesc_f16(int M, int N) {
+    return (1u << 4) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
+}
+__device__ __forceinline__ void mma_f16_ss_pair(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n\t}"
+        ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+
 // Warpgroup-wide register reallocation (all four warps of the warpgroup execute it).
 template <int NREG>
 __device__ __forceinline__ void setmaxnreg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(NREG)); }
