@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- atom-steps/s of the GMNN energy+force hot path on B200 (BASELINE.json `metric`).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload config5] [--mlp 3xtf32]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload config5] [--mlp 3xf16]
     python bench.py --impl reference ...          # the fp64 CPU oracle on the host cores
 
 One "step" is one NVE velocity-Verlet step of the workload through gmnn_md_verlet_steps: kick,
@@ -35,7 +35,9 @@ import numpy as np  # noqa: E402
 METRIC = "atom-steps/s (GMNN energy+forces)"
 UNIT = "atom-steps/s"
 N_FEATURES = 360
-MLP_NAMES = {"fp32": 0, "3xtf32": 1, "tf32": 2}
+# ncu --set full, config5, sum over the four GEMM launches of one step (profiles/ncu_r1_gemm_tc_pair.md, ncu_r1_gemm_f16.md)
+NCU_GEMM_DRAM_BYTES_PER_STEP = {"3xtf32": 20.43e9}
+MLP_NAMES = {"fp32": 0, "3xtf32": 1, "tf32": 2, "3xf16": 3}
 FP32_LANES_PER_SM = 128  # B200_PROFILING.md / B300_MICROARCH.md: 4 SMSPs x 32 FMA lanes
 N_SMS = 148
 
@@ -327,7 +329,8 @@ def run_ours(args):
     sm = stage_model(w, nl_mean, nc_mean, hidden_macs, args.mlp, args.forces)
     sm_mhz = clocks.get("sm_mhz") or peaks["sm_max_mhz"]
     fp32_peak_tflops = N_SMS * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
-    tf32_peak_tflops = 0.5 * peaks["bf16_sustained"]
+    # tensor peak of the MLP's operand type: fp16 = the measured bf16 figure, tf32 = half of it (nominal ratio)
+    tf32_peak_tflops = (1.0 if args.mlp == "3xf16" else 0.5) * peaks["bf16_sustained"]
     stage_out = {}
     per_step_ms = {}
     for name, mean_ms, cnt in stages:
@@ -360,7 +363,8 @@ def run_ours(args):
         roofline = {"kernel": dom, "bound": info["bound"], "achieved": round(ach, 3), "peak": round(peak, 3),
                     "unit": unit, "frac": round(ach / peak, 4), "traffic": None,
                     "peak_source": {"hbm": "MEASURED_PEAKS.json hbm_gbs (%s)" % peaks["source"],
-                                    "tensor": "0.5 (nominal tf32:bf16) x bf16_tflops_sustained (%s)" % peaks["source"],
+                                    "tensor": ("bf16_tflops_sustained (%s); fp16 runs at the bf16 rate" if args.mlp == "3xf16" else
+                                               "0.5 (nominal tf32:bf16) x bf16_tflops_sustained (%s)") % peaks["source"],
                                     "alu": "148 SMs x 128 fp32 lanes x 2 flop x sm_max_mhz (derived, DESIGN.md 5)"}[info["bound"]],
                     "share_of_step": round(per_step_ms[dom] / (ms_max / args.steps), 4),
                     "algorithmic_per_atom": {"bytes": info["bytes"], "flops": info["flops"]}}
@@ -371,20 +375,20 @@ def run_ours(args):
             t_b = [m for n_, m, _ in stages if n_ == "mlp_backward"][0]
             n_launch = 2 * len(w.model.hidden)
             ach = 2.0 * info["flops"] * N / ((t_f + t_b) * 1e-3) / 1e12
-            roofline.update({"kernel": "k_gemm_tc_pair" if args.mlp == "3xtf32" else "k_gemm_tc",
+            roofline.update({"kernel": {"3xf16": "k_gemm_tc_pair<F16>", "3xtf32": "k_gemm_tc_pair"}.get(args.mlp, "k_gemm_tc"),
                              "launches_per_step": n_launch, "achieved": round(ach, 3), "frac": round(ach / peak, 4),
                              "avg_launch_ms": round((t_f + t_b) / n_launch, 4),
                              "share_of_step": round((per_step_ms["mlp_forward"] + per_step_ms["mlp_backward"])
                                                     / (ms_max / args.steps), 4),
                              "algorithmic_per_atom": {"bytes": 4.0 * (2 * N_FEATURES + (8 if w.model.n_heads == 1 else 9) * w.model.hidden[0]),
                                                       "flops": 2.0 * info["flops"]}})
-            if args.workload == "config5" and args.mlp == "3xtf32":
+            if args.workload == "config5" and args.mlp in NCU_GEMM_DRAM_BYTES_PER_STEP:
                 # dram__bytes_read.sum + dram__bytes_write.sum of the four launches of one step, per launch
-                # (profiles/ncu_r1_gemm_tc_pair.md)
-                roofline["traffic"] = round(20.43e9 / n_launch)
-        if info["bound"] == "tensor" and args.mlp == "3xtf32":
-            roofline["note"] = ("achieved counts the ALGORITHMIC flops (one product per multiply-add); the 3xTF32 split "
-                                "executes 3 tensor-core MMAs per product, so tensor-pipe flops are 3x achieved")
+                roofline["traffic"] = round(NCU_GEMM_DRAM_BYTES_PER_STEP[args.mlp] / n_launch)
+        if info["bound"] == "tensor" and args.mlp in ("3xtf32", "3xf16"):
+            roofline["note"] = ("achieved counts the ALGORITHMIC flops (one product per multiply-add); the %s split "
+                                "executes 3 tensor-core MMAs per product, so tensor-pipe flops are 3x achieved"
+                                % {"3xtf32": "3xTF32", "3xf16": "3xFP16"}[args.mlp])
             roofline["executed_tflops"] = round(3 * ach, 3)
 
     # ---- end to end through the host-buffer entry ----------------------------------------------
@@ -411,6 +415,7 @@ def run_ours(args):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": {"fp32": "f32", "3xtf32": "f32 (MLP: 3xTF32 split on tcgen05, fp32 accumulate)",
+                      "3xf16": "f32 (MLP: 3xFP16 split on tcgen05, fp32 accumulate)",
                       "tf32": "tf32 MLP, f32 elsewhere"}[args.mlp],
             "data": "synthetic",
             "config": {"workload": args.workload, "n_atoms": N, "what": w.name + ", NVE velocity Verlet, dt %.2f fs, skin %.1f"
@@ -438,8 +443,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="config5",
                     help="config5 (default, 1,048,576 atoms), config2, config3_<N>")
-    ap.add_argument("--mlp", default="3xtf32", choices=sorted(MLP_NAMES),
-                    help="3xtf32 (default): tcgen05 tensor cores, fp32-accurate; fp32: SIMT FMA; tf32: single pass")
+    ap.add_argument("--mlp", default="3xf16", choices=sorted(MLP_NAMES),
+                    help="3xf16 (default) / 3xtf32: tcgen05 tensor cores, fp32-accurate three-product split on fp16 / tf32 "
+                         "operands; fp32: SIMT FMA; tf32: single pass")
     ap.add_argument("--forces", default="pairbuf", choices=["gather", "pairbuf"],
                     help="force reduction: gather form, or pair buffer with a reverse-pair index (both deterministic)")
     ap.add_argument("--no-stages", action="store_true",

@@ -120,13 +120,16 @@ void gmnn_system_destroy(gmnn_system *s);
  *   "capacity"        neighbour slots per atom for the next build (0 = estimate from the density)
  *   "mlp_precision", "force_mode": override the model's value for this system; changing force_mode
  *                     invalidates the neighbour list (call gmnn_build_neighbors again)
- *   "tc_pair"         1 (default): 3xTF32 GEMMs on CTA pairs (cta_group::2); 0: single CTAs
+ *   "tc_pair"         1 (default): 3xTF32 GEMMs on CTA pairs (cta_group::2); 0: single CTAs (3xFP16: always pairs)
  *   "tc_split_bk"     16 | 32 (default): K extent of one pipeline stage of the 3xTF32 GEMM
  *   "tc_flush_k"      multiple of 16 (default 64): K extent after which the tensor-memory accumulator
  *                     is flushed into registers (the tensor core accumulates with truncation)
- *   "tc_flush_head"   1..8 (default 2): the first two accumulator chunks of a tile of the BACKWARD GEMMs span
- *                     this many flush intervals (more run-way for the MMAs while the epilogue finishes
- *                     the previous tile; touches forces only, energies come from the forward GEMMs)
+ *   "tc_h_bk"         32 | 64 (default): K extent of one pipeline stage of the 3xFP16 GEMM
+ *   "tc_flush_head"   0..8 (default 0 = 2 for 3xTF32, 4 for 3xFP16): the first two accumulator chunks of a
+ *                     tile of the BACKWARD GEMMs span this many flush intervals (more run-way for the
+ *                     MMAs while the epilogue finishes the previous tile; touches forces only,
+ *                     energies come from the forward GEMMs)
+ *   "tc_flush_head_fwd" 1..8 (default 1): the same for the forward GEMMs (enters the energies)
  *   "tc_debug"        timing experiments of mlp_tc.cu that knock out work (WRONG results); 0 = off
  *   "cb_halves"       1 | 2 (default) | 3: block shape of the contraction backward kernel (descriptor.cu)
  *   The tc_* knobs and cb_halves are process-wide.

@@ -23,7 +23,7 @@ void set_error(const char *fmt, ...) {
 }
 
 int launch_mlp_forward_tc(gmnn_system *s, cudaStream_t st);
-extern int g_tc_split_bk, g_tc_flush_k, g_tc_debug, g_tc_pair, g_cb_halves, g_tc_flush_head, g_tc_h_bk;
+extern int g_tc_split_bk, g_tc_flush_k, g_tc_debug, g_tc_pair, g_cb_halves, g_tc_flush_head, g_tc_h_bk, g_tc_flush_head_fwd;
 int launch_mlp_backward_tc(gmnn_system *s, const float *head_w_dev, cudaStream_t st);
 
 template <class T>
@@ -375,8 +375,11 @@ int gmnn_system_set_int(gmnn_system *s, const char *key, int64_t v) {
         if (v < 1 || v > 3) return GMNN_INVALID_ARG;  // 1: 128 threads; 2: 256 threads in lock step; 3: 128, lock step
         gmnn::g_cb_halves = (int)v;
     } else if (!strcmp(key, "tc_flush_head")) {  // process-wide, see mlp_tc.cu
-        if (v < 1 || v > 8) return GMNN_INVALID_ARG;
+        if (v < 0 || v > 8) return GMNN_INVALID_ARG;  // 0: automatic (2 on tf32, 4 on fp16)
         gmnn::g_tc_flush_head = (int)v;
+    } else if (!strcmp(key, "tc_flush_head_fwd")) {
+        if (v < 1 || v > 8) return GMNN_INVALID_ARG;
+        gmnn::g_tc_flush_head_fwd = (int)v;
     } else if (!strcmp(key, "tc_pair")) {  // process-wide: 3xTF32 GEMMs on CTA pairs (1) or single CTAs (0)
         gmnn::g_tc_pair = v != 0;
     } else if (!strcmp(key, "tc_debug")) {  // timing experiments (wrong results), see mlp_tc.cu

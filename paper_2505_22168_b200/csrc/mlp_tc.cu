@@ -405,13 +405,16 @@ template <bool F16, int BK>
 struct TcPairCfg {
     static constexpr int ES = F16 ? 2 : 4;                          // operand element size
     static constexpr int ROWB = BK * ES;                            // bytes per K-major operand row = swizzle span
-    static constexpr int LAND_BYTES = F16 ? BK * TC_BM * 4 : 0;     // fp32 landing area of the A tile
+    static constexpr int LAND_BYTES = 0;                            // (F16: the fp32 A tile lands where hi and lo will be)
     static constexpr int A_BYTES = TC_BM * BK * ES;
     static constexpr int B_BYTES = (TC_BN_MAX / 2) * BK * ES;       // this CTA's half of the B tile
     static constexpr int STAGE_BYTES = LAND_BYTES + 2 * (A_BYTES + B_BYTES);  // hi and lo of both
     static constexpr int NST = TC_STAGE_BYTES_TOTAL / STAGE_BYTES;
     static constexpr int SMEM_BYTES = NST * STAGE_BYTES + 1024 + 512;
     static constexpr int KSTEP = 32 / ES;                           // K per MMA instruction
+    // registers per thread of the control / splitter / epilogue warpgroups (setmaxnreg; 128 x sum <= 65536)
+    static constexpr int REGS_CONTROL = F16 ? 32 : TC_REGS_CONTROL, REGS_SPLIT = F16 ? 96 : TC_REGS_SPLIT,
+                         REGS_EPI = F16 ? 192 : TC_REGS_EPI;
     static_assert(NST >= 2, "pipeline needs at least two stages");
 };
 
@@ -422,36 +425,32 @@ __device__ __forceinline__ int amax_exponent(uint32_t bits) {
 }
 __device__ __forceinline__ float pow2i(int e) { return __int_as_float((127 + e) << 23); }
 
-// fp32 A tile [BK][128] -> hi / lo fp16 rows (K-major, swizzled), one atom (row) per thread.
+// fp32 A tile [BK][128] -> hi / lo fp16 rows (K-major, swizzled) IN PLACE, one atom (row) per thread of the
+// four splitter warps: every thread reads its column (conflict-free: lanes are consecutive atoms) and
+// converts it in registers; after a barrier among the 128 threads the rows are written over the tile
+// (hi rows in the first half, lo rows in the second).
 template <int BK>
-__device__ __forceinline__ void split_f16_tile(const float *__restrict__ land, uint8_t *__restrict__ hi, uint8_t *__restrict__ lo,
-                                               int m, float scale, int k_valid) {
+__device__ __forceinline__ void split_f16_tile(uint8_t *__restrict__ stage, int m, float scale, int k_valid) {
     constexpr int ROWB = BK * 2;
+    const float *land = reinterpret_cast<const float *>(stage);
+    uint32_t h[BK / 2], l[BK / 2];
 #pragma unroll
-    for (int c0 = 0; c0 < BK / 8; c0 += 4) {
-        float x[4][8];
+    for (int q = 0; q < BK / 2; ++q) {
+        const bool ok = (2 * q) < k_valid;  // K is a multiple of 8: an 8-wide chunk is whole or absent
+        const float a = ok ? land[(2 * q) * TC_BM + m] * scale : 0.f, b = ok ? land[(2 * q + 1) * TC_BM + m] * scale : 0.f;
+        const __half2 hh = __floats2half2_rn(a, b);
+        const float2 hf = __half22float2(hh);
+        const __half2 ll = __floats2half2_rn(a - hf.x, b - hf.y);
+        h[q] = *reinterpret_cast<const uint32_t *>(&hh);
+        l[q] = *reinterpret_cast<const uint32_t *>(&ll);
+    }
+    asm volatile("bar.sync 1, 128;" ::: "memory");  // all columns read before any row is written
 #pragma unroll
-        for (int c = 0; c < 4; ++c)
-#pragma unroll
-            for (int k = 0; k < 8; ++k) x[c][k] = land[((c0 + c) * 8 + k) * TC_BM + m];
-#pragma unroll
-        for (int c = 0; c < 4; ++c) {
-            uint32_t h[4], l[4];
-            const bool ok = (c0 + c) * 8 < k_valid;  // K is a multiple of 8: a chunk is whole or absent
-#pragma unroll
-            for (int q = 0; q < 4; ++q) {
-                const float a = ok ? x[c][2 * q] * scale : 0.f, b = ok ? x[c][2 * q + 1] * scale : 0.f;
-                const __half2 hh = __floats2half2_rn(a, b);
-                const float2 hf = __half22float2(hh);
-                const __half2 ll = __floats2half2_rn(a - hf.x, b - hf.y);
-                h[q] = *reinterpret_cast<const uint32_t *>(&hh);
-                l[q] = *reinterpret_cast<const uint32_t *>(&ll);
-            }
-            uint32_t o = (uint32_t)(m * ROWB + (c0 + c) * 16);
-            o ^= ((o >> 7) & (uint32_t)(ROWB / 16 - 1)) << 4;  // 128- / 64-byte swizzle of the 16-byte chunk index
-            *reinterpret_cast<uint4 *>(hi + o) = make_uint4(h[0], h[1], h[2], h[3]);
-            *reinterpret_cast<uint4 *>(lo + o) = make_uint4(l[0], l[1], l[2], l[3]);
-        }
+    for (int c = 0; c < BK / 8; ++c) {
+        uint32_t o = (uint32_t)(m * ROWB + c * 16);
+        o ^= ((o >> 7) & (uint32_t)(ROWB / 16 - 1)) << 4;  // 128- / 64-byte swizzle of the 16-byte chunk index
+        *reinterpret_cast<uint4 *>(stage + o) = make_uint4(h[4 * c], h[4 * c + 1], h[4 * c + 2], h[4 * c + 3]);
+        *reinterpret_cast<uint4 *>(stage + TC_BM * ROWB + o) = make_uint4(l[4 * c], l[4 * c + 1], l[4 * c + 2], l[4 * c + 3]);
     }
 }
 
@@ -463,7 +462,7 @@ k_gemm_tc_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;  // identical offset in both CTAs
     uint8_t *smem_gen = smem_raw + (smem_base - smem_u32(smem_raw));
-    // stage: [fp32 A landing (F16) | A_hi | A_lo | B_hi | B_lo]
+    // stage: [A_hi | A_lo | B_hi | B_lo]; the fp32 A tile of the 3xFP16 mode lands on A_hi | A_lo
     auto a_hi = [&](int s) { return smem_base + (uint32_t)s * Cfg::STAGE_BYTES + Cfg::LAND_BYTES; };
     auto a_lo = [&](int s) { return a_hi(s) + Cfg::A_BYTES; };
     auto b_hi = [&](int s) { return a_hi(s) + 2 * Cfg::A_BYTES; };
@@ -504,7 +503,7 @@ k_gemm_tc_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     const uint32_t tmem_base = *tmem_slot_gen;
 
     if (warp < TC_FIRST_SPLIT_WARP) {
-        setmaxnreg_dec<TC_REGS_CONTROL>();
+        setmaxnreg_dec<Cfg::REGS_CONTROL>();
         if (warp == 0 && lane == 0) {
             // ===== TMA producer: own A rows, own half of B =====
             const uint32_t tx = (uint32_t)(TC_BM * BK * 4 + 2 * hb * BK * Cfg::ES);
@@ -516,7 +515,7 @@ k_gemm_tc_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                     mbar_wait(bar_empty(s), ((it / NST) & 1) ^ 1);
                     mbar_arrive_expect_tx(bar_full(s), tx);
                     if (F16) {
-                        tma_load_2d(a_hi(s) - Cfg::LAND_BYTES, &tmA, bar_full(s), 0, mt * p.K + kb * BK);  // [BK][128] fp32
+                        tma_load_2d(a_hi(s), &tmA, bar_full(s), 0, mt * p.K + kb * BK);  // [BK][128] fp32
                     } else {
                         for (int q = 0; q < 4; ++q)
                             tma_load_2d(a_hi(s) + q * (BK * 128), &tmA, bar_full(s), q * 32, mt * p.K + kb * BK);
@@ -550,7 +549,7 @@ k_gemm_tc_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                     // per k step: B (and a K-major A) advance 32 bytes along the row, the MN-major A one 1024-byte atom
                     const uint64_t astep = F16 ? 2 : 64;
                     uint32_t acc = !chunk_first;
-                    for (int k = 0; k < ksteps; ++k) {  // small cross terms first
+                    for (int k = 0; k < ksteps && !(p.debug & 2); ++k) {  // small cross terms first
                         const uint64_t koff = (uint64_t)(2 * k), aoff = astep * k;
                         if (F16) {
                             mma_f16_ss_pair(d_tmem, da_lo + aoff, db_hi + koff, idesc, acc);
@@ -563,8 +562,9 @@ k_gemm_tc_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                     }
                     for (int k = 0; k < ksteps; ++k) {
                         const uint64_t koff = (uint64_t)(2 * k), aoff = astep * k;
-                        if (F16) mma_f16_ss_pair(d_tmem, da_hi + aoff, db_hi + koff, idesc, 1u);
-                        else mma_tf32_ss_pair(d_tmem, da_hi + aoff, db_hi + koff, idesc, 1u);
+                        if (F16) mma_f16_ss_pair(d_tmem, da_hi + aoff, db_hi + koff, idesc, acc);
+                        else mma_tf32_ss_pair(d_tmem, da_hi + aoff, db_hi + koff, idesc, acc);
+                        acc = 1u;
                     }
                     mma_commit_pair(bar_empty(s), 3);
                     if (chunk_last) {
@@ -575,7 +575,7 @@ k_gemm_tc_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
             }
         }
     } else if (warp < TC_FIRST_EPI_WARP) {
-        setmaxnreg_dec<TC_REGS_SPLIT>();
+        setmaxnreg_dec<Cfg::REGS_SPLIT>();
         // ===== splitters: own A tile into hi and lo (B arrives split: model->Ws / WTs / Wh / WTh) =====
         const int tid = threadIdx.x - TC_FIRST_SPLIT_WARP * 32;
         const float ascale = F16 ? pow2i(14 - amax_exponent(*p.amax_a)) : 1.f;
@@ -585,9 +585,10 @@ k_gemm_tc_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                 const int s = it % NST;
                 mbar_wait(bar_full(s), (it / NST) & 1);
                 uint8_t *stage = smem_gen + (size_t)s * Cfg::STAGE_BYTES;
-                if (F16) {
-                    split_f16_tile<BK>(reinterpret_cast<const float *>(stage), stage + Cfg::LAND_BYTES,
-                                       stage + Cfg::LAND_BYTES + Cfg::A_BYTES, tid, ascale, p.K - kb * BK);
+                if (p.debug & 1) {
+                    if (F16) asm volatile("bar.sync 1, 128;" ::: "memory");
+                } else if (F16) {
+                    split_f16_tile<BK>(stage, tid, ascale, p.K - kb * BK);
                 } else {
                     float4 *ah = reinterpret_cast<float4 *>(stage);
                     split_hi_lo(ah, ah + Cfg::A_BYTES / 16, Cfg::A_BYTES / 16, tid);
@@ -598,7 +599,7 @@ k_gemm_tc_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
             }
         }
     } else {
-        setmaxnreg_inc<TC_REGS_EPI>();
+        setmaxnreg_inc<Cfg::REGS_EPI>();
         // ===== epilogue: this CTA's 128 rows =====
         const int quad = warp & 3;
         const int half = (warp - TC_FIRST_EPI_WARP) >> 2;
@@ -767,7 +768,8 @@ static int tc_launch(const CUtensorMap &tmA, const CUtensorMap &tmB, const TcArg
 }
 
 int g_tc_pair = 1;    // knob "tc_pair": 3xTF32 GEMMs on CTA pairs (cta_group::2)
-int g_tc_flush_head = 2;  // knob "tc_flush_head": first-two-chunks multiplier of the backward GEMMs (forces only)
+int g_tc_flush_head = 0;  // knob "tc_flush_head": first-two-chunks multiplier of the backward GEMMs (forces only); 0 = auto
+int g_tc_flush_head_fwd = 1;  // knob "tc_flush_head_fwd": the same for the forward GEMMs (enters the energy)
 int g_tc_debug = 0;
 int g_tc_flush_k = 64;   // knob "tc_flush_k": K extent between accumulator flushes of the 3xTF32 / 3xFP16 modes
 int g_tc_split_bk = 32;  // knob (gmnn_system_set_int "tc_split_bk"): K extent of a 3xTF32 stage, 16 or 32
@@ -842,7 +844,10 @@ int tc_gemm(bool split, int epi, int64_t M, int N, int K, const float *A, const 
     a.n_tiles_n = (N + a.bn - 1) / a.bn;
     a.n_tiles = (int)((M + TC_BM - 1) / TC_BM) * a.n_tiles_n;
     a.flush = split ? (g_tc_flush_k / BK > 0 ? g_tc_flush_k / BK : 1) : (K + BK - 1) / BK;  // TF32 mode: one chunk
-    a.flush1 = a.flush * ((split && epi != EPI_HIDDEN && epi != EPI_HIDDEN_HEAD) ? g_tc_flush_head : 1);
+    // backward GEMMs (forces only: error budget 1e-4) take longer first chunks: x2 on tf32, x4 on fp16, whose
+    // MMAs add 16 products per accumulation step instead of 8
+    const int head_bwd = g_tc_flush_head > 0 ? g_tc_flush_head : (hf ? 4 : 2);
+    a.flush1 = a.flush * (!split ? 1 : (epi != EPI_HIDDEN && epi != EPI_HIDDEN_HEAD) ? head_bwd : g_tc_flush_head_fwd);
     a.debug = g_tc_debug;
     a.C = C, a.C2 = C2, a.bias = bias, a.Dmul = Dmul;
     a.w_head = w_head, a.ypart = ypart, a.m_pad = (M + TC_BM - 1) / TC_BM * TC_BM;

@@ -134,8 +134,9 @@ def test_md_cell_list_rebuild_inside_the_loop(gm, orc, force_mode):
     assert np.abs(etot - etot[0]).max() <= 2e-3 * np.abs(ekin.cpu().numpy()).max()
 
 
+@pytest.mark.parametrize("mlp_precision", [1, 3])
 @pytest.mark.parametrize("force_mode", [0, 1])
-def test_md_graph_replay_is_bitwise_the_eager_loop(gm, force_mode):
+def test_md_graph_replay_is_bitwise_the_eager_loop(gm, force_mode, mlp_precision):
     """gmnn_md_verlet_steps replays the step as a CUDA graph (knob md_graph, default on): positions,
     velocities, both energy series and the rebuild count are bit-identical to the eager loop, across
     in-loop rebuilds and across a continued call."""
@@ -144,7 +145,7 @@ def test_md_graph_replay_is_bitwise_the_eager_loop(gm, force_mode):
     w = wl.li3po4_box(1024, hidden=(64, 64), skin=0.3)
     out = []
     for graph in (1, 0):
-        _, sysm, pos = _build(gm, w, mlp_precision=1, force_mode=force_mode)
+        _, sysm, pos = _build(gm, w, mlp_precision=mlp_precision, force_mode=force_mode)
         sysm.set_int("md_graph", graph)
         vel = torch.from_numpy(w.velocities * 6.0).cuda()
         mass = torch.from_numpy(w.masses).cuda()

@@ -1,5 +1,5 @@
 """Parity at BASELINE.json's full sizes (config 3 at 65 536 and 131 072 atoms, config 5 at 1 048 576),
-in the launch configuration bench.py times (3xTF32 MLP on CTA pairs, pair-buffer forces, the
+in the launch configuration bench.py times (3xFP16 MLP on CTA pairs, pair-buffer forces, the
 config's skin).  The oracle cannot evaluate a million atoms in test time, but E_i and F_i of ONE atom
 depend only on the atoms within 2 r_cut of it: for a seeded sample of atoms the oracle evaluates that
 neighbourhood as a free cluster (fp64 differences of the fp32 positions, minimum image applied), and
@@ -44,7 +44,7 @@ def test_full_size_sampled_atoms(gm, orc, name, n_samples):
     import torch
 
     w = wl.make_workload(name)
-    model = gm.Model(w.model, mlp_precision=gm.GMNN_MLP_3XTF32, force_mode=gm.GMNN_FORCE_PAIRBUF)
+    model = gm.Model(w.model, mlp_precision=gm.GMNN_MLP_3XF16, force_mode=gm.GMNN_FORCE_PAIRBUF)
     sysm = gm.System(model, w.species)
     pos = torch.from_numpy(w.positions).cuda()
     sysm.build_neighbors(pos, w.cell9, w.pbc, w.model.r_cut, w.skin)
@@ -92,7 +92,7 @@ def test_config5_md_steps_conserve_energy(gm):
     import torch
 
     w = wl.make_workload("config5")
-    model = gm.Model(w.model, mlp_precision=gm.GMNN_MLP_3XTF32, force_mode=gm.GMNN_FORCE_PAIRBUF)
+    model = gm.Model(w.model, mlp_precision=gm.GMNN_MLP_3XF16, force_mode=gm.GMNN_FORCE_PAIRBUF)
     sysm = gm.System(model, w.species)
     pos = torch.from_numpy(w.positions).cuda()
     vel = torch.from_numpy(w.velocities).cuda()
@@ -121,7 +121,7 @@ def test_config2_full_run(gm, orc):
     import torch
 
     w = wl.make_workload("config2")
-    model = gm.Model(w.model, mlp_precision=gm.GMNN_MLP_3XTF32, force_mode=gm.GMNN_FORCE_PAIRBUF)
+    model = gm.Model(w.model, mlp_precision=gm.GMNN_MLP_3XF16, force_mode=gm.GMNN_FORCE_PAIRBUF)
     sysm = gm.System(model, w.species)
     pos = torch.from_numpy(w.positions).cuda()
     vel = torch.from_numpy(w.velocities).cuda()
