@@ -593,7 +593,7 @@ k_gemm_tc_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                     float4 *ah = reinterpret_cast<float4 *>(stage);
                     split_hi_lo(ah, ah + Cfg::A_BYTES / 16, Cfg::A_BYTES / 16, tid);
                 }
-                fence_proxy_async_all();
+                fence_proxy_async_smem();  // own shared memory, read next by the tensor core (async proxy)
                 __syncwarp();
                 if (lane == 0) mbar_arrive_cluster(bar_split(s), 0);
             }
