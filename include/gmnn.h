@@ -131,7 +131,7 @@ void gmnn_system_destroy(gmnn_system *s);
  *                     energies come from the forward GEMMs)
  *   "tc_flush_head_fwd" 1..8 (default 1): the same for the forward GEMMs (enters the energies)
  *   "tc_debug"        timing experiments of mlp_tc.cu that knock out work (WRONG results); 0 = off
- *   "cb_halves"       1 | 2 (default) | 3: block shape of the contraction backward kernel (descriptor.cu)
+ *   "cb_halves"       1..6 (default 6): block shape / body of the contraction backward kernel (descriptor.cu)
  *   The tc_* knobs and cb_halves are process-wide.
  * Returns GMNN_INVALID_ARG for an unknown key or value. */
 int gmnn_system_set_int(gmnn_system *s, const char *key, int64_t value);

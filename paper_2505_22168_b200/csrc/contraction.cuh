@@ -194,16 +194,32 @@ struct NoStep {
 
 // step(): called after every channel-pair iteration of the straight-line body (a kernel can put a block
 // barrier there to keep its warps inside the same stretch of code).
-template <int NR, int BLOCKS = 0xFF, class PGet, class GGet, class Acc, class Step = NoStep>
+//
+// ORBIT = true evaluates only one representative of every orbit of channel tuples under the cyclic shift
+// s -> s + 1 (mod NR) of ALL channels: pairs {0, 0}, {0, 1}, ... {0, NR/2}; block 4 multisets {0,0,s3},
+// {0,1,2}, {0,1,3}; block 7 tuples with s2 = 0.  Every block is symmetric under the exchanges its loops
+// skip (s1 <-> s2; any permutation in block 4), so a caller that runs the representatives NR times, each
+// time with P and the adjoints renumbered s -> s + 1 and g looked up at the shifted tuple, covers every
+// tuple exactly once with a fifth of the code (k_contract_backward, descriptor.cu).  NR must be prime.
+template <int NR>
+GMNN_HD constexpr bool orbit_pair(int s1, int s2) { return s1 == 0 && s2 <= NR / 2; }
+template <int NR>
+GMNN_HD constexpr bool orbit_triple(int s1, int s2, int s3) {
+    return s1 == 0 && (s2 == 0 || (s2 == 1 && (s3 == 2 || s3 == 3)));
+}
+
+template <int NR, int BLOCKS = 0xFF, bool ORBIT = false, class PGet, class GGet, class Acc, class Step = NoStep>
 GMNN_HD void contract_backward(PGet P, GGet g, Acc acc, Step step = Step()) {
     using F = Feat<NR>;
+    static_assert(!ORBIT || NR == 5, "orbit representatives are written out for NR = 5");
     if constexpr ((BLOCKS & 0xF) != 0) {
 #pragma unroll
-    for (int s = 0; s < NR; ++s) acc(s, 0, g(F::OFF0 + s));
+    for (int s = 0; s < (ORBIT ? 1 : NR); ++s) acc(s, 0, g(F::OFF0 + s));
 #pragma unroll
     for (int s1 = 0; s1 < NR; ++s1) {
 #pragma unroll
         for (int s2 = s1; s2 < NR; ++s2) {
+            if (ORBIT && !orbit_pair<NR>(s1, s2)) continue;
             step();
             const float g1 = g(F::OFF1 + F::pidx(s1, s2));
             const float g2 = g(F::OFF2 + F::pidx(s1, s2));
@@ -232,6 +248,7 @@ GMNN_HD void contract_backward(PGet P, GGet g, Acc acc, Step step = Step()) {
     for (int s1 = 0; s1 < NR; ++s1) {
 #pragma unroll
         for (int s2 = s1; s2 < NR; ++s2) {
+            if (ORBIT && !orbit_triple<NR>(s1, s2, s2 == 0 ? 0 : 2)) continue;  // pairs (0,0) and (0,1)
             step();
             float S[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
 #pragma unroll
@@ -246,6 +263,7 @@ GMNN_HD void contract_backward(PGet P, GGet g, Acc acc, Step step = Step()) {
             float dS[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
 #pragma unroll
             for (int s3 = s2; s3 < NR; ++s3) {
+                if (ORBIT && !orbit_triple<NR>(s1, s2, s3)) continue;
                 const float gv = g(F::OFF4 + F::tidx(s1, s2, s3));
 #pragma unroll
                 for (int u = 0; u < 6; ++u) {
@@ -276,6 +294,7 @@ GMNN_HD void contract_backward(PGet P, GGet g, Acc acc, Step step = Step()) {
     for (int s1 = 0; s1 < NR; ++s1) {
 #pragma unroll
         for (int s2 = s1; s2 < NR; ++s2) {
+            if (ORBIT && !orbit_pair<NR>(s1, s2)) continue;
             step();
             float O[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
 #pragma unroll
@@ -312,6 +331,7 @@ GMNN_HD void contract_backward(PGet P, GGet g, Acc acc, Step step = Step()) {
     for (int s1 = 0; s1 < NR; ++s1) {
 #pragma unroll
         for (int s2 = s1; s2 < NR; ++s2) {
+            if (ORBIT && !orbit_pair<NR>(s1, s2)) continue;
             step();
             float S[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
 #pragma unroll
@@ -351,7 +371,7 @@ GMNN_HD void contract_backward(PGet P, GGet g, Acc acc, Step step = Step()) {
     // block 7
     if constexpr ((BLOCKS & 0x80) != 0) {
 #pragma unroll
-    for (int s2 = 0; s2 < NR; ++s2) {
+    for (int s2 = 0; s2 < (ORBIT ? 1 : NR); ++s2) {
 #pragma unroll
         for (int s3 = 0; s3 < NR; ++s3) {
             step();

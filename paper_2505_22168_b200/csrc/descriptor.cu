@@ -19,6 +19,7 @@
 // mono_m(u), so g_ij = dE/dd = (sum_s R'_s p_s) u + (grad_u q - (u.grad_u q) u) / r with
 // q(u) = sum_m (sum_s R_s A[s][m]) mono_m(u).
 #include <type_traits>
+#include <vector>
 
 #include "contraction.cuh"
 #include "gmnn_internal.h"
@@ -252,6 +253,48 @@ k_contract_forward(int64_t N, const float *__restrict__ psi, float *__restrict__
 // dE/dG arrives without the sigma_Z factor of Eq. 4 (the MLP backward is linear in it); it is
 // applied here.
 // ---------------------------------------------------------------------------------------------
+// c_rot[r][f]: the feature whose channel tuple is that of feature f with every channel shifted by r
+// (mod 5): what the representative-tuple code of contract_backward<.., ORBIT = true> reads in round r.
+__constant__ uint16_t c_rot[5 * Feat<5>::N];
+
+static int upload_rot_table() {
+    using F = Feat<5>;
+    constexpr int NR = 5;
+    static bool done = false;
+    if (done) return GMNN_OK;
+    std::vector<uint16_t> t((size_t)NR * F::N, 0);
+    auto sort2 = [](int &a, int &b) { if (a > b) { int x = a; a = b; b = x; } };
+    for (int r = 0; r < NR; ++r) {
+        uint16_t *row = t.data() + (size_t)r * F::N;
+        auto sh = [&](int x) { return (x + r) % NR; };
+        for (int x = 0; x < NR; ++x) row[F::OFF0 + x] = (uint16_t)(F::OFF0 + sh(x));
+        for (int s1 = 0; s1 < NR; ++s1)
+            for (int s2 = s1; s2 < NR; ++s2) {
+                int a = sh(s1), b = sh(s2);
+                sort2(a, b);
+                row[F::OFF1 + F::pidx(s1, s2)] = (uint16_t)(F::OFF1 + F::pidx(a, b));
+                row[F::OFF2 + F::pidx(s1, s2)] = (uint16_t)(F::OFF2 + F::pidx(a, b));
+                row[F::OFF3 + F::pidx(s1, s2)] = (uint16_t)(F::OFF3 + F::pidx(a, b));
+                for (int s3 = 0; s3 < NR; ++s3) {
+                    row[F::OFF5 + F::pidx(s1, s2) * NR + s3] = (uint16_t)(F::OFF5 + F::pidx(a, b) * NR + sh(s3));
+                    row[F::OFF6 + F::pidx(s1, s2) * NR + s3] = (uint16_t)(F::OFF6 + F::pidx(a, b) * NR + sh(s3));
+                }
+                for (int s3 = s2; s3 < NR; ++s3) {
+                    int x = sh(s1), y = sh(s2), z = sh(s3);
+                    sort2(x, y); sort2(y, z); sort2(x, y);
+                    row[F::OFF4 + F::tidx(s1, s2, s3)] = (uint16_t)(F::OFF4 + F::tidx(x, y, z));
+                }
+            }
+        for (int s1 = 0; s1 < NR; ++s1)
+            for (int s2 = 0; s2 < NR; ++s2)
+                for (int s3 = 0; s3 < NR; ++s3)
+                    row[F::OFF7 + (s1 * NR + s2) * NR + s3] = (uint16_t)(F::OFF7 + (sh(s1) * NR + sh(s2)) * NR + sh(s3));
+    }
+    GMNN_CUDA(cudaMemcpyToSymbol(c_rot, t.data(), t.size() * sizeof(uint16_t)));
+    done = true;
+    return GMNN_OK;
+}
+
 template <int NR>
 struct CbSmem {  // shared-memory plan of k_contract_backward, in floats
     using CH = FeatChunks<NR>;
@@ -268,7 +311,12 @@ struct CbSmem {  // shared-memory plan of k_contract_backward, in floats
 // HALVES = 2: one 256-thread block per SM works on two tiles in lock step (the block-wide barriers
 // between chunks keep all eight warps inside the same stretch of the ~12 k-instruction straight-line
 // body, so they share its instruction-cache lines); HALVES = 1: two independent 128-thread blocks per SM.
-template <int NR, int HALVES, bool LOCKSTEP>
+// ORBIT: the straight-line body holds only the representative channel tuples (contraction.cuh) and runs
+// NR times per chunk, the Psi rows and the adjoints moved down one channel (register moves) after each
+// round and the features read through c_rot: a fifth of the code, and each chunk's loop then fits
+// the 32 KB instruction cache level for four of its five rounds (the full body is ~170 KB, fetched from
+// L2 once per block: ncu shows the no_instruction stalls at every 256-byte boundary).
+template <int NR, int HALVES, bool LOCKSTEP, bool ORBIT>
 __global__ void __launch_bounds__(128 * HALVES, 3 - HALVES)
 k_contract_backward(int64_t N, const float *__restrict__ psi, const float *__restrict__ dGt,
                     const float4 *__restrict__ pos4, const float *__restrict__ scale, float *__restrict__ A) {
@@ -325,13 +373,35 @@ k_contract_backward(int64_t N, const float *__restrict__ psi, const float *__res
 
     auto run_chunk = [&](auto chunk_tag, const float *buf) {
         constexpr int C = decltype(chunk_tag)::value;
-        contract_backward<NR, CH::mask(C)>(
-            [&](int s, int m) { return P[s][m]; },
-            [&](int f) { return buf[(f - CH::begin(C)) * TB + tid]; },
-            [&](int s, int m, float v) { acc[s][m] += v; },
-            [&]() {  // keep the warps of the block in the same stretch of the instruction stream
-                if (LOCKSTEP) __syncthreads();
-            });
+        if constexpr (ORBIT) {
+#pragma unroll 1
+            for (int r = 0; r < NR; ++r) {
+                const uint16_t *rot = c_rot + r * F::N;
+                contract_backward<NR, CH::mask(C), true>(
+                    [&](int s, int m) { return P[s][m]; },
+                    [&](int f) { return buf[((int)rot[f] - CH::begin(C)) * TB + tid]; },
+                    [&](int s, int m, float v) { acc[s][m] += v; },
+                    [&]() {
+                        if (LOCKSTEP) __syncthreads();
+                    });
+                // static channel s now stands for channel s + r + 1 (after NR rounds: back in place)
+#pragma unroll
+                for (int m = 0; m < PSI; ++m) {
+                    const float p0 = P[0][m], a0 = acc[0][m];
+#pragma unroll
+                    for (int s = 0; s + 1 < NR; ++s) P[s][m] = P[s + 1][m], acc[s][m] = acc[s + 1][m];
+                    P[NR - 1][m] = p0, acc[NR - 1][m] = a0;
+                }
+            }
+        } else {
+            contract_backward<NR, CH::mask(C)>(
+                [&](int s, int m) { return P[s][m]; },
+                [&](int f) { return buf[(f - CH::begin(C)) * TB + tid]; },
+                [&](int s, int m, float v) { acc[s][m] += v; },
+                [&]() {  // keep the warps of the block in the same stretch of the instruction stream
+                    if (LOCKSTEP) __syncthreads();
+                });
+        }
     };
     if (active) tc::mbar_wait(barY, 0);
     run_chunk(std::integral_constant<int, 0>{}, sY);
@@ -675,33 +745,40 @@ int launch_contract_forward(gmnn_system *s, cudaStream_t st) {
     return GMNN_OK;
 }
 
-int g_cb_halves = 2;  // knob "cb_halves": 1 = one tile per block; 2 = two tiles, lock step (default); 3 = one tile, lock step
+// knob "cb_halves": block shape of k_contract_backward.  1 = one tile per block; 2 = two tiles, lock step;
+// 3 = one tile, lock step (all three: the full straight-line body); 4 = two tiles, lock step, 5 = one tile,
+// lock step, 6 = one tile per block (default), with the orbit-representative body.  Config 5: 2.57 / 2.25 / - /
+// 1.23 / 1.02 / 1.02 ms
+int g_cb_halves = 6;
 
-int launch_contract_backward(gmnn_system *s, cudaStream_t st) {
-    constexpr int NR = 5;
+template <int NR, int HALVES, bool LOCKSTEP, bool ORBIT>
+static int launch_cb(gmnn_system *s, cudaStream_t st) {
     static bool attr_set = false;
     if (!attr_set) {
-        GMNN_CUDA(cudaFuncSetAttribute(k_contract_backward<NR, 1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                       (int)CbSmem<NR>::bytes(1)));
-        GMNN_CUDA(cudaFuncSetAttribute(k_contract_backward<NR, 1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                       (int)CbSmem<NR>::bytes(1)));
-        GMNN_CUDA(cudaFuncSetAttribute(k_contract_backward<NR, 2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                       (int)CbSmem<NR>::bytes(2)));
+        GMNN_CUDA(cudaFuncSetAttribute(k_contract_backward<NR, HALVES, LOCKSTEP, ORBIT>,
+                                       cudaFuncAttributeMaxDynamicSharedMemorySize, (int)CbSmem<NR>::bytes(HALVES)));
         attr_set = true;
     }
     const unsigned tiles = nblocks(s->N, 128);
-    if (g_cb_halves == 2)
-        k_contract_backward<NR, 2, true><<<(tiles + 1) / 2, 256, CbSmem<NR>::bytes(2), st>>>(s->N, s->psi, s->dG, s->pos4,
-                                                                                              s->model->scale, s->A);
-    else if (g_cb_halves == 3)
-        k_contract_backward<NR, 1, true><<<tiles, 128, CbSmem<NR>::bytes(1), st>>>(s->N, s->psi, s->dG, s->pos4,
-                                                                                    s->model->scale, s->A);
-    else
-        k_contract_backward<NR, 1, false><<<tiles, 128, CbSmem<NR>::bytes(1), st>>>(s->N, s->psi, s->dG, s->pos4,
-                                                                                     s->model->scale, s->A);
+    k_contract_backward<NR, HALVES, LOCKSTEP, ORBIT><<<(tiles + HALVES - 1) / HALVES, 128 * HALVES, CbSmem<NR>::bytes(HALVES), st>>>(
+        s->N, s->psi, s->dG, s->pos4, s->model->scale, s->A);
     GMNN_LAUNCHED();
     GMNN_CUDA(cudaGetLastError());
     return GMNN_OK;
+}
+
+int launch_contract_backward(gmnn_system *s, cudaStream_t st) {
+    constexpr int NR = 5;
+    int rc;
+    if (g_cb_halves >= 4 && (rc = upload_rot_table())) return rc;
+    switch (g_cb_halves) {
+        case 1: return launch_cb<NR, 1, false, false>(s, st);
+        case 2: return launch_cb<NR, 2, true, false>(s, st);
+        case 3: return launch_cb<NR, 1, true, false>(s, st);
+        case 4: return launch_cb<NR, 2, true, true>(s, st);
+        case 5: return launch_cb<NR, 1, true, true>(s, st);
+        default: return launch_cb<NR, 1, false, true>(s, st);
+    }
 }
 
 }  // namespace gmnn

@@ -372,7 +372,7 @@ int gmnn_system_set_int(gmnn_system *s, const char *key, int64_t v) {
         if (v != 16 && v != 32) return GMNN_INVALID_ARG;
         gmnn::g_tc_split_bk = (int)v;
     } else if (!strcmp(key, "cb_halves")) {  // process-wide: tiles per block of k_contract_backward
-        if (v < 1 || v > 3) return GMNN_INVALID_ARG;  // 1: 128 threads; 2: 256 threads in lock step; 3: 128, lock step
+        if (v < 1 || v > 6) return GMNN_INVALID_ARG;  // see descriptor.cu
         gmnn::g_cb_halves = (int)v;
     } else if (!strcmp(key, "tc_flush_head")) {  // process-wide, see mlp_tc.cu
         if (v < 0 || v > 8) return GMNN_INVALID_ARG;  // 0: automatic (2 on tf32, 4 on fp16)

@@ -7,7 +7,7 @@ import numpy as np
 import pytest
 
 import workloads as wl
-from parity_utils import E_TOTAL_RTOL, F_TOL, energy_atom_error, force_error, r_list32
+from parity_utils import E_TOTAL_RTOL, F_TOL, energy_atom_error, force_error, r_list32, unique_from_full
 
 F_TOL_TF32_MEASURED = 5e-2  # characterisation bound of the unclaimed single-pass mode
 
@@ -196,15 +196,24 @@ def test_cta_pair_and_single_cta_kernels(gm, orc, name):
 
 def test_contract_backward_block_shapes(gm, orc):
     """k_contract_backward with one or two 128-atom tiles per block, with and without the lock-step
-    barriers, gives the same adjoints (odd tile count)."""
+    barriers, gives the same adjoints (odd tile count); the orbit-representative body (cb_halves 4-6: a
+    fifth of the code run five times with the channels shifted) sums the same terms in another order."""
     w = wl.li3po4_box(128 * 5 + 24, hidden=(32, 32))
+    ref = _ref(orc, w, intermediates=True)
     sysm, pos = _system(gm, w, P3X)
-    res = []
+    res = {}
     try:
-        for halves in (1, 2, 3):
+        for halves in (1, 2, 3, 4, 5, 6):
             sysm.set_int("cb_halves", halves)
-            _run(sysm, pos)
-            res.append(sysm.debug_read("A"))
+            e, ea, f = _run(sysm, pos)
+            res[halves] = sysm.debug_read("A")
+            assert force_error(f, ref.forces) <= F_TOL, halves
     finally:
-        sysm.set_int("cb_halves", 2)
-    assert np.array_equal(res[0], res[1]) and np.array_equal(res[0], res[2])
+        sysm.set_int("cb_halves", 6)
+    assert np.array_equal(res[1], res[2]) and np.array_equal(res[1], res[3])
+    assert np.array_equal(res[4], res[5]) and np.array_equal(res[4], res[6])
+    perm = sysm.debug_read("perm")
+    a_ref = unique_from_full(ref.Q, summed=True)[perm]  # adjoints with respect to the unique moments
+    for halves in (1, 4):
+        assert np.abs(res[halves] - a_ref).max() <= 1e-4 * np.abs(a_ref).max(), halves
+    assert np.abs(res[1] - res[4]).max() <= 1e-5 * np.abs(a_ref).max()
