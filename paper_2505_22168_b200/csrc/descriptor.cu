@@ -561,20 +561,18 @@ k_pair_backward(int64_t N, const float4 *__restrict__ pos4, const uint32_t *__re
                         float R[NR], dR[NR];
 #pragma unroll
                         for (int s = 0; s < NR; ++s) {
-                            float sum = 0.f, dsum = 0.f;
+                            float2 sd = make_float2(0.f, 0.f);  // (sum beta phi, sum beta phi'): one FFMA2 per term
 #pragma unroll
                             for (int kq = 0; kq < KB / 4; ++kq) {
                                 const float4 b = bt[s * (KB / 4) + kq];
                                 const float bv[4] = {b.x, b.y, b.z, b.w};
 #pragma unroll
                                 for (int c = 0; c < 4; ++c)
-                                    if (4 * kq + c < NB) {
-                                        sum = fmaf(bv[c], phi[4 * kq + c], sum);
-                                        dsum = fmaf(bv[c], dphi[4 * kq + c], dsum);
-                                    }
+                                    if (4 * kq + c < NB)
+                                        sd = __ffma2_rn(make_float2(bv[c], bv[c]), make_float2(phi[4 * kq + c], dphi[4 * kq + c]), sd);
                             }
-                            R[s] = fc * sum;
-                            dR[s] = dfc * sum + fc * dsum;
+                            R[s] = fc * sd.x;
+                            dR[s] = dfc * sd.x + fc * sd.y;
                         }
                         if (dir == 0) {
                             pair_gradient<NR>([&](int s, int qq) { return Ai[s * (PSI / 4) + qq]; }, R, dR, mono, ux, uy,
