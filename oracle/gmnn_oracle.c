@@ -12,7 +12,10 @@
  * Pins (tests/test_oracle_*.py, all `-m "not gpu"`): forces == central finite differences of the
  * energy; sum F = 0; E invariant under rotation / translation+wrap / permutation; brute-force ==
  * cell-list neighbour sets; dimer and simple-cubic closed forms; trace identities of the moments;
- * MLP == numpy matmul; Eq. 6 linearity of the ensemble; NVE dt^2 scaling and time reversal.
+ * MLP == numpy matmul; Eq. 6 linearity of the ensemble; NVE dt^2 scaling and time reversal;
+ * O-12: identical heads give sigma = 0 and the single-head NVE trajectory, the sampled trajectory does
+ * not depend on sampling_rate, sigma_E against numpy's std of the head totals, stop at the first
+ * sample over the threshold (tests/test_oracle_switching.py).
  * Parity unpinned by the paper itself: PAPER.md prints no numeric E or F for any geometry, and the
  * constants of DESIGN.md readings R1-R4, R7-R10 are readings, not quotes.
  *
@@ -26,6 +29,8 @@
  *   O-7..O-9 forces = -dE/dR ...... PAPER.md:127, 153 (gradient of the energy), chain rule by hand
  *   O-10 ensemble ................. PAPER.md:75-88 (Eq. 5 with 1/N_ens, Eq. 6)
  *   O-11 NVE velocity Verlet ...... BASELINE.json configs 2, 5; dt PAPER.md:367; skin :381
+ *   O-12 switching-mode ensemble MD  PAPER.md:175 (Eq. 6: cheap mean-energy forces every step, the
+ *        per-head pass only every N steps), :71 (uncertainty as stopping criterion), Eq. 5
  *
  * Build: gcc -O2 -std=c11 -fPIC -shared -fopenmp -ffp-contract=off gmnn_oracle.c -lm
  *        (-ffp-contract=off: the neighbour predicate is specified in unfused fp32, reading R20.)
@@ -832,5 +837,103 @@ int oracle_nve(const oracle_hparams *hp, const oracle_weights *w, int64_t N, dou
     free(pl.i);
     free(pl.j);
     free(pl.n3);
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O-12  Switching-mode shallow-ensemble MD ("switch between the two modes during a
+ * simulation ... the more expensive force uncertainty evaluation is only performed every N steps";
+ * stopping criterion PAPER.md:71; Eq. 5, 6).  The loop is O-11 on the MEAN energy
+ * E = 1/M sum_m E^(m) (left-hand side of Eq. 6: head weights 1/M in the backward pass).  After
+ * every sampling_rate-th step (k = 1, 2, ...: after step k * sampling_rate, reading R25) the full
+ * ensemble pass O-10 at the current coordinates gives (Eq. 5, divisor 1/N_ens, reading R13)
+ *   sigma_e[k-1]     = sqrt(1/M sum_m (E^(m) - mean)^2),   E^(m) = sum_i E_i^(m)   (total energy)
+ *   sigma_f_max[k-1] = max_i sqrt(sum_a f_var[i][a])        (Eq. 5 for x = F_i, "implied sum over
+ *                      components"; the worst atom decides, reading R26)
+ * and the run ends after that sample if f_sigma_stop > 0 and sigma_f_max[k-1] > f_sigma_stop.
+ * epot/ekin [n_steps + 1] valid up to index *n_steps_done.  f_var_last [N][3] nullable: f_var of
+ * the last sample.
+ * ------------------------------------------------------------------------------------------ */
+int oracle_md_switching(const oracle_hparams *hp, const oracle_weights *w, int64_t N, double *x, double *v,
+                        const double *masses, const int32_t *species, const double *L, const int32_t *pbc,
+                        double skin, double dt, int64_t n_steps, int64_t sampling_rate, double f_sigma_stop,
+                        double *epot, double *ekin, double *sigma_e, double *sigma_f_max, double *f_var_last,
+                        int64_t *n_steps_done, int64_t *n_samples, int64_t *n_rebuilds) {
+    if (sampling_rate < 1 || hp->n_heads > 64) return -1;
+    const int M = hp->n_heads;
+    pairlist_t pl = {0, 0, NULL, NULL, NULL};
+    double *F = (double *)malloc(sizeof(double) * 3 * (size_t)N);
+    double *Eh = (double *)malloc(sizeof(double) * (size_t)N * M);
+    double *xu = (double *)malloc(sizeof(double) * 3 * (size_t)N);
+    double *xref = (double *)malloc(sizeof(double) * 3 * (size_t)N);
+    double *em = (double *)malloc(sizeof(double) * (size_t)N), *ev = (double *)malloc(sizeof(double) * (size_t)N);
+    double *fm = (double *)malloc(sizeof(double) * 3 * (size_t)N), *fv = (double *)malloc(sizeof(double) * 3 * (size_t)N);
+    double hw[64];
+    for (int m = 0; m < M; ++m) hw[m] = 1.0 / M;
+    int64_t rebuilds = 0, samples = 0, done = 0;
+    for (int64_t i = 0; i < N; ++i)
+        for (int a = 0; a < 3; ++a)
+            if (pbc[a]) x[3 * i + a] -= floor(x[3 * i + a] / L[a]) * L[a];
+    memcpy(xu, x, sizeof(double) * 3 * (size_t)N);
+    memcpy(xref, x, sizeof(double) * 3 * (size_t)N);
+    build_list(&pl, N, x, L, pbc, hp->r_cut + skin);
+    oracle_energy_forces(hp, w, N, xu, species, L, pl.n, pl.i, pl.j, pl.n3, hw, Eh, F, NULL, NULL, NULL, NULL);
+    for (int64_t step = 0;; ++step) {
+        double ep = 0.0, ek = 0.0;
+        for (int64_t i = 0; i < N; ++i) {
+            for (int m = 0; m < M; ++m) ep += hw[m] * Eh[(size_t)i * M + m];
+            ek += 0.5 * masses[i] * (v[3 * i] * v[3 * i] + v[3 * i + 1] * v[3 * i + 1] + v[3 * i + 2] * v[3 * i + 2]);
+        }
+        epot[step] = ep;
+        ekin[step] = ek / ACC_CONV;
+        done = step;
+        if (step > 0 && step % sampling_rate == 0) {
+            oracle_ensemble(hp, w, N, xu, species, L, pl.n, pl.i, pl.j, pl.n3, Eh, em, ev, fm, fv, NULL);
+            double tot[64], mean = 0.0, var = 0.0, worst = 0.0;
+            for (int m = 0; m < M; ++m) {
+                tot[m] = 0.0;
+                for (int64_t i = 0; i < N; ++i) tot[m] += Eh[(size_t)i * M + m];
+                mean += tot[m];
+            }
+            mean /= M;
+            for (int m = 0; m < M; ++m) var += (tot[m] - mean) * (tot[m] - mean);
+            for (int64_t i = 0; i < N; ++i) {
+                const double sf = sqrt(fv[3 * i] + fv[3 * i + 1] + fv[3 * i + 2]);
+                if (sf > worst) worst = sf;
+            }
+            sigma_e[samples] = sqrt(var / M);
+            sigma_f_max[samples] = worst;
+            ++samples;
+            if (f_var_last) memcpy(f_var_last, fv, sizeof(double) * 3 * (size_t)N);
+            if (f_sigma_stop > 0.0 && worst > f_sigma_stop) break;
+        }
+        if (step == n_steps) break;
+        double maxd2 = 0.0;
+        for (int64_t i = 0; i < N; ++i) {
+            double d2 = 0.0;
+            for (int a = 0; a < 3; ++a) {
+                v[3 * i + a] += 0.5 * dt * F[3 * i + a] / masses[i] * ACC_CONV;
+                xu[3 * i + a] += dt * v[3 * i + a];
+                x[3 * i + a] = pbc[a] ? xu[3 * i + a] - floor(xu[3 * i + a] / L[a]) * L[a] : xu[3 * i + a];
+                double dd = xu[3 * i + a] - xref[3 * i + a];
+                d2 += dd * dd;
+            }
+            if (d2 > maxd2) maxd2 = d2;
+        }
+        if (sqrt(maxd2) > 0.5 * skin) {
+            memcpy(xu, x, sizeof(double) * 3 * (size_t)N);
+            memcpy(xref, x, sizeof(double) * 3 * (size_t)N);
+            build_list(&pl, N, x, L, pbc, hp->r_cut + skin);
+            ++rebuilds;
+        }
+        oracle_energy_forces(hp, w, N, xu, species, L, pl.n, pl.i, pl.j, pl.n3, hw, Eh, F, NULL, NULL, NULL, NULL);
+        for (int64_t i = 0; i < N; ++i)
+            for (int a = 0; a < 3; ++a) v[3 * i + a] += 0.5 * dt * F[3 * i + a] / masses[i] * ACC_CONV;
+    }
+    if (n_steps_done) *n_steps_done = done;
+    if (n_samples) *n_samples = samples;
+    if (n_rebuilds) *n_rebuilds = rebuilds;
+    free(F); free(Eh); free(xu); free(xref); free(em); free(ev); free(fm); free(fv);
+    free(pl.i); free(pl.j); free(pl.n3);
     return 0;
 }

@@ -320,3 +320,41 @@ def nve(model: Model, positions, velocities, masses, species, cell, pbc, skin: f
     if rc != 0:
         raise ValueError("oracle_nve: bad argument")
     return NVEResult(x, v, epot, ekin, int(nreb.value))
+
+
+@dataclass
+class SwitchingResult:
+    positions: np.ndarray
+    velocities: np.ndarray
+    epot: np.ndarray  # [n_steps_done + 1], mean energy over the heads
+    ekin: np.ndarray  # [n_steps_done + 1]
+    sigma_e: np.ndarray  # [n_samples]
+    sigma_f_max: np.ndarray  # [n_samples]
+    f_var_last: np.ndarray  # [N][3] of the last sample (zeros if none was taken)
+    n_steps_done: int
+    n_rebuilds: int
+
+
+def md_switching(model: Model, positions, velocities, masses, species, cell, pbc, skin: float, dt_fs: float,
+                 n_steps: int, sampling_rate: int, f_sigma_stop: float = 0.0) -> SwitchingResult:
+    """O-12 switching-mode shallow-ensemble MD (Eq. 5, 6)."""
+    x = _f64(positions).copy()
+    v = _f64(velocities).copy()
+    m = _f64(masses)
+    sp = _i32(species)
+    L = _f64(cell).reshape(-1)
+    pb = _i32(pbc)
+    epot = np.zeros(n_steps + 1)
+    ekin = np.zeros(n_steps + 1)
+    ns_max = max(n_steps // max(sampling_rate, 1), 1)
+    se, sf = np.zeros(ns_max), np.zeros(ns_max)
+    fv = np.zeros((x.shape[0], 3))
+    done, nsamp, nreb = C.c_int64(0), C.c_int64(0), C.c_int64(0)
+    rc = lib().oracle_md_switching(
+        C.byref(model.hp), C.byref(model.w), C.c_int64(x.shape[0]), _p(x), _p(v), _p(m), _p(sp), _p(L), _p(pb),
+        C.c_double(skin), C.c_double(dt_fs), C.c_int64(n_steps), C.c_int64(sampling_rate), C.c_double(f_sigma_stop),
+        _p(epot), _p(ekin), _p(se), _p(sf), _p(fv), C.byref(done), C.byref(nsamp), C.byref(nreb))
+    if rc != 0:
+        raise ValueError("oracle_md_switching: bad argument")
+    d, k = int(done.value), int(nsamp.value)
+    return SwitchingResult(x, v, epot[:d + 1], ekin[:d + 1], se[:k], sf[:k], fv, d, int(nreb.value))
