@@ -186,12 +186,34 @@ int gmnn_ensemble_energy_forces(gmnn_system *s, const float *positions, float *e
  *   masses                 DEVICE float [n_atoms] (amu)
  *   epot_series, ekin_series  DEVICE double [n_steps + 1], nullable; index 0 = state at entry
  *   n_rebuilds             HOST int32*, nullable
+ * On a model with several heads the energy integrated is their mean (left-hand side of Eq. 6).
  * Needs a list built by gmnn_build_neighbors (its cell, pbc and skin are reused).  Synchronises
  * the stream at the end; returns GMNN_NEIGHBOR_OVERFLOW if an in-loop rebuild ran out of slots
  * (results are then invalid; raise "capacity" and retry). */
 int gmnn_md_verlet_steps(gmnn_system *s, float *positions, float *velocities, const float *masses, float dt_fs,
                          int32_t n_steps, double *epot_series, double *ekin_series, int32_t *n_rebuilds,
                          void *cuda_stream);
+
+/* Switching-mode shallow-ensemble MD ("switch between the two modes
+ * during a simulation ... the more expensive force uncertainty evaluation is only performed every N
+ * steps"; stopping criterion PAPER.md:71; Eq. 5, 6).  Velocity Verlet as gmnn_md_verlet_steps on the
+ * MEAN energy of the heads (one backward pass per step).  After steps sampling_rate, 2 sampling_rate, ...
+ * the full ensemble pass of gmnn_ensemble_energy_forces runs at the current positions and sample k gets
+ *   sigma_e_series[k]     = sqrt(1/M sum_m (E^(m) - mean)^2), E^(m) = sum_i E_i^(m) (fp64 sums, fixed order)
+ *   sigma_f_max_series[k] = max_i sqrt(f_var[i][x] + f_var[i][y] + f_var[i][z])
+ * The run ends after a sample with sigma_f_max > f_sigma_stop when f_sigma_stop > 0 (<= 0: never stops).
+ * The samples do not change the trajectory (bit for bit).
+ *   positions, velocities, masses, epot_series, ekin_series   as gmnn_md_verlet_steps (DEVICE); the series
+ *                          are valid up to index *n_steps_done
+ *   sigma_e_series, sigma_f_max_series   HOST double [n_steps / sampling_rate] (the stream is synchronised
+ *                          at every sample to take the stopping decision)
+ *   f_var_last             DEVICE float [n_atoms][3], nullable: force variance of the last sample
+ *   n_steps_done, n_samples, n_rebuilds   HOST int32*, nullable
+ * Works for n_heads = 1 too (all sigma = 0).  Errors as gmnn_md_verlet_steps. */
+int gmnn_md_ensemble_steps(gmnn_system *s, float *positions, float *velocities, const float *masses, float dt_fs,
+                           int32_t n_steps, int32_t sampling_rate, float f_sigma_stop, double *epot_series,
+                           double *ekin_series, double *sigma_e_series, double *sigma_f_max_series, float *f_var_last,
+                           int32_t *n_steps_done, int32_t *n_samples, int32_t *n_rebuilds, void *cuda_stream);
 
 /* Synchronises the stream and reports a deferred device-side condition (GMNN_STALE_NEIGHBORS,
  * GMNN_NEIGHBOR_OVERFLOW, GMNN_OUT_OF_BOX) or GMNN_OK, clearing it. */

@@ -31,7 +31,7 @@ GMNN_FORCE_GATHER, GMNN_FORCE_PAIRBUF = 0, 1
 EXPORTS = (
     "gmnn_n_features", "gmnn_create", "gmnn_destroy", "gmnn_system_create", "gmnn_system_destroy",
     "gmnn_system_set_int", "gmnn_system_get_int", "gmnn_build_neighbors", "gmnn_get_neighbors",
-    "gmnn_energy_forces", "gmnn_energy_forces_host", "gmnn_ensemble_energy_forces", "gmnn_md_verlet_steps",
+    "gmnn_energy_forces", "gmnn_energy_forces_host", "gmnn_ensemble_energy_forces", "gmnn_md_verlet_steps", "gmnn_md_ensemble_steps",
     "gmnn_check", "gmnn_stage_times", "gmnn_debug_read", "gmnn_launch_count", "gmnn_last_error",
 )
 
@@ -75,6 +75,8 @@ def _load() -> C.CDLL:
     lib.gmnn_build_neighbors.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_float, C.c_float, C.c_void_p]
     lib.gmnn_md_verlet_steps.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_float, C.c_int32,
                                          C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.gmnn_md_ensemble_steps.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_float, C.c_int32, C.c_int32,
+                                           C.c_float] + [C.c_void_p] * 9
     lib.gmnn_energy_forces.argtypes = [C.c_void_p] * 6
     lib.gmnn_energy_forces_host.argtypes = [C.c_void_p] * 6
     lib.gmnn_ensemble_energy_forces.argtypes = [C.c_void_p] * 7
@@ -284,6 +286,32 @@ class System:
                                         _dev_ptr(ekin, torch.float64), C.cast(C.byref(nreb), C.c_void_p),
                                         _stream_ptr(stream)))
         return epot, ekin, int(nreb.value)
+
+    def md_ensemble_steps(self, positions, velocities, masses, dt_fs: float, n_steps: int, sampling_rate: int,
+                          f_sigma_stop: float = 0.0, want_f_var: bool = False, stream=None):
+        """In-place switching-mode ensemble MD; returns a dict: epot, ekin (f64 device, [n_steps_done + 1]),
+        sigma_e, sigma_f_max (numpy f64 [n_samples]), f_var (device [N][3] or None), n_steps_done, n_rebuilds."""
+        import torch
+
+        N = self.n_atoms
+        dev = positions.device
+        epot = torch.zeros(n_steps + 1, dtype=torch.float64, device=dev)
+        ekin = torch.zeros(n_steps + 1, dtype=torch.float64, device=dev)
+        cap = max(n_steps // max(sampling_rate, 1), 1)
+        se = np.zeros(cap, np.float64)
+        sf = np.zeros(cap, np.float64)
+        fvar = torch.zeros((N, 3), dtype=torch.float32, device=dev) if want_f_var else None
+        done, nsamp, nreb = C.c_int32(0), C.c_int32(0), C.c_int32(0)
+        _check(lib.gmnn_md_ensemble_steps(
+            self.handle, _dev_ptr(positions, torch.float32, (N, 3)), _dev_ptr(velocities, torch.float32, (N, 3)),
+            _dev_ptr(masses, torch.float32, (N,)), C.c_float(dt_fs), C.c_int32(n_steps), C.c_int32(sampling_rate),
+            C.c_float(f_sigma_stop), _dev_ptr(epot, torch.float64), _dev_ptr(ekin, torch.float64),
+            se.ctypes.data_as(C.c_void_p), sf.ctypes.data_as(C.c_void_p), _dev_ptr(fvar, torch.float32),
+            C.cast(C.byref(done), C.c_void_p), C.cast(C.byref(nsamp), C.c_void_p), C.cast(C.byref(nreb), C.c_void_p),
+            _stream_ptr(stream)))
+        d, k = int(done.value), int(nsamp.value)
+        return {"epot": epot[:d + 1], "ekin": ekin[:d + 1], "sigma_e": se[:k], "sigma_f_max": sf[:k], "f_var": fvar,
+                "n_steps_done": d, "n_rebuilds": int(nreb.value)}
 
     def check(self, stream=None) -> None:
         _check(lib.gmnn_check(self.handle, _stream_ptr(stream)))

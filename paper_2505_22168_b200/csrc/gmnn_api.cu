@@ -104,6 +104,35 @@ static int forward_backward(gmnn_system *s, const float *positions, const float 
     return GMNN_OK;
 }
 
+// a12: one forward, then one backward per head with a one-hot head weight; Welford over the heads.
+// Uses f_tmp as the per-head force buffer.
+static int ensemble_pass(gmnn_system *s, const float *positions, float *e_mean, float *e_var, float *f_mean,
+                         float *f_var, cudaStream_t st) {
+    const int M = s->model->hp.n_heads;
+    int rc;
+    const int keep_profile = s->profile;
+    s->profile = 0;
+    if ((rc = launch_gather_positions(s, positions, st, true))) return rc;
+    if ((rc = launch_pair_forward(s, st))) return rc;
+    if ((rc = launch_contract_forward(s, st))) return rc;
+    if ((rc = mlp_forward(s, st))) return rc;
+    if ((rc = launch_mlp_heads(s, s->model->head_mean_w, st))) return rc;
+    if ((rc = launch_ensemble_energy_stats(s, e_mean, e_var, st))) return rc;
+    for (int m = 0; m < M; ++m) {
+        k_set_onehot<<<1, 64, 0, st>>>(M, m, s->head_w);
+        GMNN_LAUNCHED();
+        if ((rc = mlp_backward(s, s->head_w, st))) return rc;
+        if ((rc = launch_contract_backward(s, st))) return rc;
+        if ((rc = launch_pair_backward(s, st))) return rc;
+        if ((rc = launch_scatter_outputs(s, nullptr, s->f_tmp, st))) return rc;
+        if ((rc = launch_welford(s, m, s->f_tmp, f_mean, f_var, st))) return rc;
+    }
+    if ((rc = launch_finish_var(3 * s->N, f_var, M, st))) return rc;
+    s->profile = keep_profile;
+    GMNN_CUDA(cudaGetLastError());
+    return GMNN_OK;
+}
+
 }  // namespace gmnn
 
 using namespace gmnn;
@@ -300,7 +329,7 @@ int gmnn_system_create(const gmnn_model *m, int64_t n_atoms, const int32_t *spec
     A_(s->f_int, 3 * N);
     A_(s->f_tmp, 3 * N);
     A_(s->partial, 2 * 1024);
-    A_(s->e_total, 2);
+    A_(s->e_total, 4);  // epot, ekin, sigma_E, bits of sigma_F,max (switching-mode samples)
     A_(s->flags, FLAG_WORDS);
 #undef A_
     if (!rc && cudaMallocHost((void **)&s->flags_host, sizeof(int32_t) * FLAG_WORDS) != cudaSuccess) rc = GMNN_OOM;
@@ -328,7 +357,7 @@ void gmnn_system_destroy(gmnn_system *s) {
     for (int l = 0; l < MAX_LAYERS; ++l) { dev_free(s->H[l]); dev_free(s->D[l]); }
     dev_free(s->dZ[0]); dev_free(s->dZ[1]); dev_free(s->Bv); dev_free(s->BvT); dev_free(s->BvTs); dev_free(s->BvTh); dev_free(s->amax); dev_free(s->vhead); dev_free(s->head_w);
     dev_free(s->ypart); dev_free(s->e_heads); dev_free(s->e_atom); dev_free(s->f_int); dev_free(s->f_tmp); dev_free(s->partial);
-    dev_free(s->e_total); dev_free(s->flags);
+    dev_free(s->e_total); dev_free(s->flags); dev_free(s->ens_scratch);
     dev_free(s->stage_pos); dev_free(s->stage_f); dev_free(s->stage_e);
     if (s->flags_host) cudaFreeHost(s->flags_host);
     for (cudaEvent_t e : s->events) cudaEventDestroy(e);
@@ -662,31 +691,8 @@ int gmnn_ensemble_energy_forces(gmnn_system *s, const float *positions, float *e
         set_error("no neighbour list: call gmnn_build_neighbors first");
         return GMNN_INVALID_ARG;
     }
-    cudaStream_t st = (cudaStream_t)cuda_stream;
-    const int M = s->model->hp.n_heads;
-    int rc;
     s->md_state_valid = false;
-    const int keep_profile = s->profile;
-    s->profile = 0;
-    if ((rc = launch_gather_positions(s, positions, st, true))) return rc;
-    if ((rc = launch_pair_forward(s, st))) return rc;
-    if ((rc = launch_contract_forward(s, st))) return rc;
-    if ((rc = mlp_forward(s, st))) return rc;
-    if ((rc = launch_mlp_heads(s, s->model->head_mean_w, st))) return rc;
-    if ((rc = launch_ensemble_energy_stats(s, e_mean, e_var, st))) return rc;
-    for (int m = 0; m < M; ++m) {
-        k_set_onehot<<<1, 64, 0, st>>>(M, m, s->head_w);
-        GMNN_LAUNCHED();
-        if ((rc = mlp_backward(s, s->head_w, st))) return rc;
-        if ((rc = launch_contract_backward(s, st))) return rc;
-        if ((rc = launch_pair_backward(s, st))) return rc;
-        if ((rc = launch_scatter_outputs(s, nullptr, s->f_tmp, st))) return rc;
-        if ((rc = launch_welford(s, m, s->f_tmp, f_mean, f_var, st))) return rc;
-    }
-    if ((rc = launch_finish_var(3 * s->N, f_var, M, st))) return rc;
-    s->profile = keep_profile;
-    GMNN_CUDA(cudaGetLastError());
-    return GMNN_OK;
+    return ensemble_pass(s, positions, e_mean, e_var, f_mean, f_var, (cudaStream_t)cuda_stream);
 }
 
 int gmnn_md_verlet_steps(gmnn_system *s, float *positions, float *velocities, const float *masses, float dt_fs,
@@ -699,10 +705,6 @@ int gmnn_md_verlet_steps(gmnn_system *s, float *positions, float *velocities, co
     if (!s->have_list) {
         set_error("no neighbour list: call gmnn_build_neighbors first");
         return GMNN_INVALID_ARG;
-    }
-    if (s->model->hp.n_heads != 1) {
-        set_error("MD runs on a single-head model (mean-energy MD of ensembles: DESIGN.md NEXT-1)");
-        return GMNN_UNSUPPORTED;
     }
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const float hs = 0.5f * s->skin;
@@ -806,6 +808,67 @@ int gmnn_md_verlet_steps(gmnn_system *s, float *positions, float *velocities, co
     }
     s->md_state_valid = true;
     return GMNN_OK;
+}
+
+int gmnn_md_ensemble_steps(gmnn_system *s, float *positions, float *velocities, const float *masses, float dt_fs,
+                           int32_t n_steps, int32_t sampling_rate, float f_sigma_stop, double *epot_series,
+                           double *ekin_series, double *sigma_e_series, double *sigma_f_max_series, float *f_var_last,
+                           int32_t *n_steps_done, int32_t *n_samples, int32_t *n_rebuilds, void *cuda_stream) {
+    if (!s || !positions || !velocities || !masses || n_steps < 0 || sampling_rate < 1 || !(dt_fs > 0.f) ||
+        (n_steps >= sampling_rate && (!sigma_e_series || !sigma_f_max_series))) {
+        set_error("gmnn_md_ensemble_steps: bad argument");
+        return GMNN_INVALID_ARG;
+    }
+    if (!s->have_list) {
+        set_error("no neighbour list: call gmnn_build_neighbors first");
+        return GMNN_INVALID_ARG;
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const int64_t N = s->N;
+    int rc;
+    if (!s->ens_scratch && (rc = dev_alloc(&s->ens_scratch, (size_t)11 * N))) return rc;
+    float *const f_keep = s->ens_scratch, *const e_mean = f_keep + 3 * N, *const e_var = e_mean + N,
+                 *const f_mean = e_var + N, *const f_var = f_mean + 3 * N;
+    double *const sig_e = s->e_total + 2;
+    int32_t *const sig_f_bits = (int32_t *)(s->e_total + 3);
+    const int keep_continue = s->md_continue;
+    int32_t done = 0, samples = 0, rebuilds = 0;
+    bool stopped = false;
+    rc = GMNN_OK;
+    while (done < n_steps && !stopped) {
+        // the cheap mode (left-hand side of Eq. 6): sampling_rate steps on the mean energy, one backward each
+        const int32_t chunk = (n_steps - done < sampling_rate) ? n_steps - done : sampling_rate;
+        int32_t nreb = 0;
+        s->md_continue = (done > 0) ? 1 : keep_continue;
+        rc = gmnn_md_verlet_steps(s, positions, velocities, masses, dt_fs, chunk, epot_series ? epot_series + done : nullptr,
+                                  ekin_series ? ekin_series + done : nullptr, &nreb, cuda_stream);
+        if (rc) break;
+        done += chunk;
+        rebuilds += nreb;
+        if (chunk < sampling_rate) break;
+        // the expensive mode (right-hand side): one backward per head at the current positions.  The pass
+        // borrows f_tmp; the mean-energy forces of the last step are put back afterwards so that the
+        // trajectory is bit-for-bit the one without samples.
+        GMNN_CUDA(cudaMemcpyAsync(f_keep, s->f_tmp, sizeof(float) * 3 * N, cudaMemcpyDeviceToDevice, st));
+        if ((rc = ensemble_pass(s, positions, e_mean, e_var, f_mean, f_var, st))) break;
+        if ((rc = launch_uncertainty_scalars(s, f_var, sig_e, sig_f_bits, st))) break;
+        GMNN_CUDA(cudaMemcpyAsync(s->f_tmp, f_keep, sizeof(float) * 3 * N, cudaMemcpyDeviceToDevice, st));
+        if (f_var_last) GMNN_CUDA(cudaMemcpyAsync(f_var_last, f_var, sizeof(float) * 3 * N, cudaMemcpyDeviceToDevice, st));
+        double se = 0.0;
+        float sf = 0.f;
+        GMNN_CUDA(cudaMemcpyAsync(&se, sig_e, sizeof(double), cudaMemcpyDeviceToHost, st));
+        GMNN_CUDA(cudaMemcpyAsync(&sf, sig_f_bits, sizeof(float), cudaMemcpyDeviceToHost, st));
+        GMNN_CUDA(cudaStreamSynchronize(st));
+        sigma_e_series[samples] = se;
+        sigma_f_max_series[samples] = (double)sf;
+        ++samples;
+        if (f_sigma_stop > 0.f && sf > f_sigma_stop) stopped = true;
+    }
+    s->md_continue = keep_continue;
+    if (n_steps_done) *n_steps_done = done;
+    if (n_samples) *n_samples = samples;
+    if (n_rebuilds) *n_rebuilds = rebuilds;
+    return rc;
 }
 
 int gmnn_check(gmnn_system *s, void *cuda_stream) {

@@ -128,7 +128,8 @@ struct gmnn_system {
     float *f_int = nullptr;          // [N][3]
     float *f_tmp = nullptr;          // [N][3] caller order (ensemble, MD)
     double *partial = nullptr;       // reduction scratch
-    double *e_total = nullptr;       // [2] device scalars (epot, ekin)
+    double *e_total = nullptr;       // [4] device scalars (epot, ekin, sigma_E, bits of sigma_F,max)
+    float *ens_scratch = nullptr;    // [11 N] switching-mode samples: kept forces, e_mean, e_var, f_mean, f_var (lazy)
     int32_t *flags = nullptr;        // FLAG_WORDS
     int32_t *flags_host = nullptr;   // pinned
     // knobs
@@ -184,5 +185,6 @@ int launch_series_reset(gmnn_system *s, int32_t next_index, cudaStream_t st);
 int launch_welford(gmnn_system *s, int head, const float *f_head, float *f_mean, float *f_m2, cudaStream_t st);
 int launch_ensemble_energy_stats(gmnn_system *s, float *e_mean, float *e_var, cudaStream_t st);
 int launch_finish_var(int64_t n, float *m2, int n_heads, cudaStream_t st);
+int launch_uncertainty_scalars(gmnn_system *s, const float *f_var, double *out_d, int32_t *out_bits, cudaStream_t st);
 
 }  // namespace gmnn

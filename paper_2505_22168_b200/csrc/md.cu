@@ -236,4 +236,64 @@ int launch_ensemble_energy_stats(gmnn_system *s, float *e_mean, float *e_var, cu
     return GMNN_OK;
 }
 
+// ---- uncertainty scalars of a switching-mode sample (SURVEY 8(f) NEXT-1; PAPER.md:75-77 Eq. 5, :71, :175) ----
+// Total energy of every head, E^(m) = sum_i E_i^(m), in fp64 and in a fixed order: block (b, m) sums
+// head m over a contiguous slice of atoms, one block per head adds the slices.
+__global__ void __launch_bounds__(256) k_head_totals_stage1(int64_t N, int M, const float *__restrict__ e_heads,
+                                                            double *partial) {
+    const int m = blockIdx.y;
+    const int64_t per = (N + gridDim.x - 1) / gridDim.x;
+    const int64_t b = blockIdx.x * per, e = (b + per < N) ? b + per : N;
+    double v = 0.0;
+    for (int64_t q = b + threadIdx.x; q < e; q += blockDim.x) v += (double)e_heads[q * M + m];
+    v = block_sum(v);
+    if (threadIdx.x == 0) partial[(int64_t)m * gridDim.x + blockIdx.x] = v;
+}
+
+// sigma_E = sqrt(1/M sum_m (E^(m) - mean)^2): one block, thread m owns head m (M <= 64)
+__global__ void __launch_bounds__(64) k_sigma_e(int nb, int M, const double *__restrict__ partial, double *out) {
+    __shared__ double tot[64];
+    const int m = threadIdx.x;
+    if (m < M) {
+        double v = 0.0;
+        for (int b = 0; b < nb; ++b) v += partial[(int64_t)m * nb + b];
+        tot[m] = v;
+    }
+    __syncthreads();
+    if (m == 0) {
+        double mean = 0.0, var = 0.0;
+        for (int q = 0; q < M; ++q) mean += tot[q];
+        mean /= (double)M;
+        for (int q = 0; q < M; ++q) var += (tot[q] - mean) * (tot[q] - mean);
+        *out = sqrt(var / (double)M);
+    }
+}
+
+// max_i sqrt(f_var[i][x] + f_var[i][y] + f_var[i][z]); a maximum of non-negative floats does not depend
+// on the order, so an integer atomicMax on the bit pattern keeps the result deterministic
+__global__ void __launch_bounds__(256) k_sigma_f_max(int64_t N, const float *__restrict__ f_var, int32_t *out_bits) {
+    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    float v = 0.f;
+    if (i < N) v = sqrtf(f_var[3 * i] + f_var[3 * i + 1] + f_var[3 * i + 2]);
+#pragma unroll
+    for (int o = 16; o >= 1; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
+    if ((threadIdx.x & 31) == 0 && v > 0.f) atomicMax(out_bits, __float_as_int(v));
+}
+
+// out: double sigma_e at out_d[0]; float bits of sigma_f_max at out_bits[0] (zeroed here first)
+int launch_uncertainty_scalars(gmnn_system *s, const float *f_var, double *out_d, int32_t *out_bits, cudaStream_t st) {
+    const int M = s->model->hp.n_heads;
+    int nb = red_blocks(s->N);
+    if (nb * M > 2 * RED_BLOCKS) nb = 2 * RED_BLOCKS / M;  // partial holds 2 * RED_BLOCKS doubles
+    GMNN_CUDA(cudaMemsetAsync(out_bits, 0, sizeof(int32_t), st));
+    k_head_totals_stage1<<<dim3(nb, M), 256, 0, st>>>(s->N, M, s->e_heads, s->partial);
+    GMNN_LAUNCHED();
+    k_sigma_e<<<1, 64, 0, st>>>(nb, M, s->partial, out_d);
+    GMNN_LAUNCHED();
+    k_sigma_f_max<<<nblocks(s->N, 256), 256, 0, st>>>(s->N, f_var, out_bits);
+    GMNN_LAUNCHED();
+    GMNN_CUDA(cudaGetLastError());
+    return GMNN_OK;
+}
+
 }  // namespace gmnn
