@@ -253,6 +253,57 @@ def whole_job_value(n_atoms: int, steps: int, world: int, ms_max: float) -> floa
 # ------------------------------------------------------------------------------------------------
 # our arm
 # ------------------------------------------------------------------------------------------------
+SWITCHING_MD_STEPS = 200
+
+
+def run_switching(args):
+    """--workload config4_switching: the paper's switching-mode claim ("prediction times are
+    nearly independent of the number of ensemble members") on the config-4 box under MD: ms per step of
+    gmnn_md_ensemble_steps at several sampling rates against the same MD on a single-head model.  A side
+    measurement (one GPU, graph-replayed MD loop), not the round's headline line."""
+    import torch
+
+    import paper_2505_22168_b200 as gm
+    import workloads as wl
+
+    torch.cuda.set_device(0)
+    n = SWITCHING_MD_STEPS
+    prec, fmode = MLP_NAMES[args.mlp], {"gather": 0, "pairbuf": 1}[args.forces]
+
+    def timed(n_heads, rate):
+        w = wl.li3po4_box(8192, n_heads=n_heads, skin=0.5)
+        sysm = gm.System(gm.Model(w.model, mlp_precision=prec, force_mode=fmode), w.species)
+        pos = torch.from_numpy(w.positions).cuda()
+        vel = torch.from_numpy(w.velocities).cuda()
+        mass = torch.from_numpy(w.masses).cuda()
+        sysm.build_neighbors(pos, w.cell9, w.pbc, w.model.r_cut, w.skin)
+        sysm.md_ensemble_steps(pos, vel, mass, w.dt_fs, max(args.warmup, 3) * 4, 4)  # warm-up, both modes
+        torch.cuda.synchronize()
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev0.record()
+        out = sysm.md_ensemble_steps(pos, vel, mass, w.dt_fs, n, rate)
+        ev1.record()
+        torch.cuda.synchronize()
+        assert out["n_steps_done"] == n
+        return ev0.elapsed_time(ev1) / n, len(out["sigma_e"]), out["n_rebuilds"]
+
+    rows = {}
+    for label, heads, rate in (("single_head", 1, 10 ** 9), ("m32_never", 32, 10 ** 9), ("m32_every_100", 32, 100),
+                               ("m32_every_10", 32, 10), ("m32_every_1", 32, 1)):
+        ms, ns, nreb = timed(heads, rate)
+        rows[label] = {"ms_per_step": round(ms, 4), "samples": ns, "rebuilds": nreb}
+    ms = rows["m32_every_100"]["ms_per_step"]
+    print(json.dumps({
+        "metric": "atom-steps/s (switching-mode shallow-ensemble MD)", "value": 8192 / (ms * 1e-3),
+        "unit": "atom-steps/s", "n_gpus": 1, "steps": n, "warmup": max(args.warmup, 3) * 4, "ms_per_step": ms,
+        "higher_is_better": True, "vs_baseline": None, "data": "synthetic", "dtype": "f32 (MLP mode: %s)" % args.mlp,
+        "config": {"workload": "config4_switching", "n_atoms": 8192, "n_heads": 32, "skin": 0.5, "sampling_rate": 100,
+                   "what": "li3po4_8192 with 32 heads, NVE on the mean energy, per-head pass every sampling_rate steps",
+                   "mlp": args.mlp, "forces": args.forces},
+        "rates": rows, "gpu_launches": int(gm.launch_count())}))
+    return 0
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -447,7 +498,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="config5",
-                    help="config5 (default, 1,048,576 atoms), config2, config3_<N>")
+                    help="config5 (default, 1,048,576 atoms), config2, config3_<N>; config4_switching: side measurement of "
+                         "the switching-mode ensemble MD (its own JSON line)")
     ap.add_argument("--mlp", default="3xf16", choices=sorted(MLP_NAMES),
                     help="3xf16 (default) / 3xtf32: tcgen05 tensor cores, fp32-accurate three-product split on fp16 / tf32 "
                          "operands; fp32: SIMT FMA; tf32: single pass")
@@ -459,6 +511,8 @@ def main():
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.workload == "config4_switching":
+        return run_switching(args)
     return run_ours(args)
 
 

@@ -245,6 +245,18 @@ int gmnn_create(const gmnn_hparams *hp, const gmnn_weights *w, gmnn_model **out)
         std::vector<float> hw(hp->n_heads, 1.f / (float)hp->n_heads);
         rc = upload(&m->head_mean_w, hw.data(), hw.size());
     }
+    if (!rc) {
+        // the mean of the heads is itself one linear head (Eq. 6, left-hand side): w_mean = W_last 1/M, b_mean
+        const int L = hp->n_hidden, Hd = m->dims[L], M = hp->n_heads;
+        std::vector<float> wm((size_t)Hd + 1);
+        for (int k = 0; k <= Hd; ++k) {
+            const float *row = (k < Hd) ? w->W[L] + (size_t)k * M : w->b[L];
+            double acc = 0.0;
+            for (int q = 0; q < M; ++q) acc += (double)row[q];
+            wm[k] = (float)(acc / M);
+        }
+        rc = upload(&m->w_mean, wm.data(), wm.size());
+    }
     if (rc) {
         gmnn_destroy(m);
         return rc;
@@ -256,6 +268,7 @@ int gmnn_create(const gmnn_hparams *hp, const gmnn_weights *w, gmnn_model **out)
 void gmnn_destroy(gmnn_model *m) {
     if (!m) return;
     dev_free(m->beta);
+    dev_free(m->w_mean);
     for (int l = 0; l < MAX_LAYERS; ++l) {
         dev_free(m->W[l]);
         dev_free(m->WT[l]);
@@ -712,6 +725,13 @@ int gmnn_md_verlet_steps(gmnn_system *s, float *positions, float *velocities, co
     int rc;
     StageTimer T(s, st);
     T.begin();
+    // several heads: the integrated energy is their mean, evaluated as ONE folded head (model->w_mean) so that
+    // a step costs what it costs on a single-head model; e_heads is not produced in the loop
+    struct MeanHead {
+        gmnn_system *s;
+        ~MeanHead() { s->use_mean_head = false; }
+    } mean_head_guard{s};
+    s->use_mean_head = s->model->hp.n_heads > 1;
     double *const ep = s->e_total, *const ek = s->e_total + 1;  // energies of the latest step (device)
     if (s->md_continue && s->md_state_valid) {
         // the caller continues the trajectory of the previous call: f_tmp, e_total are current

@@ -80,6 +80,7 @@ struct gmnn_model {
     float *b[gmnn::MAX_LAYERS] = {};
     float *scale = nullptr, *shift = nullptr;  // [S]
     float *head_mean_w = nullptr;  // [n_heads] = 1/M (device)
+    float *w_mean = nullptr;       // [H_last + 1]: W_last 1/M and, last, mean(b_last): the mean of the heads as one head
 };
 
 struct gmnn_system {
@@ -121,6 +122,7 @@ struct gmnn_system {
     float *vhead = nullptr;          // [H_last]
     float *head_w = nullptr;         // [n_heads] weights of the differentiated energy
     float *ypart = nullptr;          // [MAX_HEAD_SLOTS][N padded to 128]: partial head sums (mlp_tc.cu EPI_HIDDEN_HEAD)
+    bool use_mean_head = false;      // MD on a multi-head model: forward with model->w_mean as the only head
     bool heads_fused = false;        // the last mlp_forward left ypart instead of H[L-1]
     int head_slots = 0;
     float *e_heads = nullptr;        // [N][n_heads]

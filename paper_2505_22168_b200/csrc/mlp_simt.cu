@@ -210,17 +210,24 @@ __global__ void k_heads_finish(int64_t N, const float *__restrict__ ypart, int n
     for (int q = 0; q < n_slots; ++q) y += __ldg(ypart + q * m_pad + i);
     const int z = __float_as_int(pos4[i].w);
     const float em = __ldg(&scale[z]) * (y + __ldg(&bl[0])) + __ldg(&shift[z]);
-    e_heads[i] = em;
-    e_atom[i] = __ldg(&head_w[0]) * em;
+    if (e_heads) {
+        e_heads[i] = em;
+        e_atom[i] = __ldg(&head_w[0]) * em;
+    } else {  // folded mean head of a multi-head model (MD): the head's value is the energy
+        e_atom[i] = em;
+    }
 }
 
 int launch_mlp_heads(gmnn_system *s, const float *head_w_dev, cudaStream_t st) {
     const gmnn_model *m = s->model;
     const int L = m->hp.n_hidden;
     if (s->heads_fused) {
+        const bool mean = m->hp.n_heads > 1;  // fused on a multi-head model: the folded mean head (use_mean_head)
         k_heads_finish<<<(unsigned)((s->N + 255) / 256), 256, 0, st>>>(s->N, s->ypart, s->head_slots,
-                                                                        (s->N + 127) / 128 * 128, m->b[L], s->pos4, m->scale,
-                                                                        m->shift, head_w_dev, s->e_heads, s->e_atom);
+                                                                        (s->N + 127) / 128 * 128,
+                                                                        mean ? m->w_mean + m->dims[L] : m->b[L], s->pos4,
+                                                                        m->scale, m->shift, head_w_dev,
+                                                                        mean ? nullptr : s->e_heads, s->e_atom);
         GMNN_LAUNCHED();
         GMNN_CUDA(cudaGetLastError());
         return GMNN_OK;

@@ -947,13 +947,14 @@ int launch_mlp_forward_tc(gmnn_system *s, cudaStream_t st) {
     for (int l = 0; l < m->hp.n_hidden; ++l) {
         // z = X W[l]: the B operand is W[l]^T = WT[l], [fan_out][fan_in]
         // single head: the last hidden layer's epilogue takes the head's dot product itself
-        const bool fuse = l == m->hp.n_hidden - 1 && m->hp.n_heads == 1 && 2 * ((m->dims[l + 1] + 127) / 128) <= MAX_HEAD_SLOTS;
+        const bool fuse = l == m->hp.n_hidden - 1 && (m->hp.n_heads == 1 || s->use_mean_head) && 2 * ((m->dims[l + 1] + 127) / 128) <= MAX_HEAD_SLOTS;
         s->heads_fused = fuse;
         TcHalf hf;
         hf.Bh = m->WTh[l], hf.amax_b = m->wmax + l;
         hf.amax_a = s->amax + (l == 0 ? AMAX_G : AMAX_H + l - 1), hf.amax_out = s->amax + AMAX_H + l;
         int rc = tc_gemm(split, fuse ? EPI_HIDDEN_HEAD : EPI_HIDDEN, s->N, m->dims[l + 1], m->dims[l], X,
-                         split ? m->WTs[l] : m->WT[l], s->H[l], m->b[l], s->D[l], nullptr, st, m->W[l + 1], s->ypart,
+                         split ? m->WTs[l] : m->WT[l], s->H[l], m->b[l], s->D[l], nullptr, st,
+                         (fuse && s->use_mean_head) ? m->w_mean : m->W[l + 1], s->ypart,
                          &s->head_slots, f16 ? &hf : nullptr);
         if (rc) return rc;
         X = s->H[l];
