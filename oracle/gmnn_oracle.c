@@ -31,6 +31,8 @@
  *   O-11 NVE velocity Verlet ...... BASELINE.json configs 2, 5; dt PAPER.md:367; skin :381
  *   O-12 switching-mode ensemble MD  PAPER.md:175 (Eq. 6: cheap mean-energy forces every step, the
  *        per-head pass only every N steps), :71 (uncertainty as stopping criterion), Eq. 5
+ *   O-13 UDD bias (gmnn_oracle.py, numpy on O-10's per-head forces)  PAPER.md:102-107 (Eq. 9); pins in
+ *        tests/test_oracle_udd.py: forces == finite differences of mean + E_b, limits of Eq. 9, conservation
  *
  * Build: gcc -O2 -std=c11 -fPIC -shared -fopenmp -ffp-contract=off gmnn_oracle.c -lm
  *        (-ffp-contract=off: the neighbour predicate is specified in unfused fp32, reading R20.)

@@ -358,3 +358,65 @@ def md_switching(model: Model, positions, velocities, masses, species, cell, pbc
         raise ValueError("oracle_md_switching: bad argument")
     d, k = int(done.value), int(nsamp.value)
     return SwitchingResult(x, v, epot[:d + 1], ekin[:d + 1], se[:k], sf[:k], fv, d, int(nreb.value))
+
+
+@dataclass
+class UDDResult:
+    energy: float  # mean energy of the heads + bias
+    e_mean: float
+    e_bias: float
+    var_e: float  # sigma_E^2 of Eq. 5 (total energies, 1/N_ens)
+    forces: np.ndarray  # [N][3] = -d(energy)/dR
+
+
+def udd_energy_forces(model: Model, positions, species, cell, pairs: Pairs, A: float, B: float) -> UDDResult:
+    """O-13 uncertainty-driven-dynamics bias (Eq. 9):
+    E_b = A [exp(-sigma_E^2 / (N_ens N_atoms B^2)) - 1], sigma_E^2 = 1/N_ens sum_m (E^(m) - mean)^2 of the TOTAL
+    energies (Eq. 5, reading R27).  Forces of mean + E_b by the chain rule on the per-head forces of O-10:
+    -grad sigma^2 = 2/N_ens sum_m (E^(m) - mean) (F^(m) - F_mean)."""
+    ens = ensemble(model, positions, species, cell, pairs, keep_heads=True)
+    M, N = model.n_heads, ens.e_heads.shape[0]
+    tot = ens.e_heads.sum(0)
+    mean = tot.mean()
+    var = ((tot - mean) ** 2).mean()
+    width = M * N * B * B
+    e_b = A * (np.exp(-var / width) - 1.0)
+    de_b = -A / width * np.exp(-var / width)  # dE_b / d sigma^2
+    neg_grad_var = (2.0 / M) * np.einsum("m,mia->ia", tot - mean, ens.f_heads - ens.f_mean[None])
+    forces = ens.f_mean + de_b * neg_grad_var
+    return UDDResult(float(mean + e_b), float(mean), float(e_b), float(var), forces)
+
+
+def nve_udd(model: Model, positions, velocities, masses, species, cell, pbc, dt_fs: float, n_steps: int,
+            A: float, B: float):
+    """O-11's velocity Verlet on the biased energy of O-13, with a fresh list of radius r_cut at every step
+    (the trajectory does not depend on the skin: pinned for O-11).  Returns x, v, epot[n+1], ekin[n+1], e_bias[n+1]."""
+    ACC = 9.648533212e-3
+    x = _f64(positions).copy()
+    v = _f64(velocities).copy()
+    m = _f64(masses)[:, None]
+    L = _f64(cell).reshape(-1)
+    per = np.asarray(pbc).astype(bool)
+
+    def wrap(y):
+        y = y.copy()
+        y[:, per] -= np.floor(y[:, per] / L[per]) * L[per]
+        return y
+
+    def evaluate(y):
+        y32 = y.astype(np.float32)  # the neighbour predicate is specified in fp32 (R20); E and F use the fp64 y
+        y32 = np.where(y32 >= np.asarray(cell, np.float32).reshape(-1)[None, :], np.float32(0), y32)
+        return udd_energy_forces(model, y, species, cell, auto_neighbors(y32, cell, pbc, model.r_cut), A, B)
+
+    x = wrap(x)
+    r = evaluate(x)
+    epot, ekin, eb = [r.energy], [0.5 * (m * v * v).sum() / ACC], [r.e_bias]
+    for _ in range(n_steps):
+        v += 0.5 * dt_fs * r.forces / m * ACC
+        x = wrap(x + dt_fs * v)
+        r = evaluate(x)
+        v += 0.5 * dt_fs * r.forces / m * ACC
+        epot.append(r.energy)
+        ekin.append(0.5 * (m * v * v).sum() / ACC)
+        eb.append(r.e_bias)
+    return x, v, np.array(epot), np.array(ekin), np.array(eb)
