@@ -215,6 +215,17 @@ int gmnn_md_ensemble_steps(gmnn_system *s, float *positions, float *velocities, 
                            double *ekin_series, double *sigma_e_series, double *sigma_f_max_series, float *f_var_last,
                            int32_t *n_steps_done, int32_t *n_samples, int32_t *n_rebuilds, void *cuda_stream);
 
+/* Uncertainty-driven-dynamics bias (Eq. 9) on a model with several
+ * heads:  E_b = A [exp(-sigma_E^2 / (N_ens N_atoms B^2)) - 1],  sigma_E^2 = 1/N_ens sum_m (E^(m) - mean)^2 of the
+ * heads' TOTAL energies (Eq. 5).  While A != 0, gmnn_energy_forces, gmnn_energy_forces_host, gmnn_md_verlet_steps and
+ * gmnn_md_ensemble_steps return the energy mean + E_b and its forces (one backward pass with head weights
+ * 1/M + E_b' 2/M (E^(m) - mean)); per-atom energies stay the unbiased mean; gmnn_ensemble_energy_forces and the
+ * uncertainty samples are never biased.  A, B in eV; A = 0 switches the bias off (B is then ignored); B > 0.
+ * No effect on single-head models (sigma_E = 0). */
+int gmnn_system_set_udd_bias(gmnn_system *s, float A, float B);
+/* E_b and sigma_E^2 of the latest biased evaluation (zeros if it was not biased); HOST doubles; synchronises. */
+int gmnn_system_get_udd_bias(gmnn_system *s, double *e_bias /*HOST*/, double *var_e /*HOST*/, void *cuda_stream);
+
 /* Synchronises the stream and reports a deferred device-side condition (GMNN_STALE_NEIGHBORS,
  * GMNN_NEIGHBOR_OVERFLOW, GMNN_OUT_OF_BOX) or GMNN_OK, clearing it. */
 int gmnn_check(gmnn_system *s, void *cuda_stream);

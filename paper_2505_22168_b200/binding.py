@@ -31,7 +31,7 @@ GMNN_FORCE_GATHER, GMNN_FORCE_PAIRBUF = 0, 1
 EXPORTS = (
     "gmnn_n_features", "gmnn_create", "gmnn_destroy", "gmnn_system_create", "gmnn_system_destroy",
     "gmnn_system_set_int", "gmnn_system_get_int", "gmnn_build_neighbors", "gmnn_get_neighbors",
-    "gmnn_energy_forces", "gmnn_energy_forces_host", "gmnn_ensemble_energy_forces", "gmnn_md_verlet_steps", "gmnn_md_ensemble_steps",
+    "gmnn_energy_forces", "gmnn_energy_forces_host", "gmnn_ensemble_energy_forces", "gmnn_md_verlet_steps", "gmnn_md_ensemble_steps", "gmnn_system_set_udd_bias", "gmnn_system_get_udd_bias",
     "gmnn_check", "gmnn_stage_times", "gmnn_debug_read", "gmnn_launch_count", "gmnn_last_error",
 )
 
@@ -77,6 +77,8 @@ def _load() -> C.CDLL:
                                          C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
     lib.gmnn_md_ensemble_steps.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_float, C.c_int32, C.c_int32,
                                            C.c_float] + [C.c_void_p] * 9
+    lib.gmnn_system_set_udd_bias.argtypes = [C.c_void_p, C.c_float, C.c_float]
+    lib.gmnn_system_get_udd_bias.argtypes = [C.c_void_p] * 4
     lib.gmnn_energy_forces.argtypes = [C.c_void_p] * 6
     lib.gmnn_energy_forces_host.argtypes = [C.c_void_p] * 6
     lib.gmnn_ensemble_energy_forces.argtypes = [C.c_void_p] * 7
@@ -312,6 +314,16 @@ class System:
         d, k = int(done.value), int(nsamp.value)
         return {"epot": epot[:d + 1], "ekin": ekin[:d + 1], "sigma_e": se[:k], "sigma_f_max": sf[:k], "f_var": fvar,
                 "n_steps_done": d, "n_rebuilds": int(nreb.value)}
+
+    def set_udd_bias(self, A: float, B: float = 1.0) -> None:
+        _check(lib.gmnn_system_set_udd_bias(self.handle, C.c_float(A), C.c_float(B)))
+
+    def get_udd_bias(self, stream=None) -> Tuple[float, float]:
+        """(E_b, sigma_E^2) of the latest biased evaluation."""
+        eb, var = C.c_double(0), C.c_double(0)
+        _check(lib.gmnn_system_get_udd_bias(self.handle, C.cast(C.byref(eb), C.c_void_p),
+                                            C.cast(C.byref(var), C.c_void_p), _stream_ptr(stream)))
+        return float(eb.value), float(var.value)
 
     def check(self, stream=None) -> None:
         _check(lib.gmnn_check(self.handle, _stream_ptr(stream)))

@@ -83,6 +83,8 @@ static int mlp_backward(gmnn_system *s, const float *head_w, cudaStream_t st) {
 static int forward_backward(gmnn_system *s, const float *positions, const float *head_w, bool check_stale,
                             cudaStream_t st, StageTimer &T) {
     int rc;
+    s->udd_active = s->udd_A != 0.f && s->model->hp.n_heads > 1 && head_w == s->model->head_mean_w;
+    if (s->udd_active) s->use_mean_head = false;  // the bias needs every head's energy
     if ((rc = launch_gather_positions(s, positions, st, check_stale))) return rc;
     T.mark("gather");
     if (s->mlp_precision == GMNN_MLP_3XF16)  // maxima of G, H, dZ: rebuilt by this evaluation's kernels
@@ -94,6 +96,10 @@ static int forward_backward(gmnn_system *s, const float *positions, const float 
     if ((rc = mlp_forward(s, st))) return rc;
     T.mark("mlp_forward");
     if ((rc = launch_mlp_heads(s, head_w, st))) return rc;
+    if (s->udd_active) {  // UDD bias: the head weights of the backward come from this forward's head totals
+        if ((rc = launch_udd_weights(s, s->head_w, s->e_total + 4, st))) return rc;
+        head_w = s->head_w;
+    }
     T.mark("mlp_heads");
     if ((rc = mlp_backward(s, head_w, st))) return rc;
     T.mark("mlp_backward");
@@ -342,7 +348,7 @@ int gmnn_system_create(const gmnn_model *m, int64_t n_atoms, const int32_t *spec
     A_(s->f_int, 3 * N);
     A_(s->f_tmp, 3 * N);
     A_(s->partial, 2 * 1024);
-    A_(s->e_total, 4);  // epot, ekin, sigma_E, bits of sigma_F,max (switching-mode samples)
+    A_(s->e_total, 6);  // epot, ekin, sigma_E, bits of sigma_F,max (switching-mode samples)
     A_(s->flags, FLAG_WORDS);
 #undef A_
     if (!rc && cudaMallocHost((void **)&s->flags_host, sizeof(int32_t) * FLAG_WORDS) != cudaSuccess) rc = GMNN_OOM;
@@ -889,6 +895,30 @@ int gmnn_md_ensemble_steps(gmnn_system *s, float *positions, float *velocities, 
     if (n_samples) *n_samples = samples;
     if (n_rebuilds) *n_rebuilds = rebuilds;
     return rc;
+}
+
+int gmnn_system_set_udd_bias(gmnn_system *s, float A, float B) {
+    if (!s || !std::isfinite(A) || (A != 0.f && !(B > 0.f && std::isfinite(B)))) {
+        set_error("gmnn_system_set_udd_bias: A must be finite and B > 0");
+        return GMNN_INVALID_ARG;
+    }
+    s->udd_A = A;
+    if (A != 0.f) s->udd_B = B;
+    s->md_state_valid = false;
+    return GMNN_OK;
+}
+
+int gmnn_system_get_udd_bias(gmnn_system *s, double *e_bias, double *var_e, void *cuda_stream) {
+    if (!s || !e_bias || !var_e) return GMNN_INVALID_ARG;
+    double h[2] = {0.0, 0.0};
+    if (s->udd_active) {
+        cudaStream_t st = (cudaStream_t)cuda_stream;
+        GMNN_CUDA(cudaMemcpyAsync(h, s->e_total + 4, sizeof(h), cudaMemcpyDeviceToHost, st));
+        GMNN_CUDA(cudaStreamSynchronize(st));
+    }
+    *e_bias = h[0];
+    *var_e = h[1];
+    return GMNN_OK;
 }
 
 int gmnn_check(gmnn_system *s, void *cuda_stream) {

@@ -122,6 +122,8 @@ struct gmnn_system {
     float *vhead = nullptr;          // [H_last]
     float *head_w = nullptr;         // [n_heads] weights of the differentiated energy
     float *ypart = nullptr;          // [MAX_HEAD_SLOTS][N padded to 128]: partial head sums (mlp_tc.cu EPI_HIDDEN_HEAD)
+    float udd_A = 0.f, udd_B = 1.f;  // UDD bias parameters (Eq. 9); active when udd_A != 0 and n_heads > 1
+    bool udd_active = false;         // this evaluation adds the bias: e_total[4] = E_b, e_total[5] = sigma_E^2
     bool use_mean_head = false;      // MD on a multi-head model: forward with model->w_mean as the only head
     bool heads_fused = false;        // the last mlp_forward left ypart instead of H[L-1]
     int head_slots = 0;
@@ -130,7 +132,7 @@ struct gmnn_system {
     float *f_int = nullptr;          // [N][3]
     float *f_tmp = nullptr;          // [N][3] caller order (ensemble, MD)
     double *partial = nullptr;       // reduction scratch
-    double *e_total = nullptr;       // [4] device scalars (epot, ekin, sigma_E, bits of sigma_F,max)
+    double *e_total = nullptr;       // [6] device scalars (epot, ekin, sigma_E, bits of sigma_F,max, E_b, sigma_E^2 of the bias)
     float *ens_scratch = nullptr;    // [11 N] switching-mode samples: kept forces, e_mean, e_var, f_mean, f_var (lazy)
     int32_t *flags = nullptr;        // FLAG_WORDS
     int32_t *flags_host = nullptr;   // pinned
@@ -187,6 +189,7 @@ int launch_series_reset(gmnn_system *s, int32_t next_index, cudaStream_t st);
 int launch_welford(gmnn_system *s, int head, const float *f_head, float *f_mean, float *f_m2, cudaStream_t st);
 int launch_ensemble_energy_stats(gmnn_system *s, float *e_mean, float *e_var, cudaStream_t st);
 int launch_finish_var(int64_t n, float *m2, int n_heads, cudaStream_t st);
+int launch_udd_weights(gmnn_system *s, float *head_w_out, double *scal, cudaStream_t st);
 int launch_uncertainty_scalars(gmnn_system *s, const float *f_var, double *out_d, int32_t *out_bits, cudaStream_t st);
 
 }  // namespace gmnn

@@ -64,13 +64,15 @@ __global__ void __launch_bounds__(256) k_ke_stage1(int64_t N, const float *__res
     if (threadIdx.x == 0) partial[blockIdx.x] = acc;
 }
 
-__global__ void __launch_bounds__(256) k_sum_stage2(int n, const double *__restrict__ partial, double factor, double *out, double *out2) {
+__global__ void __launch_bounds__(256) k_sum_stage2(int n, const double *__restrict__ partial, double factor, double *out, double *out2,
+                                                    const double *__restrict__ add) {
     double v = 0.0;
     for (int q = threadIdx.x; q < n; q += blockDim.x) v += partial[q];
     v = block_sum(v);
     if (threadIdx.x == 0) {
-        *out = v * factor;
-        if (out2) *out2 = v * factor;
+        v = v * factor + (add ? *add : 0.0);  // add: the UDD bias of this evaluation (Eq. 9)
+        *out = v;
+        if (out2) *out2 = v;
     }
 }
 
@@ -157,7 +159,7 @@ int launch_energy_sum(gmnn_system *s, double *energy_out, cudaStream_t st, doubl
     const int nb = red_blocks(s->N);
     k_sum_stage1<<<nb, 256, 0, st>>>(s->N, s->e_atom, s->partial);
     GMNN_LAUNCHED();
-    k_sum_stage2<<<1, 256, 0, st>>>(nb, s->partial, 1.0, energy_out, energy_out2);
+    k_sum_stage2<<<1, 256, 0, st>>>(nb, s->partial, 1.0, energy_out, energy_out2, s->udd_active ? s->e_total + 4 : nullptr);
     GMNN_LAUNCHED();
     GMNN_CUDA(cudaGetLastError());
     return GMNN_OK;
@@ -167,7 +169,7 @@ int launch_ke(gmnn_system *s, const float *v, const float *m, double *ekin_out, 
     const int nb = red_blocks(s->N);
     k_ke_stage1<<<nb, 256, 0, st>>>(s->N, v, m, s->partial + RED_BLOCKS);
     GMNN_LAUNCHED();
-    k_sum_stage2<<<1, 256, 0, st>>>(nb, s->partial + RED_BLOCKS, 1.0 / ACC_CONV, ekin_out, ekin_out2);
+    k_sum_stage2<<<1, 256, 0, st>>>(nb, s->partial + RED_BLOCKS, 1.0 / ACC_CONV, ekin_out, ekin_out2, nullptr);
     GMNN_LAUNCHED();
     GMNN_CUDA(cudaGetLastError());
     return GMNN_OK;
@@ -280,11 +282,55 @@ __global__ void __launch_bounds__(256) k_sigma_f_max(int64_t N, const float *__r
     if ((threadIdx.x & 31) == 0 && v > 0.f) atomicMax(out_bits, __float_as_int(v));
 }
 
-// out: double sigma_e at out_d[0]; float bits of sigma_f_max at out_bits[0] (zeroed here first)
-int launch_uncertainty_scalars(gmnn_system *s, const float *f_var, double *out_d, int32_t *out_bits, cudaStream_t st) {
+// UDD bias (Eq. 9) on the head totals of stage 1:
+//   E_b = A [exp(-s2 / (M N B^2)) - 1],  s2 = 1/M sum_m (E^(m) - mean)^2  (Eq. 5 on total energies, reading R27)
+// The gradient of mean + E_b is sum_m c_m grad E^(m) with  c_m = 1/M + E_b'(s2) 2/M (E^(m) - mean)  (the
+// weights of the -mean term sum to zero), so ONE backward pass with head weights c gives the biased forces.
+__global__ void __launch_bounds__(64) k_udd_weights(int nb, int M, const double *__restrict__ partial, double A, double B,
+                                                    double n_atoms, float *head_w, double *scal) {
+    __shared__ double tot[64];
+    const int m = threadIdx.x;
+    if (m < M) {
+        double v = 0.0;
+        for (int b = 0; b < nb; ++b) v += partial[(int64_t)m * nb + b];
+        tot[m] = v;
+    }
+    __syncthreads();
+    double mean = 0.0, var = 0.0;
+    for (int q = 0; q < M; ++q) mean += tot[q];
+    mean /= (double)M;
+    for (int q = 0; q < M; ++q) var += (tot[q] - mean) * (tot[q] - mean);
+    var /= (double)M;
+    const double width = (double)M * n_atoms * B * B;
+    const double ex = exp(-var / width);
+    if (m < M) head_w[m] = (float)(1.0 / M + (-A / width * ex) * (2.0 / M) * (tot[m] - mean));
+    if (m == 0) {
+        scal[0] = A * (ex - 1.0);
+        scal[1] = var;
+    }
+}
+
+static int head_total_blocks(const gmnn_system *s) {
     const int M = s->model->hp.n_heads;
     int nb = red_blocks(s->N);
     if (nb * M > 2 * RED_BLOCKS) nb = 2 * RED_BLOCKS / M;  // partial holds 2 * RED_BLOCKS doubles
+    return nb;
+}
+
+// head_w_out [M] <- c;  scal[0] <- E_b, scal[1] <- sigma_E^2  (from e_heads of the forward just run)
+int launch_udd_weights(gmnn_system *s, float *head_w_out, double *scal, cudaStream_t st) {
+    const int M = s->model->hp.n_heads, nb = head_total_blocks(s);
+    k_head_totals_stage1<<<dim3(nb, M), 256, 0, st>>>(s->N, M, s->e_heads, s->partial);
+    GMNN_LAUNCHED();
+    k_udd_weights<<<1, 64, 0, st>>>(nb, M, s->partial, (double)s->udd_A, (double)s->udd_B, (double)s->N, head_w_out, scal);
+    GMNN_LAUNCHED();
+    GMNN_CUDA(cudaGetLastError());
+    return GMNN_OK;
+}
+
+// out: double sigma_e at out_d[0]; float bits of sigma_f_max at out_bits[0] (zeroed here first)
+int launch_uncertainty_scalars(gmnn_system *s, const float *f_var, double *out_d, int32_t *out_bits, cudaStream_t st) {
+    const int M = s->model->hp.n_heads, nb = head_total_blocks(s);
     GMNN_CUDA(cudaMemsetAsync(out_bits, 0, sizeof(int32_t), st));
     k_head_totals_stage1<<<dim3(nb, M), 256, 0, st>>>(s->N, M, s->e_heads, s->partial);
     GMNN_LAUNCHED();

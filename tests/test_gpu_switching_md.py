@@ -115,3 +115,76 @@ def test_bad_arguments(gm):
     with pytest.raises(gm.GmnnError) as e:
         sysm.md_ensemble_steps(pos, vel, mass, w.dt_fs, 4, 0)
     assert e.value.code == gm.GMNN_INVALID_ARG
+
+
+# ------------------------------------------------------------------ UDD bias (Eq. 9) against oracle O-13
+def _udd_setup(gm, orc, name, mlp_precision=0):
+    w = _workload(name)
+    m = orc.Model(w.model)
+    pairs = orc.auto_neighbors(w.positions, w.cell, w.pbc, w.model.r_cut)
+    var0 = orc.udd_energy_forces(m, w.positions, w.species, w.cell, pairs, 0.0, 1.0).var_e
+    B = float(np.sqrt(var0 / (w.model.n_heads * len(w.species))))  # exponent -1 at the initial state
+    return w, m, pairs, B
+
+
+@pytest.mark.parametrize("mlp_precision", [0, 3])
+@pytest.mark.parametrize("name", ["ionic384_m8", "li1024_m32"])
+def test_udd_biased_energy_and_forces(gm, orc, name, mlp_precision):
+    import torch
+
+    w, m, pairs, B = _udd_setup(gm, orc, name)
+    A = 5.0
+    ref = orc.udd_energy_forces(m, w.positions, w.species, w.cell, pairs, A, B)
+    plain = orc.udd_energy_forces(m, w.positions, w.species, w.cell, pairs, 0.0, B)
+    assert force_error(ref.forces, plain.forces) > 50 * F_TOL  # the bias force is far above the tolerance
+    sysm, pos, _, _ = _system(gm, w, mlp_precision=mlp_precision)
+    sysm.set_udd_bias(A, B)
+    e, e_atom, f = sysm.energy_forces(pos)
+    eb, var = sysm.get_udd_bias()
+    assert abs(var - ref.var_e) <= 2e-4 * ref.var_e
+    assert abs(eb - ref.e_bias) <= 5e-4 * abs(ref.e_bias)
+    assert abs(float(e) - ref.energy) <= 1e-5 * abs(ref.e_mean) + 5e-4 * abs(ref.e_bias) + 1e-4
+    assert force_error(f.cpu().numpy().astype(np.float64), ref.forces) <= F_TOL
+    # switching the bias off gives the mean-energy forces again
+    sysm.set_udd_bias(0.0)
+    e0, _, f0 = sysm.energy_forces(pos)
+    assert force_error(f0.cpu().numpy().astype(np.float64), plain.forces) <= F_TOL
+    assert sysm.get_udd_bias() == (0.0, 0.0)
+
+
+def test_udd_biased_md_matches_oracle_and_samples_stay_unbiased(gm, orc):
+    w, m, pairs, B = _udd_setup(gm, orc, "ionic384_m8")
+    A = 2.0
+    n = 10
+    x, v, ep, ek, eb = orc.nve_udd(m, w.positions, w.velocities, w.masses, w.species, w.cell, w.pbc, w.dt_fs, n, A, B)
+    sysm, pos, vel, mass = _system(gm, w)
+    sysm.set_udd_bias(A, B)
+    out = sysm.md_ensemble_steps(pos, vel, mass, w.dt_fs, n, 5)
+    L = w.cell.astype(np.float64)
+    d = pos.cpu().numpy().astype(np.float64) - x
+    d -= np.round(d / L) * L
+    assert np.abs(d).max() <= 1e-4
+    assert np.abs(vel.cpu().numpy() - v).max() <= 1e-5
+    assert np.abs(out["epot"].cpu().numpy() - ep).max() <= 1e-5 * np.abs(ep).max() + 1e-3
+    assert abs(sysm.get_udd_bias()[0] - eb[-1]) <= 1e-3 * np.abs(eb).max()
+    # and the biased run is not the plain one
+    sysm2, pos2, vel2, mass2 = _system(gm, w)
+    out2 = sysm2.md_ensemble_steps(pos2, vel2, mass2, w.dt_fs, n, 5)
+    assert np.abs(pos2.cpu().numpy() - pos.cpu().numpy()).max() > 1e-5
+    # the uncertainty sample is Eq. 5 on the unbiased heads at the biased run's positions
+    xg = pos.cpu().numpy()
+    xw = (xg.astype(np.float64) - np.floor(xg.astype(np.float64) / L) * L).astype(np.float32)
+    xw = np.where(xw >= w.cell[None, :], 0.0, xw).astype(np.float32)
+    ens = orc.ensemble(m, xw, w.species, w.cell, orc.auto_neighbors(xw, w.cell, w.pbc, w.model.r_cut))
+    assert abs(out["sigma_e"][-1] - np.std(ens.e_heads.sum(0))) <= 2e-4 * np.std(ens.e_heads.sum(0))
+
+
+def test_udd_bad_arguments_and_single_head(gm):
+    w = wl.ionic_liquid_box(n_pairs=16, hidden=(64, 64))
+    sysm, pos, _, _ = _system(gm, w)
+    with pytest.raises(gm.GmnnError):
+        sysm.set_udd_bias(1.0, 0.0)
+    e0, _, f0 = sysm.energy_forces(pos)
+    sysm.set_udd_bias(3.0, 0.5)  # one head: sigma = 0, nothing changes
+    e1, _, f1 = sysm.energy_forces(pos)
+    assert float(e0) == float(e1) and bool((f0 == f1).all())
