@@ -33,6 +33,9 @@
  *        per-head pass only every N steps), :71 (uncertainty as stopping criterion), Eq. 5
  *   O-13 UDD bias (gmnn_oracle.py, numpy on O-10's per-head forces)  PAPER.md:102-107 (Eq. 9); pins in
  *        tests/test_oracle_udd.py: forces == finite differences of mean + E_b, limits of Eq. 9, conservation
+ *   O-14 NVT, Nose-Hoover chain (gmnn_oracle.py)  PAPER.md:365-375 (thermostat_chain keys); pins in
+ *        tests/test_oracle_nvt.py: conserved extended energy at second order, tau -> inf is O-11, heating
+ *        towards the target, closed form and time reversal of one chain operator
  *
  * Build: gcc -O2 -std=c11 -fPIC -shared -fopenmp -ffp-contract=off gmnn_oracle.c -lm
  *        (-ffp-contract=off: the neighbour predicate is specified in unfused fp32, reading R20.)

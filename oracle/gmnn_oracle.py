@@ -420,3 +420,99 @@ def nve_udd(model: Model, positions, velocities, masses, species, cell, pbc, dt_
         ekin.append(0.5 * (m * v * v).sum() / ACC)
         eb.append(r.e_bias)
     return x, v, np.array(epot), np.array(ekin), np.array(eb)
+
+
+KB_EV = 8.617333262e-5  # Boltzmann constant, eV/K
+
+
+def _sy_weights(sy_steps: int):
+    """Suzuki-Yoshida weights of the chain sub-steps (1, 3 or 5)."""
+    if sy_steps == 1:
+        return [1.0]
+    if sy_steps == 3:
+        a = 1.0 / (2.0 - 2.0 ** (1.0 / 3.0))
+        return [a, 1.0 - 2.0 * a, a]
+    if sy_steps == 5:
+        a = 1.0 / (4.0 - 4.0 ** (1.0 / 3.0))
+        return [a, a, 1.0 - 4.0 * a, a, a]
+    raise ValueError("sy_steps must be 1, 3 or 5")
+
+
+def nhc_half_step(ke2: float, xi: np.ndarray, pxi: np.ndarray, Q: np.ndarray, dof: float, kT: float, dt: float,
+                  chain_steps: int, sy_steps: int) -> float:
+    """O-14a: the thermostat operator of a Nose-Hoover chain for half a time step (Martyna, Tuckerman, Tobias,
+    Klein 1996; the `thermostat_chain` of PAPER.md:365-375: chain_length, chain_steps, sy_steps, tau).
+    ke2 = sum m v^2 (eV).  Updates xi, pxi in place and returns the factor the velocities are scaled by."""
+    Mc = len(xi)
+    scale = 1.0
+    delta = dt / chain_steps
+    for _ in range(chain_steps):
+        for wgt in _sy_weights(sy_steps):
+            d2, d4, d8 = delta * wgt / 2, delta * wgt / 4, delta * wgt / 8
+            G = (pxi[Mc - 2] ** 2 / Q[Mc - 2] - kT) if Mc > 1 else (ke2 - dof * kT)
+            pxi[Mc - 1] += d4 * G
+            for k in range(Mc - 2, -1, -1):
+                G = (ke2 - dof * kT) if k == 0 else (pxi[k - 1] ** 2 / Q[k - 1] - kT)
+                s = np.exp(-d8 * pxi[k + 1] / Q[k + 1])
+                pxi[k] = s * (s * pxi[k] + d4 * G)
+            s = np.exp(-d2 * pxi[0] / Q[0])
+            scale *= s
+            ke2 *= s * s
+            xi += d2 * pxi / Q
+            G = ke2 - dof * kT
+            for k in range(Mc - 1):
+                s = np.exp(-d8 * pxi[k + 1] / Q[k + 1])
+                pxi[k] = s * (s * pxi[k] + d4 * G)
+                G = pxi[k] ** 2 / Q[k] - kT
+            pxi[Mc - 1] += d4 * G
+    return scale
+
+
+def nvt_nose_hoover(model: Model, positions, velocities, masses, species, cell, pbc, dt_fs: float, n_steps: int,
+                    temperature: float, tau_fs: float, chain_length: int = 3, chain_steps: int = 2, sy_steps: int = 3):
+    """O-14: NVT with a Nose-Hoover chain: chain half step, velocity Verlet (O-11) on the mean
+    energy, chain half step.  Q_0 = dof kT tau^2, Q_k = kT tau^2, dof = 3 N (reading R28).  Fresh list of radius
+    r_cut every step.  Returns x, v, epot, ekin, conserved (all [n_steps + 1]; conserved = epot + ekin +
+    sum pxi^2 / 2Q + dof kT xi_0 + kT sum_{k>0} xi_k)."""
+    ACC = 9.648533212e-3
+    x = _f64(positions).copy()
+    v = _f64(velocities).copy()
+    m = _f64(masses)[:, None]
+    L = _f64(cell).reshape(-1)
+    per = np.asarray(pbc).astype(bool)
+    N = x.shape[0]
+    dof, kT = 3.0 * N, KB_EV * temperature
+    Q = np.full(chain_length, kT * tau_fs ** 2)
+    Q[0] *= dof
+    xi, pxi = np.zeros(chain_length), np.zeros(chain_length)
+
+    def wrap(y):
+        y = y.copy()
+        y[:, per] -= np.floor(y[:, per] / L[per]) * L[per]
+        return y
+
+    def evaluate(y):
+        y32 = y.astype(np.float32)
+        y32 = np.where(y32 >= np.asarray(cell, np.float32).reshape(-1)[None, :], np.float32(0), y32)
+        return energy_forces(model, y, species, cell, auto_neighbors(y32, cell, pbc, model.r_cut))
+
+    def ke2():
+        return float((m * v * v).sum() / ACC)
+
+    def conserved(ep):
+        return ep + 0.5 * ke2() + float((pxi ** 2 / (2 * Q)).sum()) + dof * kT * xi[0] + kT * float(xi[1:].sum())
+
+    x = wrap(x)
+    r = evaluate(x)
+    epot, ekin, cons = [r.energy], [0.5 * ke2()], [conserved(r.energy)]
+    for _ in range(n_steps):
+        v *= nhc_half_step(ke2(), xi, pxi, Q, dof, kT, dt_fs, chain_steps, sy_steps)
+        v += 0.5 * dt_fs * r.forces / m * ACC
+        x = wrap(x + dt_fs * v)
+        r = evaluate(x)
+        v += 0.5 * dt_fs * r.forces / m * ACC
+        v *= nhc_half_step(ke2(), xi, pxi, Q, dof, kT, dt_fs, chain_steps, sy_steps)
+        epot.append(r.energy)
+        ekin.append(0.5 * ke2())
+        cons.append(conserved(r.energy))
+    return x, v, np.array(epot), np.array(ekin), np.array(cons)
