@@ -179,7 +179,7 @@ int gmnn_energy_forces_host(gmnn_system *s, const float *positions /*HOST*/, dou
 int gmnn_ensemble_energy_forces(gmnn_system *s, const float *positions, float *e_mean, float *e_var,
                                 float *f_mean, float *f_var, void *cuda_stream);
 
-/* n_steps of NVE velocity Verlet (BASELINE.json configs 2, 5; dt PAPER.md:367), whole loop on the
+/* n_steps of velocity Verlet (NVE; NVT while gmnn_system_set_nose_hoover is set) (BASELINE.json configs 2, 5; dt PAPER.md:367), whole loop on the
  * device: kick, drift, skin test, list rebuild when any atom moved > skin/2 since the last build
  * (positions are wrapped into [0, L) at each rebuild, and only then), energy+forces, kick.
  *   positions, velocities  DEVICE float [n_atoms][3], in-out (Ang, Ang/fs)
@@ -214,6 +214,19 @@ int gmnn_md_ensemble_steps(gmnn_system *s, float *positions, float *velocities, 
                            int32_t n_steps, int32_t sampling_rate, float f_sigma_stop, double *epot_series,
                            double *ekin_series, double *sigma_e_series, double *sigma_f_max_series, float *f_var_last,
                            int32_t *n_steps_done, int32_t *n_samples, int32_t *n_rebuilds, void *cuda_stream);
+
+/* NVT with a Nose-Hoover chain (PAPER.md:365-375 `thermostat_chain`: chain_length 3,
+ * chain_steps 2, sy_steps 3, tau 100 [time steps]).  While set, every step of gmnn_md_verlet_steps and
+ * gmnn_md_ensemble_steps applies the Martyna-Tuckerman-Tobias-Klein chain operator for dt/2 before and after the
+ * velocity-Verlet step, on the device (the step still replays as a CUDA graph).  Q_0 = 3 N kT tau^2, Q_k = kT tau^2.
+ *   temperature_K <= 0 switches the thermostat off (NVE); tau_fs > 0 in fs; 1 <= chain_length <= 8;
+ *   1 <= chain_steps <= 16; sy_steps in {1, 3, 5} (Suzuki-Yoshida).  Setting it resets the chain (xi = p_xi = 0). */
+int gmnn_system_set_nose_hoover(gmnn_system *s, float temperature_K, float tau_fs, int32_t chain_length,
+                                int32_t chain_steps, int32_t sy_steps);
+/* Chain state: xi, p_xi HOST double [chain_length] (p_xi in eV fs), and the thermostat's energy
+ * sum p_xi^2 / 2Q + 3 N kT xi_0 + kT sum_{k>0} xi_k (eV): epot + ekin + it is conserved.  Synchronises. */
+int gmnn_system_get_nose_hoover(gmnn_system *s, double *xi /*HOST*/, double *p_xi /*HOST*/,
+                                double *thermostat_energy /*HOST*/, void *cuda_stream);
 
 /* Uncertainty-driven-dynamics bias (Eq. 9) on a model with several
  * heads:  E_b = A [exp(-sigma_E^2 / (N_ens N_atoms B^2)) - 1],  sigma_E^2 = 1/N_ens sum_m (E^(m) - mean)^2 of the

@@ -31,7 +31,7 @@ GMNN_FORCE_GATHER, GMNN_FORCE_PAIRBUF = 0, 1
 EXPORTS = (
     "gmnn_n_features", "gmnn_create", "gmnn_destroy", "gmnn_system_create", "gmnn_system_destroy",
     "gmnn_system_set_int", "gmnn_system_get_int", "gmnn_build_neighbors", "gmnn_get_neighbors",
-    "gmnn_energy_forces", "gmnn_energy_forces_host", "gmnn_ensemble_energy_forces", "gmnn_md_verlet_steps", "gmnn_md_ensemble_steps", "gmnn_system_set_udd_bias", "gmnn_system_get_udd_bias",
+    "gmnn_energy_forces", "gmnn_energy_forces_host", "gmnn_ensemble_energy_forces", "gmnn_md_verlet_steps", "gmnn_md_ensemble_steps", "gmnn_system_set_nose_hoover", "gmnn_system_get_nose_hoover", "gmnn_system_set_udd_bias", "gmnn_system_get_udd_bias",
     "gmnn_check", "gmnn_stage_times", "gmnn_debug_read", "gmnn_launch_count", "gmnn_last_error",
 )
 
@@ -77,6 +77,8 @@ def _load() -> C.CDLL:
                                          C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
     lib.gmnn_md_ensemble_steps.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_float, C.c_int32, C.c_int32,
                                            C.c_float] + [C.c_void_p] * 9
+    lib.gmnn_system_set_nose_hoover.argtypes = [C.c_void_p, C.c_float, C.c_float, C.c_int32, C.c_int32, C.c_int32]
+    lib.gmnn_system_get_nose_hoover.argtypes = [C.c_void_p] * 5
     lib.gmnn_system_set_udd_bias.argtypes = [C.c_void_p, C.c_float, C.c_float]
     lib.gmnn_system_get_udd_bias.argtypes = [C.c_void_p] * 4
     lib.gmnn_energy_forces.argtypes = [C.c_void_p] * 6
@@ -314,6 +316,22 @@ class System:
         d, k = int(done.value), int(nsamp.value)
         return {"epot": epot[:d + 1], "ekin": ekin[:d + 1], "sigma_e": se[:k], "sigma_f_max": sf[:k], "f_var": fvar,
                 "n_steps_done": d, "n_rebuilds": int(nreb.value)}
+
+    def set_nose_hoover(self, temperature_K: float, tau_fs: float = 50.0, chain_length: int = 3, chain_steps: int = 2,
+                        sy_steps: int = 3) -> None:
+        """NVT for the MD entries (temperature_K <= 0: back to NVE); resets the chain."""
+        _check(lib.gmnn_system_set_nose_hoover(self.handle, C.c_float(temperature_K), C.c_float(tau_fs),
+                                               C.c_int32(chain_length), C.c_int32(chain_steps), C.c_int32(sy_steps)))
+        self._nhc_len = chain_length if temperature_K > 0 else 0
+
+    def get_nose_hoover(self, stream=None):
+        """(xi[chain_length], p_xi[chain_length], thermostat energy in eV)."""
+        n = getattr(self, "_nhc_len", 0)
+        xi, pxi = np.zeros(max(n, 1)), np.zeros(max(n, 1))
+        et = C.c_double(0)
+        _check(lib.gmnn_system_get_nose_hoover(self.handle, xi.ctypes.data_as(C.c_void_p), pxi.ctypes.data_as(C.c_void_p),
+                                               C.cast(C.byref(et), C.c_void_p), _stream_ptr(stream)))
+        return xi[:n], pxi[:n], float(et.value)
 
     def set_udd_bias(self, A: float, B: float = 1.0) -> None:
         _check(lib.gmnn_system_set_udd_bias(self.handle, C.c_float(A), C.c_float(B)))

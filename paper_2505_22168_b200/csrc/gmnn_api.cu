@@ -376,7 +376,7 @@ void gmnn_system_destroy(gmnn_system *s) {
     for (int l = 0; l < MAX_LAYERS; ++l) { dev_free(s->H[l]); dev_free(s->D[l]); }
     dev_free(s->dZ[0]); dev_free(s->dZ[1]); dev_free(s->Bv); dev_free(s->BvT); dev_free(s->BvTs); dev_free(s->BvTh); dev_free(s->amax); dev_free(s->vhead); dev_free(s->head_w);
     dev_free(s->ypart); dev_free(s->e_heads); dev_free(s->e_atom); dev_free(s->f_int); dev_free(s->f_tmp); dev_free(s->partial);
-    dev_free(s->e_total); dev_free(s->flags); dev_free(s->ens_scratch);
+    dev_free(s->e_total); dev_free(s->flags); dev_free(s->ens_scratch); dev_free(s->nhc);
     dev_free(s->stage_pos); dev_free(s->stage_f); dev_free(s->stage_e);
     if (s->flags_host) cudaFreeHost(s->flags_host);
     for (cudaEvent_t e : s->events) cudaEventDestroy(e);
@@ -756,6 +756,8 @@ int gmnn_md_verlet_steps(gmnn_system *s, float *positions, float *velocities, co
     // through a device-side counter), so the body can be captured once and replayed as a CUDA graph.
     auto md_step = [&](cudaStream_t q) -> int {
         int r;
+        // NVT: chain operator for dt/2 before and after the velocity-Verlet step
+        if (s->nhc_len > 0 && (r = launch_nhc_half(s, velocities, ek, dt_fs, q))) return r;
         if ((r = launch_kick_drift(s, positions, velocities, s->f_tmp, masses, dt_fs, q))) return r;
         T.mark("kick_drift");
         // rebuild (wrap first) iff the max displacement since the last build exceeds skin/2
@@ -766,6 +768,7 @@ int gmnn_md_verlet_steps(gmnn_system *s, float *positions, float *velocities, co
         if ((r = launch_energy_sum(s, ep, q, nullptr))) return r;
         T.mark("outputs");
         if ((r = launch_kick_ke(s, velocities, s->f_tmp, masses, dt_fs, ek, q, nullptr))) return r;
+        if (s->nhc_len > 0 && (r = launch_nhc_half(s, velocities, ek, dt_fs, q))) return r;
         if ((epot_series || ekin_series) && (r = launch_series_append(s, epot_series, ekin_series, q))) return r;
         T.mark("kick_ke");
         return GMNN_OK;
@@ -895,6 +898,49 @@ int gmnn_md_ensemble_steps(gmnn_system *s, float *positions, float *velocities, 
     if (n_samples) *n_samples = samples;
     if (n_rebuilds) *n_rebuilds = rebuilds;
     return rc;
+}
+
+int gmnn_system_set_nose_hoover(gmnn_system *s, float temperature_K, float tau_fs, int32_t chain_length,
+                                int32_t chain_steps, int32_t sy_steps) {
+    if (!s) return GMNN_INVALID_ARG;
+    s->md_state_valid = false;
+    if (!(temperature_K > 0.f)) {  // off: NVE
+        s->nhc_len = 0;
+        return GMNN_OK;
+    }
+    if (!(tau_fs > 0.f) || !std::isfinite(tau_fs) || !std::isfinite(temperature_K) || chain_length < 1 ||
+        chain_length > 8 || chain_steps < 1 || chain_steps > 16 || (sy_steps != 1 && sy_steps != 3 && sy_steps != 5)) {
+        set_error("gmnn_system_set_nose_hoover: tau > 0, 1 <= chain_length <= 8, 1 <= chain_steps <= 16, sy_steps in {1, 3, 5}");
+        return GMNN_INVALID_ARG;
+    }
+    int rc;
+    if (!s->nhc && (rc = dev_alloc(&s->nhc, (size_t)26))) return rc;
+    const double kT = 8.617333262e-5 * (double)temperature_K, tau = (double)tau_fs;
+    double h[26] = {};
+    for (int k = 0; k < chain_length; ++k) h[16 + k] = (k == 0 ? 3.0 * (double)s->N : 1.0) * kT * tau * tau;
+    for (int k = chain_length; k < 8; ++k) h[16 + k] = 1.0;
+    h[24] = 1.0;
+    GMNN_CUDA(cudaMemcpy(s->nhc, h, sizeof(h), cudaMemcpyHostToDevice));
+    s->nhc_len = chain_length;
+    s->nhc_chain_steps = chain_steps;
+    s->nhc_sy_steps = sy_steps;
+    s->nhc_kT = kT;
+    return GMNN_OK;
+}
+
+int gmnn_system_get_nose_hoover(gmnn_system *s, double *xi, double *p_xi, double *thermostat_energy, void *cuda_stream) {
+    if (!s || !xi || !p_xi || !thermostat_energy) return GMNN_INVALID_ARG;
+    if (s->nhc_len == 0) {
+        set_error("no Nose-Hoover chain is set");
+        return GMNN_INVALID_ARG;
+    }
+    double h[26];
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    GMNN_CUDA(cudaMemcpyAsync(h, s->nhc, sizeof(h), cudaMemcpyDeviceToHost, st));
+    GMNN_CUDA(cudaStreamSynchronize(st));
+    for (int k = 0; k < s->nhc_len; ++k) xi[k] = h[k], p_xi[k] = h[8 + k];
+    *thermostat_energy = h[25];
+    return GMNN_OK;
 }
 
 int gmnn_system_set_udd_bias(gmnn_system *s, float A, float B) {

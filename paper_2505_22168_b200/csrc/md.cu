@@ -342,4 +342,69 @@ int launch_uncertainty_scalars(gmnn_system *s, const float *f_var, double *out_d
     return GMNN_OK;
 }
 
+// ---- NVT: Nose-Hoover chain (PAPER.md:365-375 thermostat_chain) ----
+// The chain operator of Martyna, Tuckerman, Tobias and Klein for half a time step, on the device so that the
+// thermostatted step stays one replayable launch sequence: one thread, fp64, reads the kinetic energy the
+// last kick left in ek, updates (xi, p_xi), and leaves the velocity scale factor for k_scale_v.
+// st: [0, 8) xi, [8, 16) p_xi, [16, 24) Q, [24] scale factor, [25] thermostat energy
+__global__ void k_nhc_half(double *ek, double *st, int Mc, int chain_steps, int sy_steps, double dof, double kT, double dt) {
+    double *xi = st, *pxi = st + 8;
+    const double *Q = st + 16;
+    double w[5];
+    if (sy_steps == 3) {
+        const double a = 1.0 / (2.0 - cbrt(2.0));
+        w[0] = a, w[1] = 1.0 - 2.0 * a, w[2] = a;
+    } else if (sy_steps == 5) {
+        const double a = 1.0 / (4.0 - cbrt(4.0));
+        w[0] = w[1] = w[3] = w[4] = a, w[2] = 1.0 - 4.0 * a;
+    } else {
+        w[0] = 1.0;
+    }
+    double ke2 = 2.0 * *ek, scale = 1.0;
+    const double delta = dt / chain_steps;
+    for (int c = 0; c < chain_steps; ++c)
+        for (int y = 0; y < sy_steps; ++y) {
+            const double d2 = delta * w[y] / 2, d4 = delta * w[y] / 4, d8 = delta * w[y] / 8;
+            double G = (Mc > 1) ? pxi[Mc - 2] * pxi[Mc - 2] / Q[Mc - 2] - kT : ke2 - dof * kT;
+            pxi[Mc - 1] += d4 * G;
+            for (int k = Mc - 2; k >= 0; --k) {
+                G = (k == 0) ? ke2 - dof * kT : pxi[k - 1] * pxi[k - 1] / Q[k - 1] - kT;
+                const double e = exp(-d8 * pxi[k + 1] / Q[k + 1]);
+                pxi[k] = e * (e * pxi[k] + d4 * G);
+            }
+            const double e0 = exp(-d2 * pxi[0] / Q[0]);
+            scale *= e0;
+            ke2 *= e0 * e0;
+            for (int k = 0; k < Mc; ++k) xi[k] += d2 * pxi[k] / Q[k];
+            G = ke2 - dof * kT;
+            for (int k = 0; k < Mc - 1; ++k) {
+                const double e = exp(-d8 * pxi[k + 1] / Q[k + 1]);
+                pxi[k] = e * (e * pxi[k] + d4 * G);
+                G = pxi[k] * pxi[k] / Q[k] - kT;
+            }
+            pxi[Mc - 1] += d4 * G;
+        }
+    *ek = 0.5 * ke2;
+    st[24] = scale;
+    double et = dof * kT * xi[0];
+    for (int k = 0; k < Mc; ++k) et += pxi[k] * pxi[k] / (2.0 * Q[k]) + (k > 0 ? kT * xi[k] : 0.0);
+    st[25] = et;
+}
+
+__global__ void __launch_bounds__(256) k_scale_v(int64_t n3, float *v, const double *__restrict__ scale) {
+    const int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (t < n3) v[t] *= (float)*scale;
+}
+
+// chain operator for dt/2 on the kinetic energy in ek (updated), then v *= scale
+int launch_nhc_half(gmnn_system *s, float *v, double *ek, float dt, cudaStream_t st) {
+    k_nhc_half<<<1, 1, 0, st>>>(ek, s->nhc, s->nhc_len, s->nhc_chain_steps, s->nhc_sy_steps, 3.0 * (double)s->N, s->nhc_kT,
+                                (double)dt);
+    GMNN_LAUNCHED();
+    k_scale_v<<<nblocks(3 * s->N, 256), 256, 0, st>>>(3 * s->N, v, s->nhc + 24);
+    GMNN_LAUNCHED();
+    GMNN_CUDA(cudaGetLastError());
+    return GMNN_OK;
+}
+
 }  // namespace gmnn
