@@ -336,6 +336,8 @@ def run_ours(args):
         vol = float(np.prod(w.cell.astype(np.float64)))
         sysm.set_int("capacity", int(2.0 * N / vol * 4.19 * (w.model.r_cut + w.skin) ** 3) + 64)
     sysm.build_neighbors(pos, w.cell9, w.pbc, w.model.r_cut, w.skin)
+    if args.nvt > 0:
+        sysm.set_nose_hoover(args.nvt, 100.0 * w.dt_fs, 3, 2, 3)
     counts = sysm.debug_read("count").astype(np.float64)
     nl_mean = float(counts.mean())
     r_list = w.model.r_cut + w.skin
@@ -474,8 +476,8 @@ def run_ours(args):
                       "3xf16": "f32 (MLP: 3xFP16 split on tcgen05, fp32 accumulate)",
                       "tf32": "tf32 MLP, f32 elsewhere"}[args.mlp],
             "data": "synthetic",
-            "config": {"workload": args.workload, "n_atoms": N, "what": w.name + ", NVE velocity Verlet, dt %.2f fs, skin %.1f"
-                       % (w.dt_fs, w.skin), "mlp": args.mlp, "forces": args.forces, "hidden": list(w.model.hidden), "n_heads": w.model.n_heads,
+            "config": {"workload": args.workload, "n_atoms": N, "what": w.name + ", %s velocity Verlet, dt %.2f fs, skin %.1f"
+                       % ("NVT (Nose-Hoover chain 3/2/3, %g K)" % args.nvt if args.nvt > 0 else "NVE", w.dt_fs, w.skin), "mlp": args.mlp, "forces": args.forces, "hidden": list(w.model.hidden), "n_heads": w.model.n_heads,
                        "neighbors_in_list_mean": round(nl_mean, 2), "rebuilds_in_timed_region": nreb,
                        "l2": "inputs_exceed_l2" if N >= 65536 else "working set of this small case is L2-resident",
                        "replicas": world},
@@ -508,6 +510,9 @@ def main():
     ap.add_argument("--no-stages", action="store_true",
                     help="no per-stage CUDA events: the MD loop then replays its step as a CUDA graph (no roofline entry)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--nvt", type=float, default=0.0,
+                    help="temperature in K: run the steps NVT with the paper's Nose-Hoover chain (3/2/3, tau = 100 dt; "
+                         "PAPER.md:365-375) instead of NVE; recorded in config")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
