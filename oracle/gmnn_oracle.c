@@ -36,6 +36,9 @@
  *   O-14 NVT, Nose-Hoover chain (gmnn_oracle.py)  PAPER.md:365-375 (thermostat_chain keys); pins in
  *        tests/test_oracle_nvt.py: conserved extended energy at second order, tau -> inf is O-11, heating
  *        towards the target, closed form and time reversal of one chain operator
+ *   O-15 Langevin, BAOAB + counter-based normals (gmnn_oracle.py)  PAPER.md:266; pins in
+ *        tests/test_oracle_langevin.py: published splitmix64 value, moments and independence of the normals,
+ *        gamma = 0 is O-11, gamma dt >> 1 gives E_kin = 3/2 N kT (units of the noise), relaxation to the target
  *
  * Build: gcc -O2 -std=c11 -fPIC -shared -fopenmp -ffp-contract=off gmnn_oracle.c -lm
  *        (-ffp-contract=off: the neighbour predicate is specified in unfused fp32, reading R20.)

@@ -516,3 +516,65 @@ def nvt_nose_hoover(model: Model, positions, velocities, masses, species, cell, 
         ekin.append(0.5 * ke2())
         cons.append(conserved(r.energy))
     return x, v, np.array(epot), np.array(ekin), np.array(cons)
+
+
+def _splitmix64(seed: int, counters: np.ndarray) -> np.ndarray:
+    """Counter-based generator: output number `counter` (0-based) of the splitmix64 sequence started at `seed`."""
+    with np.errstate(over="ignore"):
+        z = np.uint64(seed) + (counters.astype(np.uint64) + np.uint64(1)) * np.uint64(0x9E3779B97F4A7C15)
+        z = (z ^ (z >> np.uint64(30))) * np.uint64(0xBF58476D1CE4E5B9)
+        z = (z ^ (z >> np.uint64(27))) * np.uint64(0x94D049BB133111EB)
+        return z ^ (z >> np.uint64(31))
+
+
+def langevin_normals(seed: int, step: int, n_atoms: int) -> np.ndarray:
+    """O-15a: the standard normals xi [N][3] of MD step `step` (reading R29).  Atom i takes the two 64-bit words
+    with counters (step N + i) 2 + {0, 1}; their four 32-bit halves (low first) give u = (h + 1) 2^-32 in (0, 1];
+    Box-Muller: xi_x, xi_y = sqrt(-2 ln u1) (cos, sin)(2 pi u2), xi_z = sqrt(-2 ln u3) cos(2 pi u4)."""
+    base = (np.uint64(step) * np.uint64(n_atoms) + np.arange(n_atoms, dtype=np.uint64)) * np.uint64(2)
+    w0, w1 = _splitmix64(seed, base), _splitmix64(seed, base + np.uint64(1))
+    lo, hi = np.uint64(0xFFFFFFFF), np.uint64(32)
+    u = [((h.astype(np.float64)) + 1.0) * 2.0 ** -32 for h in (w0 & lo, w0 >> hi, w1 & lo, w1 >> hi)]
+    r1, r2 = np.sqrt(-2.0 * np.log(u[0])), np.sqrt(-2.0 * np.log(u[2]))
+    return np.stack([r1 * np.cos(2 * np.pi * u[1]), r1 * np.sin(2 * np.pi * u[1]), r2 * np.cos(2 * np.pi * u[3])], 1)
+
+
+def nvt_langevin(model: Model, positions, velocities, masses, species, cell, pbc, dt_fs: float, n_steps: int,
+                 temperature: float, gamma_per_fs: float, seed: int, first_step: int = 0):
+    """O-15: Langevin dynamics ("Langevin thermostat") in the BAOAB splitting (reading R29):
+    v += dt/2 a;  x += dt/2 v;  v = c1 v + sqrt(kT (1 - c1^2) / m) xi, c1 = exp(-gamma dt);  x += dt/2 v;
+    forces;  v += dt/2 a.  Fresh list of radius r_cut every step.  Returns x, v, epot, ekin ([n_steps + 1])."""
+    ACC = 9.648533212e-3
+    x = _f64(positions).copy()
+    v = _f64(velocities).copy()
+    m = _f64(masses)[:, None]
+    L = _f64(cell).reshape(-1)
+    per = np.asarray(pbc).astype(bool)
+    N = x.shape[0]
+    kT = KB_EV * temperature
+    c1 = np.exp(-gamma_per_fs * dt_fs)
+    c2 = np.sqrt(kT * (1.0 - c1 * c1) / m * ACC)  # Ang/fs
+
+    def wrap(y):
+        y = y.copy()
+        y[:, per] -= np.floor(y[:, per] / L[per]) * L[per]
+        return y
+
+    def evaluate(y):
+        y32 = y.astype(np.float32)
+        y32 = np.where(y32 >= np.asarray(cell, np.float32).reshape(-1)[None, :], np.float32(0), y32)
+        return energy_forces(model, y, species, cell, auto_neighbors(y32, cell, pbc, model.r_cut))
+
+    x = wrap(x)
+    r = evaluate(x)
+    epot, ekin = [r.energy], [0.5 * float((m * v * v).sum()) / ACC]
+    for t in range(n_steps):
+        v += 0.5 * dt_fs * r.forces / m * ACC
+        x = x + 0.5 * dt_fs * v
+        v = c1 * v + c2 * langevin_normals(seed, first_step + t, N)
+        x = wrap(x + 0.5 * dt_fs * v)
+        r = evaluate(x)
+        v += 0.5 * dt_fs * r.forces / m * ACC
+        epot.append(r.energy)
+        ekin.append(0.5 * float((m * v * v).sum()) / ACC)
+    return x, v, np.array(epot), np.array(ekin)
