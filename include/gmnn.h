@@ -228,6 +228,14 @@ int gmnn_system_set_nose_hoover(gmnn_system *s, float temperature_K, float tau_f
 int gmnn_system_get_nose_hoover(gmnn_system *s, double *xi /*HOST*/, double *p_xi /*HOST*/,
                                 double *thermostat_energy /*HOST*/, void *cuda_stream);
 
+/* Langevin dynamics for both MD entries, BAOAB splitting: half kick, half
+ * drift, v <- c1 v + sqrt(kT (1 - c1^2) / m) xi with c1 = exp(-gamma dt), half drift, forces, half kick.  xi are
+ * standard normals from a counter-based generator (splitmix64 outputs (step N + i) 2 + {0, 1} of the stream
+ * started at `seed`, Box-Muller in fp64; reading R29), so a trajectory is a function of (seed,
+ * first_step) alone and replays as a CUDA graph; `step` counts MD steps from first_step on (device-side).
+ *   temperature_K <= 0 switches it off; gamma_per_fs >= 0.  Not together with a Nose-Hoover chain. */
+int gmnn_system_set_langevin(gmnn_system *s, float temperature_K, float gamma_per_fs, uint64_t seed, uint64_t first_step);
+
 /* Uncertainty-driven-dynamics bias (Eq. 9) on a model with several
  * heads:  E_b = A [exp(-sigma_E^2 / (N_ens N_atoms B^2)) - 1],  sigma_E^2 = 1/N_ens sum_m (E^(m) - mean)^2 of the
  * heads' TOTAL energies (Eq. 5).  While A != 0, gmnn_energy_forces, gmnn_energy_forces_host, gmnn_md_verlet_steps and

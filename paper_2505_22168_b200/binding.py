@@ -31,7 +31,7 @@ GMNN_FORCE_GATHER, GMNN_FORCE_PAIRBUF = 0, 1
 EXPORTS = (
     "gmnn_n_features", "gmnn_create", "gmnn_destroy", "gmnn_system_create", "gmnn_system_destroy",
     "gmnn_system_set_int", "gmnn_system_get_int", "gmnn_build_neighbors", "gmnn_get_neighbors",
-    "gmnn_energy_forces", "gmnn_energy_forces_host", "gmnn_ensemble_energy_forces", "gmnn_md_verlet_steps", "gmnn_md_ensemble_steps", "gmnn_system_set_nose_hoover", "gmnn_system_get_nose_hoover", "gmnn_system_set_udd_bias", "gmnn_system_get_udd_bias",
+    "gmnn_energy_forces", "gmnn_energy_forces_host", "gmnn_ensemble_energy_forces", "gmnn_md_verlet_steps", "gmnn_md_ensemble_steps", "gmnn_system_set_langevin", "gmnn_system_set_nose_hoover", "gmnn_system_get_nose_hoover", "gmnn_system_set_udd_bias", "gmnn_system_get_udd_bias",
     "gmnn_check", "gmnn_stage_times", "gmnn_debug_read", "gmnn_launch_count", "gmnn_last_error",
 )
 
@@ -77,6 +77,7 @@ def _load() -> C.CDLL:
                                          C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
     lib.gmnn_md_ensemble_steps.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_float, C.c_int32, C.c_int32,
                                            C.c_float] + [C.c_void_p] * 9
+    lib.gmnn_system_set_langevin.argtypes = [C.c_void_p, C.c_float, C.c_float, C.c_uint64, C.c_uint64]
     lib.gmnn_system_set_nose_hoover.argtypes = [C.c_void_p, C.c_float, C.c_float, C.c_int32, C.c_int32, C.c_int32]
     lib.gmnn_system_get_nose_hoover.argtypes = [C.c_void_p] * 5
     lib.gmnn_system_set_udd_bias.argtypes = [C.c_void_p, C.c_float, C.c_float]
@@ -332,6 +333,11 @@ class System:
         _check(lib.gmnn_system_get_nose_hoover(self.handle, xi.ctypes.data_as(C.c_void_p), pxi.ctypes.data_as(C.c_void_p),
                                                C.cast(C.byref(et), C.c_void_p), _stream_ptr(stream)))
         return xi[:n], pxi[:n], float(et.value)
+
+    def set_langevin(self, temperature_K: float, gamma_per_fs: float = 0.01, seed: int = 0, first_step: int = 0) -> None:
+        """Langevin (BAOAB) for the MD entries (temperature_K <= 0: off)."""
+        _check(lib.gmnn_system_set_langevin(self.handle, C.c_float(temperature_K), C.c_float(gamma_per_fs),
+                                            C.c_uint64(seed), C.c_uint64(first_step)))
 
     def set_udd_bias(self, A: float, B: float = 1.0) -> None:
         _check(lib.gmnn_system_set_udd_bias(self.handle, C.c_float(A), C.c_float(B)))

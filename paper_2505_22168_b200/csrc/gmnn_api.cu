@@ -376,7 +376,7 @@ void gmnn_system_destroy(gmnn_system *s) {
     for (int l = 0; l < MAX_LAYERS; ++l) { dev_free(s->H[l]); dev_free(s->D[l]); }
     dev_free(s->dZ[0]); dev_free(s->dZ[1]); dev_free(s->Bv); dev_free(s->BvT); dev_free(s->BvTs); dev_free(s->BvTh); dev_free(s->amax); dev_free(s->vhead); dev_free(s->head_w);
     dev_free(s->ypart); dev_free(s->e_heads); dev_free(s->e_atom); dev_free(s->f_int); dev_free(s->f_tmp); dev_free(s->partial);
-    dev_free(s->e_total); dev_free(s->flags); dev_free(s->ens_scratch); dev_free(s->nhc);
+    dev_free(s->e_total); dev_free(s->flags); dev_free(s->ens_scratch); dev_free(s->nhc); dev_free(s->lang_step);
     dev_free(s->stage_pos); dev_free(s->stage_f); dev_free(s->stage_e);
     if (s->flags_host) cudaFreeHost(s->flags_host);
     for (cudaEvent_t e : s->events) cudaEventDestroy(e);
@@ -758,7 +758,11 @@ int gmnn_md_verlet_steps(gmnn_system *s, float *positions, float *velocities, co
         int r;
         // NVT: chain operator for dt/2 before and after the velocity-Verlet step
         if (s->nhc_len > 0 && (r = launch_nhc_half(s, velocities, ek, dt_fs, q))) return r;
-        if ((r = launch_kick_drift(s, positions, velocities, s->f_tmp, masses, dt_fs, q))) return r;
+        if (s->lang_on) {  // Langevin: B A O A in one pass (the closing B is the kick below)
+            if ((r = launch_baoab(s, positions, velocities, s->f_tmp, masses, dt_fs, q))) return r;
+        } else if ((r = launch_kick_drift(s, positions, velocities, s->f_tmp, masses, dt_fs, q))) {
+            return r;
+        }
         T.mark("kick_drift");
         // rebuild (wrap first) iff the max displacement since the last build exceeds skin/2
         if ((r = launch_build(s, positions, q, s->flags + FLAG_DISP2, thr2, true, positions))) return r;
@@ -913,6 +917,10 @@ int gmnn_system_set_nose_hoover(gmnn_system *s, float temperature_K, float tau_f
         set_error("gmnn_system_set_nose_hoover: tau > 0, 1 <= chain_length <= 8, 1 <= chain_steps <= 16, sy_steps in {1, 3, 5}");
         return GMNN_INVALID_ARG;
     }
+    if (s->lang_on) {
+        set_error("a Langevin thermostat is set: switch it off first (one thermostat at a time)");
+        return GMNN_INVALID_ARG;
+    }
     int rc;
     if (!s->nhc && (rc = dev_alloc(&s->nhc, (size_t)26))) return rc;
     const double kT = 8.617333262e-5 * (double)temperature_K, tau = (double)tau_fs;
@@ -940,6 +948,31 @@ int gmnn_system_get_nose_hoover(gmnn_system *s, double *xi, double *p_xi, double
     GMNN_CUDA(cudaStreamSynchronize(st));
     for (int k = 0; k < s->nhc_len; ++k) xi[k] = h[k], p_xi[k] = h[8 + k];
     *thermostat_energy = h[25];
+    return GMNN_OK;
+}
+
+int gmnn_system_set_langevin(gmnn_system *s, float temperature_K, float gamma_per_fs, uint64_t seed, uint64_t first_step) {
+    if (!s) return GMNN_INVALID_ARG;
+    s->md_state_valid = false;
+    if (!(temperature_K > 0.f)) {  // off
+        s->lang_on = false;
+        return GMNN_OK;
+    }
+    if (!(gamma_per_fs >= 0.f) || !std::isfinite(gamma_per_fs) || !std::isfinite(temperature_K)) {
+        set_error("gmnn_system_set_langevin: gamma >= 0 (1/fs) and a finite temperature");
+        return GMNN_INVALID_ARG;
+    }
+    if (s->nhc_len > 0) {
+        set_error("a Nose-Hoover chain is set: switch it off first (one thermostat at a time)");
+        return GMNN_INVALID_ARG;
+    }
+    int rc;
+    if (!s->lang_step && (rc = dev_alloc(&s->lang_step, (size_t)1))) return rc;
+    GMNN_CUDA(cudaMemcpy(s->lang_step, &first_step, sizeof(uint64_t), cudaMemcpyHostToDevice));
+    s->lang_gamma = (double)gamma_per_fs;
+    s->lang_kT = 8.617333262e-5 * (double)temperature_K;
+    s->lang_seed = seed;
+    s->lang_on = true;
     return GMNN_OK;
 }
 

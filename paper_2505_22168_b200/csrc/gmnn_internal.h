@@ -125,6 +125,10 @@ struct gmnn_system {
     double *nhc = nullptr;           // [26] Nose-Hoover chain: xi[8], p_xi[8], Q[8], scale, thermostat energy (lazy)
     int nhc_len = 0, nhc_chain_steps = 2, nhc_sy_steps = 3;  // nhc_len == 0: NVE
     double nhc_kT = 0.0;
+    bool lang_on = false;            // Langevin (BAOAB) instead of the plain kick + drift
+    double lang_gamma = 0.0, lang_kT = 0.0;  // 1/fs, eV
+    uint64_t lang_seed = 0;
+    uint64_t *lang_step = nullptr;   // device: MD steps since the thermostat was set (counter of the generator)
     float udd_A = 0.f, udd_B = 1.f;  // UDD bias parameters (Eq. 9); active when udd_A != 0 and n_heads > 1
     bool udd_active = false;         // this evaluation adds the bias: e_total[4] = E_b, e_total[5] = sigma_E^2
     bool use_mean_head = false;      // MD on a multi-head model: forward with model->w_mean as the only head
@@ -192,6 +196,7 @@ int launch_series_reset(gmnn_system *s, int32_t next_index, cudaStream_t st);
 int launch_welford(gmnn_system *s, int head, const float *f_head, float *f_mean, float *f_m2, cudaStream_t st);
 int launch_ensemble_energy_stats(gmnn_system *s, float *e_mean, float *e_var, cudaStream_t st);
 int launch_finish_var(int64_t n, float *m2, int n_heads, cudaStream_t st);
+int launch_baoab(gmnn_system *s, float *x, float *v, const float *f, const float *m, float dt, cudaStream_t st);
 int launch_nhc_half(gmnn_system *s, float *v, double *ek, float dt, cudaStream_t st);
 int launch_udd_weights(gmnn_system *s, float *head_w_out, double *scal, cudaStream_t st);
 int launch_uncertainty_scalars(gmnn_system *s, const float *f_var, double *out_d, int32_t *out_bits, cudaStream_t st);

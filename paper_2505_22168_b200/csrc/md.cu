@@ -407,4 +407,64 @@ int launch_nhc_half(gmnn_system *s, float *v, double *ek, float dt, cudaStream_t
     return GMNN_OK;
 }
 
+// ---- Langevin dynamics, BAOAB (reading R29) ----
+__device__ __forceinline__ uint64_t splitmix64_at(uint64_t seed, uint64_t counter) {
+    uint64_t z = seed + (counter + 1ull) * 0x9E3779B97F4A7C15ull;
+    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+    z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+    return z ^ (z >> 31);
+}
+
+// B A O A of one step (the closing B is k_kick): replaces k_kick_drift, skin test included.  The three normals of
+// atom i at step t come from splitmix64 outputs (t N + i) 2 + {0, 1}, Box-Muller in fp64 (the same definition the
+// oracle implements on its own), so the trajectory does not depend on the launch geometry or on replay.
+__global__ void __launch_bounds__(256)
+k_baoab(int64_t N, float *x, float *v, const float *__restrict__ f, const float *__restrict__ m, float dt, double c1,
+        double kT_acc, uint64_t seed, const uint64_t *__restrict__ step, const float *__restrict__ xref, int32_t *flags) {
+    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    float d2 = 0.f;
+    if (i < N) {
+        const uint64_t base = (*step * (uint64_t)N + (uint64_t)i) * 2ull;
+        const uint64_t w0 = splitmix64_at(seed, base), w1 = splitmix64_at(seed, base + 1ull);
+        const double two32 = 1.0 / 4294967296.0, twopi = 6.283185307179586476925286766559;
+        const double u1 = ((double)(uint32_t)w0 + 1.0) * two32, u2 = ((double)(uint32_t)(w0 >> 32) + 1.0) * two32;
+        const double u3 = ((double)(uint32_t)w1 + 1.0) * two32, u4 = ((double)(uint32_t)(w1 >> 32) + 1.0) * two32;
+        const double r1 = sqrt(-2.0 * log(u1)), r2 = sqrt(-2.0 * log(u3));
+        double sn, cs;
+        sincos(twopi * u2, &sn, &cs);
+        const double xi[3] = {r1 * cs, r1 * sn, r2 * cos(twopi * u4)};
+        const float mi = m[i];
+        const float c = 0.5f * dt * (float)ACC_CONV / mi;
+        const float c2 = (float)sqrt(kT_acc * (1.0 - c1 * c1) / (double)mi);
+        const float hdt = 0.5f * dt, c1f = (float)c1;
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            float vv = fmaf(c, f[3 * i + a], v[3 * i + a]);
+            float xx = fmaf(hdt, vv, x[3 * i + a]);
+            vv = fmaf(c1f, vv, c2 * (float)xi[a]);
+            xx = fmaf(hdt, vv, xx);
+            v[3 * i + a] = vv;
+            x[3 * i + a] = xx;
+            const float d = xx - xref[3 * i + a];
+            d2 = fmaf(d, d, d2);
+        }
+    }
+#pragma unroll
+    for (int o = 16; o >= 1; o >>= 1) d2 = fmaxf(d2, __shfl_xor_sync(0xffffffffu, d2, o));
+    if ((threadIdx.x & 31) == 0 && d2 > 0.f) atomicMax(&flags[FLAG_DISP2], __float_as_int(d2));
+}
+
+__global__ void k_inc_u64(uint64_t *p) { *p += 1ull; }
+
+int launch_baoab(gmnn_system *s, float *x, float *v, const float *f, const float *m, float dt, cudaStream_t st) {
+    const double c1 = exp(-s->lang_gamma * (double)dt);
+    k_baoab<<<nblocks(s->N, 256), 256, 0, st>>>(s->N, x, v, f, m, dt, c1, s->lang_kT * ACC_CONV, s->lang_seed, s->lang_step,
+                                                 s->xref, s->flags);
+    GMNN_LAUNCHED();
+    k_inc_u64<<<1, 1, 0, st>>>(s->lang_step);
+    GMNN_LAUNCHED();
+    GMNN_CUDA(cudaGetLastError());
+    return GMNN_OK;
+}
+
 }  // namespace gmnn
