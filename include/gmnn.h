@@ -130,9 +130,8 @@ void gmnn_system_destroy(gmnn_system *s);
  *                     MMAs while the epilogue finishes the previous tile; touches forces only,
  *                     energies come from the forward GEMMs)
  *   "tc_flush_head_fwd" 1..8 (default 1): the same for the forward GEMMs (enters the energies)
- *   "tc_debug"        timing experiments of mlp_tc.cu that knock out work (WRONG results); 0 = off
- *   "cb_halves"       1..6 (default 6): block shape / body of the contraction backward kernel (descriptor.cu)
- *   The tc_* knobs and cb_halves are process-wide.
+ *   The tc_* knobs are process-wide.  (Builds with -DGMNN_EXPERIMENTS add "tc_debug" and "cb_halves", knock-out
+ *   and superseded-variant switches for timing studies; the shipped library rejects them as unknown keys.)
  * Returns GMNN_INVALID_ARG for an unknown key or value. */
 int gmnn_system_set_int(gmnn_system *s, const char *key, int64_t value);
 int gmnn_system_get_int(const gmnn_system *s, const char *key, int64_t *value /*HOST*/);
@@ -152,6 +151,11 @@ int gmnn_build_neighbors(gmnn_system *s, const float *positions /*DEVICE*/, cons
  * (i, j, nx, ny, nz).  Pass i = j = image = NULL to query *n_pairs.  HOST outputs
  * (i, j: int32 [n_pairs]; image: int32 [n_pairs][3]).  Synchronous. */
 int gmnn_get_neighbors(gmnn_system *s, int64_t *n_pairs /*HOST*/, int32_t *i, int32_t *j, int32_t *image);
+
+/* The same for the rows of n_sel chosen atoms only (HOST int32 atoms[n_sel], caller numbering): the parity hook
+ * for boxes whose whole list is too large to sort on the host.  Synchronous. */
+int gmnn_get_neighbor_rows(gmnn_system *s, int64_t n_sel, const int32_t *atoms /*HOST*/, int64_t *n_pairs /*HOST*/,
+                           int32_t *i, int32_t *j, int32_t *image);
 
 /* Eq. 1-4 and the analytic forces on the existing list (pairs with r >= r_cut contribute exactly
  * 0).  positions must be a continuous displacement of those the list was built from (atoms are

@@ -65,12 +65,13 @@ typedef struct {
     int32_t n_hidden;
     int32_t hidden[4];
     int32_t n_heads;
+    int32_t n_weight_sets; /* 1 (or 0): one NN for all species (Eq. 4); n_species: the (W, b) of set Z_i (O-5) */
 } oracle_hparams;
 
 typedef struct {
     const double *beta;  /* [S][S][n_radial][n_basis], centre species first */
-    const double *W[5];  /* layer l: [fan_in][fan_out] row-major */
-    const double *b[5];  /* layer l: [fan_out] */
+    const double *W[5];  /* layer l: [n_weight_sets][fan_in][fan_out] row-major, set-major */
+    const double *b[5];  /* layer l: [n_weight_sets][fan_out] */
     const double *scale; /* [S] sigma_Z */
     const double *shift; /* [S] mu_Z */
 } oracle_weights;
@@ -499,7 +500,9 @@ void oracle_invariants_bwd(int nr, const double *P, const double *gb, double *Q)
 /* ------------------------------------------------------------------------------------------
  * O-5  Readout (Eq. 4): z1 = G W1 + b1; h1 = swish(z1); ...; y = h W_last + b_last
  * in R^M.  swish(x) = x sigmoid(x) (reading R10).  zs holds the pre-activations of the hidden
- * layers back to back (sum of hidden[] doubles).
+ * layers back to back (sum of hidden[] doubles).  Eq. 4 prints one NN for all species (n_weight_sets
+ * = 1, set 0); with n_weight_sets = n_species ("the per-species atomic MLP", reading R11) atom i uses
+ * the (W, b) of set Z_i.  Pins: tests/test_oracle_species_mlp.py.
  * ------------------------------------------------------------------------------------------ */
 static inline double sigmoid_(double x) { return 1.0 / (1.0 + exp(-x)); }
 static inline double swish_(double x) { return x * sigmoid_(x); }
@@ -510,17 +513,31 @@ static inline double dswish_(double x) {
 double oracle_swish(double x) { return swish_(x); }
 double oracle_dswish(double x) { return dswish_(x); }
 
+/* Weights of layer l for weight set `wset` (0 when the NN is shared): O-5, "the (W, b) used are those of set Z_i". */
+static const double *layer_W(const oracle_hparams *hp, const oracle_weights *w, int n_in, int l, int wset) {
+    int fi = l > 0 ? hp->hidden[l - 1] : n_in;
+    int fo = l < hp->n_hidden ? hp->hidden[l] : hp->n_heads;
+    return w->W[l] + (size_t)wset * fi * fo;
+}
+static const double *layer_b(const oracle_hparams *hp, const oracle_weights *w, int l, int wset) {
+    int fo = l < hp->n_hidden ? hp->hidden[l] : hp->n_heads;
+    return w->b[l] + (size_t)wset * fo;
+}
+/* Which weight set atom of species z uses. */
+static int weight_set_of(const oracle_hparams *hp, int z) { return hp->n_weight_sets > 1 ? z : 0; }
+
 void oracle_mlp_forward(const oracle_hparams *hp, const oracle_weights *w, int n_in, const double *G, double *zs,
-                        double *y) {
+                        double *y, int wset) {
     const double *h = G;
     int fan_in = n_in;
     double hbuf[2][4096];
     double *z = zs;
     for (int l = 0; l < hp->n_hidden; ++l) {
         int fo = hp->hidden[l];
+        const double *Wl = layer_W(hp, w, n_in, l, wset), *bl = layer_b(hp, w, l, wset);
         for (int o = 0; o < fo; ++o) {
-            double acc = w->b[l][o];
-            for (int k = 0; k < fan_in; ++k) acc += h[k] * w->W[l][(size_t)k * fo + o];
+            double acc = bl[o];
+            for (int k = 0; k < fan_in; ++k) acc += h[k] * Wl[(size_t)k * fo + o];
             z[o] = acc;
         }
         double *hn = hbuf[l & 1];
@@ -530,9 +547,10 @@ void oracle_mlp_forward(const oracle_hparams *hp, const oracle_weights *w, int n
         fan_in = fo;
     }
     const int L = hp->n_hidden, M = hp->n_heads;
+    const double *WL = layer_W(hp, w, n_in, L, wset), *bL = layer_b(hp, w, L, wset);
     for (int m = 0; m < M; ++m) {
-        double acc = w->b[L][m];
-        for (int k = 0; k < fan_in; ++k) acc += h[k] * w->W[L][(size_t)k * M + m];
+        double acc = bL[m];
+        for (int k = 0; k < fan_in; ++k) acc += h[k] * WL[(size_t)k * M + m];
         y[m] = acc;
     }
 }
@@ -540,14 +558,15 @@ void oracle_mlp_forward(const oracle_hparams *hp, const oracle_weights *w, int n
 /* O-7  Backward to the features: ybar[m] given; hbar = W_last ybar; zbar = hbar * swish'(z);
  * ... ; Gbar = W1 zbar1. */
 void oracle_mlp_backward(const oracle_hparams *hp, const oracle_weights *w, int n_in, const double *zs,
-                         const double *ybar, double *Gbar) {
+                         const double *ybar, double *Gbar, int wset) {
     const int L = hp->n_hidden, M = hp->n_heads;
     double buf[2][4096];
     int width_last = L > 0 ? hp->hidden[L - 1] : n_in;
     double *hb = buf[0];
+    const double *WL = layer_W(hp, w, n_in, L, wset);
     for (int k = 0; k < width_last; ++k) {
         double acc = 0.0;
-        for (int m = 0; m < M; ++m) acc += w->W[L][(size_t)k * M + m] * ybar[m];
+        for (int m = 0; m < M; ++m) acc += WL[(size_t)k * M + m] * ybar[m];
         hb[k] = acc;
     }
     int zoff = 0;
@@ -558,10 +577,11 @@ void oracle_mlp_backward(const oracle_hparams *hp, const oracle_weights *w, int 
         zoff -= fo;
         const double *z = zs + zoff;
         double *nb = buf[(L - l) & 1];
+        const double *Wl = layer_W(hp, w, n_in, l, wset);
         for (int k = 0; k < fi; ++k) nb[k] = 0.0;
         for (int o = 0; o < fo; ++o) {
             double zb = hb[o] * dswish_(z[o]);
-            for (int k = 0; k < fi; ++k) nb[k] += w->W[l][(size_t)k * fo + o] * zb;
+            for (int k = 0; k < fi; ++k) nb[k] += Wl[(size_t)k * fo + o] * zb;
         }
         hb = nb;
     }
@@ -636,7 +656,7 @@ static void forward_all(const oracle_hparams *hp, const oracle_weights *w, int64
         double *Pi = P + (size_t)i * nr * NC;
         moments_of_atom(hp, w->beta, pos, species, L, i, off[i], off[i + 1], pj, pn, Pi);
         oracle_invariants(nr, Pi, G + (size_t)i * F);
-        oracle_mlp_forward(hp, w, F, G + (size_t)i * F, zs + (size_t)i * H, y);
+        oracle_mlp_forward(hp, w, F, G + (size_t)i * F, zs + (size_t)i * H, y, weight_set_of(hp, species[i]));
         for (int m = 0; m < M; ++m) E_heads[(size_t)i * M + m] = w->scale[species[i]] * y[m] + w->shift[species[i]];
     }
 }
@@ -653,7 +673,7 @@ static void backward_all(const oracle_hparams *hp, const oracle_weights *w, int6
     for (int64_t i = 0; i < N; ++i) {
         double ybar[64], Gbar[1024], Qloc[16 * NC];
         for (int m = 0; m < M; ++m) ybar[m] = w->scale[species[i]] * head_w[m];
-        oracle_mlp_backward(hp, w, F, zs + (size_t)i * H, ybar, Gbar);
+        oracle_mlp_backward(hp, w, F, zs + (size_t)i * H, ybar, Gbar, weight_set_of(hp, species[i]));
         oracle_invariants_bwd(nr, P + (size_t)i * nr * NC, Gbar, Qloc);
         if (dG_out) memcpy(dG_out + (size_t)i * F, Gbar, sizeof(double) * F);
         if (Q_out) memcpy(Q_out + (size_t)i * nr * NC, Qloc, sizeof(double) * nr * NC);
@@ -681,6 +701,7 @@ int oracle_energy_forces(const oracle_hparams *hp, const oracle_weights *w, int6
                          const int32_t *pj, const int32_t *pn, const double *head_w, double *E_heads, double *Fout,
                          double *P_out, double *G_out, double *dG_out, double *Q_out) {
     if (hp->n_radial > 16 || hp->n_heads > 64 || hp->n_hidden > 4) return -1;
+    if (hp->n_weight_sets > 1 && hp->n_weight_sets != hp->n_species) return -1;
     const int nr = hp->n_radial, F = oracle_n_features(nr), H = total_hidden(hp);
     if (F > 1024) return -1;
     for (int l = 0; l < hp->n_hidden; ++l)

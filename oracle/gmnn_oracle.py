@@ -36,7 +36,7 @@ class _HParams(C.Structure):
     _fields_ = [
         ("n_species", C.c_int32), ("n_basis", C.c_int32), ("n_radial", C.c_int32),
         ("r_cut", C.c_double), ("r_min", C.c_double), ("gamma", C.c_double),
-        ("n_hidden", C.c_int32), ("hidden", C.c_int32 * 4), ("n_heads", C.c_int32),
+        ("n_hidden", C.c_int32), ("hidden", C.c_int32 * 4), ("n_heads", C.c_int32), ("n_weight_sets", C.c_int32),
     ]
 
 
@@ -99,6 +99,9 @@ class Model:
         self.gamma = float(spec.gamma)
         self.hidden = tuple(int(h) for h in spec.hidden)
         self.n_heads = int(spec.n_heads)
+        # 1: one NN for all species (Eq. 4); n_species: W[l] is [S][fan_in][fan_out], b[l] is [S][fan_out] (O-5)
+        self.n_weight_sets = int(getattr(spec, "n_weight_sets", 1))
+        assert self.n_weight_sets in (1, int(spec.n_species))
         self.beta = _f64(spec.beta)
         self.W = [_f64(w) for w in spec.W]
         self.b = [_f64(b) for b in spec.b]
@@ -106,7 +109,9 @@ class Model:
         self.shift = _f64(spec.shift)
         assert len(self.W) == len(self.hidden) + 1
         self.n_features = n_features(self.n_radial)
-        assert self.W[0].shape[0] == self.n_features, (self.W[0].shape, self.n_features)
+        assert self.W[0].shape[-2] == self.n_features, (self.W[0].shape, self.n_features)
+        if self.n_weight_sets > 1:
+            assert all(w.shape[0] == self.n_weight_sets for w in self.W + self.b)
         self.hp = _HParams()
         self.hp.n_species, self.hp.n_basis, self.hp.n_radial = self.n_species, self.n_basis, self.n_radial
         self.hp.r_cut, self.hp.r_min, self.hp.gamma = self.r_cut, self.r_min, self.gamma
@@ -114,6 +119,7 @@ class Model:
         for l, h in enumerate(self.hidden):
             self.hp.hidden[l] = h
         self.hp.n_heads = self.n_heads
+        self.hp.n_weight_sets = self.n_weight_sets
         self.w = _Weights()
         self.w.beta = _p(self.beta)
         for l in range(len(self.W)):
@@ -195,21 +201,22 @@ def invariants_bwd(n_radial: int, P, gbar) -> np.ndarray:
     return Q
 
 
-def mlp_forward(model: Model, G):
-    """O-5 for one atom: (y [M], zs [sum hidden])."""
+def mlp_forward(model: Model, G, wset: int = 0):
+    """O-5 for one atom with weight set `wset`: (y [M], zs [sum hidden])."""
     G = _f64(G)
     zs = np.zeros(max(1, sum(model.hidden)))
     y = np.zeros(model.n_heads)
-    lib().oracle_mlp_forward(C.byref(model.hp), C.byref(model.w), C.c_int(G.shape[0]), _p(G), _p(zs), _p(y))
+    lib().oracle_mlp_forward(C.byref(model.hp), C.byref(model.w), C.c_int(G.shape[0]), _p(G), _p(zs), _p(y), C.c_int(wset))
     return y, zs
 
 
-def mlp_backward(model: Model, zs, ybar, n_in: int) -> np.ndarray:
-    """O-7 for one atom: dE/dG given ybar [M]."""
+def mlp_backward(model: Model, zs, ybar, n_in: int, wset: int = 0) -> np.ndarray:
+    """O-7 for one atom with weight set `wset`: dE/dG given ybar [M]."""
     zs = _f64(zs)
     ybar = _f64(ybar)
     Gbar = np.zeros(n_in)
-    lib().oracle_mlp_backward(C.byref(model.hp), C.byref(model.w), C.c_int(n_in), _p(zs), _p(ybar), _p(Gbar))
+    lib().oracle_mlp_backward(C.byref(model.hp), C.byref(model.w), C.c_int(n_in), _p(zs), _p(ybar), _p(Gbar),
+                              C.c_int(wset))
     return Gbar
 
 

@@ -15,7 +15,7 @@ from typing import Optional, Sequence, Tuple
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libgmnn_b200.so")
+LIB_PATH = os.environ.get("GMNN_B200_LIB") or os.path.join(_HERE, "libgmnn_b200.so")
 
 GMNN_OK = 0
 GMNN_INVALID_ARG = -1
@@ -30,7 +30,7 @@ GMNN_FORCE_GATHER, GMNN_FORCE_PAIRBUF = 0, 1
 
 EXPORTS = (
     "gmnn_n_features", "gmnn_create", "gmnn_destroy", "gmnn_system_create", "gmnn_system_destroy",
-    "gmnn_system_set_int", "gmnn_system_get_int", "gmnn_build_neighbors", "gmnn_get_neighbors",
+    "gmnn_system_set_int", "gmnn_system_get_int", "gmnn_build_neighbors", "gmnn_get_neighbors", "gmnn_get_neighbor_rows",
     "gmnn_energy_forces", "gmnn_energy_forces_host", "gmnn_ensemble_energy_forces", "gmnn_md_verlet_steps", "gmnn_md_ensemble_steps", "gmnn_system_set_langevin", "gmnn_system_set_nose_hoover", "gmnn_system_get_nose_hoover", "gmnn_system_set_udd_bias", "gmnn_system_get_udd_bias",
     "gmnn_check", "gmnn_stage_times", "gmnn_debug_read", "gmnn_launch_count", "gmnn_last_error",
 )
@@ -91,6 +91,7 @@ def _load() -> C.CDLL:
     lib.gmnn_system_set_int.argtypes = [C.c_void_p, C.c_char_p, C.c_int64]
     lib.gmnn_system_get_int.argtypes = [C.c_void_p, C.c_char_p, C.c_void_p]
     lib.gmnn_get_neighbors.argtypes = [C.c_void_p] * 5
+    lib.gmnn_get_neighbor_rows.argtypes = [C.c_void_p, C.c_int64] + [C.c_void_p] * 5
     lib.gmnn_check.argtypes = [C.c_void_p, C.c_void_p]
     lib.gmnn_stage_times.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p]
     lib.gmnn_debug_read.argtypes = [C.c_void_p, C.c_char_p, C.c_void_p, C.c_int64]
@@ -230,6 +231,18 @@ class System:
         _check(lib.gmnn_get_neighbors(self.handle, C.byref(n), _np_ptr(oi), _np_ptr(oj), _np_ptr(on)))
         return np.concatenate([oi[:, None], oj[:, None], on], axis=1)
 
+    def get_neighbor_rows(self, atoms) -> np.ndarray:
+        """HOST [n_pairs][5] int32 rows (i, j, nx, ny, nz), sorted, of the chosen atoms (caller indices) only."""
+        sel = np.ascontiguousarray(np.asarray(atoms), np.int32)
+        n = C.c_int64(0)
+        _check(lib.gmnn_get_neighbor_rows(self.handle, C.c_int64(sel.shape[0]), _np_ptr(sel), C.byref(n), None, None, None))
+        oi = np.empty(n.value, np.int32)
+        oj = np.empty(n.value, np.int32)
+        on = np.empty((n.value, 3), np.int32)
+        _check(lib.gmnn_get_neighbor_rows(self.handle, C.c_int64(sel.shape[0]), _np_ptr(sel), C.byref(n), _np_ptr(oi),
+                                          _np_ptr(oj), _np_ptr(on)))
+        return np.concatenate([oi[:, None], oj[:, None], on], axis=1)
+
     # -- energy and forces
     def energy_forces(self, positions, energy=None, energy_per_atom=None, forces=None, stream=None,
                       want_per_atom: bool = True):
@@ -365,7 +378,7 @@ class System:
     def debug_read(self, name: str) -> np.ndarray:
         N, m = self.n_atoms, self.model
         shapes = {
-            "perm": ((N,), np.int32), "count": ((N,), np.int32),
+            "perm": ((N,), np.int32), "count": ((N,), np.int32), "xref": ((N, 3), np.float32),
             "psi": ((N, m.n_radial, 20), np.float32), "A": ((N, m.n_radial, 20), np.float32),
             "G": ((N, m.n_features), np.float32), "dG": ((N, m.n_features), np.float32),
             "e_heads": ((N, m.n_heads), np.float32),

@@ -12,13 +12,18 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-LIB = os.path.join(HERE, "libgmnn_b200.so")
+# GMNN_B200_LIB: build to / load from another path (e.g. a -DGMNN_EXPERIMENTS build kept beside the shipped one)
+LIB = os.environ.get("GMNN_B200_LIB") or os.path.join(HERE, "libgmnn_b200.so")
 SOURCES = ["gmnn_api.cu", "neighbor.cu", "descriptor.cu", "mlp_simt.cu", "mlp_tc.cu", "md.cu"]
 HEADERS = ["gmnn_internal.h", "contraction.cuh", "tc_ptx.cuh", os.path.join("..", "..", "include", "gmnn.h")]
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
     "-Xcompiler", "-fPIC", "-cudart", "static", "--expt-relaxed-constexpr",
 ]
+
+
+if os.environ.get("GMNN_EXPERIMENTS"):  # knock-out / superseded-variant knobs for timing studies (never shipped)
+    NVCC_FLAGS.append("-DGMNN_EXPERIMENTS")
 
 
 def _nvcc() -> str:
@@ -36,7 +41,7 @@ def _stale(target: str, deps) -> bool:
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
-    objdir = os.path.join(HERE, "build")
+    objdir = os.path.join(HERE, "build_experiments" if os.environ.get("GMNN_EXPERIMENTS") else "build")
     os.makedirs(objdir, exist_ok=True)
     hdrs = [os.path.normpath(os.path.join(CSRC, h)) for h in HEADERS]
     objs = []

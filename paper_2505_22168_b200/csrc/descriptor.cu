@@ -10,10 +10,13 @@
 // loads of packed entries; each neighbour costs one float4 gather of pos4 (L1/L2 resident: atoms
 // are cell sorted).  The species-pair table beta sits in shared memory.  Per-lane partial moment
 // sums (100 registers) are combined by xor shuffles inside the lane group.
-// Force reduction is the gather form: the full list is symmetric ((i,j,n) <-> (j,i,-n)), so each
-// centre evaluates both directions of every pair itself, g_ij with its own adjoint A_i and g_ji
-// with the neighbour's A_j (a 400-byte read served by L1/L2).  No atomics, fixed summation
-// order, bit-reproducible.
+// Force reduction, two forms, both without atomics, in a fixed summation order, bit-reproducible
+// (the full list is symmetric, (i,j,n) <-> (j,i,-n)):
+//   pair buffer (GMNN_FORCE_PAIRBUF, what bench.py times): g_ij is evaluated once per directed pair with
+//     the centre's own adjoint A_i and stored into the row of j at the slot of the reverse pair (index
+//     built with the list, neighbor.cu); k_force_reduce subtracts each atom's received row in slot order;
+//   gather form (GMNN_FORCE_GATHER): each centre evaluates both directions itself, g_ij with A_i and
+//     g_ji with the neighbour's A_j (a 400-byte read served by L1/L2).
 //
 // Per-pair polynomial: E gets sum_s R_s(r) p_s(u) from pair (i,j), p_s(u) = sum_m A_i[s][m]
 // mono_m(u), so g_ij = dE/dd = (sum_s R'_s p_s) u + (grad_u q - (u.grad_u q) u) / r with
@@ -265,7 +268,8 @@ __constant__ uint16_t c_rot[5 * Feat<5>::N];
 static int upload_rot_table() {
     using F = Feat<5>;
     constexpr int NR = 5;
-    static bool done = false;
+    static bool done_on[MAX_DEVICES] = {};  // c_rot is per-device memory
+    bool &done = done_on[current_device()];
     if (done) return GMNN_OK;
     std::vector<uint16_t> t((size_t)NR * F::N, 0);
     auto sort2 = [](int &a, int &b) { if (a > b) { int x = a; a = b; b = x; } };
@@ -703,7 +707,8 @@ static int pair_backward_lpa(gmnn_system *s, cudaStream_t st, int lpa) {
     }
 #define GMNN_PB(L)                                                                                         \
     case L: {                                                                                              \
-        static size_t opted = 0;                                                                           \
+        static size_t opted_on[MAX_DEVICES] = {};                                                          \
+        size_t &opted = opted_on[current_device()];                                                        \
         if (smem > 48 * 1024 && smem > opted) {                                                            \
             GMNN_CUDA(cudaFuncSetAttribute(k_pair_backward<NR, NB, L, false>,                              \
                                            cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));       \
@@ -757,15 +762,18 @@ int launch_contract_forward(gmnn_system *s, cudaStream_t st) {
     return GMNN_OK;
 }
 
-// knob "cb_halves": block shape of k_contract_backward.  1 = one tile per block; 2 = two tiles, lock step;
-// 3 = one tile, lock step (all three: the full straight-line body); 4 = two tiles, lock step, 5 = one tile,
-// lock step, 6 = one tile per block (default), with the orbit-representative body.  Config 5: 2.57 / 2.25 / - /
-// 1.23 / 1.02 / 1.02 ms
+// The shipped kernel is k_contract_backward<NR, 1, false, true>: one tile per block, orbit-representative
+// body.  The superseded shapes (two tiles per block, lock-step barriers, the fully unrolled body: config 5
+// 2.57 / 2.25 / 1.23 ms against 1.02 ms) are instantiated only in -DGMNN_EXPERIMENTS builds, behind the
+// knob "cb_halves" (1..6).
+#ifdef GMNN_EXPERIMENTS
 int g_cb_halves = 6;
+#endif
 
 template <int NR, int HALVES, bool LOCKSTEP, bool ORBIT>
 static int launch_cb(gmnn_system *s, cudaStream_t st) {
-    static bool attr_set = false;
+    static bool attr_on[MAX_DEVICES] = {};
+    bool &attr_set = attr_on[current_device()];
     if (!attr_set) {
         GMNN_CUDA(cudaFuncSetAttribute(k_contract_backward<NR, HALVES, LOCKSTEP, ORBIT>,
                                        cudaFuncAttributeMaxDynamicSharedMemorySize, (int)CbSmem<NR>::bytes(HALVES)));
@@ -782,15 +790,18 @@ static int launch_cb(gmnn_system *s, cudaStream_t st) {
 int launch_contract_backward(gmnn_system *s, cudaStream_t st) {
     constexpr int NR = 5;
     int rc;
-    if (g_cb_halves >= 4 && (rc = upload_rot_table())) return rc;
+    if ((rc = upload_rot_table())) return rc;
+#ifdef GMNN_EXPERIMENTS
     switch (g_cb_halves) {
         case 1: return launch_cb<NR, 1, false, false>(s, st);
         case 2: return launch_cb<NR, 2, true, false>(s, st);
         case 3: return launch_cb<NR, 1, true, false>(s, st);
         case 4: return launch_cb<NR, 2, true, true>(s, st);
         case 5: return launch_cb<NR, 1, true, true>(s, st);
-        default: return launch_cb<NR, 1, false, true>(s, st);
+        default: break;
     }
+#endif
+    return launch_cb<NR, 1, false, true>(s, st);
 }
 
 }  // namespace gmnn

@@ -23,8 +23,22 @@ void set_error(const char *fmt, ...) {
 }
 
 int launch_mlp_forward_tc(gmnn_system *s, cudaStream_t st);
-extern int g_tc_split_bk, g_tc_flush_k, g_tc_debug, g_tc_pair, g_cb_halves, g_tc_flush_head, g_tc_h_bk, g_tc_flush_head_fwd;
+extern int g_tc_split_bk, g_tc_flush_k, g_tc_pair, g_tc_flush_head, g_tc_h_bk, g_tc_flush_head_fwd;
+#ifdef GMNN_EXPERIMENTS
+extern int g_tc_debug, g_cb_halves;
+#endif
 int launch_mlp_backward_tc(gmnn_system *s, const float *head_w_dev, cudaStream_t st);
+
+// A handle is bound to the device that was current at gmnn_create: per-device state (the weights, the
+// kernels' one-time attributes, __constant__ tables) would be silently wrong from another device.
+static int check_device(int device, const char *who) {
+    int cur = -1;
+    if (cudaGetDevice(&cur) != cudaSuccess || cur != device) {
+        set_error("%s: the handle belongs to CUDA device %d, the current device is %d", who, device, cur);
+        return GMNN_INVALID_ARG;
+    }
+    return GMNN_OK;
+}
 
 template <class T>
 static int dev_alloc(T **p, size_t n) {
@@ -116,9 +130,15 @@ static int ensemble_pass(gmnn_system *s, const float *positions, float *e_mean, 
                          float *f_var, cudaStream_t st) {
     const int M = s->model->hp.n_heads;
     int rc;
-    const int keep_profile = s->profile;
-    s->profile = 0;
+    struct ProfileOff {  // stage events are not recorded inside the pass; restored on every return path
+        gmnn_system *s;
+        int keep;
+        explicit ProfileOff(gmnn_system *s_) : s(s_), keep(s_->profile) { s->profile = 0; }
+        ~ProfileOff() { s->profile = keep; }
+    } profile_off(s);
     if ((rc = launch_gather_positions(s, positions, st, true))) return rc;
+    if (s->mlp_precision == GMNN_MLP_3XF16)  // operand maxima of this evaluation (as forward_backward does)
+        GMNN_CUDA(cudaMemsetAsync(s->amax, 0, sizeof(uint32_t) * AMAX_BVT, st));
     if ((rc = launch_pair_forward(s, st))) return rc;
     if ((rc = launch_contract_forward(s, st))) return rc;
     if ((rc = mlp_forward(s, st))) return rc;
@@ -127,6 +147,8 @@ static int ensemble_pass(gmnn_system *s, const float *positions, float *e_mean, 
     for (int m = 0; m < M; ++m) {
         k_set_onehot<<<1, 64, 0, st>>>(M, m, s->head_w);
         GMNN_LAUNCHED();
+        if (s->mlp_precision == GMNN_MLP_3XF16 && m > 0)  // dZ maxima belong to one head's backward
+            GMNN_CUDA(cudaMemsetAsync(s->amax + AMAX_DZ, 0, sizeof(uint32_t) * 2, st));
         if ((rc = mlp_backward(s, s->head_w, st))) return rc;
         if ((rc = launch_contract_backward(s, st))) return rc;
         if ((rc = launch_pair_backward(s, st))) return rc;
@@ -134,7 +156,6 @@ static int ensemble_pass(gmnn_system *s, const float *positions, float *e_mean, 
         if ((rc = launch_welford(s, m, s->f_tmp, f_mean, f_var, st))) return rc;
     }
     if ((rc = launch_finish_var(3 * s->N, f_var, M, st))) return rc;
-    s->profile = keep_profile;
     GMNN_CUDA(cudaGetLastError());
     return GMNN_OK;
 }
@@ -202,6 +223,7 @@ int gmnn_create(const gmnn_hparams *hp, const gmnn_weights *w, gmnn_model **out)
     }
     gmnn_model *m = new gmnn_model();
     m->hp = *hp;
+    cudaGetDevice(&m->device);
     m->n_features = gmnn_n_features(hp->n_radial);
     m->n_layers = hp->n_hidden + 1;
     m->dims[0] = m->n_features;
@@ -306,8 +328,10 @@ int gmnn_system_create(const gmnn_model *m, int64_t n_atoms, const int32_t *spec
             set_error("species[%lld] = %d out of range", (long long)i, species[i]);
             return GMNN_INVALID_ARG;
         }
+    if (int rcd = check_device(m->device, "gmnn_system_create")) return rcd;
     gmnn_system *s = new gmnn_system();
     s->model = m;
+    s->device = m->device;
     s->N = n_atoms;
     s->mlp_precision = m->hp.mlp_precision;
     s->force_mode = m->hp.force_mode;
@@ -419,9 +443,13 @@ int gmnn_system_set_int(gmnn_system *s, const char *key, int64_t v) {
     } else if (!strcmp(key, "tc_split_bk")) {  // process-wide tuning knob of mlp_tc.cu
         if (v != 16 && v != 32) return GMNN_INVALID_ARG;
         gmnn::g_tc_split_bk = (int)v;
-    } else if (!strcmp(key, "cb_halves")) {  // process-wide: tiles per block of k_contract_backward
-        if (v < 1 || v > 6) return GMNN_INVALID_ARG;  // see descriptor.cu
+#ifdef GMNN_EXPERIMENTS
+    } else if (!strcmp(key, "cb_halves")) {  // superseded block shapes of k_contract_backward (descriptor.cu)
+        if (v < 1 || v > 6) return GMNN_INVALID_ARG;
         gmnn::g_cb_halves = (int)v;
+    } else if (!strcmp(key, "tc_debug")) {  // knock-out timing experiments (wrong results), see mlp_tc.cu
+        gmnn::g_tc_debug = (int)v;
+#endif
     } else if (!strcmp(key, "tc_flush_head")) {  // process-wide, see mlp_tc.cu
         if (v < 0 || v > 8) return GMNN_INVALID_ARG;  // 0: automatic (2 on tf32, 4 on fp16)
         gmnn::g_tc_flush_head = (int)v;
@@ -430,8 +458,6 @@ int gmnn_system_set_int(gmnn_system *s, const char *key, int64_t v) {
         gmnn::g_tc_flush_head_fwd = (int)v;
     } else if (!strcmp(key, "tc_pair")) {  // process-wide: 3xTF32 GEMMs on CTA pairs (1) or single CTAs (0)
         gmnn::g_tc_pair = v != 0;
-    } else if (!strcmp(key, "tc_debug")) {  // timing experiments (wrong results), see mlp_tc.cu
-        gmnn::g_tc_debug = (int)v;
     } else if (!strcmp(key, "tc_h_bk")) {  // process-wide: K extent of a 3xFP16 stage
         if (v != 32 && v != 64) return GMNN_INVALID_ARG;
         gmnn::g_tc_h_bk = (int)v;
@@ -475,6 +501,7 @@ int gmnn_build_neighbors(gmnn_system *s, const float *positions, const float cel
         set_error("gmnn_build_neighbors: null argument");
         return GMNN_INVALID_ARG;
     }
+    if (int rcd = check_device(s->device, "gmnn_build_neighbors")) return rcd;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     if (r_cut != s->model->hp.r_cut) {
         set_error("r_cut = %g differs from the model's %g", r_cut, s->model->hp.r_cut);
@@ -497,7 +524,11 @@ int gmnn_build_neighbors(gmnn_system *s, const float *positions, const float cel
             }
         }
     s->md_state_valid = false;
-    Geometry &g = s->geo;
+    // The handle holds no usable list from here until this call succeeds: an earlier list must never
+    // sit beside the new geometry, a freed row buffer or truncated rows (every failure path below
+    // returns with have_list == false).  The new geometry is filled locally and committed once valid.
+    s->have_list = false;
+    Geometry g{};
     const float r_list = r_cut + skin;  // fl32(fl32(r_cut) + fl32(skin)): the oracle is handed the same float
     g.r_list2 = r_list * r_list;
     g.r_cut2 = r_cut * r_cut;
@@ -530,6 +561,7 @@ int gmnn_build_neighbors(gmnn_system *s, const float *positions, const float cel
         g.kimg[0] = g.kimg[1] = g.kimg[2] = 0;
     }
     for (int a = 0; a < 3; ++a) g.inv_edge[a] = (float)g.ncell[a] / g.L[a];
+    s->geo = g;
     s->small_box = small;
     s->r_cut = r_cut;
     s->skin = skin;
@@ -583,13 +615,11 @@ int gmnn_build_neighbors(gmnn_system *s, const float *positions, const float cel
         if (rc) return rc;
         if ((rc = read_flags(s, st))) return rc;
         if (s->flags_host[FLAG_OUT_OF_BOX]) {
-            s->have_list = false;
             set_error("a position is outside [0, L): wrap positions before gmnn_build_neighbors");
             return GMNN_OUT_OF_BOX;
         }
         if (s->flags_host[FLAG_MAXCOUNT] <= s->cap) {
             if (s->flags_host[FLAG_REV_MISSING]) {
-                s->have_list = false;
                 set_error("internal: the neighbour list is not symmetric (reverse pair missing)");
                 return GMNN_CUDA_ERROR;
             }
@@ -652,12 +682,68 @@ int gmnn_get_neighbors(gmnn_system *s, int64_t *n_pairs, int32_t *oi, int32_t *o
     return GMNN_OK;
 }
 
+int gmnn_get_neighbor_rows(gmnn_system *s, int64_t n_sel, const int32_t *atoms, int64_t *n_pairs, int32_t *oi, int32_t *oj,
+                           int32_t *oimg) {
+    if (!s || !n_pairs || !atoms || n_sel < 0) return GMNN_INVALID_ARG;
+    if (!s->have_list) {
+        set_error("no neighbour list: call gmnn_build_neighbors first");
+        return GMNN_INVALID_ARG;
+    }
+    const size_t N = (size_t)s->N;
+    std::vector<int32_t> perm(N), inv(N);
+    GMNN_CUDA(cudaDeviceSynchronize());
+    GMNN_CUDA(cudaMemcpy(perm.data(), s->perm, sizeof(int32_t) * N, cudaMemcpyDeviceToHost));
+    for (size_t k = 0; k < N; ++k) inv[perm[k]] = (int32_t)k;
+    struct Row { int32_t i, j, n[3]; };
+    std::vector<Row> rows;
+    std::vector<uint32_t> buf((size_t)s->cap);
+    for (int64_t q = 0; q < n_sel; ++q) {
+        if (atoms[q] < 0 || (size_t)atoms[q] >= N) {
+            set_error("gmnn_get_neighbor_rows: atom index %d out of range", atoms[q]);
+            return GMNN_INVALID_ARG;
+        }
+        const size_t k = (size_t)inv[atoms[q]];
+        int32_t cnt = 0;
+        GMNN_CUDA(cudaMemcpy(&cnt, s->count + k, sizeof(int32_t), cudaMemcpyDeviceToHost));
+        GMNN_CUDA(cudaMemcpy(buf.data(), s->nbr + k * (size_t)s->cap, sizeof(uint32_t) * (size_t)cnt, cudaMemcpyDeviceToHost));
+        for (int c = 0; c < cnt; ++c) {
+            const uint32_t e = buf[c];
+            Row r;
+            r.i = atoms[q];
+            r.j = perm[e & NBR_J_MASK];
+            r.n[0] = (int)((e >> NBR_J_BITS) & 7u) - 4;
+            r.n[1] = (int)((e >> (NBR_J_BITS + 3)) & 7u) - 4;
+            r.n[2] = (int)((e >> (NBR_J_BITS + 6)) & 7u) - 4;
+            rows.push_back(r);
+        }
+    }
+    *n_pairs = (int64_t)rows.size();
+    if (!oi && !oj && !oimg) return GMNN_OK;
+    if (!oi || !oj || !oimg) return GMNN_INVALID_ARG;
+    std::stable_sort(rows.begin(), rows.end(), [](const Row &a, const Row &b) {
+        if (a.i != b.i) return a.i < b.i;
+        if (a.j != b.j) return a.j < b.j;
+        if (a.n[0] != b.n[0]) return a.n[0] < b.n[0];
+        if (a.n[1] != b.n[1]) return a.n[1] < b.n[1];
+        return a.n[2] < b.n[2];
+    });
+    for (size_t p = 0; p < rows.size(); ++p) {
+        oi[p] = rows[p].i;
+        oj[p] = rows[p].j;
+        oimg[3 * p] = rows[p].n[0];
+        oimg[3 * p + 1] = rows[p].n[1];
+        oimg[3 * p + 2] = rows[p].n[2];
+    }
+    return GMNN_OK;
+}
+
 int gmnn_energy_forces(gmnn_system *s, const float *positions, double *energy, float *energy_per_atom, float *forces,
                        void *cuda_stream) {
     if (!s || !positions || !energy || !forces) {
         set_error("gmnn_energy_forces: null argument");
         return GMNN_INVALID_ARG;
     }
+    if (int rcd = check_device(s->device, "gmnn_energy_forces")) return rcd;
     if (!s->have_list) {
         set_error("no neighbour list: call gmnn_build_neighbors first");
         return GMNN_INVALID_ARG;
@@ -680,6 +766,7 @@ int gmnn_energy_forces_host(gmnn_system *s, const float *positions, double *ener
         set_error("gmnn_energy_forces_host: null argument");
         return GMNN_INVALID_ARG;
     }
+    if (int rcd = check_device(s->device, "gmnn_energy_forces_host")) return rcd;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const size_t N = (size_t)s->N;
     int rc = GMNN_OK;
@@ -706,6 +793,7 @@ int gmnn_ensemble_energy_forces(gmnn_system *s, const float *positions, float *e
         set_error("gmnn_ensemble_energy_forces: null argument");
         return GMNN_INVALID_ARG;
     }
+    if (int rcd = check_device(s->device, "gmnn_ensemble_energy_forces")) return rcd;
     if (!s->have_list) {
         set_error("no neighbour list: call gmnn_build_neighbors first");
         return GMNN_INVALID_ARG;
@@ -721,6 +809,7 @@ int gmnn_md_verlet_steps(gmnn_system *s, float *positions, float *velocities, co
         set_error("gmnn_md_verlet_steps: bad argument");
         return GMNN_INVALID_ARG;
     }
+    if (int rcd = check_device(s->device, "gmnn_md_verlet_steps")) return rcd;
     if (!s->have_list) {
         set_error("no neighbour list: call gmnn_build_neighbors first");
         return GMNN_INVALID_ARG;
@@ -744,8 +833,10 @@ int gmnn_md_verlet_steps(gmnn_system *s, float *positions, float *velocities, co
         if (epot_series) GMNN_CUDA(cudaMemcpyAsync(epot_series, ep, sizeof(double), cudaMemcpyDeviceToDevice, st));
         if (ekin_series) GMNN_CUDA(cudaMemcpyAsync(ekin_series, ek, sizeof(double), cudaMemcpyDeviceToDevice, st));
     } else {
-        // state at entry: forces of the current positions
-        if ((rc = forward_backward(s, positions, s->model->head_mean_w, false, st, T))) return rc;
+        // state at entry: forces of the current positions; the skin test against the list's build positions
+        // runs here too (a caller whose atoms moved > skin/2 since gmnn_build_neighbors gets
+        // GMNN_STALE_NEIGHBORS at the end of this call instead of a silently stale first step)
+        if ((rc = forward_backward(s, positions, s->model->head_mean_w, true, st, T))) return rc;
         if ((rc = launch_scatter_outputs(s, nullptr, s->f_tmp, st))) return rc;
         if ((rc = launch_energy_sum(s, ep, st, epot_series))) return rc;
         if ((rc = launch_ke(s, velocities, masses, ek, st, ekin_series))) return rc;
@@ -829,7 +920,17 @@ int gmnn_md_verlet_steps(gmnn_system *s, float *positions, float *velocities, co
     if (n_rebuilds) *n_rebuilds = s->flags_host[FLAG_REBUILDS];
     const int maxcount = s->flags_host[FLAG_MAXCOUNT];
     const int rev_missing = s->flags_host[FLAG_REV_MISSING];
+    const int stale = s->flags_host[FLAG_STALE], oob = s->flags_host[FLAG_OUT_OF_BOX];
     GMNN_CUDA(cudaMemsetAsync(s->flags, 0, sizeof(int32_t) * FLAG_WORDS, st));
+    if (stale) {  // raised by the entry evaluation of this call or by an earlier gmnn_energy_forces
+        set_error("an atom had moved more than skin/2 from the positions the neighbour list was built at when "
+                  "gmnn_md_verlet_steps was entered: call gmnn_build_neighbors first");
+        return GMNN_STALE_NEIGHBORS;
+    }
+    if (oob) {  // k_wrap folds periodic axes only: an atom left the box along a non-periodic axis
+        set_error("an atom left the box along a non-periodic axis at an in-loop rebuild (cells there clamp to the edge)");
+        return GMNN_OUT_OF_BOX;
+    }
     if (rev_missing && maxcount <= s->cap) {
         set_error("internal: an in-loop rebuild produced a neighbour list that is not symmetric");
         return GMNN_CUDA_ERROR;
@@ -852,6 +953,7 @@ int gmnn_md_ensemble_steps(gmnn_system *s, float *positions, float *velocities, 
         set_error("gmnn_md_ensemble_steps: bad argument");
         return GMNN_INVALID_ARG;
     }
+    if (int rcd = check_device(s->device, "gmnn_md_ensemble_steps")) return rcd;
     if (!s->have_list) {
         set_error("no neighbour list: call gmnn_build_neighbors first");
         return GMNN_INVALID_ARG;
@@ -1064,6 +1166,7 @@ int gmnn_debug_read(gmnn_system *s, const char *name, void *dst, int64_t bytes) 
     int64_t need = 0;
     if (!strcmp(name, "perm")) { src = s->perm; need = 4 * N; }
     else if (!strcmp(name, "count")) { src = s->count; need = 4 * N; }
+    else if (!strcmp(name, "xref")) { src = s->xref; need = 4 * 3 * N; }
     else if (!strcmp(name, "psi")) { src = s->psi; need = 4 * N * m->hp.n_radial * PSI; }
     else if (!strcmp(name, "A")) { src = s->A; need = 4 * N * m->hp.n_radial * PSI; }
     else if (!strcmp(name, "G")) { src = s->G; need = 4 * N * m->n_features; }

@@ -31,6 +31,15 @@ enum Flag { FLAG_MAXCOUNT = 0, FLAG_STALE = 1, FLAG_OUT_OF_BOX = 2, FLAG_REBUILD
 
 void set_error(const char *fmt, ...);
 extern long long g_launch_count;
+// One-time set-up (function attributes, __constant__ tables) is per DEVICE: the guards are arrays
+// indexed by the current device, never process-wide flags (a handle is bound to the device that was
+// current at gmnn_create and every call checks it).
+constexpr int MAX_DEVICES = 64;
+inline int current_device() {
+    int d = 0;
+    cudaGetDevice(&d);
+    return (d >= 0 && d < MAX_DEVICES) ? d : 0;
+}
 #define GMNN_LAUNCHED() (++::gmnn::g_launch_count)
 
 #define GMNN_CUDA(expr)                                                                          \
@@ -62,6 +71,7 @@ struct RadialParams {  // passed by value to the pair kernels
 
 struct gmnn_model {
     gmnn_hparams hp;
+    int device = 0;            // CUDA device the weights live on (current at gmnn_create)
     int n_features;
     int n_layers;              // n_hidden + 1
     int dims[gmnn::MAX_LAYERS + 1];  // dims[0] = F, hidden..., n_heads
@@ -85,6 +95,7 @@ struct gmnn_model {
 
 struct gmnn_system {
     const gmnn_model *model = nullptr;
+    int device = 0;              // = model->device; calls from another current device are rejected
     int64_t N = 0;
     int32_t *species = nullptr;  // caller order (device)
     // geometry of the last build

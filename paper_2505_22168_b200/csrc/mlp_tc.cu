@@ -43,6 +43,13 @@ namespace gmnn {
 using namespace tc;
 
 enum { EPI_PLAIN = 0, EPI_HIDDEN = 1, EPI_MUL = 2, EPI_HIDDEN_HEAD = 3 };
+// Knock-out timing experiments (wrong results) exist only in builds with -DGMNN_EXPERIMENTS; the
+// shipped library compiles them out.
+#ifdef GMNN_EXPERIMENTS
+#define TC_DBG(p) ((p).debug)
+#else
+#define TC_DBG(p) 0
+#endif
 // EPI_HIDDEN_HEAD: last hidden layer of a single-head model.  h = swish(z) is not stored (the backward
 // needs only swish'); its dot product with the head weights is: every thread writes the partial sum
 // over its columns to ypart[slot][atom], slot = 2 * column tile + column half, and k_heads_finish
@@ -77,7 +84,7 @@ struct TcArgs {
     int n_tiles;   // total
     int flush;     // pipeline stages per accumulator flush (K chunk = flush * BK)
     int flush1;    // ... of the first two chunks of a tile (>= flush)
-    int debug;     // timing experiments only (results wrong): 1 skip split work, 2 hi.hi MMA only, 4 skip stores
+    int debug;     // -DGMNN_EXPERIMENTS builds only (results wrong): 1 skip split work, 2 hi.hi MMA only, 4 skip stores
     float *C;      // [M][N]
     float *C2;     // EPI_HIDDEN: swish'(z)
     const float *bias;
@@ -151,7 +158,7 @@ __device__ __forceinline__ void tc_store_tile(const TcArgs &p, float (&acc)[4][3
     for (int gi = 0; gi < 4; ++gi) {
         const int g = 2 * gi + half;
         const int col0 = n0 + g * 32;
-        if (g >= n_groups || !row_ok || (p.debug & 4)) continue;
+        if (g >= n_groups || !row_ok || (TC_DBG(p) & 4)) continue;
         // TC_EB columns at a time: loads first, then the arithmetic, then the stores, so that the
         // dependency chains (ex2, rcp, fma; DRAM latency of the multiplier) overlap
 #pragma unroll
@@ -205,7 +212,7 @@ __device__ __forceinline__ void tc_store_tile(const TcArgs &p, float (&acc)[4][3
             }
         }
     }
-    if (EPI == EPI_HIDDEN_HEAD && row_ok && !(p.debug & 4))
+    if (EPI == EPI_HIDDEN_HEAD && row_ok && !(TC_DBG(p) & 4))
         p.ypart[(int64_t)(2 * (n0 / p.bn) + half) * p.m_pad + m0 + quad * 32 + lane] = ysum;
 }
 
@@ -293,7 +300,7 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
                     const int ksteps = krem >= BK ? BK / 8 : (krem + 7) / 8;
                     const uint64_t da_hi = make_smem_desc_mn128(a_hi(s), BK * 128), db_hi = make_smem_desc<Cfg::SWZ>(b_hi(s));
                     uint32_t acc = !chunk_first;
-                    if (SPLIT && !(p.debug & 2)) {  // small cross terms first: they meet the smallest accumulator
+                    if (SPLIT && !(TC_DBG(p) & 2)) {  // small cross terms first: they meet the smallest accumulator
                         const uint64_t da_lo = make_smem_desc_mn128(a_lo(s), BK * 128), db_lo = make_smem_desc<Cfg::SWZ>(b_lo(s));
                         for (int k = 0; k < ksteps; ++k) {
                             const uint64_t koff = (uint64_t)((k * 32) >> 4);    // B: 8 tf32 = 32 bytes along the row
@@ -329,7 +336,7 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
                     mbar_wait(bar_full(s), (it / NST) & 1);
                     float4 *ah = reinterpret_cast<float4 *>(smem_gen + (size_t)s * Cfg::STAGE_BYTES);
                     float4 *al = reinterpret_cast<float4 *>(smem_gen + (size_t)s * Cfg::STAGE_BYTES + Cfg::A_BYTES);
-                    if (!(p.debug & 1)) split_hi_lo(ah, al, n_a4, tid);  // B arrives split (model->Ws / WTs)
+                    if (!(TC_DBG(p) & 1)) split_hi_lo(ah, al, n_a4, tid);  // B arrives split (model->Ws / WTs)
                     fence_proxy_async_smem();
                     __syncwarp();
                     if (lane == 0) mbar_arrive(bar_split(s));
@@ -549,7 +556,7 @@ k_gemm_tc_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                     // per k step: B (and a K-major A) advance 32 bytes along the row, the MN-major A one 1024-byte atom
                     const uint64_t astep = F16 ? 2 : 64;
                     uint32_t acc = !chunk_first;
-                    for (int k = 0; k < ksteps && !(p.debug & 2); ++k) {  // small cross terms first
+                    for (int k = 0; k < ksteps && !(TC_DBG(p) & 2); ++k) {  // small cross terms first
                         const uint64_t koff = (uint64_t)(2 * k), aoff = astep * k;
                         if (F16) {
                             mma_f16_ss_pair(d_tmem, da_lo + aoff, db_hi + koff, idesc, acc);
@@ -585,7 +592,7 @@ k_gemm_tc_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                 const int s = it % NST;
                 mbar_wait(bar_full(s), (it / NST) & 1);
                 uint8_t *stage = smem_gen + (size_t)s * Cfg::STAGE_BYTES;
-                if (p.debug & 1) {
+                if (TC_DBG(p) & 1) {
                     if (F16) asm volatile("bar.sync 1, 128;" ::: "memory");
                 } else if (F16) {
                     split_f16_tile<BK>(stage, tid, ascale, p.K - kb * BK);
@@ -654,7 +661,8 @@ k_gemm_tc_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
 template <bool F16, int BK, int EPI>
 static int tc_launch_pair(const CUtensorMap &tmA, const CUtensorMap &tmB, const TcArgs &args, cudaStream_t st) {
     using Cfg = TcPairCfg<F16, BK>;
-    static bool attr_set = false;
+    static bool attr_on[MAX_DEVICES] = {};
+    bool &attr_set = attr_on[current_device()];
     if (!attr_set) {
         GMNN_CUDA(cudaFuncSetAttribute(k_gemm_tc_pair<F16, BK, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES));
         attr_set = true;
@@ -707,10 +715,10 @@ static int make_tmap(CUtensorMap *tm, const float *base, int64_t rows, int K, in
 }
 
 static int tc_num_sms() {
-    static int n = 0;
+    static int n_on[MAX_DEVICES] = {};
+    const int dev = current_device();
+    int &n = n_on[dev];
     if (!n) {
-        int dev = 0;
-        cudaGetDevice(&dev);
         cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev);
         if (n <= 0) n = 148;
     }
@@ -755,7 +763,8 @@ static int make_tmap_a(CUtensorMap *tm, const float *base, int64_t M, int K, int
 template <bool SPLIT, int BK, int EPI>
 static int tc_launch(const CUtensorMap &tmA, const CUtensorMap &tmB, const TcArgs &args, cudaStream_t st) {
     using Cfg = TcCfg<SPLIT, BK>;
-    static bool attr_set = false;
+    static bool attr_on[MAX_DEVICES] = {};
+    bool &attr_set = attr_on[current_device()];
     if (!attr_set) {
         GMNN_CUDA(cudaFuncSetAttribute(k_gemm_tc<SPLIT, BK, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES));
         attr_set = true;
@@ -770,7 +779,9 @@ static int tc_launch(const CUtensorMap &tmA, const CUtensorMap &tmB, const TcArg
 int g_tc_pair = 1;    // knob "tc_pair": 3xTF32 GEMMs on CTA pairs (cta_group::2)
 int g_tc_flush_head = 0;  // knob "tc_flush_head": first-two-chunks multiplier of the backward GEMMs (forces only); 0 = auto
 int g_tc_flush_head_fwd = 1;  // knob "tc_flush_head_fwd": the same for the forward GEMMs (enters the energy)
+#ifdef GMNN_EXPERIMENTS
 int g_tc_debug = 0;
+#endif
 int g_tc_flush_k = 64;   // knob "tc_flush_k": K extent between accumulator flushes of the 3xTF32 / 3xFP16 modes
 int g_tc_split_bk = 32;  // knob (gmnn_system_set_int "tc_split_bk"): K extent of a 3xTF32 stage, 16 or 32
 int g_tc_h_bk = 64;      // knob "tc_h_bk": K extent of a 3xFP16 stage, 32 or 64
@@ -848,7 +859,11 @@ int tc_gemm(bool split, int epi, int64_t M, int N, int K, const float *A, const 
     // MMAs add 16 products per accumulation step instead of 8
     const int head_bwd = g_tc_flush_head > 0 ? g_tc_flush_head : (hf ? 4 : 2);
     a.flush1 = a.flush * (!split ? 1 : (epi != EPI_HIDDEN && epi != EPI_HIDDEN_HEAD) ? head_bwd : g_tc_flush_head_fwd);
+#ifdef GMNN_EXPERIMENTS
     a.debug = g_tc_debug;
+#else
+    a.debug = 0;
+#endif
     a.C = C, a.C2 = C2, a.bias = bias, a.Dmul = Dmul;
     a.w_head = w_head, a.ypart = ypart, a.m_pad = (M + TC_BM - 1) / TC_BM * TC_BM;
     a.amax_a = hf ? hf->amax_a : nullptr, a.amax_b = hf ? hf->amax_b : nullptr, a.amax_out = hf ? hf->amax_out : nullptr;

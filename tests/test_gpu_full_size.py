@@ -24,10 +24,11 @@ def gm():
     return pkg
 
 
-def _cluster_reference(orc, model, w, i, margin=1e-3):
-    """(E_i, F_i) of atom i from the oracle on the free cluster of all atoms within 2 r_cut of it."""
+def _cluster_reference(orc, model, w, i, margin=1e-3, positions=None):
+    """(E_i, F_i) of atom i from the oracle on the free cluster of all atoms within 2 r_cut of it
+    (positions: the box's initial ones, or the ones given, in any periodic image)."""
     L = w.cell.astype(np.float64)
-    x = w.positions.astype(np.float64)
+    x = (w.positions if positions is None else positions).astype(np.float64)
     d = x - x[i]
     d -= L * np.round(d / L)  # minimum image: the boxes here are far larger than 4 r_cut
     keep = np.where((d * d).sum(1) < (2.0 * w.model.r_cut + margin) ** 2)[0]
@@ -37,6 +38,50 @@ def _cluster_reference(orc, model, w, i, margin=1e-3):
     pairs = orc.neighbors(pos, box, (0, 0, 0), w.model.r_cut)
     res = orc.energy_forces(model, pos, w.species[keep], box, pairs)
     return res.e_atom[centre], res.forces[centre], len(keep)
+
+
+def _rows_reference(orc, w, positions32, atoms, r_list):
+    """Oracle rows (i, j, nx, ny, nz) of the chosen atoms: the oracle's own brute-force search (its fp32
+    predicate, all 27 images) run on the atom's surroundings -- every atom within r_list + 0.05 Ang of it in
+    fp64 minimum-image distance; nothing farther can pass the fp32 predicate -- at the atoms' true
+    coordinates in the true cell, keeping the rows whose centre is the chosen atom."""
+    from scipy.spatial import cKDTree
+
+    L = w.cell.astype(np.float64)
+    x = positions32.astype(np.float64)
+    tree = cKDTree(np.mod(x, L), boxsize=L)
+    out = []
+    for i, near in zip(atoms, tree.query_ball_point(np.mod(x[atoms], L), r_list + 0.05)):
+        near = np.sort(np.asarray(near, dtype=np.int64))
+        centre = int(np.searchsorted(near, i))
+        assert near[centre] == i
+        pairs = orc.neighbors(positions32[near], w.cell, w.pbc, r_list, "brute").as_set_array()
+        mine = pairs[pairs[:, 0] == centre].copy()
+        mine[:, 0] = i
+        mine[:, 1] = near[mine[:, 1]]
+        out.append(mine[np.lexsort((mine[:, 4], mine[:, 3], mine[:, 2], mine[:, 1]))])
+    order = np.argsort(np.asarray(atoms), kind="stable")
+    return np.concatenate([out[k] for k in order], axis=0).astype(np.int32)
+
+
+def _check_neighbour_set(sysm, orc, w, N, positions32=None):
+    """north_star: "neighbor lists bit-exact as sorted index sets".  Up to 131 072 atoms the whole list against
+    the oracle's cell list (itself pinned against its brute force, tests/test_oracle_neighbors.py); at 1 048 576
+    atoms (150 M pairs) every row of 1 500 seeded atoms against the oracle's brute force on their surroundings."""
+    from parity_utils import r_list32
+    from workloads.inputs import splitmix64
+
+    x32 = w.positions if positions32 is None else positions32
+    r_list = r_list32(w.model.r_cut, w.skin)
+    if N <= 131072:
+        ref = orc.neighbors(x32, w.cell, w.pbc, r_list, "cells").as_set_array()
+        assert np.array_equal(sysm.get_neighbors(), ref)
+        return
+    atoms = np.unique((splitmix64(977 + N, 1500) % np.uint64(N)).astype(np.int64))
+    got = sysm.get_neighbor_rows(atoms.astype(np.int32))
+    ref = _rows_reference(orc, w, x32, atoms, r_list)
+    assert got.shape[0] > 100 * len(atoms)
+    assert np.array_equal(got, ref)
 
 
 @pytest.mark.parametrize("name,n_samples", [("config3_65536", 24), ("config3_131072", 24), ("config5", 32)])
@@ -64,6 +109,7 @@ def test_full_size_sampled_atoms(gm, orc, name, n_samples):
     r_list = w.model.r_cut + w.skin
     expect = N / float(np.prod(w.cell.astype(np.float64))) * 4.0 / 3.0 * np.pi * r_list ** 3
     assert abs(counts.mean() - expect) <= 0.15 * expect                # list density (a jittered lattice has shells)
+    _check_neighbour_set(sysm, orc, w, N)                              # bit-exact as sorted (i, j, n) sets
     e2, ea2, f2 = sysm.energy_forces(pos)
     assert np.array_equal(f2.cpu().numpy(), f.astype(np.float32))      # bit-reproducible at full size
 
@@ -85,11 +131,15 @@ def test_full_size_sampled_atoms(gm, orc, name, n_samples):
     assert worst_f <= F_TOL
 
 
-def test_config5_md_steps_conserve_energy(gm):
-    """Config 5 at full size through gmnn_md_verlet_steps in bench.py's configuration: the total
-    energy of the NVE run stays put (a property that holds at any size; the trajectory itself is
-    checked against the oracle at 1 536 and 8 192 atoms in test_gpu_ensemble_md.py)."""
+def test_config5_md_steps_conserve_energy_and_match_the_oracle_after_a_rebuild(gm, orc):
+    """Config 5 at full size through gmnn_md_verlet_steps in bench.py's configuration.  (1) The total energy
+    of the NVE run stays put and momentum stays zero (properties that hold at any size).  (2) After steps
+    that include at least one device-side rebuild: the list in the handle equals the oracle's on the rows of
+    1 500 seeded atoms at the rebuild's reference positions, and E_i, F_i of sampled atoms evaluated on the
+    GPU's own final positions match the oracle one by one (SURVEY 8(c-3) "GPU MD vs oracle: state parity")."""
     import torch
+
+    from workloads.inputs import splitmix64
 
     w = wl.make_workload("config5")
     model = gm.Model(w.model, mlp_precision=gm.GMNN_MLP_3XF16, force_mode=gm.GMNN_FORCE_PAIRBUF)
@@ -109,6 +159,37 @@ def test_config5_md_steps_conserve_energy(gm):
     p = (vel * mass[:, None]).sum(0).cpu().numpy()
     v_th = np.sqrt(wl.KB_EV * 300.0 / np.mean(w.masses) * 9.648533212e-3)
     assert np.abs(p).max() / w.masses.sum() <= 1e-5 * v_th
+
+    # (2) continue until the loop has rebuilt the list at least once
+    sysm.set_int("md_continue", 1)
+    steps = 12
+    while nreb == 0 and steps < 60:
+        _, _, more = sysm.md_verlet_steps(pos, vel, mass, w.dt_fs, 6, want_series=False)
+        nreb += more
+        steps += 6
+    assert nreb >= 1, "no in-loop rebuild within %d steps" % steps
+    N = w.n_atoms
+    xref = sysm.debug_read("xref")
+    assert (xref >= 0).all() and (xref < w.cell[None, :]).all()
+    _check_neighbour_set(sysm, orc, w, N, positions32=xref)
+    e, ea, f = sysm.energy_forces(pos)
+    sysm.check()
+    ea = ea.cpu().numpy().astype(np.float64)
+    f = f.cpu().numpy().astype(np.float64)
+    x_now = pos.cpu().numpy()
+    rms = np.sqrt((f ** 2).mean())
+    omodel = orc.Model(w.model)
+    idx = (splitmix64(4242 + N, 24) % np.uint64(N)).astype(np.int64)
+    e_scale = np.abs(ea).mean()
+    worst_e = worst_f = 0.0
+    for i in idx:
+        e_ref, f_ref, _ = _cluster_reference(orc, omodel, w, int(i), positions=x_now)
+        worst_e = max(worst_e, abs(ea[i] - e_ref) / (E_ATOM_RTOL * max(abs(e_ref), e_scale)))
+        worst_f = max(worst_f, np.abs(f[i] - f_ref).max() / rms)
+    print("config5 after %d MD steps, %d rebuilds: worst energy error %.3f x 1e-5, worst force error %.2e of rms"
+          % (steps, nreb, worst_e, worst_f))
+    assert worst_e <= 1.0
+    assert worst_f <= F_TOL
 
 
 def test_config2_full_run(gm, orc):
@@ -137,8 +218,22 @@ def test_config2_full_run(gm, orc):
     assert np.abs(vel.cpu().numpy() - ref.velocities).max() <= 2e-5
     assert np.abs(ep.cpu().numpy() - ref.epot).max() <= 1e-5 * np.abs(ref.epot).max() + 1e-3
     assert np.abs(ek.cpu().numpy() - ref.ekin).max() <= 1e-4 * np.abs(ref.ekin).max()
-    ep2, ek2, nreb2 = sysm.md_verlet_steps(pos, vel, mass, w.dt_fs, 50)
-    etot = np.concatenate([(ep + ek).cpu().numpy(), (ep2 + ek2).cpu().numpy()[1:]])
+    # state parity ten steps further on: the oracle's E, E_i, F at the GPU's own positions,
+    # while the box is still near its initial temperature (it heats up afterwards)
+    epa, eka, nreba = sysm.md_verlet_steps(pos, vel, mass, w.dt_fs, 10)
+    x = pos.cpu().numpy()
+    xw = (x.astype(np.float64) - np.floor(x.astype(np.float64) / L) * L).astype(np.float32)
+    xw = np.where(xw >= w.cell[None, :], 0.0, xw).astype(np.float32)
+    state = orc.energy_forces(orc.Model(w.model), xw, w.species, w.cell, orc.auto_neighbors(xw, w.cell, w.pbc, w.model.r_cut))
+    e20, ea20, f20 = sysm.energy_forces(pos)
+    assert abs(float(epa[-1]) - state.energy) <= 2e-6 * np.abs(state.e_atom).sum()
+    tol = E_ATOM_RTOL * np.maximum(np.abs(state.e_atom), np.abs(state.e_atom).mean())
+    assert np.all(np.abs(ea20.cpu().numpy().astype(np.float64) - state.e_atom) <= tol)
+    ferr = np.abs(f20.cpu().numpy().astype(np.float64) - state.forces).max() / np.sqrt((state.forces ** 2).mean())
+    assert ferr <= F_TOL, ferr
+    ep2, ek2, nreb2 = sysm.md_verlet_steps(pos, vel, mass, w.dt_fs, 40)
+    nreb2 += nreba
+    etot = np.concatenate([(ep + ek).cpu().numpy(), (epa + eka).cpu().numpy()[1:], (ep2 + ek2).cpu().numpy()[1:]])
     assert np.abs(etot - etot[0]).max() <= 2e-3 * np.abs(etot[0])       # 61 energies, 5 eV of 2 566 allowed
     ep3, ek3, nreb3 = sysm.md_verlet_steps(pos, vel, mass, w.dt_fs, 940)
     sysm.check()
@@ -148,3 +243,4 @@ def test_config2_full_run(gm, orc):
     # the state the loop left behind is the state a fresh evaluation gives
     e, ea, f = sysm.energy_forces(pos)
     assert abs(float(e.cpu()[0]) - float(ep3[-1])) <= 1e-6 * float(ea.abs().sum())
+

@@ -92,6 +92,7 @@ class ModelSpec:
     b: List[np.ndarray]  # layer l: [fan_out] f32
     scale: np.ndarray  # [S] f32  sigma_Z
     shift: np.ndarray  # [S] f32  mu_Z
+    n_weight_sets: int = 1  # n_species: one NN per species, W[l] is [S][fan_in][fan_out], b[l] is [S][fan_out]
 
     @property
     def n_features(self) -> int:
@@ -133,6 +134,7 @@ def make_model(
     hidden: Sequence[int] = (512, 512),
     n_heads: int = 1,
     force_scale: float = 1.0,
+    n_weight_sets: int = 1,
 ) -> ModelSpec:
     """Random-init GMNN weights: W ~ N(0, 1/fan_in), b ~ N(0, 0.1^2), beta ~ N(0, 1),
     shift ~ N(0, 1), scale = force_scale (BASELINE.json configs; R10, R17).
@@ -140,7 +142,10 @@ def make_model(
     The draws for beta, scale/shift and each layer come from separate seed streams, so a
     multi-head model (n_heads > 1) shares every tensor except the last layer with the
     single-head model of the same seed (config 4 "last MLP layer replaced by 32 heads").
+    n_weight_sets = n_species draws one NN per species ("the per-species atomic MLP" of north_star): layer l is
+    [S][fan_in][fan_out] from the same stream, so set 0 is the shared model of the same seed.
     """
+    assert n_weight_sets in (1, n_species)
     delta = (r_cut - r_min) / (n_basis - 1)
     gamma = 1.0 / (2.0 * delta * delta)
     S = n_species
@@ -149,14 +154,19 @@ def make_model(
     W, b = [], []
     for l in range(len(dims) - 1):
         fi, fo = dims[l], dims[l + 1]
-        W.append((normal01(seed * 1000 + 10 + 2 * l, fi * fo).reshape(fi, fo) / np.sqrt(fi)).astype(np.float32))
-        b.append((0.1 * normal01(seed * 1000 + 11 + 2 * l, fo)).astype(np.float32))
+        if n_weight_sets == 1:
+            W.append((normal01(seed * 1000 + 10 + 2 * l, fi * fo).reshape(fi, fo) / np.sqrt(fi)).astype(np.float32))
+            b.append((0.1 * normal01(seed * 1000 + 11 + 2 * l, fo)).astype(np.float32))
+        else:
+            T = n_weight_sets
+            W.append((normal01(seed * 1000 + 10 + 2 * l, T * fi * fo).reshape(T, fi, fo) / np.sqrt(fi)).astype(np.float32))
+            b.append((0.1 * normal01(seed * 1000 + 11 + 2 * l, T * fo).reshape(T, fo)).astype(np.float32))
     shift = normal01(seed * 1000 + 2, S).astype(np.float32)
     scale = np.full(S, force_scale, dtype=np.float32)
     return ModelSpec(
         n_species=S, n_basis=n_basis, n_radial=n_radial, r_cut=float(r_cut), r_min=float(r_min),
         gamma=float(gamma), hidden=tuple(int(h) for h in hidden), n_heads=int(n_heads),
-        beta=beta.astype(np.float32), W=W, b=b, scale=scale, shift=shift,
+        beta=beta.astype(np.float32), W=W, b=b, scale=scale, shift=shift, n_weight_sets=int(n_weight_sets),
     )
 
 
@@ -196,7 +206,8 @@ def _species_from_counts(seed: int, counts: Sequence[int]) -> np.ndarray:
     return ids[_shuffle(seed, ids.shape[0])].astype(np.int32)
 
 
-def tiny_box(hidden: Sequence[int] = (512, 512), n_heads: int = 1, seed_shift: int = 0) -> Workload:
+def tiny_box(hidden: Sequence[int] = (512, 512), n_heads: int = 1, seed_shift: int = 0,
+             n_weight_sets: int = 1) -> Workload:
     """Config 1: 64 atoms, 8.5 Ang cube, 2 species 32/32, 4x4x4 lattice + U(-0.3, 0.3) jitter,
     r_cut 5 (box < 2 r_cut, so the same neighbour appears under several images)."""
     s = BASE_SEED + 10 * 1 + seed_shift
@@ -208,14 +219,15 @@ def tiny_box(hidden: Sequence[int] = (512, 512), n_heads: int = 1, seed_shift: i
     species = _species_from_counts(s + 1, (32, 32))
     mass_table = np.array([12.011, 15.999], dtype=np.float32)
     masses = mass_table[species]
-    model = make_model(s + 2, 2, r_cut=5.0, hidden=hidden, n_heads=n_heads, force_scale=FORCE_SCALE["tiny"])
+    model = make_model(s + 2, 2, r_cut=5.0, hidden=hidden, n_heads=n_heads, force_scale=FORCE_SCALE["tiny"],
+                       n_weight_sets=n_weight_sets)
     vel = _maxwell_boltzmann(s + 3, masses, 300.0)
     return Workload("tiny", pos, species, L.astype(np.float32), (1, 1, 1), masses, vel,
                     skin=0.0, dt_fs=0.5, n_steps=0, model=model, species_names=("A", "B"))
 
 
 def ionic_liquid_box(n_pairs: int = 64, hidden: Sequence[int] = (512, 512), n_heads: int = 1,
-                     skin: float = 0.5) -> Workload:
+                     skin: float = 0.5, n_weight_sets: int = 1) -> Workload:
     """Config 2: EMIM+BF4- stoichiometry H11 C6 N2 B1 F4 per ion pair (24 atoms), 1.3 g/cm^3,
     jittered 12^3-type lattice with >= 0.9 Ang minimum distance, r_cut 6, skin 0.5, dt 0.5 fs."""
     s = BASE_SEED + 10 * 2
@@ -237,7 +249,7 @@ def ionic_liquid_box(n_pairs: int = 64, hidden: Sequence[int] = (512, 512), n_he
     species = _species_from_counts(s + 1, tuple(c * n_pairs for c in per_pair))
     masses = mass_table[species]
     model = make_model(s + 2, 5, r_cut=6.0, hidden=hidden, n_heads=n_heads,
-                       force_scale=FORCE_SCALE["ionic_liquid"])
+                       force_scale=FORCE_SCALE["ionic_liquid"], n_weight_sets=n_weight_sets)
     vel = _maxwell_boltzmann(s + 3, masses, 300.0)
     return Workload("ionic_liquid", pos, species, L.astype(np.float32), (1, 1, 1), masses, vel,
                     skin=skin, dt_fs=0.5, n_steps=1000, model=model,
@@ -245,7 +257,7 @@ def ionic_liquid_box(n_pairs: int = 64, hidden: Sequence[int] = (512, 512), n_he
 
 
 def li3po4_box(n_atoms: int, hidden: Sequence[int] = (512, 512), n_heads: int = 1, skin: float = 0.0,
-               n_steps: int = 0, config: int = 3) -> Workload:
+               n_steps: int = 0, config: int = 3, n_weight_sets: int = 1) -> Workload:
     """Configs 3, 4, 5: Li:P:O = 3:1:4 at 2.4 g/cm^3, jittered simple-cubic lattice with
     N(0, 0.1^2) noise clipped at +-0.4 Ang, r_cut 6.  Model weights depend only on the family
     (same seed for every N), positions on (config, N)."""
@@ -266,7 +278,7 @@ def li3po4_box(n_atoms: int, hidden: Sequence[int] = (512, 512), n_heads: int = 
     masses = mass_table[species]
     # one weight seed for the whole Li3PO4 family (configs 3, 4, 5 share the model body)
     model = make_model(BASE_SEED + 10 * 3 + 2, 3, r_cut=6.0, hidden=hidden, n_heads=n_heads,
-                       force_scale=FORCE_SCALE["li3po4"])
+                       force_scale=FORCE_SCALE["li3po4"], n_weight_sets=n_weight_sets)
     vel = _maxwell_boltzmann(s + n_atoms + 3, masses, 300.0)
     return Workload("li3po4_%d" % n_atoms, pos, species, L.astype(np.float32), (1, 1, 1), masses, vel,
                     skin=skin, dt_fs=0.5, n_steps=n_steps, model=model, species_names=("Li", "P", "O"))
