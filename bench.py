@@ -148,9 +148,12 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def make_bench_workload(name: str):
+def make_bench_workload(name: str, weight_sets: str = "shared"):
     import workloads as wl
 
+    if weight_sets == "species":  # one NN per species (north_star's variant of Eq. 4): 3 sets on the Li3PO4 boxes
+        n_species = {"config1": 2, "config2": 5}.get(name, 3)
+        return wl.make_workload(name, n_weight_sets=n_species)
     return wl.make_workload(name)
 
 
@@ -321,7 +324,7 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=dev)
     peaks = load_peaks()
 
-    w = make_bench_workload(args.workload)
+    w = make_bench_workload(args.workload, args.weight_sets)
     N = w.n_atoms
     mlp = MLP_NAMES[args.mlp]
     model = gm.Model(w.model, mlp_precision=mlp, force_mode={"gather": 0, "pairbuf": 1}[args.forces])
@@ -478,6 +481,7 @@ def run_ours(args):
             "data": "synthetic",
             "config": {"workload": args.workload, "n_atoms": N, "what": w.name + ", %s velocity Verlet, dt %.2f fs, skin %.1f"
                        % ("NVT (Nose-Hoover chain 3/2/3, %g K)" % args.nvt if args.nvt > 0 else "NVE", w.dt_fs, w.skin), "mlp": args.mlp, "forces": args.forces, "hidden": list(w.model.hidden), "n_heads": w.model.n_heads,
+                       "weight_sets": w.model.n_weight_sets,
                        "neighbors_in_list_mean": round(nl_mean, 2), "rebuilds_in_timed_region": nreb,
                        "l2": "inputs_exceed_l2" if N >= 65536 else "working set of this small case is L2-resident",
                        "replicas": world},
@@ -507,6 +511,9 @@ def main():
                          "operands; fp32: SIMT FMA; tf32: single pass")
     ap.add_argument("--forces", default="pairbuf", choices=["gather", "pairbuf"],
                     help="force reduction: gather form, or pair buffer with a reverse-pair index (both deterministic)")
+    ap.add_argument("--weight-sets", default="shared", choices=["shared", "species"],
+                    help="shared: one NN for all species (Eq. 4, the headline); species: one NN per species, the rows of the "
+                         "MLP stage grouped by species (a side measurement)")
     ap.add_argument("--no-stages", action="store_true",
                     help="no per-stage CUDA events: the MD loop then replays its step as a CUDA graph (no roofline entry)")
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -40,7 +40,7 @@ typedef struct gmnn_system gmnn_system; /* N atoms, species, neighbour list, all
 typedef enum {
     GMNN_OK = 0,
     GMNN_INVALID_ARG = -1,       /* null pointer, N <= 0, r_cut != model's, non-finite input       */
-    GMNN_UNSUPPORTED = -2,       /* l_max != 3, triclinic cell, per-species weight sets, ...      */
+    GMNN_UNSUPPORTED = -2,       /* l_max != 3, triclinic cell, n_radial / n_basis the kernels lack */
     GMNN_NEIGHBOR_OVERFLOW = -3, /* list capacity exceeded where it cannot be regrown (inside MD) */
     GMNN_STALE_NEIGHBORS = -4,   /* an atom moved > skin/2 since the list was built               */
     GMNN_CUDA_ERROR = -5,
@@ -80,15 +80,17 @@ typedef struct {
     int32_t n_hidden;      /* hidden layers, 1..4 (configs: 2)                                     */
     int32_t hidden[4];     /* widths, multiples of 16, <= 1024 (configs: 512, 512)                 */
     int32_t n_heads;       /* 1, or N_ens <= 64 for the shallow ensemble        */
-    int32_t n_weight_sets; /* 1 = one NN for all species (Eq. 4).  n_species: GMNN_UNSUPPORTED     */
+    int32_t n_weight_sets; /* 1 = one NN for all species (Eq. 4); n_species = one NN per
+                              species ("the per-species atomic MLP"): atom i uses the (W, b) of set Z_i       */
     int32_t mlp_precision; /* gmnn_mlp_precision                                                   */
     int32_t force_mode;    /* gmnn_force_mode                                                      */
 } gmnn_hparams;
 
 typedef struct {            /* HOST pointers, row-major, caller-owned, copied by gmnn_create       */
     const float *beta;      /* [S][S][n_radial][n_basis], centre species first               (R5)  */
-    const float *W[5];      /* layer l: [fan_in][fan_out]; fan_in(0) = n_features, last fan_out = n_heads */
-    const float *b[5];      /* layer l: [fan_out]                                                  */
+    const float *W[5];      /* layer l: [n_weight_sets][fan_in][fan_out], set-major; fan_in(0) = n_features,
+                               last fan_out = n_heads                                              */
+    const float *b[5];      /* layer l: [n_weight_sets][fan_out]                                   */
     const float *scale;     /* [S] sigma_Z                                                         */
     const float *shift;     /* [S] mu_Z                                                            */
 } gmnn_weights;

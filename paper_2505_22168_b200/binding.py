@@ -143,7 +143,14 @@ class Model:
     workloads.ModelSpec (host numpy arrays); weights are copied to the current CUDA device."""
 
     def __init__(self, spec, mlp_precision: int = GMNN_MLP_FP32, force_mode: int = GMNN_FORCE_GATHER,
-                 n_weight_sets: int = 1, l_max: int = 3):
+                 n_weight_sets: Optional[int] = None, l_max: int = 3):
+        if n_weight_sets is None:  # 1: one NN for all species; n_species: W[l] is [S][fan_in][fan_out], b[l] [S][fan_out]
+            n_weight_sets = int(getattr(spec, "n_weight_sets", 1))
+        dims = [n_features(spec.n_radial), *[int(h) for h in spec.hidden], int(spec.n_heads)]
+        for l in range(min(len(spec.W), 5)):  # the library reads n_weight_sets x fan_in x fan_out floats per layer
+            if n_weight_sets >= 1 and (np.asarray(spec.W[l]).size != n_weight_sets * dims[l] * dims[l + 1]
+                                       or np.asarray(spec.b[l]).size != n_weight_sets * dims[l + 1]):
+                raise ValueError("layer %d: weights do not hold %d set(s) of [%d][%d]" % (l, n_weight_sets, dims[l], dims[l + 1]))
         hp = _HParams()
         hp.n_species, hp.n_basis, hp.n_radial, hp.l_max = spec.n_species, spec.n_basis, spec.n_radial, l_max
         hp.r_cut, hp.r_min, hp.gauss_gamma = spec.r_cut, spec.r_min, spec.gamma

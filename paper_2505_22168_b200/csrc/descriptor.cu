@@ -98,7 +98,7 @@ template <int NR, int NB, int LPA>
 __global__ void __launch_bounds__(128)
 k_pair_forward(int64_t N, const float4 *__restrict__ pos4, const uint32_t *__restrict__ nbr,
                const int32_t *__restrict__ count, int cap, Geometry geo, RadialParams rp,
-               const float *__restrict__ beta, float *__restrict__ psi) {
+               const float *__restrict__ beta, float *__restrict__ psi, const int32_t *__restrict__ mrow) {
     constexpr int KB = (NB + 3) & ~3;
     constexpr int ROW = NR * KB;  // floats per (zi, zj) block of the table
     extern __shared__ float s_beta[];
@@ -178,7 +178,8 @@ k_pair_forward(int64_t N, const float4 *__restrict__ pos4, const uint32_t *__res
                 acc[s][q].y += __shfl_xor_sync(0xffffffffu, acc[s][q].y, o);
             }
     if (live) {
-        float4 *out = reinterpret_cast<float4 *>(psi + i * (int64_t)(NR * PSI));
+        const int64_t row = mrow ? (int64_t)mrow[i] : i;  // per-species weight sets: rows grouped by species
+        float4 *out = reinterpret_cast<float4 *>(psi + row * (int64_t)(NR * PSI));
 #pragma unroll
         for (int q = 0; q < NR * PSI / 4; ++q) {
             if (q % LPA == sub) {
@@ -328,7 +329,8 @@ struct CbSmem {  // shared-memory plan of k_contract_backward, in floats
 template <int NR, int HALVES, bool LOCKSTEP, bool ORBIT>
 __global__ void __launch_bounds__(128 * HALVES, 3 - HALVES)
 k_contract_backward(int64_t N, const float *__restrict__ psi, const float *__restrict__ dGt,
-                    const float4 *__restrict__ pos4, const float *__restrict__ scale, float *__restrict__ A) {
+                    const float4 *__restrict__ pos4, const float *__restrict__ scale, float *__restrict__ A,
+                    const int32_t *__restrict__ row_atom) {
     using F = Feat<NR>;
     using CH = FeatChunks<NR>;
     using SM = CbSmem<NR>;
@@ -366,7 +368,8 @@ k_contract_backward(int64_t N, const float *__restrict__ psi, const float *__res
             P[(4 * q + 2) / PSI][(4 * q + 2) % PSI] = v.z;
             P[(4 * q + 3) / PSI][(4 * q + 3) % PSI] = v.w;
         }
-        sig = __ldg(&scale[__float_as_int(pos4[i].w)]);
+        const int64_t atom = row_atom ? (int64_t)row_atom[i] : i;  // N counts rows; padding rows have no atom
+        sig = atom >= 0 ? __ldg(&scale[__float_as_int(pos4[atom].w)]) : 0.f;
     } else {
 #pragma unroll
         for (int s = 0; s < NR; ++s)
@@ -506,7 +509,7 @@ __global__ void __launch_bounds__(128)
 k_pair_backward(int64_t N, const float4 *__restrict__ pos4, const uint32_t *__restrict__ nbr,
                 const int32_t *__restrict__ count, int cap, Geometry geo, RadialParams rp,
                 const float *__restrict__ beta, const float *__restrict__ A, float *__restrict__ f_int,
-                const uint16_t *__restrict__ rev, float4 *__restrict__ gbuf) {
+                const uint16_t *__restrict__ rev, float4 *__restrict__ gbuf, const int32_t *__restrict__ mrow) {
     constexpr int KB = (NB + 3) & ~3;
     constexpr int ROW = NR * KB;
     constexpr int GROUPS = 128 / LPA;
@@ -525,7 +528,8 @@ k_pair_backward(int64_t N, const float4 *__restrict__ pos4, const uint32_t *__re
         const float4 *src = reinterpret_cast<const float4 *>(A);
         for (int q = threadIdx.x; q < GROUPS * (NR * PSI / 4); q += blockDim.x) {
             const int64_t ia = first + q / (NR * PSI / 4);
-            s_A[q] = ia < N ? __ldg(&src[ia * (NR * PSI / 4) + q % (NR * PSI / 4)]) : make_float4(0.f, 0.f, 0.f, 0.f);
+            const int64_t ra = (mrow && ia < N) ? (int64_t)mrow[ia] : ia;  // row of the adjoint (species-grouped rows)
+            s_A[q] = ia < N ? __ldg(&src[ra * (NR * PSI / 4) + q % (NR * PSI / 4)]) : make_float4(0.f, 0.f, 0.f, 0.f);
         }
     }
     __syncthreads();
@@ -596,7 +600,8 @@ k_pair_backward(int64_t N, const float4 *__restrict__ pos4, const uint32_t *__re
                             pair_gradient<NR>([&](int s, int qq) { return Ai[s * (PSI / 4) + qq]; }, R, dR, mono, ux, uy,
                                               uz, rinv, gxo, gyo, gzo);
                         } else {
-                            const float4 *Aj = reinterpret_cast<const float4 *>(A) + (int64_t)pg.j * (NR * PSI / 4);
+                            const float4 *Aj = reinterpret_cast<const float4 *>(A) +
+                                               (int64_t)(mrow ? mrow[pg.j] : pg.j) * (NR * PSI / 4);
                             float mono_r[PSI];  // the neighbour sees the bond reversed
                             monomials(-ux, -uy, -uz, mono_r);
                             float hx, hy, hz;  // gradient with respect to (-u): g_ji in the frame of d_ji = -d_ij
@@ -680,7 +685,7 @@ static int pair_forward_lpa(gmnn_system *s, cudaStream_t st, int lpa) {
 #define GMNN_PF(L)                                                                                        \
     case L:                                                                                               \
         k_pair_forward<NR, NB, L><<<grid, 128, smem, st>>>(s->N, s->pos4, s->nbr, s->count, s->cap, s->geo, \
-                                                           m->rp, m->beta, s->psi);                       \
+                                                           m->rp, m->beta, s->psi, s->mrow);              \
         break;
     switch (lpa) {
         GMNN_PF(1) GMNN_PF(2) GMNN_PF(4) GMNN_PF(8) GMNN_PF(16) GMNN_PF(32)
@@ -718,10 +723,10 @@ static int pair_backward_lpa(gmnn_system *s, cudaStream_t st, int lpa) {
         }                                                                                                  \
         if (pairbuf)                                                                                       \
             k_pair_backward<NR, NB, L, true><<<grid, 128, smem, st>>>(s->N, s->pos4, s->nbr, s->count, s->cap, s->geo, \
-                                                                  m->rp, m->beta, s->A, s->f_int, s->rev, s->gbuf); \
+                                                                  m->rp, m->beta, s->A, s->f_int, s->rev, s->gbuf, s->mrow); \
         else                                                                                               \
             k_pair_backward<NR, NB, L, false><<<grid, 128, smem, st>>>(s->N, s->pos4, s->nbr, s->count, s->cap, s->geo, \
-                                                                   m->rp, m->beta, s->A, s->f_int, nullptr, nullptr); \
+                                                                   m->rp, m->beta, s->A, s->f_int, nullptr, nullptr, s->mrow); \
     } break;
     switch (lpa) {
         GMNN_PB(1) GMNN_PB(2) GMNN_PB(4) GMNN_PB(8) GMNN_PB(16) GMNN_PB(32)
@@ -755,7 +760,7 @@ int launch_pair_backward(gmnn_system *s, cudaStream_t st) {
 
 int launch_contract_forward(gmnn_system *s, cudaStream_t st) {
     constexpr int NR = 5;
-    k_contract_forward<NR><<<nblocks(s->N, 128), 128, 0, st>>>(s->N, s->psi, s->G,
+    k_contract_forward<NR><<<nblocks(s->n_rows, 128), 128, 0, st>>>(s->n_rows, s->psi, s->G,
                                                                s->mlp_precision == GMNN_MLP_3XF16 ? s->amax + AMAX_G : nullptr);
     GMNN_LAUNCHED();
     GMNN_CUDA(cudaGetLastError());
@@ -779,9 +784,9 @@ static int launch_cb(gmnn_system *s, cudaStream_t st) {
                                        cudaFuncAttributeMaxDynamicSharedMemorySize, (int)CbSmem<NR>::bytes(HALVES)));
         attr_set = true;
     }
-    const unsigned tiles = nblocks(s->N, 128);
+    const unsigned tiles = nblocks(s->n_rows, 128);
     k_contract_backward<NR, HALVES, LOCKSTEP, ORBIT><<<(tiles + HALVES - 1) / HALVES, 128 * HALVES, CbSmem<NR>::bytes(HALVES), st>>>(
-        s->N, s->psi, s->dG, s->pos4, s->model->scale, s->A);
+        s->n_rows, s->psi, s->dG, s->pos4, s->model->scale, s->A, s->row_atom);
     GMNN_LAUNCHED();
     GMNN_CUDA(cudaGetLastError());
     return GMNN_OK;

@@ -193,9 +193,10 @@ int gmnn_create(const gmnn_hparams *hp, const gmnn_weights *w, gmnn_model **out)
         set_error("kernels are instantiated for n_radial = 5, n_basis = 7 (got %d, %d)", hp->n_radial, hp->n_basis);
         return GMNN_UNSUPPORTED;
     }
-    if (hp->n_weight_sets != 1) {
-        set_error("n_weight_sets = %d: per-species weight sets are not built yet (DESIGN.md R11)", hp->n_weight_sets);
-        return GMNN_UNSUPPORTED;
+    if (hp->n_weight_sets != 1 && hp->n_weight_sets != hp->n_species) {
+        set_error("n_weight_sets = %d: must be 1 (one NN for all species) or n_species = %d (one NN per species)",
+                  hp->n_weight_sets, hp->n_species);
+        return GMNN_INVALID_ARG;
     }
     if (hp->mlp_precision < 0 || hp->mlp_precision > GMNN_MLP_3XF16 || hp->force_mode < 0 ||
         hp->force_mode > GMNN_FORCE_PAIRBUF) {
@@ -248,23 +249,30 @@ int gmnn_create(const gmnn_hparams *hp, const gmnn_weights *w, gmnn_model **out)
                 for (int k = 0; k < nb; ++k) padded[((size_t)p * nr + s) * rp.kb + k] = w->beta[((size_t)p * nr + s) * nb + k];
         rc = upload(&m->beta, padded.data(), padded.size());
     }
+    const int T = m->n_sets = hp->n_weight_sets;
     for (int l = 0; l < m->n_layers && !rc; ++l) {
         const int fi = m->dims[l], fo = m->dims[l + 1];
-        rc = upload(&m->W[l], w->W[l], (size_t)fi * fo);
-        if (!rc) rc = upload(&m->b[l], w->b[l], (size_t)fo);
-        std::vector<float> t((size_t)fi * fo);
-        for (int a = 0; a < fi; ++a)
-            for (int b = 0; b < fo; ++b) t[(size_t)b * fi + a] = w->W[l][(size_t)a * fo + b];
+        const size_t ws = (size_t)fi * fo;  // one set
+        rc = upload(&m->W[l], w->W[l], ws * T);
+        if (!rc) rc = upload(&m->b[l], w->b[l], (size_t)fo * T);
+        std::vector<float> t(ws * T);
+        for (int q = 0; q < T; ++q)
+            for (int a = 0; a < fi; ++a)
+                for (int b = 0; b < fo; ++b) t[q * ws + (size_t)b * fi + a] = w->W[l][q * ws + (size_t)a * fo + b];
         if (!rc) rc = upload(&m->WT[l], t.data(), t.size());
-        if (!rc) rc = dev_alloc(&m->Ws[l], 2 * (size_t)fi * fo);
-        if (!rc) rc = dev_alloc(&m->WTs[l], 2 * (size_t)fi * fo);
-        if (!rc) rc = launch_split_stack(m->W[l], m->Ws[l], (int64_t)fi * fo, nullptr);
-        if (!rc) rc = launch_split_stack(m->WT[l], m->WTs[l], (int64_t)fi * fo, nullptr);
+        if (!rc) rc = dev_alloc(&m->Ws[l], 2 * ws * T);
+        if (!rc) rc = dev_alloc(&m->WTs[l], 2 * ws * T);
         if (!rc && l == 0) rc = dev_alloc(&m->wmax, (size_t)MAX_LAYERS);
-        if (!rc) rc = dev_alloc(&m->Wh[l], 2 * (size_t)fi * fo);
-        if (!rc) rc = dev_alloc(&m->WTh[l], 2 * (size_t)fi * fo);
-        if (!rc) rc = launch_split_stack_h(m->W[l], m->Wh[l], (int64_t)fi * fo, m->wmax + l, nullptr);
-        if (!rc) rc = launch_split_stack_h(m->WT[l], m->WTh[l], (int64_t)fi * fo, m->wmax + l, nullptr);
+        if (!rc) rc = dev_alloc(&m->Wh[l], 2 * ws * T);
+        if (!rc) rc = dev_alloc(&m->WTh[l], 2 * ws * T);
+        // one fp16 scale per layer, from the maximum over all of its sets
+        if (!rc) rc = launch_absmax(m->W[l], (int64_t)(ws * T), m->wmax + l, nullptr);
+        for (int q = 0; q < T && !rc; ++q) {
+            rc = launch_split_stack(m->W[l] + q * ws, m->Ws[l] + 2 * q * ws, (int64_t)ws, nullptr);
+            if (!rc) rc = launch_split_stack(m->WT[l] + q * ws, m->WTs[l] + 2 * q * ws, (int64_t)ws, nullptr);
+            if (!rc) rc = launch_split_stack_h(m->W[l] + q * ws, m->Wh[l] + 2 * q * ws, (int64_t)ws, m->wmax + l, nullptr);
+            if (!rc) rc = launch_split_stack_h(m->WT[l] + q * ws, m->WTh[l] + 2 * q * ws, (int64_t)ws, m->wmax + l, nullptr);
+        }
     }
     if (!rc && cudaDeviceSynchronize() != cudaSuccess) rc = GMNN_CUDA_ERROR;
     if (!rc) rc = upload(&m->scale, w->scale, (size_t)hp->n_species);
@@ -276,13 +284,14 @@ int gmnn_create(const gmnn_hparams *hp, const gmnn_weights *w, gmnn_model **out)
     if (!rc) {
         // the mean of the heads is itself one linear head (Eq. 6, left-hand side): w_mean = W_last 1/M, b_mean
         const int L = hp->n_hidden, Hd = m->dims[L], M = hp->n_heads;
-        std::vector<float> wm((size_t)Hd + 1);
-        for (int k = 0; k <= Hd; ++k) {
-            const float *row = (k < Hd) ? w->W[L] + (size_t)k * M : w->b[L];
-            double acc = 0.0;
-            for (int q = 0; q < M; ++q) acc += (double)row[q];
-            wm[k] = (float)(acc / M);
-        }
+        std::vector<float> wm(((size_t)Hd + 1) * T);
+        for (int q = 0; q < T; ++q)
+            for (int k = 0; k <= Hd; ++k) {
+                const float *row = (k < Hd) ? w->W[L] + ((size_t)q * Hd + k) * M : w->b[L] + (size_t)q * M;
+                double acc = 0.0;
+                for (int j = 0; j < M; ++j) acc += (double)row[j];
+                wm[(size_t)q * (Hd + 1) + k] = (float)(acc / M);
+            }
         rc = upload(&m->w_mean, wm.data(), wm.size());
     }
     if (rc) {
@@ -337,8 +346,22 @@ int gmnn_system_create(const gmnn_model *m, int64_t n_atoms, const int32_t *spec
     s->force_mode = m->hp.force_mode;
     const size_t N = (size_t)n_atoms;
     const int F = m->n_features, L = m->hp.n_hidden, M = m->hp.n_heads;
+    const int T = m->n_sets;
     int maxw = 0;
     for (int l = 1; l <= L; ++l) maxw = std::max(maxw, m->dims[l]);
+    // rows of the MLP stage: atom order with one weight set, species segments padded to 256 rows otherwise
+    s->n_rows = n_atoms;
+    if (T > 1) {
+        int64_t cnt[MAX_SPECIES] = {}, row = 0;
+        for (size_t i = 0; i < N; ++i) cnt[species[i]]++;
+        for (int z = 0; z < m->hp.n_species; ++z) {
+            s->seg_row0[z] = row;
+            s->seg_rows[z] = cnt[z];
+            row += (cnt[z] + 255) / 256 * 256;
+        }
+        s->n_rows = row;
+    }
+    const size_t R = (size_t)s->n_rows;
     int rc = upload(&s->species, species, N);
 #define A_(p, n) if (!rc) rc = dev_alloc(&(p), (n))
     A_(s->cell_of, N);
@@ -347,24 +370,25 @@ int gmnn_system_create(const gmnn_model *m, int64_t n_atoms, const int32_t *spec
     A_(s->pos4, N);
     A_(s->xref, 3 * N);
     A_(s->count, N);
-    A_(s->psi, N * m->hp.n_radial * PSI);
-    // every matrix of the MLP is tile-transposed, [N/128][width][128], padded to whole tiles (mlp_tc.cu)
-    const size_t NP = (size_t)((N + 127) / 128 * 128);
+    A_(s->psi, R * m->hp.n_radial * PSI);
+    // every matrix of the MLP is tile-transposed, [rows/128][width][128], padded to whole tiles (mlp_tc.cu)
+    const size_t NP = (size_t)((R + 127) / 128 * 128);
     A_(s->G, NP * F);
     A_(s->dG, NP * F);
-    A_(s->A, N * m->hp.n_radial * PSI);
+    A_(s->A, R * m->hp.n_radial * PSI);
     for (int l = 0; l < L; ++l) {
         A_(s->H[l], NP * m->dims[l + 1]);
         A_(s->D[l], NP * m->dims[l + 1]);
     }
     A_(s->dZ[0], NP * maxw);
     A_(s->dZ[1], NP * maxw);
-    A_(s->Bv, (size_t)m->dims[L] * m->dims[L - 1]);
-    A_(s->BvT, (size_t)m->dims[L] * m->dims[L - 1]);
-    A_(s->BvTs, 2 * (size_t)m->dims[L] * m->dims[L - 1]);
-    A_(s->BvTh, 2 * (size_t)m->dims[L] * m->dims[L - 1]);
+    const size_t bv = (size_t)m->dims[L] * m->dims[L - 1];  // per weight set
+    A_(s->Bv, bv * T);
+    A_(s->BvT, bv * T);
+    A_(s->BvTs, 2 * bv * T);
+    A_(s->BvTh, 2 * bv * T);
     A_(s->amax, (size_t)AMAX_SLOTS);
-    A_(s->vhead, (size_t)m->dims[L]);
+    A_(s->vhead, (size_t)m->dims[L] * T);
     A_(s->head_w, (size_t)M);
     A_(s->ypart, (size_t)MAX_HEAD_SLOTS * NP);
     A_(s->e_heads, N * M);
@@ -374,10 +398,19 @@ int gmnn_system_create(const gmnn_model *m, int64_t n_atoms, const int32_t *spec
     A_(s->partial, 2 * 1024);
     A_(s->e_total, 6);  // epot, ekin, sigma_E, bits of sigma_F,max (switching-mode samples)
     A_(s->flags, FLAG_WORDS);
+    if (T > 1) {
+        A_(s->mrow, N);
+        A_(s->row_atom, R);
+        A_(s->sp_count, ((N + 255) / 256 + 1) * MAX_SPECIES);
+    }
 #undef A_
     if (!rc && cudaMallocHost((void **)&s->flags_host, sizeof(int32_t) * FLAG_WORDS) != cudaSuccess) rc = GMNN_OOM;
     if (!rc && cudaMemset(s->flags, 0, sizeof(int32_t) * FLAG_WORDS) != cudaSuccess) rc = GMNN_CUDA_ERROR;
     if (!rc && cudaMemset(s->G, 0, sizeof(float) * NP * F) != cudaSuccess) rc = GMNN_CUDA_ERROR;  // rows of the ragged last tile
+    if (!rc && T > 1) {  // padding rows: no moments (so G = 0 there), no atom
+        if (cudaMemset(s->psi, 0, sizeof(float) * R * m->hp.n_radial * PSI) != cudaSuccess) rc = GMNN_CUDA_ERROR;
+        if (!rc && cudaMemset(s->row_atom, 0xFF, sizeof(int32_t) * R) != cudaSuccess) rc = GMNN_CUDA_ERROR;
+    }
     if (!rc && cudaMemset(s->amax, 0, sizeof(uint32_t) * AMAX_SLOTS) != cudaSuccess) rc = GMNN_CUDA_ERROR;
     if (!rc) {  // swish' lies in [-0.1, 1.1]: its scale is a constant
         const float dmax = 1.5f;
@@ -394,6 +427,7 @@ int gmnn_system_create(const gmnn_model *m, int64_t n_atoms, const int32_t *spec
 
 void gmnn_system_destroy(gmnn_system *s) {
     if (!s) return;
+    dev_free(s->mrow); dev_free(s->row_atom); dev_free(s->sp_count);
     dev_free(s->species); dev_free(s->cell_of); dev_free(s->cell_count); dev_free(s->cell_start);
     dev_free(s->cell_fill); dev_free(s->slot_tmp); dev_free(s->perm); dev_free(s->pos4); dev_free(s->xref);
     dev_free(s->nbr); dev_free(s->rev); dev_free(s->gbuf); dev_free(s->runs); dev_free(s->count); dev_free(s->psi); dev_free(s->G); dev_free(s->dG); dev_free(s->A);
@@ -1183,14 +1217,31 @@ int gmnn_debug_read(gmnn_system *s, const char *name, void *dst, int64_t bytes) 
         return GMNN_INVALID_ARG;
     }
     GMNN_CUDA(cudaDeviceSynchronize());
+    // row-order arrays are handed back in internal atom order: row of atom k = mrow[k] (identity with one weight set)
+    std::vector<int32_t> mrow;
+    if (s->mrow) {
+        mrow.resize((size_t)N);
+        GMNN_CUDA(cudaMemcpy(mrow.data(), s->mrow, sizeof(int32_t) * (size_t)N, cudaMemcpyDeviceToHost));
+    }
+    auto row_of = [&](int64_t k) { return mrow.empty() ? k : (int64_t)mrow[(size_t)k]; };
     if (!strcmp(name, "dG") || !strcmp(name, "G") || !strcmp(name, "H0") || !strcmp(name, "D0")) {
-        // stored as [N/128][F][128] tiles: hand back [N][F]
-        const int64_t F = need / (4 * N), tiles = (N + 127) / 128;
+        // stored as [rows/128][F][128] tiles: hand back [N][F]
+        const int64_t F = need / (4 * N), tiles = (s->n_rows + 127) / 128;
         std::vector<float> tmp((size_t)(tiles * 128 * F));
         GMNN_CUDA(cudaMemcpy(tmp.data(), src, tmp.size() * 4, cudaMemcpyDeviceToHost));
         float *out = static_cast<float *>(dst);
-        for (int64_t i = 0; i < N; ++i)
-            for (int64_t f = 0; f < F; ++f) out[i * F + f] = tmp[(size_t)(((i >> 7) * F + f) * 128 + (i & 127))];
+        for (int64_t k = 0; k < N; ++k) {
+            const int64_t i = row_of(k);
+            for (int64_t f = 0; f < F; ++f) out[k * F + f] = tmp[(size_t)(((i >> 7) * F + f) * 128 + (i & 127))];
+        }
+        return GMNN_OK;
+    }
+    if (!mrow.empty() && (!strcmp(name, "psi") || !strcmp(name, "A"))) {
+        const int64_t W = need / (4 * N);
+        std::vector<float> tmp((size_t)(s->n_rows * W));
+        GMNN_CUDA(cudaMemcpy(tmp.data(), src, tmp.size() * 4, cudaMemcpyDeviceToHost));
+        float *out = static_cast<float *>(dst);
+        for (int64_t k = 0; k < N; ++k) memcpy(out + k * W, tmp.data() + (size_t)(row_of(k) * W), (size_t)W * 4);
         return GMNN_OK;
     }
     GMNN_CUDA(cudaMemcpy(dst, src, (size_t)bytes, cudaMemcpyDeviceToHost));

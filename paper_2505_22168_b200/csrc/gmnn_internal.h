@@ -77,6 +77,11 @@ struct gmnn_model {
     int dims[gmnn::MAX_LAYERS + 1];  // dims[0] = F, hidden..., n_heads
     gmnn::RadialParams rp;
     float *beta = nullptr;     // [S*S][n_radial][kb] zero padded
+    // Weight sets (hp.n_weight_sets: 1 = one NN for all species, Eq. 4; n_species = one NN per species): every
+    // per-layer array below holds the sets back to back (set-major), set t of layer l at offset t * wsize(l)
+    // (bias: t * dims[l + 1]; stacked hi / lo copies: t * 2 * wsize(l)).
+    int n_sets = 1;
+    size_t wsize(int l) const { return (size_t)dims[l] * dims[l + 1]; }
     float *W[gmnn::MAX_LAYERS] = {};   // [fan_in][fan_out]
     float *WT[gmnn::MAX_LAYERS] = {};  // [fan_out][fan_in]
     // tf32 hi / lo split of the two, stacked: rows [0, R) hold hi = tf32(w), rows [R, 2R) lo = w - hi
@@ -90,7 +95,7 @@ struct gmnn_model {
     float *b[gmnn::MAX_LAYERS] = {};
     float *scale = nullptr, *shift = nullptr;  // [S]
     float *head_mean_w = nullptr;  // [n_heads] = 1/M (device)
-    float *w_mean = nullptr;       // [H_last + 1]: W_last 1/M and, last, mean(b_last): the mean of the heads as one head
+    float *w_mean = nullptr;       // per set [H_last + 1]: W_last 1/M and, last, mean(b_last): the mean of the heads as one head
 };
 
 struct gmnn_system {
@@ -121,7 +126,17 @@ struct gmnn_system {
     bool list_has_rev = false;
     int cap = 0;
     int cap_request = 0;
-    // workspaces (internal order)
+    // MLP rows.  With one weight set the per-atom matrices of the MLP stage (psi, G, H, D, dZ, dG, A) are in
+    // internal atom order: row = atom, n_rows = N, mrow = row_atom = nullptr.  With per-species sets the rows
+    // are grouped by species so that every 256-row tile pair of the GEMMs uses ONE weight set: species z owns
+    // rows [seg_row0[z], seg_row0[z] + seg_rows[z]) of a segment padded to a multiple of 256 (padding rows keep
+    // psi = 0 and are never read back); inside a segment atoms keep their internal (cell) order.  mrow[k] = row
+    // of internal atom k, row_atom[r] = internal atom of row r or -1; both are rebuilt with the list.
+    int64_t n_rows = 0;
+    int64_t seg_row0[gmnn::MAX_SPECIES] = {}, seg_rows[gmnn::MAX_SPECIES] = {};
+    int32_t *mrow = nullptr, *row_atom = nullptr;
+    int32_t *sp_count = nullptr;     // [blocks of 256 atoms][MAX_SPECIES] scratch of the row assignment
+    // workspaces (row order)
     float *psi = nullptr, *G = nullptr, *dG = nullptr, *A = nullptr;
     float *H[gmnn::MAX_LAYERS] = {}, *D[gmnn::MAX_LAYERS] = {};
     float *dZ[2] = {};
@@ -173,6 +188,30 @@ struct gmnn_system {
 
 namespace gmnn {
 
+// One launch unit of the MLP stage: a run of rows that uses one weight set.  One segment (all rows, set 0)
+// with a shared NN; one per non-empty species with per-species sets (rows padded to a multiple of 256).
+struct MlpSeg {
+    int64_t row0;  // first row (a multiple of 128: a tile boundary of the tile-transposed matrices)
+    int64_t rows;  // rows handed to the GEMMs (real rows, or the padded segment)
+    int64_t real;  // rows that carry an atom
+    int set;
+};
+inline int mlp_segments(const gmnn_system *s, MlpSeg *seg) {
+    if (s->model->n_sets == 1) {
+        seg[0] = MlpSeg{0, s->N, s->N, 0};
+        return 1;
+    }
+    int n = 0;
+    for (int z = 0; z < s->model->hp.n_species; ++z)
+        if (s->seg_rows[z] > 0) seg[n++] = MlpSeg{s->seg_row0[z], (s->seg_rows[z] + 255) / 256 * 256, s->seg_rows[z], z};
+    return n;
+}
+// first element of row block `row0` of a tile-transposed [rows/128][width][128] matrix
+template <class T>
+inline T *tile_rows(T *base, int64_t row0, int width) {
+    return base + (row0 / 128) * (int64_t)width * 128;
+}
+
 // neighbor.cu
 int launch_build(gmnn_system *s, const float *positions, cudaStream_t st, const int32_t *cond, float thr2,
                  bool wrap_first, float *positions_mut);
@@ -186,7 +225,8 @@ int launch_pair_backward(gmnn_system *s, cudaStream_t st);  // dispatches on for
 
 // mlp_tc.cu
 int launch_split_stack(const float *src, float *dst, int64_t n, cudaStream_t st);  // dst[0..n) hi, dst[n..2n) lo
-int launch_split_stack_h(const float *src, uint16_t *dst, int64_t n, uint32_t *amax, cudaStream_t st);  // fp16, scaled by *amax
+int launch_absmax(const float *src, int64_t n, uint32_t *amax, cudaStream_t st);  // *amax = max |src| (reset first)
+int launch_split_stack_h(const float *src, uint16_t *dst, int64_t n, const uint32_t *amax, cudaStream_t st);  // fp16, scaled by *amax
 
 // mlp_simt.cu
 int launch_mlp_forward_simt(gmnn_system *s, cudaStream_t st);

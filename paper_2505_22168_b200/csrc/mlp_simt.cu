@@ -129,12 +129,16 @@ static int sgemm(int epi, int64_t M, int N, int K, const float *A, const float *
 
 // One thread per atom, H tile-transposed (coalesced along atoms): y_m = h . W_last[:, m] + b_last[m];
 // E^(m) = sigma y_m + mu; e_atom = sum_m c_m E^(m).  Heads are taken 8 at a time.
+// Rows row0 .. row0 + rows of one segment (Ht, Wl, bl already point at the segment / its weight set); e_heads and
+// e_atom are indexed by the internal atom of the row (row_atom; identity when null).
 __global__ void __launch_bounds__(128)
-k_heads(int64_t N, const float *__restrict__ Ht, int Hd, const float *__restrict__ Wl, const float *__restrict__ bl,
-        int M, const float4 *__restrict__ pos4, const float *__restrict__ scale, const float *__restrict__ shift,
-        const float *__restrict__ head_w, float *__restrict__ e_heads, float *__restrict__ e_atom) {
-    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;  // blockDim.x == 128 == tile
-    if (i >= N) return;
+k_heads(int64_t row0, int64_t rows, const float *__restrict__ Ht, int Hd, const float *__restrict__ Wl,
+        const float *__restrict__ bl, int M, const float4 *__restrict__ pos4, const float *__restrict__ scale,
+        const float *__restrict__ shift, const float *__restrict__ head_w, float *__restrict__ e_heads,
+        float *__restrict__ e_atom, const int32_t *__restrict__ row_atom) {
+    const int64_t r = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;  // blockDim.x == 128 == tile
+    if (r >= rows) return;
+    const int64_t i = row_atom ? (int64_t)row_atom[row0 + r] : row0 + r;
     const float *h = Ht + (int64_t)blockIdx.x * Hd * 128 + threadIdx.x;
     const int z = __float_as_int(pos4[i].w);
     const float sg = __ldg(&scale[z]), mu = __ldg(&shift[z]);
@@ -190,24 +194,33 @@ __global__ void k_scale_cols(int rows, int cols, const float *__restrict__ W, co
 int launch_mlp_forward_simt(gmnn_system *s, cudaStream_t st) {
     const gmnn_model *m = s->model;
     s->heads_fused = false;
+    MlpSeg seg[MAX_SPECIES];
+    const int ns = mlp_segments(s, seg);
     const float *X = s->G;
     for (int l = 0; l < m->hp.n_hidden; ++l) {
-        int rc = sgemm(EPI_HIDDEN, s->N, m->dims[l + 1], m->dims[l], X, m->W[l], s->H[l], m->b[l], s->D[l], nullptr, st);
-        if (rc) return rc;
+        const int fi = m->dims[l], fo = m->dims[l + 1];
+        for (int q = 0; q < ns; ++q) {
+            const int64_t r0 = seg[q].row0;
+            int rc = sgemm(EPI_HIDDEN, seg[q].rows, fo, fi, tile_rows(X, r0, fi), m->W[l] + seg[q].set * m->wsize(l),
+                           tile_rows(s->H[l], r0, fo), m->b[l] + seg[q].set * fo, tile_rows(s->D[l], r0, fo), nullptr, st);
+            if (rc) return rc;
+        }
         X = s->H[l];
     }
     return GMNN_OK;
 }
 
 // Single head fused into the last GEMM epilogue (mlp_tc.cu): add the partial sums in slot order.
-__global__ void k_heads_finish(int64_t N, const float *__restrict__ ypart, int n_slots, int64_t m_pad,
+__global__ void k_heads_finish(int64_t row0, int64_t rows, const float *__restrict__ ypart, int n_slots, int64_t m_pad,
                                const float *__restrict__ bl, const float4 *__restrict__ pos4,
                                const float *__restrict__ scale, const float *__restrict__ shift,
-                               const float *__restrict__ head_w, float *__restrict__ e_heads, float *__restrict__ e_atom) {
-    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    if (i >= N) return;
+                               const float *__restrict__ head_w, float *__restrict__ e_heads, float *__restrict__ e_atom,
+                               const int32_t *__restrict__ row_atom) {
+    const int64_t r = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (r >= rows) return;
     float y = 0.f;
-    for (int q = 0; q < n_slots; ++q) y += __ldg(ypart + q * m_pad + i);
+    for (int q = 0; q < n_slots; ++q) y += __ldg(ypart + q * m_pad + row0 + r);
+    const int64_t i = row_atom ? (int64_t)row_atom[row0 + r] : row0 + r;
     const int z = __float_as_int(pos4[i].w);
     const float em = __ldg(&scale[z]) * (y + __ldg(&bl[0])) + __ldg(&shift[z]);
     if (e_heads) {
@@ -220,26 +233,29 @@ __global__ void k_heads_finish(int64_t N, const float *__restrict__ ypart, int n
 
 int launch_mlp_heads(gmnn_system *s, const float *head_w_dev, cudaStream_t st) {
     const gmnn_model *m = s->model;
-    const int L = m->hp.n_hidden;
-    if (s->heads_fused) {
-        const bool mean = m->hp.n_heads > 1;  // fused on a multi-head model: the folded mean head (use_mean_head)
-        k_heads_finish<<<(unsigned)((s->N + 255) / 256), 256, 0, st>>>(s->N, s->ypart, s->head_slots,
-                                                                        (s->N + 127) / 128 * 128,
-                                                                        mean ? m->w_mean + m->dims[L] : m->b[L], s->pos4,
-                                                                        m->scale, m->shift, head_w_dev,
-                                                                        mean ? nullptr : s->e_heads, s->e_atom);
-        GMNN_LAUNCHED();
-        GMNN_CUDA(cudaGetLastError());
-        return GMNN_OK;
-    }
-    if (m->dims[L] > 1024) {
+    const int L = m->hp.n_hidden, Hd = m->dims[L], M = m->dims[L + 1];
+    MlpSeg seg[MAX_SPECIES];
+    const int ns = mlp_segments(s, seg);
+    if (!s->heads_fused && Hd > 1024) {
         set_error("last hidden width > 1024");
         return GMNN_UNSUPPORTED;
     }
-    k_heads<<<(unsigned)((s->N + 127) / 128), 128, 0, st>>>(s->N, s->H[L - 1], m->dims[L], m->W[L], m->b[L],
-                                                                 m->dims[L + 1], s->pos4, m->scale, m->shift, head_w_dev,
-                                                                 s->e_heads, s->e_atom);
-    GMNN_LAUNCHED();
+    for (int q = 0; q < ns; ++q) {
+        const int64_t r0 = seg[q].row0, real = seg[q].real;
+        const int t = seg[q].set;
+        if (s->heads_fused) {
+            const bool mean = m->hp.n_heads > 1;  // fused on a multi-head model: the folded mean head (use_mean_head)
+            k_heads_finish<<<(unsigned)((real + 255) / 256), 256, 0, st>>>(
+                r0, real, s->ypart, s->head_slots, (s->n_rows + 127) / 128 * 128,
+                mean ? m->w_mean + (size_t)t * (Hd + 1) + Hd : m->b[L] + (size_t)t * M, s->pos4, m->scale, m->shift,
+                head_w_dev, mean ? nullptr : s->e_heads, s->e_atom, s->row_atom);
+        } else {
+            k_heads<<<(unsigned)((real + 127) / 128), 128, 0, st>>>(
+                r0, real, tile_rows(s->H[L - 1], r0, Hd), Hd, m->W[L] + t * m->wsize(L), m->b[L] + (size_t)t * M, M, s->pos4,
+                m->scale, m->shift, head_w_dev, s->e_heads, s->e_atom, s->row_atom);
+        }
+        GMNN_LAUNCHED();
+    }
     GMNN_CUDA(cudaGetLastError());
     return GMNN_OK;
 }
@@ -249,13 +265,17 @@ int launch_mlp_seed(gmnn_system *s, const float *head_w_dev, cudaStream_t st) {
     const gmnn_model *m = s->model;
     const int L = m->hp.n_hidden;
     const int Hd = m->dims[L], prev = m->dims[L - 1];
-    k_head_vec<<<(Hd + 127) / 128, 128, 0, st>>>(Hd, m->dims[L + 1], m->W[L], head_w_dev, s->vhead);
-    GMNN_LAUNCHED();
-    if (s->mlp_precision == GMNN_MLP_FP32)
-        k_scale_rows<<<(unsigned)(((int64_t)Hd * prev + 255) / 256), 256, 0, st>>>(Hd, prev, m->WT[L - 1], s->vhead, s->Bv);
-    else
-        k_scale_cols<<<(unsigned)(((int64_t)Hd * prev + 255) / 256), 256, 0, st>>>(prev, Hd, m->W[L - 1], s->vhead, s->BvT);
-    GMNN_LAUNCHED();
+    const size_t bv = (size_t)Hd * prev;
+    for (int t = 0; t < m->n_sets; ++t) {  // one seeded operand per weight set
+        float *v = s->vhead + (size_t)t * Hd;
+        k_head_vec<<<(Hd + 127) / 128, 128, 0, st>>>(Hd, m->dims[L + 1], m->W[L] + t * m->wsize(L), head_w_dev, v);
+        GMNN_LAUNCHED();
+        if (s->mlp_precision == GMNN_MLP_FP32)
+            k_scale_rows<<<(unsigned)((bv + 255) / 256), 256, 0, st>>>(Hd, prev, m->WT[L - 1] + t * bv, v, s->Bv + t * bv);
+        else
+            k_scale_cols<<<(unsigned)((bv + 255) / 256), 256, 0, st>>>(prev, Hd, m->W[L - 1] + t * bv, v, s->BvT + t * bv);
+        GMNN_LAUNCHED();
+    }
     GMNN_CUDA(cudaGetLastError());
     return GMNN_OK;
 }
@@ -265,20 +285,28 @@ int launch_mlp_backward_simt(gmnn_system *s, const float *head_w_dev, cudaStream
     const int L = m->hp.n_hidden;
     int rc = launch_mlp_seed(s, head_w_dev, st);
     if (rc) return rc;
+    MlpSeg seg[MAX_SPECIES];
+    const int ns = mlp_segments(s, seg);
     const float *Aop = s->D[L - 1];
-    const float *Bop = s->Bv;
     int cur = 0;
     for (int l = L - 1; l >= 0; --l) {
-        // out[N][dims[l]] = Aop[N][dims[l+1]] . Bop[dims[l+1]][dims[l]]
+        // out[rows][dims[l]] = Aop[rows][dims[l+1]] . Bop[dims[l+1]][dims[l]], Bop = diag(v) W^T of the last hidden
+        // layer first, then W^T of the layers below
+        const int fo = m->dims[l], fi = m->dims[l + 1];
+        for (int q = 0; q < ns; ++q) {
+            const int64_t r0 = seg[q].row0;
+            const float *Bop = (l == L - 1) ? s->Bv + seg[q].set * m->wsize(l) : m->WT[l] + seg[q].set * m->wsize(l);
+            if (l > 0)
+                rc = sgemm(EPI_MUL, seg[q].rows, fo, fi, tile_rows(Aop, r0, fi), Bop, tile_rows(s->dZ[cur], r0, fo), nullptr,
+                           nullptr, tile_rows(s->D[l - 1], r0, fo), st);
+            else
+                rc = sgemm(EPI_PLAIN, seg[q].rows, fo, fi, tile_rows(Aop, r0, fi), Bop, tile_rows(s->dG, r0, fo), nullptr, nullptr,
+                           nullptr, st);
+            if (rc) return rc;
+        }
         if (l > 0) {
-            rc = sgemm(EPI_MUL, s->N, m->dims[l], m->dims[l + 1], Aop, Bop, s->dZ[cur], nullptr, nullptr, s->D[l - 1], st);
-            if (rc) return rc;
             Aop = s->dZ[cur];
-            Bop = m->WT[l - 1];
             cur ^= 1;
-        } else {
-            rc = sgemm(EPI_PLAIN, s->N, m->dims[0], m->dims[1], Aop, Bop, s->dG, nullptr, nullptr, nullptr, st);
-            if (rc) return rc;
         }
     }
     return GMNN_OK;

@@ -843,7 +843,7 @@ struct TcHalf {
 // `hf` (3xFP16, always on CTA pairs) the fp16 split hf->Bh replaces Bt.
 int tc_gemm(bool split, int epi, int64_t M, int N, int K, const float *A, const float *Bt, float *C, const float *bias,
             float *C2, const float *Dmul, cudaStream_t st, const float *w_head = nullptr, float *ypart = nullptr,
-            int *n_slots = nullptr, const TcHalf *hf = nullptr) {
+            int *n_slots = nullptr, const TcHalf *hf = nullptr, int64_t m_pad_total = 0) {
     if (K % 8 != 0 || N % 8 != 0 || M <= 0 || M > INT32_MAX) {
         set_error("tensor-core MLP: widths must be multiples of 8 (K = %d, N = %d)", K, N);
         return GMNN_UNSUPPORTED;
@@ -865,7 +865,8 @@ int tc_gemm(bool split, int epi, int64_t M, int N, int K, const float *A, const 
     a.debug = 0;
 #endif
     a.C = C, a.C2 = C2, a.bias = bias, a.Dmul = Dmul;
-    a.w_head = w_head, a.ypart = ypart, a.m_pad = (M + TC_BM - 1) / TC_BM * TC_BM;
+    // ypart is [slots][m_pad]: with row segments the caller hands ypart + row0 and the padded row count of the whole matrix
+    a.w_head = w_head, a.ypart = ypart, a.m_pad = m_pad_total > 0 ? m_pad_total : (M + TC_BM - 1) / TC_BM * TC_BM;
     a.amax_a = hf ? hf->amax_a : nullptr, a.amax_b = hf ? hf->amax_b : nullptr, a.amax_out = hf ? hf->amax_out : nullptr;
     if (n_slots) *n_slots = 2 * a.n_tiles_n;
     CUtensorMap tmA, tmB;
@@ -928,11 +929,17 @@ __global__ void k_split_stack_h(const float *__restrict__ src, __half *__restric
     dst[n + t] = __float2half_rn(v - __half2float(h));
 }
 
-// *amax = max |src| (reset first), then the stacked fp16 split
-int launch_split_stack_h(const float *src, uint16_t *dst, int64_t n, uint32_t *amax, cudaStream_t st) {
+// *amax = max |src| (reset first)
+int launch_absmax(const float *src, int64_t n, uint32_t *amax, cudaStream_t st) {
     GMNN_CUDA(cudaMemsetAsync(amax, 0, sizeof(uint32_t), st));
     k_absmax<<<(unsigned)((n + 1023) / 1024 < 256 ? (n + 1023) / 1024 : 256), 256, 0, st>>>(src, n, amax);
     GMNN_LAUNCHED();
+    GMNN_CUDA(cudaGetLastError());
+    return GMNN_OK;
+}
+
+// the stacked fp16 split of src scaled by the power of two that *amax (>= max |src|) fixes
+int launch_split_stack_h(const float *src, uint16_t *dst, int64_t n, const uint32_t *amax, cudaStream_t st) {
     k_split_stack_h<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(src, reinterpret_cast<__half *>(dst), n, amax);
     GMNN_LAUNCHED();
     GMNN_CUDA(cudaGetLastError());
@@ -958,20 +965,30 @@ int launch_mlp_forward_tc(gmnn_system *s, cudaStream_t st) {
     const gmnn_model *m = s->model;
     const bool f16 = s->mlp_precision == GMNN_MLP_3XF16;
     const bool split = s->mlp_precision == GMNN_MLP_3XTF32 || f16;
+    MlpSeg seg[MAX_SPECIES];
+    const int ns = mlp_segments(s, seg);
+    const int64_t m_pad = (s->n_rows + TC_BM - 1) / TC_BM * TC_BM;
     const float *X = s->G;
     for (int l = 0; l < m->hp.n_hidden; ++l) {
         // z = X W[l]: the B operand is W[l]^T = WT[l], [fan_out][fan_in]
         // single head: the last hidden layer's epilogue takes the head's dot product itself
-        const bool fuse = l == m->hp.n_hidden - 1 && (m->hp.n_heads == 1 || s->use_mean_head) && 2 * ((m->dims[l + 1] + 127) / 128) <= MAX_HEAD_SLOTS;
+        const int fi = m->dims[l], fo = m->dims[l + 1];
+        const bool fuse = l == m->hp.n_hidden - 1 && (m->hp.n_heads == 1 || s->use_mean_head) && 2 * ((fo + 127) / 128) <= MAX_HEAD_SLOTS;
         s->heads_fused = fuse;
-        TcHalf hf;
-        hf.Bh = m->WTh[l], hf.amax_b = m->wmax + l;
-        hf.amax_a = s->amax + (l == 0 ? AMAX_G : AMAX_H + l - 1), hf.amax_out = s->amax + AMAX_H + l;
-        int rc = tc_gemm(split, fuse ? EPI_HIDDEN_HEAD : EPI_HIDDEN, s->N, m->dims[l + 1], m->dims[l], X,
-                         split ? m->WTs[l] : m->WT[l], s->H[l], m->b[l], s->D[l], nullptr, st,
-                         (fuse && s->use_mean_head) ? m->w_mean : m->W[l + 1], s->ypart,
-                         &s->head_slots, f16 ? &hf : nullptr);
-        if (rc) return rc;
+        for (int q = 0; q < ns; ++q) {  // layer-major: every segment of layer l before layer l + 1 (operand maxima)
+            const int64_t r0 = seg[q].row0;
+            const int t = seg[q].set;
+            const size_t ws = m->wsize(l);
+            TcHalf hf;
+            hf.Bh = m->WTh[l] + 2 * t * ws, hf.amax_b = m->wmax + l;
+            hf.amax_a = s->amax + (l == 0 ? AMAX_G : AMAX_H + l - 1), hf.amax_out = s->amax + AMAX_H + l;
+            const float *w_head = (fuse && s->use_mean_head) ? m->w_mean + (size_t)t * (fo + 1) : m->W[l + 1] + t * m->wsize(l + 1);
+            int rc = tc_gemm(split, fuse ? EPI_HIDDEN_HEAD : EPI_HIDDEN, seg[q].rows, fo, fi, tile_rows(X, r0, fi),
+                             split ? m->WTs[l] + 2 * t * ws : m->WT[l] + t * ws, tile_rows(s->H[l], r0, fo),
+                             m->b[l] + (size_t)t * fo, tile_rows(s->D[l], r0, fo), nullptr, st, w_head, s->ypart + r0,
+                             &s->head_slots, f16 ? &hf : nullptr, m_pad);
+            if (rc) return rc;
+        }
         X = s->H[l];
     }
     return GMNN_OK;
@@ -984,34 +1001,47 @@ int launch_mlp_backward_tc(gmnn_system *s, const float *head_w_dev, cudaStream_t
     const bool f16 = s->mlp_precision == GMNN_MLP_3XF16;
     const bool split = s->mlp_precision == GMNN_MLP_3XTF32 || f16;
     const int L = m->hp.n_hidden;
-    int rc = launch_mlp_seed(s, head_w_dev, st);  // vhead, Bv (and BvT, see mlp_simt.cu)
+    int rc = launch_mlp_seed(s, head_w_dev, st);  // vhead, BvT per weight set (see mlp_simt.cu)
     if (rc) return rc;
-    const float *Aop = s->D[L - 1];
-    const int64_t nbv = (int64_t)m->dims[L] * m->dims[L - 1];
-    if (f16) {
-        if ((rc = launch_split_stack_h(s->BvT, s->BvTh, nbv, s->amax + AMAX_BVT, st))) return rc;
-    } else if (split && (rc = launch_split_stack(s->BvT, s->BvTs, nbv, st))) {
-        return rc;
+    const size_t nbv = (size_t)m->dims[L] * m->dims[L - 1];
+    if (f16) {  // one scale for the seeded operands of all sets
+        if ((rc = launch_absmax(s->BvT, (int64_t)(nbv * m->n_sets), s->amax + AMAX_BVT, st))) return rc;
+        for (int t = 0; t < m->n_sets; ++t)
+            if ((rc = launch_split_stack_h(s->BvT + t * nbv, s->BvTh + 2 * t * nbv, (int64_t)nbv, s->amax + AMAX_BVT, st))) return rc;
+    } else if (split) {
+        for (int t = 0; t < m->n_sets; ++t)
+            if ((rc = launch_split_stack(s->BvT + t * nbv, s->BvTs + 2 * t * nbv, (int64_t)nbv, st))) return rc;
     }
-    const float *BopT = split ? s->BvTs : s->BvT;
-    TcHalf hf;
-    hf.Bh = s->BvTh, hf.amax_b = s->amax + AMAX_BVT, hf.amax_a = s->amax + AMAX_D;  // A = swish' of the last hidden layer
+    MlpSeg seg[MAX_SPECIES];
+    const int ns = mlp_segments(s, seg);
+    const float *Aop = s->D[L - 1];
     int cur = 0;
     for (int l = L - 1; l >= 0; --l) {
+        const int fo = m->dims[l], fi = m->dims[l + 1];  // out = Aop [rows][fi] . Bop [fi][fo]
+        const size_t ws = m->wsize(l);
+        for (int q = 0; q < ns; ++q) {
+            const int64_t r0 = seg[q].row0;
+            const int t = seg[q].set;
+            const bool seeded = l == L - 1;  // B operand: W[L-1] diag(v) of this set, then the plain W[l]
+            const float *BopT = seeded ? (split ? s->BvTs + 2 * t * ws : s->BvT + t * ws) : (split ? m->Ws[l] + 2 * t * ws : m->W[l] + t * ws);
+            TcHalf hf;
+            hf.Bh = seeded ? s->BvTh + 2 * t * ws : m->Wh[l] + 2 * t * ws;
+            hf.amax_b = seeded ? s->amax + AMAX_BVT : m->wmax + l;
+            hf.amax_a = seeded ? s->amax + AMAX_D : s->amax + AMAX_DZ + (cur ^ 1);  // swish' of the last hidden layer, then dZ
+            if (l > 0) {
+                hf.amax_out = s->amax + AMAX_DZ + cur;
+                rc = tc_gemm(split, EPI_MUL, seg[q].rows, fo, fi, tile_rows(Aop, r0, fi), BopT, tile_rows(s->dZ[cur], r0, fo),
+                             nullptr, nullptr, tile_rows(s->D[l - 1], r0, fo), st, nullptr, nullptr, nullptr, f16 ? &hf : nullptr);
+            } else {
+                hf.amax_out = nullptr;
+                rc = tc_gemm(split, EPI_PLAIN, seg[q].rows, fo, fi, tile_rows(Aop, r0, fi), BopT, tile_rows(s->dG, r0, fo), nullptr,
+                             nullptr, nullptr, st, nullptr, nullptr, nullptr, f16 ? &hf : nullptr);
+            }
+            if (rc) return rc;
+        }
         if (l > 0) {
-            hf.amax_out = s->amax + AMAX_DZ + cur;
-            rc = tc_gemm(split, EPI_MUL, s->N, m->dims[l], m->dims[l + 1], Aop, BopT, s->dZ[cur], nullptr, nullptr, s->D[l - 1], st,
-                         nullptr, nullptr, nullptr, f16 ? &hf : nullptr);
-            if (rc) return rc;
             Aop = s->dZ[cur];
-            BopT = split ? m->Ws[l - 1] : m->W[l - 1];
-            hf.Bh = m->Wh[l - 1], hf.amax_b = m->wmax + l - 1, hf.amax_a = s->amax + AMAX_DZ + cur;
             cur ^= 1;
-        } else {
-            hf.amax_out = nullptr;
-            rc = tc_gemm(split, EPI_PLAIN, s->N, m->dims[0], m->dims[1], Aop, BopT, s->dG, nullptr, nullptr, nullptr, st,
-                         nullptr, nullptr, nullptr, f16 ? &hf : nullptr);
-            if (rc) return rc;
         }
     }
     return GMNN_OK;

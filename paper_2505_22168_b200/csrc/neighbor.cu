@@ -398,6 +398,63 @@ k_build_rev_runs(int64_t N, const uint32_t *__restrict__ nbr, const int32_t *__r
     }
 }
 
+// ---- rows of the MLP stage for per-species weight sets (gmnn_internal.h: mrow, row_atom) ---------------
+// mrow[k] = seg_row0[z_k] + number of internal atoms before k with the same species: a stable counting
+// sort by species of the cell-ordered atoms, so rows keep the spatial order inside a species segment and
+// the assignment is a pure function of the positions (bit-reproducible).  Three small kernels per rebuild.
+struct SegRows {
+    int64_t row0[MAX_SPECIES];
+};
+
+__global__ void __launch_bounds__(256)
+k_species_block_count(int64_t N, const float4 *__restrict__ pos4, int32_t *sp_count, const int32_t *cond, float thr2) {
+    if (skip_rebuild(cond, thr2)) return;
+    __shared__ int32_t c[MAX_SPECIES];
+    if (threadIdx.x < MAX_SPECIES) c[threadIdx.x] = 0;
+    __syncthreads();
+    const int64_t k = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (k < N) atomicAdd(&c[__float_as_int(pos4[k].w)], 1);  // integer: order-free
+    __syncthreads();
+    if (threadIdx.x < MAX_SPECIES) sp_count[blockIdx.x * (int64_t)MAX_SPECIES + threadIdx.x] = c[threadIdx.x];
+}
+
+// one thread per species: exclusive scan of its per-block counts, offset by the segment's first row
+__global__ void k_species_scan(int64_t n_blocks, int32_t *sp_count, SegRows seg, const int32_t *cond, float thr2) {
+    if (skip_rebuild(cond, thr2)) return;
+    const int z = threadIdx.x;
+    if (z >= MAX_SPECIES) return;
+    int64_t run = seg.row0[z];
+    for (int64_t b = 0; b < n_blocks; ++b) {
+        const int32_t c = sp_count[b * MAX_SPECIES + z];
+        sp_count[b * MAX_SPECIES + z] = (int32_t)run;
+        run += c;
+    }
+}
+
+__global__ void __launch_bounds__(256)
+k_species_assign(int64_t N, const float4 *__restrict__ pos4, const int32_t *__restrict__ sp_count, int32_t *mrow,
+                 int32_t *row_atom, const int32_t *cond, float thr2) {
+    if (skip_rebuild(cond, thr2)) return;
+    __shared__ int32_t wc[8][MAX_SPECIES];  // per warp, per species
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int64_t k = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    const int z = k < N ? __float_as_int(pos4[k].w) : -1;
+    int rank = 0;
+#pragma unroll
+    for (int q = 0; q < MAX_SPECIES; ++q) {
+        const unsigned m = __ballot_sync(0xffffffffu, z == q);
+        if (z == q) rank = __popc(m & ((1u << lane) - 1u));
+        if (lane == 0) wc[wid][q] = __popc(m);
+    }
+    __syncthreads();
+    if (z < 0) return;
+    int before = 0;
+    for (int w = 0; w < wid; ++w) before += wc[w][z];
+    const int32_t r = sp_count[blockIdx.x * (int64_t)MAX_SPECIES + z] + before + rank;
+    mrow[k] = r;
+    row_atom[r] = (int32_t)k;
+}
+
 __global__ void k_finish_rebuild(int32_t *flags, const int32_t *cond, float thr2) {
     if (skip_rebuild(cond, thr2)) return;
     flags[FLAG_DISP2] = 0;
@@ -438,6 +495,17 @@ int launch_build(gmnn_system *s, const float *positions, cudaStream_t st, const 
     k_gather<<<nblocks(N, 256), 256, 0, st>>>(N, positions, s->species, s->perm, s->pos4, s->xref, true, 0.f,
                                               nullptr, cond, thr2);
     GMNN_LAUNCHED();
+    if (s->mrow) {  // per-species weight sets: rows of the MLP stage follow the new atom order
+        SegRows seg;
+        for (int z = 0; z < MAX_SPECIES; ++z) seg.row0[z] = s->seg_row0[z];
+        const unsigned nb = nblocks(N, 256);
+        k_species_block_count<<<nb, 256, 0, st>>>(N, s->pos4, s->sp_count, cond, thr2);
+        GMNN_LAUNCHED();
+        k_species_scan<<<1, 32, 0, st>>>((int64_t)nb, s->sp_count, seg, cond, thr2);
+        GMNN_LAUNCHED();
+        k_species_assign<<<nb, 256, 0, st>>>(N, s->pos4, s->sp_count, s->mrow, s->row_atom, cond, thr2);
+        GMNN_LAUNCHED();
+    }
     if (s->small_box)
         k_build_small<<<warp_grid(N), 256, 0, st>>>(N, s->pos4, g, s->nbr, s->count, s->cap, s->flags, cond, thr2);
     else

@@ -50,9 +50,16 @@ def test_no_cpu_fallback_and_validation(gm):
     with pytest.raises(gm.GmnnError) as e:
         gm.Model(spec, l_max=2)
     assert e.value.code == gm.GMNN_UNSUPPORTED
+    with pytest.raises(ValueError):
+        gm.Model(spec, n_weight_sets=2)  # one shared set handed in as two: refused before the library reads it
+    three = wl.li3po4_box(64, hidden=(16, 16), n_weight_sets=3).model
+    two_species = wl.tiny_box(hidden=(16, 16)).model
+    import dataclasses
+
+    bad_sets = dataclasses.replace(two_species, n_weight_sets=3, W=three.W, b=three.b)  # 3 sets, 2 species
     with pytest.raises(gm.GmnnError) as e:
-        gm.Model(spec, n_weight_sets=2)
-    assert e.value.code == gm.GMNN_UNSUPPORTED
+        gm.Model(bad_sets)
+    assert e.value.code == gm.GMNN_INVALID_ARG
     bad = wl.tiny_box(hidden=(20, 16)).model
     with pytest.raises(gm.GmnnError) as e:
         gm.Model(bad)
