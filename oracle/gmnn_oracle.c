@@ -100,13 +100,16 @@ int oracle_n_features(int n) {
 }
 
 /* ------------------------------------------------------------------------------------------
- * O-1  Neighbour set.  r_list = r_cut + skin.  Orthorhombic cell diag(L).  For every i, j and
- * image n in [-k..k]^3 (k_a = pbc_a ? ceil(r_list / L_a) : 0), excluding (j == i, n == 0):
- * keep (i, j, n) iff |x_j - x_i + n L|^2 < r_list^2, strict.  Full list (both directions).
- * The predicate is SPECIFIED in unfused fp32 (reading R20):
- *   s_a = fl(n_a * L_a);  d_a = fl(fl(x_j,a - x_i,a) + s_a);  r2 = fl(fl(dx*dx + dy*dy) + dz*dz)
- *   keep iff r2 < fl(r_list * r_list).
- * Output sorted by (i, j, nx, ny, nz).  Returns the number of pairs; writes at most cap of them.
+ * O-1  Neighbour set.  r_list = r_cut + skin.  Cell h (row-major 3x3, rows = lattice vectors a, b, c;
+ * O-16: any right- or left-handed lattice, the configs' boxes are diag(L)).  For every i, j and image
+ * n in [-k..k]^3, k_a = pbc_a ? ceil(r_list / w_a) : 0 with w_a the distance between the two cell faces
+ * that axis a connects (w_a = V / |b x c| ...; = L_a for diag(L)), excluding (j == i, n == 0):
+ * keep (i, j, n) iff |x_j - x_i + n1 a + n2 b + n3 c|^2 < r_list^2, strict.  Full list (both directions).
+ * Positions must lie inside the cell (fractional coordinates in [0, 1) on periodic axes).
+ * The predicate is SPECIFIED in unfused fp32 (reading R20; O-16 extends the shift to three terms):
+ *   s_x = fl(fl(fl(n1 a_x) + fl(n2 b_x)) + fl(n3 c_x))   (= fl(n1 L_x) for diag(L): adding a zero is exact)
+ *   d_x = fl(fl(x_j,x - x_i,x) + s_x);  r2 = fl(fl(dx*dx + dy*dy) + dz*dz);  keep iff r2 < fl(r_list * r_list).
+ * Output sorted by (i, j, n1, n2, n3).  Returns the number of pairs; writes at most cap of them.
  * ------------------------------------------------------------------------------------------ */
 static inline int pair_predicate(const float *pos, int64_t i, int64_t j, float sx, float sy, float sz, float rl2) {
     float dx = (pos[3 * j + 0] - pos[3 * i + 0]) + sx;
@@ -116,10 +119,48 @@ static inline int pair_predicate(const float *pos, int64_t i, int64_t j, float s
     return r2 < rl2;
 }
 
-int64_t oracle_neighbors_brute(int64_t N, const float *pos, const float *L, const int32_t *pbc, float r_list,
+/* fp32 lattice shift of image (n1, n2, n3), in the order the predicate fixes */
+static inline void image_shift32(const float *h, int n1, int n2, int n3, float *s) {
+    for (int x = 0; x < 3; ++x) s[x] = ((float)n1 * h[0 + x] + (float)n2 * h[3 + x]) + (float)n3 * h[6 + x];
+}
+
+/* distance between opposite faces of the cell along each lattice direction: w_a = V / |b x c|, ... */
+static void face_distances(const double *h, double *w) {
+    const double *a = h, *b = h + 3, *c = h + 6;
+    double bc[3] = {b[1] * c[2] - b[2] * c[1], b[2] * c[0] - b[0] * c[2], b[0] * c[1] - b[1] * c[0]};
+    double ca[3] = {c[1] * a[2] - c[2] * a[1], c[2] * a[0] - c[0] * a[2], c[0] * a[1] - c[1] * a[0]};
+    double ab[3] = {a[1] * b[2] - a[2] * b[1], a[2] * b[0] - a[0] * b[2], a[0] * b[1] - a[1] * b[0]};
+    double V = fabs(a[0] * bc[0] + a[1] * bc[1] + a[2] * bc[2]);
+    w[0] = V / sqrt(bc[0] * bc[0] + bc[1] * bc[1] + bc[2] * bc[2]);
+    w[1] = V / sqrt(ca[0] * ca[0] + ca[1] * ca[1] + ca[2] * ca[2]);
+    w[2] = V / sqrt(ab[0] * ab[0] + ab[1] * ab[1] + ab[2] * ab[2]);
+}
+
+/* inverse of the row-major cell: fractional coordinates s = x hinv (row vector times matrix) */
+static void cell_inverse(const double *h, double *hi) {
+    double det = h[0] * (h[4] * h[8] - h[5] * h[7]) - h[1] * (h[3] * h[8] - h[5] * h[6]) + h[2] * (h[3] * h[7] - h[4] * h[6]);
+    hi[0] = (h[4] * h[8] - h[5] * h[7]) / det;
+    hi[1] = (h[2] * h[7] - h[1] * h[8]) / det;
+    hi[2] = (h[1] * h[5] - h[2] * h[4]) / det;
+    hi[3] = (h[5] * h[6] - h[3] * h[8]) / det;
+    hi[4] = (h[0] * h[8] - h[2] * h[6]) / det;
+    hi[5] = (h[2] * h[3] - h[0] * h[5]) / det;
+    hi[6] = (h[3] * h[7] - h[4] * h[6]) / det;
+    hi[7] = (h[1] * h[6] - h[0] * h[7]) / det;
+    hi[8] = (h[0] * h[4] - h[1] * h[3]) / det;
+}
+
+static int cell_is_diagonal(const double *h) {
+    return h[1] == 0.0 && h[2] == 0.0 && h[3] == 0.0 && h[5] == 0.0 && h[6] == 0.0 && h[7] == 0.0;
+}
+
+int64_t oracle_neighbors_brute(int64_t N, const float *pos, const float *h, const int32_t *pbc, float r_list,
                                int64_t cap, int32_t *out_i, int32_t *out_j, int32_t *out_n) {
     int k[3];
-    for (int a = 0; a < 3; ++a) k[a] = pbc[a] ? (int)ceilf(r_list / L[a]) : 0;
+    double hd[9], w[3];
+    for (int q = 0; q < 9; ++q) hd[q] = (double)h[q];
+    face_distances(hd, w);
+    for (int a = 0; a < 3; ++a) k[a] = pbc[a] ? (int)ceil((double)r_list / w[a]) : 0;
     const float rl2 = r_list * r_list;
     int64_t count = 0;
     for (int64_t i = 0; i < N; ++i)
@@ -128,8 +169,9 @@ int64_t oracle_neighbors_brute(int64_t N, const float *pos, const float *L, cons
                 for (int ny = -k[1]; ny <= k[1]; ++ny)
                     for (int nz = -k[2]; nz <= k[2]; ++nz) {
                         if (j == i && nx == 0 && ny == 0 && nz == 0) continue;
-                        float sx = (float)nx * L[0], sy = (float)ny * L[1], sz = (float)nz * L[2];
-                        if (pair_predicate(pos, i, j, sx, sy, sz, rl2)) {
+                        float sh[3];
+                        image_shift32(h, nx, ny, nz, sh);
+                        if (pair_predicate(pos, i, j, sh[0], sh[1], sh[2], rl2)) {
                             if (count < cap) {
                                 out_i[count] = (int32_t)i;
                                 out_j[count] = (int32_t)j;
@@ -159,15 +201,17 @@ static int cand_cmp(const void *a, const void *b) {
 /* The oracle's own O(N) search (linked cells), used for N > 8192 and itself pinned against the
  * brute force above.  Same predicate, same output order.  Needs >= 3 cells on every periodic
  * axis (else returns -1: use the brute force). */
-int64_t oracle_neighbors_cells(int64_t N, const float *pos, const float *L, const int32_t *pbc, float r_list,
+int64_t oracle_neighbors_cells(int64_t N, const float *pos, const float *h, const int32_t *pbc, float r_list,
                                int64_t cap, int32_t *out_i, int32_t *out_j, int32_t *out_n) {
     int nc[3];
-    double edge[3];
-    for (int a = 0; a < 3; ++a) {
-        nc[a] = (int)floor((double)L[a] / ((double)r_list * (1.0 + 1e-6)));
+    double hd[9], hinv[9], w[3];
+    for (int q = 0; q < 9; ++q) hd[q] = (double)h[q];
+    face_distances(hd, w);
+    cell_inverse(hd, hinv);
+    for (int a = 0; a < 3; ++a) {  /* bins in fractional coordinates: slabs at least r_list thick */
+        nc[a] = (int)floor(w[a] / ((double)r_list * (1.0 + 1e-6)));
         if (nc[a] < 1) nc[a] = 1;
         if (pbc[a] && nc[a] < 3) return -1;
-        edge[a] = (double)L[a] / nc[a];
     }
     const float rl2 = r_list * r_list;
     int64_t ncell = (int64_t)nc[0] * nc[1] * nc[2];
@@ -178,7 +222,9 @@ int64_t oracle_neighbors_cells(int64_t N, const float *pos, const float *L, cons
     for (int64_t i = N - 1; i >= 0; --i) {
         int c[3];
         for (int a = 0; a < 3; ++a) {
-            c[a] = (int)floor((double)pos[3 * i + a] / edge[a]);
+            double frac = 0.0;
+            for (int x = 0; x < 3; ++x) frac += (double)pos[3 * i + x] * hinv[3 * x + a];
+            c[a] = (int)floor(frac * nc[a]);
             if (c[a] < 0) c[a] = 0;
             if (c[a] >= nc[a]) c[a] = nc[a] - 1;
             cidx[3 * i + a] = c[a];
@@ -216,11 +262,12 @@ int64_t oracle_neighbors_cells(int64_t N, const float *pos, const float *L, cons
                     for (int a = 0; a < 3; ++a)
                         if (!pbc[a] && nc[a] < 3 && (cidx[3 * i + a] + o[a] < 0 || cidx[3 * i + a] + o[a] >= nc[a])) dup = 1;
                     if (dup) continue;
-                    float sx = (float)n[0] * L[0], sy = (float)n[1] * L[1], sz = (float)n[2] * L[2];
+                    float sh[3];
+                    image_shift32(h, n[0], n[1], n[2], sh);
                     int64_t cc = ((int64_t)c[0] * nc[1] + c[1]) * nc[2] + c[2];
                     for (int64_t j = head[cc]; j >= 0; j = next[j]) {
                         if (j == i && n[0] == 0 && n[1] == 0 && n[2] == 0) continue;
-                        if (pair_predicate(pos, i, j, sx, sy, sz, rl2)) {
+                        if (pair_predicate(pos, i, j, sh[0], sh[1], sh[2], rl2)) {
                             if (nc_i == cand_cap) {
                                 cand_cap *= 2;
                                 cand = (cand_t *)realloc(cand, sizeof(cand_t) * cand_cap);
@@ -286,9 +333,10 @@ void oracle_radial(const oracle_hparams *hp, const double *beta, int zi, int zj,
     }
 }
 
-/* d = x_j - x_i + n L in fp64 (positions are fp32 values promoted to fp64). */
+/* d = x_j - x_i + n1 a + n2 b + n3 c in fp64 (positions are fp32 values promoted to fp64; L = the 3x3 cell, rows a, b, c). */
 static inline void pair_vector(const double *pos, const double *L, int64_t i, int64_t j, const int32_t *n, double *d) {
-    for (int a = 0; a < 3; ++a) d[a] = pos[3 * j + a] - pos[3 * i + a] + n[a] * L[a];
+    for (int x = 0; x < 3; ++x)
+        d[x] = pos[3 * j + x] - pos[3 * i + x] + (n[0] * L[0 + x] + n[1] * L[3 + x] + n[2] * L[6 + x]);
 }
 
 /* ------------------------------------------------------------------------------------------
@@ -665,7 +713,7 @@ static void forward_all(const oracle_hparams *hp, const oracle_weights *w, int64
 static void backward_all(const oracle_hparams *hp, const oracle_weights *w, int64_t N, const double *pos,
                          const int32_t *species, const double *L, int64_t npairs, const int64_t *off,
                          const int32_t *pj, const int32_t *pn, const double *P, const double *zs,
-                         const double *head_w, double *Fout, double *dG_out, double *Q_out) {
+                         const double *head_w, double *Fout, double *dG_out, double *Q_out, double *virial_out) {
     const int nr = hp->n_radial, F = oracle_n_features(nr), H = total_hidden(hp), M = hp->n_heads;
     double *gpair = (double *)malloc(sizeof(double) * 3 * (size_t)(npairs > 0 ? npairs : 1));
     memset(Fout, 0, sizeof(double) * 3 * (size_t)N);
@@ -687,6 +735,20 @@ static void backward_all(const oracle_hparams *hp, const oracle_weights *w, int6
     for (int64_t i = 0; i < N; ++i)
         for (int64_t p = off[i]; p < off[i + 1]; ++p)
             for (int a = 0; a < 3; ++a) Fout[3 * (size_t)pj[p] + a] -= gpair[3 * p + a];
+    /* O-16  Virial ("the gradient of the energy with respect to ... the strain tensor"): under a
+     * homogeneous strain d -> (1 + eps) d of every pair vector, dE/d eps_ab = sum_pairs g_a d_b with g = dE/dd
+     * of the directed pair (O-9).  W_ab = - sum_pairs d_a g_b = -dE/d eps (symmetric for a rotation-invariant
+     * E, which the pins check rather than assume); stress = -W / V. */
+    if (virial_out) {
+        for (int q = 0; q < 9; ++q) virial_out[q] = 0.0;
+        for (int64_t i = 0; i < N; ++i)
+            for (int64_t p = off[i]; p < off[i + 1]; ++p) {
+                double d[3];
+                pair_vector(pos, L, i, pj[p], pn + 3 * p, d);
+                for (int a = 0; a < 3; ++a)
+                    for (int b = 0; b < 3; ++b) virial_out[3 * a + b] -= d[a] * gpair[3 * p + b];
+            }
+    }
     free(gpair);
 }
 
@@ -699,7 +761,7 @@ static void backward_all(const oracle_hparams *hp, const oracle_weights *w, int6
 int oracle_energy_forces(const oracle_hparams *hp, const oracle_weights *w, int64_t N, const double *pos,
                          const int32_t *species, const double *L, int64_t npairs, const int32_t *pi,
                          const int32_t *pj, const int32_t *pn, const double *head_w, double *E_heads, double *Fout,
-                         double *P_out, double *G_out, double *dG_out, double *Q_out) {
+                         double *P_out, double *G_out, double *dG_out, double *Q_out, double *virial_out) {
     if (hp->n_radial > 16 || hp->n_heads > 64 || hp->n_hidden > 4) return -1;
     if (hp->n_weight_sets > 1 && hp->n_weight_sets != hp->n_species) return -1;
     const int nr = hp->n_radial, F = oracle_n_features(nr), H = total_hidden(hp);
@@ -711,7 +773,7 @@ int oracle_energy_forces(const oracle_hparams *hp, const oracle_weights *w, int6
     double *G = G_out ? G_out : (double *)malloc(sizeof(double) * (size_t)N * F);
     double *zs = (double *)malloc(sizeof(double) * (size_t)N * (H > 0 ? H : 1));
     forward_all(hp, w, N, pos, species, L, off, pj, pn, P, G, zs, E_heads);
-    if (Fout) backward_all(hp, w, N, pos, species, L, npairs, off, pj, pn, P, zs, head_w, Fout, dG_out, Q_out);
+    if (Fout) backward_all(hp, w, N, pos, species, L, npairs, off, pj, pn, P, zs, head_w, Fout, dG_out, Q_out, virial_out);
     free(off);
     if (!P_out) free(P);
     if (!G_out) free(G);
@@ -740,7 +802,7 @@ int oracle_ensemble(const oracle_hparams *hp, const oracle_weights *w, int64_t N
     for (int m = 0; m < M; ++m) {
         double hw[64];
         for (int q = 0; q < M; ++q) hw[q] = (q == m) ? 1.0 : 0.0;
-        backward_all(hp, w, N, pos, species, L, npairs, off, pj, pn, P, zs, hw, Fall + (size_t)m * N * 3, NULL, NULL);
+        backward_all(hp, w, N, pos, species, L, npairs, off, pj, pn, P, zs, hw, Fall + (size_t)m * N * 3, NULL, NULL, NULL);
     }
     for (int64_t i = 0; i < N; ++i) {
         double mean = 0.0, var = 0.0;
@@ -769,6 +831,24 @@ int oracle_ensemble(const oracle_hparams *hp, const oracle_weights *w, int64_t N
     return 0;
 }
 
+/* Fold one position into the cell along the periodic axes.  diag(L): x_a -= floor(x_a / L_a) L_a;
+ * general lattice (O-16): fractional s = x hinv, x -= floor(s_a) (lattice vector a). */
+static void wrap_position(double *x, const double *L, const int32_t *pbc) {
+    if (cell_is_diagonal(L)) {
+        for (int a = 0; a < 3; ++a)
+            if (pbc[a]) x[a] -= floor(x[a] / L[4 * a]) * L[4 * a];
+        return;
+    }
+    double hinv[9];
+    cell_inverse(L, hinv);
+    for (int a = 0; a < 3; ++a) {
+        if (!pbc[a]) continue;
+        double frac = x[0] * hinv[a] + x[1] * hinv[3 + a] + x[2] * hinv[6 + a];
+        double k = floor(frac);
+        for (int c = 0; c < 3; ++c) x[c] -= k * L[3 * a + c];
+    }
+}
+
 /* Neighbour list of fp64 positions (cast to fp32 for the predicate), growing buffers. */
 typedef struct {
     int64_t n, cap;
@@ -778,7 +858,8 @@ typedef struct {
 static void build_list(pairlist_t *pl, int64_t N, const double *pos, const double *L, const int32_t *pbc,
                        double r_list) {
     float *p32 = (float *)malloc(sizeof(float) * 3 * (size_t)N);
-    float L32[3] = {(float)L[0], (float)L[1], (float)L[2]};
+    float L32[9];
+    for (int q = 0; q < 9; ++q) L32[q] = (float)L[q];
     for (int64_t q = 0; q < 3 * N; ++q) p32[q] = (float)pos[q];
     for (;;) {
         int64_t n = oracle_neighbors_cells(N, p32, L32, pbc, (float)r_list, pl->cap, pl->i, pl->j, pl->n3);
@@ -820,13 +901,11 @@ int oracle_nve(const oracle_hparams *hp, const oracle_weights *w, int64_t N, dou
     double *xref = (double *)malloc(sizeof(double) * 3 * (size_t)N); /* xu at the last build */
     const double one = 1.0;
     int64_t rebuilds = 0;
-    for (int64_t i = 0; i < N; ++i)
-        for (int a = 0; a < 3; ++a)
-            if (pbc[a]) x[3 * i + a] -= floor(x[3 * i + a] / L[a]) * L[a];
+    for (int64_t i = 0; i < N; ++i) wrap_position(x + 3 * i, L, pbc);
     memcpy(xu, x, sizeof(double) * 3 * (size_t)N);
     memcpy(xref, x, sizeof(double) * 3 * (size_t)N);
     build_list(&pl, N, x, L, pbc, hp->r_cut + skin);
-    oracle_energy_forces(hp, w, N, xu, species, L, pl.n, pl.i, pl.j, pl.n3, &one, Ei, F, NULL, NULL, NULL, NULL);
+    oracle_energy_forces(hp, w, N, xu, species, L, pl.n, pl.i, pl.j, pl.n3, &one, Ei, F, NULL, NULL, NULL, NULL, NULL);
     for (int64_t step = 0;; ++step) {
         double ep = 0.0, ek = 0.0;
         for (int64_t i = 0; i < N; ++i) {
@@ -842,10 +921,11 @@ int oracle_nve(const oracle_hparams *hp, const oracle_weights *w, int64_t N, dou
             for (int a = 0; a < 3; ++a) {
                 v[3 * i + a] += 0.5 * dt * F[3 * i + a] / masses[i] * ACC_CONV;
                 xu[3 * i + a] += dt * v[3 * i + a];
-                x[3 * i + a] = pbc[a] ? xu[3 * i + a] - floor(xu[3 * i + a] / L[a]) * L[a] : xu[3 * i + a];
+                x[3 * i + a] = xu[3 * i + a];
                 double dd = xu[3 * i + a] - xref[3 * i + a];
                 d2 += dd * dd;
             }
+            wrap_position(x + 3 * i, L, pbc);
             if (d2 > maxd2) maxd2 = d2;
         }
         if (sqrt(maxd2) > 0.5 * skin) {
@@ -854,7 +934,7 @@ int oracle_nve(const oracle_hparams *hp, const oracle_weights *w, int64_t N, dou
             build_list(&pl, N, x, L, pbc, hp->r_cut + skin);
             ++rebuilds;
         }
-        oracle_energy_forces(hp, w, N, xu, species, L, pl.n, pl.i, pl.j, pl.n3, &one, Ei, F, NULL, NULL, NULL, NULL);
+        oracle_energy_forces(hp, w, N, xu, species, L, pl.n, pl.i, pl.j, pl.n3, &one, Ei, F, NULL, NULL, NULL, NULL, NULL);
         for (int64_t i = 0; i < N; ++i)
             for (int a = 0; a < 3; ++a) v[3 * i + a] += 0.5 * dt * F[3 * i + a] / masses[i] * ACC_CONV;
     }
@@ -900,13 +980,11 @@ int oracle_md_switching(const oracle_hparams *hp, const oracle_weights *w, int64
     double hw[64];
     for (int m = 0; m < M; ++m) hw[m] = 1.0 / M;
     int64_t rebuilds = 0, samples = 0, done = 0;
-    for (int64_t i = 0; i < N; ++i)
-        for (int a = 0; a < 3; ++a)
-            if (pbc[a]) x[3 * i + a] -= floor(x[3 * i + a] / L[a]) * L[a];
+    for (int64_t i = 0; i < N; ++i) wrap_position(x + 3 * i, L, pbc);
     memcpy(xu, x, sizeof(double) * 3 * (size_t)N);
     memcpy(xref, x, sizeof(double) * 3 * (size_t)N);
     build_list(&pl, N, x, L, pbc, hp->r_cut + skin);
-    oracle_energy_forces(hp, w, N, xu, species, L, pl.n, pl.i, pl.j, pl.n3, hw, Eh, F, NULL, NULL, NULL, NULL);
+    oracle_energy_forces(hp, w, N, xu, species, L, pl.n, pl.i, pl.j, pl.n3, hw, Eh, F, NULL, NULL, NULL, NULL, NULL);
     for (int64_t step = 0;; ++step) {
         double ep = 0.0, ek = 0.0;
         for (int64_t i = 0; i < N; ++i) {
@@ -943,10 +1021,11 @@ int oracle_md_switching(const oracle_hparams *hp, const oracle_weights *w, int64
             for (int a = 0; a < 3; ++a) {
                 v[3 * i + a] += 0.5 * dt * F[3 * i + a] / masses[i] * ACC_CONV;
                 xu[3 * i + a] += dt * v[3 * i + a];
-                x[3 * i + a] = pbc[a] ? xu[3 * i + a] - floor(xu[3 * i + a] / L[a]) * L[a] : xu[3 * i + a];
+                x[3 * i + a] = xu[3 * i + a];
                 double dd = xu[3 * i + a] - xref[3 * i + a];
                 d2 += dd * dd;
             }
+            wrap_position(x + 3 * i, L, pbc);
             if (d2 > maxd2) maxd2 = d2;
         }
         if (sqrt(maxd2) > 0.5 * skin) {
@@ -955,7 +1034,7 @@ int oracle_md_switching(const oracle_hparams *hp, const oracle_weights *w, int64
             build_list(&pl, N, x, L, pbc, hp->r_cut + skin);
             ++rebuilds;
         }
-        oracle_energy_forces(hp, w, N, xu, species, L, pl.n, pl.i, pl.j, pl.n3, hw, Eh, F, NULL, NULL, NULL, NULL);
+        oracle_energy_forces(hp, w, N, xu, species, L, pl.n, pl.i, pl.j, pl.n3, hw, Eh, F, NULL, NULL, NULL, NULL, NULL);
         for (int64_t i = 0; i < N; ++i)
             for (int a = 0; a < 3; ++a) v[3 * i + a] += 0.5 * dt * F[3 * i + a] / masses[i] * ACC_CONV;
     }

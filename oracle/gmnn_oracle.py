@@ -75,6 +75,46 @@ def _i32(a) -> np.ndarray:
     return np.ascontiguousarray(np.asarray(a), dtype=np.int32)
 
 
+def cell9(cell) -> np.ndarray:
+    """The 3x3 lattice (rows = lattice vectors) as 9 doubles, from [3] edge lengths of an orthorhombic box,
+    or a [3][3] / [9] matrix (O-16: general cells)."""
+    c = np.asarray(cell, dtype=np.float64)
+    if c.size == 3:
+        return np.diag(c.reshape(3)).reshape(9).copy()
+    assert c.size == 9
+    return np.ascontiguousarray(c.reshape(9))
+
+
+def wrap_positions(y, cell, pbc) -> np.ndarray:
+    """Positions folded into the cell along the periodic axes (diag(L): y - floor(y / L) L; general lattice: in
+    fractional coordinates)."""
+    h = cell9(cell).reshape(3, 3)
+    per = np.asarray(pbc).astype(bool)
+    y = np.array(y, dtype=np.float64, copy=True)
+    if np.count_nonzero(h - np.diag(np.diag(h))) == 0:
+        L = np.diag(h)
+        y[:, per] -= np.floor(y[:, per] / L[per]) * L[per]
+        return y
+    k = np.floor(y @ np.linalg.inv(h))
+    k[:, ~per] = 0.0
+    return y - k @ h
+
+
+def to_fp32_inside(y, cell) -> np.ndarray:
+    """fp32 copy of wrapped fp64 positions that is still inside the cell after rounding (the neighbour predicate
+    is specified on fp32 positions in [0, 1) fractional; rounding up onto the far face folds to the near one)."""
+    h = cell9(cell).reshape(3, 3)
+    y32 = np.asarray(y).astype(np.float32)
+    if np.count_nonzero(h - np.diag(np.diag(h))) == 0:
+        L32 = np.diag(h).astype(np.float32)
+        return np.where(y32 >= L32[None, :], np.float32(0), y32)
+    frac = y32.astype(np.float64) @ np.linalg.inv(h.astype(np.float32).astype(np.float64))
+    over = frac >= 1.0
+    if over.any():
+        y32 = (y32.astype(np.float64) - over.astype(np.float64) @ h).astype(np.float32)
+    return y32
+
+
 def num_threads() -> int:
     return int(lib().oracle_num_threads())
 
@@ -144,10 +184,11 @@ class Pairs:
 
 
 def neighbors(positions, cell, pbc, r_list: float, method: str = "brute") -> Pairs:
-    """O-1.  positions [N][3] are rounded to fp32 (the predicate's precision); cell [3]."""
+    """O-1.  positions [N][3] are rounded to fp32 (the predicate's precision); cell [3] (orthorhombic edge
+    lengths) or [3][3] (rows = lattice vectors, O-16), rounded to fp32 likewise."""
     pos = np.ascontiguousarray(np.asarray(positions), dtype=np.float32)
-    L = np.ascontiguousarray(np.asarray(cell), dtype=np.float32).reshape(-1)
-    assert L.shape[0] == 3
+    c = np.asarray(cell, dtype=np.float32)
+    L = np.ascontiguousarray(np.diag(c.reshape(3)).reshape(9) if c.size == 3 else c.reshape(9))
     pb = _i32(pbc)
     N = pos.shape[0]
     fn = {"brute": lib().oracle_neighbors_brute, "cells": lib().oracle_neighbors_cells}[method]
@@ -237,6 +278,7 @@ class Result:
     G: Optional[np.ndarray] = None  # [N][F]
     dG: Optional[np.ndarray] = None  # [N][F]
     Q: Optional[np.ndarray] = None  # [N][n_radial][40]
+    virial: Optional[np.ndarray] = None  # [3][3]  W = -sum_pairs d (x) g = -dE/d strain (O-16); stress = -W / V
 
     @property
     def e_atom(self) -> np.ndarray:
@@ -249,7 +291,7 @@ def energy_forces(model: Model, positions, species, cell, pairs: Pairs, head_w: 
     (default: 1 for a single head, 1/M each for an ensemble = gradient of the mean energy)."""
     pos = _f64(positions)
     sp = _i32(species)
-    L = _f64(cell).reshape(-1)
+    L = cell9(cell)
     N = pos.shape[0]
     M = model.n_heads
     hw = _f64(np.full(M, 1.0 / M) if head_w is None else head_w)
@@ -261,13 +303,14 @@ def energy_forces(model: Model, positions, species, cell, pairs: Pairs, head_w: 
     G = np.zeros((N, F)) if intermediates else None
     dG = np.zeros((N, F)) if (intermediates and forces) else None
     Q = np.zeros((N, model.n_radial, NC)) if (intermediates and forces) else None
+    vir = np.zeros((3, 3)) if forces else None
     pi, pj, pn = _i32(pairs.i), _i32(pairs.j), _i32(pairs.n)
     rc = lib().oracle_energy_forces(
         C.byref(model.hp), C.byref(model.w), C.c_int64(N), _p(pos), _p(sp), _p(L), C.c_int64(len(pairs)),
-        _p(pi), _p(pj), _p(pn), _p(hw), _p(e_heads), _p(f), _p(Pm), _p(G), _p(dG), _p(Q))
+        _p(pi), _p(pj), _p(pn), _p(hw), _p(e_heads), _p(f), _p(Pm), _p(G), _p(dG), _p(Q), _p(vir))
     if rc != 0:
         raise ValueError("oracle_energy_forces: bad argument")
-    return Result(float((e_heads @ hw).sum()), e_heads, f, Pm, G, dG, Q)
+    return Result(float((e_heads @ hw).sum()), e_heads, f, Pm, G, dG, Q, vir)
 
 
 @dataclass
@@ -284,7 +327,7 @@ def ensemble(model: Model, positions, species, cell, pairs: Pairs, keep_heads: b
     """O-10 (Eq. 5 with the 1/N_ens divisor, Eq. 6)."""
     pos = _f64(positions)
     sp = _i32(species)
-    L = _f64(cell).reshape(-1)
+    L = cell9(cell)
     N = pos.shape[0]
     M = model.n_heads
     e_heads = np.zeros((N, M))
@@ -316,7 +359,7 @@ def nve(model: Model, positions, velocities, masses, species, cell, pbc, skin: f
     v = _f64(velocities).copy()
     m = _f64(masses)
     sp = _i32(species)
-    L = _f64(cell).reshape(-1)
+    L = cell9(cell)
     pb = _i32(pbc)
     epot = np.zeros(n_steps + 1)
     ekin = np.zeros(n_steps + 1)
@@ -349,7 +392,7 @@ def md_switching(model: Model, positions, velocities, masses, species, cell, pbc
     v = _f64(velocities).copy()
     m = _f64(masses)
     sp = _i32(species)
-    L = _f64(cell).reshape(-1)
+    L = cell9(cell)
     pb = _i32(pbc)
     epot = np.zeros(n_steps + 1)
     ekin = np.zeros(n_steps + 1)
@@ -402,17 +445,12 @@ def nve_udd(model: Model, positions, velocities, masses, species, cell, pbc, dt_
     x = _f64(positions).copy()
     v = _f64(velocities).copy()
     m = _f64(masses)[:, None]
-    L = _f64(cell).reshape(-1)
-    per = np.asarray(pbc).astype(bool)
 
     def wrap(y):
-        y = y.copy()
-        y[:, per] -= np.floor(y[:, per] / L[per]) * L[per]
-        return y
+        return wrap_positions(y, cell, pbc)
 
     def evaluate(y):
-        y32 = y.astype(np.float32)  # the neighbour predicate is specified in fp32 (R20); E and F use the fp64 y
-        y32 = np.where(y32 >= np.asarray(cell, np.float32).reshape(-1)[None, :], np.float32(0), y32)
+        y32 = to_fp32_inside(y, cell)  # the neighbour predicate is specified in fp32 (R20); E and F use the fp64 y
         return udd_energy_forces(model, y, species, cell, auto_neighbors(y32, cell, pbc, model.r_cut), A, B)
 
     x = wrap(x)
@@ -485,8 +523,6 @@ def nvt_nose_hoover(model: Model, positions, velocities, masses, species, cell, 
     x = _f64(positions).copy()
     v = _f64(velocities).copy()
     m = _f64(masses)[:, None]
-    L = _f64(cell).reshape(-1)
-    per = np.asarray(pbc).astype(bool)
     N = x.shape[0]
     dof, kT = 3.0 * N, KB_EV * temperature
     Q = np.full(chain_length, kT * tau_fs ** 2)
@@ -494,13 +530,10 @@ def nvt_nose_hoover(model: Model, positions, velocities, masses, species, cell, 
     xi, pxi = np.zeros(chain_length), np.zeros(chain_length)
 
     def wrap(y):
-        y = y.copy()
-        y[:, per] -= np.floor(y[:, per] / L[per]) * L[per]
-        return y
+        return wrap_positions(y, cell, pbc)
 
     def evaluate(y):
-        y32 = y.astype(np.float32)
-        y32 = np.where(y32 >= np.asarray(cell, np.float32).reshape(-1)[None, :], np.float32(0), y32)
+        y32 = to_fp32_inside(y, cell)  # the neighbour predicate is specified in fp32 (R20); E and F use the fp64 y
         return energy_forces(model, y, species, cell, auto_neighbors(y32, cell, pbc, model.r_cut))
 
     def ke2():
@@ -555,21 +588,16 @@ def nvt_langevin(model: Model, positions, velocities, masses, species, cell, pbc
     x = _f64(positions).copy()
     v = _f64(velocities).copy()
     m = _f64(masses)[:, None]
-    L = _f64(cell).reshape(-1)
-    per = np.asarray(pbc).astype(bool)
     N = x.shape[0]
     kT = KB_EV * temperature
     c1 = np.exp(-gamma_per_fs * dt_fs)
     c2 = np.sqrt(kT * (1.0 - c1 * c1) / m * ACC)  # Ang/fs
 
     def wrap(y):
-        y = y.copy()
-        y[:, per] -= np.floor(y[:, per] / L[per]) * L[per]
-        return y
+        return wrap_positions(y, cell, pbc)
 
     def evaluate(y):
-        y32 = y.astype(np.float32)
-        y32 = np.where(y32 >= np.asarray(cell, np.float32).reshape(-1)[None, :], np.float32(0), y32)
+        y32 = to_fp32_inside(y, cell)  # the neighbour predicate is specified in fp32 (R20); E and F use the fp64 y
         return energy_forces(model, y, species, cell, auto_neighbors(y32, cell, pbc, model.r_cut))
 
     x = wrap(x)

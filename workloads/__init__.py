@@ -14,6 +14,7 @@ from .inputs import (  # noqa: F401
     ionic_liquid_box,
     li3po4_box,
     cluster,
+    triclinic_box,
     splitmix64,
     uniform01,
     normal01,

@@ -113,14 +113,22 @@ class Workload:
     n_steps: int
     model: ModelSpec
     species_names: Tuple[str, ...] = field(default_factory=tuple)
+    lattice: "np.ndarray | None" = None  # [3][3] f32, rows = lattice vectors, for non-orthorhombic boxes (else None)
 
     @property
     def n_atoms(self) -> int:
         return int(self.positions.shape[0])
 
     @property
+    def box(self) -> np.ndarray:
+        """The cell as the oracle and the binding take it: [3][3] lattice if the box is triclinic, else [3] edges."""
+        return self.cell if self.lattice is None else self.lattice
+
+    @property
     def cell9(self) -> np.ndarray:
         """Row-major 3x3 lattice (rows = lattice vectors) as the C ABI takes it."""
+        if self.lattice is not None:
+            return np.ascontiguousarray(self.lattice, np.float32).reshape(9).copy()
         return np.diag(self.cell.astype(np.float32)).reshape(9).copy()
 
 
@@ -282,6 +290,45 @@ def li3po4_box(n_atoms: int, hidden: Sequence[int] = (512, 512), n_heads: int = 
     vel = _maxwell_boltzmann(s + n_atoms + 3, masses, 300.0)
     return Workload("li3po4_%d" % n_atoms, pos, species, L.astype(np.float32), (1, 1, 1), masses, vel,
                     skin=skin, dt_fs=0.5, n_steps=n_steps, model=model, species_names=("Li", "P", "O"))
+
+
+def triclinic_box(n_atoms: int = 1000, hidden: Sequence[int] = (64, 64), skin: float = 0.0, n_heads: int = 1,
+                  shear: Sequence[float] = (0.25, 0.1, 0.35), stretch: Sequence[float] = (1.0, 1.1, 0.9)) -> Workload:
+    """Li3PO4-shaped box (density, species ratio, r_cut, model family of config 3) in a sheared cell for the
+    general-lattice path: lattice rows a = (s0 L, 0, 0), b = (shear0 L, s1 L, 0),
+    c = (shear1 L, shear2 L, s2 L); atoms on a jittered grid in fractional coordinates, wrapped into the cell."""
+    assert n_atoms % 8 == 0
+    s = BASE_SEED + 10 * 6
+    mass_table = np.array([6.94, 30.974, 15.999], dtype=np.float32)
+    fu_mass = 3 * 6.94 + 30.974 + 4 * 15.999
+    volume = (n_atoms // 8) * fu_mass / (2.4 * AVOGADRO_CM3)
+    Ls = (volume / (stretch[0] * stretch[1] * stretch[2])) ** (1.0 / 3.0)
+    h = np.array([[stretch[0] * Ls, 0.0, 0.0], [shear[0] * Ls, stretch[1] * Ls, 0.0],
+                  [shear[1] * Ls, shear[2] * Ls, stretch[2] * Ls]])
+    g = int(np.ceil(n_atoms ** (1.0 / 3.0) - 1e-9))
+    sites = _lattice_sites(s + n_atoms, g, n_atoms)
+    frac = (sites + 0.5) / g
+    jit = np.clip(0.1 * normal01(s + n_atoms + 7, 3 * n_atoms).reshape(n_atoms, 3), -0.4, 0.4)
+    h32 = h.astype(np.float32)
+    hinv = np.linalg.inv(h32.astype(np.float64))
+    f = frac + jit @ hinv
+    f -= np.floor(f)
+    pos = (f @ h32.astype(np.float64)).astype(np.float32)
+    for _ in range(3):  # fp32 rounding may leave an atom a hair outside: fold again in the fp32 cell
+        fr = pos.astype(np.float64) @ hinv
+        k = np.floor(fr)
+        if not k.any():
+            break
+        pos = (pos.astype(np.float64) - k @ h32.astype(np.float64)).astype(np.float32)
+    fu = n_atoms // 8
+    species = _species_from_counts(s + n_atoms + 1, (3 * fu, fu, 4 * fu))
+    masses = mass_table[species]
+    model = make_model(BASE_SEED + 10 * 3 + 2, 3, r_cut=6.0, hidden=hidden, n_heads=n_heads,
+                       force_scale=FORCE_SCALE["li3po4"])
+    vel = _maxwell_boltzmann(s + n_atoms + 3, masses, 300.0)
+    edges = np.linalg.norm(h32, axis=1).astype(np.float32)
+    return Workload("triclinic_%d" % n_atoms, pos, species, edges, (1, 1, 1), masses, vel, skin=skin, dt_fs=0.5,
+                    n_steps=0, model=model, species_names=("Li", "P", "O"), lattice=h32)
 
 
 def cluster(n_atoms: int = 24, n_species: int = 2, box: float = 40.0, radius: float = 3.5,
