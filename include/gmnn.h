@@ -18,7 +18,8 @@
  * of the invariants, ...) are the readings R1-R24 of DESIGN.md section 3; each is a field below.
  *
  * Units: Angstrom, eV, fs, amu.  a = F/m * 9.648533212e-3 Ang/fs^2.
- * Cells: orthorhombic only (cell[9] row-major, rows = lattice vectors, off-diagonals must be 0).
+ * Cells: cell[9] row-major, rows = lattice vectors a, b, c; any non-singular lattice with a positive diagonal
+ * (orthorhombic boxes: off-diagonals 0; sheared / triclinic cells, take the same calls).
  *
  * Return value of every int function: 0 (GMNN_OK) or a negative gmnn_status; the message of the
  * last failure on the calling thread is gmnn_last_error().  Calls are asynchronous on the given
@@ -139,13 +140,14 @@ int gmnn_system_set_int(gmnn_system *s, const char *key, int64_t value);
 int gmnn_system_get_int(const gmnn_system *s, const char *key, int64_t *value /*HOST*/);
 
 /* PAPER.md:169-171, 381 (neighbour list with skin `dr_threshold`, several images in small cells).
- * Builds the full (both directions) Verlet list of all (i, j, n) with |x_j - x_i + n L| < r_cut +
- * skin, n the integer image vector, by a cell list (>= 3 cells on every periodic axis) or an
- * all-pairs image loop (smaller boxes, n_atoms <= 16384).  The membership predicate is evaluated
- * in unfused fp32 exactly as DESIGN.md reading R20 writes it, so the set is reproducible bit for
- * bit.  positions: DEVICE float [n_atoms][3], already wrapped into [0, L) on every axis (periodic
- * or not); cell: HOST float[9]; pbc: HOST int32[3]; r_cut must equal the model's.  Synchronises
- * the stream once (capacity check; regrows and retries on overflow). */
+ * Builds the full (both directions) Verlet list of all (i, j, n) with |x_j - x_i + n1 a + n2 b + n3 c| < r_cut +
+ * skin, n the integer image vector, by a cell list (>= 3 slabs of r_cut + skin between the cell faces of every
+ * periodic axis) or an all-pairs image loop (smaller boxes, n_atoms <= 16384).  The membership predicate is
+ * evaluated in unfused fp32 exactly as DESIGN.md reading R20 writes it (three-term lattice shift for a general
+ * cell), so the set is reproducible bit for bit.  positions: DEVICE float [n_atoms][3], already inside the cell
+ * (orthorhombic: [0, L) on every axis, periodic or not; general lattice: fractional coordinates in [0, 1));
+ * cell: HOST float[9]; pbc: HOST int32[3]; r_cut must equal the model's.  Synchronises the stream once
+ * (capacity check; regrows and retries on overflow). */
 int gmnn_build_neighbors(gmnn_system *s, const float *positions /*DEVICE*/, const float cell[9] /*HOST*/,
                          const int32_t pbc[3] /*HOST*/, float r_cut, float skin, void *cuda_stream);
 
@@ -171,6 +173,15 @@ int gmnn_get_neighbor_rows(gmnn_system *s, int64_t n_sel, const int32_t *atoms /
  * the cheap force mode of Eq. 6). */
 int gmnn_energy_forces(gmnn_system *s, const float *positions, double *energy, float *energy_per_atom,
                        float *forces, void *cuda_stream);
+
+/* The same evaluation plus the virial ("the gradient of the energy with respect to
+ * positions and the strain tensor allow the prediction of forces and virials"):
+ *   virial  DEVICE double[9], row-major W[a][b] = -sum over directed pairs (i, j, n) of d_a g_b, d = x_j - x_i + n h,
+ *           g = dE/dd of the pair, = -dE/d(strain); symmetric up to rounding; stress = -W / V.  Summed from per-atom
+ *           terms in fp64 in a fixed order (bit-reproducible).  The first call allocates 36 bytes per atom.
+ * With n_heads > 1 it is the virial of the mean energy (and of the UDD-biased energy while a bias is set). */
+int gmnn_energy_forces_virial(gmnn_system *s, const float *positions, double *energy, float *energy_per_atom,
+                              float *forces, double *virial, void *cuda_stream);
 
 /* The same call with HOST buffers (pinned memory recommended): copies positions in and energy,
  * energy_per_atom (nullable), forces out on the stream, then synchronises it.  This is the

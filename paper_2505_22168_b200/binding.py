@@ -31,7 +31,7 @@ GMNN_FORCE_GATHER, GMNN_FORCE_PAIRBUF = 0, 1
 EXPORTS = (
     "gmnn_n_features", "gmnn_create", "gmnn_destroy", "gmnn_system_create", "gmnn_system_destroy",
     "gmnn_system_set_int", "gmnn_system_get_int", "gmnn_build_neighbors", "gmnn_get_neighbors", "gmnn_get_neighbor_rows",
-    "gmnn_energy_forces", "gmnn_energy_forces_host", "gmnn_ensemble_energy_forces", "gmnn_md_verlet_steps", "gmnn_md_ensemble_steps", "gmnn_system_set_langevin", "gmnn_system_set_nose_hoover", "gmnn_system_get_nose_hoover", "gmnn_system_set_udd_bias", "gmnn_system_get_udd_bias",
+    "gmnn_energy_forces", "gmnn_energy_forces_virial", "gmnn_energy_forces_host", "gmnn_ensemble_energy_forces", "gmnn_md_verlet_steps", "gmnn_md_ensemble_steps", "gmnn_system_set_langevin", "gmnn_system_set_nose_hoover", "gmnn_system_get_nose_hoover", "gmnn_system_set_udd_bias", "gmnn_system_get_udd_bias",
     "gmnn_check", "gmnn_stage_times", "gmnn_debug_read", "gmnn_launch_count", "gmnn_last_error",
 )
 
@@ -84,6 +84,7 @@ def _load() -> C.CDLL:
     lib.gmnn_system_get_udd_bias.argtypes = [C.c_void_p] * 4
     lib.gmnn_energy_forces.argtypes = [C.c_void_p] * 6
     lib.gmnn_energy_forces_host.argtypes = [C.c_void_p] * 6
+    lib.gmnn_energy_forces_virial.argtypes = [C.c_void_p] * 7
     lib.gmnn_ensemble_energy_forces.argtypes = [C.c_void_p] * 7
     lib.gmnn_system_create.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p]
     lib.gmnn_system_destroy.argtypes = [C.c_void_p]
@@ -267,6 +268,21 @@ class System:
                                       _dev_ptr(energy, torch.float64), _dev_ptr(energy_per_atom, torch.float32),
                                       _dev_ptr(forces, torch.float32, (self.n_atoms, 3)), _stream_ptr(stream)))
         return energy, energy_per_atom, forces
+
+    def energy_forces_virial(self, positions, stream=None):
+        """Returns (energy f64[1], energy_per_atom f32[N], forces f32[N][3], virial f64[3][3] = -dE/d strain), on device."""
+        import torch
+
+        dev, N = positions.device, self.n_atoms
+        energy = torch.empty(1, dtype=torch.float64, device=dev)
+        e_atom = torch.empty(N, dtype=torch.float32, device=dev)
+        forces = torch.empty(N, 3, dtype=torch.float32, device=dev)
+        virial = torch.empty(3, 3, dtype=torch.float64, device=dev)
+        _check(lib.gmnn_energy_forces_virial(self.handle, _dev_ptr(positions, torch.float32, (N, 3)),
+                                             _dev_ptr(energy, torch.float64), _dev_ptr(e_atom, torch.float32),
+                                             _dev_ptr(forces, torch.float32, (N, 3)), _dev_ptr(virial, torch.float64),
+                                             _stream_ptr(stream)))
+        return energy, e_atom, forces, virial
 
     def energy_forces_host(self, positions: np.ndarray, forces: np.ndarray, energy_per_atom: Optional[np.ndarray] = None,
                            stream=None) -> float:

@@ -46,14 +46,15 @@ __device__ __forceinline__ float image_diff(float xj, float xi, float shift) {
 }
 
 __device__ __forceinline__ PairGeom pair_geometry(uint32_t entry, const float4 &xi, const float4 *__restrict__ pos4,
-                                                  const float L0, const float L1, const float L2) {
+                                                  const Geometry &geo) {
     PairGeom g;
     g.j = (int)(entry & NBR_J_MASK);
     const float4 xj = __ldg(&pos4[g.j]);
     g.zj = __float_as_int(xj.w);
-    const float sx = (float)((int)((entry >> NBR_J_BITS) & 7u) - 4) * L0;
-    const float sy = (float)((int)((entry >> (NBR_J_BITS + 3)) & 7u) - 4) * L1;
-    const float sz = (float)((int)((entry >> (NBR_J_BITS + 6)) & 7u) - 4) * L2;
+    // lattice shift n1 a + n2 b + n3 c of the entry's image (n_x L_x on an orthorhombic cell)
+    const float n1 = (float)((int)((entry >> NBR_J_BITS) & 7u) - 4), n2 = (float)((int)((entry >> (NBR_J_BITS + 3)) & 7u) - 4),
+                n3 = (float)((int)((entry >> (NBR_J_BITS + 6)) & 7u) - 4);
+    const float sx = lattice_shift(geo, 0, n1, n2, n3), sy = lattice_shift(geo, 1, n1, n2, n3), sz = lattice_shift(geo, 2, n1, n2, n3);
     g.dx = image_diff(xj.x, xi.x, sx);
     g.dy = image_diff(xj.y, xi.y, sy);
     g.dz = image_diff(xj.z, xi.z, sz);
@@ -133,7 +134,7 @@ k_pair_forward(int64_t N, const float4 *__restrict__ pos4, const uint32_t *__res
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
                 if (k4 * 4 + q >= cnt) break;
-                const PairGeom pg = pair_geometry(ent[q], xi, pos4, geo.L[0], geo.L[1], geo.L[2]);
+                const PairGeom pg = pair_geometry(ent[q], xi, pos4, geo);
                 if (pg.r2 < rp.r_cut2) {
                     const float rinv = rsqrtf(pg.r2);
                     const float r = pg.r2 * rinv;
@@ -504,12 +505,15 @@ __device__ __forceinline__ void pair_gradient(AGet a, const float *R, const floa
 // PAIRBUF = false: gather form, both directions per entry, F_i complete.
 // PAIRBUF = true : own direction only; g_ij goes to gbuf[j][rev] (the slot of (i, -n) in the row of
 //                  j), f_int gets sum_j g_ij, and k_force_reduce subtracts the received row.
-template <int NR, int NB, int LPA, bool PAIRBUF>
+// VIRIAL: also leaves vir_atom[c][i] = -sum_j d_a g_b (c = 3 a + b) over the centre's own directed pairs, whose sum
+// over the atoms is the virial W = -sum_pairs d (x) g = -dE/d strain (oracle O-16).
+template <int NR, int NB, int LPA, bool PAIRBUF, bool VIRIAL>
 __global__ void __launch_bounds__(128)
 k_pair_backward(int64_t N, const float4 *__restrict__ pos4, const uint32_t *__restrict__ nbr,
                 const int32_t *__restrict__ count, int cap, Geometry geo, RadialParams rp,
                 const float *__restrict__ beta, const float *__restrict__ A, float *__restrict__ f_int,
-                const uint16_t *__restrict__ rev, float4 *__restrict__ gbuf, const int32_t *__restrict__ mrow) {
+                const uint16_t *__restrict__ rev, float4 *__restrict__ gbuf, const int32_t *__restrict__ mrow,
+                float *__restrict__ vir_atom) {
     constexpr int KB = (NB + 3) & ~3;
     constexpr int ROW = NR * KB;
     constexpr int GROUPS = 128 / LPA;
@@ -534,6 +538,9 @@ k_pair_backward(int64_t N, const float4 *__restrict__ pos4, const uint32_t *__re
     }
     __syncthreads();
     float fx = 0.f, fy = 0.f, fz = 0.f;
+    float vir[VIRIAL ? 9 : 1];
+#pragma unroll
+    for (int c = 0; c < (VIRIAL ? 9 : 1); ++c) vir[c] = 0.f;
     if (live) {
         const float4 xi = pos4[i];
         const int zi = __float_as_int(xi.w);
@@ -561,7 +568,7 @@ k_pair_backward(int64_t N, const float4 *__restrict__ pos4, const uint32_t *__re
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
                 if (k4 * 4 + q >= cnt) break;
-                const PairGeom pg = pair_geometry(ent[q], xi, pos4, geo.L[0], geo.L[1], geo.L[2]);
+                const PairGeom pg = pair_geometry(ent[q], xi, pos4, geo);
                 if (PAIRBUF && rv[q] == 0xFFFFu) continue;  // no partner (overflowed rebuild): flagged by k_build_rev
                 float4 *slot = PAIRBUF ? gbuf + (int64_t)pg.j * cap + rv[q] : nullptr;
                 if (PAIRBUF && pg.r2 >= rp.r_cut2) *slot = make_float4(0.f, 0.f, 0.f, 0.f);  // skin shell
@@ -611,6 +618,13 @@ k_pair_backward(int64_t N, const float4 *__restrict__ pos4, const uint32_t *__re
                         }
                     }
                     if (PAIRBUF) *slot = make_float4(gxo, gyo, gzo, 0.f);
+                    if (VIRIAL) {
+                        const float dv[3] = {pg.dx, pg.dy, pg.dz}, gv[3] = {gxo, gyo, gzo};
+#pragma unroll
+                        for (int a = 0; a < 3; ++a)
+#pragma unroll
+                            for (int b = 0; b < 3; ++b) vir[3 * a + b] = fmaf(-dv[a], gv[b], vir[3 * a + b]);
+                    }
                     // F_i += g_ij - g_ji   (g_ji = dE_j/dd_ji, d_ji = -d_ij)
                     fx += gxo - gxr;
                     fy += gyo - gyr;
@@ -629,6 +643,14 @@ k_pair_backward(int64_t N, const float4 *__restrict__ pos4, const uint32_t *__re
         f_int[3 * i] = fx;
         f_int[3 * i + 1] = fy;
         f_int[3 * i + 2] = fz;
+    }
+    if (VIRIAL) {
+#pragma unroll
+        for (int c = 0; c < 9; ++c) {
+#pragma unroll
+            for (int o = LPA / 2; o >= 1; o >>= 1) vir[c] += __shfl_xor_sync(0xffffffffu, vir[c], o);
+            if (live && sub == 0) vir_atom[(int64_t)c * N + i] = vir[c];
+        }
     }
 }
 
@@ -706,27 +728,34 @@ static int pair_backward_lpa(gmnn_system *s, cudaStream_t st, int lpa) {
     const size_t smem = sizeof(float) * (beta_floats + (128 / lpa) * NR * PSI);
     const unsigned grid = nblocks(s->N * lpa, 128);
     const bool pairbuf = s->force_mode == GMNN_FORCE_PAIRBUF;
+    const bool virial = s->want_virial && s->vir_atom != nullptr;
     if (pairbuf && !(s->list_has_rev && s->rev && s->gbuf)) {
         set_error("force_mode changed after the list was built: call gmnn_build_neighbors again");
         return GMNN_INVALID_ARG;
     }
+#define GMNN_PB_LAUNCH(L, PB, VIR)                                                                         \
+    k_pair_backward<NR, NB, L, PB, VIR><<<grid, 128, smem, st>>>(s->N, s->pos4, s->nbr, s->count, s->cap, s->geo, m->rp, \
+                                                                m->beta, s->A, s->f_int, PB ? s->rev : nullptr, \
+                                                                PB ? s->gbuf : nullptr, s->mrow, VIR ? s->vir_atom : nullptr)
 #define GMNN_PB(L)                                                                                         \
     case L: {                                                                                              \
         static size_t opted_on[MAX_DEVICES] = {};                                                          \
         size_t &opted = opted_on[current_device()];                                                        \
         if (smem > 48 * 1024 && smem > opted) {                                                            \
-            GMNN_CUDA(cudaFuncSetAttribute(k_pair_backward<NR, NB, L, false>,                              \
+            GMNN_CUDA(cudaFuncSetAttribute(k_pair_backward<NR, NB, L, false, false>,                       \
                                            cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));       \
-            GMNN_CUDA(cudaFuncSetAttribute(k_pair_backward<NR, NB, L, true>,                               \
+            GMNN_CUDA(cudaFuncSetAttribute(k_pair_backward<NR, NB, L, true, false>,                        \
+                                           cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));       \
+            GMNN_CUDA(cudaFuncSetAttribute(k_pair_backward<NR, NB, L, false, true>,                        \
+                                           cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));       \
+            GMNN_CUDA(cudaFuncSetAttribute(k_pair_backward<NR, NB, L, true, true>,                         \
                                            cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));       \
             opted = smem;                                                                                  \
         }                                                                                                  \
-        if (pairbuf)                                                                                       \
-            k_pair_backward<NR, NB, L, true><<<grid, 128, smem, st>>>(s->N, s->pos4, s->nbr, s->count, s->cap, s->geo, \
-                                                                  m->rp, m->beta, s->A, s->f_int, s->rev, s->gbuf, s->mrow); \
-        else                                                                                               \
-            k_pair_backward<NR, NB, L, false><<<grid, 128, smem, st>>>(s->N, s->pos4, s->nbr, s->count, s->cap, s->geo, \
-                                                                   m->rp, m->beta, s->A, s->f_int, nullptr, nullptr, s->mrow); \
+        if (pairbuf && virial) GMNN_PB_LAUNCH(L, true, true);                                              \
+        else if (pairbuf) GMNN_PB_LAUNCH(L, true, false);                                                  \
+        else if (virial) GMNN_PB_LAUNCH(L, false, true);                                                   \
+        else GMNN_PB_LAUNCH(L, false, false);                                                              \
     } break;
     switch (lpa) {
         GMNN_PB(1) GMNN_PB(2) GMNN_PB(4) GMNN_PB(8) GMNN_PB(16) GMNN_PB(32)
@@ -735,6 +764,7 @@ static int pair_backward_lpa(gmnn_system *s, cudaStream_t st, int lpa) {
             return GMNN_INVALID_ARG;
     }
 #undef GMNN_PB
+#undef GMNN_PB_LAUNCH
     GMNN_LAUNCHED();
     if (pairbuf) {
         k_force_reduce<8><<<nblocks(s->N * 8, 256), 256, 0, st>>>(s->N, s->count, s->cap, s->gbuf, s->f_int);

@@ -427,7 +427,7 @@ int gmnn_system_create(const gmnn_model *m, int64_t n_atoms, const int32_t *spec
 
 void gmnn_system_destroy(gmnn_system *s) {
     if (!s) return;
-    dev_free(s->mrow); dev_free(s->row_atom); dev_free(s->sp_count);
+    dev_free(s->mrow); dev_free(s->row_atom); dev_free(s->sp_count); dev_free(s->vir_atom);
     dev_free(s->species); dev_free(s->cell_of); dev_free(s->cell_count); dev_free(s->cell_start);
     dev_free(s->cell_fill); dev_free(s->slot_tmp); dev_free(s->perm); dev_free(s->pos4); dev_free(s->xref);
     dev_free(s->nbr); dev_free(s->rev); dev_free(s->gbuf); dev_free(s->runs); dev_free(s->count); dev_free(s->psi); dev_free(s->G); dev_free(s->dG); dev_free(s->A);
@@ -545,6 +545,7 @@ int gmnn_build_neighbors(gmnn_system *s, const float *positions, const float cel
         set_error("skin must be finite and >= 0");
         return GMNN_INVALID_ARG;
     }
+    bool triclinic = false;
     for (int a = 0; a < 3; ++a)
         for (int b = 0; b < 3; ++b) {
             const float v = cell[3 * a + b];
@@ -552,11 +553,28 @@ int gmnn_build_neighbors(gmnn_system *s, const float *positions, const float cel
                 set_error("cell must be finite with positive diagonal");
                 return GMNN_INVALID_ARG;
             }
-            if (a != b && v != 0.f) {
-                set_error("triclinic cells are not supported (orthorhombic only, DESIGN.md R19)");
-                return GMNN_UNSUPPORTED;
-            }
+            if (a != b && v != 0.f) triclinic = true;
         }
+    // general lattice (rows a, b, c): volume, inverse and the distances w_a between opposite faces, in fp64
+    double hd[9], hinv[9], w[3], cell_volume = 0.0;
+    for (int q = 0; q < 9; ++q) hd[q] = (double)cell[q];
+    {
+        const double *a = hd, *b = hd + 3, *c = hd + 6;
+        const double bc[3] = {b[1] * c[2] - b[2] * c[1], b[2] * c[0] - b[0] * c[2], b[0] * c[1] - b[1] * c[0]};
+        const double ca[3] = {c[1] * a[2] - c[2] * a[1], c[2] * a[0] - c[0] * a[2], c[0] * a[1] - c[1] * a[0]};
+        const double ab[3] = {a[1] * b[2] - a[2] * b[1], a[2] * b[0] - a[0] * b[2], a[0] * b[1] - a[1] * b[0]};
+        const double det = a[0] * bc[0] + a[1] * bc[1] + a[2] * bc[2];
+        if (!(std::fabs(det) > 1e-6)) {
+            set_error("cell is singular (volume %g)", det);
+            return GMNN_INVALID_ARG;
+        }
+        cell_volume = std::fabs(det);
+        w[0] = std::fabs(det) / std::sqrt(bc[0] * bc[0] + bc[1] * bc[1] + bc[2] * bc[2]);
+        w[1] = std::fabs(det) / std::sqrt(ca[0] * ca[0] + ca[1] * ca[1] + ca[2] * ca[2]);
+        w[2] = std::fabs(det) / std::sqrt(ab[0] * ab[0] + ab[1] * ab[1] + ab[2] * ab[2]);
+        // x (row) . hinv = fractional coordinates: columns of hinv are the reciprocal vectors
+        for (int x = 0; x < 3; ++x) hinv[3 * x + 0] = bc[x] / det, hinv[3 * x + 1] = ca[x] / det, hinv[3 * x + 2] = ab[x] / det;
+    }
     s->md_state_valid = false;
     // The handle holds no usable list from here until this call succeeds: an earlier list must never
     // sit beside the new geometry, a freed row buffer or truncated rows (every failure path below
@@ -566,12 +584,16 @@ int gmnn_build_neighbors(gmnn_system *s, const float *positions, const float cel
     const float r_list = r_cut + skin;  // fl32(fl32(r_cut) + fl32(skin)): the oracle is handed the same float
     g.r_list2 = r_list * r_list;
     g.r_cut2 = r_cut * r_cut;
+    g.triclinic = triclinic ? 1 : 0;
+    for (int q = 0; q < 9; ++q) g.h[q] = cell[q], g.hinv[q] = (float)hinv[q];
     bool small = false;
     for (int a = 0; a < 3; ++a) {
         g.L[a] = cell[4 * a];
         g.invL[a] = 1.f / g.L[a];
         g.pbc[a] = pbc[a] != 0;
-        int nc = (int)std::floor((double)g.L[a] / ((double)r_list * (1.0 + 1e-5)));
+        // slabs at least r_list thick between the faces of axis a (w_a = L_a for an orthorhombic cell)
+        const double width = triclinic ? w[a] : (double)g.L[a];
+        int nc = (int)std::floor(width / ((double)r_list * (1.0 + 1e-5)));
         if (nc < 1) nc = 1;
         if (nc > 1024) nc = 1024;
         g.ncell[a] = nc;
@@ -584,9 +606,10 @@ int gmnn_build_neighbors(gmnn_system *s, const float *positions, const float cel
             return GMNN_UNSUPPORTED;
         }
         for (int a = 0; a < 3; ++a) {
-            g.kimg[a] = g.pbc[a] ? (int)std::ceil(r_list / g.L[a]) : 0;  // fp32 division, as the oracle's ceilf
+            // orthorhombic: fp32 division, as the oracle's ceilf; general lattice: the face distance
+            g.kimg[a] = !g.pbc[a] ? 0 : triclinic ? (int)std::ceil((double)r_list / w[a]) : (int)std::ceil(r_list / g.L[a]);
             if (g.kimg[a] > 3) {
-                set_error("box edge %g needs more than 3 periodic images at r_list = %g", g.L[a], r_list);
+                set_error("box needs more than 3 periodic images along axis %d at r_list = %g", a, r_list);
                 return GMNN_UNSUPPORTED;
             }
             g.ncell[a] = 1;
@@ -613,11 +636,7 @@ int gmnn_build_neighbors(gmnn_system *s, const float *positions, const float cel
     // capacity: expected neighbours at uniform density x 1.3 + 32, a multiple of 32
     int want = s->cap_request;
     if (want <= 0) {
-        double vol = (double)g.L[0] * g.L[1] * g.L[2];
-        double per = (double)s->N / vol * 4.0 / 3.0 * M_PI * std::pow((double)r_list, 3.0);
-        if (small) {  // count the images as well
-            per = (double)s->N / vol * 4.0 / 3.0 * M_PI * std::pow((double)r_list, 3.0);
-        }
+        const double per = (double)s->N / cell_volume * 4.0 / 3.0 * M_PI * std::pow((double)r_list, 3.0);
         want = (int)(per * 1.3) + 32;
     }
     want = (want + 31) & ~31;
@@ -792,6 +811,26 @@ int gmnn_energy_forces(gmnn_system *s, const float *positions, double *energy, f
     if ((rc = launch_energy_sum(s, energy, st))) return rc;
     T.mark("outputs");
     return GMNN_OK;
+}
+
+int gmnn_energy_forces_virial(gmnn_system *s, const float *positions, double *energy, float *energy_per_atom,
+                              float *forces, double *virial, void *cuda_stream) {
+    if (!s || !virial) {
+        set_error("gmnn_energy_forces_virial: null argument");
+        return GMNN_INVALID_ARG;
+    }
+    if (!s->vir_atom) {  // per-atom virial terms [9][N], allocated at the first call that asks for the virial
+        int rc = dev_alloc(&s->vir_atom, (size_t)9 * (size_t)s->N);
+        if (rc) return rc;
+    }
+    struct Want {
+        gmnn_system *s;
+        ~Want() { s->want_virial = false; }
+    } guard{s};
+    s->want_virial = true;
+    int rc = gmnn_energy_forces(s, positions, energy, energy_per_atom, forces, cuda_stream);
+    if (rc) return rc;
+    return launch_virial_sum(s, virial, (cudaStream_t)cuda_stream);
 }
 
 int gmnn_energy_forces_host(gmnn_system *s, const float *positions, double *energy, float *energy_per_atom,

@@ -52,15 +52,28 @@ inline int current_device() {
     } while (0)
 
 struct Geometry {  // passed by value to kernels
-    float L[3];
+    float L[3];        // orthorhombic edge lengths = the diagonal of h
     float invL[3];
     int pbc[3];
     int ncell[3];
-    float inv_edge[3];
+    float inv_edge[3];  // orthorhombic: cells per Angstrom (ncell / L)
     int kimg[3];  // image range of the small-box path
     float r_list2;
     float r_cut2;  // rows are built inside-r_cut first, skin shell last (neighbor.cu)
+    // general lattice: h rows = lattice vectors a, b, c; fractional s = x . hinv.  triclinic = 0
+    // when every off-diagonal element is zero: the kernels then take the orthorhombic expressions, whose results
+    // the general ones reproduce bit for bit (adding an exact zero), so one list format serves both.
+    int triclinic;
+    float h[9];
+    float hinv[9];
 };
+
+// lattice shift of image (n1, n2, n3), component x: the diagonal term first, so that with zero off-diagonals the
+// value is exactly n_x L_x
+__device__ __forceinline__ float lattice_shift(const Geometry &g, int x, float n1, float n2, float n3) {
+    if (!g.triclinic) return (x == 0 ? n1 : x == 1 ? n2 : n3) * g.L[x];
+    return n1 * g.h[x] + n2 * g.h[3 + x] + n3 * g.h[6 + x];
+}
 
 struct RadialParams {  // passed by value to the pair kernels
     int n_species, n_basis, kb;  // kb = n_basis rounded up to 4 (row pitch of the beta table)
@@ -161,6 +174,8 @@ struct gmnn_system {
     bool heads_fused = false;        // the last mlp_forward left ypart instead of H[L-1]
     int head_slots = 0;
     float *e_heads = nullptr;        // [N][n_heads]
+    float *vir_atom = nullptr;       // [9][N] per-atom virial terms -sum_j d_a g_b (lazy; gmnn_energy_forces_virial)
+    bool want_virial = false;        // this evaluation's pair backward also leaves vir_atom
     float *e_atom = nullptr;         // [N]
     float *f_int = nullptr;          // [N][3]
     float *f_tmp = nullptr;          // [N][3] caller order (ensemble, MD)
@@ -237,6 +252,7 @@ int launch_mlp_backward_simt(gmnn_system *s, const float *head_w_dev, cudaStream
 // md.cu / reductions
 int launch_scatter_outputs(gmnn_system *s, float *e_atom_out, float *forces_out, cudaStream_t st);
 int launch_energy_sum(gmnn_system *s, double *energy_out, cudaStream_t st, double *energy_out2 = nullptr);
+int launch_virial_sum(gmnn_system *s, double *virial_out, cudaStream_t st);  // [9] fixed-order fp64 sums of vir_atom
 int launch_kick_drift(gmnn_system *s, float *x, float *v, const float *f, const float *m, float dt, cudaStream_t st);
 int launch_kick_ke(gmnn_system *s, float *v, const float *f, const float *m, float dt, double *ekin_out,
                    cudaStream_t st, double *ekin_out2 = nullptr);

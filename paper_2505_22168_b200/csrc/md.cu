@@ -165,6 +165,33 @@ int launch_energy_sum(gmnn_system *s, double *energy_out, cudaStream_t st, doubl
     return GMNN_OK;
 }
 
+// virial: component c = blockIdx.y of vir_atom [9][N]; same fixed two-stage order as the energy sum
+__global__ void __launch_bounds__(256) k_sum9_stage1(int64_t N, const float *__restrict__ x, double *partial) {
+    const int64_t per = (N + gridDim.x - 1) / gridDim.x;
+    const int64_t b = blockIdx.x * per, e = b + per < N ? b + per : N;
+    const float *xc = x + (int64_t)blockIdx.y * N;
+    double v = 0.0;
+    for (int64_t q = b + threadIdx.x; q < e; q += blockDim.x) v += (double)xc[q];
+    v = block_sum(v);
+    if (threadIdx.x == 0) partial[blockIdx.y * gridDim.x + blockIdx.x] = v;
+}
+__global__ void __launch_bounds__(256) k_sum9_stage2(int n, const double *__restrict__ partial, double *out) {
+    double v = 0.0;
+    for (int q = threadIdx.x; q < n; q += blockDim.x) v += partial[blockIdx.x * n + q];
+    v = block_sum(v);
+    if (threadIdx.x == 0) out[blockIdx.x] = v;
+}
+
+int launch_virial_sum(gmnn_system *s, double *virial_out, cudaStream_t st) {
+    const int nb = red_blocks(s->N) < 113 ? red_blocks(s->N) : 113;  // 9 x 113 partials fit the 2048-double scratch
+    k_sum9_stage1<<<dim3(nb, 9), 256, 0, st>>>(s->N, s->vir_atom, s->partial);
+    GMNN_LAUNCHED();
+    k_sum9_stage2<<<9, 256, 0, st>>>(nb, s->partial, virial_out);
+    GMNN_LAUNCHED();
+    GMNN_CUDA(cudaGetLastError());
+    return GMNN_OK;
+}
+
 int launch_ke(gmnn_system *s, const float *v, const float *m, double *ekin_out, cudaStream_t st, double *ekin_out2) {
     const int nb = red_blocks(s->N);
     k_ke_stage1<<<nb, 256, 0, st>>>(s->N, v, m, s->partial + RED_BLOCKS);

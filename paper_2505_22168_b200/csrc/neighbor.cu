@@ -22,8 +22,28 @@ __device__ __forceinline__ bool skip_rebuild(const int32_t *cond, float thr2) {
     return cond != nullptr && __int_as_float(*((const volatile int32_t *)cond)) <= thr2;
 }
 
+// fractional coordinate a of position p in a general lattice
+__device__ __forceinline__ float frac_coord(const Geometry &g, const float *p, int a) {
+    return p[0] * g.hinv[a] + p[1] * g.hinv[3 + a] + p[2] * g.hinv[6 + a];
+}
+
 __global__ void k_wrap(int64_t N, float *x, Geometry g, const int32_t *cond, float thr2) {
     if (skip_rebuild(cond, thr2)) return;
+    if (g.triclinic) {  // fold in fractional coordinates: x -= floor(s_a) a_a on the periodic axes
+        for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < N; i += gridDim.x * (int64_t)blockDim.x) {
+            float p[3] = {x[3 * i], x[3 * i + 1], x[3 * i + 2]};
+            for (int pass = 0; pass < 2; ++pass)  // the second pass catches a rounding step across a face
+                for (int a = 0; a < 3; ++a) {
+                    if (!g.pbc[a]) continue;
+                    const float k = floorf(frac_coord(g, p, a));
+                    if (k != 0.f) {
+                        p[0] -= k * g.h[3 * a], p[1] -= k * g.h[3 * a + 1], p[2] -= k * g.h[3 * a + 2];
+                    }
+                }
+            x[3 * i] = p[0], x[3 * i + 1] = p[1], x[3 * i + 2] = p[2];
+        }
+        return;
+    }
     for (int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; t < 3 * N; t += gridDim.x * (int64_t)blockDim.x) {
         int a = (int)(t % 3);
         if (!g.pbc[a]) continue;
@@ -46,6 +66,11 @@ __device__ __forceinline__ int cell_coord(float x, float inv_edge, int nc) {
     int c = (int)floorf(x * inv_edge);
     return c < 0 ? 0 : (c >= nc ? nc - 1 : c);
 }
+// cell index along axis a of position p: slabs in x for diag(L), in fractional coordinates for a general lattice
+__device__ __forceinline__ int cell_coord_of(const Geometry &g, const float *p, int a) {
+    if (!g.triclinic) return cell_coord(p[a], g.inv_edge[a], g.ncell[a]);
+    return cell_coord(frac_coord(g, p, a), (float)g.ncell[a], g.ncell[a]);
+}
 
 __global__ void k_cell_assign(int64_t N, const float *__restrict__ x, Geometry g, int32_t *cell_of,
                               int32_t *cell_count, int32_t *flags, const int32_t *cond, float thr2) {
@@ -56,8 +81,13 @@ __global__ void k_cell_assign(int64_t N, const float *__restrict__ x, Geometry g
         bool bad = false;
 #pragma unroll
         for (int a = 0; a < 3; ++a) {
-            bad |= !(p[a] >= 0.f && p[a] < g.L[a]);
-            c[a] = cell_coord(p[a], g.inv_edge[a], g.ncell[a]);
+            if (g.triclinic) {  // inside the cell up to the rounding of the fractional coordinate
+                const float f = frac_coord(g, p, a);
+                bad |= !(f >= -1e-5f && f < 1.f + 1e-5f);
+            } else {
+                bad |= !(p[a] >= 0.f && p[a] < g.L[a]);
+            }
+            c[a] = cell_coord_of(g, p, a);
         }
         if (bad) flags[FLAG_OUT_OF_BOX] = 1;
         int cid = (c[2] * g.ncell[1] + c[1]) * g.ncell[0] + c[0];
@@ -160,6 +190,12 @@ __device__ __forceinline__ bool in_list(const float4 &xi, const float4 &xj, floa
     return list_r2(xi, xj, sx, sy, sz) < rl2;
 }
 
+// lattice shift of the membership predicate, component x, in the unfused order reading R20 / O-16 fixes:
+// fl(fl(fl(n1 a_x) + fl(n2 b_x)) + fl(n3 c_x)); with zero off-diagonals this is fl(n_x L_x) exactly
+__device__ __forceinline__ float list_shift(const Geometry &g, int x, int n1, int n2, int n3) {
+    return __fadd_rn(__fadd_rn(__fmul_rn((float)n1, g.h[x]), __fmul_rn((float)n2, g.h[3 + x])), __fmul_rn((float)n3, g.h[6 + x]));
+}
+
 __device__ __forceinline__ uint32_t image_code(int nx, int ny, int nz) {
     return ((uint32_t)(nx + 4) << NBR_J_BITS) | ((uint32_t)(ny + 4) << (NBR_J_BITS + 3)) |
            ((uint32_t)(nz + 4) << (NBR_J_BITS + 6));
@@ -194,9 +230,8 @@ k_build_cells(int64_t N, const float4 *__restrict__ pos4, const int32_t *__restr
     const int64_t n_warps = (gridDim.x * (int64_t)blockDim.x) >> 5;
     for (int64_t i = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5; i < N; i += n_warps) {
         const float4 xi = pos4[i];
-        const int cx = cell_coord(xi.x, g.inv_edge[0], g.ncell[0]);
-        const int cy = cell_coord(xi.y, g.inv_edge[1], g.ncell[1]);
-        const int cz = cell_coord(xi.z, g.inv_edge[2], g.ncell[2]);
+        const float pi3[3] = {xi.x, xi.y, xi.z};
+        const int cx = cell_coord_of(g, pi3, 0), cy = cell_coord_of(g, pi3, 1), cz = cell_coord_of(g, pi3, 2);
         uint32_t *row = nbr + i * (int64_t)cap;
         // visit(idx, fn): candidates of cell idx in chunks of 32; fn(entry, r2, valid) per lane
         auto visit = [&](int idx, auto fn) {
@@ -212,8 +247,7 @@ k_build_cells(int64_t N, const float4 *__restrict__ pos4, const int32_t *__restr
             else if (x >= g.ncell[0]) { if (!g.pbc[0]) return; x -= g.ncell[0]; nx = 1; }
             const int c = (z * g.ncell[1] + y) * g.ncell[0] + x;
             const int b = cell_start[c], e = cell_start[c + 1];
-            const float sx = __fmul_rn((float)nx, g.L[0]), sy = __fmul_rn((float)ny, g.L[1]),
-                        sz = __fmul_rn((float)nz, g.L[2]);
+            const float sx = list_shift(g, 0, nx, ny, nz), sy = list_shift(g, 1, nx, ny, nz), sz = list_shift(g, 2, nx, ny, nz);
             const uint32_t code = image_code(nx, ny, nz);
             const bool home = (nx | ny | nz) == 0;
             for (int base = b; base < e; base += 32) {
@@ -285,8 +319,8 @@ k_build_small(int64_t N, const float4 *__restrict__ pos4, Geometry g, uint32_t *
         for (int nz = -g.kimg[2]; nz <= g.kimg[2]; ++nz)
             for (int ny = -g.kimg[1]; ny <= g.kimg[1]; ++ny)
                 for (int nx = -g.kimg[0]; nx <= g.kimg[0]; ++nx) {
-                    const float sx = __fmul_rn((float)nx, g.L[0]), sy = __fmul_rn((float)ny, g.L[1]),
-                                sz = __fmul_rn((float)nz, g.L[2]);
+                    const float sx = list_shift(g, 0, nx, ny, nz), sy = list_shift(g, 1, nx, ny, nz),
+                                sz = list_shift(g, 2, nx, ny, nz);
                     const uint32_t code = image_code(nx, ny, nz);
                     const bool home = (nx | ny | nz) == 0;
                     for (int base = 0; base < (int)N; base += 32) {
