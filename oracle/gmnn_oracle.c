@@ -66,6 +66,10 @@ typedef struct {
     int32_t hidden[4];
     int32_t n_heads;
     int32_t n_weight_sets; /* 1 (or 0): one NN for all species (Eq. 4); n_species: the (W, b) of set Z_i (O-5) */
+    int32_t basis_kind;    /* 0: equidistant Gaussians (O-2); 1: Bessel-like functions of Kocer et al. (O-17) */
+    int32_t zbl_on;        /* 1: add the ZBL repulsion (O-18) */
+    double zbl_r_max;      /* Ang, cutoff of the ZBL term (<= r_cut) */
+    double zbl_scale;      /* dimensionless prefactor of the ZBL term */
 } oracle_hparams;
 
 typedef struct {
@@ -74,6 +78,7 @@ typedef struct {
     const double *b[5];  /* layer l: [n_weight_sets][fan_out] */
     const double *scale; /* [S] sigma_Z */
     const double *shift; /* [S] mu_Z */
+    const double *atomic_number; /* [S] nuclear charges Z (O-18), nullable when zbl_on == 0 */
 } oracle_weights;
 
 int oracle_num_threads(void) {
@@ -307,6 +312,35 @@ int64_t oracle_neighbors_cells(int64_t N, const float *pos, const float *h, cons
  *   R'_s = f_c' sum_k beta Phi_k + f_c sum_k beta Phi_k (-2 gamma (r - mu_k)),
  *   f_c' = -(pi / (2 r_cut)) sin(pi r / r_cut)
  * ------------------------------------------------------------------------------------------ */
+/* O-2 / O-17  The n_basis basis functions of one distance and their derivatives (no cutoff function).
+ * kind 0 ("equidistant Gaussians"): Phi_k = exp(-gamma (r - mu_k)^2), mu_k = r_min + k Delta.
+ * kind 1 ("the non-orthogonal Bessel-like functions of Kocer et al."; reading R30), n = 0..n_b-1:
+ *   f_n(r) = (-1)^n sqrt(2) pi / r_c^(3/2) (n+1)(n+2) / sqrt((n+1)^2 + (n+2)^2)
+ *            [ sinc((n+1) pi r / r_c) + sinc((n+2) pi r / r_c) ],   sinc(x) = sin(x) / x
+ *   (unit norm under int_0^rc . r^2 dr; zero at r_c; the orthogonalisation step of that paper is not applied),
+ *   d/dr sinc(a r) = (cos(a r) - sinc(a r)) / r. */
+void oracle_basis(const oracle_hparams *hp, double r, double *phi, double *dphi) {
+    const int nb = hp->n_basis;
+    if (hp->basis_kind == 1) {
+        const double rc = hp->r_cut;
+        for (int n = 0; n < nb; ++n) {
+            double a1 = (n + 1) * M_PI / rc, a2 = (n + 2) * M_PI / rc;
+            double c = ((n & 1) ? -1.0 : 1.0) * sqrt(2.0) * M_PI / pow(rc, 1.5) * (n + 1.0) * (n + 2.0) /
+                       sqrt((n + 1.0) * (n + 1.0) + (n + 2.0) * (n + 2.0));
+            double s1 = sin(a1 * r) / (a1 * r), s2 = sin(a2 * r) / (a2 * r);
+            phi[n] = c * (s1 + s2);
+            if (dphi) dphi[n] = c * ((cos(a1 * r) - s1) + (cos(a2 * r) - s2)) / r;
+        }
+        return;
+    }
+    const double delta = (hp->r_cut - hp->r_min) / (nb - 1);
+    for (int k = 0; k < nb; ++k) {
+        double mu = hp->r_min + k * delta;
+        phi[k] = exp(-hp->gamma * (r - mu) * (r - mu));
+        if (dphi) dphi[k] = phi[k] * (-2.0 * hp->gamma * (r - mu));
+    }
+}
+
 void oracle_radial(const oracle_hparams *hp, const double *beta, int zi, int zj, double r, double *R, double *dR) {
     const int nb = hp->n_basis, nr = hp->n_radial, S = hp->n_species;
     if (r >= hp->r_cut) {
@@ -316,21 +350,48 @@ void oracle_radial(const oracle_hparams *hp, const double *beta, int zi, int zj,
         }
         return;
     }
-    const double delta = (hp->r_cut - hp->r_min) / (nb - 1);
+    double phi[64], dphi[64];
+    oracle_basis(hp, r, phi, dphi);
     const double fc = 0.5 * (1.0 + cos(M_PI * r / hp->r_cut));
     const double dfc = -0.5 * M_PI / hp->r_cut * sin(M_PI * r / hp->r_cut);
     for (int s = 0; s < nr; ++s) {
         double sum = 0.0, dsum = 0.0;
         for (int k = 0; k < nb; ++k) {
-            double mu = hp->r_min + k * delta;
-            double phi = exp(-hp->gamma * (r - mu) * (r - mu));
             double bk = beta[(((size_t)zi * S + zj) * nr + s) * nb + k];
-            sum += bk * phi;
-            dsum += bk * phi * (-2.0 * hp->gamma * (r - mu));
+            sum += bk * phi[k];
+            dsum += bk * dphi[k];
         }
         R[s] = fc * sum;
         if (dR) dR[s] = dfc * sum + fc * dsum;
     }
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O-18  ZBL repulsion ("empirical energy correction terms, such as the Ziegler-Littmark-Biersack
+ * potential, can be supplied"; reading R31).  For a pair of nuclear charges Z1, Z2 at distance r < r_zbl:
+ *   V(r) = scale k_e Z1 Z2 / r  phi(r / a)  f_c(r; r_zbl),   k_e = 14.399645 eV Ang,
+ *   a = 0.8854 a_0 / (Z1^0.23 + Z2^0.23),  a_0 = 0.529177 Ang,
+ *   phi(x) = 0.1818 e^(-3.2 x) + 0.5099 e^(-0.9423 x) + 0.2802 e^(-0.4029 x) + 0.02817 e^(-0.2016 x),
+ *   f_c = 1/2 [1 + cos(pi r / r_zbl)].
+ * E gets V once per unordered pair: every DIRECTED pair of the full list carries V/2, added to the centre's E_i
+ * (after sigma, mu: it is not a network output).  Returns V/2 and d(V/2)/dr.
+ * ------------------------------------------------------------------------------------------ */
+void oracle_zbl_half(const oracle_hparams *hp, double z1, double z2, double r, double *e, double *de) {
+    *e = 0.0;
+    if (de) *de = 0.0;
+    if (!hp->zbl_on || r >= hp->zbl_r_max) return;
+    static const double c[4] = {0.1818, 0.5099, 0.2802, 0.02817}, d[4] = {3.2, 0.9423, 0.4029, 0.2016};
+    const double a = 0.8854 * 0.529177 / (pow(z1, 0.23) + pow(z2, 0.23));
+    double phi = 0.0, dphi = 0.0;
+    for (int k = 0; k < 4; ++k) {
+        phi += c[k] * exp(-d[k] * r / a);
+        dphi += c[k] * exp(-d[k] * r / a) * (-d[k] / a);
+    }
+    const double coul = 0.5 * hp->zbl_scale * 14.399645 * z1 * z2 / r, dcoul = -coul / r;
+    const double fc = 0.5 * (1.0 + cos(M_PI * r / hp->zbl_r_max));
+    const double dfc = -0.5 * M_PI / hp->zbl_r_max * sin(M_PI * r / hp->zbl_r_max);
+    *e = coul * phi * fc;
+    if (de) *de = dcoul * phi * fc + coul * dphi * fc + coul * phi * dfc;
 }
 
 /* d = x_j - x_i + n1 a + n2 b + n3 c in fp64 (positions are fp32 values promoted to fp64; L = the 3x3 cell, rows a, b, c). */
@@ -705,7 +766,16 @@ static void forward_all(const oracle_hparams *hp, const oracle_weights *w, int64
         moments_of_atom(hp, w->beta, pos, species, L, i, off[i], off[i + 1], pj, pn, Pi);
         oracle_invariants(nr, Pi, G + (size_t)i * F);
         oracle_mlp_forward(hp, w, F, G + (size_t)i * F, zs + (size_t)i * H, y, weight_set_of(hp, species[i]));
-        for (int m = 0; m < M; ++m) E_heads[(size_t)i * M + m] = w->scale[species[i]] * y[m] + w->shift[species[i]];
+        double ezbl = 0.0;  /* O-18: half of every pair's ZBL energy, all directed pairs of the centre */
+        if (hp->zbl_on)
+            for (int64_t p = off[i]; p < off[i + 1]; ++p) {
+                double d[3], e;
+                pair_vector(pos, L, i, pj[p], pn + 3 * p, d);
+                oracle_zbl_half(hp, w->atomic_number[species[i]], w->atomic_number[species[pj[p]]],
+                                sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]), &e, NULL);
+                ezbl += e;
+            }
+        for (int m = 0; m < M; ++m) E_heads[(size_t)i * M + m] = w->scale[species[i]] * y[m] + w->shift[species[i]] + ezbl;
     }
 }
 
@@ -725,10 +795,17 @@ static void backward_all(const oracle_hparams *hp, const oracle_weights *w, int6
         oracle_invariants_bwd(nr, P + (size_t)i * nr * NC, Gbar, Qloc);
         if (dG_out) memcpy(dG_out + (size_t)i * F, Gbar, sizeof(double) * F);
         if (Q_out) memcpy(Q_out + (size_t)i * nr * NC, Qloc, sizeof(double) * nr * NC);
+        double hw_sum = 0.0;  /* every head's energy carries the ZBL term once (O-18) */
+        for (int m = 0; m < M; ++m) hw_sum += head_w[m];
         for (int64_t p = off[i]; p < off[i + 1]; ++p) {
             double d[3];
             pair_vector(pos, L, i, pj[p], pn + 3 * p, d);
             pair_gradient(hp, w->beta, species[i], species[pj[p]], d, Qloc, gpair + 3 * p);
+            if (hp->zbl_on) {
+                double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]), e, de;
+                oracle_zbl_half(hp, w->atomic_number[species[i]], w->atomic_number[species[pj[p]]], r, &e, &de);
+                for (int a = 0; a < 3; ++a) gpair[3 * p + a] += hw_sum * de * d[a] / r;
+            }
             for (int a = 0; a < 3; ++a) Fout[3 * i + a] += gpair[3 * p + a];
         }
     }

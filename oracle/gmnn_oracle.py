@@ -37,13 +37,14 @@ class _HParams(C.Structure):
         ("n_species", C.c_int32), ("n_basis", C.c_int32), ("n_radial", C.c_int32),
         ("r_cut", C.c_double), ("r_min", C.c_double), ("gamma", C.c_double),
         ("n_hidden", C.c_int32), ("hidden", C.c_int32 * 4), ("n_heads", C.c_int32), ("n_weight_sets", C.c_int32),
+        ("basis_kind", C.c_int32), ("zbl_on", C.c_int32), ("zbl_r_max", C.c_double), ("zbl_scale", C.c_double),
     ]
 
 
 class _Weights(C.Structure):
     _fields_ = [
         ("beta", C.c_void_p), ("W", C.c_void_p * 5), ("b", C.c_void_p * 5),
-        ("scale", C.c_void_p), ("shift", C.c_void_p),
+        ("scale", C.c_void_p), ("shift", C.c_void_p), ("atomic_number", C.c_void_p),
     ]
 
 
@@ -142,6 +143,13 @@ class Model:
         # 1: one NN for all species (Eq. 4); n_species: W[l] is [S][fan_in][fan_out], b[l] is [S][fan_out] (O-5)
         self.n_weight_sets = int(getattr(spec, "n_weight_sets", 1))
         assert self.n_weight_sets in (1, int(spec.n_species))
+        # O-17: radial basis 0 Gaussians / 1 Bessel-like; O-18: ZBL repulsion with nuclear charges per species
+        self.basis_kind = int(getattr(spec, "basis_kind", 0))
+        self.zbl_on = int(bool(getattr(spec, "zbl", False)))
+        self.zbl_r_max = float(getattr(spec, "zbl_r_max", 0.0))
+        self.zbl_scale = float(getattr(spec, "zbl_scale", 1.0))
+        zn = getattr(spec, "atomic_numbers", None)
+        self.atomic_numbers = _f64(zn if zn is not None else np.zeros(self.n_species))
         self.beta = _f64(spec.beta)
         self.W = [_f64(w) for w in spec.W]
         self.b = [_f64(b) for b in spec.b]
@@ -160,6 +168,8 @@ class Model:
             self.hp.hidden[l] = h
         self.hp.n_heads = self.n_heads
         self.hp.n_weight_sets = self.n_weight_sets
+        self.hp.basis_kind, self.hp.zbl_on = self.basis_kind, self.zbl_on
+        self.hp.zbl_r_max, self.hp.zbl_scale = self.zbl_r_max, self.zbl_scale
         self.w = _Weights()
         self.w.beta = _p(self.beta)
         for l in range(len(self.W)):
@@ -167,6 +177,7 @@ class Model:
             self.w.b[l] = self.b[l].ctypes.data
         self.w.scale = _p(self.scale)
         self.w.shift = _p(self.shift)
+        self.w.atomic_number = _p(self.atomic_numbers)
 
 
 @dataclass
@@ -222,6 +233,21 @@ def radial(model: Model, zi: int, zj: int, r: float):
     dR = np.zeros(model.n_radial)
     lib().oracle_radial(C.byref(model.hp), _p(model.beta), C.c_int(zi), C.c_int(zj), C.c_double(r), _p(R), _p(dR))
     return R, dR
+
+
+def basis(model: Model, r: float):
+    """O-2 / O-17: the raw basis functions of one distance and their derivatives, without the cutoff function."""
+    phi = np.zeros(model.n_basis)
+    dphi = np.zeros(model.n_basis)
+    lib().oracle_basis(C.byref(model.hp), C.c_double(r), _p(phi), _p(dphi))
+    return phi, dphi
+
+
+def zbl_half(model: Model, z1: float, z2: float, r: float):
+    """O-18: (V/2, d(V/2)/dr) of the ZBL repulsion for one directed pair."""
+    e, de = C.c_double(0), C.c_double(0)
+    lib().oracle_zbl_half(C.byref(model.hp), C.c_double(z1), C.c_double(z2), C.c_double(r), C.byref(e), C.byref(de))
+    return float(e.value), float(de.value)
 
 
 def invariants(n_radial: int, P) -> np.ndarray:

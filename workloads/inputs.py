@@ -93,6 +93,11 @@ class ModelSpec:
     scale: np.ndarray  # [S] f32  sigma_Z
     shift: np.ndarray  # [S] f32  mu_Z
     n_weight_sets: int = 1  # n_species: one NN per species, W[l] is [S][fan_in][fan_out], b[l] is [S][fan_out]
+    basis_kind: int = 0  # 0 equidistant Gaussians, 1 Bessel-like functions of Kocer et al.
+    zbl: bool = False  # add the ZBL repulsion
+    zbl_r_max: float = 0.0  # Ang
+    zbl_scale: float = 1.0
+    atomic_numbers: "np.ndarray | None" = None  # [S] f32 nuclear charges for the ZBL term
 
     @property
     def n_features(self) -> int:
