@@ -85,6 +85,14 @@ typedef struct {
                               species ("the per-species atomic MLP"): atom i uses the (W, b) of set Z_i       */
     int32_t mlp_precision; /* gmnn_mlp_precision                                                   */
     int32_t force_mode;    /* gmnn_force_mode                                                      */
+    int32_t radial_basis;  /* 0: equidistant Gaussians; 1: the non-orthogonal Bessel-like functions of Kocer et
+                              al. (reading R30; r_min and gauss_gamma are then unused):
+                              f_n(r) = (-1)^n sqrt(2) pi / r_cut^1.5 (n+1)(n+2) / sqrt((n+1)^2 + (n+2)^2)
+                                       [sinc((n+1) pi r / r_cut) + sinc((n+2) pi r / r_cut)], n = 0 .. n_basis-1 */
+    int32_t zbl;           /* 1: add the Ziegler-Littmark-Biersack repulsion (reading R31) per pair,
+                              V = zbl_scale k_e Z1 Z2 / r phi(r / a) 1/2 [1 + cos(pi r / zbl_r_max)], r < zbl_r_max */
+    float zbl_r_max;       /* Ang, 0 < zbl_r_max <= r_cut                                          */
+    float zbl_scale;       /* dimensionless                                                        */
 } gmnn_hparams;
 
 typedef struct {            /* HOST pointers, row-major, caller-owned, copied by gmnn_create       */
@@ -94,6 +102,7 @@ typedef struct {            /* HOST pointers, row-major, caller-owned, copied by
     const float *b[5];      /* layer l: [n_weight_sets][fan_out]                                   */
     const float *scale;     /* [S] sigma_Z                                                         */
     const float *shift;     /* [S] mu_Z                                                            */
+    const float *atomic_numbers; /* [S] nuclear charges for the ZBL term; may be NULL when zbl == 0 */
 } gmnn_weights;
 
 /* Number of invariants G_i for n_radial channels (360 at 5), blocks 0-7. */

@@ -48,12 +48,13 @@ class _HParams(C.Structure):
         ("r_cut", C.c_float), ("r_min", C.c_float), ("gauss_gamma", C.c_float),
         ("n_hidden", C.c_int32), ("hidden", C.c_int32 * 4), ("n_heads", C.c_int32),
         ("n_weight_sets", C.c_int32), ("mlp_precision", C.c_int32), ("force_mode", C.c_int32),
+        ("radial_basis", C.c_int32), ("zbl", C.c_int32), ("zbl_r_max", C.c_float), ("zbl_scale", C.c_float),
     ]
 
 
 class _Weights(C.Structure):
     _fields_ = [("beta", C.c_void_p), ("W", C.c_void_p * 5), ("b", C.c_void_p * 5),
-                ("scale", C.c_void_p), ("shift", C.c_void_p)]
+                ("scale", C.c_void_p), ("shift", C.c_void_p), ("atomic_numbers", C.c_void_p)]
 
 
 def _load() -> C.CDLL:
@@ -161,10 +162,17 @@ class Model:
             hp.hidden[l] = int(h)
         hp.n_heads = spec.n_heads
         hp.n_weight_sets, hp.mlp_precision, hp.force_mode = n_weight_sets, mlp_precision, force_mode
+        hp.radial_basis = int(getattr(spec, "basis_kind", 0))  # 0 Gaussians, 1 Bessel-like
+        hp.zbl = int(bool(getattr(spec, "zbl", False)))  # ZBL repulsion
+        hp.zbl_r_max, hp.zbl_scale = float(getattr(spec, "zbl_r_max", 0.0)), float(getattr(spec, "zbl_scale", 1.0))
         self._keep = [np.ascontiguousarray(spec.beta, np.float32), np.ascontiguousarray(spec.scale, np.float32),
                       np.ascontiguousarray(spec.shift, np.float32)]
         w = _Weights()
         w.beta, w.scale, w.shift = (a.ctypes.data for a in self._keep)
+        if getattr(spec, "atomic_numbers", None) is not None:
+            zn = np.ascontiguousarray(spec.atomic_numbers, np.float32)
+            self._keep.append(zn)
+            w.atomic_numbers = zn.ctypes.data
         for l in range(min(len(spec.W), 5)):
             Wl = np.ascontiguousarray(spec.W[l], np.float32)
             bl = np.ascontiguousarray(spec.b[l], np.float32)

@@ -14,8 +14,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 # GMNN_B200_LIB: build to / load from another path (e.g. a -DGMNN_EXPERIMENTS build kept beside the shipped one)
 LIB = os.environ.get("GMNN_B200_LIB") or os.path.join(HERE, "libgmnn_b200.so")
-SOURCES = ["gmnn_api.cu", "neighbor.cu", "descriptor.cu", "mlp_simt.cu", "mlp_tc.cu", "md.cu"]
-HEADERS = ["gmnn_internal.h", "contraction.cuh", "tc_ptx.cuh", os.path.join("..", "..", "include", "gmnn.h")]
+SOURCES = ["gmnn_api.cu", "neighbor.cu", "descriptor.cu", "pair_forward.cu", "pair_backward.cu", "mlp_simt.cu", "mlp_tc.cu", "md.cu"]
+HEADERS = ["gmnn_internal.h", "contraction.cuh", "pair_common.cuh", "tc_ptx.cuh", os.path.join("..", "..", "include", "gmnn.h")]
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
     "-Xcompiler", "-fPIC", "-cudart", "static", "--expt-relaxed-constexpr",

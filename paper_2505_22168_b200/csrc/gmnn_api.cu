@@ -193,6 +193,21 @@ int gmnn_create(const gmnn_hparams *hp, const gmnn_weights *w, gmnn_model **out)
         set_error("kernels are instantiated for n_radial = 5, n_basis = 7 (got %d, %d)", hp->n_radial, hp->n_basis);
         return GMNN_UNSUPPORTED;
     }
+    if (hp->radial_basis != 0 && hp->radial_basis != 1) {
+        set_error("radial_basis must be 0 (Gaussians) or 1 (Bessel-like)");
+        return GMNN_INVALID_ARG;
+    }
+    if (hp->zbl != 0) {
+        if (!w->atomic_numbers || !(hp->zbl_r_max > 0.f) || !(hp->zbl_r_max <= hp->r_cut) || !std::isfinite(hp->zbl_scale)) {
+            set_error("zbl needs atomic_numbers, 0 < zbl_r_max <= r_cut and a finite zbl_scale");
+            return GMNN_INVALID_ARG;
+        }
+        for (int z = 0; z < hp->n_species; ++z)
+            if (!(w->atomic_numbers[z] >= 1.f) || !(w->atomic_numbers[z] <= 120.f)) {
+                set_error("atomic_numbers[%d] = %g is not a nuclear charge", z, w->atomic_numbers[z]);
+                return GMNN_INVALID_ARG;
+            }
+    }
     if (hp->n_weight_sets != 1 && hp->n_weight_sets != hp->n_species) {
         set_error("n_weight_sets = %d: must be 1 (one NN for all species) or n_species = %d (one NN per species)",
                   hp->n_weight_sets, hp->n_species);
@@ -240,6 +255,20 @@ int gmnn_create(const gmnn_hparams *hp, const gmnn_weights *w, gmnn_model **out)
     rp.r_min = hp->r_min;
     rp.delta = (hp->r_cut - hp->r_min) / (float)(hp->n_basis - 1);
     rp.gamma = hp->gauss_gamma > 0.f ? hp->gauss_gamma : 1.f / (2.f * rp.delta * rp.delta);
+    rp.basis_kind = hp->radial_basis;
+    for (int n = 0; n < hp->n_basis; ++n)
+        rp.bessel_c[n] = (float)(((n & 1) ? -1.0 : 1.0) * std::sqrt(2.0) * M_PI / std::pow((double)hp->r_cut, 1.5) * (n + 1.0) *
+                                 (n + 2.0) / std::sqrt((n + 1.0) * (n + 1.0) + (n + 2.0) * (n + 2.0)));
+    rp.zbl_on = hp->zbl != 0;
+    if (rp.zbl_on) {
+        rp.zbl_r_max2 = hp->zbl_r_max * hp->zbl_r_max;
+        rp.zbl_inv_rmax = 1.f / hp->zbl_r_max;
+        rp.zbl_pref = (float)(0.5 * (double)hp->zbl_scale * 14.399645);
+        for (int z = 0; z < hp->n_species; ++z) {
+            rp.zbl_z[z] = w->atomic_numbers[z];
+            rp.zbl_zpow[z] = (float)std::pow((double)w->atomic_numbers[z], 0.23);
+        }
+    }
     int rc = GMNN_OK;
     {
         const int S = hp->n_species, nr = hp->n_radial, nb = hp->n_basis;
@@ -398,6 +427,7 @@ int gmnn_system_create(const gmnn_model *m, int64_t n_atoms, const int32_t *spec
     A_(s->partial, 2 * 1024);
     A_(s->e_total, 6);  // epot, ekin, sigma_E, bits of sigma_F,max (switching-mode samples)
     A_(s->flags, FLAG_WORDS);
+    if (m->rp.zbl_on) A_(s->e_zbl, N);
     if (T > 1) {
         A_(s->mrow, N);
         A_(s->row_atom, R);
@@ -427,7 +457,7 @@ int gmnn_system_create(const gmnn_model *m, int64_t n_atoms, const int32_t *spec
 
 void gmnn_system_destroy(gmnn_system *s) {
     if (!s) return;
-    dev_free(s->mrow); dev_free(s->row_atom); dev_free(s->sp_count); dev_free(s->vir_atom);
+    dev_free(s->mrow); dev_free(s->row_atom); dev_free(s->sp_count); dev_free(s->vir_atom); dev_free(s->e_zbl);
     dev_free(s->species); dev_free(s->cell_of); dev_free(s->cell_count); dev_free(s->cell_start);
     dev_free(s->cell_fill); dev_free(s->slot_tmp); dev_free(s->perm); dev_free(s->pos4); dev_free(s->xref);
     dev_free(s->nbr); dev_free(s->rev); dev_free(s->gbuf); dev_free(s->runs); dev_free(s->count); dev_free(s->psi); dev_free(s->G); dev_free(s->dG); dev_free(s->A);

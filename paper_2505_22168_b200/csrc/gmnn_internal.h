@@ -78,6 +78,11 @@ __device__ __forceinline__ float lattice_shift(const Geometry &g, int x, float n
 struct RadialParams {  // passed by value to the pair kernels
     int n_species, n_basis, kb;  // kb = n_basis rounded up to 4 (row pitch of the beta table)
     float r_cut, r_cut2, inv_rc, r_min, delta, gamma;
+    int basis_kind;              // 0 Gaussians, 1 Bessel-like (hparams.radial_basis)
+    float bessel_c[MAX_BASIS];   // (-1)^n sqrt(2) pi / r_cut^1.5 (n+1)(n+2) / sqrt((n+1)^2 + (n+2)^2)
+    int zbl_on;                  // ZBL repulsion (hparams.zbl)
+    float zbl_r_max2, zbl_inv_rmax, zbl_pref;  // r_max^2, 1 / r_max, 1/2 zbl_scale k_e
+    float zbl_z[MAX_SPECIES], zbl_zpow[MAX_SPECIES];  // Z and Z^0.23 per species
 };
 
 }  // namespace gmnn
@@ -176,6 +181,7 @@ struct gmnn_system {
     float *e_heads = nullptr;        // [N][n_heads]
     float *vir_atom = nullptr;       // [9][N] per-atom virial terms -sum_j d_a g_b (lazy; gmnn_energy_forces_virial)
     bool want_virial = false;        // this evaluation's pair backward also leaves vir_atom
+    float *e_zbl = nullptr;          // [N] internal order: sum over the centre's pairs of V_ZBL / 2 (models with zbl)
     float *e_atom = nullptr;         // [N]
     float *f_int = nullptr;          // [N][3]
     float *f_tmp = nullptr;          // [N][3] caller order (ensemble, MD)

@@ -135,13 +135,14 @@ __global__ void __launch_bounds__(128)
 k_heads(int64_t row0, int64_t rows, const float *__restrict__ Ht, int Hd, const float *__restrict__ Wl,
         const float *__restrict__ bl, int M, const float4 *__restrict__ pos4, const float *__restrict__ scale,
         const float *__restrict__ shift, const float *__restrict__ head_w, float *__restrict__ e_heads,
-        float *__restrict__ e_atom, const int32_t *__restrict__ row_atom) {
+        float *__restrict__ e_atom, const int32_t *__restrict__ row_atom, const float *__restrict__ e_zbl) {
     const int64_t r = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;  // blockDim.x == 128 == tile
     if (r >= rows) return;
     const int64_t i = row_atom ? (int64_t)row_atom[row0 + r] : row0 + r;
     const float *h = Ht + (int64_t)blockIdx.x * Hd * 128 + threadIdx.x;
     const int z = __float_as_int(pos4[i].w);
-    const float sg = __ldg(&scale[z]), mu = __ldg(&shift[z]);
+    // ZBL (an empirical correction outside the network): every head's energy carries it once
+    const float sg = __ldg(&scale[z]), mu = __ldg(&shift[z]) + (e_zbl ? __ldg(&e_zbl[i]) : 0.f);
     float e = 0.f;
     for (int m0 = 0; m0 < M; m0 += 8) {
         float p[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
@@ -215,14 +216,14 @@ __global__ void k_heads_finish(int64_t row0, int64_t rows, const float *__restri
                                const float *__restrict__ bl, const float4 *__restrict__ pos4,
                                const float *__restrict__ scale, const float *__restrict__ shift,
                                const float *__restrict__ head_w, float *__restrict__ e_heads, float *__restrict__ e_atom,
-                               const int32_t *__restrict__ row_atom) {
+                               const int32_t *__restrict__ row_atom, const float *__restrict__ e_zbl) {
     const int64_t r = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (r >= rows) return;
     float y = 0.f;
     for (int q = 0; q < n_slots; ++q) y += __ldg(ypart + q * m_pad + row0 + r);
     const int64_t i = row_atom ? (int64_t)row_atom[row0 + r] : row0 + r;
     const int z = __float_as_int(pos4[i].w);
-    const float em = __ldg(&scale[z]) * (y + __ldg(&bl[0])) + __ldg(&shift[z]);
+    const float em = __ldg(&scale[z]) * (y + __ldg(&bl[0])) + (__ldg(&shift[z]) + (e_zbl ? __ldg(&e_zbl[i]) : 0.f));
     if (e_heads) {
         e_heads[i] = em;
         e_atom[i] = __ldg(&head_w[0]) * em;
@@ -248,11 +249,11 @@ int launch_mlp_heads(gmnn_system *s, const float *head_w_dev, cudaStream_t st) {
             k_heads_finish<<<(unsigned)((real + 255) / 256), 256, 0, st>>>(
                 r0, real, s->ypart, s->head_slots, (s->n_rows + 127) / 128 * 128,
                 mean ? m->w_mean + (size_t)t * (Hd + 1) + Hd : m->b[L] + (size_t)t * M, s->pos4, m->scale, m->shift,
-                head_w_dev, mean ? nullptr : s->e_heads, s->e_atom, s->row_atom);
+                head_w_dev, mean ? nullptr : s->e_heads, s->e_atom, s->row_atom, s->e_zbl);
         } else {
             k_heads<<<(unsigned)((real + 127) / 128), 128, 0, st>>>(
                 r0, real, tile_rows(s->H[L - 1], r0, Hd), Hd, m->W[L] + t * m->wsize(L), m->b[L] + (size_t)t * M, M, s->pos4,
-                m->scale, m->shift, head_w_dev, s->e_heads, s->e_atom, s->row_atom);
+                m->scale, m->shift, head_w_dev, s->e_heads, s->e_atom, s->row_atom, s->e_zbl);
         }
         GMNN_LAUNCHED();
     }
