@@ -262,6 +262,15 @@ int gmnn_system_get_nose_hoover(gmnn_system *s, double *xi /*HOST*/, double *p_x
  *   temperature_K <= 0 switches it off; gamma_per_fs >= 0.  Not together with a Nose-Hoover chain. */
 int gmnn_system_set_langevin(gmnn_system *s, float temperature_K, float gamma_per_fs, uint64_t seed, uint64_t first_step);
 
+/* Temperature schedule for whichever thermostat is set ("temperature profiles
+ * oscillating between 300 K and 600 K"; reading R32): the target of MD step n (0-based, counted on the device
+ * from this call on, over both MD entries) is piecewise linear through the points (steps[k], temperatures_K[k]), constant
+ * before the first and after the last.  Both chain half steps of a Nose-Hoover step and the noise of a Langevin step take
+ * T(n); the chain masses Q stay those of gmnn_system_set_nose_hoover's temperature.  HOST arrays, 1 <= n_points <= 64,
+ * steps strictly ascending from >= 0; n_points = 0 removes the schedule.  The step still replays as a CUDA graph. */
+int gmnn_system_set_temperature_schedule(gmnn_system *s, int32_t n_points, const int64_t *steps /*HOST*/,
+                                         const float *temperatures_K /*HOST*/);
+
 /* Uncertainty-driven-dynamics bias (Eq. 9) on a model with several
  * heads:  E_b = A [exp(-sigma_E^2 / (N_ens N_atoms B^2)) - 1],  sigma_E^2 = 1/N_ens sum_m (E^(m) - mean)^2 of the
  * heads' TOTAL energies (Eq. 5).  While A != 0, gmnn_energy_forces, gmnn_energy_forces_host, gmnn_md_verlet_steps and

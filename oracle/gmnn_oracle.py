@@ -539,12 +539,25 @@ def nhc_half_step(ke2: float, xi: np.ndarray, pxi: np.ndarray, Q: np.ndarray, do
     return scale
 
 
+def schedule_temperature(schedule, n: int, default: float) -> float:
+    """O-19: the thermostat's target at MD step n (0-based, counted from where the schedule was set) of a temperature
+    schedule (steps [k] ascending, temps [k] in K): piecewise linear between the points, constant before the first and
+    after the last ("temperature profiles oscillating between 300 K and 600 K"; reading R32).
+    schedule None: the constant `default`."""
+    if schedule is None:
+        return float(default)
+    steps, temps = schedule
+    return float(np.interp(float(n), np.asarray(steps, np.float64), np.asarray(temps, np.float64)))
+
+
 def nvt_nose_hoover(model: Model, positions, velocities, masses, species, cell, pbc, dt_fs: float, n_steps: int,
-                    temperature: float, tau_fs: float, chain_length: int = 3, chain_steps: int = 2, sy_steps: int = 3):
+                    temperature: float, tau_fs: float, chain_length: int = 3, chain_steps: int = 2, sy_steps: int = 3,
+                    schedule=None):
     """O-14: NVT with a Nose-Hoover chain: chain half step, velocity Verlet (O-11) on the mean
     energy, chain half step.  Q_0 = dof kT tau^2, Q_k = kT tau^2, dof = 3 N (reading R28).  Fresh list of radius
     r_cut every step.  Returns x, v, epot, ekin, conserved (all [n_steps + 1]; conserved = epot + ekin +
-    sum pxi^2 / 2Q + dof kT xi_0 + kT sum_{k>0} xi_k)."""
+    sum pxi^2 / 2Q + dof kT xi_0 + kT sum_{k>0} xi_k).  With a `schedule` (O-19) both chain half steps of MD step n
+    take kT = k_B T(n); the thermostat masses Q stay those of `temperature` (reading R32)."""
     ACC = 9.648533212e-3
     x = _f64(positions).copy()
     v = _f64(velocities).copy()
@@ -571,7 +584,8 @@ def nvt_nose_hoover(model: Model, positions, velocities, masses, species, cell, 
     x = wrap(x)
     r = evaluate(x)
     epot, ekin, cons = [r.energy], [0.5 * ke2()], [conserved(r.energy)]
-    for _ in range(n_steps):
+    for n in range(n_steps):
+        kT = KB_EV * schedule_temperature(schedule, n, temperature)
         v *= nhc_half_step(ke2(), xi, pxi, Q, dof, kT, dt_fs, chain_steps, sy_steps)
         v += 0.5 * dt_fs * r.forces / m * ACC
         x = wrap(x + dt_fs * v)
@@ -606,10 +620,11 @@ def langevin_normals(seed: int, step: int, n_atoms: int) -> np.ndarray:
 
 
 def nvt_langevin(model: Model, positions, velocities, masses, species, cell, pbc, dt_fs: float, n_steps: int,
-                 temperature: float, gamma_per_fs: float, seed: int, first_step: int = 0):
+                 temperature: float, gamma_per_fs: float, seed: int, first_step: int = 0, schedule=None):
     """O-15: Langevin dynamics ("Langevin thermostat") in the BAOAB splitting (reading R29):
     v += dt/2 a;  x += dt/2 v;  v = c1 v + sqrt(kT (1 - c1^2) / m) xi, c1 = exp(-gamma dt);  x += dt/2 v;
-    forces;  v += dt/2 a.  Fresh list of radius r_cut every step.  Returns x, v, epot, ekin ([n_steps + 1])."""
+    forces;  v += dt/2 a.  Fresh list of radius r_cut every step.  Returns x, v, epot, ekin ([n_steps + 1]).
+    With a `schedule` (O-19) the noise of MD step n takes kT = k_B T(n)."""
     ACC = 9.648533212e-3
     x = _f64(positions).copy()
     v = _f64(velocities).copy()
@@ -617,7 +632,6 @@ def nvt_langevin(model: Model, positions, velocities, masses, species, cell, pbc
     N = x.shape[0]
     kT = KB_EV * temperature
     c1 = np.exp(-gamma_per_fs * dt_fs)
-    c2 = np.sqrt(kT * (1.0 - c1 * c1) / m * ACC)  # Ang/fs
 
     def wrap(y):
         return wrap_positions(y, cell, pbc)
@@ -632,6 +646,8 @@ def nvt_langevin(model: Model, positions, velocities, masses, species, cell, pbc
     for t in range(n_steps):
         v += 0.5 * dt_fs * r.forces / m * ACC
         x = x + 0.5 * dt_fs * v
+        kT = KB_EV * schedule_temperature(schedule, t, temperature)
+        c2 = np.sqrt(kT * (1.0 - c1 * c1) / m * ACC)  # Ang/fs
         v = c1 * v + c2 * langevin_normals(seed, first_step + t, N)
         x = wrap(x + 0.5 * dt_fs * v)
         r = evaluate(x)

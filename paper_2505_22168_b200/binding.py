@@ -31,7 +31,7 @@ GMNN_FORCE_GATHER, GMNN_FORCE_PAIRBUF = 0, 1
 EXPORTS = (
     "gmnn_n_features", "gmnn_create", "gmnn_destroy", "gmnn_system_create", "gmnn_system_destroy",
     "gmnn_system_set_int", "gmnn_system_get_int", "gmnn_build_neighbors", "gmnn_get_neighbors", "gmnn_get_neighbor_rows",
-    "gmnn_energy_forces", "gmnn_energy_forces_virial", "gmnn_energy_forces_host", "gmnn_ensemble_energy_forces", "gmnn_md_verlet_steps", "gmnn_md_ensemble_steps", "gmnn_system_set_langevin", "gmnn_system_set_nose_hoover", "gmnn_system_get_nose_hoover", "gmnn_system_set_udd_bias", "gmnn_system_get_udd_bias",
+    "gmnn_energy_forces", "gmnn_energy_forces_virial", "gmnn_energy_forces_host", "gmnn_ensemble_energy_forces", "gmnn_md_verlet_steps", "gmnn_md_ensemble_steps", "gmnn_system_set_langevin", "gmnn_system_set_temperature_schedule", "gmnn_system_set_nose_hoover", "gmnn_system_get_nose_hoover", "gmnn_system_set_udd_bias", "gmnn_system_get_udd_bias",
     "gmnn_check", "gmnn_stage_times", "gmnn_debug_read", "gmnn_launch_count", "gmnn_last_error",
 )
 
@@ -82,6 +82,7 @@ def _load() -> C.CDLL:
     lib.gmnn_system_set_nose_hoover.argtypes = [C.c_void_p, C.c_float, C.c_float, C.c_int32, C.c_int32, C.c_int32]
     lib.gmnn_system_get_nose_hoover.argtypes = [C.c_void_p] * 5
     lib.gmnn_system_set_udd_bias.argtypes = [C.c_void_p, C.c_float, C.c_float]
+    lib.gmnn_system_set_temperature_schedule.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]
     lib.gmnn_system_get_udd_bias.argtypes = [C.c_void_p] * 4
     lib.gmnn_energy_forces.argtypes = [C.c_void_p] * 6
     lib.gmnn_energy_forces_host.argtypes = [C.c_void_p] * 6
@@ -382,6 +383,13 @@ class System:
         """Langevin (BAOAB) for the MD entries (temperature_K <= 0: off)."""
         _check(lib.gmnn_system_set_langevin(self.handle, C.c_float(temperature_K), C.c_float(gamma_per_fs),
                                             C.c_uint64(seed), C.c_uint64(first_step)))
+
+    def set_temperature_schedule(self, steps=(), temperatures_K=()) -> None:
+        """Piecewise-linear target temperature over the MD step count for the thermostat that is set (empty: none)."""
+        st = np.ascontiguousarray(np.asarray(steps), np.int64)
+        tk = np.ascontiguousarray(np.asarray(temperatures_K), np.float32)
+        assert st.shape == tk.shape and st.ndim == 1
+        _check(lib.gmnn_system_set_temperature_schedule(self.handle, C.c_int32(st.shape[0]), _np_ptr(st), _np_ptr(tk)))
 
     def set_udd_bias(self, A: float, B: float = 1.0) -> None:
         _check(lib.gmnn_system_set_udd_bias(self.handle, C.c_float(A), C.c_float(B)))

@@ -465,6 +465,7 @@ void gmnn_system_destroy(gmnn_system *s) {
     dev_free(s->dZ[0]); dev_free(s->dZ[1]); dev_free(s->Bv); dev_free(s->BvT); dev_free(s->BvTs); dev_free(s->BvTh); dev_free(s->amax); dev_free(s->vhead); dev_free(s->head_w);
     dev_free(s->ypart); dev_free(s->e_heads); dev_free(s->e_atom); dev_free(s->f_int); dev_free(s->f_tmp); dev_free(s->partial);
     dev_free(s->e_total); dev_free(s->flags); dev_free(s->ens_scratch); dev_free(s->nhc); dev_free(s->lang_step);
+    dev_free(s->kT_now); dev_free(s->sched_steps); dev_free(s->sched_temps); dev_free(s->sched_step);
     dev_free(s->stage_pos); dev_free(s->stage_f); dev_free(s->stage_e);
     if (s->flags_host) cudaFreeHost(s->flags_host);
     for (cudaEvent_t e : s->events) cudaEventDestroy(e);
@@ -950,6 +951,8 @@ int gmnn_md_verlet_steps(gmnn_system *s, float *positions, float *velocities, co
     // through a device-side counter), so the body can be captured once and replayed as a CUDA graph.
     auto md_step = [&](cudaStream_t q) -> int {
         int r;
+        // temperature schedule: this step's target for whichever thermostat is set
+        if (s->sched_n > 0 && (s->nhc_len > 0 || s->lang_on) && (r = launch_schedule_eval(s, q))) return r;
         // NVT: chain operator for dt/2 before and after the velocity-Verlet step
         if (s->nhc_len > 0 && (r = launch_nhc_half(s, velocities, ek, dt_fs, q))) return r;
         if (s->lang_on) {  // Langevin: B A O A in one pass (the closing B is the kick below)
@@ -1134,6 +1137,8 @@ int gmnn_system_set_nose_hoover(gmnn_system *s, float temperature_K, float tau_f
     for (int k = chain_length; k < 8; ++k) h[16 + k] = 1.0;
     h[24] = 1.0;
     GMNN_CUDA(cudaMemcpy(s->nhc, h, sizeof(h), cudaMemcpyHostToDevice));
+    if (!s->kT_now && (rc = dev_alloc(&s->kT_now, (size_t)1))) return rc;
+    GMNN_CUDA(cudaMemcpy(s->kT_now, &kT, sizeof(double), cudaMemcpyHostToDevice));
     s->nhc_len = chain_length;
     s->nhc_chain_steps = chain_steps;
     s->nhc_sy_steps = sy_steps;
@@ -1176,8 +1181,44 @@ int gmnn_system_set_langevin(gmnn_system *s, float temperature_K, float gamma_pe
     GMNN_CUDA(cudaMemcpy(s->lang_step, &first_step, sizeof(uint64_t), cudaMemcpyHostToDevice));
     s->lang_gamma = (double)gamma_per_fs;
     s->lang_kT = 8.617333262e-5 * (double)temperature_K;
+    if (!s->kT_now && (rc = dev_alloc(&s->kT_now, (size_t)1))) return rc;
+    GMNN_CUDA(cudaMemcpy(s->kT_now, &s->lang_kT, sizeof(double), cudaMemcpyHostToDevice));
     s->lang_seed = seed;
     s->lang_on = true;
+    return GMNN_OK;
+}
+
+int gmnn_system_set_temperature_schedule(gmnn_system *s, int32_t n_points, const int64_t *steps, const float *temperatures_K) {
+    if (!s || n_points < 0 || n_points > 64 || (n_points > 0 && (!steps || !temperatures_K))) {
+        set_error("gmnn_system_set_temperature_schedule: 0 <= n_points <= 64 and non-null arrays");
+        return GMNN_INVALID_ARG;
+    }
+    for (int k = 0; k < n_points; ++k)
+        if (steps[k] < 0 || (k > 0 && steps[k] <= steps[k - 1]) || !(temperatures_K[k] > 0.f) || !std::isfinite(temperatures_K[k])) {
+            set_error("temperature schedule: steps must ascend strictly from >= 0, temperatures must be positive");
+            return GMNN_INVALID_ARG;
+        }
+    s->md_state_valid = false;
+    s->sched_n = 0;
+    if (n_points == 0) {  // back to the constant target of the thermostat that is set
+        if (s->kT_now) {
+            const double kT = s->lang_on ? s->lang_kT : s->nhc_kT;
+            GMNN_CUDA(cudaMemcpy(s->kT_now, &kT, sizeof(double), cudaMemcpyHostToDevice));
+        }
+        return GMNN_OK;
+    }
+    int rc;
+    if (!s->sched_steps) {
+        if ((rc = dev_alloc(&s->sched_steps, (size_t)64))) return rc;
+        if ((rc = dev_alloc(&s->sched_temps, (size_t)64))) return rc;
+        if ((rc = dev_alloc(&s->sched_step, (size_t)1))) return rc;
+    }
+    if (!s->kT_now && (rc = dev_alloc(&s->kT_now, (size_t)1))) return rc;
+    const uint64_t zero = 0;
+    GMNN_CUDA(cudaMemcpy(s->sched_steps, steps, sizeof(int64_t) * n_points, cudaMemcpyHostToDevice));
+    GMNN_CUDA(cudaMemcpy(s->sched_temps, temperatures_K, sizeof(float) * n_points, cudaMemcpyHostToDevice));
+    GMNN_CUDA(cudaMemcpy(s->sched_step, &zero, sizeof(uint64_t), cudaMemcpyHostToDevice));
+    s->sched_n = n_points;
     return GMNN_OK;
 }
 

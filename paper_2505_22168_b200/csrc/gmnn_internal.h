@@ -169,6 +169,13 @@ struct gmnn_system {
     double *nhc = nullptr;           // [26] Nose-Hoover chain: xi[8], p_xi[8], Q[8], scale, thermostat energy (lazy)
     int nhc_len = 0, nhc_chain_steps = 2, nhc_sy_steps = 3;  // nhc_len == 0: NVE
     double nhc_kT = 0.0;
+    // thermostat target: both thermostats read k_B T (eV) from the device scalar kT_now; a temperature schedule
+    // (piecewise linear in the MD step, gmnn_system_set_temperature_schedule) rewrites it at the start of every step
+    double *kT_now = nullptr;        // device [1] (lazy)
+    int sched_n = 0;                 // points of the schedule (0: constant target)
+    int64_t *sched_steps = nullptr;  // device [sched_n]
+    float *sched_temps = nullptr;    // device [sched_n] (K)
+    uint64_t *sched_step = nullptr;  // device: MD steps since the schedule was set
     bool lang_on = false;            // Langevin (BAOAB) instead of the plain kick + drift
     double lang_gamma = 0.0, lang_kT = 0.0;  // 1/fs, eV
     uint64_t lang_seed = 0;
@@ -271,6 +278,7 @@ int launch_ensemble_energy_stats(gmnn_system *s, float *e_mean, float *e_var, cu
 int launch_finish_var(int64_t n, float *m2, int n_heads, cudaStream_t st);
 int launch_baoab(gmnn_system *s, float *x, float *v, const float *f, const float *m, float dt, cudaStream_t st);
 int launch_nhc_half(gmnn_system *s, float *v, double *ek, float dt, cudaStream_t st);
+int launch_schedule_eval(gmnn_system *s, cudaStream_t st);  // kT_now <- k_B T(step), step += 1
 int launch_udd_weights(gmnn_system *s, float *head_w_out, double *scal, cudaStream_t st);
 int launch_uncertainty_scalars(gmnn_system *s, const float *f_var, double *out_d, int32_t *out_bits, cudaStream_t st);
 

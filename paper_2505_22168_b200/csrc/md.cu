@@ -374,7 +374,9 @@ int launch_uncertainty_scalars(gmnn_system *s, const float *f_var, double *out_d
 // thermostatted step stays one replayable launch sequence: one thread, fp64, reads the kinetic energy the
 // last kick left in ek, updates (xi, p_xi), and leaves the velocity scale factor for k_scale_v.
 // st: [0, 8) xi, [8, 16) p_xi, [16, 24) Q, [24] scale factor, [25] thermostat energy
-__global__ void k_nhc_half(double *ek, double *st, int Mc, int chain_steps, int sy_steps, double dof, double kT, double dt) {
+__global__ void k_nhc_half(double *ek, double *st, int Mc, int chain_steps, int sy_steps, double dof,
+                           const double *__restrict__ kT_now, double dt) {
+    const double kT = *kT_now;  // the step's target (constant, or this step's value of the temperature schedule)
     double *xi = st, *pxi = st + 8;
     const double *Q = st + 16;
     double w[5];
@@ -425,7 +427,7 @@ __global__ void __launch_bounds__(256) k_scale_v(int64_t n3, float *v, const dou
 
 // chain operator for dt/2 on the kinetic energy in ek (updated), then v *= scale
 int launch_nhc_half(gmnn_system *s, float *v, double *ek, float dt, cudaStream_t st) {
-    k_nhc_half<<<1, 1, 0, st>>>(ek, s->nhc, s->nhc_len, s->nhc_chain_steps, s->nhc_sy_steps, 3.0 * (double)s->N, s->nhc_kT,
+    k_nhc_half<<<1, 1, 0, st>>>(ek, s->nhc, s->nhc_len, s->nhc_chain_steps, s->nhc_sy_steps, 3.0 * (double)s->N, s->kT_now,
                                 (double)dt);
     GMNN_LAUNCHED();
     k_scale_v<<<nblocks(3 * s->N, 256), 256, 0, st>>>(3 * s->N, v, s->nhc + 24);
@@ -447,10 +449,12 @@ __device__ __forceinline__ uint64_t splitmix64_at(uint64_t seed, uint64_t counte
 // oracle implements on its own), so the trajectory does not depend on the launch geometry or on replay.
 __global__ void __launch_bounds__(256)
 k_baoab(int64_t N, float *x, float *v, const float *__restrict__ f, const float *__restrict__ m, float dt, double c1,
-        double kT_acc, uint64_t seed, const uint64_t *__restrict__ step, const float *__restrict__ xref, int32_t *flags) {
+        const double *__restrict__ kT_now, uint64_t seed, const uint64_t *__restrict__ step, const float *__restrict__ xref,
+        int32_t *flags) {
     const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     float d2 = 0.f;
     if (i < N) {
+        const double kT_acc = *kT_now * ACC_CONV;  // the step's target temperature (see k_nhc_half)
         const uint64_t base = (*step * (uint64_t)N + (uint64_t)i) * 2ull;
         const uint64_t w0 = splitmix64_at(seed, base), w1 = splitmix64_at(seed, base + 1ull);
         const double two32 = 1.0 / 4294967296.0, twopi = 6.283185307179586476925286766559;
@@ -483,10 +487,37 @@ k_baoab(int64_t N, float *x, float *v, const float *__restrict__ f, const float 
 
 __global__ void k_inc_u64(uint64_t *p) { *p += 1ull; }
 
+// Temperature schedule (reading R32): k_B T of MD step *step, piecewise linear between
+// the points, constant before the first and after the last; then the step counter moves on.  One thread.
+__global__ void k_schedule_eval(int n, const int64_t *__restrict__ steps, const float *__restrict__ temps, uint64_t *step,
+                                double *kT_now) {
+    const double t = (double)*step;
+    double T = (double)temps[n - 1];
+    if (t <= (double)steps[0]) {
+        T = (double)temps[0];
+    } else {
+        for (int k = 1; k < n; ++k)
+            if (t <= (double)steps[k]) {
+                const double a = (t - (double)steps[k - 1]) / ((double)steps[k] - (double)steps[k - 1]);
+                T = (double)temps[k - 1] + a * ((double)temps[k] - (double)temps[k - 1]);
+                break;
+            }
+    }
+    *kT_now = 8.617333262e-5 * T;
+    *step += 1ull;
+}
+
+int launch_schedule_eval(gmnn_system *s, cudaStream_t st) {
+    k_schedule_eval<<<1, 1, 0, st>>>(s->sched_n, s->sched_steps, s->sched_temps, s->sched_step, s->kT_now);
+    GMNN_LAUNCHED();
+    GMNN_CUDA(cudaGetLastError());
+    return GMNN_OK;
+}
+
 int launch_baoab(gmnn_system *s, float *x, float *v, const float *f, const float *m, float dt, cudaStream_t st) {
     const double c1 = exp(-s->lang_gamma * (double)dt);
-    k_baoab<<<nblocks(s->N, 256), 256, 0, st>>>(s->N, x, v, f, m, dt, c1, s->lang_kT * ACC_CONV, s->lang_seed, s->lang_step,
-                                                 s->xref, s->flags);
+    k_baoab<<<nblocks(s->N, 256), 256, 0, st>>>(s->N, x, v, f, m, dt, c1, s->kT_now, s->lang_seed, s->lang_step, s->xref,
+                                                 s->flags);
     GMNN_LAUNCHED();
     k_inc_u64<<<1, 1, 0, st>>>(s->lang_step);
     GMNN_LAUNCHED();
