@@ -134,14 +134,13 @@ void gmnn_system_destroy(gmnn_system *s);
  *                     invalidates the neighbour list (call gmnn_build_neighbors again)
  *   "tc_pair"         1 (default): 3xTF32 GEMMs on CTA pairs (cta_group::2); 0: single CTAs (3xFP16: always pairs)
  *   "tc_split_bk"     16 | 32 (default): K extent of one pipeline stage of the 3xTF32 GEMM
- *   "tc_flush_k"      multiple of 16 (default 64): K extent after which the tensor-memory accumulator
- *                     is flushed into registers (the tensor core accumulates with truncation)
+ *   "tc_flush_k"      multiple of 16 (default 128): K extent after which the FORWARD GEMMs of the 3xTF32 / 3xFP16 modes
+ *                     drain the tensor-memory accumulator of the hi.hi products into registers (the tensor core
+ *                     accumulates with truncation; the forward GEMMs enter the energies)
+ *   "tc_flush_k_bwd"  the same for the BACKWARD GEMMs (default 256; they enter the forces only)
  *   "tc_h_bk"         32 | 64 (default): K extent of one pipeline stage of the 3xFP16 GEMM
- *   "tc_flush_head"   0..8 (default 0 = 2 for 3xTF32, 4 for 3xFP16): the first two accumulator chunks of a
- *                     tile of the BACKWARD GEMMs span this many flush intervals (more run-way for the
- *                     MMAs while the epilogue finishes the previous tile; touches forces only,
- *                     energies come from the forward GEMMs)
- *   "tc_flush_head_fwd" 1..8 (default 1): the same for the forward GEMMs (enters the energies)
+ *   "tc_prefetch"     0..64 (default 0: measured no gain): pipeline stages by which the CTA-pair GEMMs prefetch their activation boxes
+ *                     into L2 ahead of the loads (0: off)
  *   The tc_* knobs are process-wide.  (Builds with -DGMNN_EXPERIMENTS add "tc_debug" and "cb_halves", knock-out
  *   and superseded-variant switches for timing studies; the shipped library rejects them as unknown keys.)
  * Returns GMNN_INVALID_ARG for an unknown key or value. */

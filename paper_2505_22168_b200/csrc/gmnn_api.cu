@@ -23,7 +23,7 @@ void set_error(const char *fmt, ...) {
 }
 
 int launch_mlp_forward_tc(gmnn_system *s, cudaStream_t st);
-extern int g_tc_split_bk, g_tc_flush_k, g_tc_pair, g_tc_flush_head, g_tc_h_bk, g_tc_flush_head_fwd;
+extern int g_tc_split_bk, g_tc_flush_k, g_tc_flush_k_bwd, g_tc_pair, g_tc_h_bk, g_tc_prefetch;
 #ifdef GMNN_EXPERIMENTS
 extern int g_tc_debug, g_cb_halves;
 #endif
@@ -515,12 +515,12 @@ int gmnn_system_set_int(gmnn_system *s, const char *key, int64_t v) {
     } else if (!strcmp(key, "tc_debug")) {  // knock-out timing experiments (wrong results), see mlp_tc.cu
         gmnn::g_tc_debug = (int)v;
 #endif
-    } else if (!strcmp(key, "tc_flush_head")) {  // process-wide, see mlp_tc.cu
-        if (v < 0 || v > 8) return GMNN_INVALID_ARG;  // 0: automatic (2 on tf32, 4 on fp16)
-        gmnn::g_tc_flush_head = (int)v;
-    } else if (!strcmp(key, "tc_flush_head_fwd")) {
-        if (v < 1 || v > 8) return GMNN_INVALID_ARG;
-        gmnn::g_tc_flush_head_fwd = (int)v;
+    } else if (!strcmp(key, "tc_prefetch")) {  // process-wide, see mlp_tc.cu
+        if (v < 0 || v > 64) return GMNN_INVALID_ARG;
+        gmnn::g_tc_prefetch = (int)v;
+    } else if (!strcmp(key, "tc_flush_k_bwd")) {  // process-wide, see mlp_tc.cu
+        if (v < 16 || v > 4096 || v % 16) return GMNN_INVALID_ARG;
+        gmnn::g_tc_flush_k_bwd = (int)v;
     } else if (!strcmp(key, "tc_pair")) {  // process-wide: 3xTF32 GEMMs on CTA pairs (1) or single CTAs (0)
         gmnn::g_tc_pair = v != 0;
     } else if (!strcmp(key, "tc_h_bk")) {  // process-wide: K extent of a 3xFP16 stage

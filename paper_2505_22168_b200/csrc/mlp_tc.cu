@@ -84,7 +84,10 @@ struct TcArgs {
     int n_tiles;   // total
     int flush;     // pipeline stages per accumulator flush (K chunk = flush * BK)
     int flush1;    // ... of the first two chunks of a tile (>= flush)
-    int debug;     // -DGMNN_EXPERIMENTS builds only (results wrong): 1 skip split work, 2 hi.hi MMA only, 4 skip stores
+    int xy;        // CTA-pair kernels: 1 = cross terms and hi.hi terms in accumulators of their own (forward GEMMs), 0 = ping-pong
+    int prefetch;  // CTA-pair kernels: pipeline stages by which the L2 prefetch of the A boxes runs ahead of their loads
+    int debug;     // -DGMNN_EXPERIMENTS builds only (results wrong): 1 skip split work, 2 hi.hi MMA only, 4 skip the elementwise
+                   // and the stores, 8 skip the stores only, 16 skip the tensor-memory drains
     float *C;      // [M][N]
     float *C2;     // EPI_HIDDEN: swish'(z)
     const float *bias;
@@ -117,6 +120,25 @@ __device__ __forceinline__ void swish_pair_tc(float z, float &h, float &d) {
     const float s = __fdividef(1.f, 1.f + __expf(-z));  // ex2.approx + rcp.approx: ~2 ulp, no slow path
     h = z * s;
     d = s * (1.f + z * (1.f - s));
+}
+__device__ __forceinline__ float ex2_approx(float x) {
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ float rcp_approx(float x) {
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+// swish and swish' of z = a * zs from the raw accumulator a (which already carries the bias, see tc_init_acc):
+// t = a * (-zs log2 e) -> e^-z = ex2(t); s = 1 / (1 + e^-z); h = z s; d = s + h (1 - s) = fma(-h, s, s + h).
+// Eight issue slots and two MUFU per element (the final phase of a forward tile is bound by exactly these).
+__device__ __forceinline__ void swish_pair_acc(float a, float zs, float k1, float &h, float &d) {
+    const float z = a * zs;
+    const float s = rcp_approx(1.f + ex2_approx(a * k1));
+    h = z * s;
+    d = fmaf(-h, s, s + h);
 }
 
 // hi = tf32(x) (round to nearest) in place, lo = x - hi beside it, for `n4` float4 of one operand
@@ -181,6 +203,10 @@ __device__ __forceinline__ void tc_store_tile(const TcArgs &p, float (&acc)[4][3
                 for (int c = 0; c < TC_EB; ++c)
                     if (c < nc) {
                         ysum = fmaf(h[c], wh[c], ysum);
+                        if (TC_DBG(p) & 8) {
+                            tmax = fmaxf(tmax, d[c]);
+                            continue;
+                        }
                         C2out[o + c * TC_BM] = d[c];
                     }
             } else if (EPI == EPI_HIDDEN) {
@@ -191,6 +217,10 @@ __device__ __forceinline__ void tc_store_tile(const TcArgs &p, float (&acc)[4][3
 #pragma unroll
                 for (int c = 0; c < TC_EB; ++c)
                     if (c < nc) {
+                        if (TC_DBG(p) & 8) {  // knock-out: arithmetic without the stores
+                            tmax = fmaxf(tmax, fabsf(h[c]) + d[c]);
+                            continue;
+                        }
                         Cout[o + c * TC_BM] = h[c];
                         C2out[o + c * TC_BM] = d[c];
                         if (SCALED) tmax = fmaxf(tmax, fabsf(h[c]));
@@ -202,8 +232,9 @@ __device__ __forceinline__ void tc_store_tile(const TcArgs &p, float (&acc)[4][3
                 for (int c = 0; c < TC_EB; ++c)
                     if (c < nc) {
                         const float v = (SCALED ? acc[gi][j0 + c] * oscale : acc[gi][j0 + c]) * in[c];
-                        Cout[o + c * TC_BM] = v;
                         if (SCALED) tmax = fmaxf(tmax, fabsf(v));
+                        if (TC_DBG(p) & 8) continue;
+                        Cout[o + c * TC_BM] = v;
                     }
             } else {
 #pragma unroll
@@ -214,6 +245,74 @@ __device__ __forceinline__ void tc_store_tile(const TcArgs &p, float (&acc)[4][3
     }
     if (EPI == EPI_HIDDEN_HEAD && row_ok && !(TC_DBG(p) & 4))
         p.ypart[(int64_t)(2 * (n0 / p.bn) + half) * p.m_pad + m0 + quad * 32 + lane] = ysum;
+}
+
+
+// ---- epilogue of the CTA-pair kernels ------------------------------------------------------------------------------
+// The forward bias is folded into the register accumulators when a tile starts (acc = bias / oscale, while the first MMAs
+// of the tile run), so the final phase has no loads; every thread keeps base pointers of its row, so the stores take
+// immediate column offsets.  Valid columns of a 32-column group: multiples of 8 (N and bn are).
+__device__ __forceinline__ int tc_group_valid(const TcArgs &p, int n0, int g) {
+    int v = p.N - (n0 + g * 32);
+    const int w = p.bn - g * 32;
+    v = v < w ? v : w;
+    return v < 0 ? 0 : (v > 32 ? 32 : v);
+}
+
+template <int EPI>
+__device__ __forceinline__ void tc_init_acc(const TcArgs &p, float (&acc)[4][32], int n0, int half, float inv_oscale) {
+#pragma unroll
+    for (int gi = 0; gi < 4; ++gi) {
+        const int g = 2 * gi + half;
+        const int nv = (EPI == EPI_HIDDEN || EPI == EPI_HIDDEN_HEAD) ? tc_group_valid(p, n0, g) : 0;
+        const float4 *__restrict__ b = reinterpret_cast<const float4 *>(p.bias + n0 + g * 32);  // 16-byte aligned: n0, widths % 16 == 0
+#pragma unroll
+        for (int q = 0; q < 8; ++q) {
+            const float4 t = 4 * q < nv ? __ldg(b + q) : make_float4(0.f, 0.f, 0.f, 0.f);
+            acc[gi][4 * q] = t.x * inv_oscale, acc[gi][4 * q + 1] = t.y * inv_oscale;
+            acc[gi][4 * q + 2] = t.z * inv_oscale, acc[gi][4 * q + 3] = t.w * inv_oscale;
+        }
+    }
+}
+
+template <int EPI, bool SCALED>
+__device__ __forceinline__ void tc_finish_tile(const TcArgs &p, float (&acc)[4][32], int m0, int n0, int quad, int lane,
+                                               int half, bool row_ok, float oscale, float &tmax) {
+    // forward epilogues (EPI_HIDDEN, EPI_HIDDEN_HEAD).  Tile-transposed [M / 128][N][128]: column c of this tile is 128
+    // consecutive floats, each warp store one full 128-byte line at a compile-time offset from the thread's base pointer.
+    const int64_t tbase = (int64_t)(m0 / TC_BM) * p.N * TC_BM + quad * 32 + lane + (int64_t)(n0 + half * 32) * TC_BM;
+    float *__restrict__ cp = p.C + tbase;
+    float *__restrict__ dp = p.C2 + tbase;
+    const float k1 = -oscale * 1.4426950408889634f;
+    float ysum = 0.f;
+    if (row_ok && !(TC_DBG(p) & 4)) {
+#pragma unroll
+        for (int gi = 0; gi < 4; ++gi) {
+            const int g = 2 * gi + half;
+            const int nv = tc_group_valid(p, n0, g);
+            const float *__restrict__ wh = p.w_head + n0 + g * 32;
+#pragma unroll
+            for (int j0 = 0; j0 < 32; j0 += 8) {
+                if (j0 >= nv) continue;  // warp-uniform
+                float h[8], d[8];
+#pragma unroll
+                for (int c = 0; c < 8; ++c) swish_pair_acc(acc[gi][j0 + c], oscale, k1, h[c], d[c]);
+#pragma unroll
+                for (int c = 0; c < 8; ++c) {
+                    const int off = (gi * 64 + j0 + c) * TC_BM;  // compile-time column offset of the store
+                    if (EPI == EPI_HIDDEN_HEAD) ysum = fmaf(h[c], __ldg(wh + j0 + c), ysum);
+                    if (SCALED && EPI == EPI_HIDDEN) tmax = fmaxf(tmax, fabsf(h[c]));
+                    if (TC_DBG(p) & 8) {  // knock-out: arithmetic without the stores
+                        tmax = fmaxf(tmax, d[c]);
+                        continue;
+                    }
+                    if (EPI == EPI_HIDDEN) cp[off] = h[c];
+                    dp[off] = d[c];
+                }
+            }
+        }
+        if (EPI == EPI_HIDDEN_HEAD) p.ypart[(int64_t)(2 * (n0 / p.bn) + half) * p.m_pad + m0 + quad * 32 + lane] = ysum;
+    }
 }
 
 template <bool SPLIT, int BK, int EPI>
@@ -400,6 +499,13 @@ static int tc_num_sms();
 // read by the tensor core, which is what bounds the single-CTA kernel (shared-memory bandwidth).
 // Hand-shakes across the pair: split-done and accumulator-drained arrivals go to the leader's
 // barriers (mapa + remote arrive); the leader's tcgen05.commit multicasts to both CTAs' barriers.
+// Accumulators.  The tensor core adds into its fp32 accumulator with truncation, so long accumulation chains of LARGE
+// terms bias the result.  The three products of the split are therefore kept apart: the cross terms
+// a_lo.b_hi + a_hi.b_lo, 2^-11 of the result, go to accumulator X (tensor-memory columns [0, 256)) for the whole K range of a
+// tile -- their truncation errors are 2^-11 of the hi.hi ones -- and only the hi.hi terms go to accumulator Y (columns
+// [256, 512)), which the epilogue warps drain into fp32 registers (round-to-nearest adds) every p.flush pipeline stages.  Y is
+// single-buffered: while it is drained the MMA pipe runs the next stage's cross terms, and during the final phase of a
+// tile (elementwise + stores) the issuer has a whole group of stages plus one stage of cross terms of run-way.
 // F16 = true is the 3xFP16 mode (GMNN_MLP_3XF16): the same three-product split on kind::f16, whose
 // MMAs run at twice the tf32 rate on half the operand bytes.  a' = a * 2^s with 2^14 <= max |a'| < 2^15
 // (s from the matrix's absolute maximum, a device scalar the producing kernel left), hi = fp16(a'),
@@ -513,12 +619,42 @@ k_gemm_tc_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
         setmaxnreg_dec<Cfg::REGS_CONTROL>();
         if (warp == 0 && lane == 0) {
             // ===== TMA producer: own A rows, own half of B =====
+            // The activations come from HBM (each GEMM's A is the previous kernel's 1.5 - 2 GB output); with 192 KB of
+            // stages a load that pays the HBM latency inside the ring cannot keep the MMA pipe fed (stage occupancy =
+            // latency + split + MMA).  Every A box is therefore prefetched into L2 p.prefetch stages ahead (about one
+            // tile), and the ring's own load then is an L2 hit.  The weights stay in L2 by themselves.
             const uint32_t tx = (uint32_t)(TC_BM * BK * 4 + 2 * hb * BK * Cfg::ES);
+            const int my_tiles = p.n_tiles > pair ? (p.n_tiles - pair + n_pairs - 1) / n_pairs : 0;
+            const int64_t n_stage_total = (int64_t)my_tiles * nkb;
+            auto a_row = [&](int64_t j, int &kb) {  // stage j of this CTA -> row coordinate of its A box
+                const int t = pair + (int)(j / nkb) * n_pairs;
+                kb = (int)(j % nkb);
+                return (2 * (t / p.n_tiles_n) + (int)rank) * p.K + kb * BK;
+            };
+            auto prefetch_a = [&](int64_t j) {
+                if (j >= n_stage_total) return;
+                int kb;
+                const int row = a_row(j, kb);
+                if (F16) {
+                    tma_prefetch_2d(&tmA, 0, row);
+                } else {
+                    for (int q = 0; q < 4; ++q) tma_prefetch_2d(&tmA, q * 32, row);
+                }
+            };
+            for (int j = 0; j < p.prefetch; ++j) prefetch_a(j);
             uint32_t it = 0;
             for (int t = pair; t < p.n_tiles; t += n_pairs) {
                 const int mt = 2 * (t / p.n_tiles_n) + (int)rank, n0 = (t % p.n_tiles_n) * p.bn;
+                if (EPI == EPI_MUL && (int64_t)mt * TC_BM < p.M) {
+                    // the multiplier block of this tile (swish' of the layer below: bn columns x 128 rows, contiguous in both
+                    // layouts) is read by the epilogue at the END of the tile, from HBM: bring it into L2 now
+                    const int cols = p.N - n0 < p.bn ? p.N - n0 : p.bn;
+                    const char *blk = reinterpret_cast<const char *>(p.Dmul + ((int64_t)mt * p.N + n0) * TC_BM);
+                    for (int c = 0; c < cols; c += 64) bulk_prefetch_l2(blk + (int64_t)c * TC_BM * 4, (uint32_t)((cols - c < 64 ? cols - c : 64) * TC_BM * 4));
+                }
                 for (int kb = 0; kb < nkb; ++kb, ++it) {
                     const int s = it % NST;
+                    if (p.prefetch > 0) prefetch_a((int64_t)it + p.prefetch);
                     mbar_wait(bar_empty(s), ((it / NST) & 1) ^ 1);
                     mbar_arrive_expect_tx(bar_full(s), tx);
                     if (F16) {
@@ -533,19 +669,61 @@ k_gemm_tc_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
             }
         } else if (warp == 1 && lane == 0 && rank == 0) {
             // ===== MMA issuer (leader CTA only) =====
+            // Two accumulators in tensor memory (see the header of this kernel): X, columns [0, 256), takes the cross terms
+            // a_lo.b_hi + a_hi.b_lo of the WHOLE K range of a tile and is drained once per tile; Y, columns [256, 512), takes the
+            // hi.hi terms and is drained every p.flush pipeline stages.
             const uint32_t idesc = F16 ? make_idesc_f16(2 * TC_BM, p.bn) : make_idesc_tf32(2 * TC_BM, p.bn, true);
-            uint32_t it = 0, chunk = 0;
+            const uint32_t d_x = tmem_base, d_y = tmem_base + TC_BN_MAX;
+            uint32_t it = 0, ygrp = 0, xt = 0;
             for (int t = pair; t < p.n_tiles; t += n_pairs) {
                 for (int kb = 0; kb < nkb; ++kb, ++it) {
-                    bool chunk_first, chunk_last;
-                    chunk_pos(p, kb, nkb, chunk_first, chunk_last);
-                    const int a = chunk & 1;
-                    const uint32_t d_tmem = tmem_base + (uint32_t)a * TC_BN_MAX;
-                    if (chunk_first) {
-                        mbar_wait(bar_tempty(a), ((chunk >> 1) & 1) ^ 1);
-                        tcgen05_fence_after();
-                    }
+                    const int pos = kb % p.flush;
+                    const bool y_first = pos == 0, y_last = pos == p.flush - 1 || kb == nkb - 1;
                     const int s = it % NST;
+                    if (!p.xy) {
+                        // ping-pong scheme (backward GEMMs: forces only, chunks of tc_flush_k_bwd): all three products of a
+                        // chunk of p.flush stages go to ONE of the two 256-column buffers, which alternate from chunk to
+                        // chunk; with two chunks per tile the MMAs of the next tile run through the whole final phase of
+                        // this one
+                        const int a = ygrp & 1;
+                        const uint32_t d_tmem = tmem_base + (uint32_t)a * TC_BN_MAX;
+                        if (y_first) {
+                            mbar_wait(bar_tempty(a), ((ygrp >> 1) & 1) ^ 1);
+                            tcgen05_fence_after();
+                        }
+                        mbar_wait(bar_split(s), (it / NST) & 1);
+                        tcgen05_fence_after();
+                        const int krem = p.K - kb * BK;
+                        const int ksteps = krem >= BK ? BK / Cfg::KSTEP : (krem + Cfg::KSTEP - 1) / Cfg::KSTEP;
+                        const uint64_t db_hi = make_smem_desc<Cfg::ROWB>(b_hi(s)), db_lo = make_smem_desc<Cfg::ROWB>(b_lo(s));
+                        const uint64_t da_hi = F16 ? make_smem_desc<Cfg::ROWB>(a_hi(s)) : make_smem_desc_mn128(a_hi(s), BK * 128);
+                        const uint64_t da_lo = F16 ? make_smem_desc<Cfg::ROWB>(a_lo(s)) : make_smem_desc_mn128(a_lo(s), BK * 128);
+                        const uint64_t astep = F16 ? 2 : 64;
+                        uint32_t acc = !y_first;
+                        for (int k = 0; k < ksteps && !(TC_DBG(p) & 2); ++k) {  // small cross terms first
+                            const uint64_t koff = (uint64_t)(2 * k), aoff = astep * k;
+                            if (F16) {
+                                mma_f16_ss_pair(d_tmem, da_lo + aoff, db_hi + koff, idesc, acc);
+                                mma_f16_ss_pair(d_tmem, da_hi + aoff, db_lo + koff, idesc, 1u);
+                            } else {
+                                mma_tf32_ss_pair(d_tmem, da_lo + aoff, db_hi + koff, idesc, acc);
+                                mma_tf32_ss_pair(d_tmem, da_hi + aoff, db_lo + koff, idesc, 1u);
+                            }
+                            acc = 1u;
+                        }
+                        for (int k = 0; k < ksteps; ++k) {
+                            const uint64_t koff = (uint64_t)(2 * k), aoff = astep * k;
+                            if (F16) mma_f16_ss_pair(d_tmem, da_hi + aoff, db_hi + koff, idesc, acc);
+                            else mma_tf32_ss_pair(d_tmem, da_hi + aoff, db_hi + koff, idesc, acc);
+                            acc = 1u;
+                        }
+                        mma_commit_pair(bar_empty(s), 3);
+                        if (y_last) {
+                            mma_commit_pair(bar_tfull(a), 3);
+                            ++ygrp;
+                        }
+                        continue;
+                    }
                     mbar_wait(bar_split(s), (it / NST) & 1);
                     tcgen05_fence_after();
                     const int krem = p.K - kb * BK;
@@ -555,28 +733,41 @@ k_gemm_tc_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                     const uint64_t da_lo = F16 ? make_smem_desc<Cfg::ROWB>(a_lo(s)) : make_smem_desc_mn128(a_lo(s), BK * 128);
                     // per k step: B (and a K-major A) advance 32 bytes along the row, the MN-major A one 1024-byte atom
                     const uint64_t astep = F16 ? 2 : 64;
-                    uint32_t acc = !chunk_first;
-                    for (int k = 0; k < ksteps && !(TC_DBG(p) & 2); ++k) {  // small cross terms first
+                    if (kb == 0) {  // X of the previous tile drained by both CTAs
+                        mbar_wait(bar_tempty(1), (xt & 1) ^ 1);
+                        tcgen05_fence_after();
+                    }
+                    uint32_t acc = kb != 0;
+                    for (int k = 0; k < ksteps && !(TC_DBG(p) & 2); ++k) {
                         const uint64_t koff = (uint64_t)(2 * k), aoff = astep * k;
                         if (F16) {
-                            mma_f16_ss_pair(d_tmem, da_lo + aoff, db_hi + koff, idesc, acc);
-                            mma_f16_ss_pair(d_tmem, da_hi + aoff, db_lo + koff, idesc, 1u);
+                            mma_f16_ss_pair(d_x, da_lo + aoff, db_hi + koff, idesc, acc);
+                            mma_f16_ss_pair(d_x, da_hi + aoff, db_lo + koff, idesc, 1u);
                         } else {
-                            mma_tf32_ss_pair(d_tmem, da_lo + aoff, db_hi + koff, idesc, acc);
-                            mma_tf32_ss_pair(d_tmem, da_hi + aoff, db_lo + koff, idesc, 1u);
+                            mma_tf32_ss_pair(d_x, da_lo + aoff, db_hi + koff, idesc, acc);
+                            mma_tf32_ss_pair(d_x, da_hi + aoff, db_lo + koff, idesc, 1u);
                         }
                         acc = 1u;
                     }
+                    if (y_first) {  // Y of the previous group drained (the cross terms above keep the pipe busy meanwhile)
+                        mbar_wait(bar_tempty(0), (ygrp & 1) ^ 1);
+                        tcgen05_fence_after();
+                    }
+                    acc = !y_first;
                     for (int k = 0; k < ksteps; ++k) {
                         const uint64_t koff = (uint64_t)(2 * k), aoff = astep * k;
-                        if (F16) mma_f16_ss_pair(d_tmem, da_hi + aoff, db_hi + koff, idesc, acc);
-                        else mma_tf32_ss_pair(d_tmem, da_hi + aoff, db_hi + koff, idesc, acc);
+                        if (F16) mma_f16_ss_pair(d_y, da_hi + aoff, db_hi + koff, idesc, acc);
+                        else mma_tf32_ss_pair(d_y, da_hi + aoff, db_hi + koff, idesc, acc);
                         acc = 1u;
                     }
                     mma_commit_pair(bar_empty(s), 3);
-                    if (chunk_last) {
-                        mma_commit_pair(bar_tfull(a), 3);
-                        ++chunk;
+                    if (y_last) {
+                        mma_commit_pair(bar_tfull(0), 3);
+                        ++ygrp;
+                    }
+                    if (kb == nkb - 1) {
+                        mma_commit_pair(bar_tfull(1), 3);
+                        ++xt;
                     }
                 }
             }
@@ -611,30 +802,32 @@ k_gemm_tc_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
         const int quad = warp & 3;
         const int half = (warp - TC_FIRST_EPI_WARP) >> 2;
         const int n_groups = (p.bn + 31) / 32;
-        const int n_chunks = chunk_count(p, nkb);
+        const int n_ygroups = (nkb + p.flush - 1) / p.flush;
         const uint32_t lane_base = tmem_base + ((uint32_t)(quad * 32) << 16);
-        const float oscale = F16 ? pow2i(amax_exponent(*p.amax_a) + amax_exponent(*p.amax_b) - 28) : 1.f;
+        const int osc_e = F16 ? amax_exponent(*p.amax_a) + amax_exponent(*p.amax_b) - 28 : 0;
+        const float oscale = pow2i(osc_e), inv_oscale = pow2i(-osc_e);
         float tmax = 0.f;
-        uint32_t chunk = 0;
+        uint32_t ygrp = 0, xt = 0;
         for (int t = pair; t < p.n_tiles; t += n_pairs) {
             const int m0 = (2 * (t / p.n_tiles_n) + (int)rank) * TC_BM, n0 = (t % p.n_tiles_n) * p.bn;
             const int row = m0 + quad * 32 + lane;
             const bool row_ok = row < p.M;
             float acc[4][32];
-#pragma unroll
-            for (int gi = 0; gi < 4; ++gi)
-#pragma unroll
-                for (int j = 0; j < 32; ++j) acc[gi][j] = 0.f;
-            for (int c = 0; c < n_chunks; ++c, ++chunk) {
-                const int a = chunk & 1;
-                mbar_wait(bar_tfull(a), (chunk >> 1) & 1);
+            tc_init_acc<EPI>(p, acc, n0, half, inv_oscale);  // the forward bias rides in the accumulators
+            // the hi.hi groups (accumulator Y), then the tile's cross terms (accumulator X): round-to-nearest adds in registers
+            for (int c = 0; c < n_ygroups + (p.xy ? 1 : 0); ++c) {
+                // X / Y scheme: buffer 0 = Y (columns 256..511) for the hi.hi groups, then buffer 1 = X (columns 0..255);
+                // ping-pong scheme: chunk c sits in buffer (chunk number) & 1 at columns 256 * buffer
+                const int a = p.xy ? (c < n_ygroups ? 0 : 1) : (int)(ygrp & 1);
+                mbar_wait(bar_tfull(a), p.xy ? ((a == 0 ? ygrp : xt) & 1) : ((ygrp >> 1) & 1));
                 tcgen05_fence_after();
+                const uint32_t col0 = p.xy ? (a == 0 ? TC_BN_MAX : 0) : (uint32_t)a * TC_BN_MAX;
 #pragma unroll
                 for (int gi = 0; gi < 4; ++gi) {
                     const int g = 2 * gi + half;
-                    if (g < n_groups) {
+                    if (g < n_groups && !(a == 1 && (TC_DBG(p) & 2)) && !(TC_DBG(p) & 16)) {  // 16: knock-out of the drains
                         uint32_t v[32];
-                        tmem_ld_32x32(lane_base + (uint32_t)(a * TC_BN_MAX + g * 32), v);
+                        tmem_ld_32x32(lane_base + col0 + (uint32_t)(g * 32), v);
                         tmem_ld_wait();
 #pragma unroll
                         for (int j = 0; j < 32; ++j) acc[gi][j] += __uint_as_float(v[j]);
@@ -643,8 +836,13 @@ k_gemm_tc_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                 tcgen05_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive_cluster(bar_tempty(a), 0);
+                if (!p.xy || a == 0) ++ygrp;
+                else ++xt;
             }
-            tc_store_tile<EPI, F16>(p, acc, m0, n0, quad, lane, half, n_groups, row_ok, oscale, tmax);
+            if (EPI == EPI_HIDDEN || EPI == EPI_HIDDEN_HEAD)
+                tc_finish_tile<EPI, F16>(p, acc, m0, n0, quad, lane, half, row_ok, oscale, tmax);
+            else  // backward: multiplier loads in bursts of 16 ahead of their use
+                tc_store_tile<EPI, F16>(p, acc, m0, n0, quad, lane, half, n_groups, row_ok, oscale, tmax);
         }
         if (F16 && p.amax_out && (EPI == EPI_HIDDEN || EPI == EPI_MUL)) {
 #pragma unroll
@@ -777,12 +975,12 @@ static int tc_launch(const CUtensorMap &tmA, const CUtensorMap &tmB, const TcArg
 }
 
 int g_tc_pair = 1;    // knob "tc_pair": 3xTF32 GEMMs on CTA pairs (cta_group::2)
-int g_tc_flush_head = 0;  // knob "tc_flush_head": first-two-chunks multiplier of the backward GEMMs (forces only); 0 = auto
-int g_tc_flush_head_fwd = 1;  // knob "tc_flush_head_fwd": the same for the forward GEMMs (enters the energy)
+int g_tc_prefetch = 0;  // knob "tc_prefetch": stages of L2 prefetch ahead of the A loads of the CTA-pair kernels (0: off)
+int g_tc_flush_k_bwd = 256;  // knob "tc_flush_k_bwd": K extent between drains of the hi.hi accumulator, backward GEMMs
 #ifdef GMNN_EXPERIMENTS
 int g_tc_debug = 0;
 #endif
-int g_tc_flush_k = 64;   // knob "tc_flush_k": K extent between accumulator flushes of the 3xTF32 / 3xFP16 modes
+int g_tc_flush_k = 128;  // knob "tc_flush_k": K extent between drains of the hi.hi accumulator, forward GEMMs (CTA pairs)
 int g_tc_split_bk = 32;  // knob (gmnn_system_set_int "tc_split_bk"): K extent of a 3xTF32 stage, 16 or 32
 int g_tc_h_bk = 64;      // knob "tc_h_bk": K extent of a 3xFP16 stage, 32 or 64
 
@@ -854,11 +1052,18 @@ int tc_gemm(bool split, int epi, int64_t M, int N, int K, const float *A, const 
     a.bn = pick_bn(N);
     a.n_tiles_n = (N + a.bn - 1) / a.bn;
     a.n_tiles = (int)((M + TC_BM - 1) / TC_BM) * a.n_tiles_n;
-    a.flush = split ? (g_tc_flush_k / BK > 0 ? g_tc_flush_k / BK : 1) : (K + BK - 1) / BK;  // TF32 mode: one chunk
-    // backward GEMMs (forces only: error budget 1e-4) take longer first chunks: x2 on tf32, x4 on fp16, whose
-    // MMAs add 16 products per accumulation step instead of 8
-    const int head_bwd = g_tc_flush_head > 0 ? g_tc_flush_head : (hf ? 4 : 2);
-    a.flush1 = a.flush * (!split ? 1 : (epi != EPI_HIDDEN && epi != EPI_HIDDEN_HEAD) ? head_bwd : g_tc_flush_head_fwd);
+    // Accumulator flushes (the tensor core adds into its fp32 accumulator with truncation):
+    //   CTA-pair kernels: the hi.hi accumulator is drained every tc_flush_k of K on the forward GEMMs (they enter the
+    //     energies) and every tc_flush_k_bwd on the backward GEMMs (forces only: error budget 1e-4); the cross terms have
+    //     an accumulator of their own that lasts the whole tile;
+    //   single-CTA kernel (tc_pair = 0, and the single-pass TF32 mode: one chunk): mixed accumulator, every 64 of K.
+    const bool fwd = epi == EPI_HIDDEN || epi == EPI_HIDDEN_HEAD;
+    const bool pair_kernel = hf != nullptr || (split && g_tc_pair);
+    const int flush_k = pair_kernel ? (fwd ? g_tc_flush_k : g_tc_flush_k_bwd) : 64;
+    a.flush = split ? (flush_k / BK > 0 ? flush_k / BK : 1) : (K + BK - 1) / BK;
+    a.flush1 = a.flush;
+    a.prefetch = g_tc_prefetch;
+    a.xy = fwd ? 1 : 0;
 #ifdef GMNN_EXPERIMENTS
     a.debug = g_tc_debug;
 #else

@@ -64,9 +64,11 @@ __device__ __forceinline__ void pair_gradient(AGet a, const float *R, const floa
 // PAIRBUF = false: gather form, both directions per entry, F_i complete.
 // PAIRBUF = true : own direction only; g_ij goes to gbuf[j][rev] (the slot of (i, -n) in the row of
 //                  j), f_int gets sum_j g_ij, and k_force_reduce subtracts the received row.
-// VIRIAL: also leaves vir_atom[c][i] = -sum_j d_a g_b (c = 3 a + b) over the centre's own directed pairs, whose sum
-// over the atoms is the virial W = -sum_pairs d (x) g = -dE/d strain (oracle O-16).
-template <int NR, int NB, int LPA, bool PAIRBUF, bool VIRIAL>
+// GENERAL = false: the configs' model (Gaussian basis, no ZBL, no virial).  GENERAL = true: run-time switches for the
+// Bessel-like basis and the ZBL term, and with vir_atom != nullptr the kernel also leaves vir_atom[c][i] = -sum_j d_a g_b
+// (c = 3 a + b) over the centre's own directed pairs, whose sum over the atoms is the virial W = -sum_pairs d (x) g =
+// -dE/d strain (oracle O-16).
+template <int NR, int NB, int LPA, bool PAIRBUF, bool GENERAL>
 __global__ void __launch_bounds__(128)
 k_pair_backward(int64_t N, const float4 *__restrict__ pos4, const uint32_t *__restrict__ nbr,
                 const int32_t *__restrict__ count, int cap, Geometry geo, RadialParams rp,
@@ -97,9 +99,10 @@ k_pair_backward(int64_t N, const float4 *__restrict__ pos4, const uint32_t *__re
     }
     __syncthreads();
     float fx = 0.f, fy = 0.f, fz = 0.f;
-    float vir[VIRIAL ? 9 : 1];
+    const bool VIRIAL = GENERAL && vir_atom != nullptr;
+    float vir[GENERAL ? 9 : 1];
 #pragma unroll
-    for (int c = 0; c < (VIRIAL ? 9 : 1); ++c) vir[c] = 0.f;
+    for (int c = 0; c < (GENERAL ? 9 : 1); ++c) vir[c] = 0.f;
     if (live) {
         const float4 xi = pos4[i];
         const int zi = __float_as_int(xi.w);
@@ -135,7 +138,7 @@ k_pair_backward(int64_t N, const float4 *__restrict__ pos4, const uint32_t *__re
                     const float rinv = rsqrtf(pg.r2);
                     const float r = pg.r2 * rinv;
                     float phi[NB], dphi[NB], fc, dfc;
-                    radial_basis<NB, true>(rp, r, rinv, phi, dphi, fc, dfc);
+                    radial_basis<NB, true, GENERAL>(rp, r, rinv, phi, dphi, fc, dfc);
                     const float ux = pg.dx * rinv, uy = pg.dy * rinv, uz = pg.dz * rinv;
                     float mono[PSI];
                     monomials(ux, uy, uz, mono);
@@ -176,19 +179,21 @@ k_pair_backward(int64_t N, const float4 *__restrict__ pos4, const uint32_t *__re
                             gxr = hx, gyr = hy, gzr = hz;
                         }
                     }
-                    if (rp.zbl_on && pg.r2 < rp.zbl_r_max2) {  // ZBL: g += d(V/2)/dr u in both directions of the pair
+                    if (GENERAL && rp.zbl_on && pg.r2 < rp.zbl_r_max2) {  // ZBL: g += d(V/2)/dr u in both directions of the pair
                         float e, de;
                         zbl_half<true>(rp, zi, pg.zj, r, rinv, e, de);
                         gxo = fmaf(de, ux, gxo), gyo = fmaf(de, uy, gyo), gzo = fmaf(de, uz, gzo);
                         if (!PAIRBUF) gxr = fmaf(-de, ux, gxr), gyr = fmaf(-de, uy, gyr), gzr = fmaf(-de, uz, gzr);
                     }
                     if (PAIRBUF) *slot = make_float4(gxo, gyo, gzo, 0.f);
-                    if (VIRIAL) {
-                        const float dv[3] = {pg.dx, pg.dy, pg.dz}, gv[3] = {gxo, gyo, gzo};
+                    if (GENERAL) {
+                        if (VIRIAL) {
+                            const float dv[3] = {pg.dx, pg.dy, pg.dz}, gv[3] = {gxo, gyo, gzo};
 #pragma unroll
-                        for (int a = 0; a < 3; ++a)
+                            for (int a = 0; a < 3; ++a)
 #pragma unroll
-                            for (int b = 0; b < 3; ++b) vir[3 * a + b] = fmaf(-dv[a], gv[b], vir[3 * a + b]);
+                                for (int b = 0; b < 3; ++b) vir[3 * a + b] = fmaf(-dv[a], gv[b], vir[3 * a + b]);
+                        }
                     }
                     // F_i += g_ij - g_ji   (g_ji = dE_j/dd_ji, d_ji = -d_ij)
                     fx += gxo - gxr;
@@ -209,7 +214,7 @@ k_pair_backward(int64_t N, const float4 *__restrict__ pos4, const uint32_t *__re
         f_int[3 * i + 1] = fy;
         f_int[3 * i + 2] = fz;
     }
-    if (VIRIAL) {
+    if (GENERAL && VIRIAL) {
 #pragma unroll
         for (int c = 0; c < 9; ++c) {
 #pragma unroll
@@ -258,14 +263,15 @@ static int pair_backward_lpa(gmnn_system *s, cudaStream_t st, int lpa) {
     const unsigned grid = nblocks(s->N * lpa, 128);
     const bool pairbuf = s->force_mode == GMNN_FORCE_PAIRBUF;
     const bool virial = s->want_virial && s->vir_atom != nullptr;
+    const bool general = virial || m->rp.basis_kind != 0 || m->rp.zbl_on;
     if (pairbuf && !(s->list_has_rev && s->rev && s->gbuf)) {
         set_error("force_mode changed after the list was built: call gmnn_build_neighbors again");
         return GMNN_INVALID_ARG;
     }
-#define GMNN_PB_LAUNCH(L, PB, VIR)                                                                         \
-    k_pair_backward<NR, NB, L, PB, VIR><<<grid, 128, smem, st>>>(s->N, s->pos4, s->nbr, s->count, s->cap, s->geo, m->rp, \
+#define GMNN_PB_LAUNCH(L, PB, GEN)                                                                         \
+    k_pair_backward<NR, NB, L, PB, GEN><<<grid, 128, smem, st>>>(s->N, s->pos4, s->nbr, s->count, s->cap, s->geo, m->rp, \
                                                                 m->beta, s->A, s->f_int, PB ? s->rev : nullptr, \
-                                                                PB ? s->gbuf : nullptr, s->mrow, VIR ? s->vir_atom : nullptr)
+                                                                PB ? s->gbuf : nullptr, s->mrow, (GEN && virial) ? s->vir_atom : nullptr)
 #define GMNN_PB(L)                                                                                         \
     case L: {                                                                                              \
         static size_t opted_on[MAX_DEVICES] = {};                                                          \
@@ -281,9 +287,9 @@ static int pair_backward_lpa(gmnn_system *s, cudaStream_t st, int lpa) {
                                            cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));       \
             opted = smem;                                                                                  \
         }                                                                                                  \
-        if (pairbuf && virial) GMNN_PB_LAUNCH(L, true, true);                                              \
+        if (pairbuf && general) GMNN_PB_LAUNCH(L, true, true);                                             \
         else if (pairbuf) GMNN_PB_LAUNCH(L, true, false);                                                  \
-        else if (virial) GMNN_PB_LAUNCH(L, false, true);                                                   \
+        else if (general) GMNN_PB_LAUNCH(L, false, true);                                                  \
         else GMNN_PB_LAUNCH(L, false, false);                                                              \
     } break;
     switch (lpa) {

@@ -40,11 +40,14 @@ __device__ __forceinline__ PairGeom pair_geometry(uint32_t entry, const float4 &
 }
 
 // Phi_k(r) = exp(-gamma (r - mu_k)^2), f_c = 1/2 (1 + cos(pi r / r_cut))   (readings R1-R3)
-template <int NB, bool WITH_DERIV>
+// GENERAL = false: the instantiation for the configs' model (Gaussians, no ZBL); GENERAL = true adds the run-time
+// switches of the other basis (and, in the kernels, the ZBL term and the virial) -- kept out of the default path,
+// where the extra branches and live values cost 40 % on k_pair_forward.
+template <int NB, bool WITH_DERIV, bool GENERAL>
 __device__ __forceinline__ void radial_basis(const RadialParams &rp, float r, float rinv, float *phi, float *dphi,
                                              float &fc, float &dfc) {
     const float t = r * rp.inv_rc;
-    if (rp.basis_kind == 1) {
+    if (GENERAL && rp.basis_kind == 1) {
         // Bessel-like functions of Kocer et al. (reading R30): f_n = c_n [sinc(a_{n+1} r) + sinc(a_{n+2} r)],
         // a_k = k pi / r_cut.  sin and cos of k pi t, k = 1 .. NB + 1, by the Chebyshev recurrence from the sine and
         // cosine of pi t that the cutoff function needs anyway; d/dr sinc(a r) = (cos(a r) - sinc(a r)) / r.

@@ -10,7 +10,7 @@ namespace gmnn {
 // ---------------------------------------------------------------------------------------------
 // a4 + a5: pair radial functions and moment accumulation
 // ---------------------------------------------------------------------------------------------
-template <int NR, int NB, int LPA>
+template <int NR, int NB, int LPA, bool GENERAL>
 __global__ void __launch_bounds__(128)
 k_pair_forward(int64_t N, const float4 *__restrict__ pos4, const uint32_t *__restrict__ nbr,
                const int32_t *__restrict__ count, int cap, Geometry geo, RadialParams rp,
@@ -56,8 +56,8 @@ k_pair_forward(int64_t N, const float4 *__restrict__ pos4, const uint32_t *__res
                     const float rinv = rsqrtf(pg.r2);
                     const float r = pg.r2 * rinv;
                     float phi[NB], fc, dummy;
-                    radial_basis<NB, false>(rp, r, rinv, phi, nullptr, fc, dummy);
-                    if (rp.zbl_on && pg.r2 < rp.zbl_r_max2) {
+                    radial_basis<NB, false, GENERAL>(rp, r, rinv, phi, nullptr, fc, dummy);
+                    if (GENERAL && rp.zbl_on && pg.r2 < rp.zbl_r_max2) {
                         float e, de;
                         zbl_half<false>(rp, zi, pg.zj, r, rinv, e, de);
                         ez += e;
@@ -100,7 +100,7 @@ k_pair_forward(int64_t N, const float4 *__restrict__ pos4, const uint32_t *__res
                 acc[s][q].x += __shfl_xor_sync(0xffffffffu, acc[s][q].x, o);
                 acc[s][q].y += __shfl_xor_sync(0xffffffffu, acc[s][q].y, o);
             }
-    if (e_zbl) {
+    if (GENERAL && e_zbl) {
 #pragma unroll
         for (int o = LPA / 2; o >= 1; o >>= 1) ez += __shfl_xor_sync(0xffffffffu, ez, o);
         if (live && sub == 0) e_zbl[i] = ez;
@@ -123,10 +123,15 @@ static int pair_forward_lpa(gmnn_system *s, cudaStream_t st, int lpa) {
     const gmnn_model *m = s->model;
     const size_t smem = sizeof(float) * m->rp.n_species * m->rp.n_species * NR * m->rp.kb;
     const unsigned grid = nblocks(s->N * lpa, 128);
+    const bool general = m->rp.basis_kind != 0 || m->rp.zbl_on;
 #define GMNN_PF(L)                                                                                        \
     case L:                                                                                               \
-        k_pair_forward<NR, NB, L><<<grid, 128, smem, st>>>(s->N, s->pos4, s->nbr, s->count, s->cap, s->geo, \
-                                                           m->rp, m->beta, s->psi, s->mrow, s->e_zbl);    \
+        if (general)                                                                                      \
+            k_pair_forward<NR, NB, L, true><<<grid, 128, smem, st>>>(s->N, s->pos4, s->nbr, s->count, s->cap, s->geo, \
+                                                                     m->rp, m->beta, s->psi, s->mrow, s->e_zbl); \
+        else                                                                                              \
+            k_pair_forward<NR, NB, L, false><<<grid, 128, smem, st>>>(s->N, s->pos4, s->nbr, s->count, s->cap, s->geo, \
+                                                                      m->rp, m->beta, s->psi, s->mrow, nullptr); \
         break;
     switch (lpa) {
         GMNN_PF(1) GMNN_PF(2) GMNN_PF(4) GMNN_PF(8) GMNN_PF(16) GMNN_PF(32)

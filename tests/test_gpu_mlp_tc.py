@@ -49,10 +49,10 @@ def _run(sysm, pos):
     return float(e.cpu()[0]), ea.cpu().numpy().astype(np.float64), f.cpu().numpy().astype(np.float64)
 
 
-@pytest.mark.parametrize("split_bk,flush_k", [(16, 32), (32, 32), (16, 16), (32, 64)])
+@pytest.mark.parametrize("split_bk,flush_k", [(16, 32), (32, 64), (16, 128), (32, 128)])
 @pytest.mark.parametrize("name", ["config1", "config2", "config3_1024", "config3_8192"])
 def test_3xtf32_meets_fp32_tolerance(gm, orc, name, split_bk, flush_k):
-    """Both stage shapes (64 B and 128 B swizzle) and several accumulator-flush intervals."""
+    """Both stage shapes (64 B and 128 B swizzle) and several drain intervals of the hi.hi accumulator (128 = default)."""
     w = wl.make_workload(name)
     ref = _ref(orc, w)
     sysm, pos = _system(gm, w, P3X)
@@ -62,7 +62,7 @@ def test_3xtf32_meets_fp32_tolerance(gm, orc, name, split_bk, flush_k):
         e, ea, f = _run(sysm, pos)
     finally:
         sysm.set_int("tc_split_bk", 32)
-        sysm.set_int("tc_flush_k", 64)
+        sysm.set_int("tc_flush_k", 128)
     print("3xTF32 %s bk %d flush %d: energy err %.3f x 1e-5, force err %.2e" % (
         name, split_bk, flush_k, energy_atom_error(ea, ref.e_atom), force_error(f, ref.forces)))
     assert energy_atom_error(ea, ref.e_atom) <= 1.0
@@ -70,7 +70,7 @@ def test_3xtf32_meets_fp32_tolerance(gm, orc, name, split_bk, flush_k):
     assert abs(e - ref.energy) <= E_TOTAL_RTOL * np.abs(ref.e_atom).sum()
 
 
-@pytest.mark.parametrize("h_bk,flush_k", [(64, 64), (32, 64), (32, 32)])
+@pytest.mark.parametrize("h_bk,flush_k", [(64, 128), (64, 64), (32, 128), (32, 32)])
 @pytest.mark.parametrize("name", ["config1", "config2", "config3_1024", "config3_8192"])
 def test_3xf16_meets_fp32_tolerance(gm, orc, name, h_bk, flush_k):
     """3xFP16: both stage shapes (128 B and 64 B swizzle of the fp16 operand rows, 3 and 6 stages)."""
@@ -83,7 +83,7 @@ def test_3xf16_meets_fp32_tolerance(gm, orc, name, h_bk, flush_k):
         e, ea, f = _run(sysm, pos)
     finally:
         sysm.set_int("tc_h_bk", 64)
-        sysm.set_int("tc_flush_k", 64)
+        sysm.set_int("tc_flush_k", 128)
     print("3xFP16 %s bk %d flush %d: energy err %.3f x 1e-5, force err %.2e" % (
         name, h_bk, flush_k, energy_atom_error(ea, ref.e_atom), force_error(f, ref.forces)))
     assert energy_atom_error(ea, ref.e_atom) <= 1.0

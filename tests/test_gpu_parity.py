@@ -188,11 +188,15 @@ def test_error_codes(gm):
     with pytest.raises(gm.GmnnError) as e:
         sysm.build_neighbors(pos, w.cell9, w.pbc, 5.0, 0.5)  # r_cut differs from the model's
     assert e.value.code == gm.GMNN_INVALID_ARG
-    tri = w.cell9.copy()
-    tri[1] = 0.3
+    flat = w.cell9.copy()
+    flat[3:6] = flat[0:3]  # b = a: no volume (sheared cells themselves are supported, tests/test_gpu_triclinic.py)
     with pytest.raises(gm.GmnnError) as e:
-        sysm.build_neighbors(pos, tri, w.pbc, 6.0, 0.5)
-    assert e.value.code == gm.GMNN_UNSUPPORTED
+        sysm.build_neighbors(pos, flat, w.pbc, 6.0, 0.5)
+    assert e.value.code == gm.GMNN_INVALID_ARG
+    # a failed build leaves no list behind (never an old list beside a new geometry)
+    with pytest.raises(gm.GmnnError) as e:
+        sysm.energy_forces(pos)
+    assert e.value.code == gm.GMNN_INVALID_ARG
     bad = pos.clone()
     bad[5, 0] = -0.25
     with pytest.raises(gm.GmnnError) as e:
