@@ -35,11 +35,7 @@ import numpy as np  # noqa: E402
 METRIC = "atom-steps/s (GMNN energy+forces)"
 UNIT = "atom-steps/s"
 N_FEATURES = 360
-# ncu --set full, config5, sum over the four GEMM launches of one step (profiles/ncu_r1_gemm_3xtf32.md, ncu_r1_gemm_f16.md)
-NCU_GEMM_DRAM_BYTES_PER_STEP = {"3xtf32": 20.43e9, "3xf16": 20.99e9}
 MLP_NAMES = {"fp32": 0, "3xtf32": 1, "tf32": 2, "3xf16": 3}
-FP32_LANES_PER_SM = 128  # B200_PROFILING.md / B300_MICROARCH.md: 4 SMSPs x 32 FMA lanes
-N_SMS = 148
 
 
 def load_peaks():
@@ -185,18 +181,24 @@ def oracle_prepare(w):
 
 def oracle_step(orc, model, w, pairs):
     t0 = time.perf_counter()
-    orc.energy_forces(model, w.positions, w.species, w.cell, pairs)
+    if w.model.n_heads > 1:  # config 4: the step is the full ensemble evaluation (one forward, one backward per head)
+        orc.ensemble(model, w.positions, w.species, w.cell, pairs)
+    else:
+        orc.energy_forces(model, w.positions, w.species, w.cell, pairs)
     return time.perf_counter() - t0
 
 
 def cpu_baseline(workload_name: str, n_sample: int = 16384):
+    if workload_name == "config4":
+        n_sample = 2048  # 32 backward passes per evaluation
     w = oracle_sample_workload(workload_name, n_sample)
     orc, model, pairs = oracle_prepare(w)
     dt = oracle_step(orc, model, w, pairs)
     return {"value": w.n_atoms / dt, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle",
-            "sample": "one fp64 energy+forces evaluation (oracle/gmnn_oracle.c, OpenMP) of a %d-atom box of the "
+            "sample": "one fp64 %s evaluation (oracle/gmnn_oracle.c, OpenMP) of a %d-atom box of the "
                       "same family as %s (same density, species ratio, r_cut, skin, model), neighbour list prebuilt; "
-                      "%.2f s" % (w.n_atoms, workload_name, dt)}
+                      "%.2f s" % ("shallow-ensemble (32 heads)" if w.model.n_heads > 1 else "energy+forces", w.n_atoms,
+                                  workload_name, dt)}
 
 
 def run_reference(args):
@@ -307,6 +309,64 @@ def run_switching(args):
     return 0
 
 
+def measure_run_peaks(dev, mlp):
+    """Roofline denominators measured in THIS run ("measure them in the same run"): the fp32 FMA rate
+    from the library's register-only FMA kernel, and dense fp16 / tf32 matmul rates (8192^3, cuBLAS through torch, the
+    method of MEASURED_PEAKS.json) as the tensor roofs of the two split modes."""
+    import torch
+
+    import paper_2505_22168_b200 as gm
+
+    out = {"fp32_fma_tflops": gm.measure_fp32_peak()}
+    n = 8192
+
+    def mm_rate(dtype, allow_tf32):
+        torch.backends.cuda.matmul.allow_tf32 = allow_tf32
+        a = torch.randn(n, n, device=dev, dtype=dtype)
+        b = torch.randn(n, n, device=dev, dtype=dtype)
+        torch.matmul(a, b)
+        torch.cuda.synchronize()
+        best = 0.0
+        for _ in range(5):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            torch.matmul(a, b)
+            e1.record()
+            torch.cuda.synchronize()
+            best = max(best, 2.0 * n ** 3 / (e0.elapsed_time(e1) * 1e-3) / 1e12)
+        # sustained: back to back for about a second (the power cap pulls the clock down)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        reps = max(4, int(1.0 * best * 1e12 / (2.0 * n ** 3)))
+        e0.record()
+        for _ in range(reps):
+            torch.matmul(a, b)
+        e1.record()
+        torch.cuda.synchronize()
+        return best, 2.0 * n ** 3 * reps / (e0.elapsed_time(e1) * 1e-3) / 1e12
+
+    if mlp in ("3xf16", "3xtf32", "tf32"):
+        out["fp16_matmul_tflops_burst"], out["fp16_matmul_tflops_sustained"] = mm_rate(torch.float16, False)
+    if mlp in ("3xtf32", "tf32"):
+        out["tf32_matmul_tflops_burst"], out["tf32_matmul_tflops_sustained"] = mm_rate(torch.float32, True)
+        torch.backends.cuda.matmul.allow_tf32 = False
+    return out
+
+
+def recorded_traffic(workload, mlp):
+    """dram__bytes_read.sum + dram__bytes_write.sum per GEMM launch from the committed ncu capture of this workload and MLP
+    mode (profiles/ncu_r2_gemm_traffic.json, written from `ncu --set full`, command inside), or None: never a constant
+    pasted into this file."""
+    path = os.path.join(ROOT, "profiles", "ncu_r2_gemm_traffic.json")
+    if not os.path.exists(path):
+        return None, None
+    with open(path) as f:
+        rec = json.load(f)
+    ent = rec.get("%s/%s" % (workload, mlp))
+    if not ent:
+        return None, None
+    return ent["dram_bytes_per_launch"], "profiles/ncu_r2_gemm_traffic.json (ncu --set full of commit %s)" % rec.get("commit", "?")
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -324,6 +384,9 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=dev)
     peaks = load_peaks()
 
+    # what one "step" is: an MD step (default: every row of SURVEY 8(a) but a12), one gmnn_energy_forces call (--ef:
+    # BASELINE.json config 3, "energy+forces throughput per N"), or one gmnn_ensemble_energy_forces call (config 4)
+    mode = "ensemble" if args.workload == "config4" else ("ef" if args.ef else "md")
     w = make_bench_workload(args.workload, args.weight_sets)
     N = w.n_atoms
     mlp = MLP_NAMES[args.mlp]
@@ -333,7 +396,7 @@ def run_ours(args):
     pos = pos0.clone()
     vel = torch.from_numpy(w.velocities).to(dev)
     masses = torch.from_numpy(w.masses).to(dev)
-    if args.workload != "config5":
+    if args.workload != "config5" and mode == "md":
         # long runs of the small boxes densify locally under the random-weight model: leave head room
         # (the list has a static capacity, like the paper's `extra_capacity`)
         vol = float(np.prod(w.cell.astype(np.float64)))
@@ -353,40 +416,66 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    # ---- device-resident MD steps -------------------------------------------------------------
+    e_out = torch.empty(1, dtype=torch.float64, device=dev)
+    ea_out = torch.empty(N, dtype=torch.float32, device=dev)
+    f_out = torch.empty(N, 3, dtype=torch.float32, device=dev)
+
+    def run_steps(n, series):
+        """n steps of the timed kind; returns (epot + ekin series or None, rebuilds)."""
+        if mode == "md":
+            ep, ek, nr = sysm.md_verlet_steps(pos, vel, masses, w.dt_fs, n, want_series=series)
+            return ((ep + ek) if series else None), nr
+        for _ in range(n):
+            if mode == "ef":
+                sysm.energy_forces(pos, e_out, ea_out, f_out)
+            else:
+                sysm.ensemble_energy_forces(pos)
+        return None, 0
+
+    # ---- device-resident steps ----------------------------------------------------------------
     sysm.set_int("md_continue", 1)
     stream = torch.cuda.current_stream()
     total_rebuilds = 0
     if args.warmup > 0:
-        _, _, nreb = sysm.md_verlet_steps(pos, vel, masses, w.dt_fs, args.warmup, want_series=False)
-        total_rebuilds += nreb
-    sysm.set_int("profile", 0 if args.no_stages else 1)
+        total_rebuilds += run_steps(args.warmup, False)[1]
+    stages_on = not args.no_stages and mode != "ensemble"
+    sysm.set_int("profile", 1 if stages_on else 0)
     sampler = ClockSampler(local)
     sampler.start()
     barrier()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     launches0 = gm.launch_count()
     ev0.record(stream)
-    epot, ekin, nreb = sysm.md_verlet_steps(pos, vel, masses, w.dt_fs, args.steps, want_series=True)
+    etot_series, nreb = run_steps(args.steps, True)
     ev1.record(stream)
     barrier()
     launches = gm.launch_count() - launches0
     clocks = sampler.stop()
     total_rebuilds += nreb
     ms = ev0.elapsed_time(ev1)
-    stages = [] if args.no_stages else sysm.stage_times()
+    stages = sysm.stage_times() if stages_on else []
     sysm.set_int("profile", 0)
     ms_max = max_over_ranks(ms, world, dev)
     value = whole_job_value(N, args.steps, world, ms_max)
-    etot = (epot + ekin).cpu().numpy()
-    drift = float(np.abs(etot - etot[0]).max() / N)
+    drift = None
+    if etot_series is not None:
+        etot = etot_series.cpu().numpy()
+        drift = float(np.abs(etot - etot[0]).max() / N)
+
+    # ---- roofs measured in this run, after the timed region (a second of dense matmul heats the part) ------------
+    run_peaks = measure_run_peaks(dev, args.mlp)
 
     # ---- per-stage roofline (live CUDA events of the timed region) ------------------------------
     sm = stage_model(w, nl_mean, nc_mean, hidden_macs, args.mlp, args.forces)
-    sm_mhz = clocks.get("sm_mhz") or peaks["sm_max_mhz"]
-    fp32_peak_tflops = N_SMS * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
-    # tensor peak of the MLP's operand type: fp16 = the measured bf16 figure, tf32 = half of it (nominal ratio)
-    tf32_peak_tflops = (1.0 if args.mlp == "3xf16" else 0.5) * peaks["bf16_sustained"]
+    # roofs: HBM and the fp16/bf16 tensor rate from MEASURED_PEAKS.json (driver-measured on this pool; sustained: the
+    # kernels are timed inside a long step); fp32 FMA and tf32 measured in this run
+    fp32_peak_tflops = run_peaks.get("fp32_fma_tflops") or float("nan")
+    if args.mlp == "3xf16":
+        tensor_peak, tensor_src = peaks["bf16_sustained"], "bf16_tflops_sustained of MEASURED_PEAKS.json (%s); fp16 runs at the bf16 rate: %.0f TFLOP/s sustained in this run" % (
+            peaks["source"], run_peaks.get("fp16_matmul_tflops_sustained", float("nan")))
+    else:
+        tensor_peak = run_peaks.get("tf32_matmul_tflops_sustained", 0.5 * peaks["bf16_sustained"])
+        tensor_src = "tf32 8192^3 matmul, sustained, measured in this run"
     stage_out = {}
     per_step_ms = {}
     for name, mean_ms, cnt in stages:
@@ -402,7 +491,7 @@ def run_ours(args):
         if sec > 0 and info["flops"] > 0:
             tf = info["flops"] * N / sec / 1e12
             ent["tflops"] = round(tf, 2)
-            ent["flop_frac"] = round(tf / (tf32_peak_tflops if info["bound"] == "tensor" else fp32_peak_tflops), 4)
+            ent["flop_frac"] = round(tf / (tensor_peak if info["bound"] == "tensor" else fp32_peak_tflops), 4)
         stage_out[name] = ent
     dom = max(per_step_ms, key=per_step_ms.get) if per_step_ms else None
     if dom is not None and args.mlp != "fp32" and "mlp_forward" in per_step_ms and "mlp_backward" in per_step_ms:
@@ -418,15 +507,13 @@ def run_ours(args):
         if info["bound"] == "hbm":
             ach, peak, unit = info["bytes"] * N / sec / 1e9, peaks["hbm_gbs"], "GB/s"
         elif info["bound"] == "tensor":
-            ach, peak, unit = info["flops"] * N / sec / 1e12, tf32_peak_tflops, "TFLOP/s"
+            ach, peak, unit = info["flops"] * N / sec / 1e12, tensor_peak, "TFLOP/s"
         else:
             ach, peak, unit = info["flops"] * N / sec / 1e12, fp32_peak_tflops, "TFLOP/s"
         roofline = {"kernel": dom, "bound": info["bound"], "achieved": round(ach, 3), "peak": round(peak, 3),
                     "unit": unit, "frac": round(ach / peak, 4), "traffic": None,
-                    "peak_source": {"hbm": "MEASURED_PEAKS.json hbm_gbs (%s)" % peaks["source"],
-                                    "tensor": ("bf16_tflops_sustained (%s); fp16 runs at the bf16 rate" if args.mlp == "3xf16" else
-                                               "0.5 (nominal tf32:bf16) x bf16_tflops_sustained (%s)") % peaks["source"],
-                                    "alu": "148 SMs x 128 fp32 lanes x 2 flop x sm_max_mhz (derived, DESIGN.md 5)"}[info["bound"]],
+                    "peak_source": {"hbm": "MEASURED_PEAKS.json hbm_gbs (%s)" % peaks["source"], "tensor": tensor_src,
+                                    "alu": "fp32 FMA rate measured in this run (gmnn_measure_fp32_peak)"}[info["bound"]],
                     "share_of_step": round(per_step_ms[dom] / (ms_max / args.steps), 4),
                     "algorithmic_per_atom": {"bytes": info["bytes"], "flops": info["flops"]}}
         if info["bound"] == "tensor":
@@ -434,23 +521,25 @@ def run_ours(args):
             # report them together, per launch
             t_f = [m for n_, m, _ in stages if n_ == "mlp_forward"][0]
             t_b = [m for n_, m, _ in stages if n_ == "mlp_backward"][0]
-            n_launch = 2 * len(w.model.hidden)
+            n_launch = 2 * len(w.model.hidden) * w.model.n_weight_sets
             ach = 2.0 * info["flops"] * N / ((t_f + t_b) * 1e-3) / 1e12
+            traffic, traffic_src = recorded_traffic(args.workload, args.mlp)
             roofline.update({"kernel": {"3xf16": "k_gemm_tc_pair<F16>", "3xtf32": "k_gemm_tc_pair"}.get(args.mlp, "k_gemm_tc"),
                              "launches_per_step": n_launch, "achieved": round(ach, 3), "frac": round(ach / peak, 4),
                              "avg_launch_ms": round((t_f + t_b) / n_launch, 4),
                              "share_of_step": round((per_step_ms["mlp_forward"] + per_step_ms["mlp_backward"])
                                                     / (ms_max / args.steps), 4),
-                             "algorithmic_per_atom": {"bytes": 4.0 * (2 * N_FEATURES + (8 if w.model.n_heads == 1 else 9) * w.model.hidden[0]),
-                                                      "flops": 2.0 * info["flops"]}})
-            if args.workload == "config5" and args.mlp in NCU_GEMM_DRAM_BYTES_PER_STEP:
-                # dram__bytes_read.sum + dram__bytes_write.sum of the four launches of one step, per launch
-                roofline["traffic"] = round(NCU_GEMM_DRAM_BYTES_PER_STEP[args.mlp] / n_launch)
+                             # algorithmic = the fused count of SURVEY 8(d): G in, dG out, E_i out; what the unfused
+                             # layers actually move through HBM (H, D, dZ written and re-read as fp32) is listed beside it
+                             "algorithmic_per_atom": {"bytes": 4.0 * (2 * N_FEATURES + 1), "flops": 2.0 * info["flops"]},
+                             "unfused_hbm_bytes_per_atom": 4.0 * (2 * N_FEATURES + (8 if w.model.n_heads == 1 else 9) * w.model.hidden[0]),
+                             "traffic": traffic, "traffic_source": traffic_src})
         if info["bound"] == "tensor" and args.mlp in ("3xtf32", "3xf16"):
             roofline["note"] = ("achieved counts the ALGORITHMIC flops (one product per multiply-add); the %s split "
                                 "executes 3 tensor-core MMAs per product, so tensor-pipe flops are 3x achieved"
                                 % {"3xtf32": "3xTF32", "3xf16": "3xFP16"}[args.mlp])
             roofline["executed_tflops"] = round(3 * ach, 3)
+            roofline["executed_frac"] = round(3 * ach / peak, 4)
 
     # ---- end to end through the host-buffer entry ----------------------------------------------
     e2e_steps = max(3, min(args.steps, 10))
@@ -458,20 +547,44 @@ def run_ours(args):
     hfrc = torch.empty(N, 3, dtype=torch.float32).pin_memory()
     sysm.build_neighbors(pos0, w.cell9, w.pbc, w.model.r_cut, w.skin)
     hp_np, hf_np = hpos.numpy(), hfrc.numpy()
+    if mode == "ensemble":
+        # the ensemble call has no host-buffer entry: positions from pinned memory in, the four statistics out, every call
+        dpos = torch.empty_like(pos0)
+        houts = [torch.empty(N, dtype=torch.float32).pin_memory(), torch.empty(N, dtype=torch.float32).pin_memory(),
+                 torch.empty(N, 3, dtype=torch.float32).pin_memory(), torch.empty(N, 3, dtype=torch.float32).pin_memory()]
+
+        def e2e_call():
+            dpos.copy_(hpos, non_blocking=True)
+            outs = sysm.ensemble_energy_forces(dpos)
+            for h, o in zip(houts, outs):
+                h.copy_(o, non_blocking=True)
+            torch.cuda.synchronize()
+
+        d2h = 32 * N
+    else:
+        def e2e_call():
+            sysm.energy_forces_host(hp_np, hf_np)
+
+        d2h = 12 * N + 8
     for _ in range(2):
-        sysm.energy_forces_host(hp_np, hf_np)
+        e2e_call()
     barrier()
     t0 = time.perf_counter()
     for _ in range(e2e_steps):
-        e_host = sysm.energy_forces_host(hp_np, hf_np)
+        e2e_call()
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
     e2e = {"value": world * N * e2e_steps / max_over_ranks(e2e_s, world, dev), "unit": UNIT, "h2d_bytes_per_step": 12 * N,
-           "d2h_bytes_per_step": 12 * N + 8, "steps": e2e_steps,
-           "what": "gmnn_energy_forces_host: pinned positions in, forces and total energy out, every step"}
+           "d2h_bytes_per_step": d2h, "steps": e2e_steps,
+           "what": ("gmnn_ensemble_energy_forces: pinned positions in, e_mean, e_var, f_mean, f_var out, every call" if mode == "ensemble"
+                    else "gmnn_energy_forces_host: pinned positions in, forces and total energy out, every step")}
     sysm.check()
 
     if rank == 0:
+        what = {"md": w.name + ", %s velocity Verlet, dt %.2f fs, skin %.1f" % (
+                    "NVT (Nose-Hoover chain 3/2/3, %g K)" % args.nvt if args.nvt > 0 else "NVE", w.dt_fs, w.skin),
+                "ef": w.name + ", one gmnn_energy_forces call per step on a prebuilt list (skin %.1f)" % w.skin,
+                "ensemble": w.name + ", one gmnn_ensemble_energy_forces call per step (%d heads: e_mean, e_var, f_mean, f_var)" % w.model.n_heads}[mode]
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -479,13 +592,13 @@ def run_ours(args):
                       "3xf16": "f32 (MLP: 3xFP16 split on tcgen05, fp32 accumulate)",
                       "tf32": "tf32 MLP, f32 elsewhere"}[args.mlp],
             "data": "synthetic",
-            "config": {"workload": args.workload, "n_atoms": N, "what": w.name + ", %s velocity Verlet, dt %.2f fs, skin %.1f"
-                       % ("NVT (Nose-Hoover chain 3/2/3, %g K)" % args.nvt if args.nvt > 0 else "NVE", w.dt_fs, w.skin), "mlp": args.mlp, "forces": args.forces, "hidden": list(w.model.hidden), "n_heads": w.model.n_heads,
-                       "weight_sets": w.model.n_weight_sets,
+            "config": {"workload": args.workload, "step": mode, "n_atoms": N, "what": what, "mlp": args.mlp, "forces": args.forces,
+                       "hidden": list(w.model.hidden), "n_heads": w.model.n_heads, "weight_sets": w.model.n_weight_sets,
                        "neighbors_in_list_mean": round(nl_mean, 2), "rebuilds_in_timed_region": nreb,
                        "l2": "inputs_exceed_l2" if N >= 65536 else "working set of this small case is L2-resident",
                        "replicas": world},
             "gpu_launches": launches, "clocks": clocks, "e2e": e2e, "roofline": roofline, "stages": stage_out,
+            "peaks_measured_in_this_run": {k: round(v, 2) for k, v in run_peaks.items()},
             "energy_drift_ev_per_atom": drift, "ns_per_atom_step": ms_max * 1e6 / args.steps / N,
         }
         if world == 1 and not args.no_cpu_baseline:
@@ -504,8 +617,11 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="config5",
-                    help="config5 (default, 1,048,576 atoms), config2, config3_<N>; config4_switching: side measurement of "
-                         "the switching-mode ensemble MD (its own JSON line)")
+                    help="config5 (default, 1,048,576 atoms), config2, config3_<N>; config4: one gmnn_ensemble_energy_forces call per "
+                         "step (32 heads); config4_switching: side measurement of the switching-mode ensemble MD (its own JSON line)")
+    ap.add_argument("--ef", action="store_true",
+                    help="a step is one gmnn_energy_forces call on a prebuilt list instead of one MD step (BASELINE.json config 3: "
+                         "energy+forces throughput per N)")
     ap.add_argument("--mlp", default="3xf16", choices=sorted(MLP_NAMES),
                     help="3xf16 (default) / 3xtf32: tcgen05 tensor cores, fp32-accurate three-product split on fp16 / tf32 "
                          "operands; fp32: SIMT FMA; tf32: single pass")

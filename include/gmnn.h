@@ -300,6 +300,10 @@ int gmnn_stage_times(gmnn_system *s, int32_t max_stages, const char **names /*HO
  * Synchronous. */
 int gmnn_debug_read(gmnn_system *s, const char *name, void *dst /*HOST*/, int64_t bytes);
 
+/* Calibration for bench.py's roofline: the fp32 FMA rate (TFLOP/s, 2 flop per FMA) the current device sustains now, from
+ * a register-only kernel of independent FMA chains on every SM (about 10 ms; best of three).  HOST double.  Synchronises. */
+int gmnn_measure_fp32_peak(double *tflops /*HOST*/, void *cuda_stream);
+
 /* Number of kernel launches issued by this library since it was loaded (bench.py's gpu_launches). */
 int64_t gmnn_launch_count(void);
 

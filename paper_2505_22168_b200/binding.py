@@ -32,7 +32,7 @@ EXPORTS = (
     "gmnn_n_features", "gmnn_create", "gmnn_destroy", "gmnn_system_create", "gmnn_system_destroy",
     "gmnn_system_set_int", "gmnn_system_get_int", "gmnn_build_neighbors", "gmnn_get_neighbors", "gmnn_get_neighbor_rows",
     "gmnn_energy_forces", "gmnn_energy_forces_virial", "gmnn_energy_forces_host", "gmnn_ensemble_energy_forces", "gmnn_md_verlet_steps", "gmnn_md_ensemble_steps", "gmnn_system_set_langevin", "gmnn_system_set_temperature_schedule", "gmnn_system_set_nose_hoover", "gmnn_system_get_nose_hoover", "gmnn_system_set_udd_bias", "gmnn_system_get_udd_bias",
-    "gmnn_check", "gmnn_stage_times", "gmnn_debug_read", "gmnn_launch_count", "gmnn_last_error",
+    "gmnn_check", "gmnn_measure_fp32_peak", "gmnn_stage_times", "gmnn_debug_read", "gmnn_launch_count", "gmnn_last_error",
 )
 
 
@@ -107,6 +107,13 @@ lib = _load()
 def _check(rc: int) -> None:
     if rc != GMNN_OK:
         raise GmnnError(rc, (lib.gmnn_last_error() or b"").decode())
+
+
+def measure_fp32_peak(stream=None) -> float:
+    """TFLOP/s of fp32 FMA the current device sustains now (gmnn_measure_fp32_peak)."""
+    v = C.c_double(0)
+    _check(lib.gmnn_measure_fp32_peak(C.byref(v), _stream_ptr(stream)))
+    return float(v.value)
 
 
 def launch_count() -> int:

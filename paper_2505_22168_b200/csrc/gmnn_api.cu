@@ -1246,6 +1246,39 @@ int gmnn_system_get_udd_bias(gmnn_system *s, double *e_bias, double *var_e, void
     return GMNN_OK;
 }
 
+int gmnn_measure_fp32_peak(double *tflops, void *cuda_stream) {
+    if (!tflops) return GMNN_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int dev = 0, sms = 0;
+    GMNN_CUDA(cudaGetDevice(&dev));
+    GMNN_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    const int blocks = sms * 8, iters = 4096;  // 8 blocks of 256 threads per SM: 16 warps per scheduler, 16 chains each
+    float *scratch = nullptr;
+    int rc = dev_alloc(&scratch, (size_t)blocks * 256);
+    if (rc) return rc;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0);
+    cudaEventCreate(&e1);
+    rc = launch_fma_peak(blocks, 64, scratch, st);  // warm-up
+    double best = 0.0;
+    for (int rep = 0; rep < 3 && !rc; ++rep) {
+        cudaEventRecord(e0, st);
+        rc = launch_fma_peak(blocks, iters, scratch, st);
+        cudaEventRecord(e1, st);
+        if (cudaEventSynchronize(e1) != cudaSuccess) rc = GMNN_CUDA_ERROR;
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        const double tf = 2.0 * 128.0 * (double)iters * 256.0 * (double)blocks / ((double)ms * 1e-3) / 1e12;
+        if (tf > best) best = tf;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    dev_free(scratch);
+    if (rc) return rc;
+    *tflops = best;
+    return GMNN_OK;
+}
+
 int gmnn_check(gmnn_system *s, void *cuda_stream) {
     if (!s) return GMNN_INVALID_ARG;
     cudaStream_t st = (cudaStream_t)cuda_stream;

@@ -278,7 +278,8 @@ int launch_ensemble_energy_stats(gmnn_system *s, float *e_mean, float *e_var, cu
 int launch_finish_var(int64_t n, float *m2, int n_heads, cudaStream_t st);
 int launch_baoab(gmnn_system *s, float *x, float *v, const float *f, const float *m, float dt, cudaStream_t st);
 int launch_nhc_half(gmnn_system *s, float *v, double *ek, float dt, cudaStream_t st);
-int launch_schedule_eval(gmnn_system *s, cudaStream_t st);  // kT_now <- k_B T(step), step += 1
+int launch_schedule_eval(gmnn_system *s, cudaStream_t st);
+int launch_fma_peak(int blocks, int iters, float *scratch, cudaStream_t st);  // blocks x 256 threads x iters x 128 FMA  // kT_now <- k_B T(step), step += 1
 int launch_udd_weights(gmnn_system *s, float *head_w_out, double *scal, cudaStream_t st);
 int launch_uncertainty_scalars(gmnn_system *s, const float *f_var, double *out_d, int32_t *out_bits, cudaStream_t st);
 

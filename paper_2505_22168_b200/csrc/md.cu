@@ -525,4 +525,32 @@ int launch_baoab(gmnn_system *s, float *x, float *v, const float *f, const float
     return GMNN_OK;
 }
 
+
+// ---- calibration: the fp32 FMA rate this GPU sustains right now (bench.py's "alu" roof, measured in the same run) ----
+// Every thread runs 16 independent dependent-FMA chains (registers only); 2 flop per FMA.  The result is stored so that
+// nothing is optimised away.
+__global__ void __launch_bounds__(256) k_fma_peak(int iters, float seed, float *out) {
+    float a[16];
+#pragma unroll
+    for (int q = 0; q < 16; ++q) a[q] = seed + (float)(threadIdx.x + q);
+    const float b = 1.0000001f, c = 1e-7f;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int u = 0; u < 8; ++u)
+#pragma unroll
+            for (int q = 0; q < 16; ++q) a[q] = fmaf(a[q], b, c);
+    }
+    float sum = 0.f;
+#pragma unroll
+    for (int q = 0; q < 16; ++q) sum += a[q];
+    if (sum == 12345.678f) out[blockIdx.x * blockDim.x + threadIdx.x] = sum;  // practically never: keeps the chains alive
+}
+
+int launch_fma_peak(int blocks, int iters, float *scratch, cudaStream_t st) {
+    k_fma_peak<<<blocks, 256, 0, st>>>(iters, 1.0f, scratch);
+    GMNN_LAUNCHED();
+    GMNN_CUDA(cudaGetLastError());
+    return GMNN_OK;
+}
+
 }  // namespace gmnn
