@@ -154,7 +154,7 @@ template <int NR, int HALVES, bool LOCKSTEP, bool ORBIT>
 __global__ void __launch_bounds__(128 * HALVES, 3 - HALVES)
 k_contract_backward(int64_t N, const float *__restrict__ psi, const float *__restrict__ dGt,
                     const float4 *__restrict__ pos4, const float *__restrict__ scale, float *__restrict__ A,
-                    const int32_t *__restrict__ row_atom) {
+                    const int32_t *__restrict__ row_atom, int heads) {
     using F = Feat<NR>;
     using CH = FeatChunks<NR>;
     using SM = CbSmem<NR>;
@@ -164,10 +164,15 @@ k_contract_backward(int64_t N, const float *__restrict__ psi, const float *__res
     float *sX = s_cb + hf * (SM::X + SM::Y), *sY = sX + SM::X;
     const uint32_t barX = tc::smem_u32(s_cb + HALVES * (SM::X + SM::Y)) + 16 * hf, barY = barX + 8;
     const int tid = threadIdx.x & 127, lane = tid & 31, wid = tid >> 5;
-    const int64_t tile = blockIdx.x * (int64_t)HALVES + hf;
+    // heads > 1 (batched shallow ensemble, gmnn_api.cu): row tile rt = atom tile * heads + head holds dE^(head)/dG of the
+    // atoms of tile rt / heads; Psi and sigma are the atom's, the adjoints go to row rt * 128 + tid of A.  N counts atoms
+    // (rows of psi); dGt / A are then the batched buffers.
+    const int64_t rtile = blockIdx.x * (int64_t)HALVES + hf;
+    const int64_t tile = heads > 1 ? rtile / heads : rtile;
     const bool active = tile * TB < N;  // the last block of an odd tile count has an idle half
     const int64_t i = tile * TB + tid;
-    const float *gt = dGt + tile * (int64_t)(F::N * TB);  // this half's [F][128] tile
+    const float *gt = dGt + rtile * (int64_t)(F::N * TB);  // this half's [F][128] tile
+
     auto issue = [&](float *dst, int c, uint32_t bar) {
         tc::bulk_load_1d(tc::smem_u32(dst), gt + CH::begin(c) * TB, (uint32_t)(SM::len(c) * TB * 4), bar);
     };
@@ -274,7 +279,7 @@ k_contract_backward(int64_t N, const float *__restrict__ psi, const float *__res
     for (int a = 0; a < 32; ++a) {
         const int64_t ia = i0 + a;
         if (ia >= N) break;
-        float *dst = A + ia * (int64_t)(NR * PSI);
+        float *dst = A + (rtile * TB + (ia - tile * TB)) * (int64_t)(NR * PSI);
         for (int q = lane; q < NR * PSI; q += 32) dst[q] = sP[q * CW + a];
     }
 }
@@ -305,9 +310,11 @@ static int launch_cb(gmnn_system *s, cudaStream_t st) {
                                        cudaFuncAttributeMaxDynamicSharedMemorySize, (int)CbSmem<NR>::bytes(HALVES)));
         attr_set = true;
     }
-    const unsigned tiles = nblocks(s->n_rows, 128);
+    const int heads = s->ens_batch > 1 ? s->ens_batch : 1;  // batched ensemble pass: dG / A of `heads` heads per atom tile
+    const unsigned tiles = nblocks(s->n_rows, 128) * heads;
     k_contract_backward<NR, HALVES, LOCKSTEP, ORBIT><<<(tiles + HALVES - 1) / HALVES, 128 * HALVES, CbSmem<NR>::bytes(HALVES), st>>>(
-        s->n_rows, s->psi, s->dG, s->pos4, s->model->scale, s->A, s->row_atom);
+        s->n_rows, s->psi, heads > 1 ? s->ens_dG : s->dG, s->pos4, s->model->scale, heads > 1 ? s->ens_A : s->A, s->row_atom,
+        heads);
     GMNN_LAUNCHED();
     GMNN_CUDA(cudaGetLastError());
     return GMNN_OK;

@@ -144,16 +144,59 @@ static int ensemble_pass(gmnn_system *s, const float *positions, float *e_mean, 
     if ((rc = mlp_forward(s, st))) return rc;
     if ((rc = launch_mlp_heads(s, s->model->head_mean_w, st))) return rc;
     if ((rc = launch_ensemble_energy_stats(s, e_mean, e_var, st))) return rc;
-    for (int m = 0; m < M; ++m) {
-        k_set_onehot<<<1, 64, 0, st>>>(M, m, s->head_w);
-        GMNN_LAUNCHED();
-        if (s->mlp_precision == GMNN_MLP_3XF16 && m > 0)  // dZ maxima belong to one head's backward
+    // Heads batched through the backward GEMMs and the contraction backward (mlp_tc.cu launch_mlp_backward_tc_heads): as many
+    // heads per pass as 2 GB of batch buffers hold; tensor-core split modes with one weight set.  Else head by head.
+    const gmnn_model *mdl = s->model;
+    const int L = mdl->hp.n_hidden;
+    int HB = 1;
+    if (M > 1 && mdl->n_sets == 1 && (s->mlp_precision == GMNN_MLP_3XF16 || s->mlp_precision == GMNN_MLP_3XTF32)) {
+        int maxw = 0;
+        for (int l = 1; l <= L; ++l) maxw = std::max(maxw, mdl->dims[l]);
+        const size_t NP = (size_t)((s->N + 127) / 128 * 128);
+        const double per_head = (double)NP * (2.0 * maxw + mdl->n_features + mdl->hp.n_radial * PSI) * 4.0;
+        HB = (int)std::min<double>((double)M, std::floor(2.0e9 / per_head));
+        if (HB >= 2 && s->ens_cap < HB) {
+            dev_free(s->ens_dZ[0]); dev_free(s->ens_dZ[1]); dev_free(s->ens_dG); dev_free(s->ens_A);
+            dev_free(s->ens_BvT); dev_free(s->ens_BvTs); dev_free(s->ens_BvTh);
+            s->ens_cap = 0;
+            const size_t bv = (size_t)mdl->dims[L] * mdl->dims[L - 1] * HB;
+            if ((rc = dev_alloc(&s->ens_dZ[0], NP * HB * maxw)) || (rc = dev_alloc(&s->ens_dZ[1], NP * HB * maxw)) ||
+                (rc = dev_alloc(&s->ens_dG, NP * HB * mdl->n_features)) ||
+                (rc = dev_alloc(&s->ens_A, NP * HB * mdl->hp.n_radial * PSI)) || (rc = dev_alloc(&s->ens_BvT, bv)) ||
+                (rc = dev_alloc(&s->ens_BvTs, 2 * bv)) || (rc = dev_alloc(&s->ens_BvTh, 2 * bv))) {
+                set_error("out of device memory for the batched ensemble buffers (%d heads x %lld atoms)", HB, (long long)s->N);
+                return rc;
+            }
+            s->ens_cap = HB;
+        }
+    }
+    struct BatchOff {  // the batch state never outlives the pass
+        gmnn_system *s;
+        ~BatchOff() { s->ens_batch = 0, s->ens_head = 0; }
+    } batch_off{s};
+    for (int m0 = 0; m0 < M; m0 += HB) {
+        const int hb = std::min(HB, M - m0);
+        if (s->mlp_precision == GMNN_MLP_3XF16 && m0 > 0)  // dZ maxima belong to one backward pass
             GMNN_CUDA(cudaMemsetAsync(s->amax + AMAX_DZ, 0, sizeof(uint32_t) * 2, st));
-        if ((rc = mlp_backward(s, s->head_w, st))) return rc;
-        if ((rc = launch_contract_backward(s, st))) return rc;
-        if ((rc = launch_pair_backward(s, st))) return rc;
-        if ((rc = launch_scatter_outputs(s, nullptr, s->f_tmp, st))) return rc;
-        if ((rc = launch_welford(s, m, s->f_tmp, f_mean, f_var, st))) return rc;
+        if (HB >= 2) {
+            if ((rc = launch_mlp_backward_tc_heads(s, m0, hb, st))) return rc;
+            s->ens_batch = hb;
+            if ((rc = launch_contract_backward(s, st))) return rc;
+        }
+        for (int mm = 0; mm < hb; ++mm) {
+            const int m = m0 + mm;
+            if (HB >= 2) {
+                s->ens_head = mm;
+            } else {
+                k_set_onehot<<<1, 64, 0, st>>>(M, m, s->head_w);
+                GMNN_LAUNCHED();
+                if ((rc = mlp_backward(s, s->head_w, st))) return rc;
+                if ((rc = launch_contract_backward(s, st))) return rc;
+            }
+            // pair backward of head m; its force goes straight into the statistics over the heads (no scatter, no store)
+            if ((rc = launch_pair_backward_welford(s, m, f_mean, f_var, st))) return rc;
+        }
+        s->ens_batch = 0;
     }
     if ((rc = launch_finish_var(3 * s->N, f_var, M, st))) return rc;
     GMNN_CUDA(cudaGetLastError());
@@ -465,6 +508,8 @@ void gmnn_system_destroy(gmnn_system *s) {
     dev_free(s->dZ[0]); dev_free(s->dZ[1]); dev_free(s->Bv); dev_free(s->BvT); dev_free(s->BvTs); dev_free(s->BvTh); dev_free(s->amax); dev_free(s->vhead); dev_free(s->head_w);
     dev_free(s->ypart); dev_free(s->e_heads); dev_free(s->e_atom); dev_free(s->f_int); dev_free(s->f_tmp); dev_free(s->partial);
     dev_free(s->e_total); dev_free(s->flags); dev_free(s->ens_scratch); dev_free(s->nhc); dev_free(s->lang_step);
+    dev_free(s->ens_dZ[0]); dev_free(s->ens_dZ[1]); dev_free(s->ens_dG); dev_free(s->ens_A);
+    dev_free(s->ens_BvT); dev_free(s->ens_BvTs); dev_free(s->ens_BvTh);
     dev_free(s->kT_now); dev_free(s->sched_steps); dev_free(s->sched_temps); dev_free(s->sched_step);
     dev_free(s->stage_pos); dev_free(s->stage_f); dev_free(s->stage_e);
     if (s->flags_host) cudaFreeHost(s->flags_host);

@@ -194,6 +194,12 @@ struct gmnn_system {
     float *f_tmp = nullptr;          // [N][3] caller order (ensemble, MD)
     double *partial = nullptr;       // reduction scratch
     double *e_total = nullptr;       // [6] device scalars (epot, ekin, sigma_E, bits of sigma_F,max, E_b, sigma_E^2 of the bias)
+    // batched shallow-ensemble backward (gmnn_api.cu ensemble_pass): ens_batch heads per pass in buffers whose row tiles
+    // are ordered [atom tile][head]; 0 / 1 outside such a pass.  ens_head: the head the pair backward reads.
+    int ens_batch = 0, ens_head = 0, ens_cap = 0;  // ens_cap: heads the buffers below hold
+    float *ens_dZ[2] = {}, *ens_dG = nullptr, *ens_A = nullptr;
+    float *ens_BvT = nullptr, *ens_BvTs = nullptr;
+    uint16_t *ens_BvTh = nullptr;
     float *ens_scratch = nullptr;    // [11 N] switching-mode samples: kept forces, e_mean, e_var, f_mean, f_var (lazy)
     int32_t *flags = nullptr;        // FLAG_WORDS
     int32_t *flags_host = nullptr;   // pinned
@@ -250,6 +256,7 @@ int launch_pair_forward(gmnn_system *s, cudaStream_t st);
 int launch_contract_forward(gmnn_system *s, cudaStream_t st);
 int launch_contract_backward(gmnn_system *s, cudaStream_t st);
 int launch_pair_backward(gmnn_system *s, cudaStream_t st);  // dispatches on force_mode
+int launch_pair_backward_welford(gmnn_system *s, int head, float *f_mean, float *f_m2, cudaStream_t st);  // a12, one head
 
 // mlp_tc.cu
 int launch_split_stack(const float *src, float *dst, int64_t n, cudaStream_t st);  // dst[0..n) hi, dst[n..2n) lo
@@ -261,6 +268,7 @@ int launch_mlp_forward_simt(gmnn_system *s, cudaStream_t st);
 int launch_mlp_heads(gmnn_system *s, const float *head_w_dev, cudaStream_t st);
 int launch_mlp_seed(gmnn_system *s, const float *head_w_dev, cudaStream_t st);
 int launch_mlp_backward_simt(gmnn_system *s, const float *head_w_dev, cudaStream_t st);
+int launch_mlp_backward_tc_heads(gmnn_system *s, int head0, int n_heads, cudaStream_t st);  // mlp_tc.cu: heads batched
 
 // md.cu / reductions
 int launch_scatter_outputs(gmnn_system *s, float *e_atom_out, float *forces_out, cudaStream_t st);
@@ -273,7 +281,6 @@ int launch_ke(gmnn_system *s, const float *v, const float *m, double *ekin_out, 
               double *ekin_out2 = nullptr);
 int launch_series_append(gmnn_system *s, double *epot_series, double *ekin_series, cudaStream_t st);
 int launch_series_reset(gmnn_system *s, int32_t next_index, cudaStream_t st);
-int launch_welford(gmnn_system *s, int head, const float *f_head, float *f_mean, float *f_m2, cudaStream_t st);
 int launch_ensemble_energy_stats(gmnn_system *s, float *e_mean, float *e_var, cudaStream_t st);
 int launch_finish_var(int64_t n, float *m2, int n_heads, cudaStream_t st);
 int launch_baoab(gmnn_system *s, float *x, float *v, const float *f, const float *m, float dt, cudaStream_t st);

@@ -109,22 +109,6 @@ k_kick(int64_t N, float *v, const float *__restrict__ f, const float *__restrict
 }
 
 // Welford update in head order: after head h (0-based), mean/M2 of heads 0..h.
-__global__ void k_welford(int64_t n, int head, const float *__restrict__ x, float *mean, float *m2) {
-    const int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    if (t >= n) return;
-    const float v = x[t];
-    if (head == 0) {
-        mean[t] = v;
-        m2[t] = 0.f;
-    } else {
-        const float mu = mean[t];
-        const float d = v - mu;
-        const float mu2 = mu + d / (float)(head + 1);
-        mean[t] = mu2;
-        m2[t] = fmaf(d, v - mu2, m2[t]);
-    }
-}
-
 __global__ void k_finish_var(int64_t n, float *m2, float inv_heads) {
     const int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (t < n) m2[t] *= inv_heads;
@@ -238,13 +222,6 @@ int launch_series_append(gmnn_system *s, double *epot_series, double *ekin_serie
 
 int launch_series_reset(gmnn_system *s, int32_t next_index, cudaStream_t st) {
     k_set_int<<<1, 1, 0, st>>>(s->flags + FLAG_MD_STEP, next_index);
-    GMNN_LAUNCHED();
-    GMNN_CUDA(cudaGetLastError());
-    return GMNN_OK;
-}
-
-int launch_welford(gmnn_system *s, int head, const float *f_head, float *f_mean, float *f_m2, cudaStream_t st) {
-    k_welford<<<nblocks(3 * s->N, 256), 256, 0, st>>>(3 * s->N, head, f_head, f_mean, f_m2);
     GMNN_LAUNCHED();
     GMNN_CUDA(cudaGetLastError());
     return GMNN_OK;

@@ -91,7 +91,9 @@ struct TcArgs {
     float *C;      // [M][N]
     float *C2;     // EPI_HIDDEN: swish'(z)
     const float *bias;
-    const float *Dmul;  // EPI_MUL: [M][N]
+    const float *Dmul;  // EPI_MUL: [M][N]; batched ensemble backward: row tile rt reads row tile rt / dmul_row_div and column
+                        // c reads column c % dmul_N of a multiplier that is [M / dmul_row_div][dmul_N]
+    int dmul_N, dmul_row_div;
     const float *w_head;  // EPI_HIDDEN_HEAD: [N] weights of the single head
     float *ypart;         // EPI_HIDDEN_HEAD: [2 * n_tiles_n][m_pad]
     int64_t m_pad;
@@ -226,8 +228,10 @@ __device__ __forceinline__ void tc_store_tile(const TcArgs &p, float (&acc)[4][3
                         if (SCALED) tmax = fmaxf(tmax, fabsf(h[c]));
                     }
             } else if (EPI == EPI_MUL) {
+                const int64_t om = (int64_t)((m0 / TC_BM) / p.dmul_row_div) * p.dmul_N * TC_BM + quad * 32 + lane +
+                                   (int64_t)((col0 + j0) % p.dmul_N) * TC_BM;
 #pragma unroll
-                for (int c = 0; c < TC_EB; ++c) in[c] = c < nc ? __ldg(Dmul + o + c * TC_BM) : 0.f;
+                for (int c = 0; c < TC_EB; ++c) in[c] = c < nc ? __ldg(Dmul + om + c * TC_BM) : 0.f;
 #pragma unroll
                 for (int c = 0; c < TC_EB; ++c)
                     if (c < nc) {
@@ -649,7 +653,8 @@ k_gemm_tc_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                     // the multiplier block of this tile (swish' of the layer below: bn columns x 128 rows, contiguous in both
                     // layouts) is read by the epilogue at the END of the tile, from HBM: bring it into L2 now
                     const int cols = p.N - n0 < p.bn ? p.N - n0 : p.bn;
-                    const char *blk = reinterpret_cast<const char *>(p.Dmul + ((int64_t)mt * p.N + n0) * TC_BM);
+                    const char *blk = reinterpret_cast<const char *>(
+                        p.Dmul + ((int64_t)(mt / p.dmul_row_div) * p.dmul_N + n0 % p.dmul_N) * TC_BM);
                     for (int c = 0; c < cols; c += 64) bulk_prefetch_l2(blk + (int64_t)c * TC_BM * 4, (uint32_t)((cols - c < 64 ? cols - c : 64) * TC_BM * 4));
                 }
                 for (int kb = 0; kb < nkb; ++kb, ++it) {
@@ -1041,7 +1046,7 @@ struct TcHalf {
 // `hf` (3xFP16, always on CTA pairs) the fp16 split hf->Bh replaces Bt.
 int tc_gemm(bool split, int epi, int64_t M, int N, int K, const float *A, const float *Bt, float *C, const float *bias,
             float *C2, const float *Dmul, cudaStream_t st, const float *w_head = nullptr, float *ypart = nullptr,
-            int *n_slots = nullptr, const TcHalf *hf = nullptr, int64_t m_pad_total = 0) {
+            int *n_slots = nullptr, const TcHalf *hf = nullptr, int64_t m_pad_total = 0, int dmul_N = 0, int dmul_row_div = 1) {
     if (K % 8 != 0 || N % 8 != 0 || M <= 0 || M > INT32_MAX) {
         set_error("tensor-core MLP: widths must be multiples of 8 (K = %d, N = %d)", K, N);
         return GMNN_UNSUPPORTED;
@@ -1070,6 +1075,7 @@ int tc_gemm(bool split, int epi, int64_t M, int N, int K, const float *A, const 
     a.debug = 0;
 #endif
     a.C = C, a.C2 = C2, a.bias = bias, a.Dmul = Dmul;
+    a.dmul_N = dmul_N > 0 ? dmul_N : N, a.dmul_row_div = dmul_row_div > 0 ? dmul_row_div : 1;
     // ypart is [slots][m_pad]: with row segments the caller hands ypart + row0 and the padded row count of the whole matrix
     a.w_head = w_head, a.ypart = ypart, a.m_pad = m_pad_total > 0 ? m_pad_total : (M + TC_BM - 1) / TC_BM * TC_BM;
     a.amax_a = hf ? hf->amax_a : nullptr, a.amax_b = hf ? hf->amax_b : nullptr, a.amax_out = hf ? hf->amax_out : nullptr;
@@ -1249,6 +1255,71 @@ int launch_mlp_backward_tc(gmnn_system *s, const float *head_w_dev, cudaStream_t
             cur ^= 1;
         }
     }
+    return GMNN_OK;
+}
+
+
+// ---- batched shallow-ensemble backward (a12; Eq. 5, 6) -------------------------------------------------
+// The backward of head m differs from that of any other head only in the seed v_m = W_last[:, m].  For HB heads at once:
+//   first GEMM  (seeded): dZ[rows][HB x w] = D_last[rows][Hd] . [B_0 | B_1 | ... ]^T-stacked, B_m = W[L-1] diag(v_m), one wide
+//               GEMM whose column block m is head m (its swish' multiplier is read with column c % w);
+//   its output, tile-transposed [row tile][HB x w][128], IS a matrix of HB x as many row tiles of width w, ordered
+//               [atom tile][head]: the GEMMs below it run on those stacked rows with the shared weights, and so does the
+//               contraction backward (descriptor.cu, `heads`); the pair backward of head m reads rows [tile][m] (a_heads).
+// 32 heads x 8 192 atoms become GEMMs of 16 384 columns / 262 144 rows that fill the machine, instead of 32 under-filled ones.
+__global__ void k_seed_heads(int prev, int Hd, const float *__restrict__ W, const float *__restrict__ Wlast, int M, int head0,
+                             int HB, float *__restrict__ out) {
+    const int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;  // out[m][n][k] = W[n][k] Wlast[k][head0 + m]
+    const int64_t per = (int64_t)prev * Hd;
+    if (t >= per * HB) return;
+    const int m = (int)(t / per);
+    const int k = (int)(t % Hd);
+    out[t] = __ldg(&W[t % per]) * __ldg(&Wlast[(int64_t)k * M + head0 + m]);
+}
+
+int launch_mlp_backward_tc_heads(gmnn_system *s, int head0, int HB, cudaStream_t st) {
+    const gmnn_model *m = s->model;
+    const bool f16 = s->mlp_precision == GMNN_MLP_3XF16;
+    const int L = m->hp.n_hidden, M = m->hp.n_heads;
+    const int Hd = m->dims[L], prev = m->dims[L - 1];
+    const int64_t nbv = (int64_t)prev * Hd * HB;
+    int rc;
+    k_seed_heads<<<(unsigned)((nbv + 255) / 256), 256, 0, st>>>(prev, Hd, m->W[L - 1], m->W[L], M, head0, HB, s->ens_BvT);
+    GMNN_LAUNCHED();
+    if (f16) {
+        if ((rc = launch_absmax(s->ens_BvT, nbv, s->amax + AMAX_BVT, st))) return rc;
+        if ((rc = launch_split_stack_h(s->ens_BvT, s->ens_BvTh, nbv, s->amax + AMAX_BVT, st))) return rc;
+    } else if ((rc = launch_split_stack(s->ens_BvT, s->ens_BvTs, nbv, st))) {
+        return rc;
+    }
+    const int64_t rows = s->N, row_tiles = (rows + TC_BM - 1) / TC_BM;
+    const float *Aop = s->D[L - 1];
+    int cur = 0;
+    for (int l = L - 1; l >= 0; --l) {
+        const int fo = m->dims[l], fi = m->dims[l + 1];
+        const bool seeded = l == L - 1;
+        // seeded: [rows] x [HB fo] = [rows][fi] . stacked seeds; below: [row_tiles HB 128] x [fo] with the shared W[l]
+        const int64_t Mrows = seeded ? rows : row_tiles * HB * TC_BM;
+        const int Ncols = seeded ? HB * fo : fo;
+        TcHalf hf;
+        hf.Bh = seeded ? s->ens_BvTh : m->Wh[l];
+        hf.amax_b = seeded ? s->amax + AMAX_BVT : m->wmax + l;
+        hf.amax_a = seeded ? s->amax + AMAX_D : s->amax + AMAX_DZ + (cur ^ 1);
+        const float *BopT = seeded ? s->ens_BvTs : m->Ws[l];
+        if (l > 0) {
+            hf.amax_out = s->amax + AMAX_DZ + cur;
+            rc = tc_gemm(true, EPI_MUL, Mrows, Ncols, fi, Aop, BopT, s->ens_dZ[cur], nullptr, nullptr, s->D[l - 1], st, nullptr, nullptr,
+                         nullptr, f16 ? &hf : nullptr, 0, fo, seeded ? 1 : HB);
+            Aop = s->ens_dZ[cur];
+            cur ^= 1;
+        } else {
+            hf.amax_out = nullptr;
+            rc = tc_gemm(true, EPI_PLAIN, Mrows, Ncols, fi, Aop, BopT, s->ens_dG, nullptr, nullptr, nullptr, st, nullptr, nullptr, nullptr,
+                         f16 ? &hf : nullptr);
+        }
+        if (rc) return rc;
+    }
+    GMNN_CUDA(cudaGetLastError());
     return GMNN_OK;
 }
 

@@ -74,7 +74,7 @@ k_pair_backward(int64_t N, const float4 *__restrict__ pos4, const uint32_t *__re
                 const int32_t *__restrict__ count, int cap, Geometry geo, RadialParams rp,
                 const float *__restrict__ beta, const float *__restrict__ A, float *__restrict__ f_int,
                 const uint16_t *__restrict__ rev, float4 *__restrict__ gbuf, const int32_t *__restrict__ mrow,
-                float *__restrict__ vir_atom) {
+                float *__restrict__ vir_atom, int a_heads, int a_head) {
     constexpr int KB = (NB + 3) & ~3;
     constexpr int ROW = NR * KB;
     constexpr int GROUPS = 128 / LPA;
@@ -93,7 +93,9 @@ k_pair_backward(int64_t N, const float4 *__restrict__ pos4, const uint32_t *__re
         const float4 *src = reinterpret_cast<const float4 *>(A);
         for (int q = threadIdx.x; q < GROUPS * (NR * PSI / 4); q += blockDim.x) {
             const int64_t ia = first + q / (NR * PSI / 4);
-            const int64_t ra = (mrow && ia < N) ? (int64_t)mrow[ia] : ia;  // row of the adjoint (species-grouped rows)
+            // row of the adjoint: species-grouped rows (mrow), or head a_head of the batched ensemble buffers
+            // ([atom tile][head][128] rows, gmnn_api.cu), else the atom itself
+            const int64_t ra = a_heads > 1 ? ((ia >> 7) * a_heads + a_head) * 128 + (ia & 127) : ((mrow && ia < N) ? (int64_t)mrow[ia] : ia);
             s_A[q] = ia < N ? __ldg(&src[ra * (NR * PSI / 4) + q % (NR * PSI / 4)]) : make_float4(0.f, 0.f, 0.f, 0.f);
         }
     }
@@ -169,8 +171,9 @@ k_pair_backward(int64_t N, const float4 *__restrict__ pos4, const uint32_t *__re
                             pair_gradient<NR>([&](int s, int qq) { return Ai[s * (PSI / 4) + qq]; }, R, dR, mono, ux, uy,
                                               uz, rinv, gxo, gyo, gzo);
                         } else {
-                            const float4 *Aj = reinterpret_cast<const float4 *>(A) +
-                                               (int64_t)(mrow ? mrow[pg.j] : pg.j) * (NR * PSI / 4);
+                            const int64_t rj = a_heads > 1 ? (((int64_t)pg.j >> 7) * a_heads + a_head) * 128 + (pg.j & 127)
+                                                           : (int64_t)(mrow ? mrow[pg.j] : pg.j);
+                            const float4 *Aj = reinterpret_cast<const float4 *>(A) + rj * (NR * PSI / 4);
                             float mono_r[PSI];  // the neighbour sees the bond reversed
                             monomials(-ux, -uy, -uz, mono_r);
                             float hx, hy, hz;  // gradient with respect to (-u): g_ji in the frame of d_ji = -d_ij
@@ -226,10 +229,27 @@ k_pair_backward(int64_t N, const float4 *__restrict__ pos4, const uint32_t *__re
 
 // a11 (pair-buffer form): F_i = sum_j g_ij (already in f_int) - sum_k gbuf[i][k], the g_ji received
 // from the neighbours, summed in slot order by LPA lanes (fixed order: bit-reproducible).
-template <int LPA>
+// WELFORD (shallow-ensemble pass, a12): the force of this head is not stored but goes straight into the running
+// mean / sum of squared deviations over the heads, at the caller's index perm[i] (Eq. 5: means first, then squared
+// deviations; same arithmetic as k_welford on the scattered forces, so the statistics are bit-identical).
+__device__ __forceinline__ void welford_update(int head, float v, float *mean, float *m2) {
+    if (head == 0) {
+        *mean = v;
+        *m2 = 0.f;
+    } else {
+        const float mu = *mean;
+        const float d = v - mu;
+        const float mu2 = mu + d / (float)(head + 1);
+        *mean = mu2;
+        *m2 = fmaf(d, v - mu2, *m2);
+    }
+}
+
+template <int LPA, bool WELFORD>
 __global__ void __launch_bounds__(256)
 k_force_reduce(int64_t N, const int32_t *__restrict__ count, int cap, const float4 *__restrict__ gbuf,
-               float *__restrict__ f_int) {
+               float *__restrict__ f_int, const int32_t *__restrict__ perm, int head, float *__restrict__ f_mean,
+               float *__restrict__ f_m2) {
     const int64_t gt = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     const int64_t i = gt / LPA;
     const int sub = (int)(gt % LPA);
@@ -249,19 +269,40 @@ k_force_reduce(int64_t N, const int32_t *__restrict__ count, int cap, const floa
         fz += __shfl_xor_sync(0xffffffffu, fz, o);
     }
     if (i < N && sub == 0) {
-        f_int[3 * i] -= fx;
-        f_int[3 * i + 1] -= fy;
-        f_int[3 * i + 2] -= fz;
+        if (WELFORD) {
+            const int64_t c = perm[i];
+            welford_update(head, f_int[3 * i] - fx, f_mean + 3 * c, f_m2 + 3 * c);
+            welford_update(head, f_int[3 * i + 1] - fy, f_mean + 3 * c + 1, f_m2 + 3 * c + 1);
+            welford_update(head, f_int[3 * i + 2] - fz, f_mean + 3 * c + 2, f_m2 + 3 * c + 2);
+        } else {
+            f_int[3 * i] -= fx;
+            f_int[3 * i + 1] -= fy;
+            f_int[3 * i + 2] -= fz;
+        }
     }
 }
 
+// gather form: the complete force of this head is in f_int; the Welford update alone
+__global__ void __launch_bounds__(256)
+k_welford_perm(int64_t N, const float *__restrict__ f_int, const int32_t *__restrict__ perm, int head,
+               float *__restrict__ f_mean, float *__restrict__ f_m2) {
+    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const int64_t c = perm[i];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) welford_update(head, f_int[3 * i + a], f_mean + 3 * c + a, f_m2 + 3 * c + a);
+}
+
+// wf_head >= 0: the ensemble pass of head wf_head; the force goes into the Welford statistics (f_mean, f_m2: caller order)
 template <int NR, int NB>
-static int pair_backward_lpa(gmnn_system *s, cudaStream_t st, int lpa) {
+static int pair_backward_lpa(gmnn_system *s, cudaStream_t st, int lpa, int wf_head = -1, float *f_mean = nullptr,
+                             float *f_m2 = nullptr) {
     const gmnn_model *m = s->model;
     const int beta_floats = (m->rp.n_species * m->rp.n_species * NR * m->rp.kb + 3) & ~3;
     const size_t smem = sizeof(float) * (beta_floats + (128 / lpa) * NR * PSI);
     const unsigned grid = nblocks(s->N * lpa, 128);
     const bool pairbuf = s->force_mode == GMNN_FORCE_PAIRBUF;
+    const int a_heads = s->ens_batch > 1 ? s->ens_batch : 1;  // batched ensemble pass: adjoints of head s->ens_head
     const bool virial = s->want_virial && s->vir_atom != nullptr;
     const bool general = virial || m->rp.basis_kind != 0 || m->rp.zbl_on;
     if (pairbuf && !(s->list_has_rev && s->rev && s->gbuf)) {
@@ -270,8 +311,9 @@ static int pair_backward_lpa(gmnn_system *s, cudaStream_t st, int lpa) {
     }
 #define GMNN_PB_LAUNCH(L, PB, GEN)                                                                         \
     k_pair_backward<NR, NB, L, PB, GEN><<<grid, 128, smem, st>>>(s->N, s->pos4, s->nbr, s->count, s->cap, s->geo, m->rp, \
-                                                                m->beta, s->A, s->f_int, PB ? s->rev : nullptr, \
-                                                                PB ? s->gbuf : nullptr, s->mrow, (GEN && virial) ? s->vir_atom : nullptr)
+                                                                m->beta, a_heads > 1 ? s->ens_A : s->A, s->f_int, PB ? s->rev : nullptr, \
+                                                                PB ? s->gbuf : nullptr, s->mrow, (GEN && virial) ? s->vir_atom : nullptr, \
+                                                                a_heads, s->ens_head)
 #define GMNN_PB(L)                                                                                         \
     case L: {                                                                                              \
         static size_t opted_on[MAX_DEVICES] = {};                                                          \
@@ -302,7 +344,15 @@ static int pair_backward_lpa(gmnn_system *s, cudaStream_t st, int lpa) {
 #undef GMNN_PB_LAUNCH
     GMNN_LAUNCHED();
     if (pairbuf) {
-        k_force_reduce<8><<<nblocks(s->N * 8, 256), 256, 0, st>>>(s->N, s->count, s->cap, s->gbuf, s->f_int);
+        if (wf_head >= 0)
+            k_force_reduce<8, true><<<nblocks(s->N * 8, 256), 256, 0, st>>>(s->N, s->count, s->cap, s->gbuf, s->f_int, s->perm,
+                                                                           wf_head, f_mean, f_m2);
+        else
+            k_force_reduce<8, false><<<nblocks(s->N * 8, 256), 256, 0, st>>>(s->N, s->count, s->cap, s->gbuf, s->f_int, nullptr, 0,
+                                                                            nullptr, nullptr);
+        GMNN_LAUNCHED();
+    } else if (wf_head >= 0) {
+        k_welford_perm<<<nblocks(s->N, 256), 256, 0, st>>>(s->N, s->f_int, s->perm, wf_head, f_mean, f_m2);
         GMNN_LAUNCHED();
     }
     GMNN_CUDA(cudaGetLastError());
@@ -312,6 +362,14 @@ static int pair_backward_lpa(gmnn_system *s, cudaStream_t st, int lpa) {
 int launch_pair_backward(gmnn_system *s, cudaStream_t st) {
     const gmnn_model *m = s->model;
     if (m->hp.n_radial == 5 && m->hp.n_basis == 7) return pair_backward_lpa<5, 7>(s, st, pick_lpa(s));
+    set_error("pair kernels are instantiated for n_radial = 5, n_basis = 7 only");
+    return GMNN_UNSUPPORTED;
+}
+
+// a12: pair backward of one head of the shallow ensemble, its force folded into the running statistics over the heads
+int launch_pair_backward_welford(gmnn_system *s, int head, float *f_mean, float *f_m2, cudaStream_t st) {
+    const gmnn_model *m = s->model;
+    if (m->hp.n_radial == 5 && m->hp.n_basis == 7) return pair_backward_lpa<5, 7>(s, st, pick_lpa(s), head, f_mean, f_m2);
     set_error("pair kernels are instantiated for n_radial = 5, n_basis = 7 only");
     return GMNN_UNSUPPORTED;
 }
