@@ -361,7 +361,7 @@ static int pair_backward_lpa(gmnn_system *s, cudaStream_t st, int lpa, int wf_he
 
 int launch_pair_backward(gmnn_system *s, cudaStream_t st) {
     const gmnn_model *m = s->model;
-    if (m->hp.n_radial == 5 && m->hp.n_basis == 7) return pair_backward_lpa<5, 7>(s, st, pick_lpa(s));
+    if (m->hp.n_radial == 5 && m->hp.n_basis == 7) return pair_backward_lpa<5, 7>(s, st, pick_lpa(s, true));
     set_error("pair kernels are instantiated for n_radial = 5, n_basis = 7 only");
     return GMNN_UNSUPPORTED;
 }
@@ -369,7 +369,7 @@ int launch_pair_backward(gmnn_system *s, cudaStream_t st) {
 // a12: pair backward of one head of the shallow ensemble, its force folded into the running statistics over the heads
 int launch_pair_backward_welford(gmnn_system *s, int head, float *f_mean, float *f_m2, cudaStream_t st) {
     const gmnn_model *m = s->model;
-    if (m->hp.n_radial == 5 && m->hp.n_basis == 7) return pair_backward_lpa<5, 7>(s, st, pick_lpa(s), head, f_mean, f_m2);
+    if (m->hp.n_radial == 5 && m->hp.n_basis == 7) return pair_backward_lpa<5, 7>(s, st, pick_lpa(s, true), head, f_mean, f_m2);
     set_error("pair kernels are instantiated for n_radial = 5, n_basis = 7 only");
     return GMNN_UNSUPPORTED;
 }

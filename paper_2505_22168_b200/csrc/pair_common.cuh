@@ -121,14 +121,15 @@ __device__ __forceinline__ void monomials(float x, float y, float z, float *m) {
 
 static inline unsigned nblocks(int64_t n, int per) { return (unsigned)((n + per - 1) / per); }
 
-static int pick_lpa(const gmnn_system *s) {
+static int pick_lpa(const gmnn_system *s, bool backward = false) {
     if (s->lanes_per_atom > 0) return s->lanes_per_atom;
-    // enough warps to fill 148 SMs several times over: small systems spread one atom over more lanes
-    if (s->N >= 262144) return 2;  // measured at 524 288 atoms: 2 beats 4 by 5 % in both pair kernels
+    // enough warps to fill 148 SMs several times over: small systems spread one atom over more lanes.  Measured at config 5
+    // (1 048 576 atoms, round 2): k_pair_forward 1.44 / 1.58 / 1.99 ms at 2 / 4 / 8 lanes, k_pair_backward + k_force_reduce
+    // 4.55 / 3.33 / 2.99 / 3.17 ms at 1 / 2 / 4 / 8 (its A_i staging in shared memory is shared by the lanes of an atom)
+    if (s->N >= 262144) return backward ? 4 : 2;
     if (s->N >= 65536) return 4;
     if (s->N >= 8192) return 8;
     return 32;
 }
-
 
 }  // namespace gmnn
