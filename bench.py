@@ -83,7 +83,7 @@ def stage_model(w, nl_mean, nc_mean, n_hidden_macs, mlp, forces="pairbuf"):
 class ClockSampler:
     """nvidia-smi clocks and throttle reasons, sampled every 200 ms while the timed region runs."""
 
-    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+    Q = ("timestamp,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
 
@@ -107,7 +107,10 @@ class ClockSampler:
         except Exception:
             self.proc = None
 
-    def stop(self):
+    def stop(self, t_begin=None, t_end=None):
+        """Summary of the samples taken between the wall-clock times t_begin and t_end (time.time(); None: all).  The
+        sampler is started BEFORE the warm-up steps, so that its start-up (a fork and ~100 ms of nvidia-smi initialisation)
+        does not leave the GPU idle, and clocked down, right before the timed region."""
         if self.proc is None:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
         time.sleep(0.25)
@@ -117,13 +120,23 @@ class ClockSampler:
         except Exception:
             self.proc.kill()
         self.out.close()
+        import datetime
+
         sm, smax, power, reasons = [], [], [], set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         with open(self.path) as f:
             for line in f:
                 c = [x.strip() for x in line.split(",")]
-                if len(c) < 8:
+                if len(c) < 9:
                     continue
+                if t_begin is not None and t_end is not None:
+                    try:  # "2026/11/05 02:38:11.123": local time of the box, like time.time() through fromtimestamp
+                        ts = datetime.datetime.strptime(c[0], "%Y/%m/%d %H:%M:%S.%f").timestamp()
+                        if ts < t_begin - 0.25 or ts > t_end + 0.25:
+                            continue
+                    except ValueError:
+                        pass
+                c = c[1:]
                 try:
                     sm.append(float(c[0]))
                     smax.append(float(c[1]))
@@ -436,21 +449,24 @@ def run_ours(args):
     sysm.set_int("md_continue", 1)
     stream = torch.cuda.current_stream()
     total_rebuilds = 0
-    if args.warmup > 0:
-        total_rebuilds += run_steps(args.warmup, False)[1]
-    stages_on = not args.no_stages and mode != "ensemble"
-    sysm.set_int("profile", 1 if stages_on else 0)
     sampler = ClockSampler(local)
     sampler.start()
+    stages_on = not args.no_stages and mode != "ensemble"
+    sysm.set_int("profile", 1 if stages_on else 0)  # the warm-up steps run the code path that is timed (events included)
+    if args.warmup > 0:
+        total_rebuilds += run_steps(args.warmup, True)[1]
+    sysm.set_int("profile", 1 if stages_on else 0)  # drops the warm-up's stage events
     barrier()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     launches0 = gm.launch_count()
+    t_begin = time.time()
     ev0.record(stream)
     etot_series, nreb = run_steps(args.steps, True)
     ev1.record(stream)
     barrier()
+    t_end = time.time()
     launches = gm.launch_count() - launches0
-    clocks = sampler.stop()
+    clocks = sampler.stop(t_begin, t_end)
     total_rebuilds += nreb
     ms = ev0.elapsed_time(ev1)
     stages = sysm.stage_times() if stages_on else []

@@ -533,6 +533,13 @@ int gmnn_system_set_int(gmnn_system *s, const char *key, int64_t v) {
     } else if (!strcmp(key, "profile")) {
         s->profile = v != 0;
         s->n_stage_events = 0;
+        // events are created here, not lazily inside the calls being timed (a few microseconds each, 13 per MD step)
+        while (s->profile && s->events.size() < 2048) {
+            cudaEvent_t e;
+            if (cudaEventCreate(&e) != cudaSuccess) break;
+            s->events.push_back(e);
+            s->stage_names.push_back(nullptr);
+        }
     } else if (!strcmp(key, "md_continue")) {
         s->md_continue = v != 0;
     } else if (!strcmp(key, "md_graph")) {
