@@ -139,8 +139,14 @@ void gmnn_system_destroy(gmnn_system *s);
  *                     accumulates with truncation; the forward GEMMs enter the energies)
  *   "tc_flush_k_bwd"  the same for the BACKWARD GEMMs (default 256; they enter the forces only)
  *   "tc_h_bk"         32 | 64 (default): K extent of one pipeline stage of the 3xFP16 GEMM
- *   "tc_prefetch"     0..64 (default 0: measured no gain): pipeline stages by which the CTA-pair GEMMs prefetch their activation boxes
- *                     into L2 ahead of the loads (0: off)
+ *   "tc_fwd_scheme"   accumulator scheme of the forward 3xFP16 / 3xTF32 GEMMs: 2 (default) = chunks of tc_flush_k alternate between
+ *                     two tensor-memory buffers, all cross terms of a chunk issued before its hi.hi terms; 1 = cross terms of the whole
+ *                     tile in an accumulator of their own, hi.hi terms drained every tc_flush_k (also taken when a chunk does not
+ *                     fit the stage ring)
+ *   "tc_tile_order"   0..3: bit 0 forward GEMMs, bit 1 backward GEMMs: 0 (default) = tiles dealt round-robin to the CTA pairs,
+ *                     1 = a pair runs the column tiles of one row tile back to back
+ *   "tc_dmul_prefetch" -1 (never), 0 (default) .. 64: the backward GEMM prefetches a tile's multiplier block into L2 this many
+ *                     pipeline stages before the tile's last
  *   The tc_* knobs are process-wide.  (Builds with -DGMNN_EXPERIMENTS add "tc_debug" and "cb_halves", knock-out
  *   and superseded-variant switches for timing studies; the shipped library rejects them as unknown keys.)
  * Returns GMNN_INVALID_ARG for an unknown key or value. */

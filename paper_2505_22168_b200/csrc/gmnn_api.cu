@@ -23,7 +23,7 @@ void set_error(const char *fmt, ...) {
 }
 
 int launch_mlp_forward_tc(gmnn_system *s, cudaStream_t st);
-extern int g_tc_split_bk, g_tc_flush_k, g_tc_flush_k_bwd, g_tc_pair, g_tc_h_bk, g_tc_prefetch;
+extern int g_tc_split_bk, g_tc_flush_k, g_tc_flush_k_bwd, g_tc_pair, g_tc_h_bk, g_tc_tile_order, g_tc_dmul_prefetch, g_tc_fwd_scheme;
 #ifdef GMNN_EXPERIMENTS
 extern int g_tc_debug, g_cb_halves;
 #endif
@@ -567,9 +567,15 @@ int gmnn_system_set_int(gmnn_system *s, const char *key, int64_t v) {
     } else if (!strcmp(key, "tc_debug")) {  // knock-out timing experiments (wrong results), see mlp_tc.cu
         gmnn::g_tc_debug = (int)v;
 #endif
-    } else if (!strcmp(key, "tc_prefetch")) {  // process-wide, see mlp_tc.cu
-        if (v < 0 || v > 64) return GMNN_INVALID_ARG;
-        gmnn::g_tc_prefetch = (int)v;
+    } else if (!strcmp(key, "tc_fwd_scheme")) {  // process-wide, see mlp_tc.cu
+        if (v < 1 || v > 2) return GMNN_INVALID_ARG;
+        gmnn::g_tc_fwd_scheme = (int)v;
+    } else if (!strcmp(key, "tc_tile_order")) {  // process-wide, see mlp_tc.cu
+        if (v < 0 || v > 3) return GMNN_INVALID_ARG;
+        gmnn::g_tc_tile_order = (int)v;
+    } else if (!strcmp(key, "tc_dmul_prefetch")) {  // process-wide, see mlp_tc.cu
+        if (v < -1 || v > 64) return GMNN_INVALID_ARG;
+        gmnn::g_tc_dmul_prefetch = (int)v;
     } else if (!strcmp(key, "tc_flush_k_bwd")) {  // process-wide, see mlp_tc.cu
         if (v < 16 || v > 4096 || v % 16) return GMNN_INVALID_ARG;
         gmnn::g_tc_flush_k_bwd = (int)v;

@@ -47,8 +47,20 @@ enum { EPI_PLAIN = 0, EPI_HIDDEN = 1, EPI_MUL = 2, EPI_HIDDEN_HEAD = 3 };
 // shipped library compiles them out.
 #ifdef GMNN_EXPERIMENTS
 #define TC_DBG(p) ((p).debug)
+// cycle accounting of the CTA-pair kernel's roles (experiments build only): [EPI][CTA][slot]
+__device__ long long g_tc_prof[4 * 160 * 8];
+#define TC_PROF_DECL long long prof_[8] = {0, 0, 0, 0, 0, 0, 0, 0}
+#define TC_PROF(slot, ...) { const long long t0_ = clock64(); __VA_ARGS__; prof_[slot] += clock64() - t0_; }
+#define TC_PROF_BEGIN(name) const long long name = clock64()
+#define TC_PROF_END(slot, name) prof_[slot] += clock64() - name
+#define TC_PROF_FLUSH(epi) { for (int q_ = 0; q_ < 8; ++q_) if (prof_[q_]) atomicAdd((unsigned long long *)&g_tc_prof[((epi) * 160 + blockIdx.x) * 8 + q_], (unsigned long long)prof_[q_]); }
 #else
 #define TC_DBG(p) 0
+#define TC_PROF_DECL
+#define TC_PROF(slot, ...) { __VA_ARGS__; }
+#define TC_PROF_BEGIN(name)
+#define TC_PROF_END(slot, name)
+#define TC_PROF_FLUSH(epi)
 #endif
 // EPI_HIDDEN_HEAD: last hidden layer of a single-head model.  h = swish(z) is not stored (the backward
 // needs only swish'); its dot product with the head weights is: every thread writes the partial sum
@@ -84,8 +96,10 @@ struct TcArgs {
     int n_tiles;   // total
     int flush;     // pipeline stages per accumulator flush (K chunk = flush * BK)
     int flush1;    // ... of the first two chunks of a tile (>= flush)
-    int xy;        // CTA-pair kernels: 1 = cross terms and hi.hi terms in accumulators of their own (forward GEMMs), 0 = ping-pong
-    int prefetch;  // CTA-pair kernels: pipeline stages by which the L2 prefetch of the A boxes runs ahead of their loads
+    int xy;        // CTA-pair kernels: 0 = ping-pong of mixed chunks (backward GEMMs), 1 = cross terms and hi.hi terms in accumulators
+                   // of their own, 2 = ping-pong of chunks whose cross terms all precede their hi.hi terms (forward GEMMs)
+    int order;     // CTA-pair kernels: 0 = tiles dealt round-robin to the pairs, 1 = a pair runs the column tiles of a row tile back to back
+    int dmul_pf;   // EPI_MUL: the multiplier block of a tile is prefetched into L2 this many pipeline stages before the tile's last (< 0: never)
     int debug;     // -DGMNN_EXPERIMENTS builds only (results wrong): 1 skip split work, 2 hi.hi MMA only, 4 skip the elementwise
                    // and the stores, 8 skip the stores only, 16 skip the tensor-memory drains
     float *C;      // [M][N]
@@ -171,7 +185,9 @@ template <int EPI, bool SCALED = false>
 __device__ __forceinline__ void tc_store_tile(const TcArgs &p, float (&acc)[4][32], int m0, int n0, int quad, int lane,
                                               int half, int n_groups, bool row_ok, float oscale, float &tmax) {
     // every matrix the MLP touches is tile-transposed, [M / 128][N][128]: column c of this tile is
-    // 128 consecutive floats, so each warp store / load below is one full 128-byte line
+    // 128 consecutive floats, so each warp store / load below is one full 128-byte line.  The stores are streaming
+    // (st.global.cs): the outputs are 1.5 - 4 GB that only the next kernel reads, and left to the default policy
+    // their dirty lines push the activation boxes out of L2 between the reads of the two column tiles of a row tile
     const int64_t tbase = (int64_t)(m0 / TC_BM) * p.N * TC_BM + quad * 32 + lane;
     float *__restrict__ Cout = p.C;
     float *__restrict__ C2out = p.C2;
@@ -209,7 +225,7 @@ __device__ __forceinline__ void tc_store_tile(const TcArgs &p, float (&acc)[4][3
                             tmax = fmaxf(tmax, d[c]);
                             continue;
                         }
-                        C2out[o + c * TC_BM] = d[c];
+                        __stcs(C2out + o + c * TC_BM, d[c]);
                     }
             } else if (EPI == EPI_HIDDEN) {
 #pragma unroll
@@ -223,8 +239,8 @@ __device__ __forceinline__ void tc_store_tile(const TcArgs &p, float (&acc)[4][3
                             tmax = fmaxf(tmax, fabsf(h[c]) + d[c]);
                             continue;
                         }
-                        Cout[o + c * TC_BM] = h[c];
-                        C2out[o + c * TC_BM] = d[c];
+                        __stcs(Cout + o + c * TC_BM, h[c]);
+                        __stcs(C2out + o + c * TC_BM, d[c]);
                         if (SCALED) tmax = fmaxf(tmax, fabsf(h[c]));
                     }
             } else if (EPI == EPI_MUL) {
@@ -238,12 +254,12 @@ __device__ __forceinline__ void tc_store_tile(const TcArgs &p, float (&acc)[4][3
                         const float v = (SCALED ? acc[gi][j0 + c] * oscale : acc[gi][j0 + c]) * in[c];
                         if (SCALED) tmax = fmaxf(tmax, fabsf(v));
                         if (TC_DBG(p) & 8) continue;
-                        Cout[o + c * TC_BM] = v;
+                        __stcs(Cout + o + c * TC_BM, v);
                     }
             } else {
 #pragma unroll
                 for (int c = 0; c < TC_EB; ++c)
-                    if (c < nc) Cout[o + c * TC_BM] = SCALED ? acc[gi][j0 + c] * oscale : acc[gi][j0 + c];
+                    if (c < nc) __stcs(Cout + o + c * TC_BM, SCALED ? acc[gi][j0 + c] * oscale : acc[gi][j0 + c]);
             }
         }
     }
@@ -310,8 +326,8 @@ __device__ __forceinline__ void tc_finish_tile(const TcArgs &p, float (&acc)[4][
                         tmax = fmaxf(tmax, d[c]);
                         continue;
                     }
-                    if (EPI == EPI_HIDDEN) cp[off] = h[c];
-                    dp[off] = d[c];
+                    if (EPI == EPI_HIDDEN) __stcs(cp + off, h[c]);
+                    __stcs(dp + off, d[c]);
                 }
             }
         }
@@ -619,48 +635,44 @@ k_gemm_tc_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     tcgen05_fence_after();
     const uint32_t tmem_base = *tmem_slot_gen;
 
+    // Tile order.  p.order = 0: tile t of the launch goes to pair t % n_pairs, so that the column tiles of one row tile run
+    // on neighbouring pairs at about the same time.  p.order = 1: a pair takes whole row tiles and runs their column tiles
+    // back to back, so that the second read of the row tile's activation boxes follows the first by one tile time whatever
+    // the drift between pairs.
+    const int n_row_tiles = p.n_tiles / p.n_tiles_n;
+    const int t_end = p.order ? ((n_row_tiles + n_pairs - 1) / n_pairs) * p.n_tiles_n * n_pairs : p.n_tiles;
+    auto tile_of = [&](int tt) {
+        if (!p.order) return tt;
+        const int k = tt / n_pairs;
+        return ((k / p.n_tiles_n) * n_pairs + pair) * p.n_tiles_n + k % p.n_tiles_n;
+    };
+
     if (warp < TC_FIRST_SPLIT_WARP) {
         setmaxnreg_dec<Cfg::REGS_CONTROL>();
         if (warp == 0 && lane == 0) {
             // ===== TMA producer: own A rows, own half of B =====
-            // The activations come from HBM (each GEMM's A is the previous kernel's 1.5 - 2 GB output); with 192 KB of
-            // stages a load that pays the HBM latency inside the ring cannot keep the MMA pipe fed (stage occupancy =
-            // latency + split + MMA).  Every A box is therefore prefetched into L2 p.prefetch stages ahead (about one
-            // tile), and the ring's own load then is an L2 hit.  The weights stay in L2 by themselves.
             const uint32_t tx = (uint32_t)(TC_BM * BK * 4 + 2 * hb * BK * Cfg::ES);
-            const int my_tiles = p.n_tiles > pair ? (p.n_tiles - pair + n_pairs - 1) / n_pairs : 0;
-            const int64_t n_stage_total = (int64_t)my_tiles * nkb;
-            auto a_row = [&](int64_t j, int &kb) {  // stage j of this CTA -> row coordinate of its A box
-                const int t = pair + (int)(j / nkb) * n_pairs;
-                kb = (int)(j % nkb);
-                return (2 * (t / p.n_tiles_n) + (int)rank) * p.K + kb * BK;
-            };
-            auto prefetch_a = [&](int64_t j) {
-                if (j >= n_stage_total) return;
-                int kb;
-                const int row = a_row(j, kb);
-                if (F16) {
-                    tma_prefetch_2d(&tmA, 0, row);
-                } else {
-                    for (int q = 0; q < 4; ++q) tma_prefetch_2d(&tmA, q * 32, row);
-                }
-            };
-            for (int j = 0; j < p.prefetch; ++j) prefetch_a(j);
+            TC_PROF_DECL;
             uint32_t it = 0;
-            for (int t = pair; t < p.n_tiles; t += n_pairs) {
+            const int pf_kb = p.dmul_pf < 0 ? -1 : (nkb - 1 - p.dmul_pf > 0 ? nkb - 1 - p.dmul_pf : 0);
+            TC_PROF_BEGIN(t_all);
+            for (int tt = pair; tt < t_end; tt += n_pairs) {
+                const int t = tile_of(tt);
+                if (t >= p.n_tiles) continue;  // same decision in every role of both CTAs
                 const int mt = 2 * (t / p.n_tiles_n) + (int)rank, n0 = (t % p.n_tiles_n) * p.bn;
-                if (EPI == EPI_MUL && (int64_t)mt * TC_BM < p.M) {
-                    // the multiplier block of this tile (swish' of the layer below: bn columns x 128 rows, contiguous in both
-                    // layouts) is read by the epilogue at the END of the tile, from HBM: bring it into L2 now
-                    const int cols = p.N - n0 < p.bn ? p.N - n0 : p.bn;
-                    const char *blk = reinterpret_cast<const char *>(
-                        p.Dmul + ((int64_t)(mt / p.dmul_row_div) * p.dmul_N + n0 % p.dmul_N) * TC_BM);
-                    for (int c = 0; c < cols; c += 64) bulk_prefetch_l2(blk + (int64_t)c * TC_BM * 4, (uint32_t)((cols - c < 64 ? cols - c : 64) * TC_BM * 4));
-                }
                 for (int kb = 0; kb < nkb; ++kb, ++it) {
                     const int s = it % NST;
-                    if (p.prefetch > 0) prefetch_a((int64_t)it + p.prefetch);
-                    mbar_wait(bar_empty(s), ((it / NST) & 1) ^ 1);
+                    if (EPI == EPI_MUL && kb == pf_kb && (int64_t)mt * TC_BM < p.M) {
+                        // the multiplier block of this tile (swish' of the layer below: bn columns x 128 rows, contiguous) is read
+                        // by the epilogue at the END of the tile, from HBM: bring it into L2 shortly before that (measured at
+                        // config 5: issued at the start of the tile the block is evicted again before its use, 7.4 GB of DRAM
+                        // reads per launch instead of 5.3; at the last stage 5.4 GB and 3 % less time than without)
+                        const int cols = p.N - n0 < p.bn ? p.N - n0 : p.bn;
+                        const char *blk = reinterpret_cast<const char *>(
+                            p.Dmul + ((int64_t)(mt / p.dmul_row_div) * p.dmul_N + n0 % p.dmul_N) * TC_BM);
+                        for (int c = 0; c < cols; c += 64) bulk_prefetch_l2(blk + (int64_t)c * TC_BM * 4, (uint32_t)((cols - c < 64 ? cols - c : 64) * TC_BM * 4));
+                    }
+                    TC_PROF(0, mbar_wait(bar_empty(s), ((it / NST) & 1) ^ 1));
                     mbar_arrive_expect_tx(bar_full(s), tx);
                     if (F16) {
                         tma_load_2d(a_hi(s), &tmA, bar_full(s), 0, mt * p.K + kb * BK);  // [BK][128] fp32
@@ -672,6 +684,8 @@ k_gemm_tc_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                     tma_load_2d(b_lo(s), &tmB, bar_full(s), kb * BK, p.N + n0 + (int)rank * hb);  // lo rows follow the hi rows
                 }
             }
+            TC_PROF_END(5, t_all);
+            TC_PROF_FLUSH(EPI);
         } else if (warp == 1 && lane == 0 && rank == 0) {
             // ===== MMA issuer (leader CTA only) =====
             // Two accumulators in tensor memory (see the header of this kernel): X, columns [0, 256), takes the cross terms
@@ -680,7 +694,67 @@ k_gemm_tc_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
             const uint32_t idesc = F16 ? make_idesc_f16(2 * TC_BM, p.bn) : make_idesc_tf32(2 * TC_BM, p.bn, true);
             const uint32_t d_x = tmem_base, d_y = tmem_base + TC_BN_MAX;
             uint32_t it = 0, ygrp = 0, xt = 0;
-            for (int t = pair; t < p.n_tiles; t += n_pairs) {
+            TC_PROF_DECL;
+            for (int tt = pair; tt < t_end; tt += n_pairs) {
+                const int t = tile_of(tt);
+                if (t >= p.n_tiles) continue;  // same decision in every role of both CTAs
+                if (p.xy == 2) {
+                    // cross-first ping-pong (forward GEMMs): the chunks of p.flush stages alternate between the two 256-column
+                    // buffers as below, but inside a chunk ALL cross terms are issued before the first hi.hi product: an MMA
+                    // adds into its accumulator with truncation, an error of one ulp of the ACCUMULATOR whatever the size of
+                    // the addend, so the 2 * 8 cross additions per stage must land while the accumulator is still small; the
+                    // large additions per drain are then the hi.hi ones only, as with an accumulator of their own, and two
+                    // chunks of run-way remain for the final phase of the previous tile.  p.flush <= NST (host-checked).
+                    for (int kb0 = 0; kb0 < nkb; kb0 += p.flush) {
+                        const int nst = nkb - kb0 < p.flush ? nkb - kb0 : p.flush;
+                        const int a = ygrp & 1;
+                        const uint32_t d_tmem = tmem_base + (uint32_t)a * TC_BN_MAX;
+                        TC_PROF(2, mbar_wait(bar_tempty(a), ((ygrp >> 1) & 1) ^ 1));
+                        tcgen05_fence_after();
+                        const uint64_t astep = F16 ? 2 : 64;
+                        uint32_t acc = 0u;
+                        for (int pass = 0; pass < 2; ++pass) {
+                            for (int q = 0; q < nst; ++q) {
+                                const uint32_t itq = it + (uint32_t)q;
+                                const int s = itq % NST;
+                                if (pass == 0) {
+                                    TC_PROF(1, mbar_wait(bar_split(s), (itq / NST) & 1));
+                                    tcgen05_fence_after();
+                                }
+                                const int krem = p.K - (kb0 + q) * BK;
+                                const int ksteps = krem >= BK ? BK / Cfg::KSTEP : (krem + Cfg::KSTEP - 1) / Cfg::KSTEP;
+                                const uint64_t db_hi = make_smem_desc<Cfg::ROWB>(b_hi(s)), db_lo = make_smem_desc<Cfg::ROWB>(b_lo(s));
+                                const uint64_t da_hi = F16 ? make_smem_desc<Cfg::ROWB>(a_hi(s)) : make_smem_desc_mn128(a_hi(s), BK * 128);
+                                const uint64_t da_lo = F16 ? make_smem_desc<Cfg::ROWB>(a_lo(s)) : make_smem_desc_mn128(a_lo(s), BK * 128);
+                                if (pass == 0) {
+                                    for (int k = 0; k < ksteps && !(TC_DBG(p) & 2); ++k) {
+                                        const uint64_t koff = (uint64_t)(2 * k), aoff = astep * k;
+                                        if (F16) {
+                                            mma_f16_ss_pair(d_tmem, da_lo + aoff, db_hi + koff, idesc, acc);
+                                            mma_f16_ss_pair(d_tmem, da_hi + aoff, db_lo + koff, idesc, 1u);
+                                        } else {
+                                            mma_tf32_ss_pair(d_tmem, da_lo + aoff, db_hi + koff, idesc, acc);
+                                            mma_tf32_ss_pair(d_tmem, da_hi + aoff, db_lo + koff, idesc, 1u);
+                                        }
+                                        acc = 1u;
+                                    }
+                                } else {
+                                    for (int k = 0; k < ksteps; ++k) {
+                                        const uint64_t koff = (uint64_t)(2 * k), aoff = astep * k;
+                                        if (F16) mma_f16_ss_pair(d_tmem, da_hi + aoff, db_hi + koff, idesc, acc);
+                                        else mma_tf32_ss_pair(d_tmem, da_hi + aoff, db_hi + koff, idesc, acc);
+                                        acc = 1u;
+                                    }
+                                    mma_commit_pair(bar_empty(s), 3);
+                                }
+                            }
+                        }
+                        mma_commit_pair(bar_tfull(a), 3);
+                        ++ygrp;
+                        it += (uint32_t)nst;
+                    }
+                    continue;
+                }
                 for (int kb = 0; kb < nkb; ++kb, ++it) {
                     const int pos = kb % p.flush;
                     const bool y_first = pos == 0, y_last = pos == p.flush - 1 || kb == nkb - 1;
@@ -693,10 +767,10 @@ k_gemm_tc_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                         const int a = ygrp & 1;
                         const uint32_t d_tmem = tmem_base + (uint32_t)a * TC_BN_MAX;
                         if (y_first) {
-                            mbar_wait(bar_tempty(a), ((ygrp >> 1) & 1) ^ 1);
+                            TC_PROF(2, mbar_wait(bar_tempty(a), ((ygrp >> 1) & 1) ^ 1));
                             tcgen05_fence_after();
                         }
-                        mbar_wait(bar_split(s), (it / NST) & 1);
+                        TC_PROF(1, mbar_wait(bar_split(s), (it / NST) & 1));
                         tcgen05_fence_after();
                         const int krem = p.K - kb * BK;
                         const int ksteps = krem >= BK ? BK / Cfg::KSTEP : (krem + Cfg::KSTEP - 1) / Cfg::KSTEP;
@@ -729,7 +803,7 @@ k_gemm_tc_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                         }
                         continue;
                     }
-                    mbar_wait(bar_split(s), (it / NST) & 1);
+                    TC_PROF(1, mbar_wait(bar_split(s), (it / NST) & 1));
                     tcgen05_fence_after();
                     const int krem = p.K - kb * BK;
                     const int ksteps = krem >= BK ? BK / Cfg::KSTEP : (krem + Cfg::KSTEP - 1) / Cfg::KSTEP;
@@ -739,7 +813,7 @@ k_gemm_tc_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                     // per k step: B (and a K-major A) advance 32 bytes along the row, the MN-major A one 1024-byte atom
                     const uint64_t astep = F16 ? 2 : 64;
                     if (kb == 0) {  // X of the previous tile drained by both CTAs
-                        mbar_wait(bar_tempty(1), (xt & 1) ^ 1);
+                        TC_PROF(2, mbar_wait(bar_tempty(1), (xt & 1) ^ 1));
                         tcgen05_fence_after();
                     }
                     uint32_t acc = kb != 0;
@@ -755,7 +829,7 @@ k_gemm_tc_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                         acc = 1u;
                     }
                     if (y_first) {  // Y of the previous group drained (the cross terms above keep the pipe busy meanwhile)
-                        mbar_wait(bar_tempty(0), (ygrp & 1) ^ 1);
+                        TC_PROF(2, mbar_wait(bar_tempty(0), (ygrp & 1) ^ 1));
                         tcgen05_fence_after();
                     }
                     acc = !y_first;
@@ -776,6 +850,7 @@ k_gemm_tc_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                     }
                 }
             }
+            TC_PROF_FLUSH(EPI);
         }
     } else if (warp < TC_FIRST_EPI_WARP) {
         setmaxnreg_dec<Cfg::REGS_SPLIT>();
@@ -783,10 +858,13 @@ k_gemm_tc_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
         const int tid = threadIdx.x - TC_FIRST_SPLIT_WARP * 32;
         const float ascale = F16 ? pow2i(14 - amax_exponent(*p.amax_a)) : 1.f;
         uint32_t it = 0;
-        for (int t = pair; t < p.n_tiles; t += n_pairs) {
+        TC_PROF_DECL;
+        for (int tt = pair; tt < t_end; tt += n_pairs) {
+                const int t = tile_of(tt);
+                if (t >= p.n_tiles) continue;  // same decision in every role of both CTAs
             for (int kb = 0; kb < nkb; ++kb, ++it) {
                 const int s = it % NST;
-                mbar_wait(bar_full(s), (it / NST) & 1);
+                TC_PROF(6, mbar_wait(bar_full(s), (it / NST) & 1));
                 uint8_t *stage = smem_gen + (size_t)s * Cfg::STAGE_BYTES;
                 if (TC_DBG(p) & 1) {
                     if (F16) asm volatile("bar.sync 1, 128;" ::: "memory");
@@ -801,6 +879,7 @@ k_gemm_tc_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                 if (lane == 0) mbar_arrive_cluster(bar_split(s), 0);
             }
         }
+        if (tid == 0) TC_PROF_FLUSH(EPI);
     } else {
         setmaxnreg_inc<Cfg::REGS_EPI>();
         // ===== epilogue: this CTA's 128 rows =====
@@ -813,20 +892,25 @@ k_gemm_tc_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
         const float oscale = pow2i(osc_e), inv_oscale = pow2i(-osc_e);
         float tmax = 0.f;
         uint32_t ygrp = 0, xt = 0;
-        for (int t = pair; t < p.n_tiles; t += n_pairs) {
+        const bool xy = p.xy == 1;  // X / Y accumulators; otherwise chunks alternate between the two buffers
+        TC_PROF_DECL;
+        for (int tt = pair; tt < t_end; tt += n_pairs) {
+                const int t = tile_of(tt);
+                if (t >= p.n_tiles) continue;  // same decision in every role of both CTAs
             const int m0 = (2 * (t / p.n_tiles_n) + (int)rank) * TC_BM, n0 = (t % p.n_tiles_n) * p.bn;
             const int row = m0 + quad * 32 + lane;
             const bool row_ok = row < p.M;
             float acc[4][32];
             tc_init_acc<EPI>(p, acc, n0, half, inv_oscale);  // the forward bias rides in the accumulators
             // the hi.hi groups (accumulator Y), then the tile's cross terms (accumulator X): round-to-nearest adds in registers
-            for (int c = 0; c < n_ygroups + (p.xy ? 1 : 0); ++c) {
+            for (int c = 0; c < n_ygroups + (xy ? 1 : 0); ++c) {
                 // X / Y scheme: buffer 0 = Y (columns 256..511) for the hi.hi groups, then buffer 1 = X (columns 0..255);
                 // ping-pong scheme: chunk c sits in buffer (chunk number) & 1 at columns 256 * buffer
-                const int a = p.xy ? (c < n_ygroups ? 0 : 1) : (int)(ygrp & 1);
-                mbar_wait(bar_tfull(a), p.xy ? ((a == 0 ? ygrp : xt) & 1) : ((ygrp >> 1) & 1));
+                const int a = xy ? (c < n_ygroups ? 0 : 1) : (int)(ygrp & 1);
+                TC_PROF(3, mbar_wait(bar_tfull(a), xy ? ((a == 0 ? ygrp : xt) & 1) : ((ygrp >> 1) & 1)));
                 tcgen05_fence_after();
-                const uint32_t col0 = p.xy ? (a == 0 ? TC_BN_MAX : 0) : (uint32_t)a * TC_BN_MAX;
+                TC_PROF_BEGIN(t_drain);
+                const uint32_t col0 = xy ? (a == 0 ? TC_BN_MAX : 0) : (uint32_t)a * TC_BN_MAX;
 #pragma unroll
                 for (int gi = 0; gi < 4; ++gi) {
                     const int g = 2 * gi + half;
@@ -838,17 +922,21 @@ k_gemm_tc_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                         for (int j = 0; j < 32; ++j) acc[gi][j] += __uint_as_float(v[j]);
                     }
                 }
+                TC_PROF_END(7, t_drain);
                 tcgen05_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive_cluster(bar_tempty(a), 0);
-                if (!p.xy || a == 0) ++ygrp;
+                if (!xy || a == 0) ++ygrp;
                 else ++xt;
             }
+            TC_PROF_BEGIN(t_final);
             if (EPI == EPI_HIDDEN || EPI == EPI_HIDDEN_HEAD)
                 tc_finish_tile<EPI, F16>(p, acc, m0, n0, quad, lane, half, row_ok, oscale, tmax);
             else  // backward: multiplier loads in bursts of 16 ahead of their use
                 tc_store_tile<EPI, F16>(p, acc, m0, n0, quad, lane, half, n_groups, row_ok, oscale, tmax);
+            TC_PROF_END(4, t_final);
         }
+        if (warp == TC_FIRST_EPI_WARP && lane == 0) TC_PROF_FLUSH(EPI);
         if (F16 && p.amax_out && (EPI == EPI_HIDDEN || EPI == EPI_MUL)) {
 #pragma unroll
             for (int o = 16; o >= 1; o >>= 1) tmax = fmaxf(tmax, __shfl_xor_sync(0xffffffffu, tmax, o));
@@ -980,10 +1068,22 @@ static int tc_launch(const CUtensorMap &tmA, const CUtensorMap &tmB, const TcArg
 }
 
 int g_tc_pair = 1;    // knob "tc_pair": 3xTF32 GEMMs on CTA pairs (cta_group::2)
-int g_tc_prefetch = 0;  // knob "tc_prefetch": stages of L2 prefetch ahead of the A loads of the CTA-pair kernels (0: off)
+int g_tc_dmul_prefetch = 0;  // knob "tc_dmul_prefetch": stages before the last of a tile at which the backward GEMM prefetches its multiplier block (-1: never)
+int g_tc_fwd_scheme = 2;  // knob "tc_fwd_scheme": accumulator scheme of the forward GEMMs (TcArgs::xy): 1 or 2
+int g_tc_tile_order = 0;  // knob "tc_tile_order": bit 0 forward GEMMs, bit 1 backward GEMMs: column tiles of a row tile back to back on one pair
 int g_tc_flush_k_bwd = 256;  // knob "tc_flush_k_bwd": K extent between drains of the hi.hi accumulator, backward GEMMs
 #ifdef GMNN_EXPERIMENTS
 int g_tc_debug = 0;
+}  // namespace gmnn
+extern "C" int gmnn_debug_tc_prof(long long *out, int reset) {  // experiments build: [4][160][8] cycle counters
+    if (out && cudaMemcpyFromSymbol(out, gmnn::g_tc_prof, sizeof(gmnn::g_tc_prof)) != cudaSuccess) return -1;
+    if (reset) {
+        static long long zero[4 * 160 * 8] = {};
+        if (cudaMemcpyToSymbol(gmnn::g_tc_prof, zero, sizeof(zero)) != cudaSuccess) return -1;
+    }
+    return 0;
+}
+namespace gmnn {
 #endif
 int g_tc_flush_k = 128;  // knob "tc_flush_k": K extent between drains of the hi.hi accumulator, forward GEMMs (CTA pairs)
 int g_tc_split_bk = 32;  // knob (gmnn_system_set_int "tc_split_bk"): K extent of a 3xTF32 stage, 16 or 32
@@ -1052,7 +1152,7 @@ int tc_gemm(bool split, int epi, int64_t M, int N, int K, const float *A, const 
         return GMNN_UNSUPPORTED;
     }
     const int BK = hf ? g_tc_h_bk : (split ? g_tc_split_bk : 32);
-    TcArgs a;
+    TcArgs a = {};
     a.M = (int)M, a.N = N, a.K = K;
     a.bn = pick_bn(N);
     a.n_tiles_n = (N + a.bn - 1) / a.bn;
@@ -1067,8 +1167,13 @@ int tc_gemm(bool split, int epi, int64_t M, int N, int K, const float *A, const 
     const int flush_k = pair_kernel ? (fwd ? g_tc_flush_k : g_tc_flush_k_bwd) : 64;
     a.flush = split ? (flush_k / BK > 0 ? flush_k / BK : 1) : (K + BK - 1) / BK;
     a.flush1 = a.flush;
-    a.prefetch = g_tc_prefetch;
-    a.xy = fwd ? 1 : 0;
+    a.dmul_pf = g_tc_dmul_prefetch;
+    a.xy = fwd ? g_tc_fwd_scheme : 0;
+    {  // scheme 2 holds a whole chunk in the stage ring
+        const int es = hf ? 2 : 4, n_stages = TC_STAGE_BYTES_TOTAL / (2 * (TC_BM * BK * es + (TC_BN_MAX / 2) * BK * es));
+        if (a.xy == 2 && a.flush > n_stages) a.xy = 1;
+    }
+    a.order = (g_tc_tile_order >> (fwd ? 0 : 1)) & 1;
 #ifdef GMNN_EXPERIMENTS
     a.debug = g_tc_debug;
 #else

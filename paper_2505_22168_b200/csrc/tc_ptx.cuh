@@ -55,12 +55,6 @@ __device__ __forceinline__ void tma_load_2d(uint32_t dst, const void *tmap, uint
         : "memory");
 }
 
-// Prefetch of the same box into L2 only (no shared-memory destination, no barrier): issued a tile ahead of the load
-// so that the load itself is an L2 hit instead of paying the HBM latency inside the stage ring.
-__device__ __forceinline__ void tma_prefetch_2d(const void *tmap, int c0, int c1) {
-    asm volatile("cp.async.bulk.prefetch.tensor.2d.L2.global.tile [%0, {%1, %2}];" ::"l"((uint64_t)tmap), "r"(c0), "r"(c1)
-                 : "memory");
-}
 // 1-D L2 prefetch of `bytes` (multiple of 16) from a 16-byte aligned global address.
 __device__ __forceinline__ void bulk_prefetch_l2(const void *src, uint32_t bytes) {
     asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"((uint64_t)src), "r"(bytes) : "memory");
