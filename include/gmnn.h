@@ -310,6 +310,19 @@ int gmnn_debug_read(gmnn_system *s, const char *name, void *dst /*HOST*/, int64_
  * a register-only kernel of independent FMA chains on every SM (about 10 ms; best of three).  HOST double.  Synchronises. */
 int gmnn_measure_fp32_peak(double *tflops /*HOST*/, void *cuda_stream);
 
+/* Total energy without any allocation (for callers that cannot call cudaMalloc: code under CUDA graph capture, tight
+ * serving loops): *energy = sum_i e_atom[i] in fp64, by the same two fixed-order reduction kernels that produce the total
+ * energy of gmnn_energy_forces (Eq. 4: E = sum_i E_i), so the result depends on
+ * n_atoms only, never on scheduling.  e_atom: DEVICE float[n_atoms] (e.g. the e_atom output of gmnn_energy_forces);
+ * energy: DEVICE double[1]; both owned by the caller, on the current device; asynchronous on `cuda_stream`.
+ * The block partials live in a file-scope device array of the library (8 KB, held by every GPU that loads the library
+ * until exit), which sets the limit n_atoms <= GMNN_STATIC_SUM_MAX_ATOMS: more returns GMNN_INVALID_ARG with a message
+ * and launches nothing.  The call makes no cudaMalloc / cudaFree and no allocating library call.  All calls share that
+ * array: calls that overlap on the GPU (different streams or host threads) race; calls in stream order do not, and no
+ * call reads what an earlier one left (every slot read is written first by the same call). */
+#define GMNN_STATIC_SUM_MAX_ATOMS 16777216
+int gmnn_sum_energies_static(const float *e_atom /*DEVICE*/, int64_t n_atoms, double *energy /*DEVICE*/, void *cuda_stream);
+
 /* Number of kernel launches issued by this library since it was loaded (bench.py's gpu_launches). */
 int64_t gmnn_launch_count(void);
 

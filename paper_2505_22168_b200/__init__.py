@@ -8,7 +8,7 @@ is missing it is built in-tree with nvcc; if that is impossible the import fails
 never imports oracle/ and has no CPU fallback.
 """
 _NAMES = (
-    "EXPORTS", "LIB_PATH", "GmnnError", "Model", "System", "launch_count", "measure_fp32_peak", "n_features", "lib",
+    "EXPORTS", "LIB_PATH", "GmnnError", "Model", "System", "launch_count", "measure_fp32_peak", "n_features", "lib", "sum_energies_static", "STATIC_SUM_MAX_ATOMS",
     "GMNN_OK", "GMNN_INVALID_ARG", "GMNN_UNSUPPORTED", "GMNN_NEIGHBOR_OVERFLOW", "GMNN_STALE_NEIGHBORS",
     "GMNN_CUDA_ERROR", "GMNN_OOM", "GMNN_OUT_OF_BOX", "GMNN_MLP_FP32", "GMNN_MLP_3XTF32", "GMNN_MLP_TF32", "GMNN_MLP_3XF16",
     "GMNN_FORCE_GATHER", "GMNN_FORCE_PAIRBUF",

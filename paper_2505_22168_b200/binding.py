@@ -32,7 +32,7 @@ EXPORTS = (
     "gmnn_n_features", "gmnn_create", "gmnn_destroy", "gmnn_system_create", "gmnn_system_destroy",
     "gmnn_system_set_int", "gmnn_system_get_int", "gmnn_build_neighbors", "gmnn_get_neighbors", "gmnn_get_neighbor_rows",
     "gmnn_energy_forces", "gmnn_energy_forces_virial", "gmnn_energy_forces_host", "gmnn_ensemble_energy_forces", "gmnn_md_verlet_steps", "gmnn_md_ensemble_steps", "gmnn_system_set_langevin", "gmnn_system_set_temperature_schedule", "gmnn_system_set_nose_hoover", "gmnn_system_get_nose_hoover", "gmnn_system_set_udd_bias", "gmnn_system_get_udd_bias",
-    "gmnn_check", "gmnn_measure_fp32_peak", "gmnn_stage_times", "gmnn_debug_read", "gmnn_launch_count", "gmnn_last_error",
+    "gmnn_check", "gmnn_measure_fp32_peak", "gmnn_sum_energies_static", "gmnn_stage_times", "gmnn_debug_read", "gmnn_launch_count", "gmnn_last_error",
 )
 
 
@@ -114,6 +114,21 @@ def measure_fp32_peak(stream=None) -> float:
     v = C.c_double(0)
     _check(lib.gmnn_measure_fp32_peak(C.byref(v), _stream_ptr(stream)))
     return float(v.value)
+
+
+STATIC_SUM_MAX_ATOMS = 16777216  # GMNN_STATIC_SUM_MAX_ATOMS of include/gmnn.h
+
+
+def sum_energies_static(e_atom, energy_out, n_atoms: Optional[int] = None, stream=None) -> None:
+    """energy_out[0] (device float64) = sum of e_atom (device float32 [n]) through gmnn_sum_energies_static: no
+    allocation on the call path (the output tensor is the caller's); n_atoms <= STATIC_SUM_MAX_ATOMS."""
+    import torch
+
+    n = int(e_atom.numel()) if n_atoms is None else int(n_atoms)
+    if n_atoms is None:
+        _dev_ptr(e_atom, torch.float32, (n,))  # dtype / device / contiguity checks
+    _check(lib.gmnn_sum_energies_static(C.c_void_p(e_atom.data_ptr()), C.c_int64(n), _dev_ptr(energy_out, torch.float64, (1,)),
+                                        _stream_ptr(stream)))
 
 
 def launch_count() -> int:

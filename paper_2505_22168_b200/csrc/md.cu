@@ -531,3 +531,58 @@ int launch_fma_peak(int blocks, int iters, float *scratch, cudaStream_t st) {
 }
 
 }  // namespace gmnn
+
+// ---------------------------------------------------------------------------------------------------------------------
+// gmnn_sum_energies_static (include/gmnn.h): the two-stage fp64 sum of per-atom energies (stage 1 / stage 2 above,
+// the kernels behind the total energy of every evaluation) for callers that may not allocate: the block partials
+// that launch_energy_sum keeps in a cudaMalloc'ed buffer of the system live here in a file-scope device array.
+// Every GPU that loads the library holds these 8 KB until exit.  Every call shares them: stage 1 overwrites the
+// slots [0, blocks) that stage 2 of the same call reads, so nothing has to start at zero and stale contents of an
+// earlier call are never read; calls that overlap on the GPU (two streams, two host threads) race on them.
+// ---------------------------------------------------------------------------------------------------------------------
+namespace gmnn {
+constexpr int64_t STATIC_SUM_MAX_ATOMS = (int64_t)RED_BLOCKS * 256 * 64;  // 16 777 216 = GMNN_STATIC_SUM_MAX_ATOMS
+static_assert(STATIC_SUM_MAX_ATOMS == GMNN_STATIC_SUM_MAX_ATOMS, "include/gmnn.h states the limit");
+static __device__ __align__(256) double g_static_partial[RED_BLOCKS];
+// In host code the name g_static_partial is a host-side stand-in, not a device address: the address the kernels get
+// is looked up once per device, with that device current.
+static double *g_static_partial_dev[MAX_DEVICES] = {};
+
+static int static_partial_ptr(double **ptr) {
+    const int dev = current_device();
+    if (!g_static_partial_dev[dev]) {
+        void *p = nullptr;
+        GMNN_CUDA(cudaGetSymbolAddress(&p, g_static_partial));
+        g_static_partial_dev[dev] = static_cast<double *>(p);
+    }
+    *ptr = g_static_partial_dev[dev];
+    return GMNN_OK;
+}
+}  // namespace gmnn
+
+extern "C" int gmnn_sum_energies_static(const float *e_atom, int64_t n_atoms, double *energy, void *cuda_stream) {
+    using namespace gmnn;
+    if (!e_atom || !energy || n_atoms < 0) {
+        set_error("gmnn_sum_energies_static: null pointer or negative atom count");
+        return GMNN_INVALID_ARG;
+    }
+    if (n_atoms > STATIC_SUM_MAX_ATOMS) {
+        set_error("gmnn_sum_energies_static: %lld atoms exceed the static scratch limit of %lld "
+                  "(GMNN_STATIC_SUM_MAX_ATOMS); use gmnn_energy_forces' own total instead",
+                  (long long)n_atoms, (long long)STATIC_SUM_MAX_ATOMS);
+        return GMNN_INVALID_ARG;
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    double *partial = nullptr;
+    int rc = static_partial_ptr(&partial);
+    if (rc) return rc;
+    const int nb = red_blocks(n_atoms);
+    if (nb > 0) {
+        k_sum_stage1<<<nb, 256, 0, st>>>(n_atoms, e_atom, partial);
+        GMNN_LAUNCHED();
+    }
+    k_sum_stage2<<<1, 256, 0, st>>>(nb, partial, 1.0, energy, nullptr, nullptr);
+    GMNN_LAUNCHED();
+    GMNN_CUDA(cudaGetLastError());
+    return GMNN_OK;
+}
