@@ -153,7 +153,9 @@ static int ensemble_pass(gmnn_system *s, const float *positions, float *e_mean, 
         int maxw = 0;
         for (int l = 1; l <= L; ++l) maxw = std::max(maxw, mdl->dims[l]);
         const size_t NP = (size_t)((s->N + 127) / 128 * 128);
-        const double per_head = (double)NP * (2.0 * maxw + mdl->n_features + mdl->hp.n_radial * PSI) * 4.0;
+        const bool pairbuf = s->force_mode == GMNN_FORCE_PAIRBUF && s->list_has_rev;
+        const double per_head = (double)NP * (2.0 * maxw + mdl->n_features + mdl->hp.n_radial * PSI) * 4.0 +
+                                (pairbuf ? (double)s->N * (16.0 * s->cap + 12.0) : 0.0);
         HB = (int)std::min<double>((double)M, std::floor(2.0e9 / per_head));
         if (HB >= 2 && s->ens_cap < HB) {
             dev_free(s->ens_dZ[0]); dev_free(s->ens_dZ[1]); dev_free(s->ens_dG); dev_free(s->ens_A);
@@ -169,7 +171,17 @@ static int ensemble_pass(gmnn_system *s, const float *positions, float *e_mean, 
             }
             s->ens_cap = HB;
         }
+        if (HB >= 2 && pairbuf && (!s->ens_gbuf || s->ens_gcap < s->cap || s->ens_gheads < HB)) {  // heads' pair buffers
+            dev_free(s->ens_gbuf); dev_free(s->ens_f);
+            s->ens_gcap = 0, s->ens_gheads = 0;
+            if ((rc = dev_alloc(&s->ens_gbuf, (size_t)s->N * s->cap * HB)) || (rc = dev_alloc(&s->ens_f, (size_t)3 * s->N * HB))) {
+                set_error("out of device memory for the batched pair buffers (%d heads x %lld atoms x %d)", HB, (long long)s->N, s->cap);
+                return rc;
+            }
+            s->ens_gcap = s->cap, s->ens_gheads = HB;
+        }
     }
+    const bool heads_kernel = HB >= 2 && s->force_mode == GMNN_FORCE_PAIRBUF && s->list_has_rev && s->ens_gbuf;
     struct BatchOff {  // the batch state never outlives the pass
         gmnn_system *s;
         ~BatchOff() { s->ens_batch = 0, s->ens_head = 0; }
@@ -182,6 +194,11 @@ static int ensemble_pass(gmnn_system *s, const float *positions, float *e_mean, 
             if ((rc = launch_mlp_backward_tc_heads(s, m0, hb, st))) return rc;
             s->ens_batch = hb;
             if ((rc = launch_contract_backward(s, st))) return rc;
+        }
+        if (heads_kernel) {  // pair backward of the whole batch: geometry and radial functions once per pair and head chunk
+            if ((rc = launch_pair_backward_heads_welford(s, m0, hb, f_mean, f_var, st))) return rc;
+            s->ens_batch = 0;
+            continue;
         }
         for (int mm = 0; mm < hb; ++mm) {
             const int m = m0 + mm;
@@ -508,7 +525,7 @@ void gmnn_system_destroy(gmnn_system *s) {
     dev_free(s->dZ[0]); dev_free(s->dZ[1]); dev_free(s->Bv); dev_free(s->BvT); dev_free(s->BvTs); dev_free(s->BvTh); dev_free(s->amax); dev_free(s->vhead); dev_free(s->head_w);
     dev_free(s->ypart); dev_free(s->e_heads); dev_free(s->e_atom); dev_free(s->f_int); dev_free(s->f_tmp); dev_free(s->partial);
     dev_free(s->e_total); dev_free(s->flags); dev_free(s->ens_scratch); dev_free(s->nhc); dev_free(s->lang_step);
-    dev_free(s->ens_dZ[0]); dev_free(s->ens_dZ[1]); dev_free(s->ens_dG); dev_free(s->ens_A);
+    dev_free(s->ens_dZ[0]); dev_free(s->ens_dZ[1]); dev_free(s->ens_dG); dev_free(s->ens_A); dev_free(s->ens_gbuf); dev_free(s->ens_f);
     dev_free(s->ens_BvT); dev_free(s->ens_BvTs); dev_free(s->ens_BvTh);
     dev_free(s->kT_now); dev_free(s->sched_steps); dev_free(s->sched_temps); dev_free(s->sched_step);
     dev_free(s->stage_pos); dev_free(s->stage_f); dev_free(s->stage_e);

@@ -198,6 +198,11 @@ struct gmnn_system {
     // are ordered [atom tile][head]; 0 / 1 outside such a pass.  ens_head: the head the pair backward reads.
     int ens_batch = 0, ens_head = 0, ens_cap = 0;  // ens_cap: heads the buffers below hold
     float *ens_dZ[2] = {}, *ens_dG = nullptr, *ens_A = nullptr;
+    // pair-buffer force mode: per-head own-direction force sums [heads][3 N] and pair buffers [heads][N cap] of the batch
+    // (k_pair_backward_heads); ens_gcap = the list capacity they were sized for
+    float *ens_f = nullptr;
+    float4 *ens_gbuf = nullptr;
+    int ens_gcap = 0, ens_gheads = 0;
     float *ens_BvT = nullptr, *ens_BvTs = nullptr;
     uint16_t *ens_BvTh = nullptr;
     float *ens_scratch = nullptr;    // [11 N] switching-mode samples: kept forces, e_mean, e_var, f_mean, f_var (lazy)
@@ -257,6 +262,7 @@ int launch_contract_forward(gmnn_system *s, cudaStream_t st);
 int launch_contract_backward(gmnn_system *s, cudaStream_t st);
 int launch_pair_backward(gmnn_system *s, cudaStream_t st);  // dispatches on force_mode
 int launch_pair_backward_welford(gmnn_system *s, int head, float *f_mean, float *f_m2, cudaStream_t st);  // a12, one head
+int launch_pair_backward_heads_welford(gmnn_system *s, int head_first, int n_heads, float *f_mean, float *f_m2, cudaStream_t st);  // a12, a batch of heads
 
 // mlp_tc.cu
 int launch_split_stack(const float *src, float *dst, int64_t n, cudaStream_t st);  // dst[0..n) hi, dst[n..2n) lo

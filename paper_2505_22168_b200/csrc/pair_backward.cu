@@ -293,6 +293,240 @@ k_welford_perm(int64_t N, const float *__restrict__ f_int, const int32_t *__rest
     for (int a = 0; a < 3; ++a) welford_update(head, f_int[3 * i + a], f_mean + 3 * c + a, f_m2 + 3 * c + a);
 }
 
+// ---------------------------------------------------------------------------------------------
+// a12, pair-buffer form, several heads per launch (batched shallow-ensemble pass, gmnn_api.cu ensemble_pass).
+// The geometry of a pair, its radial functions R_s, R'_s and the 20 monomials do not depend on the head: they are
+// evaluated once per pair and chunk of HC heads (blockIdx.y = chunk), and only the gradient polynomial runs per head with
+// that head's adjoint A^(m)_i (rows [atom tile][head][128] of ens_A, staged in shared memory: HC x 400 bytes per centre).
+// Head m's own-direction sums go to f_h[m][3 N], its g_ij into gbuf_h[m][N cap]: the same values and the same summation
+// order as k_pair_backward<PAIRBUF> launched once per head.
+// ---------------------------------------------------------------------------------------------
+constexpr int PB_HC = 8;  // heads per chunk at most
+
+template <int NR, int NB, int LPA, bool GENERAL>
+__global__ void __launch_bounds__(128)
+k_pair_backward_heads(int64_t N, const float4 *__restrict__ pos4, const uint32_t *__restrict__ nbr,
+                      const int32_t *__restrict__ count, int cap, Geometry geo, RadialParams rp,
+                      const float *__restrict__ beta, const float *__restrict__ A, float *__restrict__ f_h,
+                      const uint16_t *__restrict__ rev, float4 *__restrict__ gbuf_h, int a_heads, int hc_max) {
+    constexpr int KB = (NB + 3) & ~3;
+    constexpr int ROW = NR * KB;
+    constexpr int GROUPS = 128 / LPA;
+    constexpr int AQ = NR * PSI / 4;  // float4 per adjoint row
+    extern __shared__ float s_mem[];
+    float *s_beta = s_mem;
+    float4 *s_A = reinterpret_cast<float4 *>(s_mem + ((rp.n_species * rp.n_species * ROW + 3) & ~3));
+    for (int q = threadIdx.x; q < rp.n_species * rp.n_species * ROW; q += blockDim.x) s_beta[q] = beta[q];
+    const int head0 = blockIdx.y * hc_max;
+    const int hc = a_heads - head0 < hc_max ? a_heads - head0 : hc_max;
+    const int64_t gt = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    const int64_t i = gt / LPA;
+    const int sub = (int)(gt % LPA);
+    const int grp = threadIdx.x / LPA;
+    const bool live = i < N;
+    {  // stage A^(m)_i of the block's centres and the chunk's heads: [group][head][AQ]
+        const int64_t first = blockIdx.x * (int64_t)GROUPS;
+        const float4 *src = reinterpret_cast<const float4 *>(A);
+        for (int q = threadIdx.x; q < GROUPS * hc * AQ; q += blockDim.x) {
+            const int g = q / (hc * AQ), h = (q / AQ) % hc, e = q % AQ;
+            const int64_t ia = first + g;
+            const int64_t ra = ((ia >> 7) * a_heads + head0 + h) * 128 + (ia & 127);
+            s_A[(g * hc_max + h) * AQ + e] = ia < N ? __ldg(&src[ra * AQ + e]) : make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+    }
+    __syncthreads();
+    // own-direction force sums of this thread, one triple per head of the chunk, in shared memory ([head][component][thread]:
+    // conflict-free), so that the head loop below stays rolled (one instance of the gradient polynomial in the code)
+    float *s_f = reinterpret_cast<float *>(s_A + GROUPS * hc_max * AQ);
+    for (int q = 0; q < 3 * hc; ++q) s_f[q * 128 + threadIdx.x] = 0.f;
+    if (live) {
+        const float4 xi = pos4[i];
+        const int zi = __float_as_int(xi.w);
+        const int cnt = count[i];
+        const uint4 *row = reinterpret_cast<const uint4 *>(nbr + i * (int64_t)cap);
+        const uint2 *rrow = reinterpret_cast<const uint2 *>(rev + i * (int64_t)cap);
+        const float4 *Ai = s_A + grp * hc_max * AQ;
+        const int64_t hstride = N * (int64_t)cap;  // float4 per head in gbuf_h
+        uint4 e_next = make_uint4(0u, 0u, 0u, 0u);
+        uint2 r_next = make_uint2(0u, 0u);
+        if (sub * 4 < cnt) {
+            e_next = __ldg(&row[sub]);
+            r_next = __ldg(&rrow[sub]);
+        }
+        for (int k4 = sub; k4 * 4 < cnt; k4 += LPA) {
+            const uint4 e4 = e_next;
+            const uint2 r2 = r_next;
+            if ((k4 + LPA) * 4 < cnt) {
+                e_next = __ldg(&row[k4 + LPA]);
+                r_next = __ldg(&rrow[k4 + LPA]);
+            }
+#pragma unroll 1
+            for (int q = 0; q < 4; ++q) {
+                if (k4 * 4 + q >= cnt) break;
+                const uint32_t ent = q == 0 ? e4.x : q == 1 ? e4.y : q == 2 ? e4.z : e4.w;
+                const uint32_t rv = ((q < 2 ? r2.x : r2.y) >> ((q & 1) * 16)) & 0xFFFFu;
+                const PairGeom pg = pair_geometry(ent, xi, pos4, geo);
+                if (rv == 0xFFFFu) continue;  // no partner (overflowed rebuild): flagged by k_build_rev
+                float4 *slot = gbuf_h + (int64_t)head0 * hstride + (int64_t)pg.j * cap + rv;
+                if (pg.r2 >= rp.r_cut2) {  // skin shell
+                    for (int h = 0; h < hc; ++h) slot[h * hstride] = make_float4(0.f, 0.f, 0.f, 0.f);
+                    continue;
+                }
+                const float rinv = rsqrtf(pg.r2);
+                const float r = pg.r2 * rinv;
+                float phi[NB], dphi[NB], fc, dfc;
+                radial_basis<NB, true, GENERAL>(rp, r, rinv, phi, dphi, fc, dfc);
+                const float ux = pg.dx * rinv, uy = pg.dy * rinv, uz = pg.dz * rinv;
+                float mono[PSI];
+                monomials(ux, uy, uz, mono);
+                const float4 *bt = reinterpret_cast<const float4 *>(s_beta + (zi * rp.n_species + pg.zj) * ROW);
+                float R[NR], dR[NR];
+#pragma unroll
+                for (int s = 0; s < NR; ++s) {
+                    float2 sd = make_float2(0.f, 0.f);
+#pragma unroll
+                    for (int kq = 0; kq < KB / 4; ++kq) {
+                        const float4 b = bt[s * (KB / 4) + kq];
+                        const float bv[4] = {b.x, b.y, b.z, b.w};
+#pragma unroll
+                        for (int c = 0; c < 4; ++c)
+                            if (4 * kq + c < NB)
+                                sd = __ffma2_rn(make_float2(bv[c], bv[c]), make_float2(phi[4 * kq + c], dphi[4 * kq + c]), sd);
+                    }
+                    R[s] = fc * sd.x;
+                    dR[s] = dfc * sd.x + fc * sd.y;
+                }
+                float de = 0.f;
+                if (GENERAL && rp.zbl_on && pg.r2 < rp.zbl_r_max2) {  // ZBL: the same term in every head
+                    float e;
+                    zbl_half<true>(rp, zi, pg.zj, r, rinv, e, de);
+                }
+#pragma unroll 1
+                for (int h = 0; h < hc; ++h) {
+                    const float4 *Ah = Ai + h * AQ;
+                    float gx, gy, gz;
+                    pair_gradient<NR>([&](int s, int qq) { return Ah[s * (PSI / 4) + qq]; }, R, dR, mono, ux, uy, uz, rinv,
+                                      gx, gy, gz);
+                    if (GENERAL) gx = fmaf(de, ux, gx), gy = fmaf(de, uy, gy), gz = fmaf(de, uz, gz);
+                    slot[h * hstride] = make_float4(gx, gy, gz, 0.f);
+                    float *f = s_f + (3 * h) * 128 + threadIdx.x;
+                    f[0] += gx, f[128] += gy, f[256] += gz;
+                }
+            }
+        }
+    }
+    for (int h = 0; h < hc; ++h) {
+        float fx = s_f[(3 * h) * 128 + threadIdx.x], fy = s_f[(3 * h + 1) * 128 + threadIdx.x], fz = s_f[(3 * h + 2) * 128 + threadIdx.x];
+#pragma unroll
+        for (int o = LPA / 2; o >= 1; o >>= 1) {
+            fx += __shfl_xor_sync(0xffffffffu, fx, o);
+            fy += __shfl_xor_sync(0xffffffffu, fy, o);
+            fz += __shfl_xor_sync(0xffffffffu, fz, o);
+        }
+        if (live && sub == 0) {
+            float *f = f_h + (int64_t)(head0 + h) * 3 * N + 3 * i;
+            f[0] = fx, f[1] = fy, f[2] = fz;
+        }
+    }
+}
+
+// Force of every head of the batch (f_h[m] minus the received row of gbuf_h[m], summed as in k_force_reduce), folded into
+// the running statistics over the heads in head order (Eq. 5; welford_update as in the head-by-head path).
+template <int LPA>
+__global__ void __launch_bounds__(256)
+k_force_reduce_heads(int64_t N, const int32_t *__restrict__ count, int cap, const float4 *__restrict__ gbuf_h,
+                     const float *__restrict__ f_h, const int32_t *__restrict__ perm, int head_first, int n_heads,
+                     float *__restrict__ f_mean, float *__restrict__ f_m2) {
+    const int64_t gt = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    const int64_t i = gt / LPA;
+    const int sub = (int)(gt % LPA);
+    const int cnt = i < N ? count[i] : 0;
+    const int64_t hstride = N * (int64_t)cap;
+    for (int h = 0; h < n_heads; ++h) {
+        float fx = 0.f, fy = 0.f, fz = 0.f;
+        if (i < N) {
+            const float4 *row = gbuf_h + h * hstride + i * (int64_t)cap;
+            for (int k = sub; k < cnt; k += LPA) {
+                const float4 g = __ldcs(&row[k]);
+                fx += g.x, fy += g.y, fz += g.z;
+            }
+        }
+#pragma unroll
+        for (int o = LPA / 2; o >= 1; o >>= 1) {
+            fx += __shfl_xor_sync(0xffffffffu, fx, o);
+            fy += __shfl_xor_sync(0xffffffffu, fy, o);
+            fz += __shfl_xor_sync(0xffffffffu, fz, o);
+        }
+        if (i < N && sub == 0) {
+            const int64_t c = perm[i];
+            const float *f = f_h + (int64_t)h * 3 * N + 3 * i;
+            welford_update(head_first + h, f[0] - fx, f_mean + 3 * c, f_m2 + 3 * c);
+            welford_update(head_first + h, f[1] - fy, f_mean + 3 * c + 1, f_m2 + 3 * c + 1);
+            welford_update(head_first + h, f[2] - fz, f_mean + 3 * c + 2, f_m2 + 3 * c + 2);
+        }
+    }
+}
+
+template <int NR, int NB>
+static int pair_backward_heads_lpa(gmnn_system *s, cudaStream_t st, int lpa, int head_first, int n_heads, float *f_mean,
+                                   float *f_m2) {
+    const gmnn_model *m = s->model;
+    if (!(s->force_mode == GMNN_FORCE_PAIRBUF && s->list_has_rev && s->rev && s->ens_gbuf && s->ens_f)) {
+        set_error("batched pair backward needs the pair-buffer force mode and its batch buffers");
+        return GMNN_INVALID_ARG;
+    }
+    const int beta_floats = (m->rp.n_species * m->rp.n_species * NR * m->rp.kb + 3) & ~3;
+    const int groups = 128 / lpa;
+    // heads per chunk: at most PB_HC, and at most what 96 KB of shared memory hold beside the table
+    int hc = (96 * 1024 - (int)sizeof(float) * beta_floats) / (groups * NR * PSI * (int)sizeof(float));
+    hc = hc > PB_HC ? PB_HC : (hc < 1 ? 1 : hc);
+    hc = hc > n_heads ? n_heads : hc;
+    const size_t smem = sizeof(float) * (beta_floats + (size_t)groups * hc * NR * PSI + (size_t)3 * hc * 128);
+    const dim3 grid(nblocks(s->N * lpa, 128), (unsigned)((n_heads + hc - 1) / hc));
+    const bool general = m->rp.basis_kind != 0 || m->rp.zbl_on;
+#define GMNN_PBH_LAUNCH(L, GEN)                                                                                      \
+    k_pair_backward_heads<NR, NB, L, GEN><<<grid, 128, smem, st>>>(s->N, s->pos4, s->nbr, s->count, s->cap, s->geo, m->rp, \
+                                                                  m->beta, s->ens_A, s->ens_f, s->rev, s->ens_gbuf, n_heads, hc)
+#define GMNN_PBH(L)                                                                                                  \
+    case L: {                                                                                                        \
+        static size_t opted_on[MAX_DEVICES] = {};                                                                    \
+        size_t &opted = opted_on[current_device()];                                                                  \
+        if (smem > 48 * 1024 && smem > opted) {                                                                      \
+            GMNN_CUDA(cudaFuncSetAttribute(k_pair_backward_heads<NR, NB, L, false>,                                  \
+                                           cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));                 \
+            GMNN_CUDA(cudaFuncSetAttribute(k_pair_backward_heads<NR, NB, L, true>,                                   \
+                                           cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));                 \
+            opted = smem;                                                                                            \
+        }                                                                                                            \
+        if (general) GMNN_PBH_LAUNCH(L, true);                                                                       \
+        else GMNN_PBH_LAUNCH(L, false);                                                                              \
+    } break;
+    switch (lpa) {
+        GMNN_PBH(1) GMNN_PBH(2) GMNN_PBH(4) GMNN_PBH(8) GMNN_PBH(16) GMNN_PBH(32)
+        default:
+            set_error("lanes_per_atom must be 1, 2, 4, 8, 16 or 32");
+            return GMNN_INVALID_ARG;
+    }
+#undef GMNN_PBH
+#undef GMNN_PBH_LAUNCH
+    GMNN_LAUNCHED();
+    k_force_reduce_heads<8><<<nblocks(s->N * 8, 256), 256, 0, st>>>(s->N, s->count, s->cap, s->ens_gbuf, s->ens_f, s->perm,
+                                                                   head_first, n_heads, f_mean, f_m2);
+    GMNN_LAUNCHED();
+    GMNN_CUDA(cudaGetLastError());
+    return GMNN_OK;
+}
+
+// a12, batched: pair backward and force statistics of heads [head_first, head_first + n_heads) of the ensemble, whose
+// adjoints are the batch in ens_A (n_heads = s->ens_batch)
+int launch_pair_backward_heads_welford(gmnn_system *s, int head_first, int n_heads, float *f_mean, float *f_m2, cudaStream_t st) {
+    const gmnn_model *m = s->model;
+    if (m->hp.n_radial == 5 && m->hp.n_basis == 7)
+        return pair_backward_heads_lpa<5, 7>(s, st, pick_lpa(s, true), head_first, n_heads, f_mean, f_m2);
+    set_error("pair kernels are instantiated for n_radial = 5, n_basis = 7 only");
+    return GMNN_UNSUPPORTED;
+}
+
 // wf_head >= 0: the ensemble pass of head wf_head; the force goes into the Welford statistics (f_mean, f_m2: caller order)
 template <int NR, int NB>
 static int pair_backward_lpa(gmnn_system *s, cudaStream_t st, int lpa, int wf_head = -1, float *f_mean = nullptr,
