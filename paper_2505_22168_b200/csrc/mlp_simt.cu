@@ -127,24 +127,31 @@ static int sgemm(int epi, int64_t M, int N, int K, const float *A, const float *
     return GMNN_OK;
 }
 
-// One thread per atom, H tile-transposed (coalesced along atoms): y_m = h . W_last[:, m] + b_last[m];
-// E^(m) = sigma y_m + mu; e_atom = sum_m c_m E^(m).  Heads are taken 8 at a time.
+// H tile-transposed (coalesced along atoms): y_m = h . W_last[:, m] + b_last[m]; E^(m) = sigma y_m + mu;
+// e_atom = sum_m c_m E^(m).
 // Rows row0 .. row0 + rows of one segment (Ht, Wl, bl already point at the segment / its weight set); e_heads and
 // e_atom are indexed by the internal atom of the row (row_atom; identity when null).
-__global__ void __launch_bounds__(128)
+// One thread per (atom, group of 8 heads): 64 atoms x ceil(M / 8) groups per block, so that a 32-head model spreads
+// 8 192 atoms over 128 blocks of 8 warps (one thread per atom for all heads left 64 blocks of 4 warps: 0.54 ms at
+// config 4).  Every head's sum runs over k in the same order as before; e_atom = sum_m head_w[m] E^(m) is chained in
+// head order by the first group's thread from the energies the groups leave in shared memory.
+constexpr int HEADS_ATOMS = 64, HEADS_MAX = 64;
+__global__ void __launch_bounds__(HEADS_ATOMS *(HEADS_MAX / 8))
 k_heads(int64_t row0, int64_t rows, const float *__restrict__ Ht, int Hd, const float *__restrict__ Wl,
         const float *__restrict__ bl, int M, const float4 *__restrict__ pos4, const float *__restrict__ scale,
         const float *__restrict__ shift, const float *__restrict__ head_w, float *__restrict__ e_heads,
         float *__restrict__ e_atom, const int32_t *__restrict__ row_atom, const float *__restrict__ e_zbl) {
-    const int64_t r = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;  // blockDim.x == 128 == tile
-    if (r >= rows) return;
-    const int64_t i = row_atom ? (int64_t)row_atom[row0 + r] : row0 + r;
-    const float *h = Ht + (int64_t)blockIdx.x * Hd * 128 + threadIdx.x;
-    const int z = __float_as_int(pos4[i].w);
-    // ZBL (an empirical correction outside the network): every head's energy carries it once
-    const float sg = __ldg(&scale[z]), mu = __ldg(&shift[z]) + (e_zbl ? __ldg(&e_zbl[i]) : 0.f);
-    float e = 0.f;
-    for (int m0 = 0; m0 < M; m0 += 8) {
+    __shared__ float s_em[HEADS_MAX * HEADS_ATOMS];
+    const int a = threadIdx.x % HEADS_ATOMS, g = threadIdx.x / HEADS_ATOMS;
+    const int64_t r = blockIdx.x * (int64_t)HEADS_ATOMS + a;
+    const bool live = r < rows;
+    const int64_t i = live ? (row_atom ? (int64_t)row_atom[row0 + r] : row0 + r) : 0;
+    if (live) {
+        const float *h = Ht + (r >> 7) * Hd * 128 + (r & 127);  // tile-transposed [rows / 128][Hd][128]
+        const int z = __float_as_int(pos4[i].w);
+        // ZBL (an empirical correction outside the network): every head's energy carries it once
+        const float sg = __ldg(&scale[z]), mu = __ldg(&shift[z]) + (e_zbl ? __ldg(&e_zbl[i]) : 0.f);
+        const int m0 = 8 * g;
         float p[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
         const int nm = M - m0 < 8 ? M - m0 : 8;
         if (nm == 1) {
@@ -163,10 +170,15 @@ k_heads(int64_t row0, int64_t rows, const float *__restrict__ Ht, int Hd, const 
             if (c < nm) {
                 const float em = sg * (p[c] + __ldg(&bl[m0 + c])) + mu;
                 e_heads[i * (int64_t)M + m0 + c] = em;
-                e = fmaf(__ldg(&head_w[m0 + c]), em, e);
+                s_em[(m0 + c) * HEADS_ATOMS + a] = em;
             }
     }
-    e_atom[i] = e;
+    __syncthreads();
+    if (live && g == 0) {
+        float e = 0.f;
+        for (int m = 0; m < M; ++m) e = fmaf(__ldg(&head_w[m]), s_em[m * HEADS_ATOMS + a], e);
+        e_atom[i] = e;
+    }
 }
 
 // v[k] = sum_m c_m W_last[k][m]
@@ -251,7 +263,7 @@ int launch_mlp_heads(gmnn_system *s, const float *head_w_dev, cudaStream_t st) {
                 mean ? m->w_mean + (size_t)t * (Hd + 1) + Hd : m->b[L] + (size_t)t * M, s->pos4, m->scale, m->shift,
                 head_w_dev, mean ? nullptr : s->e_heads, s->e_atom, s->row_atom, s->e_zbl);
         } else {
-            k_heads<<<(unsigned)((real + 127) / 128), 128, 0, st>>>(
+            k_heads<<<(unsigned)((real + HEADS_ATOMS - 1) / HEADS_ATOMS), HEADS_ATOMS * ((M + 7) / 8), 0, st>>>(
                 r0, real, tile_rows(s->H[L - 1], r0, Hd), Hd, m->W[L] + t * m->wsize(L), m->b[L] + (size_t)t * M, M, s->pos4,
                 m->scale, m->shift, head_w_dev, s->e_heads, s->e_atom, s->row_atom, s->e_zbl);
         }
