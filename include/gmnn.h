@@ -121,6 +121,8 @@ void gmnn_system_destroy(gmnn_system *s);
 
 /* Tuning / diagnostics knobs (never needed for correctness):
  *   "lanes_per_atom"  1,2,4,8,16,32: lanes that share one centre atom in the pair kernels (0 = auto)
+ *   "ensemble_batch"  0 (default: as many as 4 GB of batch buffers hold) .. 64: heads per batch of the shallow-ensemble
+ *                     backward at most (1 = head by head)
  *   "profile"         1: record a CUDA event after every stage of every later energy_forces / md call
  *                     (gmnn_stage_times); setting it (to 0 or 1) discards what was recorded
  *   "md_continue"     1: a gmnn_md_verlet_steps call whose positions and velocities are exactly the

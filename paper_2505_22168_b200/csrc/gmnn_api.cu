@@ -145,7 +145,7 @@ static int ensemble_pass(gmnn_system *s, const float *positions, float *e_mean, 
     if ((rc = launch_mlp_heads(s, s->model->head_mean_w, st))) return rc;
     if ((rc = launch_ensemble_energy_stats(s, e_mean, e_var, st))) return rc;
     // Heads batched through the backward GEMMs and the contraction backward (mlp_tc.cu launch_mlp_backward_tc_heads): as many
-    // heads per pass as 2 GB of batch buffers hold; tensor-core split modes with one weight set.  Else head by head.
+    // heads per pass as 4 GB of batch buffers hold (at least one); tensor-core split modes with one weight set.  Else head by head.
     const gmnn_model *mdl = s->model;
     const int L = mdl->hp.n_hidden;
     int HB = 1;
@@ -156,7 +156,8 @@ static int ensemble_pass(gmnn_system *s, const float *positions, float *e_mean, 
         const bool pairbuf = s->force_mode == GMNN_FORCE_PAIRBUF && s->list_has_rev;
         const double per_head = (double)NP * (2.0 * maxw + mdl->n_features + mdl->hp.n_radial * PSI) * 4.0 +
                                 (pairbuf ? (double)s->N * (16.0 * s->cap + 12.0) : 0.0);
-        HB = (int)std::min<double>((double)M, std::floor(2.0e9 / per_head));
+        HB = (int)std::max(1.0, std::min<double>((double)M, std::floor(4.0e9 / per_head)));
+        if (s->ens_batch_max > 0 && HB > s->ens_batch_max) HB = s->ens_batch_max;  // knob "ensemble_batch"
         if (HB >= 2 && s->ens_cap < HB) {
             dev_free(s->ens_dZ[0]); dev_free(s->ens_dZ[1]); dev_free(s->ens_dG); dev_free(s->ens_A);
             dev_free(s->ens_BvT); dev_free(s->ens_BvTs); dev_free(s->ens_BvTh);
@@ -557,6 +558,12 @@ int gmnn_system_set_int(gmnn_system *s, const char *key, int64_t v) {
             s->events.push_back(e);
             s->stage_names.push_back(nullptr);
         }
+    } else if (!strcmp(key, "ensemble_batch")) {
+        if (v < 0 || v > 64) {
+            set_error("ensemble_batch must be in [0, 64]");
+            return GMNN_INVALID_ARG;
+        }
+        s->ens_batch_max = (int)v;
     } else if (!strcmp(key, "md_continue")) {
         s->md_continue = v != 0;
     } else if (!strcmp(key, "md_graph")) {
@@ -614,6 +621,7 @@ int gmnn_system_set_int(gmnn_system *s, const char *key, int64_t v) {
 int gmnn_system_get_int(const gmnn_system *s, const char *key, int64_t *v) {
     if (!s || !key || !v) return GMNN_INVALID_ARG;
     if (!strcmp(key, "lanes_per_atom")) *v = s->lanes_per_atom;
+    else if (!strcmp(key, "ensemble_batch")) *v = s->ens_batch_max;
     else if (!strcmp(key, "profile")) *v = s->profile;
     else if (!strcmp(key, "md_continue")) *v = s->md_continue;
     else if (!strcmp(key, "md_graph")) *v = s->md_graph;

@@ -49,6 +49,31 @@ def test_ensemble_statistics(gm, orc, name):
     assert energy_atom_error(ea.cpu().numpy().astype(np.float64), e_mean) <= 1.0
 
 
+@pytest.mark.parametrize("batch", [1, 5, 12])
+@pytest.mark.parametrize("mlp_precision", [2, 3])
+def test_ensemble_batches_of_heads(gm, orc, batch, mlp_precision):
+    """The batched pass (all heads through one backward GEMM chain, one pair-backward kernel for 8 heads at a time) in
+    uneven batches -- 5 + 5 + 5 + 5 + 5 + 5 + 2, 12 + 12 + 8, and head by head -- against the oracle, at the bounds of the
+    unbatched test; batches differ from one another only by the power-of-two operand scales of the split GEMMs."""
+    w = wl.li3po4_box(1024, n_heads=32)
+    m = orc.Model(w.model)
+    pairs = orc.auto_neighbors(w.positions, w.cell, w.pbc, r_list32(w.model.r_cut, w.skin))
+    ref = orc.ensemble(m, w.positions, w.species, w.cell, pairs)
+    mode = gm.GMNN_MLP_3XF16 if mlp_precision == 3 else gm.GMNN_MLP_3XTF32
+    _, sysm, pos = _build(gm, w, mlp_precision=mode, force_mode=gm.GMNN_FORCE_PAIRBUF)
+    full = [t.cpu().numpy().astype(np.float64) for t in sysm.ensemble_energy_forces(pos)]
+    sysm.set_int("ensemble_batch", batch)
+    part = [t.cpu().numpy().astype(np.float64) for t in sysm.ensemble_energy_forces(pos)]
+    sysm.set_int("ensemble_batch", 0)
+    for e_mean, e_var, f_mean, f_var in (full, part):
+        assert energy_atom_error(e_mean, ref.e_mean) <= 1.0
+        assert force_error(f_mean, ref.f_mean) <= F_TOL
+        assert np.abs(e_var - ref.e_var).max() <= 2e-4 * ref.e_var.max()
+        assert np.abs(f_var - ref.f_var).max() <= 2e-4 * ref.f_var.max()
+    assert force_error(part[2], full[2]) <= 2e-5 and np.abs(part[3] - full[3]).max() <= 1e-4 * full[3].max()
+    assert np.array_equal(part[0], full[0]) and np.array_equal(part[1], full[1])  # the forward does not depend on the batching
+
+
 def test_config4_full_size(gm, orc):
     """Config 4 at its stated size (8 192 atoms, 32 heads): e_mean, e_var, f_mean and f_var element by
     element against oracle O-10 (one forward, 32 backward passes in fp64; about 20 s on 16 cores), at the
