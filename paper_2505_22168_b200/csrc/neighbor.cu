@@ -222,7 +222,6 @@ k_build_cells(int64_t N, const float4 *__restrict__ pos4, const int32_t *__restr
               uint16_t *runs) {
     if (skip_rebuild(cond, thr2)) return;
     __shared__ uint32_t s_shell[8][SHELL_BUF];
-    __shared__ int s_rel[8][28];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     const unsigned below = (1u << lane) - 1u;
     // grid-stride over atoms (one warp each): the launch is a few waves of blocks, so that the
@@ -233,23 +232,40 @@ k_build_cells(int64_t N, const float4 *__restrict__ pos4, const int32_t *__restr
         const float pi3[3] = {xi.x, xi.y, xi.z};
         const int cx = cell_coord_of(g, pi3, 0), cy = cell_coord_of(g, pi3, 1), cz = cell_coord_of(g, pi3, 2);
         uint32_t *row = nbr + i * (int64_t)cap;
+        // The 27 neighbouring cells are described once, lane l < 27 computing cell l (periodic wrap, candidate range in
+        // the cell-sorted order, lattice shift and image code of the cell's image); the scan below takes cell idx's
+        // description from lane idx by shuffles.  (Every lane recomputing every cell's description cost two thirds
+        // of this kernel's 5.9 G warp instructions at config 5: it is instruction-bound.)
+        int cb = 0, ce = 0;
+        float csx = 0.f, csy = 0.f, csz = 0.f;
+        uint32_t ccode = 0u;
+        if (lane < 27) {
+            const int oz = lane / 9 - 1, oy = (lane / 3) % 3 - 1, ox = lane % 3 - 1;
+            bool ok = true;
+            int z = cz + oz, nz = 0;
+            if (z < 0) { ok = ok && g.pbc[2]; z += g.ncell[2]; nz = -1; }
+            else if (z >= g.ncell[2]) { ok = ok && g.pbc[2]; z -= g.ncell[2]; nz = 1; }
+            int y = cy + oy, ny = 0;
+            if (y < 0) { ok = ok && g.pbc[1]; y += g.ncell[1]; ny = -1; }
+            else if (y >= g.ncell[1]) { ok = ok && g.pbc[1]; y -= g.ncell[1]; ny = 1; }
+            int x = cx + ox, nx = 0;
+            if (x < 0) { ok = ok && g.pbc[0]; x += g.ncell[0]; nx = -1; }
+            else if (x >= g.ncell[0]) { ok = ok && g.pbc[0]; x -= g.ncell[0]; nx = 1; }
+            if (ok) {
+                const int c = (z * g.ncell[1] + y) * g.ncell[0] + x;
+                cb = cell_start[c], ce = cell_start[c + 1];
+            }
+            csx = list_shift(g, 0, nx, ny, nz), csy = list_shift(g, 1, nx, ny, nz), csz = list_shift(g, 2, nx, ny, nz);
+            ccode = image_code(nx, ny, nz);
+        }
+        const uint32_t home_code = image_code(0, 0, 0);
         // visit(idx, fn): candidates of cell idx in chunks of 32; fn(entry, r2, valid) per lane
         auto visit = [&](int idx, auto fn) {
-            const int oz = idx / 9 - 1, oy = (idx / 3) % 3 - 1, ox = idx % 3 - 1;
-            int z = cz + oz, nz = 0;
-            if (z < 0) { if (!g.pbc[2]) return; z += g.ncell[2]; nz = -1; }
-            else if (z >= g.ncell[2]) { if (!g.pbc[2]) return; z -= g.ncell[2]; nz = 1; }
-            int y = cy + oy, ny = 0;
-            if (y < 0) { if (!g.pbc[1]) return; y += g.ncell[1]; ny = -1; }
-            else if (y >= g.ncell[1]) { if (!g.pbc[1]) return; y -= g.ncell[1]; ny = 1; }
-            int x = cx + ox, nx = 0;
-            if (x < 0) { if (!g.pbc[0]) return; x += g.ncell[0]; nx = -1; }
-            else if (x >= g.ncell[0]) { if (!g.pbc[0]) return; x -= g.ncell[0]; nx = 1; }
-            const int c = (z * g.ncell[1] + y) * g.ncell[0] + x;
-            const int b = cell_start[c], e = cell_start[c + 1];
-            const float sx = list_shift(g, 0, nx, ny, nz), sy = list_shift(g, 1, nx, ny, nz), sz = list_shift(g, 2, nx, ny, nz);
-            const uint32_t code = image_code(nx, ny, nz);
-            const bool home = (nx | ny | nz) == 0;
+            const int b = __shfl_sync(0xffffffffu, cb, idx), e = __shfl_sync(0xffffffffu, ce, idx);
+            const float sx = __shfl_sync(0xffffffffu, csx, idx), sy = __shfl_sync(0xffffffffu, csy, idx),
+                        sz = __shfl_sync(0xffffffffu, csz, idx);
+            const uint32_t code = __shfl_sync(0xffffffffu, ccode, idx);
+            const bool home = code == home_code;
             for (int base = b; base < e; base += 32) {
                 const int j = base + lane;
                 const bool valid = j < e && !(home && j == (int)i);
@@ -258,11 +274,9 @@ k_build_cells(int64_t N, const float4 *__restrict__ pos4, const int32_t *__restr
             }
         };
         int n_in = 0, n_out = 0;
+        int run_in = 0, run_out = 0;  // lane idx: the counts when the scan reached cell idx
         for (int idx = 0; idx < 27; ++idx) {
-            if (lane == 0) {
-                if (runs) runs[i * RUNS_PITCH + idx] = (uint16_t)(n_in < cap ? n_in : cap);
-                s_rel[wid][idx] = n_out;
-            }
+            if (lane == idx) run_in = n_in, run_out = n_out;
             visit(idx, [&](uint32_t entry, float r2, bool valid) {
                 const bool kin = valid && r2 < g.r_cut2 && r2 < g.r_list2;
                 const bool kout = valid && !(r2 < g.r_cut2) && r2 < g.r_list2;
@@ -291,14 +305,17 @@ k_build_cells(int64_t N, const float4 *__restrict__ pos4, const int32_t *__restr
         }
         const int n = n_in + n_out;
         if (runs) {
-            if (lane < 27) runs[i * RUNS_PITCH + 27 + lane] = (uint16_t)(n_in + s_rel[wid][lane] < cap ? n_in + s_rel[wid][lane] : cap);
+            if (lane < 27) {
+                runs[i * RUNS_PITCH + lane] = (uint16_t)(run_in < cap ? run_in : cap);
+                runs[i * RUNS_PITCH + 27 + lane] = (uint16_t)(n_in + run_out < cap ? n_in + run_out : cap);
+            }
             if (lane == 0) runs[i * RUNS_PITCH + 54] = (uint16_t)(n < cap ? n : cap);
         }
         if (lane == 0) {
             count[i] = n < cap ? n : cap;
             if (n > cap) atomicMax(&flags[FLAG_MAXCOUNT], n);
         }
-        __syncwarp();  // s_shell / s_rel are reused for the warp's next atom
+        __syncwarp();  // s_shell is reused for the warp's next atom
     }
 }
 
