@@ -519,9 +519,11 @@ static inline unsigned small_grid(int64_t n_items) {
     const int64_t want = (n_items + 255) / 256, cap = 148 * 8;
     return (unsigned)(want < cap ? (want > 0 ? want : 1) : cap);
 }
-// blocks of 256 threads for a warp-per-atom grid-stride kernel: at most 16 waves of 148 SMs x 8 blocks
+// blocks of 256 threads for a warp-per-atom grid-stride kernel: at most 4 waves of 148 SMs x 8 blocks.  Measured at
+// config 5 (full build / the skipped launches of one MD step): 16 waves 6.25 ms / 0.14 ms, 8: 6.37 / 0.095, 4: 6.61 / 0.074,
+// 2: 7.3 / 0.064 -- at one rebuild per 20 to 50 steps 4 waves cost the least per step
 static inline unsigned warp_grid(int64_t n_atoms) {
-    const int64_t want = (n_atoms * 32 + 255) / 256, cap = 148 * 8 * 16;
+    const int64_t want = (n_atoms * 32 + 255) / 256, cap = 148 * 8 * 4;
     return (unsigned)(want < cap ? want : cap);
 }
 
