@@ -131,6 +131,11 @@ void gmnn_system_destroy(gmnn_system *s);
  *   "md_graph"        1 (default): gmnn_md_verlet_steps captures one step as a CUDA graph after the first
  *                     step and replays it (runs of >= 4 steps, not while "profile" is on); 0: eager loop.
  *                     Results are bit-identical either way
+ *   "ef_graph"        1 (default): gmnn_energy_forces (and the _host entry) captures the launches between the gather of the
+ *                     caller's positions and the scatter to the caller's outputs as a CUDA graph at the second call of an
+ *                     unchanged configuration and replays it afterwards (any gmnn_system_set_int, gmnn_build_neighbors or
+ *                     gmnn_system_set_udd_bias call drops it; not while "profile" is on, not for virial calls); 0: eager
+ *                     launches.  Results are bit-identical either way
  *   "capacity"        neighbour slots per atom for the next build (0 = estimate from the density)
  *   "mlp_precision", "force_mode": override the model's value for this system; changing force_mode
  *                     invalidates the neighbour list (call gmnn_build_neighbors again)

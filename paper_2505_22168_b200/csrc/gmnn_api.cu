@@ -93,34 +93,92 @@ static int mlp_backward(gmnn_system *s, const float *head_w, cudaStream_t st) {
     return launch_mlp_backward_tc(s, head_w, st);
 }
 
-// positions -> E_i, F (internal order), for the energy whose head weights are head_w (device)
+// Bumped by every call that can change what an evaluation launches (knobs, including the process-wide tc_* ones, a list
+// build, the UDD bias): a captured evaluation (below) is replayed only while the value it was captured at stands.
+static long long g_config_gen = 1;
+
+// positions -> E_i, F (internal order), for the energy whose head weights are head_w (device).
+// allow_graph (gmnn_energy_forces only): everything between the gather of the caller's positions and the scatter to the
+// caller's outputs touches library buffers only, so its launches (about 20; what bounds the call below some 10^4 atoms)
+// are captured once as a CUDA graph -- at the second call of an unchanged configuration, the first having done the
+// one-time set-up eagerly -- and replayed by later calls.  Not while stage events are recorded or a virial is asked for.
 static int forward_backward(gmnn_system *s, const float *positions, const float *head_w, bool check_stale,
-                            cudaStream_t st, StageTimer &T) {
+                            cudaStream_t st, StageTimer &T, bool allow_graph = false) {
     int rc;
     s->udd_active = s->udd_A != 0.f && s->model->hp.n_heads > 1 && head_w == s->model->head_mean_w;
     if (s->udd_active) s->use_mean_head = false;  // the bias needs every head's energy
     if ((rc = launch_gather_positions(s, positions, st, check_stale))) return rc;
     T.mark("gather");
-    if (s->mlp_precision == GMNN_MLP_3XF16)  // maxima of G, H, dZ: rebuilt by this evaluation's kernels
-        GMNN_CUDA(cudaMemsetAsync(s->amax, 0, sizeof(uint32_t) * AMAX_BVT, st));
-    if ((rc = launch_pair_forward(s, st))) return rc;
-    T.mark("pair_forward");
-    if ((rc = launch_contract_forward(s, st))) return rc;
-    T.mark("contract_forward");
-    if ((rc = mlp_forward(s, st))) return rc;
-    T.mark("mlp_forward");
-    if ((rc = launch_mlp_heads(s, head_w, st))) return rc;
-    if (s->udd_active) {  // UDD bias: the head weights of the backward come from this forward's head totals
-        if ((rc = launch_udd_weights(s, s->head_w, s->e_total + 4, st))) return rc;
-        head_w = s->head_w;
+    auto core = [&](cudaStream_t q, StageTimer &TT) -> int {
+        int r;
+        const float *hw = head_w;
+        if (s->mlp_precision == GMNN_MLP_3XF16)  // maxima of G, H, dZ: rebuilt by this evaluation's kernels
+            GMNN_CUDA(cudaMemsetAsync(s->amax, 0, sizeof(uint32_t) * AMAX_BVT, q));
+        if ((r = launch_pair_forward(s, q))) return r;
+        TT.mark("pair_forward");
+        if ((r = launch_contract_forward(s, q))) return r;
+        TT.mark("contract_forward");
+        if ((r = mlp_forward(s, q))) return r;
+        TT.mark("mlp_forward");
+        if ((r = launch_mlp_heads(s, hw, q))) return r;
+        if (s->udd_active) {  // UDD bias: the head weights of the backward come from this forward's head totals
+            if ((r = launch_udd_weights(s, s->head_w, s->e_total + 4, q))) return r;
+            hw = s->head_w;
+        }
+        TT.mark("mlp_heads");
+        if ((r = mlp_backward(s, hw, q))) return r;
+        TT.mark("mlp_backward");
+        if ((r = launch_contract_backward(s, q))) return r;
+        TT.mark("contract_backward");
+        if ((r = launch_pair_backward(s, q))) return r;
+        TT.mark("pair_backward");
+        return GMNN_OK;
+    };
+    if (!(allow_graph && s->ef_graph && !s->profile && !s->want_virial)) return core(st, T);
+    if (s->ef_exec && s->ef_gen == g_config_gen) {  // replay
+        GMNN_CUDA(cudaGraphLaunch(s->ef_exec, st));
+        g_launch_count += s->ef_launches;
+        return GMNN_OK;
     }
-    T.mark("mlp_heads");
-    if ((rc = mlp_backward(s, head_w, st))) return rc;
-    T.mark("mlp_backward");
-    if ((rc = launch_contract_backward(s, st))) return rc;
-    T.mark("contract_backward");
-    if ((rc = launch_pair_backward(s, st))) return rc;
-    T.mark("pair_backward");
+    if (s->ef_exec) {
+        cudaGraphExecDestroy(s->ef_exec);
+        s->ef_exec = nullptr;
+    }
+    if (s->ef_seen_gen != g_config_gen) {  // first call of this configuration: eagerly
+        s->ef_seen_gen = g_config_gen;
+        return core(st, T);
+    }
+    // second call: capture on the library's own stream (the caller's may be the legacy stream), then launch
+    if (!s->graph_stream) {
+        GMNN_CUDA(cudaStreamCreateWithFlags(&s->graph_stream, cudaStreamNonBlocking));
+        GMNN_CUDA(cudaEventCreateWithFlags(&s->graph_ev[0], cudaEventDisableTiming));
+        GMNN_CUDA(cudaEventCreateWithFlags(&s->graph_ev[1], cudaEventDisableTiming));
+    }
+    const long long launches_before = g_launch_count;
+    cudaGraph_t graph = nullptr;
+    GMNN_CUDA(cudaStreamBeginCapture(s->graph_stream, cudaStreamCaptureModeThreadLocal));
+    rc = core(s->graph_stream, T);
+    const cudaError_t cap = cudaStreamEndCapture(s->graph_stream, &graph);
+    s->ef_launches = g_launch_count - launches_before;
+    g_launch_count = launches_before;
+    if (rc || cap != cudaSuccess) {
+        if (graph) cudaGraphDestroy(graph);
+        if (!rc) {
+            set_error("CUDA graph capture of the energy-and-force evaluation failed: %s", cudaGetErrorString(cap));
+            rc = GMNN_CUDA_ERROR;
+        }
+        return rc;
+    }
+    const cudaError_t ge = cudaGraphInstantiate(&s->ef_exec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (ge != cudaSuccess) {
+        s->ef_exec = nullptr;
+        set_error("CUDA graph instantiation of the energy-and-force evaluation failed: %s", cudaGetErrorString(ge));
+        return GMNN_CUDA_ERROR;
+    }
+    s->ef_gen = g_config_gen;
+    GMNN_CUDA(cudaGraphLaunch(s->ef_exec, st));
+    g_launch_count += s->ef_launches;
     return GMNN_OK;
 }
 
@@ -518,6 +576,7 @@ int gmnn_system_create(const gmnn_model *m, int64_t n_atoms, const int32_t *spec
 
 void gmnn_system_destroy(gmnn_system *s) {
     if (!s) return;
+    if (s->ef_exec) cudaGraphExecDestroy(s->ef_exec);
     dev_free(s->mrow); dev_free(s->row_atom); dev_free(s->sp_count); dev_free(s->vir_atom); dev_free(s->e_zbl);
     dev_free(s->species); dev_free(s->cell_of); dev_free(s->cell_count); dev_free(s->cell_start);
     dev_free(s->cell_fill); dev_free(s->slot_tmp); dev_free(s->perm); dev_free(s->pos4); dev_free(s->xref);
@@ -542,6 +601,7 @@ void gmnn_system_destroy(gmnn_system *s) {
 
 int gmnn_system_set_int(gmnn_system *s, const char *key, int64_t v) {
     if (!s || !key) return GMNN_INVALID_ARG;
+    ++g_config_gen;  // any knob may change what an evaluation launches
     if (!strcmp(key, "lanes_per_atom")) {
         if (v != 0 && v != 1 && v != 2 && v != 4 && v != 8 && v != 16 && v != 32) {
             set_error("lanes_per_atom must be 0, 1, 2, 4, 8, 16 or 32");
@@ -568,6 +628,8 @@ int gmnn_system_set_int(gmnn_system *s, const char *key, int64_t v) {
         s->md_continue = v != 0;
     } else if (!strcmp(key, "md_graph")) {
         s->md_graph = v != 0;
+    } else if (!strcmp(key, "ef_graph")) {
+        s->ef_graph = v != 0;
     } else if (!strcmp(key, "capacity")) {
         if (v < 0 || v > 4096) {
             set_error("capacity must be in [0, 4096]");
@@ -625,6 +687,7 @@ int gmnn_system_get_int(const gmnn_system *s, const char *key, int64_t *v) {
     else if (!strcmp(key, "profile")) *v = s->profile;
     else if (!strcmp(key, "md_continue")) *v = s->md_continue;
     else if (!strcmp(key, "md_graph")) *v = s->md_graph;
+    else if (!strcmp(key, "ef_graph")) *v = s->ef_graph;
     else if (!strcmp(key, "capacity")) *v = s->cap;
     else if (!strcmp(key, "mlp_precision")) *v = s->mlp_precision;
     else if (!strcmp(key, "force_mode")) *v = s->force_mode;
@@ -650,6 +713,7 @@ int gmnn_build_neighbors(gmnn_system *s, const float *positions, const float cel
         return GMNN_INVALID_ARG;
     }
     if (int rcd = check_device(s->device, "gmnn_build_neighbors")) return rcd;
+    ++g_config_gen;  // geometry, capacity and buffers may change
     cudaStream_t st = (cudaStream_t)cuda_stream;
     if (r_cut != s->model->hp.r_cut) {
         set_error("r_cut = %g differs from the model's %g", r_cut, s->model->hp.r_cut);
@@ -919,7 +983,7 @@ int gmnn_energy_forces(gmnn_system *s, const float *positions, double *energy, f
     s->md_state_valid = false;
     StageTimer T(s, st);
     T.begin();
-    int rc = forward_backward(s, positions, s->model->head_mean_w, true, st, T);
+    int rc = forward_backward(s, positions, s->model->head_mean_w, true, st, T, true);
     if (rc) return rc;
     if ((rc = launch_scatter_outputs(s, energy_per_atom, forces, st))) return rc;
     if ((rc = launch_energy_sum(s, energy, st))) return rc;
@@ -1310,6 +1374,7 @@ int gmnn_system_set_udd_bias(gmnn_system *s, float A, float B) {
         set_error("gmnn_system_set_udd_bias: A must be finite and B > 0");
         return GMNN_INVALID_ARG;
     }
+    ++g_config_gen;
     s->udd_A = A;
     if (A != 0.f) s->udd_B = B;
     s->md_state_valid = false;

@@ -214,6 +214,11 @@ struct gmnn_system {
     int profile = 0;
     int md_graph = 1;                // knob: replay the MD step as a CUDA graph (not while profiling stages)
     cudaStream_t graph_stream = nullptr;  // capture / replay stream (the caller's may be the legacy stream)
+    // gmnn_energy_forces: the launches between the gather and the output scatter, captured at the second call of an unchanged
+    // configuration (gmnn_api.cu forward_backward); knob "ef_graph"
+    int ef_graph = 1;
+    cudaGraphExec_t ef_exec = nullptr;
+    long long ef_gen = 0, ef_seen_gen = 0, ef_launches = 0;
     cudaEvent_t graph_ev[2] = {};
     int md_continue = 0;             // knob: the next md call continues the previous one
     bool md_state_valid = false;     // f_tmp / e_total hold the forces and energies of the last md step

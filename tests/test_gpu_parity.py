@@ -269,3 +269,46 @@ def test_pair_buffer_force_mode(gm, orc, name):
     sysg.build_neighbors(pos, w.cell9, w.pbc, w.model.r_cut, w.skin)
     _, _, fp = sysg.energy_forces(pos)
     assert np.array_equal(fp.cpu().numpy(), f1.cpu().numpy())
+
+
+@pytest.mark.parametrize("mlp_precision", [0, 3])
+def test_energy_forces_graph_replay_is_bitwise_the_eager_call(gm, mlp_precision):
+    """gmnn_energy_forces replays its inner launches as a CUDA graph from the third call of an unchanged configuration
+    (knob "ef_graph"): same bits as the eager call, also at new positions, after a knob change, after a new list build
+    and after MD steps that rebuilt the list inside their loop."""
+    import torch
+
+    w = wl.li3po4_box(2000, hidden=(64, 64))
+    _, sysm, pos = _gpu_system(gm, w, mlp_precision=mlp_precision, force_mode=1)
+
+    def call(p):
+        e, ea, f = sysm.energy_forces(p)[:3]
+        return float(e.cpu()[0]), ea.cpu().numpy().copy(), f.cpu().numpy().copy()
+
+    def both(p, n=4):
+        sysm.set_int("ef_graph", 0)
+        ref = call(p)
+        sysm.set_int("ef_graph", 1)
+        n0 = gm.launch_count()
+        outs = [call(p) for _ in range(n)]  # eager, capture, replay, replay
+        per_call = (gm.launch_count() - n0) / n
+        for o in outs:
+            assert o[0] == ref[0] and np.array_equal(o[1], ref[1]) and np.array_equal(o[2], ref[2])
+        return per_call
+
+    launches = both(pos)
+    assert launches > 10  # replayed launches are counted
+    pos2 = pos + 0.02 * torch.randn_like(pos)  # inside the skin: same list, new positions through the same graph
+    both(pos2, n=1)
+    sysm.set_int("lanes_per_atom", 8)
+    both(pos2)
+    sysm.set_int("lanes_per_atom", 0)
+    sysm.build_neighbors(pos2, w.cell9, w.pbc, w.model.r_cut, w.skin)
+    both(pos2)
+    vel = 0.05 * torch.randn_like(pos2)
+    mass = torch.full((pos2.shape[0],), 10.0, device="cuda")
+    p3 = pos2.clone()
+    _, _, nreb = sysm.md_verlet_steps(p3, vel, mass, 1.0, 30)
+    sysm.check()
+    both(p3)
+    sysm.check()
