@@ -368,9 +368,9 @@ def measure_run_peaks(dev, mlp):
 
 def recorded_traffic(workload, mlp):
     """dram__bytes_read.sum + dram__bytes_write.sum per GEMM launch from the committed ncu capture of this workload and MLP
-    mode (profiles/ncu_r2_gemm_traffic.json, written from `ncu --set full`, command inside), or None: never a constant
+    mode (profiles/ncu_r2_gemm_traffic.json.txt, written from `ncu --set full`, command inside), or None: never a constant
     pasted into this file."""
-    path = os.path.join(ROOT, "profiles", "ncu_r2_gemm_traffic.json")
+    path = os.path.join(ROOT, "profiles", "ncu_r2_gemm_traffic.json.txt")
     if not os.path.exists(path):
         return None, None
     with open(path) as f:
@@ -378,7 +378,7 @@ def recorded_traffic(workload, mlp):
     ent = rec.get("%s/%s" % (workload, mlp))
     if not ent:
         return None, None
-    return ent["dram_bytes_per_launch"], "profiles/ncu_r2_gemm_traffic.json (ncu --set full of commit %s)" % rec.get("commit", "?")
+    return ent["dram_bytes_per_launch"], "profiles/ncu_r2_gemm_traffic.json.txt (ncu --set full of commit %s)" % rec.get("commit", "?")
 
 
 def run_ours(args):
