@@ -602,6 +602,7 @@ void gmnn_system_destroy(gmnn_system *s) {
 int gmnn_system_set_int(gmnn_system *s, const char *key, int64_t v) {
     if (!s || !key) return GMNN_INVALID_ARG;
     ++g_config_gen;  // any knob may change what an evaluation launches
+    s->seed_w = nullptr;
     if (!strcmp(key, "lanes_per_atom")) {
         if (v != 0 && v != 1 && v != 2 && v != 4 && v != 8 && v != 16 && v != 32) {
             set_error("lanes_per_atom must be 0, 1, 2, 4, 8, 16 or 32");

@@ -197,6 +197,8 @@ struct gmnn_system {
     // batched shallow-ensemble backward (gmnn_api.cu ensemble_pass): ens_batch heads per pass in buffers whose row tiles
     // are ordered [atom tile][head]; 0 / 1 outside such a pass.  ens_head: the head the pair backward reads.
     int ens_batch = 0, ens_head = 0, ens_cap = 0;  // ens_cap: heads the buffers below hold
+    const float *seed_w = nullptr;  // head weights the kept backward seed (vhead, Bv / BvT, its split and maximum) was prepared for
+    int seed_prec = -1;             // ... and the MLP mode
     int ens_batch_max = 0;                          // knob "ensemble_batch": heads per batch at most (0: as many as fit)
     float *ens_dZ[2] = {}, *ens_dG = nullptr, *ens_A = nullptr;
     // pair-buffer force mode: per-head own-direction force sums [heads][3 N] and pair buffers [heads][N cap] of the batch

@@ -296,8 +296,13 @@ int launch_mlp_seed(gmnn_system *s, const float *head_w_dev, cudaStream_t st) {
 int launch_mlp_backward_simt(gmnn_system *s, const float *head_w_dev, cudaStream_t st) {
     const gmnn_model *m = s->model;
     const int L = m->hp.n_hidden;
-    int rc = launch_mlp_seed(s, head_w_dev, st);
-    if (rc) return rc;
+    int rc = GMNN_OK;
+    const bool keep = head_w_dev == m->head_mean_w;  // see launch_mlp_backward_tc
+    if (!(keep && s->seed_w == head_w_dev && s->seed_prec == s->mlp_precision)) {
+        s->seed_w = nullptr;
+        if ((rc = launch_mlp_seed(s, head_w_dev, st))) return rc;
+        if (keep) s->seed_w = head_w_dev, s->seed_prec = s->mlp_precision;
+    }
     MlpSeg seg[MAX_SPECIES];
     const int ns = mlp_segments(s, seg);
     const float *Aop = s->D[L - 1];

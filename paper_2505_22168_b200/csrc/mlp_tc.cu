@@ -1317,16 +1317,25 @@ int launch_mlp_backward_tc(gmnn_system *s, const float *head_w_dev, cudaStream_t
     const bool f16 = s->mlp_precision == GMNN_MLP_3XF16;
     const bool split = s->mlp_precision == GMNN_MLP_3XTF32 || f16;
     const int L = m->hp.n_hidden;
-    int rc = launch_mlp_seed(s, head_w_dev, st);  // vhead, BvT per weight set (see mlp_simt.cu)
-    if (rc) return rc;
+    int rc = GMNN_OK;
     const size_t nbv = (size_t)m->dims[L] * m->dims[L - 1];
-    if (f16) {  // one scale for the seeded operands of all sets
-        if ((rc = launch_absmax(s->BvT, (int64_t)(nbv * m->n_sets), s->amax + AMAX_BVT, st))) return rc;
-        for (int t = 0; t < m->n_sets; ++t)
-            if ((rc = launch_split_stack_h(s->BvT + t * nbv, s->BvTh + 2 * t * nbv, (int64_t)nbv, s->amax + AMAX_BVT, st))) return rc;
-    } else if (split) {
-        for (int t = 0; t < m->n_sets; ++t)
-            if ((rc = launch_split_stack(s->BvT + t * nbv, s->BvTs + 2 * t * nbv, (int64_t)nbv, st))) return rc;
+    // The seeded operand W[L-1] diag(W_last c), its maximum and its split depend on the head weights c only: for the
+    // model's constant mean-head weights (every gmnn_energy_forces call and MD step) they are prepared once and kept
+    // (4 - 5 small launches less per evaluation: 15 % of the launches of a step); any other c (one-hot ensemble heads,
+    // UDD weights) prepares them anew.  Dropped by any gmnn_system_set_int and by the batched ensemble pass.
+    const bool keep = head_w_dev == m->head_mean_w;
+    if (!(keep && s->seed_w == head_w_dev && s->seed_prec == s->mlp_precision)) {
+        s->seed_w = nullptr;
+        if ((rc = launch_mlp_seed(s, head_w_dev, st))) return rc;  // vhead, BvT per weight set (see mlp_simt.cu)
+        if (f16) {  // one scale for the seeded operands of all sets
+            if ((rc = launch_absmax(s->BvT, (int64_t)(nbv * m->n_sets), s->amax + AMAX_BVT, st))) return rc;
+            for (int t = 0; t < m->n_sets; ++t)
+                if ((rc = launch_split_stack_h(s->BvT + t * nbv, s->BvTh + 2 * t * nbv, (int64_t)nbv, s->amax + AMAX_BVT, st))) return rc;
+        } else if (split) {
+            for (int t = 0; t < m->n_sets; ++t)
+                if ((rc = launch_split_stack(s->BvT + t * nbv, s->BvTs + 2 * t * nbv, (int64_t)nbv, st))) return rc;
+        }
+        if (keep) s->seed_w = head_w_dev, s->seed_prec = s->mlp_precision;
     }
     MlpSeg seg[MAX_SPECIES];
     const int ns = mlp_segments(s, seg);
@@ -1389,6 +1398,7 @@ int launch_mlp_backward_tc_heads(gmnn_system *s, int head0, int HB, cudaStream_t
     const int Hd = m->dims[L], prev = m->dims[L - 1];
     const int64_t nbv = (int64_t)prev * Hd * HB;
     int rc;
+    s->seed_w = nullptr;  // the batch's maximum goes to the scale word of the kept single-head seed
     k_seed_heads<<<(unsigned)((nbv + 255) / 256), 256, 0, st>>>(prev, Hd, m->W[L - 1], m->W[L], M, head0, HB, s->ens_BvT);
     GMNN_LAUNCHED();
     if (f16) {
