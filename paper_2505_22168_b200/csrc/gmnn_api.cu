@@ -135,6 +135,13 @@ static int forward_backward(gmnn_system *s, const float *positions, const float 
         return GMNN_OK;
     };
     if (!(allow_graph && s->ef_graph && !s->profile && !s->want_virial)) return core(st, T);
+    // (the captured launches rely on the backward seed kept in the system's buffers, mlp_tc.cu launch_mlp_backward_tc: an
+    // ensemble pass or a biased evaluation in between overwrites those buffers and clears seed_w)
+    if (s->ef_exec && s->ef_gen == g_config_gen && s->seed_w != s->ef_seed_w) {
+        cudaGraphExecDestroy(s->ef_exec);
+        s->ef_exec = nullptr;
+        return core(st, T);  // prepares the seed again; the next call captures
+    }
     if (s->ef_exec && s->ef_gen == g_config_gen) {  // replay
         GMNN_CUDA(cudaGraphLaunch(s->ef_exec, st));
         g_launch_count += s->ef_launches;
@@ -177,6 +184,7 @@ static int forward_backward(gmnn_system *s, const float *positions, const float 
         return GMNN_CUDA_ERROR;
     }
     s->ef_gen = g_config_gen;
+    s->ef_seed_w = s->seed_w;
     GMNN_CUDA(cudaGraphLaunch(s->ef_exec, st));
     g_launch_count += s->ef_launches;
     return GMNN_OK;

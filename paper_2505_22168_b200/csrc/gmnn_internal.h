@@ -221,6 +221,7 @@ struct gmnn_system {
     int ef_graph = 1;
     cudaGraphExec_t ef_exec = nullptr;
     long long ef_gen = 0, ef_seen_gen = 0, ef_launches = 0;
+    const float *ef_seed_w = nullptr;  // seed_w (below) at the capture: the graph is valid while the kept seed is the same
     cudaEvent_t graph_ev[2] = {};
     int md_continue = 0;             // knob: the next md call continues the previous one
     bool md_state_valid = false;     // f_tmp / e_total hold the forces and energies of the last md step

@@ -312,3 +312,57 @@ def test_energy_forces_graph_replay_is_bitwise_the_eager_call(gm, mlp_precision)
     sysm.check()
     both(p3)
     sysm.check()
+
+
+@pytest.mark.parametrize("mlp_precision", [0, 3])
+def test_kept_state_survives_other_calls(gm, mlp_precision):
+    """What gmnn_energy_forces keeps between calls (its CUDA graph, the backward seed of the constant mean-head weights)
+    must not leak into or out of the calls that change the head weights or the buffers: an ensemble pass, a UDD-biased
+    evaluation, a switch of the MLP mode.  Reference: a fresh system with the kept state off, same positions."""
+    import torch
+
+    w = wl.li3po4_box(1600, hidden=(64, 64), n_heads=8)
+    _, sysm, pos = _gpu_system(gm, w, mlp_precision=mlp_precision, force_mode=1)
+    _, ref_sys, _ = _gpu_system(gm, w, mlp_precision=mlp_precision, force_mode=1)
+    ref_sys.set_int("ef_graph", 0)
+
+    def out(system):
+        e, ea, f = system.energy_forces(pos)[:3]
+        return float(e.cpu()[0]), ea.cpu().numpy().copy(), f.cpu().numpy().copy()
+
+    def same(a, b):
+        return a[0] == b[0] and np.array_equal(a[1], b[1]) and np.array_equal(a[2], b[2])
+
+    ref = out(ref_sys)
+    for _ in range(3):
+        assert same(out(sysm), ref)  # eager, capture, replay
+    ens = [t.cpu().numpy().copy() for t in sysm.ensemble_energy_forces(pos)]
+    ens_ref = [t.cpu().numpy().copy() for t in ref_sys.ensemble_energy_forces(pos)]
+    assert all(np.array_equal(a, b) for a, b in zip(ens, ens_ref))
+    for _ in range(2):
+        assert same(out(sysm), ref)  # after the ensemble pass (one-hot or stacked head weights) the mean-head seed is rebuilt
+    ref_sys.set_udd_bias(0.5, 1.0)
+    out(ref_sys)
+    _, var_e = ref_sys.get_udd_bias()
+    B = float(np.sqrt(var_e / (8 * pos.shape[0])))  # sigma_E^2 / (M N B^2) = 1: a bias force of the size of the forces
+    sysm.set_udd_bias(0.5, B)
+    ref_sys.set_udd_bias(0.5, B)
+    biased_ref = out(ref_sys)
+    assert not np.array_equal(biased_ref[2], ref[2])
+    for _ in range(3):
+        assert same(out(sysm), biased_ref)
+    sysm.set_udd_bias(0.0, B)
+    ref_sys.set_udd_bias(0.0, B)
+    for _ in range(3):
+        assert same(out(sysm), ref)
+    other = 0 if mlp_precision == 3 else 3
+    for system in (sysm, ref_sys):
+        system.set_int("mlp_precision", other)
+    ref_other = out(ref_sys)
+    for _ in range(3):
+        assert same(out(sysm), ref_other)
+    for system in (sysm, ref_sys):
+        system.set_int("mlp_precision", mlp_precision)
+    for _ in range(3):
+        assert same(out(sysm), ref)
+    sysm.check()
