@@ -74,6 +74,25 @@ def test_ensemble_batches_of_heads(gm, orc, batch, mlp_precision):
     assert np.array_equal(part[0], full[0]) and np.array_equal(part[1], full[1])  # the forward does not depend on the batching
 
 
+@pytest.mark.parametrize("lanes", [1, 2, 4, 32])
+def test_ensemble_heads_kernel_lane_groupings_sheared_cell(gm, orc, lanes):
+    """The batched pair backward stages the adjoints of as many heads per chunk as 96 KB of shared memory hold beside the
+    128 / lanes centres of a block (1 head at one lane per atom, 3 at two, 7 at four, 8 from eight lanes on): every
+    chunking against the oracle, on a sheared cell (lattice shifts inside the kernel), 12 heads."""
+    w = wl.triclinic_box(1000, hidden=(64, 64), n_heads=12)
+    m = orc.Model(w.model)
+    pairs = orc.auto_neighbors(w.positions, w.box, w.pbc, r_list32(w.model.r_cut, w.skin))
+    ref = orc.ensemble(m, w.positions, w.species, w.box, pairs)
+    _, sysm, pos = _build(gm, w, mlp_precision=gm.GMNN_MLP_3XF16, force_mode=gm.GMNN_FORCE_PAIRBUF)
+    sysm.set_int("lanes_per_atom", lanes)
+    e_mean, e_var, f_mean, f_var = (t.cpu().numpy().astype(np.float64) for t in sysm.ensemble_energy_forces(pos))
+    sysm.check()
+    assert energy_atom_error(e_mean, ref.e_mean) <= 1.0
+    assert force_error(f_mean, ref.f_mean) <= F_TOL
+    assert np.abs(e_var - ref.e_var).max() <= 2e-4 * ref.e_var.max()
+    assert np.abs(f_var - ref.f_var).max() <= 2e-4 * ref.f_var.max()
+
+
 def test_config4_full_size(gm, orc):
     """Config 4 at its stated size (8 192 atoms, 32 heads): e_mean, e_var, f_mean and f_var element by
     element against oracle O-10 (one forward, 32 backward passes in fp64; about 20 s on 16 cores), at the
