@@ -314,14 +314,15 @@ def test_energy_forces_graph_replay_is_bitwise_the_eager_call(gm, mlp_precision)
     sysm.check()
 
 
+@pytest.mark.parametrize("n_weight_sets", [1, 3])
 @pytest.mark.parametrize("mlp_precision", [0, 3])
-def test_kept_state_survives_other_calls(gm, mlp_precision):
+def test_kept_state_survives_other_calls(gm, mlp_precision, n_weight_sets):
     """What gmnn_energy_forces keeps between calls (its CUDA graph, the backward seed of the constant mean-head weights)
     must not leak into or out of the calls that change the head weights or the buffers: an ensemble pass, a UDD-biased
     evaluation, a switch of the MLP mode.  Reference: a fresh system with the kept state off, same positions."""
     import torch
 
-    w = wl.li3po4_box(1600, hidden=(64, 64), n_heads=8)
+    w = wl.li3po4_box(1600, hidden=(64, 64), n_heads=8, n_weight_sets=n_weight_sets)
     _, sysm, pos = _gpu_system(gm, w, mlp_precision=mlp_precision, force_mode=1)
     _, ref_sys, _ = _gpu_system(gm, w, mlp_precision=mlp_precision, force_mode=1)
     ref_sys.set_int("ef_graph", 0)
